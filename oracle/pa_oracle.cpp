@@ -1,0 +1,493 @@
+// pa_oracle.cpp -- CPU ORACLE for the population-annealing (PA) hot path of the 2D Ising model.
+//
+// THIS FILE IS TEST INFRASTRUCTURE.  It is the plain, slow, step-by-step statement of what the
+// method computes, written from the paper (/root/reference/PAPER.md, cited below as "L<line>")
+// and from the readings listed in DESIGN.md section 3 ("O1".."O10").  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may build, load or
+// call it.  It shares no code with the CUDA library under paper_1703_03676_b200/csrc/ and
+// neither includes the other.
+//
+// One uint8 per spin (1 = up = sigma +1, 0 = down), spin[j][s] with s = y*L + x, scalar Philox,
+// fp64 everywhere a floating-point number appears.  Loops over replicas are marked
+// "#pragma omp parallel for": replicas are independent (L149) and the random stream is
+// counter-based (L163), so the result does not depend on the thread count.
+//
+// Parity pins (tests/test_oracle_*.py, -m "not gpu"):
+//   philox4x32_10 ........ cuRAND's curand_philox4x32_x.h (independent implementation), bijectivity
+//   thresholds ........... closed forms (beta = 0, monotonicity, exact powers of two)
+//   sweep (O3) ........... L=4 brute-force Boltzmann distribution (chi^2), global-flip symmetry
+//   init / beta=0 ........ closed-form moments of i.i.d. spins
+//   energies (O4) ........ brute force with numpy.roll, all-up and checkerboard states
+//   weights, lnQ (O5) .... dbeta=0 closed form, histogram regrouping, Kaufman lnZ (4 sigma)
+//   copy numbers (O6) .... sum tau = R, r in {floor, floor+1}, identity at dbeta=0, |R_i-R| bound
+//   scan / copy (O7) ..... serial scan, new[d]==old[parent(d)], monotone parent map
+//   observables (O8) ..... L=4 exact enumeration, Kaufman e and C at L=16 (4 sigma over seeds)
+//   multi-histogram (O9) . sum H = R_i, sum H*E = SE, ln Omega vs exact ln g(E) at L=4
+//   adaptive step (O10) .. alpha(0) closed form, monotonicity, bracket property
+//   whole method vs the paper's own figures: "parity unpinned" (Figs. 2-3 data and the authors'
+//   code are not available); pinned instead by the exact Ising results above.
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// O1  Random stream.  L163: "Philox_4x32_10 ... sequence number determined from the grid and
+// block indices of the thread and a global iteration parameter".  Philox4x32-10 as published in
+// ref. [33] (L368): 10 rounds; per round  (hi0,lo0) = M0*c0, (hi1,lo1) = M1*c2,
+// c <- (hi1^c1^k0, lo1, hi0^c3^k1, lo0); the key is bumped by the Weyl constants between rounds.
+// ---------------------------------------------------------------------------------------------
+const uint32_t PHILOX_M0 = 0xD2511F53u, PHILOX_M1 = 0xCD9E8D57u;
+const uint32_t PHILOX_W0 = 0x9E3779B9u, PHILOX_W1 = 0xBB67AE85u;
+
+void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                   uint32_t k0, uint32_t k1, uint32_t out[4]) {
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)PHILOX_M0 * (uint64_t)c0;
+        uint64_t p1 = (uint64_t)PHILOX_M1 * (uint64_t)c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0, n1 = lo1, n2 = hi0 ^ c3 ^ k1, n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += PHILOX_W0; k1 += PHILOX_W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Stream tags (O1): the fourth counter word separates the three uses.
+const uint32_t TAG_INIT = 0u, TAG_SWEEP = 1u, TAG_RESAMPLE = 2u;
+
+inline uint32_t key0(uint64_t seed) { return (uint32_t)(seed & 0xffffffffull); }
+inline uint32_t key1(uint64_t seed) { return (uint32_t)(seed >> 32); }
+
+// INIT: the 32-bit word for (site s, group g) is philox(s, g>>2, 0, TAG_INIT)[g&3]; the spin of
+// replica j at site s is bit (j&31) of the word of group j>>5.   (L55, L65: i.i.d. uniform spins)
+inline uint8_t x_init(uint64_t seed, int64_t j, uint32_t s) {
+    uint32_t g = (uint32_t)(j >> 5), out[4];
+    philox4x32_10(s, g >> 2, 0u, TAG_INIT, key0(seed), key1(seed), out);
+    return (uint8_t)((out[g & 3u] >> (uint32_t)(j & 31)) & 1u);
+}
+// SWEEP: x(j,s,t,c) = philox(s, j>>2, 2t+c, TAG_SWEEP)[j&3]; j = replica slot, t = sweep counter.
+inline uint32_t x_sweep(uint64_t seed, int64_t j, uint32_t s, uint32_t t, uint32_t c) {
+    uint32_t out[4];
+    philox4x32_10(s, (uint32_t)(j >> 2), 2u * t + c, TAG_SWEEP, key0(seed), key1(seed), out);
+    return out[j & 3];
+}
+// RESAMPLE: x(j,k) = philox(j>>2, 0, k, TAG_RESAMPLE)[j&3]; k = resample counter.
+inline uint32_t x_resample(uint64_t seed, int64_t j, uint32_t k) {
+    uint32_t out[4];
+    philox4x32_10((uint32_t)(j >> 2), 0u, k, TAG_RESAMPLE, key0(seed), key1(seed), out);
+    return out[j & 3];
+}
+
+// ---------------------------------------------------------------------------------------------
+// O2  Thresholds.  L163 "pre-calculated tables of the Metropolis factors exp(-beta dE)".
+// T(p) = (uint32) min(floor(p * 2^32), 2^32 - 1); a flip with dE > 0 is accepted iff x < T.
+// ---------------------------------------------------------------------------------------------
+uint32_t threshold(double p) {
+    double v = std::floor(p * 4294967296.0);
+    if (v > 4294967295.0) v = 4294967295.0;
+    if (v < 0.0) v = 0.0;
+    return (uint32_t)v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// O3  One checkerboard Metropolis sweep of one replica.  L151-L157 (checkerboard, one
+// sub-lattice, synchronise, the other), L73 (Metropolis), Eq. 10 L135 (H = -sum s_i s_j,
+// periodic, L137).  u = number of the 4 neighbours anti-parallel to the centre spin;
+// dE = 2*sigma*sum_nn sigma = 8 - 4u; flip iff dE <= 0 or x < T(dE).
+// Colour 0 = (x+y) even is updated first, then colour 1.
+// ---------------------------------------------------------------------------------------------
+void sweep_one_replica(uint8_t* sp, int L, uint64_t seed, int64_t slot, uint32_t t,
+                       uint32_t T4, uint32_t T8) {
+    for (uint32_t c = 0; c < 2; ++c) {
+        for (int y = 0; y < L; ++y) {
+            for (int x = 0; x < L; ++x) {
+                if ((uint32_t)((x + y) & 1) != c) continue;
+                int s = y * L + x;
+                int xm = x == 0 ? L - 1 : x - 1, xp = x == L - 1 ? 0 : x + 1;      // periodic, L137
+                int ym = y == 0 ? L - 1 : y - 1, yp = y == L - 1 ? 0 : y + 1;
+                int u = (sp[y * L + xm] != sp[s]) + (sp[y * L + xp] != sp[s]) +
+                        (sp[ym * L + x] != sp[s]) + (sp[yp * L + x] != sp[s]);
+                uint32_t xr = x_sweep(seed, slot, (uint32_t)s, t, c);   // drawn for every (j,s,t)
+                bool flip = (u >= 2) || (u == 1 && xr < T4) || (u == 0 && xr < T8);
+                if (flip) sp[s] ^= 1u;
+            }
+        }
+    }
+}
+
+// O4  Energy and magnetisation of one replica.  Eq. 10 L135 (each bond once: right and down
+// neighbour of every site), L173.  E = -sum_bonds sigma_a sigma_b, M = sum sigma.
+void energy_one_replica(const uint8_t* sp, int L, int32_t* E, int32_t* M) {
+    int32_t e = 0, m = 0;
+    for (int y = 0; y < L; ++y)
+        for (int x = 0; x < L; ++x) {
+            int sg = sp[y * L + x] ? 1 : -1;
+            int sr = sp[y * L + (x == L - 1 ? 0 : x + 1)] ? 1 : -1;
+            int sd = sp[(y == L - 1 ? 0 : y + 1) * L + x] ? 1 : -1;
+            e -= sg * (sr + sd);
+            m += sg;
+        }
+    *E = e; *M = m;
+}
+
+// O5  TREE1024: the fixed summation order of the weight sum (L165: "deterministic ... sum the
+// per-block partial results in a subsequent kernel call").  Pad with +0.0 to a multiple of 1024;
+// inside every aligned run of 32 values: for off = 16,8,4,2,1: a[i] += a[i+off] for i < off;
+// the 32 run sums of an aligned block of 1024 are combined by the same 5-level tree; the block
+// sums are added sequentially in ascending block index.
+double tree1024(const double* a, int64_t n) {
+    double total = 0.0;
+    for (int64_t b0 = 0; b0 < n; b0 += 1024) {
+        double run[32];
+        for (int r = 0; r < 32; ++r) {
+            double v[32];
+            for (int i = 0; i < 32; ++i) {
+                int64_t idx = b0 + 32 * r + i;
+                v[i] = (idx < n) ? a[idx] : 0.0;
+            }
+            for (int off = 16; off >= 1; off >>= 1)
+                for (int i = 0; i < off; ++i) v[i] += v[i + off];
+            run[r] = v[0];
+        }
+        for (int off = 16; off >= 1; off >>= 1)
+            for (int i = 0; i < off; ++i) run[i] += run[i + off];
+        total += run[0];
+    }
+    return total;
+}
+
+int64_t capacity_for(int64_t R) {                       // DESIGN.md O7 (paper silent on capacity)
+    int64_t slack = (int64_t)std::ceil(8.0 * std::sqrt((double)R));
+    if (slack < 1024) slack = 1024;
+    return 32 * ((R + slack + 31) / 32);
+}
+
+double logaddexp(double a, double b) {
+    if (a == -std::numeric_limits<double>::infinity()) return b;
+    if (b == -std::numeric_limits<double>::infinity()) return a;
+    double hi = a > b ? a : b, lo = a > b ? b : a;
+    return hi + std::log1p(std::exp(lo - hi));
+}
+
+struct Oracle {
+    int L = 0, N = 0;
+    int64_t R_target = 0, R_cur = 0, R_cap = 0;
+    uint64_t seed = 0;
+    uint32_t t = 0;          // global sweep counter
+    uint32_t k = 0;          // resample counter
+    double lnZ = 0.0;        // = -beta F(beta), Eq. 4; starts at N ln 2 (L93)
+    double lnQ_last = 0.0;
+    std::vector<uint8_t> spin;        // [R_cap][N]
+    std::vector<int64_t> Hsum;        // [N+1]  running sum of energy histograms, Eq. 9 numerator
+    std::vector<double> lnD;          // [N+1]  log of the Eq. 9 denominator
+    // last resample, kept for inspection
+    double W_last = 0.0;
+    std::vector<double> w_last;
+    std::vector<uint32_t> r_last, o_last;
+};
+
+void all_energies(const Oracle* o, std::vector<int32_t>& E, std::vector<int32_t>& M) {
+    E.resize(o->R_cur); M.resize(o->R_cur);
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < o->R_cur; ++j)
+        energy_one_replica(&o->spin[(size_t)j * o->N], o->L, &E[j], &M[j]);
+}
+
+// O5 weights for a given dbeta: E_ref = min_j E_j, wtab[d] = exp(-(dbeta*(double)(4d))),
+// w_j = wtab[(E_j-E_ref)/4], W = TREE1024(w).   Eq. 1 L58 with the common factor exp(-dbeta E_ref)
+// taken out (paper silent on overflow; O5).
+void weights_for(const std::vector<int32_t>& E, double dbeta, int32_t* E_ref_out,
+                 std::vector<double>& w, double* W) {
+    int64_t R = (int64_t)E.size();
+    int32_t E_ref = E[0], E_max = E[0];
+    for (int64_t j = 1; j < R; ++j) { if (E[j] < E_ref) E_ref = E[j]; if (E[j] > E_max) E_max = E[j]; }
+    int32_t dmax = (E_max - E_ref) / 4;
+    std::vector<double> wtab(dmax + 1);
+    for (int32_t d = 0; d <= dmax; ++d) wtab[d] = std::exp(-(dbeta * (double)(4 * d)));
+    w.resize(R);
+    for (int64_t j = 0; j < R; ++j) w[j] = wtab[(E[j] - E_ref) / 4];
+    *W = tree1024(w.data(), R);
+    *E_ref_out = E_ref;
+}
+
+// O10 overlap, Eq. 8: alpha = (1/R_cur) sum_j min(1, tau_hat_j), tau_hat_j = R_target*w_j/W
+// (= R exp(-dbeta E_j) / (R_cur Q), Eq. 1), summed in the TREE1024 order.
+double overlap_for(const std::vector<int32_t>& E, int64_t R_target, double dbeta) {
+    std::vector<double> w; double W; int32_t E_ref;
+    weights_for(E, dbeta, &E_ref, w, &W);
+    int64_t R = (int64_t)E.size();
+    std::vector<double> a(R);
+    for (int64_t j = 0; j < R; ++j) {
+        double tau = ((double)R_target * w[j]) / W;
+        a[j] = tau < 1.0 ? tau : 1.0;
+    }
+    return tree1024(a.data(), R) / (double)R;
+}
+
+}  // namespace
+
+extern "C" {
+
+typedef struct { double beta, e, C, absm, m2, m4, betaF_per_N, S_per_N, lnQ; int64_t R; } ora_obs_t;
+
+enum { ORA_OK = 0, ORA_ERR_INVALID_ARG = -1, ORA_ERR_CAPACITY = -2, ORA_ERR_NOMEM = -3 };
+
+// ---- stateless pieces (also used for the sampled parity checks at the large configs) --------
+
+void ora_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    philox4x32_10(ctr[0], ctr[1], ctr[2], ctr[3], key[0], key[1], out);
+}
+uint32_t ora_threshold(double p) { return threshold(p); }
+void ora_thresholds(double beta, uint32_t* T4, uint32_t* T8) {
+    *T4 = threshold(std::exp(-4.0 * beta));
+    *T8 = threshold(std::exp(-8.0 * beta));
+}
+double ora_tree1024(const double* a, int64_t n) { return tree1024(a, n); }
+int64_t ora_capacity(int64_t R) { return capacity_for(R); }
+
+// theta sweeps (O3) of nslots replicas given as spins[nslots][N], replica i living in population
+// slot slot_ids[i]; the sweep counter runs t0, t0+1, ..., t0+theta-1.
+int ora_sweep_slots(int L, uint64_t seed, uint32_t t0, double beta, int theta,
+                    int64_t nslots, const int64_t* slot_ids, uint8_t* spins) {
+    if (L < 4 || (L & 1) || theta < 0 || nslots < 0) return ORA_ERR_INVALID_ARG;
+    uint32_t T4, T8; ora_thresholds(beta, &T4, &T8);
+    int N = L * L;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < nslots; ++i)
+        for (int it = 0; it < theta; ++it)
+            sweep_one_replica(spins + (size_t)i * N, L, seed, slot_ids[i], t0 + (uint32_t)it, T4, T8);
+    return ORA_OK;
+}
+
+int ora_energies_of(int L, int64_t n, const uint8_t* spins, int32_t* E, int32_t* M) {
+    if (L < 4 || (L & 1) || n < 0) return ORA_ERR_INVALID_ARG;
+    int N = L * L;
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < n; ++j) {
+        int32_t e, m; energy_one_replica(spins + (size_t)j * N, L, &e, &m);
+        E[j] = e; if (M) M[j] = m;
+    }
+    return ORA_OK;
+}
+
+// O5-O7 from an energy vector alone: weights, W, copy numbers, offsets, R_new, lnQ.
+// Any output pointer may be NULL.  Eq. 1, Eq. 2 L67, L69 (tau_hat = (R/R_{i-1}) tau).
+int ora_resample_plan(int64_t R_target, int64_t R_cur, const int32_t* E, uint64_t seed, uint32_t k,
+                      double dbeta, double* W_out, double* w_out, uint32_t* r_out, uint32_t* o_out,
+                      int64_t* R_new_out, double* lnQ_out) {
+    if (R_cur < 1 || R_target < 1) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> Ev(E, E + R_cur);
+    std::vector<double> w; double W; int32_t E_ref;
+    weights_for(Ev, dbeta, &E_ref, w, &W);
+    uint64_t run = 0;
+    for (int64_t j = 0; j < R_cur; ++j) {
+        double tau = ((double)R_target * w[j]) / W;          // one multiply, one divide (O6)
+        double n = std::floor(tau);
+        double f = tau - n;                                   // exact
+        double u = (double)x_resample(seed, j, k) * (1.0 / 4294967296.0);   // exact, in [0,1)
+        uint32_t r = (uint32_t)n + (u < f ? 1u : 0u);        // Eq. 2 with strict '<' (O6)
+        if (r_out) r_out[j] = r;
+        if (o_out) o_out[j] = (uint32_t)run;                  // exclusive prefix sum (O7, L165)
+        if (w_out) w_out[j] = w[j];
+        run += r;
+    }
+    if (W_out) *W_out = W;
+    if (R_new_out) *R_new_out = (int64_t)run;
+    if (lnQ_out) *lnQ_out = -dbeta * (double)E_ref + std::log(W / (double)R_cur);   // Eq. 1 shifted
+    return ORA_OK;
+}
+
+double ora_overlap_of(int64_t R_target, int64_t R_cur, const int32_t* E, double dbeta) {
+    std::vector<int32_t> Ev(E, E + R_cur);
+    return overlap_for(Ev, R_target, dbeta);
+}
+
+// ---- the population handle (the same calls as include/pa.h, prefixed ora_) -------------------
+
+int ora_create(int L, int64_t R, uint64_t seed, Oracle** out) {
+    if (!out || L < 4 || (L & 1) || R < 1) return ORA_ERR_INVALID_ARG;
+    Oracle* o = new (std::nothrow) Oracle();
+    if (!o) return ORA_ERR_NOMEM;
+    o->L = L; o->N = L * L; o->R_target = R; o->R_cur = R; o->R_cap = capacity_for(R);
+    o->seed = seed; o->t = 0; o->k = 0;
+    o->lnZ = (double)o->N * std::log(2.0);                    // Z_{beta_0} = 2^N, L93
+    try { o->spin.assign((size_t)o->R_cap * o->N, 0); } catch (...) { delete o; return ORA_ERR_NOMEM; }
+    o->Hsum.assign(o->N + 1, 0);
+    o->lnD.assign(o->N + 1, -std::numeric_limits<double>::infinity());
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < R; ++j)                           // step 1, L55, L65
+        for (int s = 0; s < o->N; ++s) o->spin[(size_t)j * o->N + s] = x_init(seed, j, (uint32_t)s);
+    *out = o;
+    return ORA_OK;
+}
+
+void ora_destroy(Oracle* o) { delete o; }
+int64_t ora_population(const Oracle* o) { return o->R_cur; }
+int64_t ora_capacity_of(const Oracle* o) { return o->R_cap; }
+uint32_t ora_sweep_counter(const Oracle* o) { return o->t; }
+uint32_t ora_resample_counter(const Oracle* o) { return o->k; }
+double ora_lnZ(const Oracle* o) { return o->lnZ; }
+
+// step 3, L61: theta rounds of MCMC at inverse temperature beta.
+int ora_sweep(Oracle* o, double beta, int theta) {
+    if (!o || theta < 0) return ORA_ERR_INVALID_ARG;
+    uint32_t T4, T8; ora_thresholds(beta, &T4, &T8);
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < o->R_cur; ++j)
+        for (int it = 0; it < theta; ++it)
+            sweep_one_replica(&o->spin[(size_t)j * o->N], o->L, o->seed, j, o->t + (uint32_t)it, T4, T8);
+    o->t += (uint32_t)theta;
+    return ORA_OK;
+}
+
+int ora_energies(Oracle* o, int32_t* E_out, int32_t* M_out) {
+    if (!o || !E_out) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> E, M; all_energies(o, E, M);
+    std::memcpy(E_out, E.data(), sizeof(int32_t) * o->R_cur);
+    if (M_out) std::memcpy(M_out, M.data(), sizeof(int32_t) * o->R_cur);
+    return ORA_OK;
+}
+
+// step 2, L56-L58 and L65-L69: resample from beta to beta_new.
+int ora_resample(Oracle* o, double beta, double beta_new, int64_t* R_new_out) {
+    if (!o || !(beta_new >= beta)) return ORA_ERR_INVALID_ARG;
+    double dbeta = beta_new - beta;
+    std::vector<int32_t> E, M; all_energies(o, E, M);
+    std::vector<double> w(o->R_cur); std::vector<uint32_t> r(o->R_cur), off(o->R_cur);
+    double W, lnQ; int64_t R_new;
+    ora_resample_plan(o->R_target, o->R_cur, E.data(), o->seed, o->k, dbeta,
+                      &W, w.data(), r.data(), off.data(), &R_new, &lnQ);
+    if (R_new > o->R_cap) return ORA_ERR_CAPACITY;            // state unchanged (O7)
+    if (R_new < 1) return ORA_ERR_CAPACITY;
+    // new[o_j + c] = old[j], c = 0..r_j-1: slots keep parent order (O7, L165 "new population vector")
+    std::vector<uint8_t> fresh((size_t)o->R_cap * o->N, 0);
+    for (int64_t j = 0; j < o->R_cur; ++j)
+        for (uint32_t c = 0; c < r[j]; ++c)
+            std::memcpy(&fresh[((size_t)off[j] + c) * o->N], &o->spin[(size_t)j * o->N], o->N);
+    o->spin.swap(fresh);
+    o->R_cur = R_new; o->k += 1; o->lnZ += lnQ; o->lnQ_last = lnQ;   // Eq. 4
+    o->W_last = W; o->w_last.swap(w); o->r_last.swap(r); o->o_last.swap(off);
+    if (R_new_out) *R_new_out = R_new;
+    return ORA_OK;
+}
+
+// O10, L118 "for instance, bisection": hi = beta_max - beta; if alpha(hi) >= target return hi;
+// lo = 0; 40 times: mid = (lo+hi)/2; alpha(mid) >= target ? lo = mid : hi = mid; return lo.
+int ora_adapt_dbeta(Oracle* o, double target, double beta, double beta_max, double* dbeta_out) {
+    if (!o || !dbeta_out || !(target > 0.0 && target < 1.0) || !(beta_max > beta)) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> E, M; all_energies(o, E, M);
+    double hi = beta_max - beta;
+    if (overlap_for(E, o->R_target, hi) >= target) { *dbeta_out = hi; return ORA_OK; }
+    double lo = 0.0;
+    for (int it = 0; it < 40; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (overlap_for(E, o->R_target, mid) >= target) lo = mid; else hi = mid;
+    }
+    *dbeta_out = lo;
+    return ORA_OK;
+}
+
+int ora_overlap(Oracle* o, double dbeta, double* alpha) {
+    if (!o || !alpha) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> E, M; all_energies(o, E, M);
+    *alpha = overlap_for(E, o->R_target, dbeta);
+    return ORA_OK;
+}
+
+// step 4, L62; Eq. 3, Eq. 4, Eq. 5; output fields of L179-L181.
+int ora_observables(Oracle* o, double beta, ora_obs_t* out) {
+    if (!o || !out) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> E, M; all_energies(o, E, M);
+    int64_t R = o->R_cur, N = o->N;
+    int64_t SE = 0, SE2 = 0, SA = 0, SM2 = 0;
+    std::vector<double> q(R);
+    for (int64_t j = 0; j < R; ++j) {
+        SE += E[j]; SE2 += (int64_t)E[j] * E[j];
+        SA += M[j] < 0 ? -(int64_t)M[j] : (int64_t)M[j];
+        SM2 += (int64_t)M[j] * M[j];
+        double m = (double)M[j] / (double)N, mm = m * m;
+        q[j] = mm * mm;
+    }
+    double SM4 = tree1024(q.data(), R);
+    __int128 num = (__int128)R * (__int128)SE2 - (__int128)SE * (__int128)SE;   // exact
+    out->beta = beta;
+    out->e = (double)SE / ((double)R * (double)N);
+    out->C = beta * beta * ((double)num / ((double)R * (double)R * (double)N));
+    out->absm = (double)SA / ((double)R * (double)N);
+    out->m2 = (double)SM2 / ((double)R * (double)N * (double)N);
+    out->m4 = SM4 / (double)R;
+    out->betaF_per_N = -o->lnZ / (double)N;
+    out->S_per_N = beta * out->e + o->lnZ / (double)N;
+    out->lnQ = o->lnQ_last;
+    out->R = R;
+    return ORA_OK;
+}
+
+// O9, Eq. 9: fold the energy histogram at beta into the running sums.
+int ora_hist_accumulate(Oracle* o, double beta) {
+    if (!o) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> E, M; all_energies(o, E, M);
+    int N = o->N;
+    std::vector<int64_t> H(N + 1, 0);
+    for (int64_t j = 0; j < o->R_cur; ++j) H[(E[j] + 2 * N) / 4] += 1;
+    double lnR = std::log((double)o->R_cur);
+    for (int m = 0; m <= N; ++m) {
+        o->Hsum[m] += H[m];
+        double Em = (double)(-2 * N + 4 * m);
+        // R_i exp[beta_i F(beta_i) - beta_i E], with -beta_i F = lnZ (Eq. 4)
+        o->lnD[m] = logaddexp(o->lnD[m], lnR - o->lnZ - beta * Em);
+    }
+    return ORA_OK;
+}
+
+int ora_get_histogram(const Oracle* o, int64_t* Hsum, double* lnD) {
+    if (!o) return ORA_ERR_INVALID_ARG;
+    if (Hsum) std::memcpy(Hsum, o->Hsum.data(), sizeof(int64_t) * (o->N + 1));
+    if (lnD) std::memcpy(lnD, o->lnD.data(), sizeof(double) * (o->N + 1));
+    return ORA_OK;
+}
+
+// spins as +1/-1, [nrep][N], site = y*L + x
+int ora_get_spins(const Oracle* o, int64_t j0, int64_t nrep, int8_t* out) {
+    if (!o || j0 < 0 || nrep < 0 || j0 + nrep > o->R_cur) return ORA_ERR_INVALID_ARG;
+    for (int64_t i = 0; i < nrep * o->N; ++i) out[i] = o->spin[(size_t)j0 * o->N + i] ? 1 : -1;
+    return ORA_OK;
+}
+int ora_set_spins(Oracle* o, int64_t j0, int64_t nrep, const int8_t* in) {
+    if (!o || j0 < 0 || nrep < 0 || j0 + nrep > o->R_cur) return ORA_ERR_INVALID_ARG;
+    for (int64_t i = 0; i < nrep * o->N; ++i) o->spin[(size_t)j0 * o->N + i] = in[i] > 0 ? 1 : 0;
+    return ORA_OK;
+}
+
+int ora_get_resample_debug(const Oracle* o, double* W, double* w, uint32_t* r, uint32_t* off) {
+    if (!o) return ORA_ERR_INVALID_ARG;
+    if (W) *W = o->W_last;
+    if (w) std::memcpy(w, o->w_last.data(), sizeof(double) * o->w_last.size());
+    if (r) std::memcpy(r, o->r_last.data(), sizeof(uint32_t) * o->r_last.size());
+    if (off) std::memcpy(off, o->o_last.data(), sizeof(uint32_t) * o->o_last.size());
+    return ORA_OK;
+}
+
+int ora_num_threads(void) {
+    int n = 1;
+#ifdef _OPENMP
+#pragma omp parallel
+    {
+#pragma omp master
+        n = omp_get_num_threads();
+    }
+#endif
+    return n;
+}
+
+}  // extern "C"
