@@ -1,0 +1,167 @@
+/* pa.h -- C ABI of the B200 population-annealing (PA) hot path for the 2D Ising model.
+ *
+ * The calls follow the paper's statement of the algorithm (Sec. 2.1, steps
+ * 1-5) and BASELINE.json's north_star: pa_create = step 1, pa_resample = step 2,
+ * pa_sweep = step 3, pa_observables = step 4; the caller owns the loop and the beta schedule
+ * (equal steps, L71, or pa_adapt_dbeta, Sec. 2.3).  "L<n>" below cites a line of
+ * /root/reference/PAPER.md; "O<n>" cites the reading of that passage listed in DESIGN.md Sec. 3.
+ *
+ * One handle = one population of replicas of the L x L periodic ferromagnetic Ising model
+ * (Eq. 10), resident in device memory, bit-packed 32 replicas per 32-bit word
+ * (asynchronous multi-spin coding, L185).  All work is enqueued on the handle's CUDA stream.
+ * Calls that return a host scalar synchronise that stream; the others are asynchronous.
+ * A handle is not thread-safe; different handles are independent.  There is no global state.
+ *
+ * Pointers: every `out`/`in` buffer below may be a HOST pointer or a DEVICE pointer (of the
+ * handle's device); the library asks the CUDA runtime which it is.  Buffers are caller-owned;
+ * the library never keeps them after the call returns.
+ *
+ * Every function returning int returns PA_OK (0) or a negative PA_ERR_* code; on error the
+ * population is unchanged unless stated otherwise.  There is no CPU fallback: without a CUDA
+ * device pa_create / pa_create_ex return PA_ERR_CUDA.
+ */
+#ifndef PA_B200_PA_H
+#define PA_B200_PA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pa_handle pa_t; /* opaque */
+
+enum {
+    PA_OK = 0,
+    PA_ERR_INVALID_ARG = -1, /* L odd or < 4 or > 512, R < 1, theta < 0, beta' < beta, alpha* not in (0,1), NULL */
+    PA_ERR_CAPACITY = -2,    /* resampling would exceed the capacity R_cap (or produce an empty population) */
+    PA_ERR_CUDA = -3,        /* a CUDA call failed (sticky: see pa_last_cuda_error) */
+    PA_ERR_WORKSPACE = -4,   /* caller-provided workspace too small or not 256-byte aligned */
+    PA_ERR_NOMEM = -5
+};
+
+/* One output line of the paper's program (L179-L181): beta, energy per site, specific heat,
+ * |m|, m^2, m^4 (Eq. 3), beta F / N (Eq. 4), S / N (Eq. 5), population size,
+ * ln Q of the last resampling step (Eq. 1). */
+typedef struct {
+    double beta, e, C, absm, m2, m4, betaF_per_N, S_per_N, lnQ;
+    int64_t R;
+} pa_obs_t;
+
+/* Capacity in replicas of a population with target size R (O7; the paper is silent):
+ * R_cap = 32 * ceil((R + max(1024, ceil(8 sqrt R))) / 32).  sigma(R_i) <= sqrt(R)/2 by Eq. 2. */
+int64_t pa_capacity(int64_t R);
+
+/* Bytes of device workspace pa_create_ex needs for (L, R): two packed spin buffers of R_cap
+ * replicas (the population and the "new population vector" of L165) plus per-replica vectors,
+ * tables and scalars. */
+int pa_workspace_bytes(int L, int64_t R, size_t* bytes);
+
+/* Step 1 (L55, L65): R independent replicas with i.i.d. uniform +-1 spins (equilibrium at
+ * beta_0 = 0), drawn from the INIT stream of the Philox4x32-10 generator keyed by `seed` (O1).
+ * Sets ln Z = N ln 2 (L93), sweep counter t = 0, resample counter k = 0, empty histograms.
+ * L even, 4 <= L <= 512; 1 <= R <= 2^31.
+ * pa_create allocates with cudaMalloc on the current device and uses its own stream.
+ * pa_create_ex borrows `dev_ws` (device memory, >= pa_workspace_bytes, 256-byte aligned; e.g.
+ * a torch tensor's data_ptr()) and enqueues on `cuda_stream` (a cudaStream_t; NULL = the
+ * legacy default stream).  The handle must be destroyed before the workspace is freed. */
+int pa_create(int L, int64_t R, uint64_t seed, pa_t** out);
+int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out);
+void pa_destroy(pa_t* h);
+
+/* Step 3 (L61; L151-L157): theta checkerboard Metropolis sweeps of every replica at inverse
+ * temperature beta.  One sweep = colour 0 ((x+y) even), then colour 1.  A spin with u
+ * anti-parallel neighbours (dE = 8 - 4u) flips iff u >= 2, or u = 1 and x < T4, or u = 0 and
+ * x < T8, with x = the SWEEP-stream uint32 of (slot j, site s, sweep t, colour c) (O1, O3) and
+ * T4, T8 = floor(exp(-4 beta) 2^32), floor(exp(-8 beta) 2^32) clamped to 2^32-1, computed on
+ * the host (O2; L163).  Advances t by theta.  Asynchronous. */
+int pa_sweep(pa_t* h, double beta, int theta);
+
+/* Configurational energies E_j = -sum_<ab> s_a s_b and magnetisations M_j = sum_a s_a of the
+ * current replicas j = 0..R_cur-1 (Eq. 10; L173).  E_out, M_out: int32[>= R_cur], host or
+ * device; M_out may be NULL.  Synchronises if an output is a host pointer. */
+int pa_energies(pa_t* h, int32_t* E_out, int32_t* M_out);
+
+/* Step 2 (L56-L58, L65-L69): resample from beta to beta_new >= beta.
+ *   w_j = exp(-(beta_new - beta)(E_j - E_min))          (Eq. 1 with the common factor taken out, O5)
+ *   W = sum_j w_j in the fixed TREE1024 order (O5; L165: deterministic),  ln Q = -dbeta E_min + ln(W / R_cur)
+ *   tau_j = R w_j / W,  r_j = floor(tau_j) + [u_j < frac(tau_j)],  u_j = RESAMPLE-stream uniform (Eq. 2, O6)
+ *   o_j = sum_{i<j} r_i,  R_new = sum_j r_j,  new[o_j + c] = old[j] for c < r_j   (L165, O7)
+ * Then R_cur = R_new, k += 1, ln Z += ln Q (Eq. 4).  R_new is also written to *R_new (may be NULL).
+ * PA_ERR_CAPACITY if R_new > R_cap or R_new = 0: population, k and ln Z unchanged.  Synchronises. */
+int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new);
+
+/* Sec. 2.3 (L113-L118), Eq. 8: the overlap alpha(dbeta) = (1/R_cur) sum_j min(1, tau_j(dbeta)),
+ * summed in the TREE1024 order.  0 < target_overlap < 1, beta_max > beta.
+ * Returns in *dbeta: beta_max - beta if alpha(beta_max - beta) >= target; otherwise the lower end
+ * of the bracket after exactly 40 bisection steps starting from [0, beta_max - beta] (O10), so
+ * that alpha(*dbeta) >= target.  Does not change the population.  Synchronises. */
+int pa_adapt_dbeta(pa_t* h, double target_overlap, double beta, double beta_max, double* dbeta);
+/* alpha(dbeta) of Eq. 8 for one dbeta >= 0 (the function pa_adapt_dbeta bisects on). */
+int pa_overlap(pa_t* h, double dbeta, double* alpha);
+
+/* Step 4 (L62): population averages of the current population at `beta` (Eq. 3-5; field list
+ * L179-L181).  Integer sums are exact; the m^4 sum uses the TREE1024 order (O8).  No side
+ * effects.  Synchronises. */
+int pa_observables(pa_t* h, double beta, pa_obs_t* out);
+
+/* Sec. 2.4, Eq. 9 (L124-L129): fold the energy histogram of the current population at `beta`
+ * into the running sums  Hsum[m] += #{j : E_j = -2N + 4m}  and
+ * lnD[m] = logaddexp(lnD[m], ln R_cur - ln Z - beta (-2N + 4m))   (O9).
+ * Call once per temperature, after the sweeps.  Asynchronous. */
+int pa_hist_accumulate(pa_t* h, double beta);
+/* Hsum: int64[N+1], lnD: double[N+1] (either may be NULL); ln Omega(E_m) = ln Hsum[m] - lnD[m]. */
+int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD);
+
+/* State export / import (parity tests, checkpoints, the end-to-end benchmark).
+ * Spins are +1 / -1, one int8 per spin, out[i][s] with site s = y*L + x.
+ * pa_get_spins: replicas j0 .. j0+nrep-1.  pa_get_spins_at: replicas slots[0..n-1] (host int64).
+ * pa_set_spins overwrites replicas j0 .. j0+nrep-1 (j0 + nrep <= R_cur).
+ * pa_get_words / pa_set_words move the packed population, uint32 words[ceil(R_cur/32)][N] with
+ * word (g, s) holding replica 32g+b at site s = y*L + x in bit b (the interchange layout; the
+ * resident layout is colour-split).  pa_set_words also sets R_cur = R
+ * (1 <= R <= R_cap) and leaves t, k, ln Z untouched. */
+int pa_get_spins(pa_t* h, int64_t j0, int64_t nrep, int8_t* out);
+int pa_get_spins_at(pa_t* h, const int64_t* slots, int64_t n, int8_t* out);
+int pa_set_spins(pa_t* h, int64_t j0, int64_t nrep, const int8_t* in);
+int pa_get_words(pa_t* h, uint32_t* words);
+int pa_set_words(pa_t* h, int64_t R, const uint32_t* words);
+
+/* Vectors of the last pa_resample, indexed by the parent slot j < R_prev (any may be NULL):
+ * W (one double), w[R_prev] double, r[R_prev] uint32 copy numbers, o[R_prev] uint32 offsets. */
+int pa_get_resample_debug(pa_t* h, double* W, double* w, uint32_t* r, uint32_t* o);
+
+/* Scalars of the handle. */
+int64_t pa_population(const pa_t* h);       /* R_cur */
+int64_t pa_capacity_of(const pa_t* h);      /* R_cap */
+uint32_t pa_sweep_counter(const pa_t* h);   /* t */
+uint32_t pa_resample_counter(const pa_t* h);/* k */
+double pa_lnZ(const pa_t* h);               /* = -beta F(beta), Eq. 4 */
+/* Overwrite the counters (restart from a checkpoint; sampled parity checks at the large configs). */
+int pa_set_counters(pa_t* h, uint32_t t, uint32_t k, double lnZ);
+
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+int64_t pa_launch_count(const pa_t* h);
+/* Device time in milliseconds of the last pa_sweep / the last pa_resample on this handle,
+ * measured with CUDA events on the handle's stream; the kernel that dominates each is the
+ * sweep kernel / the replica-copy kernel (time of that kernel alone in *kernel_ms).
+ * Synchronises.  Either pointer may be NULL. */
+int pa_last_sweep_ms(pa_t* h, float* kernel_ms);
+int pa_last_resample_ms(pa_t* h, float* total_ms, float* copy_kernel_ms);
+
+/* Integer-pipe calibration for the roofline denominator: runs a dependent
+ * chain of `kind` = 0: LOP3, 1: IMAD.WIDE.U32, 2: the Philox round's mix (2 IMAD.WIDE + 2 LOP3),
+ * on every SM and returns the achieved thread-instructions per nanosecond of the whole GPU in
+ * *ginstr_per_ns and the SM clock it ran at in *sm_mhz (from the cycle counter).  Uses the
+ * current device and the default stream; synchronises. */
+int pa_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz);
+
+const char* pa_strerror(int code);
+const char* pa_last_cuda_error(const pa_t* h);
+const char* pa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PA_B200_PA_H */

@@ -1,0 +1,461 @@
+// pa_api.cu -- the C ABI of include/pa.h: handle, workspace layout, host-side step logic
+// (threshold and weight tables, bisection, observables from exact integer sums).
+// All arithmetic that decides an integer (thresholds, weight table) is computed here on the host in
+// fp64 with libm and handed to the kernels as data (O2, O5); the device never calls exp for a decision.
+#include "pa_common.cuh"
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <new>
+
+#define PA_ALIGN 256
+#define PA_STAGE_BYTES ((size_t)32 << 20)
+#define PA_SLOTS_CAP 65536
+
+static size_t pa_align_up(size_t v) { return (v + PA_ALIGN - 1) / PA_ALIGN * PA_ALIGN; }
+
+void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const char* file, int line) {
+    if (h) snprintf(h->cuda_err, sizeof(h->cuda_err), "%s: %s (%s:%d)", cudaGetErrorString(e), what, file, line);
+}
+
+struct PaLayout {
+    size_t spins0, spins1, E, M, w, r, o, parent, partials, wtab, scan, Hsum, Hcur, lnD, scal, slots, stage, total;
+    size_t stage_bytes;
+    int64_t R_cap, G_cap, tiles;
+};
+
+static PaLayout pa_layout(int L, int64_t R) {
+    PaLayout y;
+    const size_t N = (size_t)L * L;
+    y.R_cap = pa_capacity(R);
+    y.G_cap = y.R_cap / 32;
+    y.tiles = (y.R_cap + PA_TILE - 1) / PA_TILE;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t at = off; off = pa_align_up(off + bytes); return at; };
+    y.spins0 = take((size_t)y.G_cap * N * 4);
+    y.spins1 = take((size_t)y.G_cap * N * 4);
+    y.E = take((size_t)y.R_cap * 4);
+    y.M = take((size_t)y.R_cap * 4);
+    y.w = take((size_t)y.R_cap * 8);
+    y.r = take((size_t)y.R_cap * 4);
+    y.o = take((size_t)y.R_cap * 4);
+    y.parent = take((size_t)y.R_cap * 4);
+    y.partials = take((size_t)y.tiles * 8);
+    y.wtab = take((N + 1) * 8);
+    y.scan = take((size_t)y.tiles * 8);
+    y.Hsum = take((N + 1) * 8);
+    y.Hcur = take((N + 1) * 4);
+    y.lnD = take((N + 1) * 8);
+    y.scal = take(sizeof(PaScalars));
+    y.slots = take((size_t)PA_SLOTS_CAP * 8);
+    y.stage_bytes = (size_t)y.R_cap * N < PA_STAGE_BYTES ? pa_align_up((size_t)y.R_cap * N) : PA_STAGE_BYTES;
+    if (y.stage_bytes < (size_t)N * 4 * 4) y.stage_bytes = pa_align_up((size_t)N * 4 * 4);
+    y.stage = take(y.stage_bytes);
+    y.total = off;
+    return y;
+}
+
+static bool pa_args_ok(int L, int64_t R) { return L >= 4 && L <= 512 && (L & 1) == 0 && R >= 1 && R <= (int64_t)1 << 31; }
+
+// O2: T(p) = (uint32) min(floor(p * 2^32), 2^32 - 1)
+static uint32_t pa_threshold(double p) {
+    double v = floor(p * 4294967296.0);
+    if (v > 4294967295.0) v = 4294967295.0;
+    if (v < 0.0) v = 0.0;
+    return (uint32_t)v;
+}
+
+static bool pa_is_device_ptr(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+static int pa_copy_out(pa_handle* h, void* dst, const void* dev_src, size_t bytes, bool* synced) {
+    if (bytes == 0) return PA_OK;
+    if (pa_is_device_ptr(dst)) {
+        PA_CUDA(h, cudaMemcpyAsync(dst, dev_src, bytes, cudaMemcpyDeviceToDevice, h->stream));
+    } else {
+        PA_CUDA(h, cudaMemcpyAsync(dst, dev_src, bytes, cudaMemcpyDeviceToHost, h->stream));
+        PA_CUDA(h, cudaStreamSynchronize(h->stream));
+        if (synced) *synced = true;
+    }
+    return PA_OK;
+}
+
+static int pa_read_scalars(pa_handle* h) {
+    PA_CUDA(h, cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToHost, h->stream));
+    PA_CUDA(h, cudaStreamSynchronize(h->stream));
+    return PA_OK;
+}
+
+static int pa_ensure_energies(pa_handle* h) { return h->em_valid ? PA_OK : pa_launch_energy(h); }
+
+// O5: wtab[d] = exp(-(dbeta * (double)(4 d))), d = 0..dmax, uploaded to the device table
+static int pa_upload_wtab(pa_handle* h, double dbeta, int dmax) {
+    for (int d = 0; d <= dmax; ++d) h->h_wtab[d] = exp(-(dbeta * (double)(4 * d)));
+    PA_CUDA(h, cudaMemcpyAsync(h->wtab, h->h_wtab, sizeof(double) * (size_t)(dmax + 1), cudaMemcpyHostToDevice, h->stream));
+    return PA_OK;
+}
+
+extern "C" {
+
+int64_t pa_capacity(int64_t R) {
+    int64_t slack = (int64_t)ceil(8.0 * sqrt((double)R));
+    if (slack < 1024) slack = 1024;
+    return 32 * ((R + slack + 31) / 32);
+}
+
+int pa_workspace_bytes(int L, int64_t R, size_t* bytes) {
+    if (!bytes || !pa_args_ok(L, R)) return PA_ERR_INVALID_ARG;
+    *bytes = pa_layout(L, R).total;
+    return PA_OK;
+}
+
+int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out) {
+    if (!out || !pa_args_ok(L, R)) return PA_ERR_INVALID_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return PA_ERR_CUDA; }
+    const PaLayout y = pa_layout(L, R);
+    pa_handle* h = new (std::nothrow) pa_handle();
+    if (!h) return PA_ERR_NOMEM;
+    memset(h, 0, sizeof(*h));
+    h->L = L; h->N = L * L; h->R_target = R; h->R_cur = R; h->R_cap = y.R_cap; h->G_cap = y.G_cap;
+    h->seed = seed; h->keys = pa_make_keys(seed);
+    h->lnZ = (double)h->N * log(2.0);           // Z_{beta_0} = 2^N (L93)
+    h->n_tiles_cap = y.tiles;
+    int rc = PA_OK;
+    if (dev_ws) {
+        if (ws_bytes < y.total || ((uintptr_t)dev_ws % PA_ALIGN) != 0) { delete h; return PA_ERR_WORKSPACE; }
+        h->ws = dev_ws; h->owns_ws = false; h->stream = (cudaStream_t)cuda_stream; h->owns_stream = false;
+    } else {
+        cudaError_t e = cudaMalloc(&h->ws, y.total);
+        if (e != cudaSuccess) { cudaGetLastError(); delete h; return e == cudaErrorMemoryAllocation ? PA_ERR_NOMEM : PA_ERR_CUDA; }
+        h->owns_ws = true;
+        if (cudaStreamCreateWithFlags(&h->stream, cudaStreamNonBlocking) != cudaSuccess) { cudaFree(h->ws); delete h; return PA_ERR_CUDA; }
+        h->owns_stream = true;
+    }
+    h->ws_bytes = y.total;
+    char* b = (char*)h->ws;
+    h->spins[0] = (uint32_t*)(b + y.spins0); h->spins[1] = (uint32_t*)(b + y.spins1); h->cur = 0;
+    h->E = (int32_t*)(b + y.E); h->M = (int32_t*)(b + y.M);
+    h->w = (double*)(b + y.w); h->r = (uint32_t*)(b + y.r); h->o = (uint32_t*)(b + y.o); h->parent = (uint32_t*)(b + y.parent);
+    h->partials = (double*)(b + y.partials); h->wtab = (double*)(b + y.wtab);
+    h->scan_state = (unsigned long long*)(b + y.scan);
+    h->Hsum = (unsigned long long*)(b + y.Hsum); h->Hcur = (uint32_t*)(b + y.Hcur); h->lnD = (double*)(b + y.lnD);
+    h->d_scal = (PaScalars*)(b + y.scal);
+    h->d_slots = (int64_t*)(b + y.slots);
+    h->stage = (int8_t*)(b + y.stage); h->stage_bytes = y.stage_bytes;
+    // pinned host mirrors
+    if (cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
+        cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->N + 1)) != cudaSuccess) { rc = PA_ERR_CUDA; }
+    for (int i = 0; i < 6 && rc == PA_OK; ++i)
+        if (cudaEventCreate(&h->ev[i]) != cudaSuccess) rc = PA_ERR_CUDA;
+    if (rc == PA_OK) rc = pa_sweep_configure(h);
+    if (rc == PA_OK) {
+        // empty histograms: Hsum = 0, Hcur = 0, lnD = -inf
+        cudaMemsetAsync(h->Hsum, 0, ((size_t)h->N + 1) * 8, h->stream);
+        cudaMemsetAsync(h->Hcur, 0, ((size_t)h->N + 1) * 4, h->stream);
+        for (int m = 0; m <= h->N; ++m) h->h_wtab[m] = -INFINITY;
+        if (cudaMemcpyAsync(h->lnD, h->h_wtab, ((size_t)h->N + 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
+        if (rc == PA_OK) rc = pa_launch_init(h);
+        if (rc == PA_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
+    }
+    if (rc != PA_OK) { pa_destroy(h); return rc; }
+    *out = h;
+    return PA_OK;
+}
+
+int pa_create(int L, int64_t R, uint64_t seed, pa_t** out) { return pa_create_ex(L, R, seed, nullptr, 0, nullptr, out); }
+
+void pa_destroy(pa_t* h) {
+    if (!h) return;
+    cudaStreamSynchronize(h->stream);
+    for (int i = 0; i < 6; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    if (h->h_scal) cudaFreeHost(h->h_scal);
+    if (h->h_wtab) cudaFreeHost(h->h_wtab);
+    if (h->owns_stream && h->stream) cudaStreamDestroy(h->stream);
+    if (h->owns_ws && h->ws) cudaFree(h->ws);
+    delete h;
+}
+
+int pa_sweep(pa_t* h, double beta, int theta) {
+    if (!h || theta < 0 || !(beta == beta)) return PA_ERR_INVALID_ARG;
+    if (theta == 0) return PA_OK;
+    const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
+    PA_CUDA(h, cudaEventRecord(h->ev[0], h->stream));
+    int rc = pa_launch_sweep(h, T4, T8, theta);
+    if (rc != PA_OK) return rc;
+    PA_CUDA(h, cudaEventRecord(h->ev[1], h->stream));
+    h->sweep_timed = true;
+    h->t += (uint32_t)theta;
+    h->em_valid = false;
+    return PA_OK;
+}
+
+int pa_energies(pa_t* h, int32_t* E_out, int32_t* M_out) {
+    if (!h || !E_out) return PA_ERR_INVALID_ARG;
+    int rc = pa_ensure_energies(h);
+    if (rc != PA_OK) return rc;
+    rc = pa_copy_out(h, E_out, h->E, sizeof(int32_t) * (size_t)h->R_cur, nullptr);
+    if (rc == PA_OK && M_out) rc = pa_copy_out(h, M_out, h->M, sizeof(int32_t) * (size_t)h->R_cur, nullptr);
+    return rc;
+}
+
+int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
+    if (!h || !(beta_new >= beta)) return PA_ERR_INVALID_ARG;
+    const double dbeta = beta_new - beta;
+    int rc;
+    PA_CUDA(h, cudaEventRecord(h->ev[2], h->stream));
+    if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
+    if ((rc = pa_launch_minmax(h)) != PA_OK) return rc;
+    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    const int Emin = h->h_scal->Emin, Emax = h->h_scal->Emax;
+    if ((rc = pa_upload_wtab(h, dbeta, (Emax - Emin) / 4)) != PA_OK) return rc;
+    if ((rc = pa_launch_tree_weights(h, 0, h->w)) != PA_OK) return rc;
+    if ((rc = pa_launch_plan(h)) != PA_OK) return rc;
+    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    const int64_t R_new = (int64_t)h->h_scal->R_new;
+    const double W = h->h_scal->W;
+    h->R_prev = h->R_cur; h->W_last = W;
+    if (R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;      // population, k, lnZ unchanged (O7)
+    PA_CUDA(h, cudaEventRecord(h->ev[4], h->stream));
+    if ((rc = pa_launch_copy(h, R_new)) != PA_OK) return rc;
+    PA_CUDA(h, cudaEventRecord(h->ev[5], h->stream));
+    PA_CUDA(h, cudaEventRecord(h->ev[3], h->stream));
+    h->resample_timed = true;
+    const double lnQ = -dbeta * (double)Emin + log(W / (double)h->R_cur);   // Eq. 1 with the shift (O5)
+    h->cur ^= 1;
+    h->R_cur = R_new;
+    h->k += 1;
+    h->lnZ += lnQ;                                                    // Eq. 4 (L90)
+    h->lnQ_last = lnQ;
+    h->em_valid = false;
+    if (R_new_out) *R_new_out = R_new;
+    return PA_OK;
+}
+
+// alpha(dbeta) of Eq. 8 given Emin/Emax already on the host
+static int pa_eval_overlap(pa_handle* h, double dbeta, int Emin, int Emax, double* alpha) {
+    int rc;
+    if ((rc = pa_upload_wtab(h, dbeta, (Emax - Emin) / 4)) != PA_OK) return rc;
+    if ((rc = pa_launch_tree_weights(h, 0, nullptr)) != PA_OK) return rc;
+    if ((rc = pa_launch_tree_weights(h, 1, nullptr)) != PA_OK) return rc;
+    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    *alpha = h->h_scal->sum / (double)h->R_cur;
+    return PA_OK;
+}
+
+static int pa_overlap_prepare(pa_handle* h, int* Emin, int* Emax) {
+    int rc;
+    if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
+    if ((rc = pa_launch_minmax(h)) != PA_OK) return rc;
+    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    *Emin = h->h_scal->Emin; *Emax = h->h_scal->Emax;
+    return PA_OK;
+}
+
+int pa_overlap(pa_t* h, double dbeta, double* alpha) {
+    if (!h || !alpha || !(dbeta >= 0.0)) return PA_ERR_INVALID_ARG;
+    int Emin, Emax, rc;
+    if ((rc = pa_overlap_prepare(h, &Emin, &Emax)) != PA_OK) return rc;
+    return pa_eval_overlap(h, dbeta, Emin, Emax, alpha);
+}
+
+int pa_adapt_dbeta(pa_t* h, double target, double beta, double beta_max, double* dbeta_out) {
+    if (!h || !dbeta_out || !(target > 0.0 && target < 1.0) || !(beta_max > beta)) return PA_ERR_INVALID_ARG;
+    int Emin, Emax, rc;
+    if ((rc = pa_overlap_prepare(h, &Emin, &Emax)) != PA_OK) return rc;
+    double hi = beta_max - beta, a;
+    if ((rc = pa_eval_overlap(h, hi, Emin, Emax, &a)) != PA_OK) return rc;
+    if (a >= target) { *dbeta_out = hi; return PA_OK; }
+    double lo = 0.0;
+    for (int it = 0; it < 40; ++it) {                                // O10: exactly 40 bisection steps
+        const double mid = 0.5 * (lo + hi);
+        if ((rc = pa_eval_overlap(h, mid, Emin, Emax, &a)) != PA_OK) return rc;
+        if (a >= target) lo = mid; else hi = mid;
+    }
+    *dbeta_out = lo;
+    return PA_OK;
+}
+
+int pa_observables(pa_t* h, double beta, pa_obs_t* out) {
+    if (!h || !out) return PA_ERR_INVALID_ARG;
+    int rc;
+    if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
+    if ((rc = pa_launch_obs_sums(h)) != PA_OK) return rc;
+    if ((rc = pa_launch_tree_weights(h, 2, nullptr)) != PA_OK) return rc;
+    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    const PaScalars& s = *h->h_scal;
+    const double R = (double)h->R_cur, N = (double)h->N;
+    const __int128 num = (__int128)h->R_cur * (__int128)s.SE2 - (__int128)s.SE * (__int128)s.SE;   // exact (O8)
+    out->beta = beta;
+    out->e = (double)s.SE / (R * N);
+    out->C = beta * beta * ((double)num / (R * R * N));
+    out->absm = (double)s.SA / (R * N);
+    out->m2 = (double)s.SM2 / (R * N * N);
+    out->m4 = s.sum / R;
+    out->betaF_per_N = -h->lnZ / N;
+    out->S_per_N = beta * out->e + h->lnZ / N;
+    out->lnQ = h->lnQ_last;
+    out->R = h->R_cur;
+    return PA_OK;
+}
+
+int pa_hist_accumulate(pa_t* h, double beta) {
+    if (!h) return PA_ERR_INVALID_ARG;
+    int rc;
+    if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
+    return pa_launch_hist(h, beta);
+}
+
+int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD) {
+    if (!h) return PA_ERR_INVALID_ARG;
+    int rc = PA_OK;
+    if (Hsum) rc = pa_copy_out(h, Hsum, h->Hsum, ((size_t)h->N + 1) * 8, nullptr);
+    if (rc == PA_OK && lnD) rc = pa_copy_out(h, lnD, h->lnD, ((size_t)h->N + 1) * 8, nullptr);
+    return rc;
+}
+
+static int pa_get_spins_impl(pa_handle* h, const int64_t* slots, int64_t j0, int64_t n, int8_t* out) {
+    const bool dev_out = pa_is_device_ptr(out);
+    const size_t N = (size_t)h->N;
+    int64_t chunk = (int64_t)(h->stage_bytes / N);
+    if (chunk > PA_SLOTS_CAP) chunk = PA_SLOTS_CAP;
+    if (chunk < 1) return PA_ERR_WORKSPACE;
+    int64_t* d_slots = h->d_slots;
+    for (int64_t a = 0; a < n; a += chunk) {
+        const int64_t m = n - a < chunk ? n - a : chunk;
+        if (slots) PA_CUDA(h, cudaMemcpyAsync(d_slots, slots + a, sizeof(int64_t) * (size_t)m, cudaMemcpyHostToDevice, h->stream));
+        int8_t* target = dev_out ? out + (size_t)a * N : h->stage;
+        int rc = pa_launch_unpack(h, slots ? d_slots : nullptr, j0 + a, m, target);
+        if (rc != PA_OK) return rc;
+        if (!dev_out) {
+            PA_CUDA(h, cudaMemcpyAsync(out + (size_t)a * N, h->stage, (size_t)m * N, cudaMemcpyDeviceToHost, h->stream));
+            PA_CUDA(h, cudaStreamSynchronize(h->stream));
+        } else if (slots) {
+            PA_CUDA(h, cudaStreamSynchronize(h->stream));
+        }
+    }
+    return PA_OK;
+}
+
+int pa_get_spins(pa_t* h, int64_t j0, int64_t nrep, int8_t* out) {
+    if (!h || !out || j0 < 0 || nrep < 0 || j0 + nrep > h->R_cur) return PA_ERR_INVALID_ARG;
+    return pa_get_spins_impl(h, nullptr, j0, nrep, out);
+}
+
+int pa_get_spins_at(pa_t* h, const int64_t* slots, int64_t n, int8_t* out) {
+    if (!h || !out || !slots || n < 0) return PA_ERR_INVALID_ARG;
+    for (int64_t i = 0; i < n; ++i) if (slots[i] < 0 || slots[i] >= h->R_cur) return PA_ERR_INVALID_ARG;
+    return pa_get_spins_impl(h, slots, 0, n, out);
+}
+
+int pa_set_spins(pa_t* h, int64_t j0, int64_t nrep, const int8_t* in) {
+    if (!h || !in || j0 < 0 || nrep < 0 || j0 + nrep > h->R_cur) return PA_ERR_INVALID_ARG;
+    const bool dev_in = pa_is_device_ptr(in);
+    const size_t N = (size_t)h->N;
+    const int64_t chunk = (int64_t)(h->stage_bytes / N);
+    for (int64_t a = 0; a < nrep; a += chunk) {
+        const int64_t m = nrep - a < chunk ? nrep - a : chunk;
+        const int8_t* src = in + (size_t)a * N;
+        if (!dev_in) {
+            PA_CUDA(h, cudaMemcpyAsync(h->stage, src, (size_t)m * N, cudaMemcpyHostToDevice, h->stream));
+            src = h->stage;
+        }
+        int rc = pa_launch_pack(h, j0 + a, m, src);
+        if (rc != PA_OK) return rc;
+        PA_CUDA(h, cudaStreamSynchronize(h->stream));
+    }
+    h->em_valid = false;
+    return PA_OK;
+}
+
+int pa_get_words(pa_t* h, uint32_t* words) {
+    if (!h || !words) return PA_ERR_INVALID_ARG;
+    const size_t bytes = (size_t)((h->R_cur + 31) / 32) * h->N * 4;
+    if (pa_is_device_ptr(words)) return pa_launch_words_out(h, words);
+    // host destination: convert into the spare population buffer, then copy out
+    int rc = pa_launch_words_out(h, h->spins[1 - h->cur]);
+    if (rc != PA_OK) return rc;
+    PA_CUDA(h, cudaMemcpyAsync(words, h->spins[1 - h->cur], bytes, cudaMemcpyDeviceToHost, h->stream));
+    PA_CUDA(h, cudaStreamSynchronize(h->stream));
+    return PA_OK;
+}
+
+int pa_set_words(pa_t* h, int64_t R, const uint32_t* words) {
+    if (!h || !words || R < 1 || R > h->R_cap) return PA_ERR_INVALID_ARG;
+    const size_t bytes = (size_t)((R + 31) / 32) * h->N * 4;
+    const uint32_t* src = words;
+    if (!pa_is_device_ptr(words)) {
+        PA_CUDA(h, cudaMemcpyAsync(h->spins[1 - h->cur], words, bytes, cudaMemcpyHostToDevice, h->stream));
+        src = h->spins[1 - h->cur];
+    }
+    int rc = pa_launch_words_in(h, R, src);
+    if (rc != PA_OK) return rc;
+    h->R_cur = R;
+    h->em_valid = false;
+    return PA_OK;
+}
+
+int pa_get_resample_debug(pa_t* h, double* W, double* w, uint32_t* r, uint32_t* o) {
+    if (!h) return PA_ERR_INVALID_ARG;
+    int rc = PA_OK;
+    const size_t n = (size_t)h->R_prev;
+    if (W) *W = h->W_last;
+    if (w) rc = pa_copy_out(h, w, h->w, n * 8, nullptr);
+    if (rc == PA_OK && r) rc = pa_copy_out(h, r, h->r, n * 4, nullptr);
+    if (rc == PA_OK && o) rc = pa_copy_out(h, o, h->o, n * 4, nullptr);
+    return rc;
+}
+
+int64_t pa_population(const pa_t* h) { return h ? h->R_cur : 0; }
+int64_t pa_capacity_of(const pa_t* h) { return h ? h->R_cap : 0; }
+uint32_t pa_sweep_counter(const pa_t* h) { return h ? h->t : 0; }
+uint32_t pa_resample_counter(const pa_t* h) { return h ? h->k : 0; }
+double pa_lnZ(const pa_t* h) { return h ? h->lnZ : 0.0; }
+int pa_set_counters(pa_t* h, uint32_t t, uint32_t k, double lnZ) {
+    if (!h) return PA_ERR_INVALID_ARG;
+    h->t = t; h->k = k; h->lnZ = lnZ;
+    return PA_OK;
+}
+int64_t pa_launch_count(const pa_t* h) { return h ? h->launches : 0; }
+
+int pa_last_sweep_ms(pa_t* h, float* kernel_ms) {
+    if (!h || !h->sweep_timed) return PA_ERR_INVALID_ARG;
+    PA_CUDA(h, cudaEventSynchronize(h->ev[1]));
+    float ms = 0.f;
+    PA_CUDA(h, cudaEventElapsedTime(&ms, h->ev[0], h->ev[1]));
+    if (kernel_ms) *kernel_ms = ms;
+    return PA_OK;
+}
+int pa_last_resample_ms(pa_t* h, float* total_ms, float* copy_kernel_ms) {
+    if (!h || !h->resample_timed) return PA_ERR_INVALID_ARG;
+    PA_CUDA(h, cudaEventSynchronize(h->ev[3]));
+    float a = 0.f, b = 0.f;
+    PA_CUDA(h, cudaEventElapsedTime(&a, h->ev[2], h->ev[3]));
+    PA_CUDA(h, cudaEventElapsedTime(&b, h->ev[4], h->ev[5]));
+    if (total_ms) *total_ms = a;
+    if (copy_kernel_ms) *copy_kernel_ms = b;
+    return PA_OK;
+}
+
+int pa_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz) { return pa_run_calibrate(kind, ginstr_per_ns, sm_mhz); }
+
+const char* pa_strerror(int code) {
+    switch (code) {
+        case PA_OK: return "ok";
+        case PA_ERR_INVALID_ARG: return "invalid argument";
+        case PA_ERR_CAPACITY: return "resampled population would exceed the capacity (or be empty)";
+        case PA_ERR_CUDA: return "CUDA error";
+        case PA_ERR_WORKSPACE: return "workspace too small or misaligned";
+        case PA_ERR_NOMEM: return "out of memory";
+        default: return "unknown error";
+    }
+}
+const char* pa_last_cuda_error(const pa_t* h) { return h ? h->cuda_err : ""; }
+const char* pa_version(void) { return "pa-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

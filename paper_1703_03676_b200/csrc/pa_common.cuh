@@ -1,0 +1,133 @@
+// pa_common.cuh -- shared declarations of the CUDA library (handle, layout, Philox, error macros).
+// Product code: shares nothing with oracle/.  Citations "L<n>" = /root/reference/PAPER.md line n,
+// "O<n>" = reading n of DESIGN.md Sec. 3.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/pa.h"
+
+// ------------------------------------------------------------------------------------------------
+// Resident layout.  One "group" = 32 replica slots = one uint32 per site
+// (asynchronous multi-spin coding with p = 32, L185); bit b of a word of group g = replica 32g+b.
+// Inside a group the N = L*L words are split by checkerboard colour c = (x+y)&1 (the paper stores
+// the two sub-lattices separately too, L157):   index(c, y, xh) = c*(N/2) + y*(L/2) + xh,
+// xh = x >> 1.   Site (x,y) of colour c in row y has x = 2*xh + ((y+c)&1).
+// ------------------------------------------------------------------------------------------------
+#define PA_TAG_INIT 0u
+#define PA_TAG_SWEEP 1u
+#define PA_TAG_RESAMPLE 2u
+
+#define PA_PHILOX_M0 0xD2511F53u
+#define PA_PHILOX_M1 0xCD9E8D57u
+#define PA_PHILOX_W0 0x9E3779B9u
+#define PA_PHILOX_W1 0xBB67AE85u
+
+#define PA_TILE 1024  // elements per reduction / scan tile (TREE1024, O5)
+
+struct PhiloxKeys {  // the 10 round keys of Philox4x32-10 for one 64-bit seed (uniform per launch)
+    uint32_t k0[10], k1[10];
+};
+
+static inline PhiloxKeys pa_make_keys(uint64_t seed) {
+    PhiloxKeys k;
+    uint32_t a = (uint32_t)(seed & 0xffffffffull), b = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) { k.k0[r] = a; k.k1[r] = b; a += PA_PHILOX_W0; b += PA_PHILOX_W1; }
+    return k;
+}
+
+#ifdef __CUDACC__
+__device__ __forceinline__ void pa_mulhilo(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo) {
+    unsigned long long p = (unsigned long long)a * (unsigned long long)b;   // IMAD.WIDE.U32
+    hi = (uint32_t)(p >> 32);
+    lo = (uint32_t)p;
+}
+// Plain Philox4x32-10 (ref. [33], L368; L163), used where the call is not the bottleneck.
+__device__ __forceinline__ uint4 pa_philox(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, const PhiloxKeys& K) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0, lo0, hi1, lo1;
+        pa_mulhilo(PA_PHILOX_M0, c0, hi0, lo0);
+        pa_mulhilo(PA_PHILOX_M1, c2, hi1, lo1);
+        uint32_t n0 = hi1 ^ c1 ^ K.k0[r], n2 = hi0 ^ c3 ^ K.k1[r];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+#endif
+
+// device-resident scalars (one block, also mirrored in pinned host memory for small D2H reads)
+struct PaScalars {
+    int32_t Emin, Emax;
+    uint32_t tile_counter;
+    uint32_t R_new;
+    double sum;              // result of the last TREE1024 reduction
+    double W;                // normaliser of the current weight table
+    long long SE, SE2, SA, SM2;
+    uint32_t pad[4];
+};
+
+struct pa_handle {
+    int L, N;
+    int64_t R_target, R_cur, R_cap;
+    int64_t G_cap;           // groups at capacity
+    uint64_t seed;
+    uint32_t t, k;
+    double lnZ, lnQ_last;
+    PhiloxKeys keys;
+
+    cudaStream_t stream;
+    bool owns_stream, owns_ws;
+    void* ws; size_t ws_bytes;
+
+    uint32_t* spins[2]; int cur;        // two packed populations [G_cap][N] (L165 "new population vector")
+    int32_t *E, *M; bool em_valid;      // per-replica energy / magnetisation of the current population
+    double* w;                          // weights of the last resample (debug export)
+    uint32_t *r, *o, *parent;           // copy numbers, exclusive offsets, parent map
+    double* partials;                   // per-tile partial sums (TREE1024)
+    double* wtab;                       // weight table, device, N+1 entries
+    unsigned long long* scan_state;     // decoupled look-back tile states
+    unsigned long long* Hsum;           // [N+1]
+    uint32_t* Hcur;                     // [N+1] histogram of the current temperature
+    double* lnD;                        // [N+1]
+    int64_t* d_slots;                   // slot list for pa_get_spins_at
+    int8_t* stage;                      // staging for unpacked spin export/import
+    size_t stage_bytes;
+    PaScalars* d_scal;
+    int64_t n_tiles_cap;
+
+    PaScalars* h_scal;                  // pinned
+    double* h_wtab;                     // pinned, N+1
+    int64_t R_prev; double W_last;      // of the last resample
+
+    cudaEvent_t ev[6];                  // sweep begin/end, resample begin/end, copy begin/end
+    bool sweep_timed, resample_timed;
+    int64_t launches;
+    int sweep_C, sweep_T, sweep_cmp;    // sweep launch geometry (cluster size, threads) and compare variant
+    char cuda_err[256];
+};
+
+#define PA_CUDA(h, call)                                                                      \
+    do {                                                                                      \
+        cudaError_t e__ = (call);                                                             \
+        if (e__ != cudaSuccess) { pa_note_cuda_error((h), e__, #call, __FILE__, __LINE__); return PA_ERR_CUDA; } \
+    } while (0)
+
+void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const char* file, int line);
+
+// kernels' host launchers (each returns PA_OK / PA_ERR_CUDA and counts its launches in h->launches)
+int pa_launch_init(pa_handle* h);
+int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta);
+int pa_sweep_configure(pa_handle* h);
+int pa_launch_energy(pa_handle* h);
+int pa_launch_minmax(pa_handle* h);
+int pa_launch_tree_weights(pa_handle* h, int mode, double* w_out);   // mode 0: w, 1: min(1,tau), 2: m^4
+int pa_launch_plan(pa_handle* h);                                      // tau, r, scan, parent map
+int pa_launch_copy(pa_handle* h, int64_t R_new);
+int pa_launch_obs_sums(pa_handle* h);
+int pa_launch_hist(pa_handle* h, double beta);
+int pa_launch_unpack(pa_handle* h, const int64_t* d_slots, int64_t j0, int64_t n, int8_t* d_out);
+int pa_launch_pack(pa_handle* h, int64_t j0, int64_t n, const int8_t* d_in);
+int pa_launch_words_out(pa_handle* h, uint32_t* d_words);
+int pa_launch_words_in(pa_handle* h, int64_t R, const uint32_t* d_words);
+int pa_run_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz);

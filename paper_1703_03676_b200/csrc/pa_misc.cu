@@ -1,0 +1,263 @@
+// pa_misc.cu -- initial population (a0), observable sums (a8), energy histogram and multi-histogram
+// accumulation (a9), spin import/export, and the integer-pipe calibration kernels.
+#include "pa_common.cuh"
+#include <math.h>
+
+// site index s = y*L + x of the word at resident index idx (see pa_common.cuh)
+__device__ __forceinline__ int pa_site_of_index(int idx, int L) {
+    const int Lh = L >> 1, half = (L * L) >> 1;
+    const int c = idx >= half ? 1 : 0;
+    const int rem = idx - c * half;
+    const int y = rem / Lh, xh = rem - y * Lh;
+    return y * L + 2 * xh + ((y + c) & 1);
+}
+__device__ __forceinline__ int pa_index_of_site(int s, int L) {
+    const int y = s / L, x = s - y * L;
+    const int c = (x + y) & 1;
+    return c * ((L * L) >> 1) + y * (L >> 1) + (x >> 1);
+}
+
+// a0 (L55, L65; O1): word(g, s) = philox(s, g>>2, 0, TAG_INIT)[g&3]; lanes >= R are cleared.
+__global__ void pa_init_kernel(uint32_t* __restrict__ pop, int L, int N, long long R, PhiloxKeys K) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    const long long G = (R + 31) / 32;
+    if (i >= G * N) return;
+    const long long g = i / N;
+    const int idx = (int)(i - g * N);
+    const int s = pa_site_of_index(idx, L);
+    uint4 x = pa_philox((uint32_t)s, (uint32_t)(g >> 2), 0u, PA_TAG_INIT, K);
+    const uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+    uint32_t w = xs[g & 3];
+    const long long live = R - g * 32;
+    if (live < 32) w &= (1u << live) - 1u;
+    pop[i] = w;
+}
+
+int pa_launch_init(pa_handle* h) {
+    const long long n = ((h->R_cur + 31) / 32) * (long long)h->N;
+    pa_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, h->keys);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
+
+// a8 (Eq. 3; O8): exact integer sums of E, E^2, |M|, M^2 (order-independent).
+__global__ void pa_obs_zero_kernel(PaScalars* sc) { sc->SE = sc->SE2 = sc->SA = sc->SM2 = 0; }
+
+__global__ void pa_obs_sums_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, long long R, PaScalars* sc) {
+    long long se = 0, se2 = 0, sa = 0, sm2 = 0;
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x) {
+        long long e = E[j], m = M[j];
+        se += e; se2 += e * e; sa += m < 0 ? -m : m; sm2 += m * m;
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        se += __shfl_xor_sync(0xffffffffu, se, off);
+        se2 += __shfl_xor_sync(0xffffffffu, se2, off);
+        sa += __shfl_xor_sync(0xffffffffu, sa, off);
+        sm2 += __shfl_xor_sync(0xffffffffu, sm2, off);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd((unsigned long long*)&sc->SE, (unsigned long long)se);
+        atomicAdd((unsigned long long*)&sc->SE2, (unsigned long long)se2);
+        atomicAdd((unsigned long long*)&sc->SA, (unsigned long long)sa);
+        atomicAdd((unsigned long long*)&sc->SM2, (unsigned long long)sm2);
+    }
+}
+
+int pa_launch_obs_sums(pa_handle* h) {
+    pa_obs_zero_kernel<<<1, 1, 0, h->stream>>>(h->d_scal);
+    int blocks = (int)((h->R_cur + 1023) / 1024);
+    if (blocks > 592) blocks = 592;
+    pa_obs_sums_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->M, h->R_cur, h->d_scal);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 2;
+    return PA_OK;
+}
+
+// a9 (Eq. 9; O9)
+__global__ void pa_hist_kernel(const int32_t* __restrict__ E, long long R, int N, uint32_t* __restrict__ Hcur) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x)
+        atomicAdd(&Hcur[(E[j] + 2 * N) >> 2], 1u);
+}
+__global__ void pa_hist_fold_kernel(uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ Hsum,
+                                    double* __restrict__ lnD, int N, double lnR_minus_lnZ, double beta) {
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m > N) return;
+    Hsum[m] += Hcur[m];
+    Hcur[m] = 0;
+    const double Em = (double)(-2 * N + 4 * m);
+    const double term = lnR_minus_lnZ - beta * Em;
+    const double a = lnD[m];
+    double out;
+    if (a == -INFINITY) out = term;
+    else { const double hi = fmax(a, term), lo = fmin(a, term); out = hi + log1p(exp(lo - hi)); }
+    lnD[m] = out;
+}
+
+int pa_launch_hist(pa_handle* h, double beta) {
+    int blocks = (int)((h->R_cur + 255) / 256);
+    if (blocks > 1184) blocks = 1184;
+    pa_hist_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->R_cur, h->N, h->Hcur);
+    const double c = log((double)h->R_cur) - h->lnZ;
+    pa_hist_fold_kernel<<<(h->N + 1 + 255) / 256, 256, 0, h->stream>>>(h->Hcur, h->Hsum, h->lnD, h->N, c, beta);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 2;
+    return PA_OK;
+}
+
+// ---- spin export / import ------------------------------------------------------------------------
+__global__ void pa_unpack_kernel(const uint32_t* __restrict__ pop, int L, int N, const long long* __restrict__ slots,
+                                 long long j0, long long n, int8_t* __restrict__ out) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n * N) return;
+    const long long r = i / N;
+    const int s = (int)(i - r * N);
+    const long long j = slots ? slots[r] : j0 + r;
+    const uint32_t w = pop[(j >> 5) * N + pa_index_of_site(s, L)];
+    out[i] = ((w >> (j & 31)) & 1u) ? 1 : -1;
+}
+__global__ void pa_pack_kernel(uint32_t* __restrict__ pop, int L, int N, long long j0, long long n, const int8_t* __restrict__ in) {
+    // one thread per (group, site): rewrites the bits of replicas j0..j0+n-1 that fall in this word
+    const long long g0 = j0 >> 5, g1 = (j0 + n - 1) >> 5;
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= (g1 - g0 + 1) * N) return;
+    const long long g = g0 + i / N;
+    const int s = (int)(i % N);
+    const long long idx = g * N + pa_index_of_site(s, L);
+    uint32_t w = pop[idx];
+    for (int b = 0; b < 32; ++b) {
+        const long long j = g * 32 + b;
+        if (j >= j0 && j < j0 + n) {
+            const uint32_t bit = in[(j - j0) * N + s] > 0 ? 1u : 0u;
+            w = (w & ~(1u << b)) | (bit << b);
+        }
+    }
+    pop[idx] = w;
+}
+__global__ void pa_words_out_kernel(const uint32_t* __restrict__ pop, int L, int N, long long G, uint32_t* __restrict__ out) {
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= G * N) return;
+    const long long g = i / N;
+    const int s = (int)(i - g * N);
+    out[i] = pop[g * N + pa_index_of_site(s, L)];
+}
+__global__ void pa_words_in_kernel(uint32_t* __restrict__ pop, int L, int N, long long R, const uint32_t* __restrict__ in) {
+    const long long G = (R + 31) / 32;
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= G * N) return;
+    const long long g = i / N;
+    const int s = (int)(i - g * N);
+    uint32_t w = in[i];
+    const long long live = R - g * 32;
+    if (live < 32) w &= (1u << live) - 1u;
+    pop[g * N + pa_index_of_site(s, L)] = w;
+}
+
+int pa_launch_unpack(pa_handle* h, const int64_t* d_slots, int64_t j0, int64_t n, int8_t* d_out) {
+    const long long tot = n * (long long)h->N;
+    if (tot == 0) return PA_OK;
+    pa_unpack_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N,
+                                                                          (const long long*)d_slots, j0, n, d_out);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
+int pa_launch_pack(pa_handle* h, int64_t j0, int64_t n, const int8_t* d_in) {
+    if (n == 0) return PA_OK;
+    const long long ng = ((j0 + n - 1) >> 5) - (j0 >> 5) + 1;
+    const long long tot = ng * h->N;
+    pa_pack_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, j0, n, d_in);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
+int pa_launch_words_out(pa_handle* h, uint32_t* d_words) {
+    const long long G = (h->R_cur + 31) / 32, tot = G * h->N;
+    pa_words_out_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, G, d_words);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
+int pa_launch_words_in(pa_handle* h, int64_t R, const uint32_t* d_words) {
+    const long long G = (R + 31) / 32, tot = G * h->N;
+    pa_words_in_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, R, d_words);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
+
+// ---- integer-pipe calibration -------------------------------------------------
+// Dependent chains with enough independent copies per thread to saturate a pipe; the result is
+// written so nothing is optimised away.  Each loop iteration issues `PER_ITER` instructions of the kind.
+template <int KIND>
+__global__ void __launch_bounds__(256)
+pa_calib_kernel(uint32_t* out, int iters, uint32_t seed, unsigned long long* cycles) {
+    uint32_t a[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = seed + threadIdx.x * 8 + i;
+    unsigned long long q[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) q[i] = ((unsigned long long)a[i] << 32) | (seed * 2654435761u + i);
+    uint32_t k = seed ^ 0x9E3779B9u;
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int rep = 0; rep < 4; ++rep) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                if (KIND == 0) {                       // LOP3: 3-input xor chain
+                    a[i] = a[i] ^ a[(i + 1) & 7] ^ k;
+                } else if (KIND == 1) {                // IMAD.WIDE.U32 chain: p = hi(p) * M0 + p
+                    q[i] = (unsigned long long)(uint32_t)(q[i] >> 32) * PA_PHILOX_M0 + q[i];
+                } else {                               // the Philox round mix: 2 IMAD.WIDE + 2 LOP3
+                    uint32_t h0, l0, h1, l1;
+                    pa_mulhilo(PA_PHILOX_M0, a[i], h0, l0);
+                    pa_mulhilo(PA_PHILOX_M1, a[(i + 4) & 7], h1, l1);
+                    a[i] = h1 ^ l0 ^ k;
+                    a[(i + 4) & 7] = h0 ^ l1 ^ k;
+                }
+            }
+        }
+    }
+    const long long t1 = clock64();
+    uint32_t r = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) r ^= a[i] ^ (uint32_t)q[i] ^ (uint32_t)(q[i] >> 32);
+    out[blockIdx.x * blockDim.x + threadIdx.x] = r;
+    if (threadIdx.x == 0 && blockIdx.x == 0) *cycles = (unsigned long long)(t1 - t0);
+}
+
+int pa_run_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz) {
+    if (kind < 0 || kind > 2) return PA_ERR_INVALID_ARG;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return PA_ERR_CUDA;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int blocks = sms * 8, threads = 256, iters = 4096;
+    uint32_t* d_out = nullptr; unsigned long long* d_cyc = nullptr;
+    if (cudaMalloc(&d_out, (size_t)blocks * threads * 4) != cudaSuccess) return PA_ERR_CUDA;
+    if (cudaMalloc(&d_cyc, 8) != cudaSuccess) { cudaFree(d_out); return PA_ERR_CUDA; }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0);
+        if (kind == 0) pa_calib_kernel<0><<<blocks, threads>>>(d_out, iters, 12345u + rep, d_cyc);
+        else if (kind == 1) pa_calib_kernel<1><<<blocks, threads>>>(d_out, iters, 12345u + rep, d_cyc);
+        else pa_calib_kernel<2><<<blocks, threads>>>(d_out, iters, 12345u + rep, d_cyc);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d_out); cudaFree(d_cyc); return PA_ERR_CUDA; }
+        float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    unsigned long long cyc = 0;
+    cudaMemcpy(&cyc, d_cyc, 8, cudaMemcpyDeviceToHost);
+    // instructions of the measured kind per thread per iteration
+    const double per_iter = (kind == 2) ? 4.0 * 8.0 * 4.0 : 4.0 * 8.0;   // kind 2: 4 reps x 8 x (2 IMAD.WIDE + 2 LOP3)
+    const double total = per_iter * (double)iters * (double)blocks * (double)threads;
+    if (ginstr_per_ns) *ginstr_per_ns = total / ((double)best * 1e6);
+    if (sm_mhz) *sm_mhz = (double)cyc / ((double)best * 1e3);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(d_out); cudaFree(d_cyc);
+    return PA_OK;
+}

@@ -1,0 +1,295 @@
+// pa_resample.cu -- the resampling chain:
+//   E_min/E_max reduction, weights + TREE1024 normaliser, tau / copy numbers / decoupled look-back
+//   exclusive scan / parent map, and the bit-lane gather copy into the new population.
+#include "pa_common.cuh"
+
+// ------------------------------------------------------------------------------------------------
+// E_min, E_max (integer min/max: order-independent, atomics are deterministic)
+// ------------------------------------------------------------------------------------------------
+__global__ void pa_minmax_kernel(const int32_t* __restrict__ E, long long R, PaScalars* sc) {
+    int lo = INT32_MAX, hi = INT32_MIN;
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x) {
+        int e = E[j];
+        lo = min(lo, e); hi = max(hi, e);
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, off));
+        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, off));
+    }
+    if ((threadIdx.x & 31) == 0) { atomicMin(&sc->Emin, lo); atomicMax(&sc->Emax, hi); }
+}
+
+__global__ void pa_reset_scalars_kernel(PaScalars* sc) {
+    sc->Emin = INT32_MAX; sc->Emax = INT32_MIN; sc->tile_counter = 0; sc->R_new = 0;
+    sc->SE = sc->SE2 = sc->SA = sc->SM2 = 0;
+}
+
+int pa_launch_minmax(pa_handle* h) {
+    pa_reset_scalars_kernel<<<1, 1, 0, h->stream>>>(h->d_scal);
+    int blocks = (int)((h->R_cur + 1023) / 1024);
+    if (blocks > 592) blocks = 592;
+    pa_minmax_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->R_cur, h->d_scal);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 2;
+    return PA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// TREE1024 (O5; L165 "sum the per-block partial results in a subsequent kernel call"): one CTA of
+// 1024 threads per aligned block of 1024 values.  __shfl_down trees give, in lane 0, exactly
+// a[i] += a[i+off] (off = 16,8,4,2,1); the 32 run sums are combined by the same tree; the block
+// sums are then added sequentially in ascending block order by pa_tree_final_kernel.
+//   mode 0: v_j = w_j = wtab[(E_j - E_min)/4]                      (also stored to w_out if given)
+//   mode 1: v_j = min(1, R_target * w_j / W)                        (Eq. 8 summand)
+//   mode 2: v_j = (M_j / N)^4                                       (Eq. 3, m^4)
+// ------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(PA_TILE)
+pa_tree_partials_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, const double* __restrict__ wtab,
+                        const PaScalars* __restrict__ sc, long long R, double R_target, double Nd,
+                        double* __restrict__ w_out, double* __restrict__ partials) {
+    __shared__ double run[32];
+    const long long j = (long long)blockIdx.x * PA_TILE + threadIdx.x;
+    double v = 0.0;
+    if (j < R) {
+        if (MODE == 2) {
+            double m = __ddiv_rn((double)M[j], Nd);
+            double mm = __dmul_rn(m, m);
+            v = __dmul_rn(mm, mm);
+        } else {
+            double w = wtab[(E[j] - sc->Emin) >> 2];
+            if (MODE == 0) { v = w; if (w_out) w_out[j] = w; }
+            else { double tau = __ddiv_rn(__dmul_rn(R_target, w), sc->W); v = tau < 1.0 ? tau : 1.0; }
+        }
+    }
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) v = __dadd_rn(v, __shfl_down_sync(0xffffffffu, v, off));
+    if ((threadIdx.x & 31) == 0) run[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        v = run[threadIdx.x];
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) v = __dadd_rn(v, __shfl_down_sync(0xffffffffu, v, off));
+        if (threadIdx.x == 0) partials[blockIdx.x] = v;
+    }
+}
+
+__global__ void pa_tree_final_kernel(const double* __restrict__ partials, int n, PaScalars* sc, int store_W) {
+    extern __shared__ double sp[];
+    for (int i = threadIdx.x; i < n; i += blockDim.x) sp[i] = partials[i];
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double total = 0.0;
+        for (int i = 0; i < n; ++i) total = __dadd_rn(total, sp[i]);     // ascending block index
+        sc->sum = total;
+        if (store_W) sc->W = total;
+    }
+}
+
+int pa_launch_tree_weights(pa_handle* h, int mode, double* w_out) {
+    const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
+    const double Rt = (double)h->R_target, Nd = (double)h->N;
+    if (mode == 0)
+        pa_tree_partials_kernel<0><<<n, PA_TILE, 0, h->stream>>>(h->E, h->M, h->wtab, h->d_scal, h->R_cur, Rt, Nd, w_out, h->partials);
+    else if (mode == 1)
+        pa_tree_partials_kernel<1><<<n, PA_TILE, 0, h->stream>>>(h->E, h->M, h->wtab, h->d_scal, h->R_cur, Rt, Nd, nullptr, h->partials);
+    else
+        pa_tree_partials_kernel<2><<<n, PA_TILE, 0, h->stream>>>(h->E, h->M, h->wtab, h->d_scal, h->R_cur, Rt, Nd, nullptr, h->partials);
+    pa_tree_final_kernel<<<1, 256, n * sizeof(double), h->stream>>>(h->partials, n, h->d_scal, mode == 0 ? 1 : 0);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 2;
+    return PA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Plan: tau_j = R w_j / W (one multiply, one divide, O6), r_j = floor(tau_j) + [u_j < frac tau_j]
+// (Eq. 2 L67 with strict '<'), o_j = exclusive prefix sum (L165 CalcParSum), parent[o_j + c] = j.
+// Single-pass decoupled look-back scan over tiles of 1024 (256 threads x 4), no library.
+// Tile ids are handed out by an atomic counter so that a tile's predecessors have always started.
+// ------------------------------------------------------------------------------------------------
+#define PA_FLAG_AGG (1ull << 32)
+#define PA_FLAG_PREFIX (2ull << 32)
+
+__global__ void __launch_bounds__(256)
+pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* sc,
+               long long R, double R_target, PhiloxKeys K, uint32_t kcount, long long R_cap,
+               uint32_t* __restrict__ r_out, uint32_t* __restrict__ o_out, uint32_t* __restrict__ parent,
+               unsigned long long* __restrict__ state, int n_tiles) {
+    __shared__ uint32_t s_tile, s_warp[8], s_excl;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_tile = atomicAdd(&sc->tile_counter, 1u);
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const long long j0 = (long long)tile * PA_TILE + tid * 4;
+
+    uint32_t r[4] = {0, 0, 0, 0};
+    if (j0 < R) {
+        const double W = sc->W;
+        const int Emin = sc->Emin;
+        // x(j,k) = philox(j>>2, 0, k, TAG_RESAMPLE)[j&3]   (O1)
+        uint4 x = pa_philox((uint32_t)(j0 >> 2), 0u, kcount, PA_TAG_RESAMPLE, K);
+        const uint32_t xs[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (j0 + q < R) {
+                double w = wtab[(E[j0 + q] - Emin) >> 2];
+                double tau = __ddiv_rn(__dmul_rn(R_target, w), W);
+                double n = floor(tau);
+                double f = __dsub_rn(tau, n);
+                double u = __dmul_rn((double)xs[q], 1.0 / 4294967296.0);
+                r[q] = (uint32_t)n + (u < f ? 1u : 0u);
+            }
+        }
+    }
+    const uint32_t tsum = r[0] + r[1] + r[2] + r[3];
+    // block-wide exclusive scan of tsum
+    uint32_t inc = tsum;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        uint32_t t = __shfl_up_sync(0xffffffffu, inc, off);
+        if (lane >= off) inc += t;
+    }
+    if (lane == 31) s_warp[warp] = inc;
+    __syncthreads();
+    uint32_t wbase = 0, btotal = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) { uint32_t v = s_warp[w]; if (w < warp) wbase += v; btotal += v; }
+    const uint32_t local_excl = wbase + inc - tsum;
+
+    // decoupled look-back: publish this tile's aggregate, then walk the predecessors
+    if (warp == 0) {
+        uint32_t excl = 0;
+        if (tile == 0) {
+            if (lane == 0) atomicExch(&state[0], PA_FLAG_PREFIX | (unsigned long long)btotal);
+        } else {
+            if (lane == 0) atomicExch(&state[tile], PA_FLAG_AGG | (unsigned long long)btotal);
+            long long idx = (long long)tile - 1;
+            while (true) {
+                long long my = idx - lane;
+                unsigned long long s;
+                if (my >= 0) {
+                    do { s = *((volatile unsigned long long*)&state[my]); } while ((s >> 32) == 0ull);
+                } else {
+                    s = PA_FLAG_PREFIX;   // before tile 0: prefix 0
+                }
+                const unsigned pref = __ballot_sync(0xffffffffu, (s >> 32) == 2ull);
+                uint32_t val = (uint32_t)s;
+                if (pref) {
+                    const int first = __ffs(pref) - 1;           // nearest predecessor holding a full prefix
+                    val = lane <= first ? val : 0u;
+                }
+#pragma unroll
+                for (int off = 16; off >= 1; off >>= 1) val += __shfl_xor_sync(0xffffffffu, val, off);
+                excl += val;
+                if (pref) break;
+                idx -= 32;
+            }
+            if (lane == 0) atomicExch(&state[tile], PA_FLAG_PREFIX | (unsigned long long)(excl + btotal));
+        }
+        if (lane == 0) {
+            s_excl = excl;
+            if ((int)tile == n_tiles - 1) sc->R_new = excl + btotal;
+        }
+    }
+    __syncthreads();
+    uint32_t o = s_excl + local_excl;
+    if (j0 < R) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (j0 + q < R) {
+                r_out[j0 + q] = r[q];
+                o_out[j0 + q] = o;
+                for (uint32_t c = 0; c < r[q]; ++c)
+                    if ((long long)o + c < R_cap) parent[o + c] = (uint32_t)(j0 + q);
+                o += r[q];
+            }
+        }
+    }
+}
+
+int pa_launch_plan(pa_handle* h) {
+    const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
+    PA_CUDA(h, cudaMemsetAsync(h->scan_state, 0, sizeof(unsigned long long) * n, h->stream));
+    pa_plan_kernel<<<n, 256, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, h->keys, h->k,
+                                             h->R_cap, h->r, h->o, h->parent, h->scan_state, n);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Copy (L165-L171 resampleKer; O7): new[d] = old[parent(d)].  The 32 slots of a destination group
+// come from a monotone run of parents, so the word of the destination group at a site is an OR of a
+// few "segments": a rotated, masked source word.  One warp builds the segment list of the group
+// once; all threads then stream the group's N words with 128-bit loads and stores.
+// ------------------------------------------------------------------------------------------------
+struct __align__(16) PaSeg { uint32_t src_group, rot, mask, pad; };
+
+__global__ void __launch_bounds__(128)
+pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, const uint32_t* __restrict__ parent,
+               long long R_new, int N) {
+    __shared__ PaSeg segs[32];
+    __shared__ int nseg;
+    const long long g = blockIdx.x;
+    const int tid = threadIdx.x;
+    if (tid < 32) {
+        const long long d = g * 32 + tid;
+        const bool valid = d < R_new;
+        const uint32_t p = valid ? parent[d] : 0xffffffffu;
+        const uint32_t pprev = __shfl_up_sync(0xffffffffu, p, 1);
+        const bool vprev = __shfl_up_sync(0xffffffffu, (int)valid, 1) != 0;
+        // a segment continues while parents are consecutive slots of one source group
+        bool start = valid && (tid == 0 || !vprev || p != pprev + 1u || (p >> 5) != (pprev >> 5));
+        const unsigned starts = __ballot_sync(0xffffffffu, start);
+        const unsigned valids = __ballot_sync(0xffffffffu, valid);
+        if (start) {
+            const unsigned later = starts & ~((2u << tid) - 1u);               // starts after this lane
+            const int nvalid = __popc(valids);
+            const int end = later ? (__ffs(later) - 1) : nvalid;                // first lane past the segment
+            const int len = end - tid;
+            const int idx = __popc(starts & ((1u << tid) - 1u));
+            PaSeg s;
+            s.src_group = p >> 5;
+            s.rot = (uint32_t)(tid - (int)(p & 31u)) & 31u;                     // rotate left: src bit -> dst bit
+            s.mask = (len >= 32 ? 0xffffffffu : ((1u << len) - 1u)) << tid;
+            s.pad = 0u;
+            segs[idx] = s;
+        }
+        if (tid == 0) nseg = __popc(starts);
+    }
+    __syncthreads();
+    const int ns = nseg;
+    const int chunks = N >> 2;
+    uint4* out = reinterpret_cast<uint4*>(dst + g * (long long)N);
+    for (int i = blockIdx.y * blockDim.x + tid; i < chunks; i += gridDim.y * blockDim.x) {
+        uint4 acc = make_uint4(0, 0, 0, 0);
+        uint32_t cur_group = 0xffffffffu;
+        uint4 w = make_uint4(0, 0, 0, 0);
+        for (int k = 0; k < ns; ++k) {
+            const PaSeg s = segs[k];
+            if (s.src_group != cur_group) {
+                cur_group = s.src_group;
+                w = reinterpret_cast<const uint4*>(src + (long long)cur_group * N)[i];
+            }
+            acc.x |= __funnelshift_l(w.x, w.x, s.rot) & s.mask;
+            acc.y |= __funnelshift_l(w.y, w.y, s.rot) & s.mask;
+            acc.z |= __funnelshift_l(w.z, w.z, s.rot) & s.mask;
+            acc.w |= __funnelshift_l(w.w, w.w, s.rot) & s.mask;
+        }
+        out[i] = acc;
+    }
+}
+
+int pa_launch_copy(pa_handle* h, int64_t R_new) {
+    const int64_t G = (R_new + 31) / 32;
+    const int chunks = h->N / 4;
+    int gy = 1;
+    // small populations: split a group's words over several CTAs to fill the GPU
+    while (G * gy < 592 && gy * 128 * 2 <= chunks) gy *= 2;
+    dim3 grid((unsigned)G, (unsigned)gy, 1);
+    pa_copy_kernel<<<grid, 128, 0, h->stream>>>(h->spins[h->cur], h->spins[1 - h->cur], h->parent, R_new, h->N);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}

@@ -1,0 +1,268 @@
+// pa_sweep.cu -- the checkerboard Metropolis sweep kernel.
+//
+// One thread-block cluster of C CTAs owns one group (32 replicas, one uint32 per site).  Each CTA
+// stages H = L/C lattice rows of both colours in shared memory, runs all theta sweeps of the launch
+// on chip (colour 0, barrier, colour 1, barrier -- the paper's "blue, synchronise, white", L157) and
+// writes the rows back: HBM traffic is one read and one write of the population per launch.  Rows
+// at a strip boundary read their vertical neighbour from the adjacent CTA's shared memory (DSMEM).
+//
+// Per word (32 spins) the work is: 8 Philox4x32-10 calls sharing their first rounds (the 8 counters
+// differ only in c1 = 8g+i), 64 threshold tests, and a dozen bit-sliced logic ops for the neighbour
+// count.  The kernel is bound by integer issue (IMAD.WIDE on the FMA pipe, LOP3 on the ALU pipe);
+// see DESIGN.md Sec. 6 for the instruction budget.
+#include "pa_common.cuh"
+#include <cooperative_groups.h>
+#include <stdlib.h>
+namespace cg = cooperative_groups;
+
+struct SweepParams {
+    PhiloxKeys K;
+    uint32_t T4, T8;                 // acceptance thresholds for dE = 4, 8 (O2)
+    uint32_t t0;                     // sweep counter at launch
+    int theta;
+    int L, Lh, H, C, N;
+};
+
+// m = 2*m + (x < T): the borrow of x - T shifted into the mask.  ptxas emits one carry-out IADD3 (ALU
+// pipe) and one IMAD.X (FMA pipe), which balances the two integer pipes.
+__device__ __forceinline__ void pa_shift_in_lt(uint32_t& m, uint32_t x, uint32_t T) {
+    asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 2, 0;\n\t}" : "+r"(m) : "r"(x), "r"(T));
+}
+
+// Flip mask of one word: bit b set iff replica 32g+b flips its spin at `site` (O3).
+//   s: centre word, n0..n3: the four neighbour words.
+//   c0base = hi(M1*c2) ^ k0[0] ^ 8g, lo1u = lo(M1*c2), c2 = 2t+colour (uniform per half-sweep).
+template <int CMP>
+__device__ __forceinline__ uint32_t pa_flip_mask(uint32_t s, uint32_t n0, uint32_t n1, uint32_t n2, uint32_t n3,
+                                                 uint32_t site, uint32_t c0base, uint32_t lo1u,
+                                                 const SweepParams& P) {
+    // bit-sliced count u of anti-parallel neighbours per lane: dE = 8 - 4u (Eq. 10)
+    uint32_t a0 = s ^ n0, a1 = s ^ n1, a2 = s ^ n2, a3 = s ^ n3;
+    uint32_t U1 = a0 | a1 | a2 | a3;                                   // u >= 1
+    uint32_t U2 = (a0 & a1) | (a2 & a3) | ((a0 ^ a1) & (a2 ^ a3));     // u >= 2: always flips
+
+    // ---- 8 Philox4x32-10 calls, counters (site, 8g+i, 2t+c, TAG_SWEEP), i = 0..7 (O1) ----
+    uint32_t x0[8], x1[8], x2[8], x3[8];
+    // round 1: only c0' depends on i
+    uint32_t hi0, lo0;
+    pa_mulhilo(PA_PHILOX_M0, site, hi0, lo0);
+    const uint32_t c2w = hi0 ^ PA_TAG_SWEEP ^ P.K.k1[0];
+    const uint32_t c3w = lo0;
+    // round 2: the M1 product and c0'', c1'' are shared by the 8 calls
+    uint32_t hi1w, lo1w;
+    pa_mulhilo(PA_PHILOX_M1, c2w, hi1w, lo1w);
+    const uint32_t c0w = hi1w ^ lo1u ^ P.K.k0[1];
+    const uint32_t c1w = lo1w;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        uint32_t h, l;
+        pa_mulhilo(PA_PHILOX_M0, c0base ^ (uint32_t)i, h, l);
+        x2[i] = h ^ c3w ^ P.K.k1[1];
+        x3[i] = l;
+    }
+    // round 3: the M0 product is shared
+    uint32_t hi0w, lo0w;
+    pa_mulhilo(PA_PHILOX_M0, c0w, hi0w, lo0w);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        uint32_t h, l;
+        pa_mulhilo(PA_PHILOX_M1, x2[i], h, l);
+        x0[i] = h ^ c1w ^ P.K.k0[2];
+        x1[i] = l;
+        x2[i] = hi0w ^ x3[i] ^ P.K.k1[2];
+        x3[i] = lo0w;
+    }
+    // rounds 4..10
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            uint32_t h0, l0, h1, l1;
+            pa_mulhilo(PA_PHILOX_M0, x0[i], h0, l0);
+            pa_mulhilo(PA_PHILOX_M1, x2[i], h1, l1);
+            x0[i] = h1 ^ x1[i] ^ P.K.k0[r];
+            x1[i] = l1;
+            x2[i] = h0 ^ x3[i] ^ P.K.k1[r];
+            x3[i] = l0;
+        }
+    }
+    // ---- acceptance: flip iff u >= 2, or u = 1 and x < T4, or u = 0 and x < T8 (O3) ----
+    uint32_t acc = 0;
+    if (CMP == 1) {
+        uint32_t m4 = 0, m8 = 0;               // built most-significant bit first
+#pragma unroll
+        for (int i = 7; i >= 0; --i) {
+            const uint32_t xs[4] = {x0[i], x1[i], x2[i], x3[i]};
+#pragma unroll
+            for (int q = 3; q >= 0; --q) {
+                pa_shift_in_lt(m4, xs[q], P.T4);
+                pa_shift_in_lt(m8, xs[q], P.T8);
+            }
+        }
+        acc = m4 & (U1 | m8);
+    } else {
+        uint32_t m4 = 0, m8 = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const uint32_t xs[4] = {x0[i], x1[i], x2[i], x3[i]};
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                if (xs[q] < P.T4) m4 |= 1u << (4 * i + q);
+                if (xs[q] < P.T8) m8 |= 1u << (4 * i + q);
+            }
+        }
+        acc = m4 & (U1 | m8);
+    }
+    return U2 | acc;
+}
+
+template <int CMP, bool CLUSTER>
+__global__ void __launch_bounds__(256)
+pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
+    extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
+    const int T = blockDim.x, tid = threadIdx.x;
+    const int C = CLUSTER ? P.C : 1;
+    unsigned cr = 0;
+    if (CLUSTER) cr = cg::this_cluster().block_rank();
+    const long long g = blockIdx.x / C;
+    const int H = P.H, Lh = P.Lh, L = P.L;
+    const int y0 = (int)cr * H;
+    const int half = H * Lh;
+    uint32_t* gbase = pop + g * (long long)P.N;
+    const int goff = y0 * Lh, gcol = P.N >> 1;
+
+    // stage both colours of this strip
+    if ((Lh & 3) == 0) {
+        for (int c = 0; c < 2; ++c) {
+            const uint4* src = reinterpret_cast<const uint4*>(gbase + c * gcol + goff);
+            uint4* dst = reinterpret_cast<uint4*>(tile + c * half);
+            for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+        }
+    } else {
+        for (int c = 0; c < 2; ++c)
+            for (int i = tid; i < half; i += T) tile[c * half + i] = gbase[c * gcol + goff + i];
+    }
+    const uint32_t* up_tile = tile;
+    const uint32_t* dn_tile = tile;
+    if (CLUSTER) {
+        cg::cluster_group cl = cg::this_cluster();
+        up_tile = cl.map_shared_rank(tile, (cr + C - 1) % C);
+        dn_tile = cl.map_shared_rank(tile, (cr + 1) % C);
+        cl.sync();
+    } else {
+        __syncthreads();
+    }
+
+    const int dy = T / Lh, dx = T % Lh;
+    const uint32_t g8 = (uint32_t)(8 * g);
+    for (int it = 0; it < P.theta; ++it) {
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t c2 = 2u * (P.t0 + (uint32_t)it) + (uint32_t)c;
+            uint32_t hi1u, lo1u;
+            pa_mulhilo(PA_PHILOX_M1, c2, hi1u, lo1u);
+            const uint32_t c0base = hi1u ^ P.K.k0[0] ^ g8;
+            uint32_t* mine = tile + c * half;
+            const uint32_t* oth = tile + (1 - c) * half;
+            const uint32_t* up_oth = up_tile + (1 - c) * half;
+            const uint32_t* dn_oth = dn_tile + (1 - c) * half;
+            int yl = tid / Lh, xh = tid % Lh;
+#pragma unroll 1
+            for (int w = tid; w < half; w += T) {
+                const int y = y0 + yl;
+                const int p = (y + c) & 1;
+                const int row = yl * Lh;
+                const uint32_t s = mine[row + xh];
+                const uint32_t nS = oth[row + xh];
+                const int xh2 = p ? (xh + 1 == Lh ? 0 : xh + 1) : (xh == 0 ? Lh - 1 : xh - 1);
+                const uint32_t nX = oth[row + xh2];
+                uint32_t nU, nD;
+                if (yl > 0) nU = oth[row - Lh + xh]; else nU = up_oth[(H - 1) * Lh + xh];
+                if (yl < H - 1) nD = oth[row + Lh + xh]; else nD = dn_oth[xh];
+                const uint32_t site = (uint32_t)(y * L + 2 * xh + p);
+                const uint32_t flip = pa_flip_mask<CMP>(s, nS, nX, nU, nD, site, c0base, lo1u, P);
+                mine[row + xh] = s ^ flip;
+                xh += dx; yl += dy;
+                if (xh >= Lh) { xh -= Lh; yl += 1; }
+            }
+            if (CLUSTER) cg::this_cluster().sync(); else __syncthreads();
+        }
+    }
+
+    if ((Lh & 3) == 0) {
+        for (int c = 0; c < 2; ++c) {
+            uint4* dst = reinterpret_cast<uint4*>(gbase + c * gcol + goff);
+            const uint4* src = reinterpret_cast<const uint4*>(tile + c * half);
+            for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+        }
+    } else {
+        for (int c = 0; c < 2; ++c)
+            for (int i = tid; i < half; i += T) gbase[c * gcol + goff + i] = tile[c * half + i];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+static int pa_env_int(const char* name, int dflt) {
+    const char* v = getenv(name);
+    return v ? atoi(v) : dflt;
+}
+
+// Launch geometry: the smallest cluster size C in {1,2,4,8} dividing L whose strip (L/C rows of both
+// colours, L*L*4/C bytes) fits the shared-memory budget per CTA; threads = min(256, words per colour).
+int pa_sweep_configure(pa_handle* h) {
+    const int L = h->L;
+    const size_t budget = (size_t)pa_env_int("PA_SWEEP_SMEM_KB", 64) * 1024;
+    int C = 1;
+    while (C <= 8 && (((L % C) != 0) || (size_t)L * L * 4 / C > budget)) C *= 2;
+    int forceC = pa_env_int("PA_SWEEP_C", 0);
+    if (forceC > 0 && L % forceC == 0) C = forceC;
+    if (C > 8 || (size_t)L * L * 4 / C > 224 * 1024) return PA_ERR_INVALID_ARG;
+    int half = (L / C) * (L / 2);
+    int T = 256;
+    while (T > 32 && T > half) T >>= 1;
+    int forceT = pa_env_int("PA_SWEEP_T", 0);
+    if (forceT >= 32 && forceT <= 256) T = forceT;
+    h->sweep_C = C; h->sweep_T = T;
+    h->sweep_cmp = pa_env_int("PA_SWEEP_CMP", 1) ? 1 : 0;
+    return PA_OK;
+}
+
+template <int CMP, bool CLUSTER>
+static cudaError_t pa_sweep_launch_t(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
+    auto kern = pa_sweep_kernel<CMP, CLUSTER>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3((unsigned)h->sweep_T, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CLUSTER ? (unsigned)P.C : 1u;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, h->spins[h->cur], P);
+}
+
+int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
+    if (theta == 0) return PA_OK;
+    SweepParams P;
+    P.K = h->keys;
+    P.T4 = T4; P.T8 = T8;
+    P.t0 = h->t; P.theta = theta;
+    P.L = h->L; P.Lh = h->L / 2; P.C = h->sweep_C; P.H = h->L / h->sweep_C; P.N = h->N;
+    const size_t smem = (size_t)P.H * h->L * 4;
+    const int64_t G = (h->R_cur + 31) / 32;
+    const unsigned grid = (unsigned)(G * P.C);
+    cudaError_t e;
+    if (P.C > 1) e = h->sweep_cmp ? pa_sweep_launch_t<1, true>(h, P, smem, grid) : pa_sweep_launch_t<0, true>(h, P, smem, grid);
+    else         e = h->sweep_cmp ? pa_sweep_launch_t<1, false>(h, P, smem, grid) : pa_sweep_launch_t<0, false>(h, P, smem, grid);
+    PA_CUDA(h, e);
+    h->launches += 1;
+    return PA_OK;
+}

@@ -1,0 +1,313 @@
+"""Thin Python binding of the C-ABI library declared in include/pa.h (argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels behind these calls; this module computes
+nothing.  PyTorch is used for device memory (the workspace tensor handed to pa_create_ex), for
+the CUDA stream and for moving result vectors; there is no CPU fallback -- if the library or a
+CUDA device is missing the calls raise.
+
+The module-level functions have the names of the C entry points (pa_create, pa_sweep, ...).
+`Population` wraps a handle with the same verbs (sweep, energies, resample, adapt_dbeta,
+observables, hist_accumulate, ...), which is also the interface of oracle.pa_oracle.Oracle, so
+that tests can drive both with one loop (tests/pa_driver.py).
+"""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libpa_b200.so")
+HEADER = os.path.join(os.path.dirname(HERE), "include", "pa.h")
+
+PA_OK, PA_ERR_INVALID_ARG, PA_ERR_CAPACITY, PA_ERR_CUDA, PA_ERR_WORKSPACE, PA_ERR_NOMEM = 0, -1, -2, -3, -4, -5
+
+
+class PaError(RuntimeError):
+    def __init__(self, code, what, detail=""):
+        self.code = code
+        super().__init__(f"{what}: {strerror(code)} ({code}) {detail}".strip())
+
+
+class pa_obs_t(C.Structure):
+    _fields_ = [("beta", C.c_double), ("e", C.c_double), ("C", C.c_double), ("absm", C.c_double),
+                ("m2", C.c_double), ("m4", C.c_double), ("betaF_per_N", C.c_double),
+                ("S_per_N", C.c_double), ("lnQ", C.c_double), ("R", C.c_int64)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def declared_symbols():
+    """Names of the functions include/pa.h declares."""
+    text = open(HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(pa_[a-z0-9_]+)\s*\(", text)))
+
+
+def lib():
+    """Load libpa_b200.so (building it first if the sources are newer).  Raises if it cannot be loaded."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        from . import build as _build
+        _build.build()
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, u32, u64, dbl, sz = C.c_void_p, C.c_int, C.c_int64, C.c_uint32, C.c_uint64, C.c_double, C.c_size_t
+    sig = {
+        "pa_capacity": ([i64], i64),
+        "pa_workspace_bytes": ([i32, i64, C.POINTER(sz)], i32),
+        "pa_create": ([i32, i64, u64, C.POINTER(vp)], i32),
+        "pa_create_ex": ([i32, i64, u64, vp, sz, vp, C.POINTER(vp)], i32),
+        "pa_destroy": ([vp], None),
+        "pa_sweep": ([vp, dbl, i32], i32),
+        "pa_energies": ([vp, vp, vp], i32),
+        "pa_resample": ([vp, dbl, dbl, C.POINTER(i64)], i32),
+        "pa_adapt_dbeta": ([vp, dbl, dbl, dbl, C.POINTER(dbl)], i32),
+        "pa_overlap": ([vp, dbl, C.POINTER(dbl)], i32),
+        "pa_observables": ([vp, dbl, C.POINTER(pa_obs_t)], i32),
+        "pa_hist_accumulate": ([vp, dbl], i32),
+        "pa_get_histogram": ([vp, vp, vp], i32),
+        "pa_get_spins": ([vp, i64, i64, vp], i32),
+        "pa_get_spins_at": ([vp, vp, i64, vp], i32),
+        "pa_set_spins": ([vp, i64, i64, vp], i32),
+        "pa_get_words": ([vp, vp], i32),
+        "pa_set_words": ([vp, i64, vp], i32),
+        "pa_get_resample_debug": ([vp, C.POINTER(dbl), vp, vp, vp], i32),
+        "pa_population": ([vp], i64),
+        "pa_capacity_of": ([vp], i64),
+        "pa_sweep_counter": ([vp], u32),
+        "pa_resample_counter": ([vp], u32),
+        "pa_lnZ": ([vp], dbl),
+        "pa_set_counters": ([vp, u32, u32, dbl], i32),
+        "pa_launch_count": ([vp], i64),
+        "pa_last_sweep_ms": ([vp, C.POINTER(C.c_float)], i32),
+        "pa_last_resample_ms": ([vp, C.POINTER(C.c_float), C.POINTER(C.c_float)], i32),
+        "pa_calibrate": ([i32, C.POINTER(dbl), C.POINTER(dbl)], i32),
+        "pa_strerror": ([i32], C.c_char_p),
+        "pa_last_cuda_error": ([vp], C.c_char_p),
+        "pa_version": ([], C.c_char_p),
+    }
+    for name, (args, res) in sig.items():
+        f = getattr(L, name)
+        f.argtypes = args
+        f.restype = res
+    _lib = L
+    return L
+
+
+def strerror(code):
+    return lib().pa_strerror(int(code)).decode()
+
+
+def _ptr(x):
+    """A raw address for a numpy array (host) or a torch tensor (host or device); None -> NULL."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        assert x.flags.c_contiguous
+        return C.c_void_p(x.ctypes.data)
+    return C.c_void_p(x.data_ptr())       # torch tensor
+
+
+# ---- module-level functions with the C names ------------------------------------------------
+
+def pa_capacity(R):
+    return int(lib().pa_capacity(int(R)))
+
+
+def pa_workspace_bytes(L, R):
+    n = C.c_size_t()
+    rc = lib().pa_workspace_bytes(L, R, C.byref(n))
+    if rc:
+        raise PaError(rc, "pa_workspace_bytes")
+    return n.value
+
+
+def pa_calibrate(kind):
+    g, mhz = C.c_double(), C.c_double()
+    rc = lib().pa_calibrate(kind, C.byref(g), C.byref(mhz))
+    if rc:
+        raise PaError(rc, "pa_calibrate")
+    return g.value, mhz.value
+
+
+def pa_create(L, R, seed):
+    h = C.c_void_p()
+    rc = lib().pa_create(L, R, seed, C.byref(h))
+    if rc:
+        raise PaError(rc, "pa_create")
+    return h
+
+
+def pa_create_ex(L, R, seed, dev_ws_ptr, ws_bytes, cuda_stream):
+    h = C.c_void_p()
+    rc = lib().pa_create_ex(L, R, seed, C.c_void_p(dev_ws_ptr), ws_bytes, C.c_void_p(cuda_stream), C.byref(h))
+    if rc:
+        raise PaError(rc, "pa_create_ex")
+    return h
+
+
+def pa_destroy(h):
+    lib().pa_destroy(h)
+
+
+class Population:
+    """One population on the current CUDA device.  Workspace and stream come from PyTorch
+    (pa_create_ex) unless own_memory=True (pa_create: cudaMalloc + private stream)."""
+
+    def __init__(self, L, R, seed, stream=None, own_memory=False):
+        import torch
+        if not torch.cuda.is_available():
+            raise PaError(PA_ERR_CUDA, "Population", "no CUDA device: this library has no CPU path")
+        self.L, self.N, self.R_target, self.seed = L, L * L, R, seed
+        self._torch = torch
+        self._ws = None
+        if own_memory:
+            self._h = pa_create(L, R, seed)
+        else:
+            nbytes = pa_workspace_bytes(L, R)
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+            self._stream = stream if stream is not None else torch.cuda.current_stream()
+            self._h = pa_create_ex(L, R, seed, self._ws.data_ptr(), nbytes, self._stream.cuda_stream)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            pa_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc:
+            raise PaError(rc, what, lib().pa_last_cuda_error(self._h).decode() if rc == PA_ERR_CUDA else "")
+
+    # scalars
+    @property
+    def population(self):
+        return int(lib().pa_population(self._h))
+
+    @property
+    def capacity(self):
+        return int(lib().pa_capacity_of(self._h))
+
+    @property
+    def sweep_counter(self):
+        return int(lib().pa_sweep_counter(self._h))
+
+    @property
+    def resample_counter(self):
+        return int(lib().pa_resample_counter(self._h))
+
+    @property
+    def lnZ(self):
+        return float(lib().pa_lnZ(self._h))
+
+    @property
+    def launch_count(self):
+        return int(lib().pa_launch_count(self._h))
+
+    def set_counters(self, t, k, lnZ):
+        self._check(lib().pa_set_counters(self._h, t, k, float(lnZ)), "pa_set_counters")
+
+    # the path
+    def sweep(self, beta, theta):
+        self._check(lib().pa_sweep(self._h, float(beta), int(theta)), "pa_sweep")
+
+    def energies(self, device=False):
+        """(E, M) as numpy int32 arrays, or as torch cuda tensors if device=True."""
+        R = self.population
+        if device:
+            E = self._torch.empty(R, dtype=self._torch.int32, device="cuda")
+            M = self._torch.empty(R, dtype=self._torch.int32, device="cuda")
+        else:
+            E = np.empty(R, dtype=np.int32); M = np.empty(R, dtype=np.int32)
+        self._check(lib().pa_energies(self._h, _ptr(E), _ptr(M)), "pa_energies")
+        return E, M
+
+    def energies_into(self, E, M=None):
+        self._check(lib().pa_energies(self._h, _ptr(E), _ptr(M)), "pa_energies")
+
+    def resample(self, beta, beta_new):
+        Rn = C.c_int64()
+        self._check(lib().pa_resample(self._h, float(beta), float(beta_new), C.byref(Rn)), "pa_resample")
+        return Rn.value
+
+    def resample_rc(self, beta, beta_new):
+        Rn = C.c_int64()
+        return lib().pa_resample(self._h, float(beta), float(beta_new), C.byref(Rn)), Rn.value
+
+    def adapt_dbeta(self, target, beta, beta_max):
+        d = C.c_double()
+        self._check(lib().pa_adapt_dbeta(self._h, float(target), float(beta), float(beta_max), C.byref(d)), "pa_adapt_dbeta")
+        return d.value
+
+    def overlap(self, dbeta):
+        a = C.c_double()
+        self._check(lib().pa_overlap(self._h, float(dbeta), C.byref(a)), "pa_overlap")
+        return a.value
+
+    def observables(self, beta):
+        o = pa_obs_t()
+        self._check(lib().pa_observables(self._h, float(beta), C.byref(o)), "pa_observables")
+        return o.as_dict()
+
+    def hist_accumulate(self, beta):
+        self._check(lib().pa_hist_accumulate(self._h, float(beta)), "pa_hist_accumulate")
+
+    def histogram(self):
+        H = np.empty(self.N + 1, dtype=np.int64); D = np.empty(self.N + 1, dtype=np.float64)
+        self._check(lib().pa_get_histogram(self._h, _ptr(H), _ptr(D)), "pa_get_histogram")
+        return H, D
+
+    # state export / import
+    def get_spins(self, j0=0, nrep=None):
+        nrep = self.population - j0 if nrep is None else nrep
+        out = np.empty((nrep, self.N), dtype=np.int8)
+        self._check(lib().pa_get_spins(self._h, j0, nrep, _ptr(out)), "pa_get_spins")
+        return out
+
+    def get_spins_at(self, slots):
+        slots = np.ascontiguousarray(slots, dtype=np.int64)
+        out = np.empty((slots.size, self.N), dtype=np.int8)
+        self._check(lib().pa_get_spins_at(self._h, _ptr(slots), slots.size, _ptr(out)), "pa_get_spins_at")
+        return out
+
+    def set_spins(self, j0, spins_pm1):
+        s = np.ascontiguousarray(spins_pm1, dtype=np.int8)
+        self._check(lib().pa_set_spins(self._h, j0, s.shape[0], _ptr(s)), "pa_set_spins")
+
+    def get_words(self, out=None):
+        if out is None:
+            out = np.empty(((self.population + 31) // 32, self.N), dtype=np.uint32)
+        self._check(lib().pa_get_words(self._h, _ptr(out)), "pa_get_words")
+        return out
+
+    def set_words(self, R, words):
+        self._check(lib().pa_set_words(self._h, int(R), _ptr(words)), "pa_set_words")
+
+    def resample_debug(self, R_prev):
+        W = C.c_double()
+        w = np.empty(R_prev, dtype=np.float64); r = np.empty(R_prev, dtype=np.uint32); o = np.empty(R_prev, dtype=np.uint32)
+        self._check(lib().pa_get_resample_debug(self._h, C.byref(W), _ptr(w), _ptr(r), _ptr(o)), "pa_get_resample_debug")
+        return {"W": W.value, "w": w, "r": r, "o": o}
+
+    # timing (CUDA events recorded by the library on its stream)
+    def last_sweep_ms(self):
+        ms = C.c_float()
+        self._check(lib().pa_last_sweep_ms(self._h, C.byref(ms)), "pa_last_sweep_ms")
+        return ms.value
+
+    def last_resample_ms(self):
+        a, b = C.c_float(), C.c_float()
+        self._check(lib().pa_last_resample_ms(self._h, C.byref(a), C.byref(b)), "pa_last_resample_ms")
+        return a.value, b.value

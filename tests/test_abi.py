@@ -1,0 +1,68 @@
+"""The C-ABI library builds for sm_100a on a CPU-only box, loads, and exports every symbol that
+include/pa.h declares; host-only entry points behave; there is no CPU fallback (-m "not gpu")."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import pytest
+
+from paper_1703_03676_b200 import build as pa_build
+from paper_1703_03676_b200 import pa
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def libpath():
+    return pa_build.build()
+
+
+def test_library_exports_every_declared_symbol(libpath):
+    declared = pa.declared_symbols()
+    assert len(declared) >= 30 and "pa_create" in declared and "pa_sweep" in declared and "pa_resample" in declared
+    out = subprocess.run(["nm", "-D", "--defined-only", libpath], check=True, capture_output=True, text=True).stdout
+    exported = {line.split()[-1] for line in out.splitlines() if " T " in line}
+    missing = [s for s in declared if s not in exported]
+    assert not missing, missing
+    L = pa.lib()
+    for s in declared:
+        assert hasattr(L, s)
+
+
+def test_library_contains_sm100a_code(libpath):
+    out = subprocess.run(["cuobjdump", "-lelf", libpath], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+
+
+def test_host_only_entry_points():
+    assert pa.pa_capacity(1000) == 32 * ((1000 + 1024 + 31) // 32)
+    assert pa.pa_capacity(1000000) == 32 * ((1000000 + 8000 + 31) // 32)
+    assert pa.pa_workspace_bytes(256, 1000000) > 2 * 31250 * 65536 * 4          # two packed buffers at cfg 5
+    assert pa.pa_workspace_bytes(256, 1000000) < 20 * 2**30
+    n = C.c_size_t()
+    assert pa.lib().pa_workspace_bytes(15, 100, C.byref(n)) == pa.PA_ERR_INVALID_ARG   # odd L
+    assert pa.lib().pa_workspace_bytes(2, 100, C.byref(n)) == pa.PA_ERR_INVALID_ARG
+    assert pa.lib().pa_workspace_bytes(16, 0, C.byref(n)) == pa.PA_ERR_INVALID_ARG
+    assert pa.strerror(pa.PA_ERR_CAPACITY).startswith("resampled population")
+    assert pa.lib().pa_version().decode().startswith("pa-b200")
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present: the fallback check is for CPU-only boxes")
+    h = C.c_void_p()
+    assert pa.lib().pa_create(16, 64, 1, C.byref(h)) == pa.PA_ERR_CUDA
+    with pytest.raises(pa.PaError):
+        pa.Population(16, 64, 1)
+
+
+def test_product_does_not_import_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1703_03676_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+\.*oracle", text, flags=re.M), f
+                assert not re.search(r"#include\s*[<\"][^>\"]*oracle", text), f

@@ -1,0 +1,205 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs (-m gpu).  Bar: bit-exact for spins, energies, copy numbers, offsets, R_new and
+histogram counts; relative 1e-9 for fp64 observables (BASELINE.json north_star)."""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():
+    pytest.skip("no CUDA device", allow_module_level=True)
+
+from oracle import pa_oracle as po                      # noqa: E402
+from paper_1703_03676_b200 import pa                    # noqa: E402
+from paper_1703_03676_b200.workloads import CONFIGS     # noqa: E402
+import pa_driver                                        # noqa: E402
+
+REL = 1e-9
+OBS_KEYS = ("beta", "e", "C", "absm", "m2", "m4", "betaF_per_N", "S_per_N", "lnQ")
+
+
+def assert_obs_close(a, b):
+    assert a["R"] == b["R"]
+    for k in OBS_KEYS:
+        assert a[k] == pytest.approx(b[k], rel=REL, abs=1e-300), (k, a[k], b[k])
+
+
+def assert_same_state(g, o, full=True):
+    assert g.population == o.population
+    assert g.sweep_counter == o.sweep_counter and g.resample_counter == o.resample_counter
+    if full:
+        assert np.array_equal(g.get_spins(), o.get_spins())
+    Eg, Mg = g.energies()
+    Eo, Mo = o.energies()
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+
+
+# ---------------------------------------------------------------------------------------------
+# a0 init, ragged populations
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("L,R,seed", [(4, 1, 3), (4, 33, 4), (6, 100, 5), (16, 1000, 1), (64, 257, 2**40 + 7)])
+def test_init_bit_exact(L, R, seed):
+    g, o = pa.Population(L, R, seed), po.Oracle(L, R, seed)
+    assert g.capacity == o.capacity
+    assert_same_state(g, o)
+    assert g.lnZ == o.lnZ
+    # interchange layout: word (g, s) bit b = replica 32g+b at site s
+    words = g.get_words()
+    sp = o.get_spins()
+    j = R - 1
+    bits = (words[j >> 5] >> np.uint32(j & 31)) & 1
+    assert np.array_equal(bits.astype(np.int8) * 2 - 1, sp[j])
+    if R % 32:
+        assert np.all(words[-1] >> np.uint32(R % 32) == 0)          # unused lanes are zero
+
+
+# ---------------------------------------------------------------------------------------------
+# a2 sweep: per call, several tile geometries (one CTA per group, clusters of 2/4 with DSMEM halos)
+# ---------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("L,R", [(4, 40), (6, 70), (10, 33), (16, 200), (32, 100), (64, 96), (128, 64), (256, 40)])
+def test_sweep_bit_exact(L, R):
+    seed = 1000 + L
+    g, o = pa.Population(L, R, seed), po.Oracle(L, R, seed)
+    for beta, theta in [(0.0, 1), (0.3, 2), (0.4406868, 3), (1.0, 1), (0.7, 0)]:
+        g.sweep(beta, theta); o.sweep(beta, theta)
+        assert_same_state(g, o)
+
+
+def test_sweep_split_calls_and_special_states():
+    L, R = 16, 64
+    g, o = pa.Population(L, R, 9), po.Oracle(L, R, 9)
+    N = L * L
+    yy, xx = np.divmod(np.arange(N), L)
+    states = np.stack([np.ones(N), -np.ones(N), ((xx + yy) & 1) * 2 - 1, (yy & 1) * 2 - 1]).astype(np.int8)
+    g.set_spins(3, states); o.set_spins(3, states)
+    assert_same_state(g, o)
+    E, M = g.energies()
+    assert E[3:7].tolist() == [-2 * N, -2 * N, 2 * N, 0] and M[3:7].tolist() == [N, -N, 0, 0]
+    # theta = 5 in one call on the GPU, 2 + 3 on the oracle: the sweep counter carries the stream
+    g.sweep(0.5, 5)
+    o.sweep(0.5, 2); o.sweep(0.5, 3)
+    assert_same_state(g, o)
+
+
+# ---------------------------------------------------------------------------------------------
+# a4-a7 resample chain, per step
+# ---------------------------------------------------------------------------------------------
+
+def _compare_resample(g, o, beta, beta_new):
+    R_prev = g.population
+    Rg = g.resample(beta, beta_new)
+    Ro = o.resample(beta, beta_new)
+    assert Rg == Ro
+    dg, do = g.resample_debug(R_prev), o.resample_debug(R_prev)
+    assert dg["W"] == do["W"]                                        # fixed-order fp64 sum: bit-exact
+    assert np.array_equal(dg["w"], do["w"])
+    assert np.array_equal(dg["r"], do["r"])
+    assert np.array_equal(dg["o"], do["o"])
+    assert g.lnZ == pytest.approx(o.lnZ, rel=1e-15)
+
+
+@pytest.mark.parametrize("L,R", [(8, 50), (16, 1000), (16, 3333), (64, 2500)])
+def test_resample_chain_bit_exact(L, R):
+    g, o = pa.Population(L, R, 31), po.Oracle(L, R, 31)
+    beta = 0.0
+    for step, db in enumerate([0.0, 0.05, 0.1, 0.02, 0.3]):
+        _compare_resample(g, o, beta, beta + db)
+        beta += db
+        assert_same_state(g, o)
+        g.sweep(beta, 2); o.sweep(beta, 2)
+        assert_same_state(g, o)
+        assert_obs_close(g.observables(beta), o.observables(beta))
+
+
+def test_resample_identity_capacity_and_errors():
+    L, R = 16, 500
+    g, o = pa.Population(L, R, 5), po.Oracle(L, R, 5)
+    before = g.get_spins()
+    assert g.resample(0.0, 0.0) == R                                 # dbeta = 0: r = 1, identity copy
+    assert np.array_equal(g.get_spins(), before)
+    rc, _ = g.resample_rc(0.5, 0.4)
+    assert rc == pa.PA_ERR_INVALID_ARG
+    # shrink the population to a handful of replicas, then resample: R_new ~ R_target >> R_cur
+    g.sweep(0.3, 3); o.sweep(0.3, 3)
+    words = g.get_words()
+    g.set_words(70, words[:3])
+    sp = g.get_spins()
+    # the oracle has no set_words: compare with the plan computed from the energies instead
+    E, _ = g.energies()
+    plan = po.resample_plan(R, E, 5, g.resample_counter, 0.01)
+    R_prev = g.population
+    assert g.resample(0.3, 0.31) == plan["R_new"]
+    d = g.resample_debug(R_prev)
+    assert np.array_equal(d["r"], plan["r"]) and np.array_equal(d["o"], plan["o"]) and d["W"] == plan["W"]
+    parent = np.repeat(np.arange(R_prev), plan["r"])
+    assert np.array_equal(g.get_spins(), sp[parent])
+
+
+# ---------------------------------------------------------------------------------------------
+# whole runs
+# ---------------------------------------------------------------------------------------------
+
+def test_config1_full_run_every_step():
+    """BASELINE.json configs[0]: L=16, R=1000, beta 0..1 in 100 steps, theta=10, seed 1."""
+    wl = CONFIGS[1]
+    g, o = pa.Population(wl.L, wl.R, wl.seed), po.Oracle(wl.L, wl.R, wl.seed)
+    betas = wl.betas()
+    assert_obs_close(g.observables(betas[0]), o.observables(betas[0]))
+    for i in range(1, len(betas)):
+        _compare_resample(g, o, betas[i - 1], betas[i])
+        g.sweep(betas[i], wl.theta); o.sweep(betas[i], wl.theta)
+        assert_same_state(g, o)
+        assert_obs_close(g.observables(betas[i]), o.observables(betas[i]))
+
+
+def test_config2_first_steps():
+    """BASELINE.json configs[1]: L=64, R=20000, dbeta=0.005, theta=10, seed 2 (first 3 steps in full)."""
+    wl = CONFIGS[2]
+    g, o = pa.Population(wl.L, wl.R, wl.seed), po.Oracle(wl.L, wl.R, wl.seed)
+    betas = wl.betas()
+    for i in range(1, 4):
+        _compare_resample(g, o, betas[i - 1], betas[i])
+        g.sweep(betas[i], wl.theta); o.sweep(betas[i], wl.theta)
+        assert_same_state(g, o)
+        assert_obs_close(g.observables(betas[i]), o.observables(betas[i]))
+
+
+def test_adaptive_run_with_multihistogram():
+    """The adaptive schedule and Eq. 9 accumulation (shape of configs[3], scaled to L=16, R=2000)."""
+    L, R, seed, theta, target = 16, 2000, 4, 3, 0.85
+    g, o = pa.Population(L, R, seed), po.Oracle(L, R, seed)
+    bg, og = pa_driver.run_adaptive(g, 0.0, 0.6, theta, target, hist=True, max_steps=25)
+    bo, oo = pa_driver.run_adaptive(o, 0.0, 0.6, theta, target, hist=True, max_steps=25)
+    assert bg == bo                                                  # the beta sequence is bit-identical
+    assert len(bg) > 5
+    for a, b in zip(og, oo):
+        assert_obs_close(a, b)
+    assert_same_state(g, o)
+    Hg, Dg = g.histogram()
+    Ho, Do = o.histogram()
+    assert np.array_equal(Hg, Ho)
+    fin = np.isfinite(Do)
+    assert np.array_equal(np.isfinite(Dg), fin)
+    assert np.allclose(Dg[fin], Do[fin], rtol=REL, atol=0)
+    # the overlap function itself
+    for d in (0.0, 0.003, 0.02):
+        assert g.overlap(d) == o.overlap(d)
+
+
+def test_determinism_and_geometry_independence(monkeypatch):
+    """Same seed -> same bytes; a different launch geometry -> same bytes."""
+    outs = []
+    for env in ({}, {}, {"PA_SWEEP_C": "2", "PA_SWEEP_T": "64"}, {"PA_SWEEP_C": "4", "PA_SWEEP_T": "128", "PA_SWEEP_CMP": "0"}):
+        for k in ("PA_SWEEP_C", "PA_SWEEP_T", "PA_SWEEP_CMP"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        g = pa.Population(32, 300, 77)
+        obs = pa_driver.run_fixed(g, [0.0, 0.2, 0.4, 0.5], 3)
+        outs.append((g.get_spins().tobytes(), repr(obs)))
+    assert outs[0] == outs[1] == outs[2] == outs[3]
