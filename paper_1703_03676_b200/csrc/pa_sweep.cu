@@ -23,9 +23,11 @@ struct SweepParams {
     int L, Lh, H, C, N;
 };
 
-// m = 2*m + (x < T): the borrow of x - T shifted into the mask.  ptxas emits one carry-out IADD3 (ALU
-// pipe) and one IMAD.X (FMA pipe), which balances the two integer pipes.
-__device__ __forceinline__ void pa_shift_in_lt(uint32_t& m, uint32_t x, uint32_t T) {
+// m = 2*m + (x >= T).  "sub.cc" leaves the hardware carry of x + ~T + 1 in CC.CF, i.e. NOT borrow, and
+// "madc" adds it: ptxas emits one carry-out IADD3 (ALU pipe) and one IMAD.X (FMA pipe), which balances
+// the two integer pipes.  Exact for every T including 0 (always 1) -- checked on the
+// device by tests/test_parity_gpu.py::test_sweep_threshold_extremes.
+__device__ __forceinline__ void pa_shift_in_ge(uint32_t& m, uint32_t x, uint32_t T) {
     asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 2, 0;\n\t}" : "+r"(m) : "r"(x), "r"(T));
 }
 
@@ -89,17 +91,17 @@ __device__ __forceinline__ uint32_t pa_flip_mask(uint32_t s, uint32_t n0, uint32
     // ---- acceptance: flip iff u >= 2, or u = 1 and x < T4, or u = 0 and x < T8 (O3) ----
     uint32_t acc = 0;
     if (CMP == 1) {
-        uint32_t m4 = 0, m8 = 0;               // built most-significant bit first
+        uint32_t g4 = 0, g8 = 0;               // bit b = (x_b >= T): built most-significant bit first
 #pragma unroll
         for (int i = 7; i >= 0; --i) {
             const uint32_t xs[4] = {x0[i], x1[i], x2[i], x3[i]};
 #pragma unroll
             for (int q = 3; q >= 0; --q) {
-                pa_shift_in_lt(m4, xs[q], P.T4);
-                pa_shift_in_lt(m8, xs[q], P.T8);
+                pa_shift_in_ge(g4, xs[q], P.T4);
+                pa_shift_in_ge(g8, xs[q], P.T8);
             }
         }
-        acc = m4 & (U1 | m8);
+        acc = ~g4 & (U1 | ~g8);                // (x < T4) and (u >= 1 or x < T8)
     } else {
         uint32_t m4 = 0, m8 = 0;
 #pragma unroll

@@ -131,7 +131,7 @@ def test_resample_identity_capacity_and_errors():
     sp = g.get_spins()
     # the oracle has no set_words: compare with the plan computed from the energies instead
     E, _ = g.energies()
-    plan = po.resample_plan(R, E, 5, g.resample_counter, 0.01)
+    plan = po.resample_plan(R, E, 5, g.resample_counter, 0.31 - 0.3)
     R_prev = g.population
     assert g.resample(0.3, 0.31) == plan["R_new"]
     d = g.resample_debug(R_prev)
@@ -203,3 +203,14 @@ def test_determinism_and_geometry_independence(monkeypatch):
         obs = pa_driver.run_fixed(g, [0.0, 0.2, 0.4, 0.5], 3)
         outs.append((g.get_spins().tobytes(), repr(obs)))
     assert outs[0] == outs[1] == outs[2] == outs[3]
+
+
+def test_sweep_threshold_extremes():
+    """T = 2^32-1 (beta = 0), tiny thresholds and T8 = 0 (beta = 3: exp(-24) 2^32 < 1) on both compare paths."""
+    L, R = 8, 96
+    for beta in (0.0, 3.0, 5.0, 2.7):
+        g, o = pa.Population(L, R, 123), po.Oracle(L, R, 123)
+        assert po.thresholds(3.0)[1] == 0
+        g.sweep(0.2, 1); o.sweep(0.2, 1)
+        g.sweep(beta, 3); o.sweep(beta, 3)
+        assert_same_state(g, o)
