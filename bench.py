@@ -1,0 +1,309 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the population-annealing hot path on B200 (contract in the task prompt).
+
+    python bench.py --gpus 1 --steps K --warmup W            # this library, one JSON line
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle on the host cores
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one temperature step of PAPER.md Sec. 2.1 (L56-L62) over one synthetic population:
+resample beta_{i-1} -> beta_i (energies, weights, TREE1024 normaliser, copy numbers, prefix sum,
+replica copy), theta checkerboard Metropolis sweeps at beta_i, energies + observables
+(+ multi-histogram accumulation where the workload asks for it).  metric = spin updates per ns.
+
+N > 1: the path shards as independent populations ("replicas only"): every rank
+anneals its own population (seed + rank) with no data-path collective; weak scaling.
+"""
+import argparse
+import ctypes
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1703_03676_b200.workloads import CONFIGS  # noqa: E402
+
+METRIC = "spin_updates_per_ns"
+UNIT = "updates/ns"
+# Algorithmic work of the dominant kernel (the sweep): 131 IMAD.WIDE.U32 per word of
+# 32 spins (8 Philox4x32-10 calls sharing rounds 1-3) = 4.09375 wide multiplies per spin update; the
+# FMA-heavy pipe issues 32 of them per clock per SM on 148 SMs.
+WIDE_MUL_PER_UPDATE = 131.0 / 32.0
+WIDE_MUL_PER_CLK_PER_SM = 32.0
+N_SM = 148
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2]))
+                for n, v in zip(names, r[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        busy = [c for c in sm if mx and c > 0.5 * max(mx)] or sm
+        return {"sm_mhz": statistics.median(busy) if busy else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def one_step(pop, wl, beta_prev, beta):
+    pop.resample(beta_prev, beta)
+    pop.sweep(beta, wl.theta)
+    obs = pop.observables(beta)
+    if wl.multi_histogram:
+        pop.hist_accumulate(beta)
+    return obs
+
+
+def next_beta(pop, wl, betas, i, beta_prev):
+    if wl.n_steps is not None:
+        return betas[min(i, len(betas) - 1)]
+    d = pop.adapt_dbeta(wl.target_overlap, beta_prev, wl.beta_f)
+    return min(wl.beta_f, beta_prev + d)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1703_03676_b200 import pa
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the library has no CPU path (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    wl = CONFIGS[args.config]
+    K, Wm = args.steps, args.warmup
+    pop = pa.Population(wl.L, wl.R, wl.seed + rank)
+    betas = wl.betas() if wl.n_steps is not None else None
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
+    peaks, peak_src = measured_peaks()
+
+    beta_prev, i = wl.beta0, 0
+    pop.observables(beta_prev)
+    for _ in range(Wm):                                                        # warm-up steps (untimed)
+        i += 1
+        beta = next_beta(pop, wl, betas, i, beta_prev)
+        one_step(pop, wl, beta_prev, beta)
+        beta_prev = beta
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches0 = pop.launch_count
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    updates, sweep_ms, sweep_updates, res_ms, copy_ms, copy_bytes = 0, [], [], [], [], []
+    obs = None
+    for s in range(K):
+        i += 1
+        flush.zero_()                                                          # L2 flush, outside the timed events
+        beta = next_beta(pop, wl, betas, i, beta_prev) if wl.n_steps is not None else None
+        ev[s][0].record()
+        if beta is None:                                                       # adaptive: the bisection is part of the step
+            beta = next_beta(pop, wl, betas, i, beta_prev)
+        obs = one_step(pop, wl, beta_prev, beta)
+        ev[s][1].record()
+        beta_prev = beta
+        R = obs["R"]
+        updates += R * wl.N * wl.theta
+        sweep_ms.append(pop.last_sweep_ms()); sweep_updates.append(R * wl.N * wl.theta)
+        t, c = pop.last_resample_ms()
+        res_ms.append(t); copy_ms.append(c); copy_bytes.append(2 * ((R + 31) // 32) * wl.N * 4)
+    torch.cuda.synchronize()
+    launches = pop.launch_count - launches0
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    clocks = sampler.stop() if rank == 0 else None
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        u = torch.tensor([float(updates)], dtype=torch.float64, device="cuda")
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        total_ms, updates_all = float(t.item()), float(u.item())
+        dist.barrier()
+    else:
+        updates_all = float(updates)
+    value = updates_all / (total_ms * 1e6)
+
+    # ---- end to end through the C ABI with HOST buffers: the population lives in pinned host memory between steps
+    e2e = None
+    if rank == 0 or world > 1:
+        Ke = max(1, min(K, args.e2e_steps))
+        G = (pop.capacity + 31) // 32
+        host_words = torch.empty((G, wl.N), dtype=torch.int32).pin_memory()
+        host_E = torch.empty(pop.capacity, dtype=torch.int32).pin_memory()
+        host_M = torch.empty(pop.capacity, dtype=torch.int32).pin_memory()
+        pop.get_words(host_words)
+        R_host = pop.population
+        h2d = d2h = 0
+        upd_e = 0
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for s in range(Ke):
+            i += 1
+            beta = next_beta(pop, wl, betas, i, beta_prev)
+            nb = ((R_host + 31) // 32) * wl.N * 4
+            pop.set_words(R_host, host_words); h2d += nb
+            o = one_step(pop, wl, beta_prev, beta)
+            pop.energies_into(host_E, host_M)
+            pop.get_words(host_words)
+            R_host = pop.population
+            d2h += ((R_host + 31) // 32) * wl.N * 4 + 8 * R_host + ctypes.sizeof(pa.pa_obs_t)
+            upd_e += o["R"] * wl.N * wl.theta
+            beta_prev = beta
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            u = torch.tensor([float(upd_e)], dtype=torch.float64, device="cuda"); dist.all_reduce(u, op=dist.ReduceOp.SUM)
+            dt, upd_e = float(t.item()), float(u.item())
+        e2e = {"value": upd_e / (dt * 1e9), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke,
+               "steps": Ke, "what": "population words pinned-host -> device, one step, energies + words + observables back to host"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # ---- roofline of the dominant kernel (the sweep), live from the library's CUDA events on its stream
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    k_ms = sum(sweep_ms) / len(sweep_ms)
+    k_upd = sum(sweep_updates) / len(sweep_updates)
+    achieved = WIDE_MUL_PER_UPDATE * k_upd / (k_ms * 1e6)                     # G wide-multiplies / s
+    peak = N_SM * WIDE_MUL_PER_CLK_PER_SM * sm_max * 1e-3                      # G wide-multiplies / s at the max SM clock
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get(wl.name)
+    roofline = {"bound": "alu", "kernel": "pa_sweep_kernel", "achieved": achieved, "peak": peak, "unit": "G IMAD.WIDE.U32/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": f"148 SM x 32/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
+                "kernel_ms": k_ms, "kernel_updates_per_ns": k_upd / (k_ms * 1e6), "share_of_step": sum(sweep_ms) / total_ms,
+                "algorithmic_per_update": WIDE_MUL_PER_UPDATE}
+    cms = sum(copy_ms) / len(copy_ms)
+    resample = {"ms_per_step": sum(res_ms) / len(res_ms), "copy_kernel_ms": cms,
+                "copy_gbs": (sum(copy_bytes) / len(copy_bytes)) / (cms * 1e6) if cms > 0 else None,
+                "copy_frac_of_hbm": ((sum(copy_bytes) / len(copy_bytes)) / (cms * 1e6)) / float(peaks["hbm_gbs"]) if cms > 0 else None,
+                "hbm_peak_gbs": float(peaks["hbm_gbs"]), "peak_source": peak_src}
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+           "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "u32", "data": "synthetic",
+           "config": {"workload": wl.name, "L": wl.L, "R_per_gpu": wl.R, "theta": wl.theta, "beta_from": wl.beta0,
+                      "schedule": "adaptive" if wl.n_steps is None else f"{wl.n_steps} equal steps to {wl.beta_f}",
+                      "l2": "flushed between timed steps (256 MiB memset outside the CUDA events)",
+                      "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "resample": resample,
+           "last_observables": obs}
+    out["cpu_baseline"] = cpu_baseline(wl) if world == 1 and not args.no_cpu else None
+    print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def oracle_step_rate(wl, R_sample, steps, warmup):
+    """The oracle, as it stands, on a population of R_sample replicas of the workload's shape."""
+    from oracle import pa_oracle as po
+    o = po.Oracle(wl.L, R_sample, wl.seed)
+    betas = wl.betas() if wl.n_steps is not None else [wl.beta0 + 0.005 * i for i in range(steps + warmup + 2)]
+    i, beta_prev = 0, betas[0]
+    for _ in range(warmup):
+        i += 1
+        o.resample(beta_prev, betas[i]); o.sweep(betas[i], wl.theta); o.observables(betas[i]); beta_prev = betas[i]
+    upd, t0 = 0, time.perf_counter()
+    for _ in range(steps):
+        i += 1
+        o.resample(beta_prev, betas[i]); o.sweep(betas[i], wl.theta); ob = o.observables(betas[i]); beta_prev = betas[i]
+        upd += ob["R"] * wl.N * wl.theta
+    dt = time.perf_counter() - t0
+    return upd / (dt * 1e9), dt / steps * 1e3, po.num_threads()
+
+
+def cpu_baseline(wl):
+    R_s = min(wl.R, max(256, int(1.0e9 / (wl.N * wl.theta))))               # ~1e9 spin updates of CPU work
+    v, ms, cores = oracle_step_rate(wl, R_s, 1, 0)
+    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": ms,
+            "sample": f"one temperature step (resample + {wl.theta} sweeps + observables) of R={R_s} replicas, L={wl.L}, oracle/pa_oracle.cpp -O2 OpenMP"}
+
+
+def run_reference(args):
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    wl = CONFIGS[args.config]
+    R_s = min(wl.R, max(256, int(2.0e8 / (wl.N * wl.theta))))               # bounded sample per step
+    v, ms, cores = oracle_step_rate(wl, R_s, args.steps, args.warmup)
+    sample = f"each step = one temperature step of R={R_s} replicas of {wl.name} (L={wl.L}, theta={wl.theta}); CPU oracle, OpenMP"
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+           "config": {"workload": wl.name, "L": wl.L, "R_per_gpu": wl.R, "theta": wl.theta, "sample_R": R_s},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=sorted(CONFIGS), help="BASELINE.json configs index + 1")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

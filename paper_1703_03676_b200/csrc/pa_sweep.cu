@@ -31,6 +31,14 @@ __device__ __forceinline__ void pa_shift_in_ge(uint32_t& m, uint32_t x, uint32_t
     asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 2, 0;\n\t}" : "+r"(m) : "r"(x), "r"(T));
 }
 
+// m |= bit if x < T, with both instructions on the ALU pipe (ISETP + predicated LOP3).  The FMA pipe is
+// the bottleneck of this kernel (IMAD.WIDE.U32 issues at 32 lanes/clk/SM), so the acceptance test must
+// not add to it.
+template <uint32_t BIT>
+__device__ __forceinline__ void pa_or_if_lt(uint32_t& m, uint32_t x, uint32_t T) {
+    asm("{\n\t.reg .pred q;\n\tsetp.lt.u32 q, %1, %2;\n\t@q or.b32 %0, %0, %3;\n\t}" : "+r"(m) : "r"(x), "r"(T), "n"(BIT));
+}
+
 // Flip mask of one word: bit b set iff replica 32g+b flips its spin at `site` (O3).
 //   s: centre word, n0..n3: the four neighbour words.
 //   c0base = hi(M1*c2) ^ k0[0] ^ 8g, lo1u = lo(M1*c2), c2 = 2t+colour (uniform per half-sweep).
@@ -102,6 +110,14 @@ __device__ __forceinline__ uint32_t pa_flip_mask(uint32_t s, uint32_t n0, uint32
             }
         }
         acc = ~g4 & (U1 | ~g8);                // (x < T4) and (u >= 1 or x < T8)
+    } else if (CMP == 2) {
+        uint32_t m4 = 0, m8 = 0;
+#define PA_CMP4(I, Q, X) pa_or_if_lt<(1u << (4 * I + Q))>(m4, X, P.T4); pa_or_if_lt<(1u << (4 * I + Q))>(m8, X, P.T8);
+#define PA_CMPI(I) PA_CMP4(I, 0, x0[I]) PA_CMP4(I, 1, x1[I]) PA_CMP4(I, 2, x2[I]) PA_CMP4(I, 3, x3[I])
+        PA_CMPI(0) PA_CMPI(1) PA_CMPI(2) PA_CMPI(3) PA_CMPI(4) PA_CMPI(5) PA_CMPI(6) PA_CMPI(7)
+#undef PA_CMPI
+#undef PA_CMP4
+        acc = m4 & (U1 | m8);
     } else {
         uint32_t m4 = 0, m8 = 0;
 #pragma unroll
@@ -227,7 +243,8 @@ int pa_sweep_configure(pa_handle* h) {
     int forceT = pa_env_int("PA_SWEEP_T", 0);
     if (forceT >= 32 && forceT <= 256) T = forceT;
     h->sweep_C = C; h->sweep_T = T;
-    h->sweep_cmp = pa_env_int("PA_SWEEP_CMP", 1) ? 1 : 0;
+    h->sweep_cmp = pa_env_int("PA_SWEEP_CMP", 2);
+    if (h->sweep_cmp < 0 || h->sweep_cmp > 2) h->sweep_cmp = 2;
     return PA_OK;
 }
 
@@ -262,8 +279,9 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     const int64_t G = (h->R_cur + 31) / 32;
     const unsigned grid = (unsigned)(G * P.C);
     cudaError_t e;
-    if (P.C > 1) e = h->sweep_cmp ? pa_sweep_launch_t<1, true>(h, P, smem, grid) : pa_sweep_launch_t<0, true>(h, P, smem, grid);
-    else         e = h->sweep_cmp ? pa_sweep_launch_t<1, false>(h, P, smem, grid) : pa_sweep_launch_t<0, false>(h, P, smem, grid);
+    const int v = h->sweep_cmp;
+    if (P.C > 1) e = v == 2 ? pa_sweep_launch_t<2, true>(h, P, smem, grid) : v == 1 ? pa_sweep_launch_t<1, true>(h, P, smem, grid) : pa_sweep_launch_t<0, true>(h, P, smem, grid);
+    else         e = v == 2 ? pa_sweep_launch_t<2, false>(h, P, smem, grid) : v == 1 ? pa_sweep_launch_t<1, false>(h, P, smem, grid) : pa_sweep_launch_t<0, false>(h, P, smem, grid);
     PA_CUDA(h, e);
     h->launches += 1;
     return PA_OK;
