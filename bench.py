@@ -89,6 +89,24 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def reduce_over_ranks(ms, units, device, dist=None):
+    """N > 1 (replicas only): the job's time is the MAX over ranks, its work the SUM over ranks.
+    `dist` = torch.distributed when a process group is up (nccl on the GPU box, gloo in tests/test_multirank_gloo.py)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms), float(units)
+    import torch
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def rank_seed(wl, rank):
+    """Every rank anneals its own independent population (no data-path collective)."""
+    return wl.seed + rank
+
+
 def one_step(pop, wl, beta_prev, beta):
     pop.resample(beta_prev, beta)
     pop.sweep(beta, wl.theta)
@@ -119,7 +137,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     wl = CONFIGS[args.config]
     K, Wm = args.steps, args.warmup
-    pop = pa.Population(wl.L, wl.R, wl.seed + rank)
+    pop = pa.Population(wl.L, wl.R, rank_seed(wl, rank))
     betas = wl.betas() if wl.n_steps is not None else None
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
     peaks, peak_src = measured_peaks()
@@ -160,15 +178,9 @@ def run_ours(args):
     launches = pop.launch_count - launches0
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     clocks = sampler.stop() if rank == 0 else None
+    total_ms, updates_all = reduce_over_ranks(total_ms, updates, "cuda", dist if world > 1 else None)
     if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        u = torch.tensor([float(updates)], dtype=torch.float64, device="cuda")
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        total_ms, updates_all = float(t.item()), float(u.item())
         dist.barrier()
-    else:
-        updates_all = float(updates)
     value = updates_all / (total_ms * 1e6)
 
     # ---- end to end through the C ABI with HOST buffers: the population lives in pinned host memory between steps
@@ -201,10 +213,7 @@ def run_ours(args):
             beta_prev = beta
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            u = torch.tensor([float(upd_e)], dtype=torch.float64, device="cuda"); dist.all_reduce(u, op=dist.ReduceOp.SUM)
-            dt, upd_e = float(t.item()), float(u.item())
+        dt, upd_e = reduce_over_ranks(dt, upd_e, "cuda", dist if world > 1 else None)
         e2e = {"value": upd_e / (dt * 1e9), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke,
                "steps": Ke, "what": "population words pinned-host -> device, one step, energies + words + observables back to host"}
 

@@ -1,0 +1,67 @@
+"""N > 1 on CPU (gloo, world size 2): the path shards as independent populations, so the
+multi-rank logic is bench.py's rank seeding and its max-over-ranks time / sum-over-ranks work reduction.
+The oracle stands in for the per-rank population here (no GPU in this test): two ranks anneal different
+seeds, and the whole-job throughput is (sum of updates) / (max of times)."""
+import os
+import socket
+import sys
+
+import pytest
+
+torch = pytest.importorskip("torch")
+import torch.distributed as dist            # noqa: E402
+import torch.multiprocessing as mp          # noqa: E402
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _free_port():
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close()
+    return p
+
+
+def _worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    from oracle import pa_oracle as po
+    from paper_1703_03676_b200.workloads import CONFIGS
+    wl = CONFIGS[1]
+    seed = bench.rank_seed(wl, rank)
+    o = po.Oracle(wl.L, 64, seed)
+    betas = wl.betas()
+    o.resample(betas[0], betas[1]); o.sweep(betas[1], 2)
+    E, _ = o.energies()
+    units = o.population * wl.N * 2
+    ms = 10.0 * (rank + 1)                                   # rank 1 is the slow one
+    t, u = bench.reduce_over_ranks(ms, units, "cpu", dist)
+    allu = [None] * world
+    dist.all_gather_object(allu, (seed, int(units), int(E.sum())))
+    dist.barrier()
+    if rank == 0:
+        q.put((t, u, allu))
+    dist.destroy_process_group()
+
+
+def test_two_ranks_independent_populations_and_reduction():
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.SimpleQueue()
+    procs = [ctx.Process(target=_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    for p in procs:
+        p.join(120)
+        assert p.exitcode == 0
+    t, u, allu = q.get()
+    assert t == 20.0                                         # max over ranks
+    assert u == float(sum(x[1] for x in allu))               # sum over ranks
+    assert allu[0][0] != allu[1][0]                          # different seeds ...
+    assert allu[0][2] != allu[1][2]                          # ... different populations
+
+
+def test_single_rank_reduction_is_identity():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.reduce_over_ranks(3.5, 7, "cpu", None) == (3.5, 7.0)
