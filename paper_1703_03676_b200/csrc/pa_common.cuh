@@ -103,7 +103,7 @@ struct pa_handle {
     cudaEvent_t ev[6];                  // sweep begin/end, resample begin/end, copy begin/end
     bool sweep_timed, resample_timed;
     int64_t launches;
-    int sweep_C, sweep_T, sweep_cmp;    // sweep launch geometry (cluster size, threads) and compare variant
+    int sweep_C, sweep_T, sweep_cmp, sweep_kind;   // sweep launch geometry (cluster size, threads), compare variant, kernel kind
     char cuda_err[256];
 };
 

@@ -19,16 +19,19 @@ struct SweepParams {
     PhiloxKeys K;
     uint32_t T4, T8;                 // acceptance thresholds for dE = 4, 8 (O2)
     uint32_t t0;                     // sweep counter at launch
+    uint32_t two;                    // the constant 2, opaque to ptxas (see pa_shift_in_ge)
     int theta;
     int L, Lh, H, C, N;
 };
 
 // m = 2*m + (x >= T).  "sub.cc" leaves the hardware carry of x + ~T + 1 in CC.CF, i.e. NOT borrow, and
-// "madc" adds it: ptxas emits one carry-out IADD3 (ALU pipe) and one IMAD.X (FMA pipe), which balances
-// the two integer pipes.  Exact for every T including 0 (always 1) -- checked on the
-// device by tests/test_parity_gpu.py::test_sweep_threshold_extremes.
-__device__ __forceinline__ void pa_shift_in_ge(uint32_t& m, uint32_t x, uint32_t T) {
-    asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, 2, 0;\n\t}" : "+r"(m) : "r"(x), "r"(T));
+// "madc" adds it: ptxas emits one carry-out IADD3 (ALU pipe) and one IMAD.X (FMA pipe).  The multiplier is
+// passed as a register holding 2 (a kernel parameter) so that ptxas cannot turn the shift-in into an ALU-pipe
+// LEA.X / IADD3.X: on B200 every IMAD.WIDE also blocks the ALU pipe for two cycles, which makes the ALU pipe
+// the binding one, so the insert has to stay on the FMA pipe.  Exact for every T
+// including 0 (always 1) -- checked on the device by tests/test_parity_gpu.py::test_sweep_threshold_extremes.
+__device__ __forceinline__ void pa_shift_in_ge(uint32_t& m, uint32_t x, uint32_t T, uint32_t two) {
+    asm("{\n\t.reg .u32 t;\n\tsub.cc.u32 t, %1, %2;\n\tmadc.lo.u32 %0, %0, %3, 0;\n\t}" : "+r"(m) : "r"(x), "r"(T), "r"(two));
 }
 
 // m |= bit if x < T, with both instructions on the ALU pipe (ISETP + predicated LOP3).  The FMA pipe is
@@ -105,8 +108,8 @@ __device__ __forceinline__ uint32_t pa_flip_mask(uint32_t s, uint32_t n0, uint32
             const uint32_t xs[4] = {x0[i], x1[i], x2[i], x3[i]};
 #pragma unroll
             for (int q = 3; q >= 0; --q) {
-                pa_shift_in_ge(g4, xs[q], P.T4);
-                pa_shift_in_ge(g8, xs[q], P.T8);
+                pa_shift_in_ge(g4, xs[q], P.T4, P.two);
+                pa_shift_in_ge(g8, xs[q], P.T8, P.two);
             }
         }
         acc = ~g4 & (U1 | ~g8);                // (x < T4) and (u >= 1 or x < T8)
@@ -220,6 +223,95 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Column-walk variant for power-of-two L >= 64 (all of BASELINE.json's configs but L = 16).
+// A thread owns one column xh of the strip and walks down `rpt` consecutive rows, two rows per
+// iteration (the two rows have opposite x-parity, so the pair is the natural unit).  Every shared-memory
+// address is the thread's base pointer plus a compile-time immediate, the up-neighbour of the second row
+// and the down-neighbour of the first are words the pair has loaded anyway, and the site index advances by
+// a constant: the per-word addressing overhead of the generic kernel (about 35 ALU-pipe instructions per
+// word, 8 % of the kernel) disappears.  The ALU pipe is the binding one.
+// Requirements (checked by pa_sweep_configure): Lh = 2^LOG_LH >= 32, T >= Lh, H*Lh/T even and >= 2, H even.
+// ------------------------------------------------------------------------------------------------
+#ifndef PA_SWEEP_MINB
+#define PA_SWEEP_MINB 1
+#endif
+template <int CMP, int LOG_LH, bool CLUSTER>
+__global__ void __launch_bounds__(256, PA_SWEEP_MINB)
+pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
+    extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
+    constexpr int Lh = 1 << LOG_LH;
+    const int T = blockDim.x, tid = threadIdx.x;
+    const int C = CLUSTER ? P.C : 1;
+    unsigned cr = 0;
+    if (CLUSTER) cr = cg::this_cluster().block_rank();
+    const long long g = blockIdx.x / C;
+    const int H = P.H;
+    const int y0 = (int)cr * H;
+    const int half = H * Lh;
+    uint32_t* gbase = pop + g * (long long)P.N;
+    const int goff = y0 * Lh, gcol = P.N >> 1;
+
+    for (int c = 0; c < 2; ++c) {
+        const uint4* src = reinterpret_cast<const uint4*>(gbase + c * gcol + goff);
+        uint4* dst = reinterpret_cast<uint4*>(tile + c * half);
+        for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+    }
+    const uint32_t* up_tile = tile;
+    const uint32_t* dn_tile = tile;
+    if (CLUSTER) {
+        cg::cluster_group cl = cg::this_cluster();
+        up_tile = cl.map_shared_rank(tile, (cr + C - 1) % C);
+        dn_tile = cl.map_shared_rank(tile, (cr + 1) % C);
+        cl.sync();
+    } else {
+        __syncthreads();
+    }
+
+    const int xh = tid & (Lh - 1), rb = tid >> LOG_LH;
+    const int rpt = half / T;                          // rows per thread: even, >= 2
+    const int ya = rb * rpt;                           // first local row (even)
+    const int dL = ((xh - 1) & (Lh - 1)) - xh, dR = ((xh + 1) & (Lh - 1)) - xh;
+    const int b0 = ya * Lh + xh;
+    const uint32_t g8 = (uint32_t)(8 * g);
+    const uint32_t site_base = 2u * (uint32_t)((y0 + ya) * Lh + xh);   // site of (row y0+ya, x = 2 xh)
+    for (int it = 0; it < P.theta; ++it) {
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t c2 = 2u * (P.t0 + (uint32_t)it) + (uint32_t)c;
+            uint32_t hi1u, lo1u;
+            pa_mulhilo(PA_PHILOX_M1, c2, hi1u, lo1u);
+            const uint32_t c0base = hi1u ^ P.K.k0[0] ^ g8;
+            uint32_t* mine = tile + c * half + b0;
+            const uint32_t* oth = tile + (1 - c) * half + b0;
+            // rows y0+ya+2k have x-parity p = c (x = 2 xh + c), rows y0+ya+2k+1 have p = 1 - c
+            const int dA = c ? dR : dL, dB = c ? dL : dR;
+            uint32_t site = site_base + (uint32_t)c;
+#pragma unroll 1
+            for (int k = 0; k < rpt; k += 2) {
+                const uint32_t s0 = mine[0], s1 = mine[Lh];
+                const uint32_t nS0 = oth[0], nS1 = oth[Lh];
+                const uint32_t nX0 = oth[dA], nX1 = oth[Lh + dB];
+                uint32_t nU0, nD1;
+                if (ya + k > 0) nU0 = oth[-Lh]; else nU0 = up_tile[(1 - c) * half + (H - 1) * Lh + xh];
+                if (ya + k + 2 < H) nD1 = oth[2 * Lh]; else nD1 = dn_tile[(1 - c) * half + xh];
+                const uint32_t f0 = pa_flip_mask<CMP>(s0, nS0, nX0, nU0, nS1, site, c0base, lo1u, P);
+                const uint32_t f1 = pa_flip_mask<CMP>(s1, nS1, nX1, nS0, nD1, site + (uint32_t)(2 * Lh + 1 - 2 * c), c0base, lo1u, P);
+                mine[0] = s0 ^ f0;
+                mine[Lh] = s1 ^ f1;
+                mine += 2 * Lh; oth += 2 * Lh; site += 4u * Lh;
+            }
+            if (CLUSTER) cg::this_cluster().sync(); else __syncthreads();
+        }
+    }
+
+    for (int c = 0; c < 2; ++c) {
+        uint4* dst = reinterpret_cast<uint4*>(gbase + c * gcol + goff);
+        const uint4* src = reinterpret_cast<const uint4*>(tile + c * half);
+        for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
 static int pa_env_int(const char* name, int dflt) {
@@ -229,6 +321,7 @@ static int pa_env_int(const char* name, int dflt) {
 
 // Launch geometry: the smallest cluster size C in {1,2,4,8} dividing L whose strip (L/C rows of both
 // colours, L*L*4/C bytes) fits the shared-memory budget per CTA; threads = min(256, words per colour).
+// kind 1 = column-walk kernel (power-of-two L >= 64), kind 0 = generic kernel (any even L).
 int pa_sweep_configure(pa_handle* h) {
     const int L = h->L;
     const size_t budget = (size_t)pa_env_int("PA_SWEEP_SMEM_KB", 64) * 1024;
@@ -242,15 +335,22 @@ int pa_sweep_configure(pa_handle* h) {
     while (T > 32 && T > half) T >>= 1;
     int forceT = pa_env_int("PA_SWEEP_T", 0);
     if (forceT >= 32 && forceT <= 256) T = forceT;
-    h->sweep_C = C; h->sweep_T = T;
-    h->sweep_cmp = pa_env_int("PA_SWEEP_CMP", 2);
-    if (h->sweep_cmp < 0 || h->sweep_cmp > 2) h->sweep_cmp = 2;
+    int kind = ((L & (L - 1)) == 0 && L >= 64) ? 1 : 0;
+    kind = pa_env_int("PA_SWEEP_KIND", kind);
+    if (kind == 1) {
+        const int Lh = L / 2, H = L / C;
+        const bool ok = (L & (L - 1)) == 0 && L >= 64 && (H & 1) == 0 && T >= Lh && (T & (T - 1)) == 0 &&
+                        half % T == 0 && half / T >= 2 && ((half / T) & 1) == 0;
+        if (!ok) kind = 0;
+    }
+    h->sweep_C = C; h->sweep_T = T; h->sweep_kind = kind;
+    h->sweep_cmp = pa_env_int("PA_SWEEP_CMP", 1);
+    if (h->sweep_cmp < 0 || h->sweep_cmp > 2) h->sweep_cmp = 1;
     return PA_OK;
 }
 
-template <int CMP, bool CLUSTER>
-static cudaError_t pa_sweep_launch_t(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
-    auto kern = pa_sweep_kernel<CMP, CLUSTER>;
+template <typename Kern>
+static cudaError_t pa_sweep_launch_k(pa_handle* h, Kern kern, const SweepParams& P, size_t smem, unsigned grid, bool cluster) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
@@ -260,7 +360,7 @@ static cudaError_t pa_sweep_launch_t(pa_handle* h, const SweepParams& P, size_t 
     cfg.stream = h->stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = CLUSTER ? (unsigned)P.C : 1u;
+    attr[0].val.clusterDim.x = cluster ? (unsigned)P.C : 1u;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
@@ -268,20 +368,35 @@ static cudaError_t pa_sweep_launch_t(pa_handle* h, const SweepParams& P, size_t 
     return cudaLaunchKernelEx(&cfg, kern, h->spins[h->cur], P);
 }
 
+template <int CMP>
+static cudaError_t pa_sweep_dispatch(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
+    const bool cl = P.C > 1;
+    if (h->sweep_kind == 1) {
+        switch (P.Lh) {
+#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_col_kernel<CMP, LOG, true>, P, smem, grid, true) \
+                                                      : pa_sweep_launch_k(h, pa_sweep_col_kernel<CMP, LOG, false>, P, smem, grid, false);
+            PA_COL_CASE(5) PA_COL_CASE(6) PA_COL_CASE(7) PA_COL_CASE(8)
+#undef PA_COL_CASE
+            default: break;
+        }
+    }
+    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<CMP, true>, P, smem, grid, true)
+              : pa_sweep_launch_k(h, pa_sweep_kernel<CMP, false>, P, smem, grid, false);
+}
+
 int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     if (theta == 0) return PA_OK;
     SweepParams P;
     P.K = h->keys;
     P.T4 = T4; P.T8 = T8;
-    P.t0 = h->t; P.theta = theta;
+    P.t0 = h->t; P.theta = theta; P.two = 2u;
     P.L = h->L; P.Lh = h->L / 2; P.C = h->sweep_C; P.H = h->L / h->sweep_C; P.N = h->N;
     const size_t smem = (size_t)P.H * h->L * 4;
     const int64_t G = (h->R_cur + 31) / 32;
     const unsigned grid = (unsigned)(G * P.C);
-    cudaError_t e;
     const int v = h->sweep_cmp;
-    if (P.C > 1) e = v == 2 ? pa_sweep_launch_t<2, true>(h, P, smem, grid) : v == 1 ? pa_sweep_launch_t<1, true>(h, P, smem, grid) : pa_sweep_launch_t<0, true>(h, P, smem, grid);
-    else         e = v == 2 ? pa_sweep_launch_t<2, false>(h, P, smem, grid) : v == 1 ? pa_sweep_launch_t<1, false>(h, P, smem, grid) : pa_sweep_launch_t<0, false>(h, P, smem, grid);
+    const cudaError_t e = v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)
+                                                                                    : pa_sweep_dispatch<0>(h, P, smem, grid);
     PA_CUDA(h, e);
     h->launches += 1;
     return PA_OK;
