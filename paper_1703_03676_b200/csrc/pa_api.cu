@@ -20,7 +20,7 @@ void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const cha
 }
 
 struct PaLayout {
-    size_t spins0, spins1, E, M, w, r, o, parent, partials, wtab, scan, Hsum, Hcur, lnD, scal, slots, stage, total;
+    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, lnD, scal, slots, stage, total;
     size_t stage_bytes;
     int64_t R_cap, G_cap, tiles;
 };
@@ -42,6 +42,7 @@ static PaLayout pa_layout(int L, int64_t R) {
     y.o = take((size_t)y.R_cap * 4);
     y.parent = take((size_t)y.R_cap * 4);
     y.partials = take((size_t)y.tiles * 8);
+    y.runsum = take((size_t)y.G_cap * 8);
     y.wtab = take((N + 1) * 8);
     y.scan = take((size_t)y.tiles * 8);
     y.Hsum = take((N + 1) * 8);
@@ -90,7 +91,20 @@ static int pa_read_scalars(pa_handle* h) {
     return PA_OK;
 }
 
-static int pa_ensure_energies(pa_handle* h) { return h->em_valid ? PA_OK : pa_launch_energy(h); }
+static int pa_ensure_energies(pa_handle* h) { return h->em_valid ? PA_OK : pa_launch_measure(h); }
+
+// E, M, the integer sums and the range of m = (E + 2N)/4 of the current population, mirrored on the host:
+// one measure launch (if the population changed) and one small device-to-host read (if not read yet).
+static int pa_ensure_host_scalars(pa_handle* h) {
+    int rc = pa_ensure_energies(h);
+    if (rc != PA_OK) return rc;
+    if (h->host_scal_valid) return PA_OK;
+    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    h->host_scal_valid = true;
+    h->Emin = -2 * h->N + 4 * (int)(0xffffffffu - h->h_scal->mmin_inv);
+    h->Emax = -2 * h->N + 4 * (int)h->h_scal->mmax;
+    return PA_OK;
+}
 
 // O5: wtab[d] = exp(-(dbeta * (double)(4 d))), d = 0..dmax, uploaded to the device table
 static int pa_upload_wtab(pa_handle* h, double dbeta, int dmax) {
@@ -142,7 +156,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     h->spins[0] = (uint32_t*)(b + y.spins0); h->spins[1] = (uint32_t*)(b + y.spins1); h->cur = 0;
     h->E = (int32_t*)(b + y.E); h->M = (int32_t*)(b + y.M);
     h->w = (double*)(b + y.w); h->r = (uint32_t*)(b + y.r); h->o = (uint32_t*)(b + y.o); h->parent = (uint32_t*)(b + y.parent);
-    h->partials = (double*)(b + y.partials); h->wtab = (double*)(b + y.wtab);
+    h->partials = (double*)(b + y.partials); h->runsum = (double*)(b + y.runsum); h->wtab = (double*)(b + y.wtab);
     h->scan_state = (unsigned long long*)(b + y.scan);
     h->Hsum = (unsigned long long*)(b + y.Hsum); h->Hcur = (uint32_t*)(b + y.Hcur); h->lnD = (double*)(b + y.lnD);
     h->d_scal = (PaScalars*)(b + y.scal);
@@ -151,11 +165,12 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     // pinned host mirrors
     if (cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
         cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->N + 1)) != cudaSuccess) { rc = PA_ERR_CUDA; }
-    for (int i = 0; i < 6 && rc == PA_OK; ++i)
+    for (int i = 0; i < 7 && rc == PA_OK; ++i)
         if (cudaEventCreate(&h->ev[i]) != cudaSuccess) rc = PA_ERR_CUDA;
     if (rc == PA_OK) rc = pa_sweep_configure(h);
     if (rc == PA_OK) {
         // empty histograms: Hsum = 0, Hcur = 0, lnD = -inf
+        cudaMemsetAsync(h->d_scal, 0, sizeof(PaScalars), h->stream);
         cudaMemsetAsync(h->Hsum, 0, ((size_t)h->N + 1) * 8, h->stream);
         cudaMemsetAsync(h->Hcur, 0, ((size_t)h->N + 1) * 4, h->stream);
         for (int m = 0; m <= h->N; ++m) h->h_wtab[m] = -INFINITY;
@@ -173,7 +188,7 @@ int pa_create(int L, int64_t R, uint64_t seed, pa_t** out) { return pa_create_ex
 void pa_destroy(pa_t* h) {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
-    for (int i = 0; i < 6; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    for (int i = 0; i < 7; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->h_wtab) cudaFreeHost(h->h_wtab);
     if (h->owns_stream && h->stream) cudaStreamDestroy(h->stream);
@@ -191,7 +206,7 @@ int pa_sweep(pa_t* h, double beta, int theta) {
     PA_CUDA(h, cudaEventRecord(h->ev[1], h->stream));
     h->sweep_timed = true;
     h->t += (uint32_t)theta;
-    h->em_valid = false;
+    h->em_valid = false; h->host_scal_valid = false;
     return PA_OK;
 }
 
@@ -209,40 +224,46 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     const double dbeta = beta_new - beta;
     int rc;
     PA_CUDA(h, cudaEventRecord(h->ev[2], h->stream));
-    if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
-    if ((rc = pa_launch_minmax(h)) != PA_OK) return rc;
-    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
-    const int Emin = h->h_scal->Emin, Emax = h->h_scal->Emax;
+    // E_min / E_max: already on the host if pa_observables ran on this population (the usual loop, L62);
+    // otherwise one measure launch and one read
+    if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
+    const int Emin = h->Emin, Emax = h->Emax;
     if ((rc = pa_upload_wtab(h, dbeta, (Emax - Emin) / 4)) != PA_OK) return rc;
-    if ((rc = pa_launch_tree_weights(h, 0, h->w)) != PA_OK) return rc;
-    if ((rc = pa_launch_plan(h)) != PA_OK) return rc;
-    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    // weights + W, plan (tau, r, scan, parents, R_new), copy: queued back to back; the copy reads R_new on
+    // the device, so the host waits once, at the end
+    if ((rc = pa_launch_weights(h, Emin, h->w)) != PA_OK) return rc;
+    if ((rc = pa_launch_plan(h, Emin)) != PA_OK) return rc;
+    // R_new and W travel to the host right after the plan kernel; the copy is queued behind them and runs
+    // while the host wakes up, so the stream never idles on this call's one synchronisation
+    PA_CUDA(h, cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToHost, h->stream));
+    PA_CUDA(h, cudaEventRecord(h->ev[6], h->stream));
+    PA_CUDA(h, cudaEventRecord(h->ev[4], h->stream));
+    if ((rc = pa_launch_copy(h)) != PA_OK) return rc;
+    PA_CUDA(h, cudaEventRecord(h->ev[5], h->stream));
+    PA_CUDA(h, cudaEventRecord(h->ev[3], h->stream));
+    PA_CUDA(h, cudaEventSynchronize(h->ev[6]));
+    h->resample_timed = true;
     const int64_t R_new = (int64_t)h->h_scal->R_new;
     const double W = h->h_scal->W;
     h->R_prev = h->R_cur; h->W_last = W;
-    if (R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;      // population, k, lnZ unchanged (O7)
-    PA_CUDA(h, cudaEventRecord(h->ev[4], h->stream));
-    if ((rc = pa_launch_copy(h, R_new)) != PA_OK) return rc;
-    PA_CUDA(h, cudaEventRecord(h->ev[5], h->stream));
-    PA_CUDA(h, cudaEventRecord(h->ev[3], h->stream));
-    h->resample_timed = true;
+    if (R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;      // population, k, lnZ unchanged (O7): only the spare buffer was written
     const double lnQ = -dbeta * (double)Emin + log(W / (double)h->R_cur);   // Eq. 1 with the shift (O5)
     h->cur ^= 1;
     h->R_cur = R_new;
     h->k += 1;
     h->lnZ += lnQ;                                                    // Eq. 4 (L90)
     h->lnQ_last = lnQ;
-    h->em_valid = false;
+    h->em_valid = false; h->host_scal_valid = false;
     if (R_new_out) *R_new_out = R_new;
     return PA_OK;
 }
 
-// alpha(dbeta) of Eq. 8 given Emin/Emax already on the host
+// alpha(dbeta) of Eq. 8 given Emin/Emax already on the host: two launches, one read
 static int pa_eval_overlap(pa_handle* h, double dbeta, int Emin, int Emax, double* alpha) {
     int rc;
     if ((rc = pa_upload_wtab(h, dbeta, (Emax - Emin) / 4)) != PA_OK) return rc;
-    if ((rc = pa_launch_tree_weights(h, 0, nullptr)) != PA_OK) return rc;
-    if ((rc = pa_launch_tree_weights(h, 1, nullptr)) != PA_OK) return rc;
+    if ((rc = pa_launch_weights(h, Emin, nullptr)) != PA_OK) return rc;
+    if ((rc = pa_launch_overlap(h, Emin)) != PA_OK) return rc;
     if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
     *alpha = h->h_scal->sum / (double)h->R_cur;
     return PA_OK;
@@ -250,10 +271,8 @@ static int pa_eval_overlap(pa_handle* h, double dbeta, int Emin, int Emax, doubl
 
 static int pa_overlap_prepare(pa_handle* h, int* Emin, int* Emax) {
     int rc;
-    if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
-    if ((rc = pa_launch_minmax(h)) != PA_OK) return rc;
-    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
-    *Emin = h->h_scal->Emin; *Emax = h->h_scal->Emax;
+    if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
+    *Emin = h->Emin; *Emax = h->Emax;
     return PA_OK;
 }
 
@@ -284,10 +303,7 @@ int pa_adapt_dbeta(pa_t* h, double target, double beta, double beta_max, double*
 int pa_observables(pa_t* h, double beta, pa_obs_t* out) {
     if (!h || !out) return PA_ERR_INVALID_ARG;
     int rc;
-    if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
-    if ((rc = pa_launch_obs_sums(h)) != PA_OK) return rc;
-    if ((rc = pa_launch_tree_weights(h, 2, nullptr)) != PA_OK) return rc;
-    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
     const PaScalars& s = *h->h_scal;
     const double R = (double)h->R_cur, N = (double)h->N;
     const __int128 num = (__int128)h->R_cur * (__int128)s.SE2 - (__int128)s.SE * (__int128)s.SE;   // exact (O8)
@@ -296,7 +312,7 @@ int pa_observables(pa_t* h, double beta, pa_obs_t* out) {
     out->C = beta * beta * ((double)num / (R * R * N));
     out->absm = (double)s.SA / (R * N);
     out->m2 = (double)s.SM2 / (R * N * N);
-    out->m4 = s.sum / R;
+    out->m4 = s.m4sum / R;
     out->betaF_per_N = -h->lnZ / N;
     out->S_per_N = beta * out->e + h->lnZ / N;
     out->lnQ = h->lnQ_last;
@@ -369,7 +385,7 @@ int pa_set_spins(pa_t* h, int64_t j0, int64_t nrep, const int8_t* in) {
         if (rc != PA_OK) return rc;
         PA_CUDA(h, cudaStreamSynchronize(h->stream));
     }
-    h->em_valid = false;
+    h->em_valid = false; h->host_scal_valid = false;
     return PA_OK;
 }
 
@@ -396,7 +412,7 @@ int pa_set_words(pa_t* h, int64_t R, const uint32_t* words) {
     int rc = pa_launch_words_in(h, R, src);
     if (rc != PA_OK) return rc;
     h->R_cur = R;
-    h->em_valid = false;
+    h->em_valid = false; h->host_scal_valid = false;
     return PA_OK;
 }
 

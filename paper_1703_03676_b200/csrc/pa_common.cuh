@@ -58,13 +58,19 @@ __device__ __forceinline__ uint4 pa_philox(uint32_t c0, uint32_t c1, uint32_t c2
 
 // device-resident scalars (one block, also mirrored in pinned host memory for small D2H reads)
 struct PaScalars {
-    int32_t Emin, Emax;
-    uint32_t tile_counter;
-    uint32_t R_new;
-    double sum;              // result of the last TREE1024 reduction
-    double W;                // normaliser of the current weight table
-    long long SE, SE2, SA, SM2;
-    uint32_t pad[4];
+    // --- written by pa_measure_kernel; zeroed (cudaMemsetAsync up to R_new) before it runs
+    uint32_t mmin_inv, mmax;     // 2^32-1 - min_j m_j and max_j m_j, m = (E + 2N)/4
+    uint32_t done_counter;       // ticket of the measure kernel's last-CTA stage
+    uint32_t pad0;
+    long long SE, SE2, SA, SM2;  // exact integer sums (O8)
+    double m4sum;                // TREE1024 of (M_j/N)^4
+    // --- written by the resample kernels
+    uint32_t R_new;              // sum of the copy numbers (pa_plan_kernel)
+    uint32_t tile_counter;       // scan tile tickets (reset by pa_tree_kernel<0>)
+    uint32_t tree_ticket;        // ticket of pa_tree_kernel's last-CTA stage (self-resetting)
+    uint32_t pad1;
+    double W;                    // normaliser of the last weight table, TREE1024 order (pa_tree_kernel<0>)
+    double sum;                  // TREE1024 of min(1, tau_j) (pa_tree_kernel<1>)
 };
 
 struct pa_handle {
@@ -81,7 +87,10 @@ struct pa_handle {
     void* ws; size_t ws_bytes;
 
     uint32_t* spins[2]; int cur;        // two packed populations [G_cap][N] (L165 "new population vector")
-    int32_t *E, *M; bool em_valid;      // per-replica energy / magnetisation of the current population
+    int32_t *E, *M; bool em_valid;      // per-replica energy / magnetisation of the current population (+ sums in d_scal)
+    bool host_scal_valid;               // h_scal mirrors d_scal's measure block for the current population
+    int Emin, Emax;                     // range of E_j of the current population (valid with host_scal_valid)
+    double* runsum;                     // [G_cap] run-of-32 sums of the measure kernel
     double* w;                          // weights of the last resample (debug export)
     uint32_t *r, *o, *parent;           // copy numbers, exclusive offsets, parent map
     double* partials;                   // per-tile partial sums (TREE1024)
@@ -100,9 +109,10 @@ struct pa_handle {
     double* h_wtab;                     // pinned, N+1
     int64_t R_prev; double W_last;      // of the last resample
 
-    cudaEvent_t ev[6];                  // sweep begin/end, resample begin/end, copy begin/end
+    cudaEvent_t ev[7];                  // sweep begin/end, resample begin/end, copy begin/end, plan scalars on the host
     bool sweep_timed, resample_timed;
     int64_t launches;
+    bool sweep_C_forced;
     int sweep_C, sweep_T, sweep_cmp, sweep_kind;   // sweep launch geometry (cluster size, threads), compare variant, kernel kind
     char cuda_err[256];
 };
@@ -119,12 +129,11 @@ void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const cha
 int pa_launch_init(pa_handle* h);
 int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta);
 int pa_sweep_configure(pa_handle* h);
-int pa_launch_energy(pa_handle* h);
-int pa_launch_minmax(pa_handle* h);
-int pa_launch_tree_weights(pa_handle* h, int mode, double* w_out);   // mode 0: w, 1: min(1,tau), 2: m^4
-int pa_launch_plan(pa_handle* h);                                      // tau, r, scan, parent map
-int pa_launch_copy(pa_handle* h, int64_t R_new);
-int pa_launch_obs_sums(pa_handle* h);
+int pa_launch_measure(pa_handle* h);                                   // E, M, integer sums, m range, m^4 sum
+int pa_launch_weights(pa_handle* h, int Emin, double* w_out);          // w_j, W = TREE1024(w) -> d_scal->W
+int pa_launch_overlap(pa_handle* h, int Emin);                         // TREE1024(min(1, tau_j)) -> d_scal->sum
+int pa_launch_plan(pa_handle* h, int Emin);                            // tau, r, scan, parent map, R_new
+int pa_launch_copy(pa_handle* h);                                      // new[d] = old[parent(d)], d < R_new (read on the device)
 int pa_launch_hist(pa_handle* h, double beta);
 int pa_launch_unpack(pa_handle* h, const int64_t* d_slots, int64_t j0, int64_t n, int8_t* d_out);
 int pa_launch_pack(pa_handle* h, int64_t j0, int64_t n, const int8_t* d_in);

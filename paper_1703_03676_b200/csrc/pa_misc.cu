@@ -1,4 +1,4 @@
-// pa_misc.cu -- initial population (a0), observable sums (a8), energy histogram and multi-histogram
+// pa_misc.cu -- initial population (a0), energy histogram and multi-histogram
 // accumulation (a9), spin import/export, and the integer-pipe calibration kernels.
 #include "pa_common.cuh"
 #include <math.h>
@@ -38,40 +38,6 @@ int pa_launch_init(pa_handle* h) {
     pa_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, h->keys);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
-    return PA_OK;
-}
-
-// a8 (Eq. 3; O8): exact integer sums of E, E^2, |M|, M^2 (order-independent).
-__global__ void pa_obs_zero_kernel(PaScalars* sc) { sc->SE = sc->SE2 = sc->SA = sc->SM2 = 0; }
-
-__global__ void pa_obs_sums_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, long long R, PaScalars* sc) {
-    long long se = 0, se2 = 0, sa = 0, sm2 = 0;
-    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x) {
-        long long e = E[j], m = M[j];
-        se += e; se2 += e * e; sa += m < 0 ? -m : m; sm2 += m * m;
-    }
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) {
-        se += __shfl_xor_sync(0xffffffffu, se, off);
-        se2 += __shfl_xor_sync(0xffffffffu, se2, off);
-        sa += __shfl_xor_sync(0xffffffffu, sa, off);
-        sm2 += __shfl_xor_sync(0xffffffffu, sm2, off);
-    }
-    if ((threadIdx.x & 31) == 0) {
-        atomicAdd((unsigned long long*)&sc->SE, (unsigned long long)se);
-        atomicAdd((unsigned long long*)&sc->SE2, (unsigned long long)se2);
-        atomicAdd((unsigned long long*)&sc->SA, (unsigned long long)sa);
-        atomicAdd((unsigned long long*)&sc->SM2, (unsigned long long)sm2);
-    }
-}
-
-int pa_launch_obs_sums(pa_handle* h) {
-    pa_obs_zero_kernel<<<1, 1, 0, h->stream>>>(h->d_scal);
-    int blocks = (int)((h->R_cur + 1023) / 1024);
-    if (blocks > 592) blocks = 592;
-    pa_obs_sums_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->M, h->R_cur, h->d_scal);
-    PA_CUDA(h, cudaGetLastError());
-    h->launches += 2;
     return PA_OK;
 }
 

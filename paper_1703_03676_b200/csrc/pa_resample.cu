@@ -1,67 +1,32 @@
 // pa_resample.cu -- the resampling chain:
-//   E_min/E_max reduction, weights + TREE1024 normaliser, tau / copy numbers / decoupled look-back
-//   exclusive scan / parent map, and the bit-lane gather copy into the new population.
+//   weights + TREE1024 normaliser, tau / copy numbers / decoupled look-back exclusive scan / parent map,
+//   and the bit-lane gather copy into the new population.  Three launches per resampling step, no host
+//   round trip between them (E_min comes from the measure kernel of the previous step's observables).
 #include "pa_common.cuh"
-
-// ------------------------------------------------------------------------------------------------
-// E_min, E_max (integer min/max: order-independent, atomics are deterministic)
-// ------------------------------------------------------------------------------------------------
-__global__ void pa_minmax_kernel(const int32_t* __restrict__ E, long long R, PaScalars* sc) {
-    int lo = INT32_MAX, hi = INT32_MIN;
-    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x) {
-        int e = E[j];
-        lo = min(lo, e); hi = max(hi, e);
-    }
-#pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) {
-        lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, off));
-        hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, off));
-    }
-    if ((threadIdx.x & 31) == 0) { atomicMin(&sc->Emin, lo); atomicMax(&sc->Emax, hi); }
-}
-
-__global__ void pa_reset_scalars_kernel(PaScalars* sc) {
-    sc->Emin = INT32_MAX; sc->Emax = INT32_MIN; sc->tile_counter = 0; sc->R_new = 0;
-    sc->SE = sc->SE2 = sc->SA = sc->SM2 = 0;
-}
-
-int pa_launch_minmax(pa_handle* h) {
-    pa_reset_scalars_kernel<<<1, 1, 0, h->stream>>>(h->d_scal);
-    int blocks = (int)((h->R_cur + 1023) / 1024);
-    if (blocks > 592) blocks = 592;
-    pa_minmax_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->R_cur, h->d_scal);
-    PA_CUDA(h, cudaGetLastError());
-    h->launches += 2;
-    return PA_OK;
-}
 
 // ------------------------------------------------------------------------------------------------
 // TREE1024 (O5; L165 "sum the per-block partial results in a subsequent kernel call"): one CTA of
 // 1024 threads per aligned block of 1024 values.  __shfl_down trees give, in lane 0, exactly
 // a[i] += a[i+off] (off = 16,8,4,2,1); the 32 run sums are combined by the same tree; the block
-// sums are then added sequentially in ascending block order by pa_tree_final_kernel.
-//   mode 0: v_j = w_j = wtab[(E_j - E_min)/4]                      (also stored to w_out if given)
-//   mode 1: v_j = min(1, R_target * w_j / W)                        (Eq. 8 summand)
-//   mode 2: v_j = (M_j / N)^4                                       (Eq. 3, m^4)
+// sums are then added sequentially in ascending block order -- by the last CTA to finish (atomic
+// ticket), which replaces the paper's second kernel call and keeps the fixed order.
+//   MODE 0: v_j = w_j = wtab[(E_j - E_min)/4]  (stored to w_out if given)   -> sc->W
+//           also clears this tile's look-back state and the tile ticket for the plan kernel
+//   MODE 1: v_j = min(1, R_target * w_j / W)    (Eq. 8 summand)             -> sc->sum
 // ------------------------------------------------------------------------------------------------
 template <int MODE>
 __global__ void __launch_bounds__(PA_TILE)
-pa_tree_partials_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, const double* __restrict__ wtab,
-                        const PaScalars* __restrict__ sc, long long R, double R_target, double Nd,
-                        double* __restrict__ w_out, double* __restrict__ partials) {
+pa_tree_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* __restrict__ sc,
+               long long R, double R_target, int Emin, double* __restrict__ w_out, double* __restrict__ partials,
+               unsigned long long* __restrict__ scan_state) {
     __shared__ double run[32];
+    __shared__ bool s_last;
     const long long j = (long long)blockIdx.x * PA_TILE + threadIdx.x;
     double v = 0.0;
     if (j < R) {
-        if (MODE == 2) {
-            double m = __ddiv_rn((double)M[j], Nd);
-            double mm = __dmul_rn(m, m);
-            v = __dmul_rn(mm, mm);
-        } else {
-            double w = wtab[(E[j] - sc->Emin) >> 2];
-            if (MODE == 0) { v = w; if (w_out) w_out[j] = w; }
-            else { double tau = __ddiv_rn(__dmul_rn(R_target, w), sc->W); v = tau < 1.0 ? tau : 1.0; }
-        }
+        const double w = wtab[(E[j] - Emin) >> 2];
+        if (MODE == 0) { v = w; if (w_out) w_out[j] = w; }
+        else { const double tau = __ddiv_rn(__dmul_rn(R_target, w), sc->W); v = tau < 1.0 ? tau : 1.0; }
     }
 #pragma unroll
     for (int off = 16; off >= 1; off >>= 1) v = __dadd_rn(v, __shfl_down_sync(0xffffffffu, v, off));
@@ -71,34 +36,51 @@ pa_tree_partials_kernel(const int32_t* __restrict__ E, const int32_t* __restrict
         v = run[threadIdx.x];
 #pragma unroll
         for (int off = 16; off >= 1; off >>= 1) v = __dadd_rn(v, __shfl_down_sync(0xffffffffu, v, off));
-        if (threadIdx.x == 0) partials[blockIdx.x] = v;
+        if (threadIdx.x == 0) {
+            partials[blockIdx.x] = v;
+            if (MODE == 0) { scan_state[blockIdx.x] = 0ull; if (blockIdx.x == 0) sc->tile_counter = 0u; }
+            __threadfence();
+            s_last = atomicAdd(&sc->tree_ticket, 1u) == gridDim.x - 1;
+        }
     }
-}
-
-__global__ void pa_tree_final_kernel(const double* __restrict__ partials, int n, PaScalars* sc, int store_W) {
-    extern __shared__ double sp[];
-    for (int i = threadIdx.x; i < n; i += blockDim.x) sp[i] = partials[i];
     __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    // last CTA: block sums in ascending order, staged through shared memory 1024 at a time
+    __shared__ double stage[PA_TILE];
+    double total = 0.0;
+    const int n = gridDim.x;
+    for (int base = 0; base < n; base += PA_TILE) {
+        const int i = base + threadIdx.x;
+        stage[threadIdx.x] = i < n ? __ldcg(partials + i) : 0.0;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const int m = min(PA_TILE, n - base);
+            for (int q = 0; q < m; ++q) total = __dadd_rn(total, stage[q]);
+        }
+        __syncthreads();
+    }
     if (threadIdx.x == 0) {
-        double total = 0.0;
-        for (int i = 0; i < n; ++i) total = __dadd_rn(total, sp[i]);     // ascending block index
-        sc->sum = total;
-        if (store_W) sc->W = total;
+        if (MODE == 0) sc->W = total; else sc->sum = total;
+        sc->tree_ticket = 0u;
     }
 }
 
-int pa_launch_tree_weights(pa_handle* h, int mode, double* w_out) {
+int pa_launch_weights(pa_handle* h, int Emin, double* w_out) {
     const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
-    const double Rt = (double)h->R_target, Nd = (double)h->N;
-    if (mode == 0)
-        pa_tree_partials_kernel<0><<<n, PA_TILE, 0, h->stream>>>(h->E, h->M, h->wtab, h->d_scal, h->R_cur, Rt, Nd, w_out, h->partials);
-    else if (mode == 1)
-        pa_tree_partials_kernel<1><<<n, PA_TILE, 0, h->stream>>>(h->E, h->M, h->wtab, h->d_scal, h->R_cur, Rt, Nd, nullptr, h->partials);
-    else
-        pa_tree_partials_kernel<2><<<n, PA_TILE, 0, h->stream>>>(h->E, h->M, h->wtab, h->d_scal, h->R_cur, Rt, Nd, nullptr, h->partials);
-    pa_tree_final_kernel<<<1, 256, n * sizeof(double), h->stream>>>(h->partials, n, h->d_scal, mode == 0 ? 1 : 0);
+    pa_tree_kernel<0><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, Emin, w_out,
+                                                    h->partials, h->scan_state);
     PA_CUDA(h, cudaGetLastError());
-    h->launches += 2;
+    h->launches += 1;
+    return PA_OK;
+}
+
+int pa_launch_overlap(pa_handle* h, int Emin) {
+    const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
+    pa_tree_kernel<1><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, Emin, nullptr,
+                                                    h->partials, h->scan_state);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
     return PA_OK;
 }
 
@@ -113,7 +95,7 @@ int pa_launch_tree_weights(pa_handle* h, int mode, double* w_out) {
 
 __global__ void __launch_bounds__(256)
 pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* sc,
-               long long R, double R_target, PhiloxKeys K, uint32_t kcount, long long R_cap,
+               long long R, double R_target, int Emin, PhiloxKeys K, uint32_t kcount, long long R_cap,
                uint32_t* __restrict__ r_out, uint32_t* __restrict__ o_out, uint32_t* __restrict__ parent,
                unsigned long long* __restrict__ state, int n_tiles) {
     __shared__ uint32_t s_tile, s_warp[8], s_excl;
@@ -126,7 +108,6 @@ pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
     uint32_t r[4] = {0, 0, 0, 0};
     if (j0 < R) {
         const double W = sc->W;
-        const int Emin = sc->Emin;
         // x(j,k) = philox(j>>2, 0, k, TAG_RESAMPLE)[j&3]   (O1)
         uint4 x = pa_philox((uint32_t)(j0 >> 2), 0u, kcount, PA_TAG_RESAMPLE, K);
         const uint32_t xs[4] = {x.x, x.y, x.z, x.w};
@@ -208,10 +189,9 @@ pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
     }
 }
 
-int pa_launch_plan(pa_handle* h) {
+int pa_launch_plan(pa_handle* h, int Emin) {
     const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
-    PA_CUDA(h, cudaMemsetAsync(h->scan_state, 0, sizeof(unsigned long long) * n, h->stream));
-    pa_plan_kernel<<<n, 256, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, h->keys, h->k,
+    pa_plan_kernel<<<n, 256, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, Emin, h->keys, h->k,
                                              h->R_cap, h->r, h->o, h->parent, h->scan_state, n);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
@@ -228,11 +208,16 @@ struct __align__(16) PaSeg { uint32_t src_group, rot, mask, pad; };
 
 __global__ void __launch_bounds__(128)
 pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, const uint32_t* __restrict__ parent,
-               long long R_new, int N) {
+               const PaScalars* __restrict__ sc, long long R_cap, int N) {
     __shared__ PaSeg segs[32];
     __shared__ int nseg;
     const long long g = blockIdx.x;
     const int tid = threadIdx.x;
+    // R_new is read on the device: the launch does not wait for the host to see it, the grid covers the
+    // capacity and groups past the new population exit.  R_new > R_cap is the PA_ERR_CAPACITY case: nothing
+    // of the live population is touched (dst is the spare buffer) and the host discards the copy.
+    const long long R_new = min((long long)sc->R_new, R_cap);
+    if (g * 32 >= R_new) return;
     if (tid < 32) {
         const long long d = g * 32 + tid;
         const bool valid = d < R_new;
@@ -281,14 +266,14 @@ pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, con
     }
 }
 
-int pa_launch_copy(pa_handle* h, int64_t R_new) {
-    const int64_t G = (R_new + 31) / 32;
+int pa_launch_copy(pa_handle* h) {
+    const int64_t G = h->G_cap;
     const int chunks = h->N / 4;
     int gy = 1;
     // small populations: split a group's words over several CTAs to fill the GPU
     while (G * gy < 592 && gy * 128 * 2 <= chunks) gy *= 2;
     dim3 grid((unsigned)G, (unsigned)gy, 1);
-    pa_copy_kernel<<<grid, 128, 0, h->stream>>>(h->spins[h->cur], h->spins[1 - h->cur], h->parent, R_new, h->N);
+    pa_copy_kernel<<<grid, 128, 0, h->stream>>>(h->spins[h->cur], h->spins[1 - h->cur], h->parent, h->d_scal, h->R_cap, h->N);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;

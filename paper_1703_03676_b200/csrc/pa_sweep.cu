@@ -12,6 +12,7 @@
 // see DESIGN.md Sec. 6 for the instruction budget.
 #include "pa_common.cuh"
 #include <cooperative_groups.h>
+#include <math.h>
 #include <stdlib.h>
 namespace cg = cooperative_groups;
 
@@ -232,11 +233,11 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 // word, 8 % of the kernel) disappears.  The ALU pipe is the binding one.
 // Requirements (checked by pa_sweep_configure): Lh = 2^LOG_LH >= 32, T >= Lh, H*Lh/T even and >= 2, H even.
 // ------------------------------------------------------------------------------------------------
-#ifndef PA_SWEEP_MINB
-#define PA_SWEEP_MINB 1
+#ifndef PA_SWEEP_BOUNDS
+#define PA_SWEEP_BOUNDS __launch_bounds__(256)
 #endif
 template <int CMP, int LOG_LH, bool CLUSTER>
-__global__ void __launch_bounds__(256, PA_SWEEP_MINB)
+__global__ void PA_SWEEP_BOUNDS
 pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
     constexpr int Lh = 1 << LOG_LH;
@@ -319,34 +320,62 @@ static int pa_env_int(const char* name, int dflt) {
     return v ? atoi(v) : dflt;
 }
 
-// Launch geometry: the smallest cluster size C in {1,2,4,8} dividing L whose strip (L/C rows of both
+// Launch geometry.  C_min = the smallest cluster size in {1,2,4,8} dividing L whose strip (L/C rows of both
 // colours, L*L*4/C bytes) fits the shared-memory budget per CTA; threads = min(256, words per colour).
 // kind 1 = column-walk kernel (power-of-two L >= 64), kind 0 = generic kernel (any even L).
+// Environment overrides (tests, tuning): PA_SWEEP_C, PA_SWEEP_T, PA_SWEEP_KIND, PA_SWEEP_CMP, PA_SWEEP_SMEM_KB.
+static bool pa_col_ok(int L, int C, int T) {
+    if ((L & (L - 1)) != 0 || L < 64 || L % C != 0) return false;
+    const int Lh = L / 2, H = L / C, half = H * Lh;
+    return (H & 1) == 0 && T >= Lh && (T & (T - 1)) == 0 && half % T == 0 && half / T >= 2 && ((half / T) & 1) == 0;
+}
+
 int pa_sweep_configure(pa_handle* h) {
     const int L = h->L;
     const size_t budget = (size_t)pa_env_int("PA_SWEEP_SMEM_KB", 64) * 1024;
     int C = 1;
     while (C <= 8 && (((L % C) != 0) || (size_t)L * L * 4 / C > budget)) C *= 2;
+    h->sweep_C_forced = false;
     int forceC = pa_env_int("PA_SWEEP_C", 0);
-    if (forceC > 0 && L % forceC == 0) C = forceC;
+    if (forceC > 0 && L % forceC == 0) { C = forceC; h->sweep_C_forced = true; }
     if (C > 8 || (size_t)L * L * 4 / C > 224 * 1024) return PA_ERR_INVALID_ARG;
     int half = (L / C) * (L / 2);
     int T = 256;
     while (T > 32 && T > half) T >>= 1;
     int forceT = pa_env_int("PA_SWEEP_T", 0);
     if (forceT >= 32 && forceT <= 256) T = forceT;
-    int kind = ((L & (L - 1)) == 0 && L >= 64) ? 1 : 0;
+    int kind = pa_col_ok(L, C, T) ? 1 : 0;
     kind = pa_env_int("PA_SWEEP_KIND", kind);
-    if (kind == 1) {
-        const int Lh = L / 2, H = L / C;
-        const bool ok = (L & (L - 1)) == 0 && L >= 64 && (H & 1) == 0 && T >= Lh && (T & (T - 1)) == 0 &&
-                        half % T == 0 && half / T >= 2 && ((half / T) & 1) == 0;
-        if (!ok) kind = 0;
-    }
+    if (kind == 1 && !pa_col_ok(L, C, T)) kind = 0;
     h->sweep_C = C; h->sweep_T = T; h->sweep_kind = kind;
     h->sweep_cmp = pa_env_int("PA_SWEEP_CMP", 1);
     if (h->sweep_cmp < 0 || h->sweep_cmp > 2) h->sweep_cmp = 1;
     return PA_OK;
+}
+
+// Small populations: one CTA per group leaves a ragged last wave (cfg2: 625 groups on 444 CTA slots = 1.4
+// waves).  Splitting every group over a cluster of 2 or 4 CTAs makes the work items smaller.  Estimated
+// efficiency of C = (waves / ceil(waves)) x measured cluster cost (C=2: 0.97; C=4 also strands 16 of the 148
+// SMs); only applied below 4 waves, where the wave model is accurate (measured).
+static int pa_sweep_pick_C(const pa_handle* h, int64_t G) {
+    const int Cmin = h->sweep_C;
+    if (h->sweep_C_forced || h->sweep_kind != 1) return Cmin;
+    const int L = h->L;
+    double best = -1.0; int bestC = Cmin;
+    for (int C = Cmin; C <= 8; C *= 2) {
+        if (!pa_col_ok(L, C, h->sweep_T)) break;
+        const size_t smem = (size_t)L * L * 4 / C;
+        int per_sm = (int)((227 * 1024) / (smem + 1024));
+        if (per_sm > 3) per_sm = 3;                        // 80 registers x 256 threads
+        if (per_sm < 1) per_sm = 1;
+        const double slots = (C >= 4 ? 132.0 : 148.0) * per_sm;
+        const double waves = (double)G * C / slots;
+        if (C == Cmin && waves >= 4.0) return Cmin;
+        const double cost = C == 1 ? 1.0 : C == 2 ? 0.97 : C == 4 ? 0.93 : 0.85;
+        const double eff = waves / ceil(waves) * cost;
+        if (eff > best) { best = eff; bestC = C; }
+    }
+    return bestC;
 }
 
 template <typename Kern>
@@ -390,9 +419,9 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     P.K = h->keys;
     P.T4 = T4; P.T8 = T8;
     P.t0 = h->t; P.theta = theta; P.two = 2u;
-    P.L = h->L; P.Lh = h->L / 2; P.C = h->sweep_C; P.H = h->L / h->sweep_C; P.N = h->N;
-    const size_t smem = (size_t)P.H * h->L * 4;
     const int64_t G = (h->R_cur + 31) / 32;
+    P.L = h->L; P.Lh = h->L / 2; P.C = pa_sweep_pick_C(h, G); P.H = h->L / P.C; P.N = h->N;
+    const size_t smem = (size_t)P.H * h->L * 4;
     const unsigned grid = (unsigned)(G * P.C);
     const int v = h->sweep_cmp;
     const cudaError_t e = v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)
