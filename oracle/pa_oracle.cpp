@@ -234,6 +234,60 @@ double overlap_for(const std::vector<int32_t>& E, int64_t R_target, double dbeta
     return tree1024(a.data(), R) / (double)R;
 }
 
+// O10, L118 "for instance, bisection": hi = beta_max - beta; if alpha(hi) >= target return hi;
+// lo = 0; 40 times: mid = (lo+hi)/2; alpha(mid) >= target ? lo = mid : hi = mid; return lo.
+double adapt_for(const std::vector<int32_t>& E, int64_t R_target, double target, double hi) {
+    if (overlap_for(E, R_target, hi) >= target) return hi;
+    double lo = 0.0;
+    for (int it = 0; it < 40; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (overlap_for(E, R_target, mid) >= target) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+struct obs_values { double e, C, absm, m2, m4, betaF_per_N, S_per_N; };
+
+// step 4, L62; Eq. 3, Eq. 4, Eq. 5 L95 from the vectors E_j, M_j and lnZ = -beta F.
+obs_values observables_for(const std::vector<int32_t>& E, const std::vector<int32_t>& M, int64_t N,
+                           double beta, double lnZ) {
+    int64_t R = (int64_t)E.size();
+    int64_t SE = 0, SE2 = 0, SA = 0, SM2 = 0;
+    std::vector<double> q(R);
+    for (int64_t j = 0; j < R; ++j) {
+        SE += E[j]; SE2 += (int64_t)E[j] * E[j];
+        SA += M[j] < 0 ? -(int64_t)M[j] : (int64_t)M[j];
+        SM2 += (int64_t)M[j] * M[j];
+        double m = (double)M[j] / (double)N, mm = m * m;
+        q[j] = mm * mm;
+    }
+    double SM4 = tree1024(q.data(), R);
+    __int128 num = (__int128)R * (__int128)SE2 - (__int128)SE * (__int128)SE;   // exact
+    obs_values v;
+    v.e = (double)SE / ((double)R * (double)N);
+    v.C = beta * beta * ((double)num / ((double)R * (double)R * (double)N));
+    v.absm = (double)SA / ((double)R * (double)N);
+    v.m2 = (double)SM2 / ((double)R * (double)N * (double)N);
+    v.m4 = SM4 / (double)R;
+    v.betaF_per_N = -lnZ / (double)N;
+    v.S_per_N = beta * v.e + lnZ / (double)N;
+    return v;
+}
+
+// O9, Eq. 9 L124-L129: fold the energy histogram at beta into the running sums.
+void hist_fold_for(const std::vector<int32_t>& E, int N, double lnZ, double beta, int64_t* Hsum, double* lnD) {
+    int64_t R = (int64_t)E.size();
+    std::vector<int64_t> H(N + 1, 0);
+    for (int64_t j = 0; j < R; ++j) H[(E[j] + 2 * N) / 4] += 1;
+    double lnR = std::log((double)R);
+    for (int m = 0; m <= N; ++m) {
+        Hsum[m] += H[m];
+        double Em = (double)(-2 * N + 4 * m);
+        // R_i exp[beta_i F(beta_i) - beta_i E], with -beta_i F = lnZ (Eq. 4)
+        lnD[m] = logaddexp(lnD[m], lnR - lnZ - beta * Em);
+    }
+}
+
 }  // namespace
 
 extern "C" {
@@ -312,6 +366,27 @@ double ora_overlap_of(int64_t R_target, int64_t R_cur, const int32_t* E, double 
     return overlap_for(Ev, R_target, dbeta);
 }
 
+// O10 from an energy vector alone (sampled parity checks at the large configs)
+int ora_adapt_dbeta_of(int64_t R_target, int64_t R_cur, const int32_t* E, double target, double beta,
+                       double beta_max, double* dbeta_out) {
+    if (R_cur < 1 || !dbeta_out || !(target > 0.0 && target < 1.0) || !(beta_max > beta)) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> Ev(E, E + R_cur);
+    *dbeta_out = adapt_for(Ev, R_target, target, beta_max - beta);
+    return ORA_OK;
+}
+
+// O8 from the vectors E_j, M_j; lnZ and lnQ are the caller's running values (Eq. 4)
+int ora_observables_of(int L, int64_t R_cur, const int32_t* E, const int32_t* M, double beta, double lnZ,
+                       double lnQ, ora_obs_t* out);
+
+// O9 from an energy vector: Hsum[N+1], lnD[N+1] are updated in place
+int ora_hist_fold_of(int L, int64_t R_cur, const int32_t* E, double lnZ, double beta, int64_t* Hsum, double* lnD) {
+    if (L < 4 || (L & 1) || R_cur < 1 || !Hsum || !lnD) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> Ev(E, E + R_cur);
+    hist_fold_for(Ev, L * L, lnZ, beta, Hsum, lnD);
+    return ORA_OK;
+}
+
 // ---- the population handle (the same calls as include/pa.h, prefixed ora_) -------------------
 
 int ora_create(int L, int64_t R, uint64_t seed, Oracle** out) {
@@ -381,19 +456,10 @@ int ora_resample(Oracle* o, double beta, double beta_new, int64_t* R_new_out) {
     return ORA_OK;
 }
 
-// O10, L118 "for instance, bisection": hi = beta_max - beta; if alpha(hi) >= target return hi;
-// lo = 0; 40 times: mid = (lo+hi)/2; alpha(mid) >= target ? lo = mid : hi = mid; return lo.
 int ora_adapt_dbeta(Oracle* o, double target, double beta, double beta_max, double* dbeta_out) {
     if (!o || !dbeta_out || !(target > 0.0 && target < 1.0) || !(beta_max > beta)) return ORA_ERR_INVALID_ARG;
     std::vector<int32_t> E, M; all_energies(o, E, M);
-    double hi = beta_max - beta;
-    if (overlap_for(E, o->R_target, hi) >= target) { *dbeta_out = hi; return ORA_OK; }
-    double lo = 0.0;
-    for (int it = 0; it < 40; ++it) {
-        double mid = 0.5 * (lo + hi);
-        if (overlap_for(E, o->R_target, mid) >= target) lo = mid; else hi = mid;
-    }
-    *dbeta_out = lo;
+    *dbeta_out = adapt_for(E, o->R_target, target, beta_max - beta);
     return ORA_OK;
 }
 
@@ -404,49 +470,31 @@ int ora_overlap(Oracle* o, double dbeta, double* alpha) {
     return ORA_OK;
 }
 
-// step 4, L62; Eq. 3, Eq. 4, Eq. 5; output fields of L179-L181.
-int ora_observables(Oracle* o, double beta, ora_obs_t* out) {
-    if (!o || !out) return ORA_ERR_INVALID_ARG;
-    std::vector<int32_t> E, M; all_energies(o, E, M);
-    int64_t R = o->R_cur, N = o->N;
-    int64_t SE = 0, SE2 = 0, SA = 0, SM2 = 0;
-    std::vector<double> q(R);
-    for (int64_t j = 0; j < R; ++j) {
-        SE += E[j]; SE2 += (int64_t)E[j] * E[j];
-        SA += M[j] < 0 ? -(int64_t)M[j] : (int64_t)M[j];
-        SM2 += (int64_t)M[j] * M[j];
-        double m = (double)M[j] / (double)N, mm = m * m;
-        q[j] = mm * mm;
-    }
-    double SM4 = tree1024(q.data(), R);
-    __int128 num = (__int128)R * (__int128)SE2 - (__int128)SE * (__int128)SE;   // exact
-    out->beta = beta;
-    out->e = (double)SE / ((double)R * (double)N);
-    out->C = beta * beta * ((double)num / ((double)R * (double)R * (double)N));
-    out->absm = (double)SA / ((double)R * (double)N);
-    out->m2 = (double)SM2 / ((double)R * (double)N * (double)N);
-    out->m4 = SM4 / (double)R;
-    out->betaF_per_N = -o->lnZ / (double)N;
-    out->S_per_N = beta * out->e + o->lnZ / (double)N;
-    out->lnQ = o->lnQ_last;
-    out->R = R;
+// output fields of L179-L181
+static void fill_obs(ora_obs_t* out, const obs_values& v, double beta, double lnQ, int64_t R) {
+    out->beta = beta; out->e = v.e; out->C = v.C; out->absm = v.absm; out->m2 = v.m2; out->m4 = v.m4;
+    out->betaF_per_N = v.betaF_per_N; out->S_per_N = v.S_per_N; out->lnQ = lnQ; out->R = R;
+}
+
+int ora_observables_of(int L, int64_t R_cur, const int32_t* E, const int32_t* M, double beta, double lnZ,
+                       double lnQ, ora_obs_t* out) {
+    if (L < 4 || (L & 1) || R_cur < 1 || !out) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> Ev(E, E + R_cur), Mv(M, M + R_cur);
+    fill_obs(out, observables_for(Ev, Mv, (int64_t)L * L, beta, lnZ), beta, lnQ, R_cur);
     return ORA_OK;
 }
 
-// O9, Eq. 9 L124-L129: fold the energy histogram at beta into the running sums.
+int ora_observables(Oracle* o, double beta, ora_obs_t* out) {
+    if (!o || !out) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> E, M; all_energies(o, E, M);
+    fill_obs(out, observables_for(E, M, o->N, beta, o->lnZ), beta, o->lnQ_last, o->R_cur);
+    return ORA_OK;
+}
+
 int ora_hist_accumulate(Oracle* o, double beta) {
     if (!o) return ORA_ERR_INVALID_ARG;
     std::vector<int32_t> E, M; all_energies(o, E, M);
-    int N = o->N;
-    std::vector<int64_t> H(N + 1, 0);
-    for (int64_t j = 0; j < o->R_cur; ++j) H[(E[j] + 2 * N) / 4] += 1;
-    double lnR = std::log((double)o->R_cur);
-    for (int m = 0; m <= N; ++m) {
-        o->Hsum[m] += H[m];
-        double Em = (double)(-2 * N + 4 * m);
-        // R_i exp[beta_i F(beta_i) - beta_i E], with -beta_i F = lnZ (Eq. 4)
-        o->lnD[m] = logaddexp(o->lnD[m], lnR - o->lnZ - beta * Em);
-    }
+    hist_fold_for(E, o->N, o->lnZ, beta, o->Hsum.data(), o->lnD.data());
     return ORA_OK;
 }
 

@@ -37,6 +37,9 @@ def lib():
         L.ora_resample_plan.argtypes = [i64, i64, vp, u64, u32, dbl, vp, vp, vp, vp, vp, vp]
         L.ora_resample_plan.restype = i32
         L.ora_overlap_of.argtypes = [i64, i64, vp, dbl]; L.ora_overlap_of.restype = dbl
+        L.ora_adapt_dbeta_of.argtypes = [i64, i64, vp, dbl, dbl, dbl, vp]; L.ora_adapt_dbeta_of.restype = i32
+        L.ora_observables_of.argtypes = [i32, i64, vp, vp, dbl, dbl, dbl, vp]; L.ora_observables_of.restype = i32
+        L.ora_hist_fold_of.argtypes = [i32, i64, vp, dbl, dbl, vp, vp]; L.ora_hist_fold_of.restype = i32
         L.ora_create.argtypes = [i32, i64, u64, vp]; L.ora_create.restype = i32
         L.ora_destroy.argtypes = [vp]; L.ora_destroy.restype = None
         L.ora_population.argtypes = [vp]; L.ora_population.restype = i64
@@ -126,6 +129,29 @@ def resample_plan(R_target, E, seed, k, dbeta):
 def overlap_of(R_target, E, dbeta):
     E = np.ascontiguousarray(E, dtype=np.int32)
     return float(lib().ora_overlap_of(R_target, E.size, _p(E), float(dbeta)))
+
+
+def adapt_dbeta_of(R_target, E, target, beta, beta_max):
+    E = np.ascontiguousarray(E, dtype=np.int32)
+    d = C.c_double()
+    _check(lib().ora_adapt_dbeta_of(R_target, E.size, _p(E), float(target), float(beta), float(beta_max), C.byref(d)),
+           "adapt_dbeta_of")
+    return d.value
+
+
+def observables_of(L, E, M, beta, lnZ, lnQ):
+    E = np.ascontiguousarray(E, dtype=np.int32); M = np.ascontiguousarray(M, dtype=np.int32)
+    o = Obs()
+    _check(lib().ora_observables_of(L, E.size, _p(E), _p(M), float(beta), float(lnZ), float(lnQ), C.byref(o)),
+           "observables_of")
+    return o.as_dict()
+
+
+def hist_fold_of(L, E, lnZ, beta, Hsum, lnD):
+    """Fold the energy histogram of E at beta into Hsum (int64[N+1]) and lnD (float64[N+1]), in place."""
+    E = np.ascontiguousarray(E, dtype=np.int32)
+    assert Hsum.dtype == np.int64 and lnD.dtype == np.float64 and Hsum.size == L * L + 1 == lnD.size
+    _check(lib().ora_hist_fold_of(L, E.size, _p(E), float(lnZ), float(beta), _p(Hsum), _p(lnD)), "hist_fold_of")
 
 
 def num_threads():
