@@ -1,0 +1,206 @@
+"""GPU parity at BASELINE.json's full sizes (configs 3, 4, 5), in the launch configuration bench.py times.
+
+The oracle cannot hold these populations (cfg5: 65.5 GB of uint8 spins, ~3e6 core-seconds), so each checked
+temperature step follows the chained spot-check protocol of SURVEY.md Sec. 8(c) / DESIGN.md Sec. 7:
+
+  (i)   the FULL energy / magnetisation vectors come back from the device (4 bytes per replica); on a random
+        sample of slots the oracle recomputes E_j, M_j from the exported spins (O4);
+  (ii)  from the full E vector the oracle recomputes W, w_j, r_j, o_j, R_new, ln Q (O5-O7): bit-exact;
+  (iii) the copy is checked on a sample of destination slots: new[d] == old[parent(d)], parent from the oracle's plan;
+  (iv)  the sampled slots are swept by the oracle (same slot ids, sweep counter, thresholds) and compared bit-exactly (O3);
+  (v)   observables / adaptive step / histogram fold are recomputed by the oracle from the full E, M vectors (O8-O10).
+
+Steps that are not checked run on the device alone; every checked step starts from device state, so a divergence
+anywhere upstream shows as an (i) or (iv) mismatch only if it breaks the algorithm, which is what parity means here.
+PA_FULLSIZE_STEPS=all runs every step of a config's schedule (minutes on a B200)."""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():
+    pytest.skip("no CUDA device", allow_module_level=True)
+
+from oracle import pa_oracle as po                      # noqa: E402
+from paper_1703_03676_b200 import pa                    # noqa: E402
+from paper_1703_03676_b200.workloads import CONFIGS     # noqa: E402
+
+REL = 1e-9
+OBS_KEYS = ("beta", "e", "C", "absm", "m2", "m4", "betaF_per_N", "S_per_N", "lnQ")
+RUN_ALL = os.environ.get("PA_FULLSIZE_STEPS", "") == "all"
+
+
+def _sample(rng, n_total, n, always=()):
+    """n distinct slots in [0, n_total): random, plus the edges (first, last, last full group boundary)."""
+    fixed = [s for s in always if 0 <= s < n_total]
+    pick = rng.choice(n_total, size=min(n, n_total), replace=False).tolist()
+    return np.array(sorted(set(fixed + pick)), dtype=np.int64)
+
+
+def _bits(spins_pm1):
+    return np.ascontiguousarray((spins_pm1 > 0).astype(np.uint8))
+
+
+def checked_step(g, wl, beta_prev, beta, rng, n_slots, lnZ_ref, hist=None):
+    """One temperature step on the device with checks (i)-(v).  Returns (observables, lnZ after the step)."""
+    L, N = wl.L, wl.N
+    R_prev = g.population
+    E, M = g.energies()
+    k = g.resample_counter
+    plan = po.resample_plan(wl.R, E, wl.seed, k, beta - beta_prev)                       # (ii) oracle side
+    R_new = plan["R_new"]
+    parent = np.repeat(np.arange(R_prev, dtype=np.int64), plan["r"])
+    assert parent.size == R_new
+    d = _sample(rng, R_new, n_slots, always=(0, 1, 31, 32, R_new - 1, (R_new // 32) * 32 - 1, (R_new // 32) * 32))
+    pre = g.get_spins_at(parent[d])
+    Eo, Mo = po.energies_of(L, _bits(pre))                                                # (i)
+    assert np.array_equal(Eo, E[parent[d]]) and np.array_equal(Mo, M[parent[d]])
+
+    assert g.resample(beta_prev, beta) == R_new                                           # (ii) device side
+    dbg = g.resample_debug(R_prev)
+    assert dbg["W"] == plan["W"]
+    assert np.array_equal(dbg["w"], plan["w"])
+    assert np.array_equal(dbg["r"], plan["r"])
+    assert np.array_equal(dbg["o"], plan["o"])
+    lnZ = lnZ_ref + plan["lnQ"]
+    assert g.lnZ == pytest.approx(lnZ, rel=1e-13)
+
+    post = g.get_spins_at(d)                                                              # (iii)
+    assert np.array_equal(post, pre)
+
+    t0 = g.sweep_counter                                                                  # (iv)
+    g.sweep(beta, wl.theta)
+    assert g.sweep_counter == t0 + wl.theta
+    want = po.sweep_slots(L, wl.seed, t0, beta, wl.theta, d, _bits(post))
+    got = g.get_spins_at(d)
+    assert np.array_equal(_bits(got), want)
+
+    E2, M2 = g.energies()                                                                 # (v)
+    Eo, Mo = po.energies_of(L, want)
+    assert np.array_equal(Eo, E2[d]) and np.array_equal(Mo, M2[d])
+    og = g.observables(beta)
+    oo = po.observables_of(L, E2, M2, beta, lnZ, plan["lnQ"])
+    assert og["R"] == oo["R"] == R_new
+    for key in OBS_KEYS:
+        assert og[key] == pytest.approx(oo[key], rel=REL, abs=1e-300), (key, og[key], oo[key])
+    if hist is not None:
+        g.hist_accumulate(beta)
+        po.hist_fold_of(L, E2, lnZ, beta, hist[0], hist[1])
+    return og, lnZ
+
+
+def plain_step(g, wl, beta_prev, beta, lnZ_ref, hist=None):
+    """One temperature step on the device alone; the oracle only tracks ln Z and the histogram sums from the E vector."""
+    E, _ = g.energies()
+    plan = po.resample_plan(wl.R, E, wl.seed, g.resample_counter, beta - beta_prev)
+    assert g.resample(beta_prev, beta) == plan["R_new"]
+    g.sweep(beta, wl.theta)
+    og = g.observables(beta)
+    lnZ = lnZ_ref + plan["lnQ"]
+    if hist is not None:
+        E2, _ = g.energies()
+        g.hist_accumulate(beta)
+        po.hist_fold_of(wl.L, E2, lnZ, beta, hist[0], hist[1])
+    return og, lnZ
+
+
+def _check_initial(g, wl, rng, n_slots):
+    """a0 at full size: sampled slots against the oracle's INIT stream (an Oracle of the sampled prefix is the
+    same stream because INIT is keyed by (site, slot)), closed forms at beta = 0 on the full vectors."""
+    R, N = wl.R, wl.N
+    assert g.population == R and g.capacity == po.capacity(R)
+    n = min(R, 2048)
+    small = po.Oracle(wl.L, n, wl.seed)
+    if n % 32 == 0 or n == R:
+        assert np.array_equal(g.get_spins(0, n), small.get_spins())
+    E, M = g.energies()
+    d = _sample(rng, R, n_slots, always=(0, R - 1))
+    Eo, Mo = po.energies_of(wl.L, _bits(g.get_spins_at(d)))
+    assert np.array_equal(Eo, E[d]) and np.array_equal(Mo, M[d])
+    # closed forms for i.i.d. spins: <E> = 0, Var E = 2N, <M^2> = N; 5 sigma of the sample mean
+    assert abs(E.mean()) < 5.0 * np.sqrt(2.0 * N / R)
+    assert abs(E.astype(np.float64).var() / (2.0 * N) - 1.0) < 5.0 * np.sqrt(2.0 / R)
+    assert abs((M.astype(np.float64) ** 2).mean() / N - 1.0) < 5.0 * np.sqrt(2.0 / R)
+    assert np.all((E + 2 * N) % 4 == 0)
+
+
+def _run_fixed_schedule(cfg, checked, n_slots, last_step):
+    wl = CONFIGS[cfg]
+    rng = np.random.default_rng(1000 + cfg)
+    g = pa.Population(wl.L, wl.R, wl.seed)
+    _check_initial(g, wl, rng, n_slots)
+    betas = wl.betas()
+    lnZ = wl.N * np.log(2.0)
+    assert g.lnZ == pytest.approx(lnZ, rel=1e-15)
+    last = len(betas) - 1 if RUN_ALL else last_step
+    for i in range(1, last + 1):
+        if i in checked:
+            og, lnZ = checked_step(g, wl, betas[i - 1], betas[i], rng, n_slots, lnZ)
+        else:
+            og, lnZ = plain_step(g, wl, betas[i - 1], betas[i], lnZ)
+        # population size stays close to R: every r_j is a Bernoulli rounding, sd <= sqrt(R)/2 per step
+        assert abs(og["R"] - wl.R) < 8.0 * np.sqrt(wl.R)
+    g.close()
+    return og
+
+
+def test_config3_full_size_sampled():
+    """BASELINE.json configs[2]: L=64, R=131072 bit-packed, 200 equal steps to beta=1, theta=10, seed 3.
+    The whole schedule runs on the device (0.7 s); steps 1, 2, 88 (beta = 0.44, next to beta_c), 150 and 200 are checked."""
+    og = _run_fixed_schedule(3, checked={1, 2, 88, 150, 200}, n_slots=1024, last_step=200)
+    assert og["beta"] == 1.0 and og["absm"] > 0.99              # ordered phase at beta = 1
+
+
+def test_config5_full_size_sampled():
+    """BASELINE.json configs[4]: L=256, R=10^6 (8.2 GB of packed spins, twice for the copy buffer), 500 steps of 0.001.
+    Default: the first 12 steps (5 s of device time), steps 1, 2 and 12 checked on 256 sampled slots each (the oracle sweeps
+    256 x 65536 x 10 spins per checked step).  PA_FULLSIZE_STEPS=all runs all 500 steps with checks around beta_c too."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 20 * 2**30:
+        pytest.skip("needs 17 GB of device memory")
+    checked = {1, 2, 12} | ({438, 441, 444, 499, 500} if RUN_ALL else set())
+    _run_fixed_schedule(5, checked=checked, n_slots=256, last_step=12)
+
+
+def test_config4_full_size_adaptive_multihistogram():
+    """BASELINE.json configs[3]: L=128, R=100000, adaptive steps at overlap 0.85, multi-histogram over all beta, seed 4.
+    Every step's adaptive dbeta is recomputed by the oracle from the device's full E vector (41 overlap evaluations,
+    O10) and must agree bit for bit; sampled-slot checks at steps 1, 2, 3, 20 and the last one run."""
+    wl = CONFIGS[4]
+    rng = np.random.default_rng(1004)
+    g = pa.Population(wl.L, wl.R, wl.seed)
+    _check_initial(g, wl, rng, 512)
+    N = wl.N
+    hist = (np.zeros(N + 1, dtype=np.int64), np.full(N + 1, -np.inf))
+    lnZ = N * np.log(2.0)
+    beta = wl.beta0
+    E, _ = g.energies()
+    g.observables(beta); g.hist_accumulate(beta)
+    po.hist_fold_of(wl.L, E, lnZ, beta, hist[0], hist[1])
+    n_steps = 100000 if RUN_ALL else 24
+    checked = {1, 2, 3, 20, n_steps}
+    i = 0
+    while beta < wl.beta_f and i < n_steps:
+        i += 1
+        E, _ = g.energies()
+        d_g = g.adapt_dbeta(wl.target_overlap, beta, wl.beta_f)
+        d_o = po.adapt_dbeta_of(wl.R, E, wl.target_overlap, beta, wl.beta_f)
+        assert d_g == d_o, (i, d_g, d_o)
+        assert 0.0 < d_g <= wl.beta_f - beta
+        assert g.overlap(d_g) == po.overlap_of(wl.R, E, d_g) >= wl.target_overlap
+        new = wl.beta_f if beta + d_g >= wl.beta_f else beta + d_g
+        if i in checked or new == wl.beta_f:
+            og, lnZ = checked_step(g, wl, beta, new, rng, 512, lnZ, hist)
+        else:
+            og, lnZ = plain_step(g, wl, beta, new, lnZ, hist)
+        beta = new
+    assert i >= 20
+    Hg, Dg = g.histogram()
+    assert np.array_equal(Hg, hist[0])                             # integer counts: bit-exact
+    fin = np.isfinite(hist[1])
+    assert np.array_equal(np.isfinite(Dg), fin)
+    assert np.allclose(Dg[fin], hist[1][fin], rtol=REL, atol=0)
+    g.close()
