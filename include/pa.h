@@ -146,9 +146,13 @@ int64_t pa_launch_count(const pa_t* h);
 /* Device time in milliseconds of the last pa_sweep / the last pa_resample on this handle,
  * measured with CUDA events on the handle's stream; the kernel that dominates each is the
  * sweep kernel / the replica-copy kernel (time of that kernel alone in *kernel_ms).
- * Synchronises.  Either pointer may be NULL. */
+ * pa_last_measure_ms: the last launch of the energy / magnetisation / observable-sums kernel (row a3 + a8),
+ * which runs inside the first of pa_energies / pa_observables / pa_resample / pa_adapt_dbeta /
+ * pa_hist_accumulate that follows a change of the population.
+ * Synchronises.  Either pointer may be NULL.  PA_ERR_INVALID_ARG if no such operation has run yet. */
 int pa_last_sweep_ms(pa_t* h, float* kernel_ms);
 int pa_last_resample_ms(pa_t* h, float* total_ms, float* copy_kernel_ms);
+int pa_last_measure_ms(pa_t* h, float* kernel_ms);
 
 /* Integer-pipe calibration for the roofline denominator: runs a dependent
  * chain of `kind` = 0: LOP3, 1: IMAD.WIDE.U32, 2: the Philox round's mix (2 IMAD.WIDE + 2 LOP3),

@@ -165,7 +165,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     // pinned host mirrors
     if (cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
         cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->N + 1)) != cudaSuccess) { rc = PA_ERR_CUDA; }
-    for (int i = 0; i < 7 && rc == PA_OK; ++i)
+    for (int i = 0; i < 9 && rc == PA_OK; ++i)
         if (cudaEventCreate(&h->ev[i]) != cudaSuccess) rc = PA_ERR_CUDA;
     if (rc == PA_OK) rc = pa_sweep_configure(h);
     if (rc == PA_OK) {
@@ -188,7 +188,7 @@ int pa_create(int L, int64_t R, uint64_t seed, pa_t** out) { return pa_create_ex
 void pa_destroy(pa_t* h) {
     if (!h) return;
     cudaStreamSynchronize(h->stream);
-    for (int i = 0; i < 7; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    for (int i = 0; i < 9; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->h_wtab) cudaFreeHost(h->h_wtab);
     if (h->owns_stream && h->stream) cudaStreamDestroy(h->stream);
@@ -455,6 +455,15 @@ int pa_last_resample_ms(pa_t* h, float* total_ms, float* copy_kernel_ms) {
     PA_CUDA(h, cudaEventElapsedTime(&b, h->ev[4], h->ev[5]));
     if (total_ms) *total_ms = a;
     if (copy_kernel_ms) *copy_kernel_ms = b;
+    return PA_OK;
+}
+
+int pa_last_measure_ms(pa_t* h, float* kernel_ms) {
+    if (!h || !h->measure_timed) return PA_ERR_INVALID_ARG;
+    PA_CUDA(h, cudaEventSynchronize(h->ev[8]));
+    float ms = 0.f;
+    PA_CUDA(h, cudaEventElapsedTime(&ms, h->ev[7], h->ev[8]));
+    if (kernel_ms) *kernel_ms = ms;
     return PA_OK;
 }
 

@@ -109,8 +109,8 @@ struct pa_handle {
     double* h_wtab;                     // pinned, N+1
     int64_t R_prev; double W_last;      // of the last resample
 
-    cudaEvent_t ev[7];                  // sweep begin/end, resample begin/end, copy begin/end, plan scalars on the host
-    bool sweep_timed, resample_timed;
+    cudaEvent_t ev[9];                  // sweep begin/end, resample begin/end, copy begin/end, plan scalars on the host, measure begin/end
+    bool sweep_timed, resample_timed, measure_timed;
     int64_t launches;
     bool sweep_C_forced;
     int sweep_C, sweep_T, sweep_cmp, sweep_kind;   // sweep launch geometry (cluster size, threads), compare variant, kernel kind

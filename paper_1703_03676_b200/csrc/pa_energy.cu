@@ -8,6 +8,7 @@
 // extracts replica b's count, and the warps' results are summed in shared memory.
 #include "pa_common.cuh"
 #include <stddef.h>
+#include <stdlib.h>
 
 #define PA_EPLANES 20   // counts up to 2N = 2^19 (L = 512)
 
@@ -45,12 +46,13 @@ struct BitCounter {          // per-thread bit-sliced counter: planes[k] holds b
 };
 
 // Sum the bit-sliced counters of the 32 threads of a warp; afterwards every lane holds the warp total.
-__device__ __forceinline__ void pa_warp_add_planes(uint32_t p[PA_EPLANES]) {
+template <int NPL>
+__device__ __forceinline__ void pa_warp_add_planes(uint32_t (&p)[NPL]) {
 #pragma unroll
     for (int off = 16; off >= 1; off >>= 1) {
         uint32_t carry = 0;
 #pragma unroll
-        for (int k = 0; k < PA_EPLANES; ++k) {
+        for (int k = 0; k < NPL; ++k) {
             uint32_t b = __shfl_xor_sync(0xffffffffu, p[k], off);
             uint32_t u = p[k] ^ b;
             uint32_t s = u ^ carry;
@@ -60,62 +62,23 @@ __device__ __forceinline__ void pa_warp_add_planes(uint32_t p[PA_EPLANES]) {
     }
 }
 
-// The kernel also folds in everything else that is measured from (E_j, M_j) -- the paper's energyKer +
-// CalcAverages (L173) and the first stage of QKer's range (our E_min, O5) -- so that a temperature step
-// needs one launch and one device-to-host read for its observables:
-//   exact integer sums  SE = sum E, SE2 = sum E^2, SA = sum |M|, SM2 = sum M^2   (order-independent atomics),
-//   m_min / m_max of m = (E + 2N)/4                                             (atomicMax, order-independent),
-//   sum_j (M_j/N)^4 in the TREE1024 order (O5, O8): the warp that finishes a group holds one replica per lane,
-//   so its __shfl_down tree IS the aligned-run-of-32 level; the run sums go to runsum[g], and the last CTA
-//   to finish (atomic ticket) does the tree over each 32 run sums and the sequential sum over 1024-blocks.
-__global__ void __launch_bounds__(256)
-pa_measure_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R_cur,
-                  int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
-                  double* __restrict__ runsum, double* __restrict__ blocksum) {
-    const long long g = blockIdx.x;
-    const uint32_t* base = pop + g * (long long)N;
-    const int Lh = L >> 1, half = N >> 1;
+// Everything after the per-thread bit-sliced counters, shared by both measure kernels.  pe / pm hold NPL planes
+// of the thread's unsatisfied-bond and up-spin counts (bit b of plane k = bit k of replica b's count).
+template <int NPL>
+__device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&pm)[NPL], long long g, int N, long long R_cur,
+                                                int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
+                                                double* __restrict__ runsum, double* __restrict__ blocksum) {
     const int T = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    BitCounter cE, cM;
-    cE.clear(); cM.clear();
-    for (int b0 = tid * 8; b0 < N; b0 += T * 8) {
-        uint32_t xa[8], xb[8], xs[8];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) {
-            int idx = b0 + q;
-            uint32_t s = 0, a = 0, b = 0;
-            if (idx < N) {
-                int c = idx >= half ? 1 : 0;
-                int rem = idx - c * half;
-                int y = rem / Lh, xh = rem - y * Lh;
-                int p = (y + c) & 1;
-                const uint32_t* oth = base + (1 - c) * half;
-                s = base[idx];
-                // right neighbour (x+1, y): other colour, same row; down neighbour (x, y+1)
-                int xr = p ? (xh + 1 == Lh ? 0 : xh + 1) : xh;
-                int yd = (y + 1 == L) ? 0 : y + 1;
-                a = s ^ oth[y * Lh + xr];
-                b = s ^ oth[yd * Lh + xh];
-            }
-            xs[q] = s; xa[q] = a; xb[q] = b;
-        }
-        cE.add8(xa); cE.add8(xb); cM.add8(xs);
-    }
     __shared__ int sE[8][32], sM[8][32];
     __shared__ bool s_last;
-    uint32_t p[PA_EPLANES];
-#pragma unroll
-    for (int k = 0; k < PA_EPLANES; ++k) p[k] = cE.plane(k);
-    pa_warp_add_planes(p);
+    pa_warp_add_planes<NPL>(pe);
     int vE = 0;
 #pragma unroll
-    for (int k = 0; k < PA_EPLANES; ++k) vE += (int)((p[k] >> lane) & 1u) << k;
-#pragma unroll
-    for (int k = 0; k < PA_EPLANES; ++k) p[k] = cM.plane(k);
-    pa_warp_add_planes(p);
+    for (int k = 0; k < NPL; ++k) vE += (int)((pe[k] >> lane) & 1u) << k;
+    pa_warp_add_planes<NPL>(pm);
     int vM = 0;
 #pragma unroll
-    for (int k = 0; k < PA_EPLANES; ++k) vM += (int)((p[k] >> lane) & 1u) << k;
+    for (int k = 0; k < NPL; ++k) vM += (int)((pm[k] >> lane) & 1u) << k;
     sE[warp][lane] = vE; sM[warp][lane] = vM;
     __syncthreads();
     if (warp == 0) {
@@ -162,12 +125,19 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R_cu
     __threadfence();
     const long long G = gridDim.x;
     const int nblk = (int)((G + 31) / 32);
-    for (int blk = warp; blk < nblk; blk += (T >> 5)) {
-        const long long i = (long long)blk * 32 + lane;
-        double v = i < G ? __ldcg(runsum + i) : 0.0;
+    for (int blk0 = warp * 8; blk0 < nblk; blk0 += (T >> 5) * 8) {       // 8 blocks of 32 run sums in flight per warp
+        double v[8];
 #pragma unroll
-        for (int off = 16; off >= 1; off >>= 1) v = __dadd_rn(v, __shfl_down_sync(0xffffffffu, v, off));
-        if (lane == 0) blocksum[blk] = v;
+        for (int u = 0; u < 8; ++u) {
+            const long long i = (long long)(blk0 + u) * 32 + lane;
+            v[u] = i < G ? __ldcg(runsum + i) : 0.0;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+#pragma unroll
+            for (int off = 16; off >= 1; off >>= 1) v[u] = __dadd_rn(v[u], __shfl_down_sync(0xffffffffu, v[u], off));
+            if (lane == 0 && blk0 + u < nblk) blocksum[blk0 + u] = v[u];
+        }
     }
     __syncthreads();
     if (tid == 0) {
@@ -177,14 +147,177 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R_cu
     }
 }
 
+
+// The kernel also folds in everything else that is measured from (E_j, M_j) -- the paper's energyKer +
+// CalcAverages (L173) and the first stage of QKer's range (our E_min, O5) -- so that a temperature step
+// needs one launch and one device-to-host read for its observables:
+//   exact integer sums  SE = sum E, SE2 = sum E^2, SA = sum |M|, SM2 = sum M^2   (order-independent atomics),
+//   m_min / m_max of m = (E + 2N)/4                                             (atomicMax, order-independent),
+//   sum_j (M_j/N)^4 in the TREE1024 order (O5, O8): the warp that finishes a group holds one replica per lane,
+//   so its __shfl_down tree IS the aligned-run-of-32 level; the run sums go to runsum[g], and the last CTA
+//   to finish (atomic ticket) does the tree over each 32 run sums and the sequential sum over 1024-blocks.
+__global__ void __launch_bounds__(256)
+pa_measure_generic_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R_cur,
+                  int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
+                  double* __restrict__ runsum, double* __restrict__ blocksum) {
+    const long long g = blockIdx.x;
+    const uint32_t* base = pop + g * (long long)N;
+    const int Lh = L >> 1, half = N >> 1;
+    const int T = blockDim.x, tid = threadIdx.x;
+    BitCounter cE, cM;
+    cE.clear(); cM.clear();
+    for (int b0 = tid * 8; b0 < N; b0 += T * 8) {
+        uint32_t xa[8], xb[8], xs[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            int idx = b0 + q;
+            uint32_t s = 0, a = 0, b = 0;
+            if (idx < N) {
+                int c = idx >= half ? 1 : 0;
+                int rem = idx - c * half;
+                int y = rem / Lh, xh = rem - y * Lh;
+                int p = (y + c) & 1;
+                const uint32_t* oth = base + (1 - c) * half;
+                s = base[idx];
+                // right neighbour (x+1, y): other colour, same row; down neighbour (x, y+1)
+                int xr = p ? (xh + 1 == Lh ? 0 : xh + 1) : xh;
+                int yd = (y + 1 == L) ? 0 : y + 1;
+                a = s ^ oth[y * Lh + xr];
+                b = s ^ oth[yd * Lh + xh];
+            }
+            xs[q] = s; xa[q] = a; xb[q] = b;
+        }
+        cE.add8(xa); cE.add8(xb); cM.add8(xs);
+    }
+    uint32_t pe[PA_EPLANES], pm[PA_EPLANES];
+#pragma unroll
+    for (int k = 0; k < PA_EPLANES; ++k) { pe[k] = cE.plane(k); pm[k] = cM.plane(k); }
+    pa_measure_tail<PA_EPLANES>(pe, pm, g, N, R_cur, E, M, sc, runsum, blocksum);
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// Fast path for L = 8, 16, ..., 256 (powers of two; every BASELINE.json config).
+// A thread owns one quad column (four consecutive xh of both colours = two uint4 per lattice row) and walks
+// down RS rows; lanes of a warp hold consecutive quads of a row (QPR = L/8 quads per row), so the one word a
+// row's horizontal bonds need from the next quad comes from a shuffle, and the row below is the thread's own
+// next load: every word is read from memory exactly once (plus one extra row per strip), two rows ahead of
+// its use.  Per row and thread: 16 bond words -> one 16-input carry-save block, 8 spin words -> one 8-input
+// block; about 12 instructions per word against 82 in the generic kernel, which made it ALU-bound
+// (profiles/r01b_summary.md).
+// ------------------------------------------------------------------------------------------------
+template <int NP>
+struct PlaneCounter {           // planes[k] holds bit k of 32 per-lane counts, counts < 2^NP
+    uint32_t pl[NP];
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int k = 0; k < NP; ++k) pl[k] = 0;
+    }
+    // ripple a carry word of weight 2^K0 into the planes K0..NP-1
+    template <int K0>
+    __device__ __forceinline__ void ripple(uint32_t e) {
+#pragma unroll
+        for (int k = K0; k < NP; ++k) { const uint32_t t = pl[k] & e; pl[k] ^= e; e = t; }
+    }
+    __device__ __forceinline__ uint32_t block8(const uint32_t* x) {     // returns the weight-8 carry
+        uint32_t tA, tB, fA, fB, e;
+        pa_csa(tA, pl[0], pl[0], x[0], x[1]);
+        pa_csa(tB, pl[0], pl[0], x[2], x[3]);
+        pa_csa(fA, pl[1], pl[1], tA, tB);
+        pa_csa(tA, pl[0], pl[0], x[4], x[5]);
+        pa_csa(tB, pl[0], pl[0], x[6], x[7]);
+        pa_csa(fB, pl[1], pl[1], tA, tB);
+        pa_csa(e, pl[2], pl[2], fA, fB);
+        return e;
+    }
+    __device__ __forceinline__ void add8(const uint32_t* x) { ripple<3>(block8(x)); }
+    __device__ __forceinline__ void add16(const uint32_t* x) {
+        const uint32_t e1 = block8(x), e2 = block8(x + 8);
+        uint32_t s;
+        pa_csa(s, pl[3], pl[3], e1, e2);
+        ripple<4>(s);
+    }
+};
+
+__host__ __device__ constexpr int pa_msr_threads(int L) { return (L * L / 8 >= 64) ? 64 : 32; }
+__host__ __device__ constexpr int pa_msr_strips(int L) { return (pa_msr_threads(L) / (L / 8) < L) ? pa_msr_threads(L) / (L / 8) : L; }
+__host__ __device__ constexpr int pa_bits(int v) { return v <= 1 ? 1 : 1 + pa_bits(v >> 1); }
+
+template <int LOG_QPR>
+__global__ void __launch_bounds__(64)
+pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
+                  int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
+                  double* __restrict__ runsum, double* __restrict__ blocksum) {
+    constexpr int QPR = 1 << LOG_QPR, L = 8 * QPR, Lq = L / 8;          // Lq = uint4 per colour row
+    constexpr int S = pa_msr_strips(L), RS = L / S;                      // strips per group, rows per strip
+    constexpr int NPE = pa_bits(16 * RS), NPM = pa_bits(8 * RS);         // planes per thread
+    constexpr int NPW = NPE + 5;                                         // planes after the warp sum
+    const long long g = blockIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const bool act = tid < S * QPR;
+    const int q = tid & (QPR - 1), strip = act ? (tid >> LOG_QPR) : 0;
+    const uint4* c0 = reinterpret_cast<const uint4*>(pop + g * (long long)N);
+    const uint4* c1 = c0 + (N >> 3);
+    const int y0 = strip * RS;
+    const int nxt_lane = (lane & ~(QPR - 1)) | ((lane + 1) & (QPR - 1));  // next quad of the same row (periodic)
+    const uint4 zero = make_uint4(0, 0, 0, 0);
+    PlaneCounter<NPE> cE; PlaneCounter<NPM> cM;
+    cE.clear(); cM.clear();
+    uint4 a = zero, b = zero, na = zero, nb = zero;
+    if (act) {
+        a = __ldg(c0 + y0 * Lq + q); b = __ldg(c1 + y0 * Lq + q);
+        const int y1 = (y0 + 1) & (L - 1);
+        na = __ldg(c0 + y1 * Lq + q); nb = __ldg(c1 + y1 * Lq + q);
+    }
+#pragma unroll 2
+    for (int r = 0; r < RS; ++r) {
+        const int y = y0 + r;
+        uint4 fa = zero, fb = zero;                                       // row y + 2, in flight while row y is counted
+        if (act && r + 1 < RS) {
+            const int y2 = (y + 2) & (L - 1);
+            fa = __ldg(c0 + y2 * Lq + q); fb = __ldg(c1 + y2 * Lq + q);
+        }
+        // colour-0 sites of row y sit at x = 2 xh + (y & 1): the bond to the right of the odd-x site of a pair
+        // leads into the next xh of the other colour
+        const bool odd = (y & 1) != 0;
+        const uint4 t = odd ? b : a, u = odd ? a : b;                     // bond u[xh] - t[xh + 1]
+        const uint32_t tn = __shfl_sync(0xffffffffu, t.x, nxt_lane);
+        uint32_t xb[16];
+        xb[0] = a.x ^ b.x; xb[1] = a.y ^ b.y; xb[2] = a.z ^ b.z; xb[3] = a.w ^ b.w;        // bonds inside a pair
+        xb[4] = u.x ^ t.y; xb[5] = u.y ^ t.z; xb[6] = u.z ^ t.w; xb[7] = u.w ^ tn;         // bonds between pairs
+        xb[8] = a.x ^ nb.x; xb[9] = a.y ^ nb.y; xb[10] = a.z ^ nb.z; xb[11] = a.w ^ nb.w;  // down bonds of colour 0
+        xb[12] = b.x ^ na.x; xb[13] = b.y ^ na.y; xb[14] = b.z ^ na.z; xb[15] = b.w ^ na.w; // down bonds of colour 1
+        const uint32_t xs[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+        cE.add16(xb);
+        cM.add8(xs);
+        a = na; b = nb; na = fa; nb = fb;
+    }
+    uint32_t pe[NPW], pm[NPW];
+#pragma unroll
+    for (int k = 0; k < NPW; ++k) { pe[k] = k < NPE ? cE.pl[k < NPE ? k : 0] : 0u; pm[k] = k < NPM ? cM.pl[k < NPM ? k : 0] : 0u; }
+    pa_measure_tail<NPW>(pe, pm, g, N, R_cur, E, M, sc, runsum, blocksum);
+}
+
 int pa_launch_measure(pa_handle* h) {
     const int64_t G = (h->R_cur + 31) / 32;
-    int T = 256;
-    while (T > 32 && T * 8 > h->N) T >>= 1;
+    const int L = h->L;
     PA_CUDA(h, cudaMemsetAsync(h->d_scal, 0, offsetof(PaScalars, R_new), h->stream));
-    pa_measure_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, h->E, h->M, h->d_scal,
-                                                        h->runsum, h->partials);
+    PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
+    const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
+    if (pow2) {
+#define PA_MSR_CASE(LOG) case (8 << LOG): pa_measure_kernel<LOG><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
+            h->spins[h->cur], h->N, h->R_cur, h->E, h->M, h->d_scal, h->runsum, h->partials); break;
+        switch (L) { PA_MSR_CASE(0) PA_MSR_CASE(1) PA_MSR_CASE(2) PA_MSR_CASE(3) PA_MSR_CASE(4) PA_MSR_CASE(5) default: break; }
+#undef PA_MSR_CASE
+    } else {
+        int T = 256;
+        while (T > 32 && T * 8 > h->N) T >>= 1;
+        pa_measure_generic_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, h->E, h->M, h->d_scal,
+                                                                    h->runsum, h->partials);
+    }
     PA_CUDA(h, cudaGetLastError());
+    PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));
+    h->measure_timed = true;
     h->launches += 1;
     h->em_valid = true;
     h->host_scal_valid = false;

@@ -87,6 +87,7 @@ def lib():
         "pa_launch_count": ([vp], i64),
         "pa_last_sweep_ms": ([vp, C.POINTER(C.c_float)], i32),
         "pa_last_resample_ms": ([vp, C.POINTER(C.c_float), C.POINTER(C.c_float)], i32),
+        "pa_last_measure_ms": ([vp, C.POINTER(C.c_float)], i32),
         "pa_calibrate": ([i32, C.POINTER(dbl), C.POINTER(dbl)], i32),
         "pa_strerror": ([i32], C.c_char_p),
         "pa_last_cuda_error": ([vp], C.c_char_p),
@@ -305,6 +306,11 @@ class Population:
     def last_sweep_ms(self):
         ms = C.c_float()
         self._check(lib().pa_last_sweep_ms(self._h, C.byref(ms)), "pa_last_sweep_ms")
+        return ms.value
+
+    def last_measure_ms(self):
+        ms = C.c_float()
+        self._check(lib().pa_last_measure_ms(self._h, C.byref(ms)), "pa_last_measure_ms")
         return ms.value
 
     def last_resample_ms(self):
