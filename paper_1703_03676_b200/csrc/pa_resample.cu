@@ -199,12 +199,21 @@ int pa_launch_plan(pa_handle* h, int Emin) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Copy (L165-L171 resampleKer; O7): new[d] = old[parent(d)].  The 32 slots of a destination group
-// come from a monotone run of parents, so the word of the destination group at a site is an OR of a
-// few "segments": a rotated, masked source word.  One warp builds the segment list of the group
-// once; all threads then stream the group's N words with 128-bit loads and stores.
+// Copy (L165-L171 resampleKer; O7): new[d] = old[parent(d)].  The parents of the 32 slots of a
+// destination group are non-decreasing, so lane d reads global source bit parent(d) = s_d + d with an
+// offset s_d = parent(d) - d that changes only where a copy number differs from 1.  All lanes with the
+// same offset are served by one funnel shift of the two neighbouring source words (a 32-bit window at
+// bit s of the concatenated source groups) and one mask: a destination word costs two instructions per
+// DISTINCT offset (typically 3-5), however the lanes interleave.  One warp builds the (source group,
+// shift, mask) classes of the group with __match_any_sync, sorted by source group so that every source
+// word is loaded once; all threads then stream the group's N words with 128-bit loads and stores.
 // ------------------------------------------------------------------------------------------------
-struct __align__(16) PaSeg { uint32_t src_group, rot, mask, pad; };
+struct __align__(16) PaSeg { int q; uint32_t shift, mask, pad; };   // window = bits [32q + shift, +32) of the source
+
+__device__ __forceinline__ uint4 pa_ld_group(const uint32_t* __restrict__ src, long long q, long long Gmax, int N, int i) {
+    q = q < 0 ? 0 : (q >= Gmax ? Gmax - 1 : q);    // a clamped word is never selected by a mask (see above)
+    return __ldg(reinterpret_cast<const uint4*>(src + q * N) + i);
+}
 
 __global__ void __launch_bounds__(128)
 pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, const uint32_t* __restrict__ parent,
@@ -221,46 +230,47 @@ pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, con
     if (tid < 32) {
         const long long d = g * 32 + tid;
         const bool valid = d < R_new;
-        const uint32_t p = valid ? parent[d] : 0xffffffffu;
-        const uint32_t pprev = __shfl_up_sync(0xffffffffu, p, 1);
-        const bool vprev = __shfl_up_sync(0xffffffffu, (int)valid, 1) != 0;
-        // a segment continues while parents are consecutive slots of one source group
-        bool start = valid && (tid == 0 || !vprev || p != pprev + 1u || (p >> 5) != (pprev >> 5));
-        const unsigned starts = __ballot_sync(0xffffffffu, start);
-        const unsigned valids = __ballot_sync(0xffffffffu, valid);
-        if (start) {
-            const unsigned later = starts & ~((2u << tid) - 1u);               // starts after this lane
-            const int nvalid = __popc(valids);
-            const int end = later ? (__ffs(later) - 1) : nvalid;                // first lane past the segment
-            const int len = end - tid;
-            const int idx = __popc(starts & ((1u << tid) - 1u));
-            PaSeg s;
-            s.src_group = p >> 5;
-            s.rot = (uint32_t)(tid - (int)(p & 31u)) & 31u;                     // rotate left: src bit -> dst bit
-            s.mask = (len >= 32 ? 0xffffffffu : ((1u << len) - 1u)) << tid;
-            s.pad = 0u;
-            segs[idx] = s;
+        // offset of this lane; invalid lanes get private keys that sort last and carry an empty mask
+        const long long s = valid ? (long long)parent[d] - tid : (1ll << 40) + tid;
+        const unsigned same = __match_any_sync(0xffffffffu, (unsigned long long)s);
+        const bool leader = (__ffs(same) - 1) == tid;
+        const unsigned leaders = __ballot_sync(0xffffffffu, leader && valid);
+        int rank = 0;
+        for (int l = 0; l < 32; ++l) {
+            const long long sl = __shfl_sync(0xffffffffu, s, l);
+            rank += (int)(((leaders >> l) & 1u) != 0u && sl < s);
         }
-        if (tid == 0) nseg = __popc(starts);
+        if (leader && valid) {
+            PaSeg e;
+            e.q = (int)(s >> 5);                    // arithmetic shift: floor, s may be negative (down to -31)
+            e.shift = (uint32_t)(s & 31);
+            e.mask = same;
+            e.pad = 0u;
+            segs[rank] = e;
+        }
+        if (tid == 0) nseg = __popc(leaders);
     }
     __syncthreads();
     const int ns = nseg;
     const int chunks = N >> 2;
+    const long long Gmax = (R_cap + 31) >> 5;
     uint4* out = reinterpret_cast<uint4*>(dst + g * (long long)N);
     for (int i = blockIdx.y * blockDim.x + tid; i < chunks; i += gridDim.y * blockDim.x) {
         uint4 acc = make_uint4(0, 0, 0, 0);
-        uint32_t cur_group = 0xffffffffu;
-        uint4 w = make_uint4(0, 0, 0, 0);
+        int cur = segs[0].q;
+        uint4 lo = pa_ld_group(src, cur, Gmax, N, i);
+        uint4 hi = pa_ld_group(src, (long long)cur + 1, Gmax, N, i);
         for (int k = 0; k < ns; ++k) {
-            const PaSeg s = segs[k];
-            if (s.src_group != cur_group) {
-                cur_group = s.src_group;
-                w = reinterpret_cast<const uint4*>(src + (long long)cur_group * N)[i];
+            const PaSeg e = segs[k];
+            if (e.q != cur) {
+                if (e.q == cur + 1) lo = hi; else lo = pa_ld_group(src, e.q, Gmax, N, i);
+                cur = e.q;
+                hi = pa_ld_group(src, (long long)cur + 1, Gmax, N, i);
             }
-            acc.x |= __funnelshift_l(w.x, w.x, s.rot) & s.mask;
-            acc.y |= __funnelshift_l(w.y, w.y, s.rot) & s.mask;
-            acc.z |= __funnelshift_l(w.z, w.z, s.rot) & s.mask;
-            acc.w |= __funnelshift_l(w.w, w.w, s.rot) & s.mask;
+            acc.x |= __funnelshift_r(lo.x, hi.x, e.shift) & e.mask;
+            acc.y |= __funnelshift_r(lo.y, hi.y, e.shift) & e.mask;
+            acc.z |= __funnelshift_r(lo.z, hi.z, e.shift) & e.mask;
+            acc.w |= __funnelshift_r(lo.w, hi.w, e.shift) & e.mask;
         }
         out[i] = acc;
     }
