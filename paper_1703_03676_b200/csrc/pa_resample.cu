@@ -204,22 +204,56 @@ int pa_launch_plan(pa_handle* h, int Emin) {
 // offset s_d = parent(d) - d that changes only where a copy number differs from 1.  All lanes with the
 // same offset are served by one funnel shift of the two neighbouring source words (a 32-bit window at
 // bit s of the concatenated source groups) and one mask: a destination word costs two instructions per
-// DISTINCT offset (typically 3-5), however the lanes interleave.  One warp builds the (source group,
-// shift, mask) classes of the group with __match_any_sync, sorted by source group so that every source
+// DISTINCT offset, however the lanes interleave.  One warp builds the (shift, mask) classes of the
+// group with __match_any_sync, sorted by offset and grouped into source windows so that every source
 // word is loaded once; all threads then stream the group's N words with 128-bit loads and stores.
 // ------------------------------------------------------------------------------------------------
-struct __align__(16) PaSeg { int q; uint32_t shift, mask, pad; };   // window = bits [32q + shift, +32) of the source
+struct __align__(8) PaSeg { uint32_t shift, mask; };              // one offset class: dst |= (window >> shift) & mask
+struct __align__(16) PaWin {                                      // one source window = two neighbouring source groups
+    uint32_t lo_g, hi_g;     // group indices of the low / high word, clamped into the buffer (a clamped word is never selected)
+    int seg_end;             // classes [previous seg_end, seg_end) read this window
+    int consecutive;         // the low word is the previous window's high word
+};
 
-__device__ __forceinline__ uint4 pa_ld_group(const uint32_t* __restrict__ src, long long q, long long Gmax, int N, int i) {
-    q = q < 0 ? 0 : (q >= Gmax ? Gmax - 1 : q);    // a clamped word is never selected by a mask (see above)
-    return __ldg(reinterpret_cast<const uint4*>(src + q * N) + i);
+// NCH chunks of 4 words per thread and pass: the class list is walked once for NCH chunks, and NCH x 2 loads are in flight.
+template <int NCH>
+__device__ __forceinline__ void pa_copy_chunks(const uint4* __restrict__ src4, uint4* __restrict__ out, const PaWin* wins, int nw,
+                                               const PaSeg* segs, int chunks, int i, int stride) {
+    uint4 acc[NCH], lo[NCH], hi[NCH];
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) { acc[c] = make_uint4(0, 0, 0, 0); lo[c] = acc[c]; hi[c] = acc[c]; }
+    int k = 0;
+    for (int w = 0; w < nw; ++w) {
+        const PaWin W = wins[w];
+        const uint4* plo = src4 + (size_t)W.lo_g * chunks + i;
+        const uint4* phi = src4 + (size_t)W.hi_g * chunks + i;
+#pragma unroll
+        for (int c = 0; c < NCH; ++c) {
+            if (W.consecutive) lo[c] = hi[c]; else lo[c] = __ldg(plo + c * stride);
+            hi[c] = __ldg(phi + c * stride);
+        }
+        for (; k < W.seg_end; ++k) {
+            const PaSeg e = segs[k];
+#pragma unroll
+            for (int c = 0; c < NCH; ++c) {
+                acc[c].x |= __funnelshift_r(lo[c].x, hi[c].x, e.shift) & e.mask;
+                acc[c].y |= __funnelshift_r(lo[c].y, hi[c].y, e.shift) & e.mask;
+                acc[c].z |= __funnelshift_r(lo[c].z, hi[c].z, e.shift) & e.mask;
+                acc[c].w |= __funnelshift_r(lo[c].w, hi[c].w, e.shift) & e.mask;
+            }
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) out[i + c * stride] = acc[c];
 }
 
 __global__ void __launch_bounds__(128)
 pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, const uint32_t* __restrict__ parent,
                const PaScalars* __restrict__ sc, long long R_cap, int N) {
     __shared__ PaSeg segs[32];
-    __shared__ int nseg;
+    __shared__ PaWin wins[32];
+    __shared__ int sq[32];
+    __shared__ int nwin;
     const long long g = blockIdx.x;
     const int tid = threadIdx.x;
     // R_new is read on the device: the launch does not wait for the host to see it, the grid covers the
@@ -230,50 +264,51 @@ pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, con
     if (tid < 32) {
         const long long d = g * 32 + tid;
         const bool valid = d < R_new;
-        // offset of this lane; invalid lanes get private keys that sort last and carry an empty mask
+        // offset of this lane; invalid lanes get private keys that sort last and carry no class
         const long long s = valid ? (long long)parent[d] - tid : (1ll << 40) + tid;
         const unsigned same = __match_any_sync(0xffffffffu, (unsigned long long)s);
-        const bool leader = (__ffs(same) - 1) == tid;
-        const unsigned leaders = __ballot_sync(0xffffffffu, leader && valid);
+        const bool leader = valid && (__ffs(same) - 1) == tid;
+        const unsigned leaders = __ballot_sync(0xffffffffu, leader);
         int rank = 0;
         for (int l = 0; l < 32; ++l) {
             const long long sl = __shfl_sync(0xffffffffu, s, l);
             rank += (int)(((leaders >> l) & 1u) != 0u && sl < s);
         }
-        if (leader && valid) {
+        if (leader) {
             PaSeg e;
-            e.q = (int)(s >> 5);                    // arithmetic shift: floor, s may be negative (down to -31)
             e.shift = (uint32_t)(s & 31);
             e.mask = same;
-            e.pad = 0u;
             segs[rank] = e;
+            sq[rank] = (int)(s >> 5);               // arithmetic shift: floor, s may be negative (down to -31)
         }
-        if (tid == 0) nseg = __popc(leaders);
+        __syncwarp();
+        // classes are sorted by offset, hence by source window q; consecutive classes with the same q share the loads
+        const int ns = __popc(leaders);
+        const long long Gmax = (R_cap + 31) >> 5;
+        const int q = tid < ns ? sq[tid] : 0;
+        const bool wstart = tid < ns && (tid == 0 || q != sq[tid - 1]);
+        const unsigned wstarts = __ballot_sync(0xffffffffu, wstart);
+        if (wstart) {
+            const unsigned later = tid == 31 ? 0u : wstarts & ~((2u << tid) - 1u);
+            PaWin W;
+            const long long ql = q, qh = (long long)q + 1;
+            W.lo_g = (uint32_t)(ql < 0 ? 0 : (ql >= Gmax ? Gmax - 1 : ql));
+            W.hi_g = (uint32_t)(qh < 0 ? 0 : (qh >= Gmax ? Gmax - 1 : qh));
+            W.seg_end = later ? (__ffs(later) - 1) : ns;
+            W.consecutive = (tid > 0 && q == sq[tid - 1] + 1) ? 1 : 0;
+            wins[__popc(wstarts & ((1u << tid) - 1u))] = W;
+        }
+        if (tid == 0) nwin = __popc(wstarts);
     }
     __syncthreads();
-    const int ns = nseg;
+    const int nw = nwin;
     const int chunks = N >> 2;
-    const long long Gmax = (R_cap + 31) >> 5;
+    const uint4* src4 = reinterpret_cast<const uint4*>(src);
     uint4* out = reinterpret_cast<uint4*>(dst + g * (long long)N);
-    for (int i = blockIdx.y * blockDim.x + tid; i < chunks; i += gridDim.y * blockDim.x) {
-        uint4 acc = make_uint4(0, 0, 0, 0);
-        int cur = segs[0].q;
-        uint4 lo = pa_ld_group(src, cur, Gmax, N, i);
-        uint4 hi = pa_ld_group(src, (long long)cur + 1, Gmax, N, i);
-        for (int k = 0; k < ns; ++k) {
-            const PaSeg e = segs[k];
-            if (e.q != cur) {
-                if (e.q == cur + 1) lo = hi; else lo = pa_ld_group(src, e.q, Gmax, N, i);
-                cur = e.q;
-                hi = pa_ld_group(src, (long long)cur + 1, Gmax, N, i);
-            }
-            acc.x |= __funnelshift_r(lo.x, hi.x, e.shift) & e.mask;
-            acc.y |= __funnelshift_r(lo.y, hi.y, e.shift) & e.mask;
-            acc.z |= __funnelshift_r(lo.z, hi.z, e.shift) & e.mask;
-            acc.w |= __funnelshift_r(lo.w, hi.w, e.shift) & e.mask;
-        }
-        out[i] = acc;
-    }
+    const int stride = gridDim.y * blockDim.x;
+    int i = blockIdx.y * blockDim.x + tid;
+    for (; i + stride < chunks; i += 2 * stride) pa_copy_chunks<2>(src4, out, wins, nw, segs, chunks, i, stride);
+    if (i < chunks) pa_copy_chunks<1>(src4, out, wins, nw, segs, chunks, i, stride);
 }
 
 int pa_launch_copy(pa_handle* h) {

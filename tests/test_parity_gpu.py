@@ -116,6 +116,19 @@ def test_resample_chain_bit_exact(L, R):
         assert_obs_close(g.observables(beta), o.observables(beta))
 
 
+@pytest.mark.parametrize("L,R", [(16, 4133), (8, 700), (64, 777)])
+def test_copy_strong_resampling(L, R):
+    """Copy kernel under strong resampling: many empty and many-fold copy numbers, parents spanning several
+    source groups, ragged last group; N/4 below, at and above two chunks per thread."""
+    g, o = pa.Population(L, R, 9), po.Oracle(L, R, 9)
+    beta = 0.0
+    for db in (0.03, 0.25, 0.4, 0.0, 1.5):
+        _compare_resample(g, o, beta, beta + db)
+        beta += db
+        assert_same_state(g, o)
+        g.sweep(beta, 1); o.sweep(beta, 1)
+
+
 def test_resample_identity_capacity_and_errors():
     L, R = 16, 500
     g, o = pa.Population(L, R, 5), po.Oracle(L, R, 5)
