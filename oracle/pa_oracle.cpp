@@ -24,6 +24,10 @@
 //   observables (O8) ..... L=4 exact enumeration, Kaufman e and C at L=16 (4 sigma over seeds)
 //   multi-histogram (O9) . sum H = R_i, sum H*E = SE, ln Omega vs exact ln g(E) at L=4
 //   adaptive step (O10) .. alpha(0) closed form, monotonicity, bracket property
+//   LCG-assisted stream (O11) recurrence against big-integer arithmetic with the constants the
+//                          paper prints (L236); the same L=4 Boltzmann chi^2, global-flip symmetry
+//                          and Kaufman pins as the Philox-per-spin sweep; variance ratio of C
+//                          against the Philox-per-spin mode (Table 1, last column = 1)
 //   whole method vs the paper's own figures: "parity unpinned" (Figs. 2-3 data and the authors'
 //   code are not available); pinned instead by the exact Ising results above.
 
@@ -81,6 +85,27 @@ inline uint32_t x_sweep(uint64_t seed, int64_t j, uint32_t s, uint32_t t, uint32
     philox4x32_10(s, (uint32_t)(j >> 2), 2u * t + c, TAG_SWEEP, key0(seed), key1(seed), out);
     return out[j & 3];
 }
+// O11  LCG-assisted stream (Sec. 4: "combining the underlying RNG with a particularly fast
+// in-line generator used to supply the p random numbers used to flip the spins stored in the same
+// word ... r_{n+1} = A r_n + C mod 2^32 with A = 1664525 and C = 1013904223 ... seeded by a call to
+// the underlying, high-quality generator (Philox)").  Reading (O11): the word of group
+// g = j>>5 at site s = (x,y) is re-seeded at EVERY visit (sweep t, colour c = (x+y)&1) with
+//   r_0 = philox(quad, g, 2t+c, TAG_LCG)[y&3],   quad = (y>>2)*(L/2) + (x>>1)
+// (one Philox call serves the four rows of a quad in one column of one sub-lattice), and the 32
+// replicas of the word take the next 32 LCG outputs, most significant lane first:
+//   x(32g+b) = r_{32-b},  r_{n+1} = A r_n + C mod 2^32.
+const uint32_t TAG_LCG = 3u;
+const uint32_t LCG_A = 1664525u, LCG_C = 1013904223u;        // L236, ref. [43]
+inline uint32_t lcg_next(uint32_t r) { return LCG_A * r + LCG_C; }   // uint32 arithmetic = mod 2^32
+inline uint32_t x_sweep_lcg(uint64_t seed, int64_t j, int L, int x, int y, uint32_t t, uint32_t c) {
+    uint32_t out[4];
+    uint32_t quad = (uint32_t)((y >> 2) * (L / 2) + (x >> 1));
+    philox4x32_10(quad, (uint32_t)(j >> 5), 2u * t + c, TAG_LCG, key0(seed), key1(seed), out);
+    uint32_t r = out[y & 3];
+    int steps = 32 - (int)(j & 31);
+    for (int n = 0; n < steps; ++n) r = lcg_next(r);
+    return r;
+}
 // RESAMPLE: x(j,k) = philox(j>>2, 0, k, TAG_RESAMPLE)[j&3]; k = resample counter.
 inline uint32_t x_resample(uint64_t seed, int64_t j, uint32_t k) {
     uint32_t out[4];
@@ -106,8 +131,10 @@ uint32_t threshold(double p) {
 // dE = 2*sigma*sum_nn sigma = 8 - 4u; flip iff dE <= 0 or x < T(dE).
 // Colour 0 = (x+y) even is updated first, then colour 1.
 // ---------------------------------------------------------------------------------------------
+enum { RNG_PHILOX = 0, RNG_LCG = 1 };   // O1 (one Philox number per spin) / O11 (Philox-seeded LCG)
+
 void sweep_one_replica(uint8_t* sp, int L, uint64_t seed, int64_t slot, uint32_t t,
-                       uint32_t T4, uint32_t T8) {
+                       uint32_t T4, uint32_t T8, int rng_mode) {
     for (uint32_t c = 0; c < 2; ++c) {
         for (int y = 0; y < L; ++y) {
             for (int x = 0; x < L; ++x) {
@@ -117,7 +144,8 @@ void sweep_one_replica(uint8_t* sp, int L, uint64_t seed, int64_t slot, uint32_t
                 int ym = y == 0 ? L - 1 : y - 1, yp = y == L - 1 ? 0 : y + 1;
                 int u = (sp[y * L + xm] != sp[s]) + (sp[y * L + xp] != sp[s]) +
                         (sp[ym * L + x] != sp[s]) + (sp[yp * L + x] != sp[s]);
-                uint32_t xr = x_sweep(seed, slot, (uint32_t)s, t, c);   // drawn for every (j,s,t)
+                uint32_t xr = rng_mode == RNG_LCG ? x_sweep_lcg(seed, slot, L, x, y, t, c)
+                                                  : x_sweep(seed, slot, (uint32_t)s, t, c);   // drawn for every (j,s,t)
                 bool flip = (u >= 2) || (u == 1 && xr < T4) || (u == 0 && xr < T8);
                 if (flip) sp[s] ^= 1u;
             }
@@ -184,6 +212,7 @@ struct Oracle {
     int64_t R_target = 0, R_cur = 0, R_cap = 0;
     uint64_t seed = 0;
     uint32_t t = 0;          // global sweep counter
+    int rng_mode = RNG_PHILOX;
     uint32_t k = 0;          // resample counter
     double lnZ = 0.0;        // = -beta F(beta), Eq. 4; starts at N ln 2 (L93)
     double lnQ_last = 0.0;
@@ -311,17 +340,22 @@ int64_t ora_capacity(int64_t R) { return capacity_for(R); }
 
 // theta sweeps (O3) of nslots replicas given as spins[nslots][N], replica i living in population
 // slot slot_ids[i]; the sweep counter runs t0, t0+1, ..., t0+theta-1.
-int ora_sweep_slots(int L, uint64_t seed, uint32_t t0, double beta, int theta,
-                    int64_t nslots, const int64_t* slot_ids, uint8_t* spins) {
-    if (L < 4 || (L & 1) || theta < 0 || nslots < 0) return ORA_ERR_INVALID_ARG;
+int ora_sweep_slots_mode(int L, uint64_t seed, uint32_t t0, double beta, int theta,
+                         int64_t nslots, const int64_t* slot_ids, uint8_t* spins, int rng_mode) {
+    if (L < 4 || (L & 1) || theta < 0 || nslots < 0 || rng_mode < 0 || rng_mode > 1) return ORA_ERR_INVALID_ARG;
     uint32_t T4, T8; ora_thresholds(beta, &T4, &T8);
     int N = L * L;
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < nslots; ++i)
         for (int it = 0; it < theta; ++it)
-            sweep_one_replica(spins + (size_t)i * N, L, seed, slot_ids[i], t0 + (uint32_t)it, T4, T8);
+            sweep_one_replica(spins + (size_t)i * N, L, seed, slot_ids[i], t0 + (uint32_t)it, T4, T8, rng_mode);
     return ORA_OK;
 }
+int ora_sweep_slots(int L, uint64_t seed, uint32_t t0, double beta, int theta,
+                    int64_t nslots, const int64_t* slot_ids, uint8_t* spins) {
+    return ora_sweep_slots_mode(L, seed, t0, beta, theta, nslots, slot_ids, spins, RNG_PHILOX);
+}
+uint32_t ora_lcg_next(uint32_t r) { return lcg_next(r); }
 
 int ora_energies_of(int L, int64_t n, const uint8_t* spins, int32_t* E, int32_t* M) {
     if (L < 4 || (L & 1) || n < 0) return ORA_ERR_INVALID_ARG;
@@ -407,6 +441,12 @@ int ora_create(int L, int64_t R, uint64_t seed, Oracle** out) {
 }
 
 void ora_destroy(Oracle* o) { delete o; }
+// 0 = one Philox number per spin (O1), 1 = Philox-seeded LCG per word (O11, L236-L241)
+int ora_set_rng_mode(Oracle* o, int mode) {
+    if (!o || mode < 0 || mode > 1) return ORA_ERR_INVALID_ARG;
+    o->rng_mode = mode;
+    return ORA_OK;
+}
 int64_t ora_population(const Oracle* o) { return o->R_cur; }
 int64_t ora_capacity_of(const Oracle* o) { return o->R_cap; }
 uint32_t ora_sweep_counter(const Oracle* o) { return o->t; }
@@ -420,7 +460,7 @@ int ora_sweep(Oracle* o, double beta, int theta) {
 #pragma omp parallel for schedule(static)
     for (int64_t j = 0; j < o->R_cur; ++j)
         for (int it = 0; it < theta; ++it)
-            sweep_one_replica(&o->spin[(size_t)j * o->N], o->L, o->seed, j, o->t + (uint32_t)it, T4, T8);
+            sweep_one_replica(&o->spin[(size_t)j * o->N], o->L, o->seed, j, o->t + (uint32_t)it, T4, T8, o->rng_mode);
     o->t += (uint32_t)theta;
     return ORA_OK;
 }

@@ -33,6 +33,9 @@ def lib():
         L.ora_tree1024.argtypes = [vp, i64]; L.ora_tree1024.restype = dbl
         L.ora_capacity.argtypes = [i64]; L.ora_capacity.restype = i64
         L.ora_sweep_slots.argtypes = [i32, u64, u32, dbl, i32, i64, vp, vp]; L.ora_sweep_slots.restype = i32
+        L.ora_sweep_slots_mode.argtypes = [i32, u64, u32, dbl, i32, i64, vp, vp, i32]; L.ora_sweep_slots_mode.restype = i32
+        L.ora_lcg_next.argtypes = [u32]; L.ora_lcg_next.restype = u32
+        L.ora_set_rng_mode.argtypes = [vp, i32]; L.ora_set_rng_mode.restype = i32
         L.ora_energies_of.argtypes = [i32, i64, vp, vp, vp]; L.ora_energies_of.restype = i32
         L.ora_resample_plan.argtypes = [i64, i64, vp, u64, u32, dbl, vp, vp, vp, vp, vp, vp]
         L.ora_resample_plan.restype = i32
@@ -99,13 +102,20 @@ def capacity(R):
     return int(lib().ora_capacity(int(R)))
 
 
-def sweep_slots(L, seed, t0, beta, theta, slot_ids, spins01):
+RNG_PHILOX, RNG_LCG = 0, 1      # O1: one Philox number per spin; O11: Philox-seeded LCG per word
+
+
+def sweep_slots(L, seed, t0, beta, theta, slot_ids, spins01, rng_mode=RNG_PHILOX):
     """theta sweeps of the replicas spins01[n][N] (uint8 0/1) living in slots slot_ids; in place."""
     slot_ids = np.ascontiguousarray(slot_ids, dtype=np.int64)
     assert spins01.dtype == np.uint8 and spins01.flags.c_contiguous
-    _check(lib().ora_sweep_slots(L, seed, t0, float(beta), theta, slot_ids.size, _p(slot_ids), _p(spins01)),
-           "sweep_slots")
+    _check(lib().ora_sweep_slots_mode(L, seed, t0, float(beta), theta, slot_ids.size, _p(slot_ids), _p(spins01),
+                                      int(rng_mode)), "sweep_slots")
     return spins01
+
+
+def lcg_next(r):
+    return int(lib().ora_lcg_next(int(r)))
 
 
 def energies_of(L, spins01):
@@ -199,6 +209,9 @@ class Oracle:
     @property
     def lnZ(self):
         return float(lib().ora_lnZ(self._h))
+
+    def set_rng_mode(self, mode):
+        _check(lib().ora_set_rng_mode(self._h, int(mode)), "set_rng_mode")
 
     def sweep(self, beta, theta):
         _check(lib().ora_sweep(self._h, float(beta), int(theta)), "sweep")

@@ -1,0 +1,145 @@
+"""Pins of the oracle's LCG-assisted sweep stream (O11; Sec. 4) against
+what the paper and the mathematics fix (-m "not gpu").  None of the expected values comes from the
+oracle itself or from the CUDA path."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import exact_ising as ex
+from oracle import pa_oracle as po
+import pa_driver
+
+LCG = po.RNG_LCG
+
+
+def test_lcg_recurrence_and_constants_of_the_paper():
+    # r_{n+1} = A r_n + C mod 2^32 with A = 1664525 and C = 1013904223 (ref. [43]);
+    # checked in unbounded integer arithmetic, including the wrap-around cases
+    rng = np.random.default_rng(0)
+    for r in [0, 1, 2**32 - 1, 2**31, 2**31 - 1] + [int(v) for v in rng.integers(0, 2**32, 200)]:
+        assert po.lcg_next(r) == (1664525 * r + 1013904223) % 2**32
+    # full period 2^32 (Hull-Dobell: C odd, A = 1 mod 4): r -> r' is a bijection, spot-checked on a block
+    outs = {po.lcg_next(r) for r in range(5000)}
+    assert len(outs) == 5000
+
+
+@pytest.mark.parametrize("beta", [0.2, 0.4406868, 0.7])
+def test_lcg_sweep_samples_boltzmann_L4(beta):
+    # detailed balance: long fixed-beta chains against the exact Boltzmann distribution of the 4x4 torus
+    L, n = 4, 40000
+    rng = np.random.default_rng(6)
+    sp = rng.integers(0, 2, (n, 16), dtype=np.uint8)
+    po.sweep_slots(L, seed=10, t0=0, beta=beta, theta=150, slot_ids=np.arange(n), spins01=sp, rng_mode=LCG)
+    E, M = po.energies_of(L, sp)
+    exact = ex.exact_small(beta, L)
+    chi2, dof = 0.0, 0
+    for Ev, p in exact["pE"].items():
+        if p * n < 5:
+            continue
+        cnt = int((E == Ev).sum())
+        chi2 += (cnt - p * n) ** 2 / (p * n)
+        dof += 1
+    assert dof >= 5
+    assert chi2 < dof + 6 * math.sqrt(2 * dof), (chi2, dof)
+    assert abs(np.abs(M).mean() / 16 - exact["absm"]) < 5 * 0.5 / math.sqrt(n)
+    assert abs(M.mean() / 16) < 5 / math.sqrt(n)
+
+
+def test_lcg_sweep_symmetry_noop_and_keying():
+    L, n = 6, 70                                                       # 70 slots: three words, the last one ragged
+    rng = np.random.default_rng(1)
+    a = rng.integers(0, 2, (n, L * L), dtype=np.uint8)
+    b = (1 - a).copy()
+    a0 = a.copy()
+    slots = np.arange(100, 100 + n)
+    po.sweep_slots(L, 3, 17, 0.35, 0, slots, a, rng_mode=LCG)
+    assert np.array_equal(a, a0)                                       # theta = 0 is a no-op
+    po.sweep_slots(L, 3, 17, 0.35, 7, slots, a, rng_mode=LCG)
+    po.sweep_slots(L, 3, 17, 0.35, 7, slots, b, rng_mode=LCG)
+    assert np.array_equal(a, 1 - b)                                    # global flip symmetry (acceptance depends on u only)
+    assert not np.array_equal(a, a0)
+    # theta = 3 split into 1 + 2 with the counter advanced: the word is re-seeded at every visit (O11)
+    base = rng.integers(0, 2, (n, L * L), dtype=np.uint8)
+    ref = po.sweep_slots(L, 3, 5, 0.4, 3, slots, base.copy(), rng_mode=LCG)
+    s = po.sweep_slots(L, 3, 5, 0.4, 1, slots, base.copy(), rng_mode=LCG)
+    s = po.sweep_slots(L, 3, 6, 0.4, 2, slots, s, rng_mode=LCG)
+    assert np.array_equal(s, ref)
+    # a replica's trajectory depends on its slot id, not on its position in the call
+    perm = np.arange(n)[::-1].copy()
+    s = po.sweep_slots(L, 3, 5, 0.4, 3, slots[perm], base[perm].copy(), rng_mode=LCG)
+    assert np.array_equal(s, ref[perm])
+    # other seed / counter / slot / generator mode -> other trajectory
+    assert not np.array_equal(po.sweep_slots(L, 4, 5, 0.4, 3, slots, base.copy(), rng_mode=LCG), ref)
+    assert not np.array_equal(po.sweep_slots(L, 3, 6, 0.4, 3, slots, base.copy(), rng_mode=LCG), ref)
+    assert not np.array_equal(po.sweep_slots(L, 3, 5, 0.4, 3, slots + 1, base.copy(), rng_mode=LCG), ref)
+    assert not np.array_equal(po.sweep_slots(L, 3, 5, 0.4, 3, slots, base.copy()), ref)
+
+
+def test_lcg_siblings_in_one_word_decorrelate():
+    # with ONE random number per word, copies of the same parent stored in the same word
+    # "are coupled and remain identical for all future times"; the LCG gives every replica of the word its own
+    # number (L236), so identical copies in one word must drift apart
+    L = 8
+    rng = np.random.default_rng(3)
+    one = rng.integers(0, 2, (1, L * L), dtype=np.uint8)
+    sp = np.repeat(one, 32, axis=0).copy()                             # 32 identical replicas = one full word
+    po.sweep_slots(L, 7, 0, 0.3, 2, np.arange(32), sp, rng_mode=LCG)
+    distinct = {row.tobytes() for row in sp}
+    assert len(distinct) == 32
+    # and their mutual overlap is that of independent chains: mean Hamming distance between siblings is the same
+    # as between the same configuration evolved in different words (statistically, 5 sigma)
+    n = 256
+    same_word = np.repeat(one, n, axis=0).copy()
+    po.sweep_slots(L, 7, 0, 0.3, 2, np.arange(n), same_word, rng_mode=LCG)
+    other_words = np.repeat(one, n, axis=0).copy()
+    po.sweep_slots(L, 7, 0, 0.3, 2, np.arange(n) * 32, other_words, rng_mode=LCG)
+    d_same = np.array([(same_word[i] != same_word[i + 1]).sum() for i in range(0, n, 2) if (i // 32) == ((i + 1) // 32)])
+    d_other = np.array([(other_words[i] != other_words[i + 1]).sum() for i in range(0, n, 2)])
+    se = math.sqrt(d_same.var(ddof=1) / d_same.size + d_other.var(ddof=1) / d_other.size)
+    assert abs(d_same.mean() - d_other.mean()) < 5 * se, (d_same.mean(), d_other.mean(), se)
+
+
+def _runs(L, R, betas, theta, seeds, mode):
+    out = []
+    for s in seeds:
+        o = po.Oracle(L, R, s)
+        o.set_rng_mode(mode)
+        out.append(pa_driver.run_fixed(o, betas, theta))
+    return out
+
+
+def test_lcg_pa_run_matches_exact_enumeration_L4():
+    L, R, theta = 4, 4000, 5
+    betas = [i / 40 for i in range(41)]
+    seeds = list(range(200, 212))
+    runs = _runs(L, R, betas, theta, seeds, LCG)
+    for i in (4, 12, 18, 24, 40):
+        exact = ex.exact_small(betas[i], L)
+        for key in ("e", "C", "absm", "m2", "m4", "betaF_per_N", "S_per_N"):
+            vals = np.array([r[i][key] for r in runs])
+            sigma = vals.std(ddof=1) / math.sqrt(len(seeds))
+            assert abs(vals.mean() - exact[key]) < 5 * sigma + 1e-12, (betas[i], key, vals.mean(), exact[key], sigma)
+
+
+def test_lcg_pa_run_matches_kaufman_and_variance_ratio_L16():
+    # configs[0] of BASELINE.json (L=16, R=1000, 100 steps, theta=10) with the LCG-assisted stream: exact finite-L
+    # results (Kaufman) within the seed scatter, and Table 1's last column (L201-L204): the variance of C is the
+    # same as with one Philox number per spin (ratio 1; here 12 + 12 seeds, F-distribution bounds at ~4 sigma)
+    L, R, theta = 16, 1000, 10
+    betas = [i / 100 for i in range(101)]
+    lcg = _runs(L, R, betas, theta, list(range(21, 33)), LCG)
+    phi = _runs(L, R, betas, theta, list(range(41, 53)), po.RNG_PHILOX)
+    for i in (10, 30, 44, 60, 100):
+        k = ex.kaufman(betas[i], L)
+        for key in ("e", "C", "betaF_per_N", "S_per_N"):
+            vals = np.array([r[i][key] for r in lcg])
+            sigma = vals.std(ddof=1) / math.sqrt(len(lcg))
+            assert abs(vals.mean() - k[key]) < 5 * sigma + 1e-9, (betas[i], key, vals.mean(), k[key], sigma)
+    ratios = []
+    for i in range(40, 101, 4):                                        # the critical and low-temperature range of Fig. 2(c)
+        v1 = np.var([r[i]["C"] for r in lcg], ddof=1)
+        v0 = np.var([r[i]["C"] for r in phi], ddof=1)
+        ratios.append(v1 / v0)
+    gm = math.exp(np.mean(np.log(ratios)))                             # geometric mean over 16 temperatures
+    assert 0.4 < gm < 2.5, (gm, ratios)                                # n_RNG = 1 without the LCG would give ~32 (Table 1)
