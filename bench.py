@@ -36,6 +36,10 @@ UNIT = "updates/ns"
 WIDE_MUL_PER_UPDATE = 131.0 / 32.0
 WIDE_MUL_PER_CLK_PER_SM = 32.0
 N_SM = 148
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (theta = 10) from the `ncu --set full` captures
+# summarised in profiles/r01c_summary.md (cfg2) and profiles/r01b_summary.md (cfg5); algorithmic = 2 x population bytes
+# (cfg2: 20.48 MB, the write-back stays in L2; cfg5: 16.38 GB).  Workloads without a capture report null.
+SWEEP_DRAM_BYTES_PER_LAUNCH = {"cfg2_L64_R20000": 10.26e6, "cfg5_L256_R1000000": 16.41e9}
 
 
 def measured_peaks():
@@ -227,10 +231,7 @@ def run_ours(args):
     k_upd = sum(sweep_updates) / len(sweep_updates)
     achieved = WIDE_MUL_PER_UPDATE * k_upd / (k_ms * 1e6)                     # G wide-multiplies / s
     peak = N_SM * WIDE_MUL_PER_CLK_PER_SM * sm_max * 1e-3                      # G wide-multiplies / s at the max SM clock
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "roofline_traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get(wl.name)
+    traffic = SWEEP_DRAM_BYTES_PER_LAUNCH.get(wl.name)
     roofline = {"bound": "alu", "kernel": "pa_sweep_kernel", "achieved": achieved, "peak": peak, "unit": "G IMAD.WIDE.U32/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": f"148 SM x 32/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
                 "kernel_ms": k_ms, "kernel_updates_per_ns": k_upd / (k_ms * 1e6), "share_of_step": sum(sweep_ms) / total_ms,
