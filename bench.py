@@ -142,6 +142,8 @@ def run_ours(args):
     wl = CONFIGS[args.config]
     K, Wm = args.steps, args.warmup
     pop = pa.Population(wl.L, wl.R, rank_seed(wl, rank))
+    if args.rng == "lcg":
+        pop.set_rng_mode(pa.PA_RNG_LCG)
     betas = wl.betas() if wl.n_steps is not None else None
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
     peaks, peak_src = measured_peaks()
@@ -244,7 +246,7 @@ def run_ours(args):
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "u32", "data": "synthetic",
-           "config": {"workload": wl.name, "L": wl.L, "R_per_gpu": wl.R, "theta": wl.theta, "beta_from": wl.beta0,
+           "config": {"workload": wl.name, "L": wl.L, "R_per_gpu": wl.R, "theta": wl.theta, "beta_from": wl.beta0, "rng": args.rng,
                       "schedule": "adaptive" if wl.n_steps is None else f"{wl.n_steps} equal steps to {wl.beta_f}",
                       "l2": "flushed between timed steps (256 MiB memset outside the CUDA events)",
                       "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
@@ -306,6 +308,8 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=sorted(CONFIGS), help="BASELINE.json configs index + 1")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--rng", default="philox", choices=["philox", "lcg"],
+                    help="sweep stream: one Philox number per spin (default, O1) or the paper's Philox-seeded LCG (O11, L236-L241)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -78,6 +78,20 @@ void pa_destroy(pa_t* h);
  * the host (O2; L163).  Advances t by theta.  Asynchronous. */
 int pa_sweep(pa_t* h, double beta, int theta);
 
+/* Source of the SWEEP-stream numbers x (the resampling always uses Philox directly, L241):
+ *   PA_RNG_PHILOX (default; O1): one Philox4x32-10 output word per spin, x(j,s,t,c) =
+ *     philox(s, j>>2, 2t+c, TAG_SWEEP)[j&3]  (Table 1's n_RNG = p rows, L193-L196);
+ *   PA_RNG_LCG (O11; Sec. 4, Table 1's last section): the paper's fast variant.  The word
+ *     of group g at site s = (x,y) is seeded at every visit (sweep t, colour c) with
+ *     r_0 = philox((y>>2)*(L/2) + (x>>1), g, 2t+c, TAG_LCG)[y&3] and its 32 replicas take the next 32
+ *     outputs of r_{n+1} = 1664525 r_n + 1013904223 mod 2^32 (L236), most significant lane first:
+ *     x(32g+b) = r_{32-b}.
+ * Both are functions of (slot, site, sweep) only, so trajectories do not depend on the launch
+ * geometry.  Takes effect from the next pa_sweep.  mode outside {0,1}: PA_ERR_INVALID_ARG. */
+enum { PA_RNG_PHILOX = 0, PA_RNG_LCG = 1 };
+int pa_set_rng_mode(pa_t* h, int mode);
+int pa_get_rng_mode(const pa_t* h);
+
 /* Configurational energies E_j = -sum_<ab> s_a s_b and magnetisations M_j = sum_a s_a of the
  * current replicas j = 0..R_cur-1 (Eq. 10; L173).  E_out, M_out: int32[>= R_cur], host or
  * device; M_out may be NULL.  Synchronises if an output is a host pointer. */

@@ -137,7 +137,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     if (!h) return PA_ERR_NOMEM;
     memset(h, 0, sizeof(*h));
     h->L = L; h->N = L * L; h->R_target = R; h->R_cur = R; h->R_cap = y.R_cap; h->G_cap = y.G_cap;
-    h->seed = seed; h->keys = pa_make_keys(seed);
+    h->seed = seed; h->keys = pa_make_keys(seed); h->rng_mode = PA_RNG_PHILOX;
     h->lnZ = (double)h->N * log(2.0);           // Z_{beta_0} = 2^N (L93)
     h->n_tiles_cap = y.tiles;
     int rc = PA_OK;
@@ -209,6 +209,13 @@ int pa_sweep(pa_t* h, double beta, int theta) {
     h->em_valid = false; h->host_scal_valid = false;
     return PA_OK;
 }
+
+int pa_set_rng_mode(pa_t* h, int mode) {
+    if (!h || (mode != PA_RNG_PHILOX && mode != PA_RNG_LCG)) return PA_ERR_INVALID_ARG;
+    h->rng_mode = mode;
+    return PA_OK;
+}
+int pa_get_rng_mode(const pa_t* h) { return h ? h->rng_mode : PA_ERR_INVALID_ARG; }
 
 int pa_energies(pa_t* h, int32_t* E_out, int32_t* M_out) {
     if (!h || !E_out) return PA_ERR_INVALID_ARG;

@@ -17,6 +17,10 @@
 #define PA_TAG_INIT 0u
 #define PA_TAG_SWEEP 1u
 #define PA_TAG_RESAMPLE 2u
+#define PA_TAG_LCG 3u
+
+#define PA_LCG_A 1664525u      // L236, ref. [43]
+#define PA_LCG_C 1013904223u
 
 #define PA_PHILOX_M0 0xD2511F53u
 #define PA_PHILOX_M1 0xCD9E8D57u
@@ -79,6 +83,7 @@ struct pa_handle {
     int64_t G_cap;           // groups at capacity
     uint64_t seed;
     uint32_t t, k;
+    int rng_mode;            // PA_RNG_PHILOX / PA_RNG_LCG (O11)
     double lnZ, lnQ_last;
     PhiloxKeys keys;
 

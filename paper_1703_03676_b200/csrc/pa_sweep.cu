@@ -138,7 +138,31 @@ __device__ __forceinline__ uint32_t pa_flip_mask(uint32_t s, uint32_t n0, uint32
     return U2 | acc;
 }
 
-template <int CMP, bool CLUSTER>
+// LCG-assisted stream (O11; Sec. 4): the 32 lanes of the word take the next 32 outputs of
+// r <- 1664525 r + 1013904223 (mod 2^32), most significant lane first (the first output is shifted in first and
+// ends up in bit 31).  One 32-bit IMAD (FMA pipe, 2 cycles) per lane replaces a quarter of a Philox call
+// (5 IMAD.WIDE + 5 LOP3); the acceptance test is the same carry-out compare with the shift-in on the FMA pipe.
+__device__ __forceinline__ uint32_t pa_flip_mask_lcg(uint32_t s, uint32_t n0, uint32_t n1, uint32_t n2, uint32_t n3,
+                                                     uint32_t r, const SweepParams& P) {
+    uint32_t a0 = s ^ n0, a1 = s ^ n1, a2 = s ^ n2, a3 = s ^ n3;
+    uint32_t U1 = a0 | a1 | a2 | a3;                                   // u >= 1
+    uint32_t U2 = (a0 & a1) | (a2 & a3) | ((a0 ^ a1) & (a2 ^ a3));     // u >= 2: always flips
+    uint32_t g4 = 0, g8 = 0;                                           // bit b = (x_b >= T)
+#pragma unroll
+    for (int b = 31; b >= 0; --b) {
+        r = r * PA_LCG_A + PA_LCG_C;
+        pa_shift_in_ge(g4, r, P.T4, P.two);
+        pa_shift_in_ge(g8, r, P.T8, P.two);
+    }
+    return U2 | (~g4 & (U1 | ~g8));                                    // u >= 2, or x < T4 and (u >= 1 or x < T8)
+}
+
+// The four LCG seeds of a quad of rows (y & ~3 .. +3) in column xh of one sub-lattice: one Philox call (O11).
+__device__ __forceinline__ uint4 pa_lcg_seeds(uint32_t quad, uint32_t g, uint32_t c2, const PhiloxKeys& K) {
+    return pa_philox(quad, g, c2, PA_TAG_LCG, K);
+}
+
+template <int CMP, bool CLUSTER, int RNG>
 __global__ void __launch_bounds__(256)
 pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
@@ -201,8 +225,15 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                 uint32_t nU, nD;
                 if (yl > 0) nU = oth[row - Lh + xh]; else nU = up_oth[(H - 1) * Lh + xh];
                 if (yl < H - 1) nD = oth[row + Lh + xh]; else nD = dn_oth[xh];
-                const uint32_t site = (uint32_t)(y * L + 2 * xh + p);
-                const uint32_t flip = pa_flip_mask<CMP>(s, nS, nX, nU, nD, site, c0base, lo1u, P);
+                uint32_t flip;
+                if (RNG == PA_RNG_LCG) {
+                    const uint4 sd = pa_lcg_seeds((uint32_t)((y >> 2) * Lh + xh), (uint32_t)g, c2, P.K);
+                    const int q = y & 3;
+                    flip = pa_flip_mask_lcg(s, nS, nX, nU, nD, q == 0 ? sd.x : q == 1 ? sd.y : q == 2 ? sd.z : sd.w, P);
+                } else {
+                    const uint32_t site = (uint32_t)(y * L + 2 * xh + p);
+                    flip = pa_flip_mask<CMP>(s, nS, nX, nU, nD, site, c0base, lo1u, P);
+                }
                 mine[row + xh] = s ^ flip;
                 xh += dx; yl += dy;
                 if (xh >= Lh) { xh -= Lh; yl += 1; }
@@ -313,6 +344,89 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Column-walk kernel for the LCG-assisted stream (O11): the same strip / cluster layout, but a thread walks
+// FOUR rows per iteration -- the quad of rows that shares one Philox call for its four LCG seeds.  The six
+// vertical-neighbour words of the quad are loaded once.  Requirements (pa_col_ok): as above and rows per thread
+// a multiple of 4, strip height a multiple of 4.
+// ------------------------------------------------------------------------------------------------
+template <int LOG_LH, bool CLUSTER>
+__global__ void PA_SWEEP_BOUNDS
+pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
+    extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
+    constexpr int Lh = 1 << LOG_LH;
+    const int T = blockDim.x, tid = threadIdx.x;
+    const int C = CLUSTER ? P.C : 1;
+    unsigned cr = 0;
+    if (CLUSTER) cr = cg::this_cluster().block_rank();
+    const long long g = blockIdx.x / C;
+    const int H = P.H;
+    const int y0 = (int)cr * H;
+    const int half = H * Lh;
+    uint32_t* gbase = pop + g * (long long)P.N;
+    const int goff = y0 * Lh, gcol = P.N >> 1;
+
+    for (int c = 0; c < 2; ++c) {
+        const uint4* src = reinterpret_cast<const uint4*>(gbase + c * gcol + goff);
+        uint4* dst = reinterpret_cast<uint4*>(tile + c * half);
+        for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+    }
+    const uint32_t* up_tile = tile;
+    const uint32_t* dn_tile = tile;
+    if (CLUSTER) {
+        cg::cluster_group cl = cg::this_cluster();
+        up_tile = cl.map_shared_rank(tile, (cr + C - 1) % C);
+        dn_tile = cl.map_shared_rank(tile, (cr + 1) % C);
+        cl.sync();
+    } else {
+        __syncthreads();
+    }
+
+    const int xh = tid & (Lh - 1), rb = tid >> LOG_LH;
+    const int rpt = half / T;                          // rows per thread: multiple of 4
+    const int ya = rb * rpt;                           // first local row (multiple of 4)
+    const int dL = ((xh - 1) & (Lh - 1)) - xh, dR = ((xh + 1) & (Lh - 1)) - xh;
+    const int b0 = ya * Lh + xh;
+    const uint32_t quad_base = (uint32_t)(((y0 + ya) >> 2) * Lh + xh);
+    for (int it = 0; it < P.theta; ++it) {
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t c2 = 2u * (P.t0 + (uint32_t)it) + (uint32_t)c;
+            uint32_t* mine = tile + c * half + b0;
+            const uint32_t* oth = tile + (1 - c) * half + b0;
+            // rows y0+ya+2k have x-parity p = c (x = 2 xh + c), rows y0+ya+2k+1 have p = 1 - c
+            const int dA = c ? dR : dL, dB = c ? dL : dR;
+            uint32_t quad = quad_base;
+#pragma unroll 1
+            for (int k = 0; k < rpt; k += 4) {
+                const uint4 sd = pa_lcg_seeds(quad, (uint32_t)g, c2, P.K);
+                const uint32_t s0 = mine[0], s1 = mine[Lh], s2 = mine[2 * Lh], s3 = mine[3 * Lh];
+                const uint32_t o0 = oth[0], o1 = oth[Lh], o2 = oth[2 * Lh], o3 = oth[3 * Lh];
+                const uint32_t x0 = oth[dA], x1 = oth[Lh + dB], x2 = oth[2 * Lh + dA], x3 = oth[3 * Lh + dB];
+                uint32_t oU, oD;
+                if (ya + k > 0) oU = oth[-Lh]; else oU = up_tile[(1 - c) * half + (H - 1) * Lh + xh];
+                if (ya + k + 4 < H) oD = oth[4 * Lh]; else oD = dn_tile[(1 - c) * half + xh];
+                const uint32_t f0 = pa_flip_mask_lcg(s0, o0, x0, oU, o1, sd.x, P);
+                const uint32_t f1 = pa_flip_mask_lcg(s1, o1, x1, o0, o2, sd.y, P);
+                const uint32_t f2 = pa_flip_mask_lcg(s2, o2, x2, o1, o3, sd.z, P);
+                const uint32_t f3 = pa_flip_mask_lcg(s3, o3, x3, o2, oD, sd.w, P);
+                mine[0] = s0 ^ f0;
+                mine[Lh] = s1 ^ f1;
+                mine[2 * Lh] = s2 ^ f2;
+                mine[3 * Lh] = s3 ^ f3;
+                mine += 4 * Lh; oth += 4 * Lh; quad += Lh;
+            }
+            if (CLUSTER) cg::this_cluster().sync(); else __syncthreads();
+        }
+    }
+
+    for (int c = 0; c < 2; ++c) {
+        uint4* dst = reinterpret_cast<uint4*>(gbase + c * gcol + goff);
+        const uint4* src = reinterpret_cast<const uint4*>(tile + c * half);
+        for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
 static int pa_env_int(const char* name, int dflt) {
@@ -324,10 +438,11 @@ static int pa_env_int(const char* name, int dflt) {
 // colours, L*L*4/C bytes) fits the shared-memory budget per CTA; threads = min(256, words per colour).
 // kind 1 = column-walk kernel (power-of-two L >= 64), kind 0 = generic kernel (any even L).
 // Environment overrides (tests, tuning): PA_SWEEP_C, PA_SWEEP_T, PA_SWEEP_KIND, PA_SWEEP_CMP, PA_SWEEP_SMEM_KB.
-static bool pa_col_ok(int L, int C, int T) {
+static bool pa_col_ok(int L, int C, int T, int rng_mode = PA_RNG_PHILOX) {
     if ((L & (L - 1)) != 0 || L < 64 || L % C != 0) return false;
     const int Lh = L / 2, H = L / C, half = H * Lh;
-    return (H & 1) == 0 && T >= Lh && (T & (T - 1)) == 0 && half % T == 0 && half / T >= 2 && ((half / T) & 1) == 0;
+    const int q = rng_mode == PA_RNG_LCG ? 4 : 2;          // rows per iteration of the column walk
+    return H % q == 0 && T >= Lh && (T & (T - 1)) == 0 && half % T == 0 && half / T >= q && (half / T) % q == 0;
 }
 
 int pa_sweep_configure(pa_handle* h) {
@@ -363,10 +478,11 @@ static int pa_sweep_pick_C(const pa_handle* h, int64_t G) {
     const int L = h->L;
     double best = -1.0; int bestC = Cmin;
     for (int C = Cmin; C <= 8; C *= 2) {
-        if (!pa_col_ok(L, C, h->sweep_T)) break;
+        if (!pa_col_ok(L, C, h->sweep_T, h->rng_mode)) break;
         const size_t smem = (size_t)L * L * 4 / C;
         int per_sm = (int)((227 * 1024) / (smem + 1024));
-        if (per_sm > 3) per_sm = 3;                        // 80 registers x 256 threads
+        const int reg_limit = h->rng_mode == PA_RNG_LCG ? 6 : 3;   // 80 (Philox) / <= 40 (LCG) registers x 256 threads
+        if (per_sm > reg_limit) per_sm = reg_limit;
         if (per_sm < 1) per_sm = 1;
         const double slots = (C >= 4 ? 132.0 : 148.0) * per_sm;
         const double waves = (double)G * C / slots;
@@ -397,6 +513,21 @@ static cudaError_t pa_sweep_launch_k(pa_handle* h, Kern kern, const SweepParams&
     return cudaLaunchKernelEx(&cfg, kern, h->spins[h->cur], P);
 }
 
+static cudaError_t pa_sweep_dispatch_lcg(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
+    const bool cl = P.C > 1;
+    if (h->sweep_kind == 1 && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG)) {
+        switch (P.Lh) {
+#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, true>, P, smem, grid, true) \
+                                                      : pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, false>, P, smem, grid, false);
+            PA_COL_CASE(5) PA_COL_CASE(6) PA_COL_CASE(7) PA_COL_CASE(8)
+#undef PA_COL_CASE
+            default: break;
+        }
+    }
+    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_LCG>, P, smem, grid, true)
+              : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_LCG>, P, smem, grid, false);
+}
+
 template <int CMP>
 static cudaError_t pa_sweep_dispatch(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
     const bool cl = P.C > 1;
@@ -409,8 +540,8 @@ static cudaError_t pa_sweep_dispatch(pa_handle* h, const SweepParams& P, size_t 
             default: break;
         }
     }
-    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<CMP, true>, P, smem, grid, true)
-              : pa_sweep_launch_k(h, pa_sweep_kernel<CMP, false>, P, smem, grid, false);
+    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<CMP, true, PA_RNG_PHILOX>, P, smem, grid, true)
+              : pa_sweep_launch_k(h, pa_sweep_kernel<CMP, false, PA_RNG_PHILOX>, P, smem, grid, false);
 }
 
 int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
@@ -424,7 +555,8 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     const size_t smem = (size_t)P.H * h->L * 4;
     const unsigned grid = (unsigned)(G * P.C);
     const int v = h->sweep_cmp;
-    const cudaError_t e = v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)
+    const cudaError_t e = h->rng_mode == PA_RNG_LCG ? pa_sweep_dispatch_lcg(h, P, smem, grid)
+                        : v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)
                                                                                     : pa_sweep_dispatch<0>(h, P, smem, grid);
     PA_CUDA(h, e);
     h->launches += 1;

@@ -21,6 +21,7 @@ LIB_PATH = os.path.join(HERE, "libpa_b200.so")
 HEADER = os.path.join(os.path.dirname(HERE), "include", "pa.h")
 
 PA_OK, PA_ERR_INVALID_ARG, PA_ERR_CAPACITY, PA_ERR_CUDA, PA_ERR_WORKSPACE, PA_ERR_NOMEM = 0, -1, -2, -3, -4, -5
+PA_RNG_PHILOX, PA_RNG_LCG = 0, 1
 
 
 class PaError(RuntimeError):
@@ -65,6 +66,8 @@ def lib():
         "pa_create_ex": ([i32, i64, u64, vp, sz, vp, C.POINTER(vp)], i32),
         "pa_destroy": ([vp], None),
         "pa_sweep": ([vp, dbl, i32], i32),
+        "pa_set_rng_mode": ([vp, i32], i32),
+        "pa_get_rng_mode": ([vp], i32),
         "pa_energies": ([vp, vp, vp], i32),
         "pa_resample": ([vp, dbl, dbl, C.POINTER(i64)], i32),
         "pa_adapt_dbeta": ([vp, dbl, dbl, dbl, C.POINTER(dbl)], i32),
@@ -221,6 +224,13 @@ class Population:
         self._check(lib().pa_set_counters(self._h, t, k, float(lnZ)), "pa_set_counters")
 
     # the path
+    def set_rng_mode(self, mode):
+        self._check(lib().pa_set_rng_mode(self._h, int(mode)), "pa_set_rng_mode")
+
+    @property
+    def rng_mode(self):
+        return int(lib().pa_get_rng_mode(self._h))
+
     def sweep(self, beta, theta):
         self._check(lib().pa_sweep(self._h, float(beta), int(theta)), "pa_sweep")
 

@@ -70,6 +70,55 @@ def test_sweep_bit_exact(L, R):
         assert_same_state(g, o)
 
 
+@pytest.mark.parametrize("L,R", [(4, 40), (6, 70), (10, 33), (16, 200), (32, 100), (64, 96), (128, 64), (256, 40)])
+def test_sweep_lcg_mode_bit_exact(L, R):
+    """LCG-assisted stream (O11): generic kernel (L < 64 or not a power of two) and the
+    quad-row column-walk kernel, ragged last group, switching modes between calls."""
+    seed = 2000 + L
+    g, o = pa.Population(L, R, seed), po.Oracle(L, R, seed)
+    g.set_rng_mode(pa.PA_RNG_LCG); o.set_rng_mode(po.RNG_LCG)
+    assert g.rng_mode == pa.PA_RNG_LCG
+    for beta, theta in [(0.0, 1), (0.3, 2), (0.4406868, 3), (1.0, 1), (0.7, 0)]:
+        g.sweep(beta, theta); o.sweep(beta, theta)
+        assert_same_state(g, o)
+    g.set_rng_mode(pa.PA_RNG_PHILOX); o.set_rng_mode(po.RNG_PHILOX)
+    g.sweep(0.5, 1); o.sweep(0.5, 1)
+    assert_same_state(g, o)
+    rc = pa.lib().pa_set_rng_mode(g._h, 2)
+    assert rc == pa.PA_ERR_INVALID_ARG and g.rng_mode == pa.PA_RNG_PHILOX
+
+
+def test_sweep_lcg_mode_geometries(monkeypatch):
+    """Same bytes for every launch geometry (clusters of 1/2/4/8 CTAs with DSMEM halos, 128/256 threads), all
+    equal to the oracle."""
+    L, R, seed = 64, 130, 77
+    o = po.Oracle(L, R, seed); o.set_rng_mode(po.RNG_LCG)
+    o.sweep(0.42, 3)
+    want = o.get_spins()
+    for env in ({}, {"PA_SWEEP_C": "2"}, {"PA_SWEEP_C": "4", "PA_SWEEP_T": "128"}, {"PA_SWEEP_C": "8", "PA_SWEEP_T": "64"},
+                {"PA_SWEEP_C": "4"}, {"PA_SWEEP_KIND": "0"}, {"PA_SWEEP_KIND": "0", "PA_SWEEP_C": "2", "PA_SWEEP_T": "96"}):
+        for k in ("PA_SWEEP_C", "PA_SWEEP_T", "PA_SWEEP_KIND"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        g = pa.Population(L, R, seed); g.set_rng_mode(pa.PA_RNG_LCG)
+        g.sweep(0.42, 3)
+        assert np.array_equal(g.get_spins(), want), env
+
+
+def test_lcg_mode_whole_run_config1():
+    """configs[0] (L=16, R=1000, 100 steps, theta=10) with the LCG-assisted sweeps: every step bit-exact."""
+    wl = CONFIGS[1]
+    g, o = pa.Population(wl.L, wl.R, wl.seed), po.Oracle(wl.L, wl.R, wl.seed)
+    g.set_rng_mode(pa.PA_RNG_LCG); o.set_rng_mode(po.RNG_LCG)
+    betas = wl.betas()
+    og = pa_driver.run_fixed(g, betas, wl.theta, on_step=lambda i, p: None)
+    oo = pa_driver.run_fixed(o, betas, wl.theta)
+    for a, b in zip(og, oo):
+        assert_obs_close(a, b)
+    assert_same_state(g, o)
+
+
 def test_sweep_split_calls_and_special_states():
     L, R = 16, 64
     g, o = pa.Population(L, R, 9), po.Oracle(L, R, 9)
