@@ -142,19 +142,36 @@ __device__ __forceinline__ uint32_t pa_flip_mask(uint32_t s, uint32_t n0, uint32
 // r <- 1664525 r + 1013904223 (mod 2^32), most significant lane first (the first output is shifted in first and
 // ends up in bit 31).  One 32-bit IMAD (FMA pipe, 2 cycles) per lane replaces a quarter of a Philox call
 // (5 IMAD.WIDE + 5 LOP3); the acceptance test is the same carry-out compare with the shift-in on the FMA pipe.
+// r <- A r + C as ONE multiply-add: written in PTX so that the compiler cannot re-associate the recurrence into
+// s <- A s + C', x = s + C'' (it does, which costs an extra ALU-pipe add per lane).
+__device__ __forceinline__ uint32_t pa_lcg_step(uint32_t r) {
+    uint32_t o;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(o) : "r"(r), "n"(PA_LCG_A), "n"(PA_LCG_C));
+    return o;
+}
+
+// NOR = number of leading lanes (31, 30, ...) whose two threshold tests run on the ALU pipe alone (ISETP +
+// predicated OR) instead of carry-out IADD3 (ALU) + IMAD.X (FMA): balances the two pipes.
+template <int NOR>
 __device__ __forceinline__ uint32_t pa_flip_mask_lcg(uint32_t s, uint32_t n0, uint32_t n1, uint32_t n2, uint32_t n3,
                                                      uint32_t r, const SweepParams& P) {
     uint32_t a0 = s ^ n0, a1 = s ^ n1, a2 = s ^ n2, a3 = s ^ n3;
     uint32_t U1 = a0 | a1 | a2 | a3;                                   // u >= 1
     uint32_t U2 = (a0 & a1) | (a2 & a3) | ((a0 ^ a1) & (a2 ^ a3));     // u >= 2: always flips
-    uint32_t g4 = 0, g8 = 0;                                           // bit b = (x_b >= T)
+    uint32_t m4 = 0, m8 = 0;                                           // bit b = (x_b <  T), lanes 31 .. 32-NOR
+    uint32_t g4 = 0, g8 = 0;                                           // bit b = (x_b >= T), lanes 31-NOR .. 0
+#define PA_LCG_OR(B) if (NOR > 31 - (B)) { r = pa_lcg_step(r); pa_or_if_lt<(1u << (B))>(m4, r, P.T4); pa_or_if_lt<(1u << (B))>(m8, r, P.T8); }
+    PA_LCG_OR(31) PA_LCG_OR(30) PA_LCG_OR(29) PA_LCG_OR(28) PA_LCG_OR(27) PA_LCG_OR(26) PA_LCG_OR(25) PA_LCG_OR(24)
+#undef PA_LCG_OR
 #pragma unroll
-    for (int b = 31; b >= 0; --b) {
-        r = r * PA_LCG_A + PA_LCG_C;
+    for (int b = 31 - NOR; b >= 0; --b) {
+        r = pa_lcg_step(r);
         pa_shift_in_ge(g4, r, P.T4, P.two);
         pa_shift_in_ge(g8, r, P.T8, P.two);
     }
-    return U2 | (~g4 & (U1 | ~g8));                                    // u >= 2, or x < T4 and (u >= 1 or x < T8)
+    constexpr uint32_t LOW = NOR == 0 ? 0xffffffffu : (0xffffffffu >> (NOR & 31));
+    const uint32_t lt4 = (~g4 & LOW) | m4, lt8 = (~g8 & LOW) | m8;
+    return U2 | (lt4 & (U1 | lt8));                                    // u >= 2, or x < T4 and (u >= 1 or x < T8)
 }
 
 // The four LCG seeds of a quad of rows (y & ~3 .. +3) in column xh of one sub-lattice: one Philox call (O11).
@@ -229,7 +246,7 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                 if (RNG == PA_RNG_LCG) {
                     const uint4 sd = pa_lcg_seeds((uint32_t)((y >> 2) * Lh + xh), (uint32_t)g, c2, P.K);
                     const int q = y & 3;
-                    flip = pa_flip_mask_lcg(s, nS, nX, nU, nD, q == 0 ? sd.x : q == 1 ? sd.y : q == 2 ? sd.z : sd.w, P);
+                    flip = pa_flip_mask_lcg<0>(s, nS, nX, nU, nD, q == 0 ? sd.x : q == 1 ? sd.y : q == 2 ? sd.z : sd.w, P);
                 } else {
                     const uint32_t site = (uint32_t)(y * L + 2 * xh + p);
                     flip = pa_flip_mask<CMP>(s, nS, nX, nU, nD, site, c0base, lo1u, P);
@@ -349,7 +366,7 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 // vertical-neighbour words of the quad are loaded once.  Requirements (pa_col_ok): as above and rows per thread
 // a multiple of 4, strip height a multiple of 4.
 // ------------------------------------------------------------------------------------------------
-template <int LOG_LH, bool CLUSTER>
+template <int LOG_LH, bool CLUSTER, int NOR>
 __global__ void PA_SWEEP_BOUNDS
 pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
@@ -405,10 +422,10 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                 uint32_t oU, oD;
                 if (ya + k > 0) oU = oth[-Lh]; else oU = up_tile[(1 - c) * half + (H - 1) * Lh + xh];
                 if (ya + k + 4 < H) oD = oth[4 * Lh]; else oD = dn_tile[(1 - c) * half + xh];
-                const uint32_t f0 = pa_flip_mask_lcg(s0, o0, x0, oU, o1, sd.x, P);
-                const uint32_t f1 = pa_flip_mask_lcg(s1, o1, x1, o0, o2, sd.y, P);
-                const uint32_t f2 = pa_flip_mask_lcg(s2, o2, x2, o1, o3, sd.z, P);
-                const uint32_t f3 = pa_flip_mask_lcg(s3, o3, x3, o2, oD, sd.w, P);
+                const uint32_t f0 = pa_flip_mask_lcg<NOR>(s0, o0, x0, oU, o1, sd.x, P);
+                const uint32_t f1 = pa_flip_mask_lcg<NOR>(s1, o1, x1, o0, o2, sd.y, P);
+                const uint32_t f2 = pa_flip_mask_lcg<NOR>(s2, o2, x2, o1, o3, sd.z, P);
+                const uint32_t f3 = pa_flip_mask_lcg<NOR>(s3, o3, x3, o2, oD, sd.w, P);
                 mine[0] = s0 ^ f0;
                 mine[Lh] = s1 ^ f1;
                 mine[2 * Lh] = s2 ^ f2;
@@ -513,15 +530,27 @@ static cudaError_t pa_sweep_launch_k(pa_handle* h, Kern kern, const SweepParams&
     return cudaLaunchKernelEx(&cfg, kern, h->spins[h->cur], P);
 }
 
+template <int NOR>
+static cudaError_t pa_sweep_dispatch_lcg_col(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
+    const bool cl = P.C > 1;
+    switch (P.Lh) {
+#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, true, NOR>, P, smem, grid, true) \
+                                                  : pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, false, NOR>, P, smem, grid, false);
+        PA_COL_CASE(5) PA_COL_CASE(6) PA_COL_CASE(7) PA_COL_CASE(8)
+#undef PA_COL_CASE
+        default: return cudaErrorInvalidValue;
+    }
+}
+
 static cudaError_t pa_sweep_dispatch_lcg(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
     const bool cl = P.C > 1;
-    if (h->sweep_kind == 1 && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG)) {
-        switch (P.Lh) {
-#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, true>, P, smem, grid, true) \
-                                                      : pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, false>, P, smem, grid, false);
-            PA_COL_CASE(5) PA_COL_CASE(6) PA_COL_CASE(7) PA_COL_CASE(8)
-#undef PA_COL_CASE
-            default: break;
+    if (h->sweep_kind == 1 && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG) && P.Lh >= 32 && P.Lh <= 256) {
+        switch (pa_env_int("PA_LCG_NOR", 4)) {       // tuning knob; every value gives the same bytes
+            case 0: return pa_sweep_dispatch_lcg_col<0>(h, P, smem, grid);
+            case 2: return pa_sweep_dispatch_lcg_col<2>(h, P, smem, grid);
+            case 6: return pa_sweep_dispatch_lcg_col<6>(h, P, smem, grid);
+            case 8: return pa_sweep_dispatch_lcg_col<8>(h, P, smem, grid);
+            default: return pa_sweep_dispatch_lcg_col<4>(h, P, smem, grid);
         }
     }
     return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_LCG>, P, smem, grid, true)
