@@ -36,6 +36,8 @@ UNIT = "updates/ns"
 WIDE_MUL_PER_UPDATE = 131.0 / 32.0
 WIDE_MUL_PER_CLK_PER_SM = 32.0
 N_SM = 148
+LCG_INSTR_PER_UPDATE = 5.0
+ISSUE_LANES_PER_CLK_PER_SM = 128.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (theta = 10) from the `ncu --set full` captures
 # summarised in profiles/r01c_summary.md (cfg2) and profiles/r01b_summary.md (cfg5); algorithmic = 2 x population bytes
 # (cfg2: 20.48 MB, the write-back stays in L2; cfg5: 16.38 GB).  Workloads without a capture report null.
@@ -231,13 +233,20 @@ def run_ours(args):
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     k_ms = sum(sweep_ms) / len(sweep_ms)
     k_upd = sum(sweep_updates) / len(sweep_updates)
-    achieved = WIDE_MUL_PER_UPDATE * k_upd / (k_ms * 1e6)                     # G wide-multiplies / s
-    peak = N_SM * WIDE_MUL_PER_CLK_PER_SM * sm_max * 1e-3                      # G wide-multiplies / s at the max SM clock
-    traffic = SWEEP_DRAM_BYTES_PER_LAUNCH.get(wl.name)
-    roofline = {"bound": "alu", "kernel": "pa_sweep_kernel", "achieved": achieved, "peak": peak, "unit": "G IMAD.WIDE.U32/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": f"148 SM x 32/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
+    if args.rng == "lcg":
+        # LCG-assisted stream: 5 thread instructions per update are the method's own (one multiply-add
+        # of the LCG, two threshold tests, two mask inserts); the binding resource is instruction issue, 4 x 32 lanes/clk/SM.
+        per_upd, per_clk, unit, kname = LCG_INSTR_PER_UPDATE, ISSUE_LANES_PER_CLK_PER_SM, "G thread-instructions/s", "pa_sweep_lcg_kernel"
+        traffic = None
+    else:
+        per_upd, per_clk, unit, kname = WIDE_MUL_PER_UPDATE, WIDE_MUL_PER_CLK_PER_SM, "G IMAD.WIDE.U32/s", "pa_sweep_col_kernel"
+        traffic = SWEEP_DRAM_BYTES_PER_LAUNCH.get(wl.name)
+    achieved = per_upd * k_upd / (k_ms * 1e6)                                  # G units / s
+    peak = N_SM * per_clk * sm_max * 1e-3                                      # G units / s at the max SM clock
+    roofline = {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": unit,
+                "frac": achieved / peak, "traffic": traffic, "peak_source": f"148 SM x {per_clk:.0f}/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
                 "kernel_ms": k_ms, "kernel_updates_per_ns": k_upd / (k_ms * 1e6), "share_of_step": sum(sweep_ms) / total_ms,
-                "algorithmic_per_update": WIDE_MUL_PER_UPDATE}
+                "algorithmic_per_update": per_upd}
     cms = sum(copy_ms) / len(copy_ms)
     resample = {"ms_per_step": sum(res_ms) / len(res_ms), "copy_kernel_ms": cms,
                 "copy_gbs": (sum(copy_bytes) / len(copy_bytes)) / (cms * 1e6) if cms > 0 else None,
@@ -252,16 +261,18 @@ def run_ours(args):
                       "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "resample": resample,
            "last_observables": obs}
-    out["cpu_baseline"] = cpu_baseline(wl) if world == 1 and not args.no_cpu else None
+    out["cpu_baseline"] = cpu_baseline(wl, args.rng) if world == 1 and not args.no_cpu else None
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
 
-def oracle_step_rate(wl, R_sample, steps, warmup):
+def oracle_step_rate(wl, R_sample, steps, warmup, rng="philox"):
     """The oracle, as it stands, on a population of R_sample replicas of the workload's shape."""
     from oracle import pa_oracle as po
     o = po.Oracle(wl.L, R_sample, wl.seed)
+    if rng == "lcg":
+        o.set_rng_mode(po.RNG_LCG)
     betas = wl.betas() if wl.n_steps is not None else [wl.beta0 + 0.005 * i for i in range(steps + warmup + 2)]
     i, beta_prev = 0, betas[0]
     for _ in range(warmup):
@@ -276,9 +287,9 @@ def oracle_step_rate(wl, R_sample, steps, warmup):
     return upd / (dt * 1e9), dt / steps * 1e3, po.num_threads()
 
 
-def cpu_baseline(wl):
+def cpu_baseline(wl, rng="philox"):
     R_s = min(wl.R, max(256, int(1.0e9 / (wl.N * wl.theta))))               # ~1e9 spin updates of CPU work
-    v, ms, cores = oracle_step_rate(wl, R_s, 1, 0)
+    v, ms, cores = oracle_step_rate(wl, R_s, 1, 0, rng)
     return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": ms,
             "sample": f"one temperature step (resample + {wl.theta} sweeps + observables) of R={R_s} replicas, L={wl.L}, oracle/pa_oracle.cpp -O2 OpenMP"}
 
@@ -288,7 +299,7 @@ def run_reference(args):
         return
     wl = CONFIGS[args.config]
     R_s = min(wl.R, max(256, int(2.0e8 / (wl.N * wl.theta))))               # bounded sample per step
-    v, ms, cores = oracle_step_rate(wl, R_s, args.steps, args.warmup)
+    v, ms, cores = oracle_step_rate(wl, R_s, args.steps, args.warmup, args.rng)
     sample = f"each step = one temperature step of R={R_s} replicas of {wl.name} (L={wl.L}, theta={wl.theta}); CPU oracle, OpenMP"
     out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",

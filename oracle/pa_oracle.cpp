@@ -24,6 +24,10 @@
 //   observables (O8) ..... L=4 exact enumeration, Kaufman e and C at L=16 (4 sigma over seeds)
 //   multi-histogram (O9) . sum H = R_i, sum H*E = SE, ln Omega vs exact ln g(E) at L=4
 //   adaptive step (O10) .. alpha(0) closed form, monotonicity, bracket property
+//   reweighting (O12) .... exact g(E) of the 4x4 torus in, exact enumeration averages out; Kaufman
+//                          e, C, lnZ at off-grid beta from L=16 runs (5 sigma over seeds)
+//   weighted averages (O13) closed forms (weight ratios, M = 1, equal F, shift invariance, dominance);
+//                          unbiasedness of exp(lnZ_m) and removal of the small-R bias at L=4 (L99)
 //   LCG-assisted stream (O11) recurrence against big-integer arithmetic with the constants the
 //                          paper prints (L236); the same L=4 Boltzmann chi^2, global-flip symmetry
 //                          and Kaufman pins as the Philox-per-spin sweep; variance ratio of C
@@ -317,6 +321,38 @@ void hist_fold_for(const std::vector<int32_t>& E, int N, double lnZ, double beta
     }
 }
 
+// O12, Sec. 2.4: what Eq. 9 is for.  ln Omega(E_m) = ln Hsum[m] - lnD[m] where Hsum[m] > 0 (Eq. 9 in the log
+// domain), and canonical averages at ANY beta follow from the density of states by the textbook sums
+//   Z(beta) = sum_m Omega_m exp(-beta E_m),  <E^k> = sum_m E_m^k Omega_m exp(-beta E_m) / Z,
+// evaluated with the largest exponent taken out; the variance is summed about the mean (two passes).
+//   e = <E>/N,  C = beta^2 (<E^2> - <E>^2)/N  (Eq. 3),  ln Z = -beta F (Eq. 4).
+void reweight_for(int N, const int64_t* Hsum, const double* lnD, double beta, double* lnZ, double* e, double* C) {
+    const double ninf = -std::numeric_limits<double>::infinity();
+    double amax = ninf;
+    for (int m = 0; m <= N; ++m) {
+        if (Hsum[m] <= 0) continue;
+        double a = (std::log((double)Hsum[m]) - lnD[m]) - beta * (double)(-2 * N + 4 * m);
+        if (a > amax) amax = a;
+    }
+    double S0 = 0.0, S1 = 0.0;
+    for (int m = 0; m <= N; ++m) {
+        if (Hsum[m] <= 0) continue;
+        double Em = (double)(-2 * N + 4 * m);
+        double p = std::exp(((std::log((double)Hsum[m]) - lnD[m]) - beta * Em) - amax);
+        S0 += p; S1 += Em * p;
+    }
+    double mean = S1 / S0, S2 = 0.0;
+    for (int m = 0; m <= N; ++m) {
+        if (Hsum[m] <= 0) continue;
+        double Em = (double)(-2 * N + 4 * m);
+        double p = std::exp(((std::log((double)Hsum[m]) - lnD[m]) - beta * Em) - amax);
+        S2 += (Em - mean) * (Em - mean) * p;
+    }
+    *lnZ = amax + std::log(S0);
+    *e = mean / (double)N;
+    *C = beta * beta * (S2 / S0) / (double)N;
+}
+
 }  // namespace
 
 extern "C" {
@@ -418,6 +454,36 @@ int ora_hist_fold_of(int L, int64_t R_cur, const int32_t* E, double lnZ, double 
     if (L < 4 || (L & 1) || R_cur < 1 || !Hsum || !lnD) return ORA_ERR_INVALID_ARG;
     std::vector<int32_t> Ev(E, E + R_cur);
     hist_fold_for(Ev, L * L, lnZ, beta, Hsum, lnD);
+    return ORA_OK;
+}
+
+// O12 from the accumulated sums alone: lnZ, e, C at every beta of a grid
+int ora_reweight_of(int L, const int64_t* Hsum, const double* lnD, int n, const double* betas,
+                    double* lnZ, double* e, double* C) {
+    if (L < 4 || (L & 1) || !Hsum || !lnD || n < 0) return ORA_ERR_INVALID_ARG;
+    bool any = false;
+    for (int m = 0; m <= L * L; ++m) any = any || Hsum[m] > 0;
+    if (!any) return ORA_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i) reweight_for(L * L, Hsum, lnD, betas[i], &lnZ[i], &e[i], &C[i]);
+    return ORA_OK;
+}
+
+// O13, Sec. 2.2 Eq. 6-7 (L99-L109): weighted average of M independent runs,
+//   omega_m = exp(-beta F_m) / sum_m exp(-beta F_m) with -beta F_m = lnZ_m (Eq. 4), A~ = sum_m omega_m A_m,
+// the largest lnZ_m taken out of the exponentials.  A is [M][nobs] row-major; omega_out may be NULL.
+int ora_weighted_average(int M, const double* lnZ, const double* A, int nobs, double* A_out, double* omega_out) {
+    if (M < 1 || nobs < 0 || !lnZ || (nobs > 0 && (!A || !A_out))) return ORA_ERR_INVALID_ARG;
+    double zmax = lnZ[0];
+    for (int m = 1; m < M; ++m) if (lnZ[m] > zmax) zmax = lnZ[m];
+    std::vector<double> w(M);
+    double S = 0.0;
+    for (int m = 0; m < M; ++m) { w[m] = std::exp(lnZ[m] - zmax); S += w[m]; }
+    for (int m = 0; m < M; ++m) { w[m] = w[m] / S; if (omega_out) omega_out[m] = w[m]; }
+    for (int k = 0; k < nobs; ++k) {
+        double acc = 0.0;
+        for (int m = 0; m < M; ++m) acc += w[m] * A[(size_t)m * nobs + k];
+        A_out[k] = acc;
+    }
     return ORA_OK;
 }
 
@@ -543,6 +609,11 @@ int ora_get_histogram(const Oracle* o, int64_t* Hsum, double* lnD) {
     if (Hsum) std::memcpy(Hsum, o->Hsum.data(), sizeof(int64_t) * (o->N + 1));
     if (lnD) std::memcpy(lnD, o->lnD.data(), sizeof(double) * (o->N + 1));
     return ORA_OK;
+}
+
+int ora_reweight(const Oracle* o, int n, const double* betas, double* lnZ, double* e, double* C) {
+    if (!o) return ORA_ERR_INVALID_ARG;
+    return ora_reweight_of(o->L, o->Hsum.data(), o->lnD.data(), n, betas, lnZ, e, C);
 }
 
 // spins as +1/-1, [nrep][N], site = y*L + x

@@ -43,6 +43,9 @@ def lib():
         L.ora_adapt_dbeta_of.argtypes = [i64, i64, vp, dbl, dbl, dbl, vp]; L.ora_adapt_dbeta_of.restype = i32
         L.ora_observables_of.argtypes = [i32, i64, vp, vp, dbl, dbl, dbl, vp]; L.ora_observables_of.restype = i32
         L.ora_hist_fold_of.argtypes = [i32, i64, vp, dbl, dbl, vp, vp]; L.ora_hist_fold_of.restype = i32
+        L.ora_reweight_of.argtypes = [i32, vp, vp, i32, vp, vp, vp, vp]; L.ora_reweight_of.restype = i32
+        L.ora_reweight.argtypes = [vp, i32, vp, vp, vp, vp]; L.ora_reweight.restype = i32
+        L.ora_weighted_average.argtypes = [i32, vp, vp, i32, vp, vp]; L.ora_weighted_average.restype = i32
         L.ora_create.argtypes = [i32, i64, u64, vp]; L.ora_create.restype = i32
         L.ora_destroy.argtypes = [vp]; L.ora_destroy.restype = None
         L.ora_population.argtypes = [vp]; L.ora_population.restype = i64
@@ -168,6 +171,25 @@ def num_threads():
     return int(lib().ora_num_threads())
 
 
+def reweight_of(L, Hsum, lnD, betas):
+    """O12 (Sec. 2.4): lnZ, e, C at every beta from the accumulated Eq. 9 sums."""
+    Hsum = np.ascontiguousarray(Hsum, dtype=np.int64); lnD = np.ascontiguousarray(lnD, dtype=np.float64)
+    betas = np.ascontiguousarray(betas, dtype=np.float64)
+    lnZ = np.empty(betas.size); e = np.empty(betas.size); Cv = np.empty(betas.size)
+    _check(lib().ora_reweight_of(L, _p(Hsum), _p(lnD), betas.size, _p(betas), _p(lnZ), _p(e), _p(Cv)), "reweight_of")
+    return {"lnZ": lnZ, "e": e, "C": Cv}
+
+
+def weighted_average(lnZ, A):
+    """O13 (Eq. 6-7): A[M][nobs] -> (A~[nobs], omega[M])."""
+    lnZ = np.ascontiguousarray(lnZ, dtype=np.float64); A = np.ascontiguousarray(A, dtype=np.float64)
+    M = lnZ.size
+    A = A.reshape(M, -1)
+    out = np.empty(A.shape[1]); w = np.empty(M)
+    _check(lib().ora_weighted_average(M, _p(lnZ), _p(A), A.shape[1], _p(out), _p(w)), "weighted_average")
+    return out, w
+
+
 # ---- the population handle -----------------------------------------------------------------
 
 class Oracle:
@@ -209,6 +231,12 @@ class Oracle:
     @property
     def lnZ(self):
         return float(lib().ora_lnZ(self._h))
+
+    def reweight(self, betas):
+        betas = np.ascontiguousarray(betas, dtype=np.float64)
+        lnZ = np.empty(betas.size); e = np.empty(betas.size); Cv = np.empty(betas.size)
+        _check(lib().ora_reweight(self._h, betas.size, _p(betas), _p(lnZ), _p(e), _p(Cv)), "reweight")
+        return {"lnZ": lnZ, "e": e, "C": Cv}
 
     def set_rng_mode(self, mode):
         _check(lib().ora_set_rng_mode(self._h, int(mode)), "set_rng_mode")
