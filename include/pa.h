@@ -128,6 +128,20 @@ int pa_hist_accumulate(pa_t* h, double beta);
 /* Hsum: int64[N+1], lnD: double[N+1] (either may be NULL); ln Omega(E_m) = ln Hsum[m] - lnD[m]. */
 int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD);
 
+/* Multi-histogram reweighting (Sec. 2.4; O12): from the sums accumulated so far, the density of
+ * states ln Omega(E_m) = ln Hsum[m] - lnD[m] (Eq. 9) and, for each of the n inverse temperatures betas[i]
+ * (any values, not only simulated ones), lnZ[i] = ln sum_m Omega_m exp(-beta E_m) (= -beta F, Eq. 4),
+ * e[i] = <E>/N and C[i] = beta^2 (<E^2> - <E>^2)/N (Eq. 3).  betas, lnZ, e, C: double[n], host or device
+ * (all four of the same kind); outputs may be NULL.  1 <= n <= 2^20.  PA_ERR_INVALID_ARG if no histogram has
+ * been accumulated.  Does not change the population.  Synchronises if the buffers are host pointers. */
+int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, double* C);
+
+/* Weighted average of M independent runs (Sec. 2.2, Eq. 6-7; O13): omega_m = exp(lnZ_m) /
+ * sum_m exp(lnZ_m) with lnZ_m = -beta F_m(beta) = pa_lnZ of run m at this temperature, A_out[k] =
+ * sum_m omega_m A[m*nobs + k].  HOST pointers; lnZ: double[M], A: double[M*nobs], A_out: double[nobs],
+ * omega_out: double[M] or NULL.  Runs on the current CUDA device (no handle needed); synchronous. */
+int pa_weighted_average(int M, const double* lnZ, const double* A, int nobs, double* A_out, double* omega_out);
+
 /* State export / import (parity tests, checkpoints, the end-to-end benchmark).
  * Spins are +1 / -1, one int8 per spin, out[i][s] with site s = y*L + x.
  * pa_get_spins: replicas j0 .. j0+nrep-1.  pa_get_spins_at: replicas slots[0..n-1] (host int64).

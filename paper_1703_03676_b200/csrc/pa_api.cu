@@ -331,6 +331,7 @@ int pa_hist_accumulate(pa_t* h, double beta) {
     if (!h) return PA_ERR_INVALID_ARG;
     int rc;
     if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
+    h->hist_any = true;
     return pa_launch_hist(h, beta);
 }
 
@@ -340,6 +341,39 @@ int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD) {
     if (Hsum) rc = pa_copy_out(h, Hsum, h->Hsum, ((size_t)h->N + 1) * 8, nullptr);
     if (rc == PA_OK && lnD) rc = pa_copy_out(h, lnD, h->lnD, ((size_t)h->N + 1) * 8, nullptr);
     return rc;
+}
+
+int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, double* C) {
+    if (!h || !betas || n < 1 || n > (1 << 20)) return PA_ERR_INVALID_ARG;
+    if ((size_t)n * 32 > h->stage_bytes) return PA_ERR_INVALID_ARG;
+    // any histogram yet?  (Hsum is all zero until the first pa_hist_accumulate)
+    if (!h->hist_any) return PA_ERR_INVALID_ARG;
+    double* d_io = (double*)h->stage;
+    const bool dev = pa_is_device_ptr(betas);
+    PA_CUDA(h, cudaMemcpyAsync(d_io, betas, (size_t)n * 8, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
+    int rc = pa_launch_reweight(h, n, d_io);
+    if (rc != PA_OK) return rc;
+    double* outs[3] = {lnZ, e, C};
+    for (int i = 0; i < 3 && rc == PA_OK; ++i)
+        if (outs[i]) rc = pa_copy_out(h, outs[i], d_io + (size_t)(i + 1) * n, (size_t)n * 8, nullptr);
+    return rc;
+}
+
+int pa_weighted_average(int M, const double* lnZ, const double* A, int nobs, double* A_out, double* omega_out) {
+    if (M < 1 || nobs < 0 || !lnZ || (nobs > 0 && (!A || !A_out))) return PA_ERR_INVALID_ARG;
+    double* d = nullptr;
+    const size_t nA = (size_t)M * nobs, total = (size_t)M * 2 + nA + (size_t)nobs;
+    if (cudaMalloc(&d, (total ? total : 1) * 8) != cudaSuccess) { cudaGetLastError(); return PA_ERR_CUDA; }
+    double *d_lnZ = d, *d_om = d + M, *d_A = d + 2 * (size_t)M, *d_out = d_A + nA;
+    cudaError_t err = cudaMemcpy(d_lnZ, lnZ, (size_t)M * 8, cudaMemcpyHostToDevice);
+    if (err == cudaSuccess && nA) err = cudaMemcpy(d_A, A, nA * 8, cudaMemcpyHostToDevice);
+    if (err == cudaSuccess) err = pa_run_wavg(M, d_lnZ, d_A, nobs, d_out, d_om, 0);
+    if (err == cudaSuccess && nobs) err = cudaMemcpy(A_out, d_out, (size_t)nobs * 8, cudaMemcpyDeviceToHost);
+    if (err == cudaSuccess && omega_out) err = cudaMemcpy(omega_out, d_om, (size_t)M * 8, cudaMemcpyDeviceToHost);
+    if (err == cudaSuccess) err = cudaDeviceSynchronize();
+    cudaFree(d);
+    if (err != cudaSuccess) { cudaGetLastError(); return PA_ERR_CUDA; }
+    return PA_OK;
 }
 
 static int pa_get_spins_impl(pa_handle* h, const int64_t* slots, int64_t j0, int64_t n, int8_t* out) {

@@ -116,6 +116,7 @@ struct pa_handle {
 
     cudaEvent_t ev[9];                  // sweep begin/end, resample begin/end, copy begin/end, plan scalars on the host, measure begin/end
     bool sweep_timed, resample_timed, measure_timed;
+    bool hist_any;                      // pa_hist_accumulate has run at least once
     int64_t launches;
     bool sweep_C_forced;
     int sweep_C, sweep_T, sweep_cmp, sweep_kind;   // sweep launch geometry (cluster size, threads), compare variant, kernel kind
@@ -140,6 +141,8 @@ int pa_launch_overlap(pa_handle* h, int Emin);                         // TREE10
 int pa_launch_plan(pa_handle* h, int Emin);                            // tau, r, scan, parent map, R_new
 int pa_launch_copy(pa_handle* h);                                      // new[d] = old[parent(d)], d < R_new (read on the device)
 int pa_launch_hist(pa_handle* h, double beta);
+int pa_launch_reweight(pa_handle* h, int n, double* d_io);              // O12: d_io = [betas | lnZ | e | C], n each
+cudaError_t pa_run_wavg(int M, const double* d_lnZ, const double* d_A, int nobs, double* d_out, double* d_omega, cudaStream_t st);
 int pa_launch_unpack(pa_handle* h, const int64_t* d_slots, int64_t j0, int64_t n, int8_t* d_out);
 int pa_launch_pack(pa_handle* h, int64_t j0, int64_t n, const int8_t* d_in);
 int pa_launch_words_out(pa_handle* h, uint32_t* d_words);

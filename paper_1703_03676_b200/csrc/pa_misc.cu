@@ -72,6 +72,108 @@ int pa_launch_hist(pa_handle* h, double beta) {
     return PA_OK;
 }
 
+// ------------------------------------------------------------------------------------------------
+// O12 (Sec. 2.4, Eq. 9): canonical averages at any beta from the accumulated sums.
+// ln Omega_m = ln Hsum[m] - lnD[m]; one CTA per beta; three passes over the N+1 levels (largest exponent,
+// Z and <E>, variance about the mean) with fixed-shape block reductions (shuffle tree, then the tree over the
+// warp results), so the result does not depend on scheduling.
+// ------------------------------------------------------------------------------------------------
+template <bool IS_MAX>
+__device__ __forceinline__ double pa_block_reduce(double v, double* sh) {
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        const double o = __shfl_down_sync(0xffffffffu, v, off);
+        v = IS_MAX ? fmax(v, o) : v + o;
+    }
+    __syncthreads();                                   // sh may still be read from the previous reduction
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        v = threadIdx.x < (blockDim.x >> 5) ? sh[threadIdx.x] : (IS_MAX ? -INFINITY : 0.0);
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+            const double o = __shfl_down_sync(0xffffffffu, v, off);
+            v = IS_MAX ? fmax(v, o) : v + o;
+        }
+        if (threadIdx.x == 0) sh[32] = v;
+    }
+    __syncthreads();
+    return sh[32];
+}
+
+__global__ void __launch_bounds__(256)
+pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __restrict__ lnD, int N,
+                   const double* __restrict__ betas, double* __restrict__ lnZ, double* __restrict__ e, double* __restrict__ C) {
+    __shared__ double sh[33];
+    const double beta = betas[blockIdx.x];
+    double amax = -INFINITY;
+    for (int m = threadIdx.x; m <= N; m += blockDim.x) {
+        const unsigned long long H = Hsum[m];
+        if (H == 0ull) continue;
+        amax = fmax(amax, (log((double)H) - lnD[m]) - beta * (double)(-2 * N + 4 * m));
+    }
+    amax = pa_block_reduce<true>(amax, sh);
+    double s0 = 0.0, s1 = 0.0;
+    for (int m = threadIdx.x; m <= N; m += blockDim.x) {
+        const unsigned long long H = Hsum[m];
+        if (H == 0ull) continue;
+        const double Em = (double)(-2 * N + 4 * m);
+        const double p = exp(((log((double)H) - lnD[m]) - beta * Em) - amax);
+        s0 += p; s1 += Em * p;
+    }
+    s0 = pa_block_reduce<false>(s0, sh);
+    s1 = pa_block_reduce<false>(s1, sh);
+    const double mean = s1 / s0;
+    double s2 = 0.0;
+    for (int m = threadIdx.x; m <= N; m += blockDim.x) {
+        const unsigned long long H = Hsum[m];
+        if (H == 0ull) continue;
+        const double Em = (double)(-2 * N + 4 * m);
+        const double p = exp(((log((double)H) - lnD[m]) - beta * Em) - amax);
+        s2 += (Em - mean) * (Em - mean) * p;
+    }
+    s2 = pa_block_reduce<false>(s2, sh);
+    if (threadIdx.x == 0) {
+        lnZ[blockIdx.x] = amax + log(s0);
+        e[blockIdx.x] = mean / (double)N;
+        C[blockIdx.x] = beta * beta * (s2 / s0) / (double)N;
+    }
+}
+
+// d_io: [betas(n) | lnZ(n) | e(n) | C(n)] in device memory
+int pa_launch_reweight(pa_handle* h, int n, double* d_io) {
+    pa_reweight_kernel<<<n, 256, 0, h->stream>>>(h->Hsum, h->lnD, h->N, d_io, d_io + n, d_io + 2 * (size_t)n, d_io + 3 * (size_t)n);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
+
+// O13 (Sec. 2.2, Eq. 6-7): omega_m = exp(lnZ_m - max) / sum, A~_k = sum_m omega_m A[m][k].  One CTA.
+__global__ void __launch_bounds__(256)
+pa_wavg_kernel(int M, const double* __restrict__ lnZ, const double* __restrict__ A, int nobs,
+               double* __restrict__ A_out, double* __restrict__ omega) {
+    __shared__ double sh[33];
+    double zmax = -INFINITY;
+    for (int m = threadIdx.x; m < M; m += blockDim.x) zmax = fmax(zmax, lnZ[m]);
+    zmax = pa_block_reduce<true>(zmax, sh);
+    double s = 0.0;
+    for (int m = threadIdx.x; m < M; m += blockDim.x) s += exp(lnZ[m] - zmax);
+    s = pa_block_reduce<false>(s, sh);
+    for (int m = threadIdx.x; m < M; m += blockDim.x) omega[m] = exp(lnZ[m] - zmax) / s;
+    __syncthreads();
+    for (int k = 0; k < nobs; ++k) {
+        double acc = 0.0;
+        for (int m = threadIdx.x; m < M; m += blockDim.x) acc += omega[m] * A[(size_t)m * nobs + k];
+        acc = pa_block_reduce<false>(acc, sh);
+        if (threadIdx.x == 0) A_out[k] = acc;
+    }
+}
+
+cudaError_t pa_run_wavg(int M, const double* d_lnZ, const double* d_A, int nobs, double* d_out, double* d_omega, cudaStream_t st) {
+    pa_wavg_kernel<<<1, 256, 0, st>>>(M, d_lnZ, d_A, nobs, d_out, d_omega);
+    return cudaGetLastError();
+}
+
 // ---- spin export / import ------------------------------------------------------------------------
 __global__ void pa_unpack_kernel(const uint32_t* __restrict__ pop, int L, int N, const long long* __restrict__ slots,
                                  long long j0, long long n, int8_t* __restrict__ out) {

@@ -75,6 +75,8 @@ def lib():
         "pa_observables": ([vp, dbl, C.POINTER(pa_obs_t)], i32),
         "pa_hist_accumulate": ([vp, dbl], i32),
         "pa_get_histogram": ([vp, vp, vp], i32),
+        "pa_reweight": ([vp, i32, vp, vp, vp, vp], i32),
+        "pa_weighted_average": ([i32, vp, vp, i32, vp, vp], i32),
         "pa_get_spins": ([vp, i64, i64, vp], i32),
         "pa_get_spins_at": ([vp, vp, i64, vp], i32),
         "pa_set_spins": ([vp, i64, i64, vp], i32),
@@ -158,6 +160,18 @@ def pa_create_ex(L, R, seed, dev_ws_ptr, ws_bytes, cuda_stream):
 
 def pa_destroy(h):
     lib().pa_destroy(h)
+
+
+def pa_weighted_average(lnZ, A):
+    """Sec. 2.2 (Eq. 6-7): A[M][nobs] of M independent runs with free-energy estimates lnZ[M] -> (A~[nobs], omega[M])."""
+    lnZ = np.ascontiguousarray(lnZ, dtype=np.float64)
+    M = lnZ.size
+    A = np.ascontiguousarray(A, dtype=np.float64).reshape(M, -1)
+    out = np.empty(A.shape[1]); w = np.empty(M)
+    rc = lib().pa_weighted_average(M, _ptr(lnZ), _ptr(A), A.shape[1], _ptr(out), _ptr(w))
+    if rc != PA_OK:
+        raise PaError(rc, "pa_weighted_average")
+    return out, w
 
 
 class Population:
@@ -279,6 +293,13 @@ class Population:
         H = np.empty(self.N + 1, dtype=np.int64); D = np.empty(self.N + 1, dtype=np.float64)
         self._check(lib().pa_get_histogram(self._h, _ptr(H), _ptr(D)), "pa_get_histogram")
         return H, D
+
+    def reweight(self, betas):
+        """Sec. 2.4 (Eq. 9): lnZ, e, C at every beta of `betas` from the accumulated multi-histogram sums."""
+        betas = np.ascontiguousarray(betas, dtype=np.float64)
+        lnZ = np.empty(betas.size); e = np.empty(betas.size); Cv = np.empty(betas.size)
+        self._check(lib().pa_reweight(self._h, betas.size, _ptr(betas), _ptr(lnZ), _ptr(e), _ptr(Cv)), "pa_reweight")
+        return {"lnZ": lnZ, "e": e, "C": Cv}
 
     # state export / import
     def get_spins(self, j0=0, nrep=None):

@@ -251,6 +251,46 @@ def test_adaptive_run_with_multihistogram():
     # the overlap function itself
     for d in (0.0, 0.003, 0.02):
         assert g.overlap(d) == o.overlap(d)
+    # O12: reweighting of the accumulated sums to a fine beta grid (Sec. 2.4), inside and beyond the simulated range
+    grid = np.concatenate([np.linspace(0.0, bg[-1], 37), [bg[-1] + 0.05, 1.5]])
+    rg, ro = g.reweight(grid), o.reweight(grid)
+    for k in ("lnZ", "e", "C"):
+        assert np.allclose(rg[k], ro[k], rtol=REL, atol=1e-300), k
+
+
+def test_reweight_errors_and_device_buffers():
+    L, R = 8, 300
+    g, o = pa.Population(L, R, 3), po.Oracle(L, R, 3)
+    grid = np.array([0.1, 0.2])
+    rc = pa.lib().pa_reweight(g._h, 2, pa._ptr(grid), None, None, None)
+    assert rc == pa.PA_ERR_INVALID_ARG                                # nothing accumulated yet
+    obs_g = pa_driver.run_fixed(g, [0.0, 0.1, 0.2, 0.3], 2, hist=True)
+    pa_driver.run_fixed(o, [0.0, 0.1, 0.2, 0.3], 2, hist=True)
+    assert pa.lib().pa_reweight(g._h, 0, pa._ptr(grid), None, None, None) == pa.PA_ERR_INVALID_ARG
+    want = o.reweight(grid)
+    tb = torch.tensor(grid, device="cuda"); te = torch.empty(2, dtype=torch.float64, device="cuda")
+    assert pa.lib().pa_reweight(g._h, 2, pa._ptr(tb), None, pa._ptr(te), None) == pa.PA_OK
+    torch.cuda.synchronize()
+    assert np.allclose(te.cpu().numpy(), want["e"], rtol=REL)
+    assert g.population == obs_g[-1]["R"]                             # state untouched
+
+
+def test_weighted_average_of_runs():
+    """O13 (Eq. 6-7): M independent GPU populations combined by their free-energy estimates."""
+    L, R, M = 8, 200, 6
+    betas = [0.0, 0.15, 0.3, 0.45]
+    lnZ, A = [], []
+    for m in range(M):
+        g = pa.Population(L, R, 900 + m)
+        ob = pa_driver.run_fixed(g, betas, 2)[-1]
+        lnZ.append(g.lnZ); A.append([ob["e"], ob["C"], ob["absm"]])
+    out_g, w_g = pa.pa_weighted_average(lnZ, A)
+    out_o, w_o = po.weighted_average(lnZ, A)
+    assert np.allclose(w_g, w_o, rtol=REL) and np.allclose(out_g, out_o, rtol=REL)
+    assert abs(w_g.sum() - 1) < 1e-12
+    big = np.array([800.0, 0.0, -800.0])
+    out_g, w_g = pa.pa_weighted_average(big, np.arange(3.0)[:, None])
+    assert w_g.tolist() == [1.0, 0.0, 0.0] and out_g[0] == 0.0
 
 
 def test_determinism_and_geometry_independence(monkeypatch):
