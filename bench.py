@@ -108,6 +108,25 @@ def reduce_over_ranks(ms, units, device, dist=None):
     return float(t.item()), float(u.item())
 
 
+COMBINE_KEYS = ("e", "C", "absm", "m2", "m4")
+
+
+def combine_over_ranks(lnZ, obs, device, dist, wavg):
+    """The one exchange step the method has across independent populations (Sec. 2.2, Eq. 6-7):
+    all-gather (lnZ_m, observables_m) -- 6 doubles per rank -- and weight run m by exp(-beta F_m) = exp(lnZ_m).
+    `wavg(lnZ[M], A[M][nobs]) -> (A~, omega)` is the library's pa_weighted_average (the oracle's in the CPU test)."""
+    import torch
+    mine = torch.tensor([float(lnZ)] + [float(obs[k]) for k in COMBINE_KEYS], dtype=torch.float64, device=device)
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        rows = mine[None, :].cpu().numpy()
+    else:
+        buf = [torch.empty_like(mine) for _ in range(dist.get_world_size())]
+        dist.all_gather(buf, mine)
+        rows = torch.stack(buf).cpu().numpy()
+    out, omega = wavg(rows[:, 0].copy(), rows[:, 1:].copy())
+    return {"runs": int(rows.shape[0]), "omega": [float(x) for x in omega], **{k: float(v) for k, v in zip(COMBINE_KEYS, out)}}
+
+
 def rank_seed(wl, rank):
     """Every rank anneals its own independent population (no data-path collective)."""
     return wl.seed + rank
@@ -225,6 +244,8 @@ def run_ours(args):
         e2e = {"value": upd_e / (dt * 1e9), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke,
                "steps": Ke, "what": "population words pinned-host -> device, one step, energies + words + observables back to host"}
 
+    # ---- weighted average of the ranks' populations at the last temperature (Eq. 6-7): the method's own exchange step
+    combined = combine_over_ranks(pop.lnZ, pop.observables(beta_prev), "cuda", dist if world > 1 else None, pa.pa_weighted_average)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -260,7 +281,7 @@ def run_ours(args):
                       "l2": "flushed between timed steps (256 MiB memset outside the CUDA events)",
                       "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "resample": resample,
-           "last_observables": obs}
+           "last_observables": obs, "combined_observables": combined}
     out["cpu_baseline"] = cpu_baseline(wl, args.rng) if world == 1 and not args.no_cpu else None
     print(json.dumps(out), flush=True)
     if world > 1:

@@ -36,8 +36,11 @@ def _worker(rank, world, port, q):
     units = o.population * wl.N * 2
     ms = 10.0 * (rank + 1)                                   # rank 1 is the slow one
     t, u = bench.reduce_over_ranks(ms, units, "cpu", dist)
+    # Eq. 6-7: the ranks' runs combined by their free-energy estimates
+    ob = o.observables(betas[1])
+    comb = bench.combine_over_ranks(o.lnZ, ob, "cpu", dist, po.weighted_average)
     allu = [None] * world
-    dist.all_gather_object(allu, (seed, int(units), int(E.sum())))
+    dist.all_gather_object(allu, (seed, int(units), int(E.sum()), o.lnZ, ob["e"], comb))
     dist.barrier()
     if rank == 0:
         q.put((t, u, allu))
@@ -59,9 +62,20 @@ def test_two_ranks_independent_populations_and_reduction():
     assert u == float(sum(x[1] for x in allu))               # sum over ranks
     assert allu[0][0] != allu[1][0]                          # different seeds ...
     assert allu[0][2] != allu[1][2]                          # ... different populations
+    # the weighted average: both ranks hold the same result; weights follow exp(lnZ_m); e~ = sum omega_m e_m
+    import math
+    c0, c1 = allu[0][5], allu[1][5]
+    assert c0 == c1 and c0["runs"] == 2
+    w0 = 1.0 / (1.0 + math.exp(allu[1][3] - allu[0][3]))
+    assert c0["omega"][0] == pytest.approx(w0, rel=1e-12) and sum(c0["omega"]) == pytest.approx(1.0, rel=1e-14)
+    assert c0["e"] == pytest.approx(w0 * allu[0][4] + (1 - w0) * allu[1][4], rel=1e-12)
 
 
 def test_single_rank_reduction_is_identity():
     sys.path.insert(0, ROOT)
     import bench
     assert bench.reduce_over_ranks(3.5, 7, "cpu", None) == (3.5, 7.0)
+    from oracle import pa_oracle as po
+    ob = {"e": -1.0, "C": 0.5, "absm": 0.2, "m2": 0.1, "m4": 0.05}
+    c = bench.combine_over_ranks(12.0, ob, "cpu", None, po.weighted_average)
+    assert c["runs"] == 1 and c["omega"] == [1.0] and all(c[k] == ob[k] for k in ob)
