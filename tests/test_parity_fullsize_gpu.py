@@ -44,7 +44,7 @@ def _bits(spins_pm1):
     return np.ascontiguousarray((spins_pm1 > 0).astype(np.uint8))
 
 
-def checked_step(g, wl, beta_prev, beta, rng, n_slots, lnZ_ref, hist=None):
+def checked_step(g, wl, beta_prev, beta, rng, n_slots, lnZ_ref, hist=None, rng_mode=po.RNG_PHILOX):
     """One temperature step on the device with checks (i)-(v).  Returns (observables, lnZ after the step)."""
     L, N = wl.L, wl.N
     R_prev = g.population
@@ -74,7 +74,7 @@ def checked_step(g, wl, beta_prev, beta, rng, n_slots, lnZ_ref, hist=None):
     t0 = g.sweep_counter                                                                  # (iv)
     g.sweep(beta, wl.theta)
     assert g.sweep_counter == t0 + wl.theta
-    want = po.sweep_slots(L, wl.seed, t0, beta, wl.theta, d, _bits(post))
+    want = po.sweep_slots(L, wl.seed, t0, beta, wl.theta, d, _bits(post), rng_mode=rng_mode)
     got = g.get_spins_at(d)
     assert np.array_equal(_bits(got), want)
 
@@ -127,10 +127,11 @@ def _check_initial(g, wl, rng, n_slots):
     assert np.all((E + 2 * N) % 4 == 0)
 
 
-def _run_fixed_schedule(cfg, checked, n_slots, last_step):
+def _run_fixed_schedule(cfg, checked, n_slots, last_step, rng_mode=po.RNG_PHILOX):
     wl = CONFIGS[cfg]
     rng = np.random.default_rng(1000 + cfg)
     g = pa.Population(wl.L, wl.R, wl.seed)
+    g.set_rng_mode(rng_mode)                                   # pa.PA_RNG_* and po.RNG_* are the same numbers (0, 1)
     _check_initial(g, wl, rng, n_slots)
     betas = wl.betas()
     lnZ = wl.N * np.log(2.0)
@@ -138,7 +139,7 @@ def _run_fixed_schedule(cfg, checked, n_slots, last_step):
     last = len(betas) - 1 if RUN_ALL else last_step
     for i in range(1, last + 1):
         if i in checked:
-            og, lnZ = checked_step(g, wl, betas[i - 1], betas[i], rng, n_slots, lnZ)
+            og, lnZ = checked_step(g, wl, betas[i - 1], betas[i], rng, n_slots, lnZ, rng_mode=rng_mode)
         else:
             og, lnZ = plain_step(g, wl, betas[i - 1], betas[i], lnZ)
         # population size stays close to R: every r_j is a Bernoulli rounding, sd <= sqrt(R)/2 per step
@@ -163,6 +164,22 @@ def test_config5_full_size_sampled():
         pytest.skip("needs 17 GB of device memory")
     checked = {1, 2, 12} | ({438, 441, 444, 499, 500} if RUN_ALL else set())
     _run_fixed_schedule(5, checked=checked, n_slots=256, last_step=12)
+
+
+def test_config3_full_size_sampled_lcg_stream():
+    """configs[2] with the paper's LCG-assisted sweep stream (O11, L236-L241): the whole schedule on the device, the same
+    sampled checks; ordered at beta = 1."""
+    assert pa.PA_RNG_LCG == po.RNG_LCG
+    og = _run_fixed_schedule(3, checked={1, 2, 88, 200}, n_slots=1024, last_step=200, rng_mode=po.RNG_LCG)
+    assert og["beta"] == 1.0 and og["absm"] > 0.99
+
+
+def test_config5_full_size_sampled_lcg_stream():
+    """configs[4] (L=256: clusters of 4 CTAs, 64-row strips, quad-row walk) with the LCG-assisted stream, first 6 steps."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 20 * 2**30:
+        pytest.skip("needs 17 GB of device memory")
+    _run_fixed_schedule(5, checked={1, 6}, n_slots=192, last_step=6, rng_mode=po.RNG_LCG)
 
 
 def test_config4_full_size_adaptive_multihistogram():
