@@ -148,6 +148,47 @@ def next_beta(pop, wl, betas, i, beta_prev):
     return min(wl.beta_f, beta_prev + d)
 
 
+def whole_run(pa, wl, seed, rng):
+    """the config's WHOLE annealing schedule on a fresh population, timed as the paper times its runs:
+    t_SF = t_run / (N theta sum_i R_i) (Eq. 11), resampling, measurement (and, for the adaptive config, the
+    bisection and the histogram fold) included; the resample cost depends on the weight distribution, so it is sampled in
+    situ at every step (median, max, and near beta = 0.1, beta_c, the last step), as is the sweep kernel's rate."""
+    import torch
+    pop = pa.Population(wl.L, wl.R, seed)
+    if rng == "lcg":
+        pop.set_rng_mode(pa.PA_RNG_LCG)
+    betas = wl.betas() if wl.n_steps is not None else None
+    beta_prev, i = wl.beta0, 0
+    pop.observables(beta_prev)
+    if wl.multi_histogram:
+        pop.hist_accumulate(beta_prev)
+    rows, flips = [], 0
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    while beta_prev < wl.beta_f and (betas is None or i < len(betas) - 1):
+        i += 1
+        beta = next_beta(pop, wl, betas, i, beta_prev)
+        obs = one_step(pop, wl, beta_prev, beta)
+        flips += obs["R"] * wl.N * wl.theta
+        rt, ct = pop.last_resample_ms()
+        rows.append((beta, obs["R"] * wl.N * wl.theta / (pop.last_sweep_ms() * 1e6), rt, ct))
+        beta_prev = beta
+    torch.cuda.synchronize()
+    t_run = time.perf_counter() - t0
+
+    def near(b):
+        return min(rows, key=lambda r: abs(r[0] - b))
+    res = sorted(r[2] for r in rows)
+    marks = {"beta_0.1": near(0.1), "beta_c": near(0.4406868), "last": rows[-1]}
+    out = {"steps": len(rows), "beta_final": beta_prev, "t_run_s": t_run, "t_SF_ns": t_run * 1e9 / flips, "updates_per_ns": flips / (t_run * 1e9),
+           "timing": "host wall clock around the whole schedule, synchronised on both sides (the paper's t_SF, Eq. 11)",
+           "resample_ms": {"median": res[len(res) // 2], "max": res[-1], **{k: v[2] for k, v in marks.items()}},
+           "sweep_updates_per_ns": {k: v[1] for k, v in marks.items()},
+           "final_observables": obs}
+    pop.close()
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -282,6 +323,8 @@ def run_ours(args):
                       "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "resample": resample,
            "last_observables": obs, "combined_observables": combined}
+    if world == 1 and (args.whole_run or (args.whole_run is None and args.config <= 4)):
+        out["whole_run"] = whole_run(pa, wl, rank_seed(wl, rank), args.rng)
     out["cpu_baseline"] = cpu_baseline(wl, args.rng) if world == 1 and not args.no_cpu else None
     print(json.dumps(out), flush=True)
     if world > 1:
@@ -340,6 +383,9 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=sorted(CONFIGS), help="BASELINE.json configs index + 1")
     ap.add_argument("--e2e-steps", type=int, default=10)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--whole-run", dest="whole_run", action="store_true", default=None,
+                    help="also time the config's whole schedule (t_SF, Eq. 11); default: on for configs 1-4 (seconds), off for 5 (minutes)")
+    ap.add_argument("--no-whole-run", dest="whole_run", action="store_false")
     ap.add_argument("--rng", default="philox", choices=["philox", "lcg"],
                     help="sweep stream: one Philox number per spin (default, O1) or the paper's Philox-seeded LCG (O11, L236-L241)")
     args = ap.parse_args()
