@@ -189,6 +189,36 @@ def whole_run(pa, wl, seed, rng):
     return out
 
 
+def theta_scan(args):
+    """PAPER.md Table 3 (t_SF against theta at L = 128, R = 50 000), Table 4 (fraction of the run time spent in the spin-update
+    kernel) re-measured on this GPU: whole runs, host wall clock.  Context for BASELINE.md, not the bench line."""
+    import torch
+    from paper_1703_03676_b200 import pa
+    from paper_1703_03676_b200.workloads import table3_workload
+    torch.cuda.set_device(0)
+    rows = []
+    for theta in (1, 5, 10, 50, 100, 500):
+        wl = table3_workload(theta)
+        pop = pa.Population(wl.L, wl.R, wl.seed)
+        if args.rng == "lcg":
+            pop.set_rng_mode(pa.PA_RNG_LCG)
+        betas = wl.betas()
+        pop.observables(betas[0])
+        flips, sweep_ms = 0, 0.0
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for i in range(1, len(betas)):
+            obs = one_step(pop, wl, betas[i - 1], betas[i])
+            flips += obs["R"] * wl.N * theta
+            sweep_ms += pop.last_sweep_ms()
+        torch.cuda.synchronize()
+        t_run = time.perf_counter() - t0
+        rows.append({"theta": theta, "t_SF_ns": t_run * 1e9 / flips, "updates_per_ns": flips / (t_run * 1e9),
+                     "sweep_kernel_fraction": sweep_ms * 1e-3 / t_run, "t_run_s": t_run})
+        pop.close()
+    print(json.dumps({"theta_scan": rows, "workload": "PAPER.md Table 3/4 shape: L=128, R=50000, 50 equal steps to beta=1", "rng": args.rng}), flush=True)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -385,13 +415,16 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--whole-run", dest="whole_run", action="store_true", default=None,
                     help="also time the config's whole schedule (t_SF, Eq. 11); default: on for configs 1-4 (seconds), off for 5 (minutes)")
+    ap.add_argument("--theta-scan", action="store_true", help="re-measure the paper's Table 3 / Table 4 theta dependence (context)")
     ap.add_argument("--no-whole-run", dest="whole_run", action="store_false")
     ap.add_argument("--rng", default="philox", choices=["philox", "lcg"],
                     help="sweep stream: one Philox number per spin (default, O1) or the paper's Philox-seeded LCG (O11, L236-L241)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
-    if args.impl == "reference":
+    if args.theta_scan:
+        theta_scan(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -49,3 +49,11 @@ CONFIGS = {
                 target_overlap=0.85, multi_histogram=True),
     5: Workload("cfg5_L256_R1000000", 256, 1000000, 5, 0.0, 0.5, 500, 10),
 }
+
+
+def table3_workload(theta: int, R: int = 50000) -> Workload:
+    """The shape of the paper's theta scan (Table 3 / Table 4 / Table 5: L = 128, R = 50 000,
+    theta = 1 .. 500 on a Tesla K80).  The paper does not restate the temperature step for these tables; Table 1's
+    (L189: dbeta = 0.02, i.e. 50 equal steps from 0 to 1) is used -- t_SF is normalised per spin flip, so the number of
+    temperatures only sets how often the resampling cost is paid per theta sweeps, which is once in either case."""
+    return Workload(f"table3_L128_R{R}_theta{theta}", 128, R, 7, 0.0, 1.0, 50, theta)
