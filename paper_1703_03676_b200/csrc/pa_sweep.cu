@@ -467,6 +467,10 @@ int pa_sweep_configure(pa_handle* h) {
     const size_t budget = (size_t)pa_env_int("PA_SWEEP_SMEM_KB", 64) * 1024;
     int C = 1;
     while (C <= 8 && (((L % C) != 0) || (size_t)L * L * 4 / C > budget)) C *= 2;
+    if (C > 8) {                                   // L = 512: no strip fits the preferred budget; take the largest that fits an SM
+        C = 1;
+        while (C <= 8 && (((L % C) != 0) || (size_t)L * L * 4 / C > (size_t)224 * 1024)) C *= 2;
+    }
     h->sweep_C_forced = false;
     int forceC = pa_env_int("PA_SWEEP_C", 0);
     if (forceC > 0 && L % forceC == 0) { C = forceC; h->sweep_C_forced = true; }

@@ -61,7 +61,7 @@ def test_init_bit_exact(L, R, seed):
 # a2 sweep: per call, several tile geometries (one CTA per group, clusters of 2/4 with DSMEM halos)
 # ---------------------------------------------------------------------------------------------
 
-@pytest.mark.parametrize("L,R", [(4, 40), (6, 70), (10, 33), (16, 200), (32, 100), (64, 96), (128, 64), (256, 40)])
+@pytest.mark.parametrize("L,R", [(4, 40), (6, 70), (10, 33), (16, 200), (32, 100), (64, 96), (128, 64), (256, 40), (192, 40), (512, 33)])
 def test_sweep_bit_exact(L, R):
     seed = 1000 + L
     g, o = pa.Population(L, R, seed), po.Oracle(L, R, seed)
@@ -70,7 +70,7 @@ def test_sweep_bit_exact(L, R):
         assert_same_state(g, o)
 
 
-@pytest.mark.parametrize("L,R", [(4, 40), (6, 70), (10, 33), (16, 200), (32, 100), (64, 96), (128, 64), (256, 40)])
+@pytest.mark.parametrize("L,R", [(4, 40), (6, 70), (10, 33), (16, 200), (32, 100), (64, 96), (128, 64), (256, 40), (192, 40), (512, 33)])
 def test_sweep_lcg_mode_bit_exact(L, R):
     """LCG-assisted stream (O11): generic kernel (L < 64 or not a power of two) and the
     quad-row column-walk kernel, ragged last group, switching modes between calls."""
