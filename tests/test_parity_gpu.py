@@ -178,6 +178,22 @@ def test_copy_strong_resampling(L, R):
         g.sweep(beta, 1); o.sweep(beta, 1)
 
 
+@pytest.mark.parametrize("L,R", [(4, 1), (4, 2), (6, 32), (8, 33), (4, 5000)])
+def test_tiny_and_ragged_populations_whole_run(L, R):
+    """Degenerate population sizes: a single replica (r_0 is always 1 because tau = R w / W = 1), exactly one word, one word
+    plus one replica, and a lattice of 4 chunks (fewer 128-bit chunks than copy threads)."""
+    g, o = pa.Population(L, R, 17), po.Oracle(L, R, 17)
+    betas = [0.0, 0.2, 0.45, 0.9]
+    og = pa_driver.run_fixed(g, betas, 3, hist=True)
+    oo = pa_driver.run_fixed(o, betas, 3, hist=True)
+    for a, b in zip(og, oo):
+        assert_obs_close(a, b)
+    assert_same_state(g, o)
+    assert np.array_equal(g.histogram()[0], o.histogram()[0])
+    d_g, d_o = g.adapt_dbeta(0.7, 0.9, 2.0), o.adapt_dbeta(0.7, 0.9, 2.0)
+    assert d_g == d_o
+
+
 def test_resample_identity_capacity_and_errors():
     L, R = 16, 500
     g, o = pa.Population(L, R, 5), po.Oracle(L, R, 5)
