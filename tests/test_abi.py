@@ -48,6 +48,41 @@ def test_host_only_entry_points():
     assert pa.lib().pa_version().decode().startswith("pa-b200")
 
 
+@pytest.fixture(scope="module")
+def c_client(libpath, tmp_path_factory):
+    """include/pa.h compiles as strict C99 and a C program links against the library."""
+    exe = str(tmp_path_factory.mktemp("abi") / "abi_c_client")
+    pkg = os.path.dirname(libpath)
+    subprocess.run(["gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"),
+                    os.path.join(ROOT, "tests", "helpers", "abi_c_client.c"), "-o", exe,
+                    "-L", pkg, "-lpa_b200", "-Wl,-rpath," + pkg], check=True)
+    return exe
+
+
+def test_c_client_links_and_reports_no_device(c_client):
+    import torch
+    r = subprocess.run([c_client], capture_output=True, text=True)
+    if torch.cuda.is_available():
+        assert r.returncode == 0, r.stdout + r.stderr
+    else:
+        assert r.returncode == 3 and "no device" in r.stdout          # PA_ERR_CUDA from pa_create: no CPU fallback
+
+
+@pytest.mark.gpu
+def test_c_client_runs_the_paper_loop(c_client):
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    r = subprocess.run([c_client, "32", "3000"], capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout + r.stderr
+    lines = r.stdout.strip().splitlines()
+    assert len(lines) >= 3 and lines[-1].startswith("reweighted to beta=0.25")
+    last = lines[-2].split()
+    betas = [float(l.split()[0]) for l in lines[:-1]]
+    assert all(b > a for a, b in zip(betas, betas[1:])) and 0.0 < betas[-1] <= 0.5    # the adaptive schedule moves forward
+    assert -2.0 < float(last[1]) < 0.0 and abs(float(last[1]) + 2.0 * betas[-1]) < 0.1   # e ~ -2 beta at high temperature
+
+
 def test_no_cpu_fallback():
     import torch
     if torch.cuda.is_available():
