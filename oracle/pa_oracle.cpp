@@ -26,6 +26,8 @@
 //   adaptive step (O10) .. alpha(0) closed form, monotonicity, bracket property
 //   reweighting (O12) .... exact g(E) of the 4x4 torus in, exact enumeration averages out; Kaufman
 //                          e, C, lnZ at off-grid beta from L=16 runs (5 sigma over seeds)
+//   magnetisation reweighting (O14) exact g(E) and exact microcanonical |M|, M^2 sums of the 4x4 torus in, exact
+//                          enumeration <|m|>, <m^2> out; L=4 runs at off-grid beta (5 sigma over seeds)
 //   weighted averages (O13) closed forms (weight ratios, M = 1, equal F, shift invariance, dominance);
 //                          unbiasedness of exp(lnZ_m) and removal of the small-R bias at L=4 (L99)
 //   LCG-assisted stream (O11) recurrence against big-integer arithmetic with the constants the
@@ -223,6 +225,7 @@ struct Oracle {
     std::vector<uint8_t> spin;        // [R_cap][N]
     std::vector<int64_t> Hsum;        // [N+1]  running sum of energy histograms, Eq. 9 numerator
     std::vector<double> lnD;          // [N+1]  log of the Eq. 9 denominator
+    std::vector<int64_t> A1sum, A2sum; // [N+1]  sums of |M_j| and M_j^2 over all folded replicas with energy level m (O14)
     // last resample, kept for inspection
     double W_last = 0.0;
     std::vector<double> w_last;
@@ -353,6 +356,40 @@ void reweight_for(int N, const int64_t* Hsum, const double* lnD, double beta, do
     *C = beta * beta * (S2 / S0) / (double)N;
 }
 
+// O14, L129 "Generalizations to other quantities such as magnetizations are possible": microcanonical magnetisation sums.
+// At every fold, for every replica j with energy level m_j: A1[m_j] += |M_j|, A2[m_j] += M_j^2 (exact integers).  The mean of
+// |M| (M^2) at fixed energy does not depend on beta, so the pooled ratio A[m]/Hsum[m] estimates it from all temperatures, and
+//   <|m|>(beta) = sum_m p_m(beta) (A1[m]/Hsum[m]) / N,   <m^2>(beta) = sum_m p_m(beta) (A2[m]/Hsum[m]) / N^2,
+// with p_m = Omega_m exp(-beta E_m) / Z from Eq. 9 exactly as in reweight_for.
+void mag_fold_for(const std::vector<int32_t>& E, const std::vector<int32_t>& M, int N, int64_t* A1, int64_t* A2) {
+    for (size_t j = 0; j < E.size(); ++j) {
+        int m = (E[j] + 2 * N) / 4;
+        int64_t a = M[j] < 0 ? -(int64_t)M[j] : (int64_t)M[j];
+        A1[m] += a; A2[m] += a * a;
+    }
+}
+void reweight_mag_for(int N, const int64_t* Hsum, const double* lnD, const int64_t* A1, const int64_t* A2, double beta,
+                      double* absm, double* m2) {
+    const double ninf = -std::numeric_limits<double>::infinity();
+    double amax = ninf;
+    for (int m = 0; m <= N; ++m) {
+        if (Hsum[m] <= 0) continue;
+        double a = (std::log((double)Hsum[m]) - lnD[m]) - beta * (double)(-2 * N + 4 * m);
+        if (a > amax) amax = a;
+    }
+    double S0 = 0.0, Sa = 0.0, Sq = 0.0;
+    for (int m = 0; m <= N; ++m) {
+        if (Hsum[m] <= 0) continue;
+        double Em = (double)(-2 * N + 4 * m);
+        double p = std::exp(((std::log((double)Hsum[m]) - lnD[m]) - beta * Em) - amax);
+        S0 += p;
+        Sa += p * ((double)A1[m] / (double)Hsum[m]);
+        Sq += p * ((double)A2[m] / (double)Hsum[m]);
+    }
+    *absm = (Sa / S0) / (double)N;
+    *m2 = (Sq / S0) / ((double)N * (double)N);
+}
+
 }  // namespace
 
 extern "C" {
@@ -468,6 +505,23 @@ int ora_reweight_of(int L, const int64_t* Hsum, const double* lnD, int n, const 
     return ORA_OK;
 }
 
+// O14 from the accumulated sums alone
+int ora_reweight_mag_of(int L, const int64_t* Hsum, const double* lnD, const int64_t* A1, const int64_t* A2, int n,
+                        const double* betas, double* absm, double* m2) {
+    if (L < 4 || (L & 1) || !Hsum || !lnD || !A1 || !A2 || n < 0) return ORA_ERR_INVALID_ARG;
+    bool any = false;
+    for (int m = 0; m <= L * L; ++m) any = any || Hsum[m] > 0;
+    if (!any) return ORA_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i) reweight_mag_for(L * L, Hsum, lnD, A1, A2, betas[i], &absm[i], &m2[i]);
+    return ORA_OK;
+}
+int ora_mag_fold_of(int L, int64_t R_cur, const int32_t* E, const int32_t* M, int64_t* A1, int64_t* A2) {
+    if (L < 4 || (L & 1) || R_cur < 1 || !E || !M || !A1 || !A2) return ORA_ERR_INVALID_ARG;
+    std::vector<int32_t> Ev(E, E + R_cur), Mv(M, M + R_cur);
+    mag_fold_for(Ev, Mv, L * L, A1, A2);
+    return ORA_OK;
+}
+
 // O13, Sec. 2.2 Eq. 6-7 (L99-L109): weighted average of M independent runs,
 //   omega_m = exp(-beta F_m) / sum_m exp(-beta F_m) with -beta F_m = lnZ_m (Eq. 4), A~ = sum_m omega_m A_m,
 // the largest lnZ_m taken out of the exponentials.  A is [M][nobs] row-major; omega_out may be NULL.
@@ -499,6 +553,7 @@ int ora_create(int L, int64_t R, uint64_t seed, Oracle** out) {
     try { o->spin.assign((size_t)o->R_cap * o->N, 0); } catch (...) { delete o; return ORA_ERR_NOMEM; }
     o->Hsum.assign(o->N + 1, 0);
     o->lnD.assign(o->N + 1, -std::numeric_limits<double>::infinity());
+    o->A1sum.assign(o->N + 1, 0); o->A2sum.assign(o->N + 1, 0);
 #pragma omp parallel for schedule(static)
     for (int64_t j = 0; j < R; ++j)                           // step 1, L55, L65
         for (int s = 0; s < o->N; ++s) o->spin[(size_t)j * o->N + s] = x_init(seed, j, (uint32_t)s);
@@ -601,7 +656,19 @@ int ora_hist_accumulate(Oracle* o, double beta) {
     if (!o) return ORA_ERR_INVALID_ARG;
     std::vector<int32_t> E, M; all_energies(o, E, M);
     hist_fold_for(E, o->N, o->lnZ, beta, o->Hsum.data(), o->lnD.data());
+    mag_fold_for(E, M, o->N, o->A1sum.data(), o->A2sum.data());
     return ORA_OK;
+}
+
+int ora_get_mag_sums(const Oracle* o, int64_t* A1, int64_t* A2) {
+    if (!o) return ORA_ERR_INVALID_ARG;
+    if (A1) std::memcpy(A1, o->A1sum.data(), sizeof(int64_t) * (o->N + 1));
+    if (A2) std::memcpy(A2, o->A2sum.data(), sizeof(int64_t) * (o->N + 1));
+    return ORA_OK;
+}
+int ora_reweight_mag(const Oracle* o, int n, const double* betas, double* absm, double* m2) {
+    if (!o) return ORA_ERR_INVALID_ARG;
+    return ora_reweight_mag_of(o->L, o->Hsum.data(), o->lnD.data(), o->A1sum.data(), o->A2sum.data(), n, betas, absm, m2);
 }
 
 int ora_get_histogram(const Oracle* o, int64_t* Hsum, double* lnD) {

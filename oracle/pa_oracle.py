@@ -45,6 +45,10 @@ def lib():
         L.ora_hist_fold_of.argtypes = [i32, i64, vp, dbl, dbl, vp, vp]; L.ora_hist_fold_of.restype = i32
         L.ora_reweight_of.argtypes = [i32, vp, vp, i32, vp, vp, vp, vp]; L.ora_reweight_of.restype = i32
         L.ora_reweight.argtypes = [vp, i32, vp, vp, vp, vp]; L.ora_reweight.restype = i32
+        L.ora_reweight_mag_of.argtypes = [i32, vp, vp, vp, vp, i32, vp, vp, vp]; L.ora_reweight_mag_of.restype = i32
+        L.ora_mag_fold_of.argtypes = [i32, i64, vp, vp, vp, vp]; L.ora_mag_fold_of.restype = i32
+        L.ora_get_mag_sums.argtypes = [vp, vp, vp]; L.ora_get_mag_sums.restype = i32
+        L.ora_reweight_mag.argtypes = [vp, i32, vp, vp, vp]; L.ora_reweight_mag.restype = i32
         L.ora_weighted_average.argtypes = [i32, vp, vp, i32, vp, vp]; L.ora_weighted_average.restype = i32
         L.ora_create.argtypes = [i32, i64, u64, vp]; L.ora_create.restype = i32
         L.ora_destroy.argtypes = [vp]; L.ora_destroy.restype = None
@@ -180,6 +184,22 @@ def reweight_of(L, Hsum, lnD, betas):
     return {"lnZ": lnZ, "e": e, "C": Cv}
 
 
+def reweight_mag_of(L, Hsum, lnD, A1, A2, betas):
+    """O14: <|m|>, <m^2> at every beta from the Eq. 9 sums and the microcanonical magnetisation sums."""
+    Hsum = np.ascontiguousarray(Hsum, dtype=np.int64); lnD = np.ascontiguousarray(lnD, dtype=np.float64)
+    A1 = np.ascontiguousarray(A1, dtype=np.int64); A2 = np.ascontiguousarray(A2, dtype=np.int64)
+    betas = np.ascontiguousarray(betas, dtype=np.float64)
+    a = np.empty(betas.size); q = np.empty(betas.size)
+    _check(lib().ora_reweight_mag_of(L, _p(Hsum), _p(lnD), _p(A1), _p(A2), betas.size, _p(betas), _p(a), _p(q)), "reweight_mag_of")
+    return {"absm": a, "m2": q}
+
+
+def mag_fold_of(L, E, M, A1, A2):
+    E = np.ascontiguousarray(E, dtype=np.int32); M = np.ascontiguousarray(M, dtype=np.int32)
+    assert A1.dtype == np.int64 and A2.dtype == np.int64
+    _check(lib().ora_mag_fold_of(L, E.size, _p(E), _p(M), _p(A1), _p(A2)), "mag_fold_of")
+
+
 def weighted_average(lnZ, A):
     """O13 (Eq. 6-7): A[M][nobs] -> (A~[nobs], omega[M])."""
     lnZ = np.ascontiguousarray(lnZ, dtype=np.float64); A = np.ascontiguousarray(A, dtype=np.float64)
@@ -237,6 +257,17 @@ class Oracle:
         lnZ = np.empty(betas.size); e = np.empty(betas.size); Cv = np.empty(betas.size)
         _check(lib().ora_reweight(self._h, betas.size, _p(betas), _p(lnZ), _p(e), _p(Cv)), "reweight")
         return {"lnZ": lnZ, "e": e, "C": Cv}
+
+    def mag_sums(self):
+        A1 = np.empty(self.N + 1, dtype=np.int64); A2 = np.empty(self.N + 1, dtype=np.int64)
+        _check(lib().ora_get_mag_sums(self._h, _p(A1), _p(A2)), "get_mag_sums")
+        return A1, A2
+
+    def reweight_mag(self, betas):
+        betas = np.ascontiguousarray(betas, dtype=np.float64)
+        a = np.empty(betas.size); q = np.empty(betas.size)
+        _check(lib().ora_reweight_mag(self._h, betas.size, _p(betas), _p(a), _p(q)), "reweight_mag")
+        return {"absm": a, "m2": q}
 
     def set_rng_mode(self, mode):
         _check(lib().ora_set_rng_mode(self._h, int(mode)), "set_rng_mode")

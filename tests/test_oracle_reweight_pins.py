@@ -90,6 +90,52 @@ def test_reweight_from_pa_runs_matches_kaufman_L16():
 
 
 # ---------------------------------------------------------------------------------------------
+# O14 magnetisation reweighting from microcanonical sums (L129)
+# ---------------------------------------------------------------------------------------------
+
+def test_reweight_mag_exact_microcanonical_sums_in_exact_averages_out():
+    # exact g(E) and the exact sums of |M| and M^2 over all states of each energy level (enumeration of the 4x4 torus):
+    # the reweighted <|m|>, <m^2> must be the exact canonical values at every beta
+    L, N = 4, 16
+    E, M = ex.enumerate_states(L)
+    H = np.zeros(N + 1, dtype=np.int64); A1 = np.zeros(N + 1, dtype=np.int64); A2 = np.zeros(N + 1, dtype=np.int64)
+    np.add.at(H, (E + 2 * N) // 4, 1)
+    np.add.at(A1, (E + 2 * N) // 4, np.abs(M))
+    np.add.at(A2, (E + 2 * N) // 4, M * M)
+    betas = np.array([0.0, 0.2, 0.4406868, 0.8, 2.0])
+    out = po.reweight_mag_of(L, H, np.zeros(N + 1), A1, A2, betas)
+    for i, b in enumerate(betas):
+        exact = ex.exact_small(float(b), L)
+        assert out["absm"][i] == pytest.approx(exact["absm"], rel=1e-12)
+        assert out["m2"][i] == pytest.approx(exact["m2"], rel=1e-12)
+    # the fold itself: |M| and M^2 land on the level of their replica's energy, exact integers
+    A1f = np.zeros(N + 1, dtype=np.int64); A2f = np.zeros(N + 1, dtype=np.int64)
+    po.mag_fold_of(L, E[:5000].astype(np.int32), M[:5000].astype(np.int32), A1f, A2f)
+    w1 = np.zeros(N + 1, dtype=np.int64); w2 = np.zeros(N + 1, dtype=np.int64)
+    np.add.at(w1, (E[:5000] + 2 * N) // 4, np.abs(M[:5000])); np.add.at(w2, (E[:5000] + 2 * N) // 4, M[:5000] ** 2)
+    assert np.array_equal(A1f, w1) and np.array_equal(A2f, w2)
+
+
+def test_reweight_mag_from_pa_runs_matches_exact_L4():
+    L, R, theta = 4, 4000, 5
+    betas = [i / 40 for i in range(41)]
+    grid = np.array([0.0125, 0.2375, 0.44, 0.6625, 0.9875])
+    runs = _runs(L, R, betas, theta, list(range(400, 412)))
+    vals = {k: np.array([o.reweight_mag(grid)[k] for o, _ in runs]) for k in ("absm", "m2")}
+    for i, b in enumerate(grid):
+        exact = ex.exact_small(float(b), L)
+        for k in ("absm", "m2"):
+            v = vals[k][:, i]
+            sigma = v.std(ddof=1) / math.sqrt(len(runs))
+            assert abs(v.mean() - exact[k]) < 5 * sigma + 1e-12, (b, k, v.mean(), exact[k], sigma)
+    # sum over levels of the folded sums = sum over all folded replicas (the direct observables times R N, R N^2)
+    o, obs = runs[0]
+    A1, A2 = o.mag_sums()
+    assert A1.sum() == round(sum(x["absm"] * x["R"] * L * L for x in obs))
+    assert A2.sum() == round(sum(x["m2"] * x["R"] * (L * L) ** 2 for x in obs))
+
+
+# ---------------------------------------------------------------------------------------------
 # O13 weighted averages over M independent runs (Eq. 6-7)
 # ---------------------------------------------------------------------------------------------
 
