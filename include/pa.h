@@ -128,13 +128,19 @@ int pa_hist_accumulate(pa_t* h, double beta);
 /* Hsum: int64[N+1], lnD: double[N+1] (either may be NULL); ln Omega(E_m) = ln Hsum[m] - lnD[m]. */
 int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD);
 
-/* Multi-histogram reweighting (Sec. 2.4; O12): from the sums accumulated so far, the density of
+/* Multi-histogram reweighting (Sec. 2.4; O12, O14): from the sums accumulated so far, the density of
  * states ln Omega(E_m) = ln Hsum[m] - lnD[m] (Eq. 9) and, for each of the n inverse temperatures betas[i]
  * (any values, not only simulated ones), lnZ[i] = ln sum_m Omega_m exp(-beta E_m) (= -beta F, Eq. 4),
- * e[i] = <E>/N and C[i] = beta^2 (<E^2> - <E>^2)/N (Eq. 3).  betas, lnZ, e, C: double[n], host or device
- * (all four of the same kind); outputs may be NULL.  1 <= n <= 2^20.  PA_ERR_INVALID_ARG if no histogram has
- * been accumulated.  Does not change the population.  Synchronises if the buffers are host pointers. */
-int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, double* C);
+ * e[i] = <E>/N and C[i] = beta^2 (<E^2> - <E>^2)/N (Eq. 3), and -- the generalisation to magnetisations of L129 --
+ * absm[i] = <|m|>, m2[i] = <m^2> from the microcanonical sums that pa_hist_accumulate keeps per energy level
+ * (A1[m] = sum |M_j|, A2[m] = sum M_j^2 over all folded replicas with E_j = E_m): <|m|> = sum_m p_m A1[m]/Hsum[m] / N.
+ * betas and the outputs: double[n], host or device (all of the same kind); outputs may be NULL.  1 <= n <= 2^20.
+ * PA_ERR_INVALID_ARG if no histogram has been accumulated.  Does not change the population.  Synchronises if the
+ * buffers are host pointers. */
+int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, double* C, double* absm, double* m2);
+
+/* The microcanonical magnetisation sums (O14): A1, A2: int64[N+1], host or device, either may be NULL. */
+int pa_get_mag_sums(pa_t* h, int64_t* A1, int64_t* A2);
 
 /* Weighted average of M independent runs (Sec. 2.2, Eq. 6-7; O13): omega_m = exp(lnZ_m) /
  * sum_m exp(lnZ_m) with lnZ_m = -beta F_m(beta) = pa_lnZ of run m at this temperature, A_out[k] =

@@ -20,7 +20,7 @@ void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const cha
 }
 
 struct PaLayout {
-    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, lnD, scal, slots, stage, total;
+    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, lnD, A1, A2, scal, slots, stage, total;
     size_t stage_bytes;
     int64_t R_cap, G_cap, tiles;
 };
@@ -48,6 +48,8 @@ static PaLayout pa_layout(int L, int64_t R) {
     y.Hsum = take((N + 1) * 8);
     y.Hcur = take((N + 1) * 4);
     y.lnD = take((N + 1) * 8);
+    y.A1 = take((N + 1) * 8);
+    y.A2 = take((N + 1) * 8);
     y.scal = take(sizeof(PaScalars));
     y.slots = take((size_t)PA_SLOTS_CAP * 8);
     y.stage_bytes = (size_t)y.R_cap * N < PA_STAGE_BYTES ? pa_align_up((size_t)y.R_cap * N) : PA_STAGE_BYTES;
@@ -159,6 +161,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     h->partials = (double*)(b + y.partials); h->runsum = (double*)(b + y.runsum); h->wtab = (double*)(b + y.wtab);
     h->scan_state = (unsigned long long*)(b + y.scan);
     h->Hsum = (unsigned long long*)(b + y.Hsum); h->Hcur = (uint32_t*)(b + y.Hcur); h->lnD = (double*)(b + y.lnD);
+    h->A1 = (unsigned long long*)(b + y.A1); h->A2 = (unsigned long long*)(b + y.A2);
     h->d_scal = (PaScalars*)(b + y.scal);
     h->d_slots = (int64_t*)(b + y.slots);
     h->stage = (int8_t*)(b + y.stage); h->stage_bytes = y.stage_bytes;
@@ -173,6 +176,8 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
         cudaMemsetAsync(h->d_scal, 0, sizeof(PaScalars), h->stream);
         cudaMemsetAsync(h->Hsum, 0, ((size_t)h->N + 1) * 8, h->stream);
         cudaMemsetAsync(h->Hcur, 0, ((size_t)h->N + 1) * 4, h->stream);
+        cudaMemsetAsync(h->A1, 0, ((size_t)h->N + 1) * 8, h->stream);
+        cudaMemsetAsync(h->A2, 0, ((size_t)h->N + 1) * 8, h->stream);
         for (int m = 0; m <= h->N; ++m) h->h_wtab[m] = -INFINITY;
         if (cudaMemcpyAsync(h->lnD, h->h_wtab, ((size_t)h->N + 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
         if (rc == PA_OK) rc = pa_launch_init(h);
@@ -343,9 +348,9 @@ int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD) {
     return rc;
 }
 
-int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, double* C) {
+int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, double* C, double* absm, double* m2) {
     if (!h || !betas || n < 1 || n > (1 << 20)) return PA_ERR_INVALID_ARG;
-    if ((size_t)n * 32 > h->stage_bytes) return PA_ERR_INVALID_ARG;
+    if ((size_t)n * 48 > h->stage_bytes) return PA_ERR_INVALID_ARG;
     // any histogram yet?  (Hsum is all zero until the first pa_hist_accumulate)
     if (!h->hist_any) return PA_ERR_INVALID_ARG;
     double* d_io = (double*)h->stage;
@@ -353,9 +358,17 @@ int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, dou
     PA_CUDA(h, cudaMemcpyAsync(d_io, betas, (size_t)n * 8, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
     int rc = pa_launch_reweight(h, n, d_io);
     if (rc != PA_OK) return rc;
-    double* outs[3] = {lnZ, e, C};
-    for (int i = 0; i < 3 && rc == PA_OK; ++i)
+    double* outs[5] = {lnZ, e, C, absm, m2};
+    for (int i = 0; i < 5 && rc == PA_OK; ++i)
         if (outs[i]) rc = pa_copy_out(h, outs[i], d_io + (size_t)(i + 1) * n, (size_t)n * 8, nullptr);
+    return rc;
+}
+
+int pa_get_mag_sums(pa_t* h, int64_t* A1, int64_t* A2) {
+    if (!h) return PA_ERR_INVALID_ARG;
+    int rc = PA_OK;
+    if (A1) rc = pa_copy_out(h, A1, h->A1, ((size_t)h->N + 1) * 8, nullptr);
+    if (rc == PA_OK && A2) rc = pa_copy_out(h, A2, h->A2, ((size_t)h->N + 1) * 8, nullptr);
     return rc;
 }
 

@@ -104,6 +104,7 @@ struct pa_handle {
     unsigned long long* Hsum;           // [N+1]
     uint32_t* Hcur;                     // [N+1] histogram of the current temperature
     double* lnD;                        // [N+1]
+    unsigned long long *A1, *A2;        // [N+1] sums of |M_j| and M_j^2 per energy level over all folded replicas (O14)
     int64_t* d_slots;                   // slot list for pa_get_spins_at
     int8_t* stage;                      // staging for unpacked spin export/import
     size_t stage_bytes;
@@ -141,7 +142,7 @@ int pa_launch_overlap(pa_handle* h, int Emin);                         // TREE10
 int pa_launch_plan(pa_handle* h, int Emin);                            // tau, r, scan, parent map, R_new
 int pa_launch_copy(pa_handle* h);                                      // new[d] = old[parent(d)], d < R_new (read on the device)
 int pa_launch_hist(pa_handle* h, double beta);
-int pa_launch_reweight(pa_handle* h, int n, double* d_io);              // O12: d_io = [betas | lnZ | e | C], n each
+int pa_launch_reweight(pa_handle* h, int n, double* d_io);              // O12, O14: d_io = [betas | lnZ | e | C | absm | m2], n each
 cudaError_t pa_run_wavg(int M, const double* d_lnZ, const double* d_A, int nobs, double* d_out, double* d_omega, cudaStream_t st);
 int pa_launch_unpack(pa_handle* h, const int64_t* d_slots, int64_t j0, int64_t n, int8_t* d_out);
 int pa_launch_pack(pa_handle* h, int64_t j0, int64_t n, const int8_t* d_in);

@@ -42,9 +42,17 @@ int pa_launch_init(pa_handle* h) {
 }
 
 // a9 (Eq. 9; O9)
-__global__ void pa_hist_kernel(const int32_t* __restrict__ E, long long R, int N, uint32_t* __restrict__ Hcur) {
-    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x)
-        atomicAdd(&Hcur[(E[j] + 2 * N) >> 2], 1u);
+// also O14 (L129): the microcanonical magnetisation sums A1[m] += |M_j|, A2[m] += M_j^2 (exact integers, order-free)
+__global__ void pa_hist_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, long long R, int N,
+                               uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ A1, unsigned long long* __restrict__ A2) {
+    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x) {
+        const int m = (E[j] + 2 * N) >> 2;
+        const long long mj = M[j];
+        const unsigned long long a = (unsigned long long)(mj < 0 ? -mj : mj);
+        atomicAdd(&Hcur[m], 1u);
+        atomicAdd(&A1[m], a);
+        atomicAdd(&A2[m], a * a);
+    }
 }
 __global__ void pa_hist_fold_kernel(uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ Hsum,
                                     double* __restrict__ lnD, int N, double lnR_minus_lnZ, double beta) {
@@ -64,7 +72,7 @@ __global__ void pa_hist_fold_kernel(uint32_t* __restrict__ Hcur, unsigned long l
 int pa_launch_hist(pa_handle* h, double beta) {
     int blocks = (int)((h->R_cur + 255) / 256);
     if (blocks > 1184) blocks = 1184;
-    pa_hist_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->R_cur, h->N, h->Hcur);
+    pa_hist_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->M, h->R_cur, h->N, h->Hcur, h->A1, h->A2);
     const double c = log((double)h->R_cur) - h->lnZ;
     pa_hist_fold_kernel<<<(h->N + 1 + 255) / 256, 256, 0, h->stream>>>(h->Hcur, h->Hsum, h->lnD, h->N, c, beta);
     PA_CUDA(h, cudaGetLastError());
@@ -102,8 +110,10 @@ __device__ __forceinline__ double pa_block_reduce(double v, double* sh) {
 }
 
 __global__ void __launch_bounds__(256)
-pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __restrict__ lnD, int N,
-                   const double* __restrict__ betas, double* __restrict__ lnZ, double* __restrict__ e, double* __restrict__ C) {
+pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __restrict__ lnD,
+                   const unsigned long long* __restrict__ A1, const unsigned long long* __restrict__ A2, int N,
+                   const double* __restrict__ betas, double* __restrict__ lnZ, double* __restrict__ e, double* __restrict__ C,
+                   double* __restrict__ absm, double* __restrict__ m2) {
     __shared__ double sh[33];
     const double beta = betas[blockIdx.x];
     double amax = -INFINITY;
@@ -113,16 +123,20 @@ pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __
         amax = fmax(amax, (log((double)H) - lnD[m]) - beta * (double)(-2 * N + 4 * m));
     }
     amax = pa_block_reduce<true>(amax, sh);
-    double s0 = 0.0, s1 = 0.0;
+    double s0 = 0.0, s1 = 0.0, sa = 0.0, sq = 0.0;
     for (int m = threadIdx.x; m <= N; m += blockDim.x) {
         const unsigned long long H = Hsum[m];
         if (H == 0ull) continue;
         const double Em = (double)(-2 * N + 4 * m);
         const double p = exp(((log((double)H) - lnD[m]) - beta * Em) - amax);
         s0 += p; s1 += Em * p;
+        sa += p * ((double)A1[m] / (double)H);           // O14: microcanonical mean of |M| at level m
+        sq += p * ((double)A2[m] / (double)H);
     }
     s0 = pa_block_reduce<false>(s0, sh);
     s1 = pa_block_reduce<false>(s1, sh);
+    sa = pa_block_reduce<false>(sa, sh);
+    sq = pa_block_reduce<false>(sq, sh);
     const double mean = s1 / s0;
     double s2 = 0.0;
     for (int m = threadIdx.x; m <= N; m += blockDim.x) {
@@ -137,12 +151,16 @@ pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __
         lnZ[blockIdx.x] = amax + log(s0);
         e[blockIdx.x] = mean / (double)N;
         C[blockIdx.x] = beta * beta * (s2 / s0) / (double)N;
+        absm[blockIdx.x] = (sa / s0) / (double)N;
+        m2[blockIdx.x] = (sq / s0) / ((double)N * (double)N);
     }
 }
 
-// d_io: [betas(n) | lnZ(n) | e(n) | C(n)] in device memory
+// d_io: [betas(n) | lnZ(n) | e(n) | C(n) | absm(n) | m2(n)] in device memory
 int pa_launch_reweight(pa_handle* h, int n, double* d_io) {
-    pa_reweight_kernel<<<n, 256, 0, h->stream>>>(h->Hsum, h->lnD, h->N, d_io, d_io + n, d_io + 2 * (size_t)n, d_io + 3 * (size_t)n);
+    const size_t z = (size_t)n;
+    pa_reweight_kernel<<<n, 256, 0, h->stream>>>(h->Hsum, h->lnD, h->A1, h->A2, h->N, d_io, d_io + z, d_io + 2 * z, d_io + 3 * z,
+                                                 d_io + 4 * z, d_io + 5 * z);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;

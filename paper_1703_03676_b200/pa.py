@@ -75,7 +75,8 @@ def lib():
         "pa_observables": ([vp, dbl, C.POINTER(pa_obs_t)], i32),
         "pa_hist_accumulate": ([vp, dbl], i32),
         "pa_get_histogram": ([vp, vp, vp], i32),
-        "pa_reweight": ([vp, i32, vp, vp, vp, vp], i32),
+        "pa_reweight": ([vp, i32, vp, vp, vp, vp, vp, vp], i32),
+        "pa_get_mag_sums": ([vp, vp, vp], i32),
         "pa_weighted_average": ([i32, vp, vp, i32, vp, vp], i32),
         "pa_get_spins": ([vp, i64, i64, vp], i32),
         "pa_get_spins_at": ([vp, vp, i64, vp], i32),
@@ -295,11 +296,17 @@ class Population:
         return H, D
 
     def reweight(self, betas):
-        """Sec. 2.4 (Eq. 9): lnZ, e, C at every beta of `betas` from the accumulated multi-histogram sums."""
+        """Sec. 2.4 (Eq. 9): lnZ, e, C, <|m|>, <m^2> at every beta of `betas` from the accumulated multi-histogram sums."""
         betas = np.ascontiguousarray(betas, dtype=np.float64)
-        lnZ = np.empty(betas.size); e = np.empty(betas.size); Cv = np.empty(betas.size)
-        self._check(lib().pa_reweight(self._h, betas.size, _ptr(betas), _ptr(lnZ), _ptr(e), _ptr(Cv)), "pa_reweight")
-        return {"lnZ": lnZ, "e": e, "C": Cv}
+        out = {k: np.empty(betas.size) for k in ("lnZ", "e", "C", "absm", "m2")}
+        self._check(lib().pa_reweight(self._h, betas.size, _ptr(betas), *[_ptr(out[k]) for k in ("lnZ", "e", "C", "absm", "m2")]),
+                    "pa_reweight")
+        return out
+
+    def mag_sums(self):
+        A1 = np.empty(self.N + 1, dtype=np.int64); A2 = np.empty(self.N + 1, dtype=np.int64)
+        self._check(lib().pa_get_mag_sums(self._h, _ptr(A1), _ptr(A2)), "pa_get_mag_sums")
+        return A1, A2
 
     # state export / import
     def get_spins(self, j0=0, nrep=None):

@@ -37,7 +37,7 @@ int main(int argc, char** argv) {
         beta = next;
         if (beta >= 0.5) break;
     }
-    if (pa_reweight(h, 1, grid, lnZ, e, C) != PA_OK) return 13;
+    if (pa_reweight(h, 1, grid, lnZ, e, C, NULL, NULL) != PA_OK) return 13;
     printf("reweighted to beta=%.2f: lnZ=%.6f e=%.6f C=%.6f\n", grid[0], lnZ[0], e[0], C[0]);
     if (pa_resample(h, 0.5, 0.4, &R_new) != PA_ERR_INVALID_ARG) return 14;     /* beta' < beta */
     free(E);

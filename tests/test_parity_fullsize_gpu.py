@@ -89,6 +89,7 @@ def checked_step(g, wl, beta_prev, beta, rng, n_slots, lnZ_ref, hist=None, rng_m
     if hist is not None:
         g.hist_accumulate(beta)
         po.hist_fold_of(L, E2, lnZ, beta, hist[0], hist[1])
+        po.mag_fold_of(L, E2, M2, hist[2], hist[3])
     return og, lnZ
 
 
@@ -101,9 +102,10 @@ def plain_step(g, wl, beta_prev, beta, lnZ_ref, hist=None):
     og = g.observables(beta)
     lnZ = lnZ_ref + plan["lnQ"]
     if hist is not None:
-        E2, _ = g.energies()
+        E2, M2 = g.energies()
         g.hist_accumulate(beta)
         po.hist_fold_of(wl.L, E2, lnZ, beta, hist[0], hist[1])
+        po.mag_fold_of(wl.L, E2, M2, hist[2], hist[3])
     return og, lnZ
 
 
@@ -191,12 +193,13 @@ def test_config4_full_size_adaptive_multihistogram():
     g = pa.Population(wl.L, wl.R, wl.seed)
     _check_initial(g, wl, rng, 512)
     N = wl.N
-    hist = (np.zeros(N + 1, dtype=np.int64), np.full(N + 1, -np.inf))
+    hist = (np.zeros(N + 1, dtype=np.int64), np.full(N + 1, -np.inf), np.zeros(N + 1, dtype=np.int64), np.zeros(N + 1, dtype=np.int64))
     lnZ = N * np.log(2.0)
     beta = wl.beta0
-    E, _ = g.energies()
+    E, M = g.energies()
     g.observables(beta); g.hist_accumulate(beta)
     po.hist_fold_of(wl.L, E, lnZ, beta, hist[0], hist[1])
+    po.mag_fold_of(wl.L, E, M, hist[2], hist[3])
     n_steps = 100000 if RUN_ALL else 24
     checked = {1, 2, 3, 20, n_steps}
     i = 0
@@ -220,4 +223,12 @@ def test_config4_full_size_adaptive_multihistogram():
     fin = np.isfinite(hist[1])
     assert np.array_equal(np.isfinite(Dg), fin)
     assert np.allclose(Dg[fin], hist[1][fin], rtol=REL, atol=0)
+    A1, A2 = g.mag_sums()                                          # O14: exact integers
+    assert np.array_equal(A1, hist[2]) and np.array_equal(A2, hist[3])
+    # O12 + O14 at full size: the reweighted curves from the device's sums against the oracle's from its own
+    grid = np.linspace(0.0, beta, 25)
+    rg = g.reweight(grid)
+    ro = {**po.reweight_of(wl.L, hist[0], hist[1], grid), **po.reweight_mag_of(wl.L, hist[0], hist[1], hist[2], hist[3], grid)}
+    for k in ("lnZ", "e", "C", "absm", "m2"):
+        assert np.allclose(rg[k], ro[k], rtol=REL, atol=1e-300), k
     g.close()

@@ -269,23 +269,26 @@ def test_adaptive_run_with_multihistogram():
         assert g.overlap(d) == o.overlap(d)
     # O12: reweighting of the accumulated sums to a fine beta grid (Sec. 2.4), inside and beyond the simulated range
     grid = np.concatenate([np.linspace(0.0, bg[-1], 37), [bg[-1] + 0.05, 1.5]])
-    rg, ro = g.reweight(grid), o.reweight(grid)
-    for k in ("lnZ", "e", "C"):
+    rg, ro = g.reweight(grid), {**o.reweight(grid), **o.reweight_mag(grid)}
+    for k in ("lnZ", "e", "C", "absm", "m2"):
         assert np.allclose(rg[k], ro[k], rtol=REL, atol=1e-300), k
+    # O14: the microcanonical magnetisation sums are exact integers
+    for a, b in zip(g.mag_sums(), o.mag_sums()):
+        assert np.array_equal(a, b)
 
 
 def test_reweight_errors_and_device_buffers():
     L, R = 8, 300
     g, o = pa.Population(L, R, 3), po.Oracle(L, R, 3)
     grid = np.array([0.1, 0.2])
-    rc = pa.lib().pa_reweight(g._h, 2, pa._ptr(grid), None, None, None)
+    rc = pa.lib().pa_reweight(g._h, 2, pa._ptr(grid), None, None, None, None, None)
     assert rc == pa.PA_ERR_INVALID_ARG                                # nothing accumulated yet
     obs_g = pa_driver.run_fixed(g, [0.0, 0.1, 0.2, 0.3], 2, hist=True)
     pa_driver.run_fixed(o, [0.0, 0.1, 0.2, 0.3], 2, hist=True)
-    assert pa.lib().pa_reweight(g._h, 0, pa._ptr(grid), None, None, None) == pa.PA_ERR_INVALID_ARG
+    assert pa.lib().pa_reweight(g._h, 0, pa._ptr(grid), None, None, None, None, None) == pa.PA_ERR_INVALID_ARG
     want = o.reweight(grid)
     tb = torch.tensor(grid, device="cuda"); te = torch.empty(2, dtype=torch.float64, device="cuda")
-    assert pa.lib().pa_reweight(g._h, 2, pa._ptr(tb), None, pa._ptr(te), None) == pa.PA_OK
+    assert pa.lib().pa_reweight(g._h, 2, pa._ptr(tb), None, pa._ptr(te), None, None, None) == pa.PA_OK
     torch.cuda.synchronize()
     assert np.allclose(te.cpu().numpy(), want["e"], rtol=REL)
     assert g.population == obs_g[-1]["R"]                             # state untouched
