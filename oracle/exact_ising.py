@@ -23,6 +23,35 @@ import numpy as np
 # brute force
 # ---------------------------------------------------------------------------------------------
 
+def enumerate_states_j(L, Jx, Jy):
+    """As enumerate_states for H = -sum_<ab> J_ab s_a s_b with couplings Jx[y*L+x] on the bond (x,y)-(x+1,y) and
+    Jy[y*L+x] on the bond (x,y)-(x,y+1), periodic (the generalisation of PAPER.md L313)."""
+    N = L * L
+    assert N <= 20
+    states = np.arange(1 << N, dtype=np.int64)
+    spins = ((states[:, None] >> np.arange(N)[None, :]) & 1).astype(np.int8) * 2 - 1
+    grid = spins.reshape(-1, L, L).astype(np.int64)
+    jx = np.asarray(Jx, dtype=np.int64).reshape(1, L, L); jy = np.asarray(Jy, dtype=np.int64).reshape(1, L, L)
+    E = -(jx * grid * np.roll(grid, -1, axis=2)).sum(axis=(1, 2)) - (jy * grid * np.roll(grid, -1, axis=1)).sum(axis=(1, 2))
+    M = grid.sum(axis=(1, 2))
+    return E.astype(np.int64), M.astype(np.int64)
+
+
+def exact_small_j(beta, L, Jx, Jy):
+    """Exact canonical averages of the +-J sample by enumeration."""
+    N = L * L
+    E, M = enumerate_states_j(L, Jx, Jy)
+    Emin = E.min()
+    w = np.exp(-beta * (E - Emin).astype(np.float64))
+    p = w / w.sum()
+    e1 = (p * E).sum(); e2 = (p * E.astype(np.float64) ** 2).sum()
+    m = M.astype(np.float64) / N
+    lnZ = math.log(w.sum()) - beta * Emin
+    return {"e": e1 / N, "C": beta * beta * (e2 - e1 * e1) / N, "absm": (p * np.abs(m)).sum(), "m2": (p * m ** 2).sum(),
+            "lnZ": lnZ, "betaF_per_N": -lnZ / N, "S_per_N": beta * e1 / N + lnZ / N,
+            "pE": {int(v): float(p[E == v].sum()) for v in np.unique(E)}}
+
+
 @lru_cache(maxsize=None)
 def enumerate_states(L=4):
     """All 2^(L*L) states: returns (E, M) int arrays indexed by the state's bit pattern

@@ -28,6 +28,9 @@
 //                          e, C, lnZ at off-grid beta from L=16 runs (5 sigma over seeds)
 //   magnetisation reweighting (O14) exact g(E) and exact microcanonical |M|, M^2 sums of the 4x4 torus in, exact
 //                          enumeration <|m|>, <m^2> out; L=4 runs at off-grid beta (5 sigma over seeds)
+//   couplings J = +-1 (O15) gauge invariance (Mattis couplings J_ab = eps_a eps_b reproduce the gauge-transformed ferromagnetic
+//                          trajectory and its energies exactly); brute-force enumeration of a frustrated 4x4 sample
+//                          (Boltzmann chi^2, whole PA runs, reweighting)
 //   weighted averages (O13) closed forms (weight ratios, M = 1, equal F, shift invariance, dominance);
 //                          unbiasedness of exp(lnZ_m) and removal of the small-R bias at L=4 (L99)
 //   LCG-assisted stream (O11) recurrence against big-integer arithmetic with the constants the
@@ -139,8 +142,12 @@ uint32_t threshold(double p) {
 // ---------------------------------------------------------------------------------------------
 enum { RNG_PHILOX = 0, RNG_LCG = 1 };   // O1 (one Philox number per spin) / O11 (Philox-seeded LCG)
 
+// O15 (L313 "the case of different couplings including spin glasses"): bimodal couplings J = +-1 on the bonds,
+// H = -sum_<ab> J_ab s_a s_b.  Jx[s] couples site s = (x,y) to (x+1,y), Jy[s] couples it to (x,y+1) (periodic);
+// NULL = ferromagnet (Eq. 10).  u then counts the UNSATISFIED bonds of the centre spin (J s_a s_b = -1) and
+// dE = 8 - 4u as before, so the thresholds and the acceptance rule are unchanged.
 void sweep_one_replica(uint8_t* sp, int L, uint64_t seed, int64_t slot, uint32_t t,
-                       uint32_t T4, uint32_t T8, int rng_mode) {
+                       uint32_t T4, uint32_t T8, int rng_mode, const int8_t* Jx = nullptr, const int8_t* Jy = nullptr) {
     for (uint32_t c = 0; c < 2; ++c) {
         for (int y = 0; y < L; ++y) {
             for (int x = 0; x < L; ++x) {
@@ -148,8 +155,14 @@ void sweep_one_replica(uint8_t* sp, int L, uint64_t seed, int64_t slot, uint32_t
                 int s = y * L + x;
                 int xm = x == 0 ? L - 1 : x - 1, xp = x == L - 1 ? 0 : x + 1;      // periodic, L137
                 int ym = y == 0 ? L - 1 : y - 1, yp = y == L - 1 ? 0 : y + 1;
-                int u = (sp[y * L + xm] != sp[s]) + (sp[y * L + xp] != sp[s]) +
+                int u;
+                if (!Jx) {
+                    u = (sp[y * L + xm] != sp[s]) + (sp[y * L + xp] != sp[s]) +
                         (sp[ym * L + x] != sp[s]) + (sp[yp * L + x] != sp[s]);
+                } else {                                      // bond unsatisfied iff (spins differ) xor (J = -1) ... for J = +1: differ
+                    u = ((sp[y * L + xm] != sp[s]) != (Jx[y * L + xm] < 0)) + ((sp[y * L + xp] != sp[s]) != (Jx[s] < 0)) +
+                        ((sp[ym * L + x] != sp[s]) != (Jy[ym * L + x] < 0)) + ((sp[yp * L + x] != sp[s]) != (Jy[s] < 0));
+                }
                 uint32_t xr = rng_mode == RNG_LCG ? x_sweep_lcg(seed, slot, L, x, y, t, c)
                                                   : x_sweep(seed, slot, (uint32_t)s, t, c);   // drawn for every (j,s,t)
                 bool flip = (u >= 2) || (u == 1 && xr < T4) || (u == 0 && xr < T8);
@@ -161,14 +174,14 @@ void sweep_one_replica(uint8_t* sp, int L, uint64_t seed, int64_t slot, uint32_t
 
 // O4  Energy and magnetisation of one replica.  Eq. 10 L135 (each bond once: right and down
 // neighbour of every site), L173.  E = -sum_bonds sigma_a sigma_b, M = sum sigma.
-void energy_one_replica(const uint8_t* sp, int L, int32_t* E, int32_t* M) {
+void energy_one_replica(const uint8_t* sp, int L, int32_t* E, int32_t* M, const int8_t* Jx = nullptr, const int8_t* Jy = nullptr) {
     int32_t e = 0, m = 0;
     for (int y = 0; y < L; ++y)
         for (int x = 0; x < L; ++x) {
             int sg = sp[y * L + x] ? 1 : -1;
             int sr = sp[y * L + (x == L - 1 ? 0 : x + 1)] ? 1 : -1;
             int sd = sp[(y == L - 1 ? 0 : y + 1) * L + x] ? 1 : -1;
-            e -= sg * (sr + sd);
+            e -= Jx ? sg * ((int)Jx[y * L + x] * sr + (int)Jy[y * L + x] * sd) : sg * (sr + sd);
             m += sg;
         }
     *E = e; *M = m;
@@ -219,6 +232,8 @@ struct Oracle {
     uint64_t seed = 0;
     uint32_t t = 0;          // global sweep counter
     int rng_mode = RNG_PHILOX;
+    std::vector<int8_t> Jx, Jy;       // [N] bimodal couplings (O15); empty = ferromagnet
+    int e0 = 0;                       // E = -2N + 4m + e0 on every reachable state: e0 = 2 (number of J = -1 bonds) mod 4
     uint32_t k = 0;          // resample counter
     double lnZ = 0.0;        // = -beta F(beta), Eq. 4; starts at N ln 2 (L93)
     double lnQ_last = 0.0;
@@ -236,7 +251,8 @@ void all_energies(const Oracle* o, std::vector<int32_t>& E, std::vector<int32_t>
     E.resize(o->R_cur); M.resize(o->R_cur);
 #pragma omp parallel for schedule(static)
     for (int64_t j = 0; j < o->R_cur; ++j)
-        energy_one_replica(&o->spin[(size_t)j * o->N], o->L, &E[j], &M[j]);
+        energy_one_replica(&o->spin[(size_t)j * o->N], o->L, &E[j], &M[j], o->Jx.empty() ? nullptr : o->Jx.data(),
+                           o->Jy.empty() ? nullptr : o->Jy.data());
 }
 
 // O5 weights for a given dbeta: E_ref = min_j E_j, wtab[d] = exp(-(dbeta*(double)(4d))),
@@ -311,14 +327,14 @@ obs_values observables_for(const std::vector<int32_t>& E, const std::vector<int3
 }
 
 // O9, Eq. 9: fold the energy histogram at beta into the running sums.
-void hist_fold_for(const std::vector<int32_t>& E, int N, double lnZ, double beta, int64_t* Hsum, double* lnD) {
+void hist_fold_for(const std::vector<int32_t>& E, int N, double lnZ, double beta, int64_t* Hsum, double* lnD, int e0 = 0) {
     int64_t R = (int64_t)E.size();
     std::vector<int64_t> H(N + 1, 0);
-    for (int64_t j = 0; j < R; ++j) H[(E[j] + 2 * N) / 4] += 1;
+    for (int64_t j = 0; j < R; ++j) H[(E[j] + 2 * N - e0) / 4] += 1;
     double lnR = std::log((double)R);
     for (int m = 0; m <= N; ++m) {
         Hsum[m] += H[m];
-        double Em = (double)(-2 * N + 4 * m);
+        double Em = (double)(-2 * N + 4 * m + e0);
         // R_i exp[beta_i F(beta_i) - beta_i E], with -beta_i F = lnZ (Eq. 4)
         lnD[m] = logaddexp(lnD[m], lnR - lnZ - beta * Em);
     }
@@ -329,25 +345,25 @@ void hist_fold_for(const std::vector<int32_t>& E, int N, double lnZ, double beta
 //   Z(beta) = sum_m Omega_m exp(-beta E_m),  <E^k> = sum_m E_m^k Omega_m exp(-beta E_m) / Z,
 // evaluated with the largest exponent taken out; the variance is summed about the mean (two passes).
 //   e = <E>/N,  C = beta^2 (<E^2> - <E>^2)/N  (Eq. 3),  ln Z = -beta F (Eq. 4).
-void reweight_for(int N, const int64_t* Hsum, const double* lnD, double beta, double* lnZ, double* e, double* C) {
+void reweight_for(int N, const int64_t* Hsum, const double* lnD, double beta, double* lnZ, double* e, double* C, int e0 = 0) {
     const double ninf = -std::numeric_limits<double>::infinity();
     double amax = ninf;
     for (int m = 0; m <= N; ++m) {
         if (Hsum[m] <= 0) continue;
-        double a = (std::log((double)Hsum[m]) - lnD[m]) - beta * (double)(-2 * N + 4 * m);
+        double a = (std::log((double)Hsum[m]) - lnD[m]) - beta * (double)(-2 * N + 4 * m + e0);
         if (a > amax) amax = a;
     }
     double S0 = 0.0, S1 = 0.0;
     for (int m = 0; m <= N; ++m) {
         if (Hsum[m] <= 0) continue;
-        double Em = (double)(-2 * N + 4 * m);
+        double Em = (double)(-2 * N + 4 * m + e0);
         double p = std::exp(((std::log((double)Hsum[m]) - lnD[m]) - beta * Em) - amax);
         S0 += p; S1 += Em * p;
     }
     double mean = S1 / S0, S2 = 0.0;
     for (int m = 0; m <= N; ++m) {
         if (Hsum[m] <= 0) continue;
-        double Em = (double)(-2 * N + 4 * m);
+        double Em = (double)(-2 * N + 4 * m + e0);
         double p = std::exp(((std::log((double)Hsum[m]) - lnD[m]) - beta * Em) - amax);
         S2 += (Em - mean) * (Em - mean) * p;
     }
@@ -361,26 +377,26 @@ void reweight_for(int N, const int64_t* Hsum, const double* lnD, double beta, do
 // |M| (M^2) at fixed energy does not depend on beta, so the pooled ratio A[m]/Hsum[m] estimates it from all temperatures, and
 //   <|m|>(beta) = sum_m p_m(beta) (A1[m]/Hsum[m]) / N,   <m^2>(beta) = sum_m p_m(beta) (A2[m]/Hsum[m]) / N^2,
 // with p_m = Omega_m exp(-beta E_m) / Z from Eq. 9 exactly as in reweight_for.
-void mag_fold_for(const std::vector<int32_t>& E, const std::vector<int32_t>& M, int N, int64_t* A1, int64_t* A2) {
+void mag_fold_for(const std::vector<int32_t>& E, const std::vector<int32_t>& M, int N, int64_t* A1, int64_t* A2, int e0 = 0) {
     for (size_t j = 0; j < E.size(); ++j) {
-        int m = (E[j] + 2 * N) / 4;
+        int m = (E[j] + 2 * N - e0) / 4;
         int64_t a = M[j] < 0 ? -(int64_t)M[j] : (int64_t)M[j];
         A1[m] += a; A2[m] += a * a;
     }
 }
 void reweight_mag_for(int N, const int64_t* Hsum, const double* lnD, const int64_t* A1, const int64_t* A2, double beta,
-                      double* absm, double* m2) {
+                      double* absm, double* m2, int e0 = 0) {
     const double ninf = -std::numeric_limits<double>::infinity();
     double amax = ninf;
     for (int m = 0; m <= N; ++m) {
         if (Hsum[m] <= 0) continue;
-        double a = (std::log((double)Hsum[m]) - lnD[m]) - beta * (double)(-2 * N + 4 * m);
+        double a = (std::log((double)Hsum[m]) - lnD[m]) - beta * (double)(-2 * N + 4 * m + e0);
         if (a > amax) amax = a;
     }
     double S0 = 0.0, Sa = 0.0, Sq = 0.0;
     for (int m = 0; m <= N; ++m) {
         if (Hsum[m] <= 0) continue;
-        double Em = (double)(-2 * N + 4 * m);
+        double Em = (double)(-2 * N + 4 * m + e0);
         double p = std::exp(((std::log((double)Hsum[m]) - lnD[m]) - beta * Em) - amax);
         S0 += p;
         Sa += p * ((double)A1[m] / (double)Hsum[m]);
@@ -562,6 +578,48 @@ int ora_create(int L, int64_t R, uint64_t seed, Oracle** out) {
 }
 
 void ora_destroy(Oracle* o) { delete o; }
+
+// O15: bimodal couplings, Jx[s] = bond (x,y)-(x+1,y), Jy[s] = bond (x,y)-(x,y+1), values +1 / -1, s = y*L + x.
+// Both NULL: back to the ferromagnet.  Only before any histogram has been folded (the level offset e0 is part of the sums).
+int ora_set_couplings(Oracle* o, const int8_t* Jx, const int8_t* Jy) {
+    if (!o || ((Jx == nullptr) != (Jy == nullptr))) return ORA_ERR_INVALID_ARG;
+    for (int m = 0; m <= o->N; ++m) if (o->Hsum[m] != 0) return ORA_ERR_INVALID_ARG;
+    if (!Jx) { o->Jx.clear(); o->Jy.clear(); o->e0 = 0; return ORA_OK; }
+    int64_t n_af = 0;
+    for (int s = 0; s < o->N; ++s) {
+        if ((Jx[s] != 1 && Jx[s] != -1) || (Jy[s] != 1 && Jy[s] != -1)) return ORA_ERR_INVALID_ARG;
+        n_af += (Jx[s] < 0) + (Jy[s] < 0);
+    }
+    o->Jx.assign(Jx, Jx + o->N); o->Jy.assign(Jy, Jy + o->N);
+    // E = 2 (unsatisfied bonds) - 2N, and a spin flip changes the number of unsatisfied bonds by 4 - 2u (even), so its parity
+    // is that of the all-up state, i.e. of the number of J = -1 bonds
+    o->e0 = (int)((2 * n_af) % 4);
+    return ORA_OK;
+}
+int ora_level_offset(const Oracle* o) { return o ? o->e0 : 0; }
+
+// stateless O15 pieces for the pins
+int ora_sweep_slots_j(int L, uint64_t seed, uint32_t t0, double beta, int theta, int64_t nslots, const int64_t* slot_ids,
+                      uint8_t* spins, int rng_mode, const int8_t* Jx, const int8_t* Jy) {
+    if (L < 4 || (L & 1) || theta < 0 || nslots < 0 || rng_mode < 0 || rng_mode > 1 || !Jx || !Jy) return ORA_ERR_INVALID_ARG;
+    uint32_t T4, T8; ora_thresholds(beta, &T4, &T8);
+    int N = L * L;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < nslots; ++i)
+        for (int it = 0; it < theta; ++it)
+            sweep_one_replica(spins + (size_t)i * N, L, seed, slot_ids[i], t0 + (uint32_t)it, T4, T8, rng_mode, Jx, Jy);
+    return ORA_OK;
+}
+int ora_energies_of_j(int L, int64_t n, const uint8_t* spins, const int8_t* Jx, const int8_t* Jy, int32_t* E, int32_t* M) {
+    if (L < 4 || (L & 1) || n < 0 || !Jx || !Jy) return ORA_ERR_INVALID_ARG;
+    int N = L * L;
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < n; ++j) {
+        int32_t e, m; energy_one_replica(spins + (size_t)j * N, L, &e, &m, Jx, Jy);
+        E[j] = e; if (M) M[j] = m;
+    }
+    return ORA_OK;
+}
 // 0 = one Philox number per spin (O1), 1 = Philox-seeded LCG per word (O11, L236-L241)
 int ora_set_rng_mode(Oracle* o, int mode) {
     if (!o || mode < 0 || mode > 1) return ORA_ERR_INVALID_ARG;
@@ -581,7 +639,8 @@ int ora_sweep(Oracle* o, double beta, int theta) {
 #pragma omp parallel for schedule(static)
     for (int64_t j = 0; j < o->R_cur; ++j)
         for (int it = 0; it < theta; ++it)
-            sweep_one_replica(&o->spin[(size_t)j * o->N], o->L, o->seed, j, o->t + (uint32_t)it, T4, T8, o->rng_mode);
+            sweep_one_replica(&o->spin[(size_t)j * o->N], o->L, o->seed, j, o->t + (uint32_t)it, T4, T8, o->rng_mode,
+                              o->Jx.empty() ? nullptr : o->Jx.data(), o->Jy.empty() ? nullptr : o->Jy.data());
     o->t += (uint32_t)theta;
     return ORA_OK;
 }
@@ -655,8 +714,8 @@ int ora_observables(Oracle* o, double beta, ora_obs_t* out) {
 int ora_hist_accumulate(Oracle* o, double beta) {
     if (!o) return ORA_ERR_INVALID_ARG;
     std::vector<int32_t> E, M; all_energies(o, E, M);
-    hist_fold_for(E, o->N, o->lnZ, beta, o->Hsum.data(), o->lnD.data());
-    mag_fold_for(E, M, o->N, o->A1sum.data(), o->A2sum.data());
+    hist_fold_for(E, o->N, o->lnZ, beta, o->Hsum.data(), o->lnD.data(), o->e0);
+    mag_fold_for(E, M, o->N, o->A1sum.data(), o->A2sum.data(), o->e0);
     return ORA_OK;
 }
 
@@ -667,8 +726,13 @@ int ora_get_mag_sums(const Oracle* o, int64_t* A1, int64_t* A2) {
     return ORA_OK;
 }
 int ora_reweight_mag(const Oracle* o, int n, const double* betas, double* absm, double* m2) {
-    if (!o) return ORA_ERR_INVALID_ARG;
-    return ora_reweight_mag_of(o->L, o->Hsum.data(), o->lnD.data(), o->A1sum.data(), o->A2sum.data(), n, betas, absm, m2);
+    if (!o || n < 0) return ORA_ERR_INVALID_ARG;
+    bool any = false;
+    for (int m = 0; m <= o->N; ++m) any = any || o->Hsum[m] > 0;
+    if (!any) return ORA_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i)
+        reweight_mag_for(o->N, o->Hsum.data(), o->lnD.data(), o->A1sum.data(), o->A2sum.data(), betas[i], &absm[i], &m2[i], o->e0);
+    return ORA_OK;
 }
 
 int ora_get_histogram(const Oracle* o, int64_t* Hsum, double* lnD) {
@@ -679,8 +743,12 @@ int ora_get_histogram(const Oracle* o, int64_t* Hsum, double* lnD) {
 }
 
 int ora_reweight(const Oracle* o, int n, const double* betas, double* lnZ, double* e, double* C) {
-    if (!o) return ORA_ERR_INVALID_ARG;
-    return ora_reweight_of(o->L, o->Hsum.data(), o->lnD.data(), n, betas, lnZ, e, C);
+    if (!o || n < 0) return ORA_ERR_INVALID_ARG;
+    bool any = false;
+    for (int m = 0; m <= o->N; ++m) any = any || o->Hsum[m] > 0;
+    if (!any) return ORA_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i) reweight_for(o->N, o->Hsum.data(), o->lnD.data(), betas[i], &lnZ[i], &e[i], &C[i], o->e0);
+    return ORA_OK;
 }
 
 // spins as +1/-1, [nrep][N], site = y*L + x

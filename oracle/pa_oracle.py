@@ -49,6 +49,10 @@ def lib():
         L.ora_mag_fold_of.argtypes = [i32, i64, vp, vp, vp, vp]; L.ora_mag_fold_of.restype = i32
         L.ora_get_mag_sums.argtypes = [vp, vp, vp]; L.ora_get_mag_sums.restype = i32
         L.ora_reweight_mag.argtypes = [vp, i32, vp, vp, vp]; L.ora_reweight_mag.restype = i32
+        L.ora_set_couplings.argtypes = [vp, vp, vp]; L.ora_set_couplings.restype = i32
+        L.ora_level_offset.argtypes = [vp]; L.ora_level_offset.restype = i32
+        L.ora_sweep_slots_j.argtypes = [i32, u64, u32, dbl, i32, i64, vp, vp, i32, vp, vp]; L.ora_sweep_slots_j.restype = i32
+        L.ora_energies_of_j.argtypes = [i32, i64, vp, vp, vp, vp, vp]; L.ora_energies_of_j.restype = i32
         L.ora_weighted_average.argtypes = [i32, vp, vp, i32, vp, vp]; L.ora_weighted_average.restype = i32
         L.ora_create.argtypes = [i32, i64, u64, vp]; L.ora_create.restype = i32
         L.ora_destroy.argtypes = [vp]; L.ora_destroy.restype = None
@@ -119,6 +123,25 @@ def sweep_slots(L, seed, t0, beta, theta, slot_ids, spins01, rng_mode=RNG_PHILOX
     _check(lib().ora_sweep_slots_mode(L, seed, t0, float(beta), theta, slot_ids.size, _p(slot_ids), _p(spins01),
                                       int(rng_mode)), "sweep_slots")
     return spins01
+
+
+def sweep_slots_j(L, seed, t0, beta, theta, slot_ids, spins01, Jx, Jy, rng_mode=RNG_PHILOX):
+    """O15: as sweep_slots, with bimodal couplings Jx, Jy (int8 [N], +-1)."""
+    slot_ids = np.ascontiguousarray(slot_ids, dtype=np.int64)
+    Jx = np.ascontiguousarray(Jx, dtype=np.int8); Jy = np.ascontiguousarray(Jy, dtype=np.int8)
+    assert spins01.dtype == np.uint8 and spins01.flags.c_contiguous and Jx.size == L * L == Jy.size
+    _check(lib().ora_sweep_slots_j(L, seed, t0, float(beta), theta, slot_ids.size, _p(slot_ids), _p(spins01), int(rng_mode),
+                                   _p(Jx), _p(Jy)), "sweep_slots_j")
+    return spins01
+
+
+def energies_of_j(L, spins01, Jx, Jy):
+    spins01 = np.ascontiguousarray(spins01, dtype=np.uint8)
+    Jx = np.ascontiguousarray(Jx, dtype=np.int8); Jy = np.ascontiguousarray(Jy, dtype=np.int8)
+    n = spins01.shape[0]
+    E = np.empty(n, dtype=np.int32); M = np.empty(n, dtype=np.int32)
+    _check(lib().ora_energies_of_j(L, n, _p(spins01), _p(Jx), _p(Jy), _p(E), _p(M)), "energies_of_j")
+    return E, M
 
 
 def lcg_next(r):
@@ -268,6 +291,19 @@ class Oracle:
         a = np.empty(betas.size); q = np.empty(betas.size)
         _check(lib().ora_reweight_mag(self._h, betas.size, _p(betas), _p(a), _p(q)), "reweight_mag")
         return {"absm": a, "m2": q}
+
+    def set_couplings(self, Jx, Jy):
+        """O15: bimodal couplings (int8 [N], +-1; Jx[s]: bond to the right of s, Jy[s]: bond below s); None, None = ferromagnet."""
+        if Jx is None:
+            _check(lib().ora_set_couplings(self._h, None, None), "set_couplings")
+            return
+        Jx = np.ascontiguousarray(Jx, dtype=np.int8); Jy = np.ascontiguousarray(Jy, dtype=np.int8)
+        assert Jx.size == self.N == Jy.size
+        _check(lib().ora_set_couplings(self._h, _p(Jx), _p(Jy)), "set_couplings")
+
+    @property
+    def level_offset(self):
+        return int(lib().ora_level_offset(self._h))
 
     def set_rng_mode(self, mode):
         _check(lib().ora_set_rng_mode(self._h, int(mode)), "set_rng_mode")
