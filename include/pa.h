@@ -92,6 +92,17 @@ enum { PA_RNG_PHILOX = 0, PA_RNG_LCG = 1 };
 int pa_set_rng_mode(pa_t* h, int mode);
 int pa_get_rng_mode(const pa_t* h);
 
+/* A second workload (L313: "the case of different couplings including spin glasses"; O15): bimodal couplings J = +-1 on
+ * the bonds, shared by all replicas of the population, H = -sum_<ab> J_ab s_a s_b.  Jx[s] couples site s = y*L+x to
+ * (x+1, y), Jy[s] couples it to (x, y+1) (periodic); int8[N] each, values +1 / -1, host or device.  Both NULL: back to
+ * the ferromagnet of Eq. 10 (the default).  The acceptance rule is unchanged with u = the number of UNSATISFIED bonds of
+ * the spin (dE = 8 - 4u); energies lie on -2N + 4m + e0 with e0 = pa_level_offset = 2 (number of J = -1 bonds) mod 4,
+ * which the histogram (Eq. 9) and reweighting calls use for E_m.  Must be called before the first pa_hist_accumulate
+ * (PA_ERR_INVALID_ARG afterwards, or if a value is not +-1).  Sweeps and energies then run on the general kernels
+ * (any even L).  Synchronous. */
+int pa_set_couplings(pa_t* h, const int8_t* Jx, const int8_t* Jy);
+int pa_level_offset(const pa_t* h);
+
 /* Configurational energies E_j = -sum_<ab> s_a s_b and magnetisations M_j = sum_a s_a of the
  * current replicas j = 0..R_cur-1 (Eq. 10; L173).  E_out, M_out: int32[>= R_cur], host or
  * device; M_out may be NULL.  Synchronises if an output is a host pointer. */

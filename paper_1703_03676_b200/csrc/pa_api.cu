@@ -20,7 +20,7 @@ void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const cha
 }
 
 struct PaLayout {
-    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, lnD, A1, A2, scal, slots, stage, total;
+    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, lnD, A1, A2, jmask, scal, slots, stage, total;
     size_t stage_bytes;
     int64_t R_cap, G_cap, tiles;
 };
@@ -50,6 +50,7 @@ static PaLayout pa_layout(int L, int64_t R) {
     y.lnD = take((N + 1) * 8);
     y.A1 = take((N + 1) * 8);
     y.A2 = take((N + 1) * 8);
+    y.jmask = take(N);
     y.scal = take(sizeof(PaScalars));
     y.slots = take((size_t)PA_SLOTS_CAP * 8);
     y.stage_bytes = (size_t)y.R_cap * N < PA_STAGE_BYTES ? pa_align_up((size_t)y.R_cap * N) : PA_STAGE_BYTES;
@@ -103,8 +104,8 @@ static int pa_ensure_host_scalars(pa_handle* h) {
     if (h->host_scal_valid) return PA_OK;
     if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
     h->host_scal_valid = true;
-    h->Emin = -2 * h->N + 4 * (int)(0xffffffffu - h->h_scal->mmin_inv);
-    h->Emax = -2 * h->N + 4 * (int)h->h_scal->mmax;
+    h->Emin = -2 * h->N + 4 * (int)(0xffffffffu - h->h_scal->mmin_inv) + h->e0;
+    h->Emax = -2 * h->N + 4 * (int)h->h_scal->mmax + h->e0;
     return PA_OK;
 }
 
@@ -162,6 +163,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     h->scan_state = (unsigned long long*)(b + y.scan);
     h->Hsum = (unsigned long long*)(b + y.Hsum); h->Hcur = (uint32_t*)(b + y.Hcur); h->lnD = (double*)(b + y.lnD);
     h->A1 = (unsigned long long*)(b + y.A1); h->A2 = (unsigned long long*)(b + y.A2);
+    h->jmask = (uint8_t*)(b + y.jmask); h->has_j = false; h->e0 = 0;
     h->d_scal = (PaScalars*)(b + y.scal);
     h->d_slots = (int64_t*)(b + y.slots);
     h->stage = (int8_t*)(b + y.stage); h->stage_bytes = y.stage_bytes;
@@ -221,6 +223,44 @@ int pa_set_rng_mode(pa_t* h, int mode) {
     return PA_OK;
 }
 int pa_get_rng_mode(const pa_t* h) { return h ? h->rng_mode : PA_ERR_INVALID_ARG; }
+
+// O15 (L313): bimodal couplings shared by all replicas.  Builds the per-word bond mask in the resident (colour-split) order.
+int pa_set_couplings(pa_t* h, const int8_t* Jx, const int8_t* Jy) {
+    if (!h || ((Jx == nullptr) != (Jy == nullptr)) || h->hist_any) return PA_ERR_INVALID_ARG;
+    h->em_valid = false; h->host_scal_valid = false;
+    if (!Jx) { h->has_j = false; h->e0 = 0; return PA_OK; }
+    const int L = h->L, N = h->N, Lh = L / 2;
+    int8_t* hx = (int8_t*)malloc((size_t)N * 2);
+    uint8_t* jm = (uint8_t*)malloc((size_t)N);
+    if (!hx || !jm) { free(hx); free(jm); return PA_ERR_NOMEM; }
+    int8_t* hy = hx + N;
+    cudaError_t err = cudaMemcpy(hx, Jx, (size_t)N, cudaMemcpyDefault);
+    if (err == cudaSuccess) err = cudaMemcpy(hy, Jy, (size_t)N, cudaMemcpyDefault);
+    if (err != cudaSuccess) { free(hx); free(jm); pa_note_cuda_error(h, err, "cudaMemcpy(couplings)", __FILE__, __LINE__); return PA_ERR_CUDA; }
+    long long n_af = 0;
+    for (int s = 0; s < N; ++s) {
+        if ((hx[s] != 1 && hx[s] != -1) || (hy[s] != 1 && hy[s] != -1)) { free(hx); free(jm); return PA_ERR_INVALID_ARG; }
+        n_af += (hx[s] < 0) + (hy[s] < 0);
+    }
+    for (int c = 0; c < 2; ++c)
+        for (int y = 0; y < L; ++y)
+            for (int xh = 0; xh < Lh; ++xh) {
+                const int p = (y + c) & 1, x = 2 * xh + p;
+                const int xl = x == 0 ? L - 1 : x - 1, yu = y == 0 ? L - 1 : y - 1;
+                const bool right = hx[y * L + x] < 0, left = hx[y * L + xl] < 0, down = hy[y * L + x] < 0, up = hy[yu * L + x] < 0;
+                // neighbour "same cell" of the other colour is x+1 for p = 0 and x-1 for p = 1; the "x" neighbour is the other one
+                const bool same = p ? left : right, other = p ? right : left;
+                jm[c * (N / 2) + y * Lh + xh] = (uint8_t)((same ? 1 : 0) | (other ? 2 : 0) | (up ? 4 : 0) | (down ? 8 : 0) | (right ? 16 : 0));
+            }
+    err = cudaMemcpyAsync(h->jmask, jm, (size_t)N, cudaMemcpyHostToDevice, h->stream);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(h->stream);
+    free(hx); free(jm);
+    if (err != cudaSuccess) { pa_note_cuda_error(h, err, "upload couplings", __FILE__, __LINE__); return PA_ERR_CUDA; }
+    h->has_j = true;
+    h->e0 = (int)((2 * n_af) % 4);
+    return PA_OK;
+}
+int pa_level_offset(const pa_t* h) { return h ? h->e0 : 0; }
 
 int pa_energies(pa_t* h, int32_t* E_out, int32_t* M_out) {
     if (!h || !E_out) return PA_ERR_INVALID_ARG;

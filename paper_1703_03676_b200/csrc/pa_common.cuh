@@ -84,6 +84,9 @@ struct pa_handle {
     uint64_t seed;
     uint32_t t, k;
     int rng_mode;            // PA_RNG_PHILOX / PA_RNG_LCG (O11)
+    bool has_j;              // O15: bimodal couplings set
+    int e0;                  // O15: every energy is -2N + 4m + e0, e0 = 2 (number of J = -1 bonds) mod 4
+    uint8_t* jmask;          // [N] resident order: bits 0-3 = bond to (same-cell, x, up, down) neighbour has J = -1; bit 4 = right bond
     double lnZ, lnQ_last;
     PhiloxKeys keys;
 

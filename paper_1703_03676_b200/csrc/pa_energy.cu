@@ -159,7 +159,7 @@ __device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&
 __global__ void __launch_bounds__(256)
 pa_measure_generic_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R_cur,
                   int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
-                  double* __restrict__ runsum, double* __restrict__ blocksum) {
+                  double* __restrict__ runsum, double* __restrict__ blocksum, const uint8_t* __restrict__ jmask) {
     const long long g = blockIdx.x;
     const uint32_t* base = pop + g * (long long)N;
     const int Lh = L >> 1, half = N >> 1;
@@ -184,6 +184,11 @@ pa_measure_generic_kernel(const uint32_t* __restrict__ pop, int L, int N, long l
                 int yd = (y + 1 == L) ? 0 : y + 1;
                 a = s ^ oth[y * Lh + xr];
                 b = s ^ oth[yd * Lh + xh];
+                if (jmask) {                     // O15: a J = -1 bond is unsatisfied when its ends are parallel
+                    const uint32_t j = jmask[idx];
+                    a ^= 0u - ((j >> 4) & 1u);   // right bond
+                    b ^= 0u - ((j >> 3) & 1u);   // down bond
+                }
             }
             xs[q] = s; xa[q] = a; xb[q] = b;
         }
@@ -303,7 +308,7 @@ int pa_launch_measure(pa_handle* h) {
     const int L = h->L;
     PA_CUDA(h, cudaMemsetAsync(h->d_scal, 0, offsetof(PaScalars, R_new), h->stream));
     PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
-    const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
+    const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr && !h->has_j;
     if (pow2) {
 #define PA_MSR_CASE(LOG) case (8 << LOG): pa_measure_kernel<LOG><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
             h->spins[h->cur], h->N, h->R_cur, h->E, h->M, h->d_scal, h->runsum, h->partials); break;
@@ -313,7 +318,7 @@ int pa_launch_measure(pa_handle* h) {
         int T = 256;
         while (T > 32 && T * 8 > h->N) T >>= 1;
         pa_measure_generic_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, h->E, h->M, h->d_scal,
-                                                                    h->runsum, h->partials);
+                                                                    h->runsum, h->partials, h->has_j ? h->jmask : nullptr);
     }
     PA_CUDA(h, cudaGetLastError());
     PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));

@@ -55,12 +55,12 @@ __global__ void pa_hist_kernel(const int32_t* __restrict__ E, const int32_t* __r
     }
 }
 __global__ void pa_hist_fold_kernel(uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ Hsum,
-                                    double* __restrict__ lnD, int N, double lnR_minus_lnZ, double beta) {
+                                    double* __restrict__ lnD, int N, double lnR_minus_lnZ, double beta, int e0) {
     const int m = blockIdx.x * blockDim.x + threadIdx.x;
     if (m > N) return;
     Hsum[m] += Hcur[m];
     Hcur[m] = 0;
-    const double Em = (double)(-2 * N + 4 * m);
+    const double Em = (double)(-2 * N + 4 * m + e0);
     const double term = lnR_minus_lnZ - beta * Em;
     const double a = lnD[m];
     double out;
@@ -74,7 +74,7 @@ int pa_launch_hist(pa_handle* h, double beta) {
     if (blocks > 1184) blocks = 1184;
     pa_hist_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->M, h->R_cur, h->N, h->Hcur, h->A1, h->A2);
     const double c = log((double)h->R_cur) - h->lnZ;
-    pa_hist_fold_kernel<<<(h->N + 1 + 255) / 256, 256, 0, h->stream>>>(h->Hcur, h->Hsum, h->lnD, h->N, c, beta);
+    pa_hist_fold_kernel<<<(h->N + 1 + 255) / 256, 256, 0, h->stream>>>(h->Hcur, h->Hsum, h->lnD, h->N, c, beta, h->e0);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 2;
     return PA_OK;
@@ -111,7 +111,7 @@ __device__ __forceinline__ double pa_block_reduce(double v, double* sh) {
 
 __global__ void __launch_bounds__(256)
 pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __restrict__ lnD,
-                   const unsigned long long* __restrict__ A1, const unsigned long long* __restrict__ A2, int N,
+                   const unsigned long long* __restrict__ A1, const unsigned long long* __restrict__ A2, int N, int e0,
                    const double* __restrict__ betas, double* __restrict__ lnZ, double* __restrict__ e, double* __restrict__ C,
                    double* __restrict__ absm, double* __restrict__ m2) {
     __shared__ double sh[33];
@@ -120,14 +120,14 @@ pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __
     for (int m = threadIdx.x; m <= N; m += blockDim.x) {
         const unsigned long long H = Hsum[m];
         if (H == 0ull) continue;
-        amax = fmax(amax, (log((double)H) - lnD[m]) - beta * (double)(-2 * N + 4 * m));
+        amax = fmax(amax, (log((double)H) - lnD[m]) - beta * (double)(-2 * N + 4 * m + e0));
     }
     amax = pa_block_reduce<true>(amax, sh);
     double s0 = 0.0, s1 = 0.0, sa = 0.0, sq = 0.0;
     for (int m = threadIdx.x; m <= N; m += blockDim.x) {
         const unsigned long long H = Hsum[m];
         if (H == 0ull) continue;
-        const double Em = (double)(-2 * N + 4 * m);
+        const double Em = (double)(-2 * N + 4 * m + e0);
         const double p = exp(((log((double)H) - lnD[m]) - beta * Em) - amax);
         s0 += p; s1 += Em * p;
         sa += p * ((double)A1[m] / (double)H);           // O14: microcanonical mean of |M| at level m
@@ -142,7 +142,7 @@ pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __
     for (int m = threadIdx.x; m <= N; m += blockDim.x) {
         const unsigned long long H = Hsum[m];
         if (H == 0ull) continue;
-        const double Em = (double)(-2 * N + 4 * m);
+        const double Em = (double)(-2 * N + 4 * m + e0);
         const double p = exp(((log((double)H) - lnD[m]) - beta * Em) - amax);
         s2 += (Em - mean) * (Em - mean) * p;
     }
@@ -159,7 +159,7 @@ pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __
 // d_io: [betas(n) | lnZ(n) | e(n) | C(n) | absm(n) | m2(n)] in device memory
 int pa_launch_reweight(pa_handle* h, int n, double* d_io) {
     const size_t z = (size_t)n;
-    pa_reweight_kernel<<<n, 256, 0, h->stream>>>(h->Hsum, h->lnD, h->A1, h->A2, h->N, d_io, d_io + z, d_io + 2 * z, d_io + 3 * z,
+    pa_reweight_kernel<<<n, 256, 0, h->stream>>>(h->Hsum, h->lnD, h->A1, h->A2, h->N, h->e0, d_io, d_io + z, d_io + 2 * z, d_io + 3 * z,
                                                  d_io + 4 * z, d_io + 5 * z);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;

@@ -23,6 +23,7 @@ struct SweepParams {
     uint32_t two;                    // the constant 2, opaque to ptxas (see pa_shift_in_ge)
     int theta;
     int L, Lh, H, C, N;
+    const uint8_t* jmask;            // O15: per resident word, bit k = bond to neighbour k (same, x, up, down) has J = -1; NULL = ferromagnet
 };
 
 // m = 2*m + (x >= T).  "sub.cc" leaves the hardware carry of x + ~T + 1 in CC.CF, i.e. NOT borrow, and
@@ -179,7 +180,7 @@ __device__ __forceinline__ uint4 pa_lcg_seeds(uint32_t quad, uint32_t g, uint32_
     return pa_philox(quad, g, c2, PA_TAG_LCG, K);
 }
 
-template <int CMP, bool CLUSTER, int RNG>
+template <int CMP, bool CLUSTER, int RNG, bool HASJ>
 __global__ void __launch_bounds__(256)
 pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
@@ -242,14 +243,20 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                 uint32_t nU, nD;
                 if (yl > 0) nU = oth[row - Lh + xh]; else nU = up_oth[(H - 1) * Lh + xh];
                 if (yl < H - 1) nD = oth[row + Lh + xh]; else nD = dn_oth[xh];
+                uint32_t nS_ = nS, nX_ = nX;
+                if (HASJ) {
+                    // O15: a bond with J = -1 is unsatisfied when the spins are parallel: complement that neighbour's word
+                    const uint32_t j = P.jmask[c * gcol + y * Lh + xh];
+                    nS_ ^= 0u - (j & 1u); nX_ ^= 0u - ((j >> 1) & 1u); nU ^= 0u - ((j >> 2) & 1u); nD ^= 0u - ((j >> 3) & 1u);
+                }
                 uint32_t flip;
                 if (RNG == PA_RNG_LCG) {
                     const uint4 sd = pa_lcg_seeds((uint32_t)((y >> 2) * Lh + xh), (uint32_t)g, c2, P.K);
                     const int q = y & 3;
-                    flip = pa_flip_mask_lcg<0>(s, nS, nX, nU, nD, q == 0 ? sd.x : q == 1 ? sd.y : q == 2 ? sd.z : sd.w, P);
+                    flip = pa_flip_mask_lcg<0>(s, nS_, nX_, nU, nD, q == 0 ? sd.x : q == 1 ? sd.y : q == 2 ? sd.z : sd.w, P);
                 } else {
                     const uint32_t site = (uint32_t)(y * L + 2 * xh + p);
-                    flip = pa_flip_mask<CMP>(s, nS, nX, nU, nD, site, c0base, lo1u, P);
+                    flip = pa_flip_mask<CMP>(s, nS_, nX_, nU, nD, site, c0base, lo1u, P);
                 }
                 mine[row + xh] = s ^ flip;
                 xh += dx; yl += dy;
@@ -557,8 +564,8 @@ static cudaError_t pa_sweep_dispatch_lcg(pa_handle* h, const SweepParams& P, siz
             default: return pa_sweep_dispatch_lcg_col<4>(h, P, smem, grid);
         }
     }
-    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_LCG>, P, smem, grid, true)
-              : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_LCG>, P, smem, grid, false);
+    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_LCG, false>, P, smem, grid, true)
+              : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_LCG, false>, P, smem, grid, false);
 }
 
 template <int CMP>
@@ -573,8 +580,8 @@ static cudaError_t pa_sweep_dispatch(pa_handle* h, const SweepParams& P, size_t 
             default: break;
         }
     }
-    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<CMP, true, PA_RNG_PHILOX>, P, smem, grid, true)
-              : pa_sweep_launch_k(h, pa_sweep_kernel<CMP, false, PA_RNG_PHILOX>, P, smem, grid, false);
+    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<CMP, true, PA_RNG_PHILOX, false>, P, smem, grid, true)
+              : pa_sweep_launch_k(h, pa_sweep_kernel<CMP, false, PA_RNG_PHILOX, false>, P, smem, grid, false);
 }
 
 int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
@@ -588,7 +595,15 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     const size_t smem = (size_t)P.H * h->L * 4;
     const unsigned grid = (unsigned)(G * P.C);
     const int v = h->sweep_cmp;
-    const cudaError_t e = h->rng_mode == PA_RNG_LCG ? pa_sweep_dispatch_lcg(h, P, smem, grid)
+    P.jmask = h->has_j ? h->jmask : nullptr;
+    const bool cl = P.C > 1;
+    const cudaError_t e = h->has_j       // O15: couplings run on the generic kernel (any even L, both streams)
+                        ? (h->rng_mode == PA_RNG_LCG
+                               ? (cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_LCG, true>, P, smem, grid, true)
+                                     : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_LCG, true>, P, smem, grid, false))
+                               : (cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_PHILOX, true>, P, smem, grid, true)
+                                     : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_PHILOX, true>, P, smem, grid, false)))
+                        : h->rng_mode == PA_RNG_LCG ? pa_sweep_dispatch_lcg(h, P, smem, grid)
                         : v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)
                                                                                     : pa_sweep_dispatch<0>(h, P, smem, grid);
     PA_CUDA(h, e);

@@ -67,6 +67,8 @@ def lib():
         "pa_destroy": ([vp], None),
         "pa_sweep": ([vp, dbl, i32], i32),
         "pa_set_rng_mode": ([vp, i32], i32),
+        "pa_set_couplings": ([vp, vp, vp], i32),
+        "pa_level_offset": ([vp], i32),
         "pa_get_rng_mode": ([vp], i32),
         "pa_energies": ([vp, vp, vp], i32),
         "pa_resample": ([vp, dbl, dbl, C.POINTER(i64)], i32),
@@ -239,6 +241,19 @@ class Population:
         self._check(lib().pa_set_counters(self._h, t, k, float(lnZ)), "pa_set_counters")
 
     # the path
+    def set_couplings(self, Jx, Jy):
+        """Bimodal couplings (int8 [N], +-1; Jx[s]: bond to the right of s = y*L+x, Jy[s]: bond below); None, None = ferromagnet."""
+        if Jx is None:
+            self._check(lib().pa_set_couplings(self._h, None, None), "pa_set_couplings")
+            return
+        Jx = np.ascontiguousarray(Jx, dtype=np.int8); Jy = np.ascontiguousarray(Jy, dtype=np.int8)
+        assert Jx.size == self.N == Jy.size
+        self._check(lib().pa_set_couplings(self._h, _ptr(Jx), _ptr(Jy)), "pa_set_couplings")
+
+    @property
+    def level_offset(self):
+        return int(lib().pa_level_offset(self._h))
+
     def set_rng_mode(self, mode):
         self._check(lib().pa_set_rng_mode(self._h, int(mode)), "pa_set_rng_mode")
 
