@@ -236,6 +236,9 @@ def run_ours(args):
     pop = pa.Population(wl.L, wl.R, rank_seed(wl, rank))
     if args.rng == "lcg":
         pop.set_rng_mode(pa.PA_RNG_LCG)
+    if args.couplings == "pmj":
+        from paper_1703_03676_b200.workloads import random_couplings
+        pop.set_couplings(*random_couplings(wl.L, wl.seed))
     betas = wl.betas() if wl.n_steps is not None else None
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
     peaks, peak_src = measured_peaks()
@@ -347,15 +350,15 @@ def run_ours(args):
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "u32", "data": "synthetic",
-           "config": {"workload": wl.name, "L": wl.L, "R_per_gpu": wl.R, "theta": wl.theta, "beta_from": wl.beta0, "rng": args.rng,
+           "config": {"workload": wl.name, "L": wl.L, "R_per_gpu": wl.R, "theta": wl.theta, "beta_from": wl.beta0, "rng": args.rng, "couplings": args.couplings,
                       "schedule": "adaptive" if wl.n_steps is None else f"{wl.n_steps} equal steps to {wl.beta_f}",
                       "l2": "flushed between timed steps (256 MiB memset outside the CUDA events)",
                       "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "resample": resample,
            "last_observables": obs, "combined_observables": combined}
-    if world == 1 and (args.whole_run or (args.whole_run is None and args.config <= 4)):
+    if world == 1 and args.couplings == "ferro" and (args.whole_run or (args.whole_run is None and args.config <= 4)):
         out["whole_run"] = whole_run(pa, wl, rank_seed(wl, rank), args.rng)
-    out["cpu_baseline"] = cpu_baseline(wl, args.rng) if world == 1 and not args.no_cpu else None
+    out["cpu_baseline"] = cpu_baseline(wl, args.rng) if world == 1 and not args.no_cpu and args.couplings == "ferro" else None
     print(json.dumps(out), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -415,6 +418,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--whole-run", dest="whole_run", action="store_true", default=None,
                     help="also time the config's whole schedule (t_SF, Eq. 11); default: on for configs 1-4 (seconds), off for 5 (minutes)")
+    ap.add_argument("--couplings", default="ferro", choices=["ferro", "pmj"],
+                    help="ferromagnet (default, Eq. 10) or a seeded random +-J sample (second workload, PAPER.md L313; context)")
     ap.add_argument("--theta-scan", action="store_true", help="re-measure the paper's Table 3 / Table 4 theta dependence (context)")
     ap.add_argument("--no-whole-run", dest="whole_run", action="store_false")
     ap.add_argument("--rng", default="philox", choices=["philox", "lcg"],

@@ -180,6 +180,9 @@ __device__ __forceinline__ uint4 pa_lcg_seeds(uint32_t quad, uint32_t g, uint32_
     return pa_philox(quad, g, c2, PA_TAG_LCG, K);
 }
 
+// O15: neighbour word as the acceptance logic must see it: complemented if bond k of this site has J = -1
+__device__ __forceinline__ uint32_t pa_jx(uint32_t n, uint32_t j, int k) { return n ^ (0u - ((j >> k) & 1u)); }
+
 template <int CMP, bool CLUSTER, int RNG, bool HASJ>
 __global__ void __launch_bounds__(256)
 pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
@@ -291,7 +294,7 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 #ifndef PA_SWEEP_BOUNDS
 #define PA_SWEEP_BOUNDS __launch_bounds__(256)
 #endif
-template <int CMP, int LOG_LH, bool CLUSTER>
+template <int CMP, int LOG_LH, bool CLUSTER, bool HASJ>
 __global__ void PA_SWEEP_BOUNDS
 pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
@@ -342,6 +345,7 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
             // rows y0+ya+2k have x-parity p = c (x = 2 xh + c), rows y0+ya+2k+1 have p = 1 - c
             const int dA = c ? dR : dL, dB = c ? dL : dR;
             uint32_t site = site_base + (uint32_t)c;
+            const uint8_t* jm = HASJ ? P.jmask + c * gcol + goff + b0 : nullptr;     // bond masks of this thread's column (O15)
 #pragma unroll 1
             for (int k = 0; k < rpt; k += 2) {
                 const uint32_t s0 = mine[0], s1 = mine[Lh];
@@ -350,8 +354,17 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                 uint32_t nU0, nD1;
                 if (ya + k > 0) nU0 = oth[-Lh]; else nU0 = up_tile[(1 - c) * half + (H - 1) * Lh + xh];
                 if (ya + k + 2 < H) nD1 = oth[2 * Lh]; else nD1 = dn_tile[(1 - c) * half + xh];
-                const uint32_t f0 = pa_flip_mask<CMP>(s0, nS0, nX0, nU0, nS1, site, c0base, lo1u, P);
-                const uint32_t f1 = pa_flip_mask<CMP>(s1, nS1, nX1, nS0, nD1, site + (uint32_t)(2 * Lh + 1 - 2 * c), c0base, lo1u, P);
+                uint32_t f0, f1;
+                if (HASJ) {
+                    const uint32_t j0 = jm[0], j1 = jm[Lh];
+                    f0 = pa_flip_mask<CMP>(s0, pa_jx(nS0, j0, 0), pa_jx(nX0, j0, 1), pa_jx(nU0, j0, 2), pa_jx(nS1, j0, 3), site, c0base, lo1u, P);
+                    f1 = pa_flip_mask<CMP>(s1, pa_jx(nS1, j1, 0), pa_jx(nX1, j1, 1), pa_jx(nS0, j1, 2), pa_jx(nD1, j1, 3),
+                                           site + (uint32_t)(2 * Lh + 1 - 2 * c), c0base, lo1u, P);
+                    jm += 2 * Lh;
+                } else {
+                    f0 = pa_flip_mask<CMP>(s0, nS0, nX0, nU0, nS1, site, c0base, lo1u, P);
+                    f1 = pa_flip_mask<CMP>(s1, nS1, nX1, nS0, nD1, site + (uint32_t)(2 * Lh + 1 - 2 * c), c0base, lo1u, P);
+                }
                 mine[0] = s0 ^ f0;
                 mine[Lh] = s1 ^ f1;
                 mine += 2 * Lh; oth += 2 * Lh; site += 4u * Lh;
@@ -373,7 +386,7 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 // vertical-neighbour words of the quad are loaded once.  Requirements (pa_col_ok): as above and rows per thread
 // a multiple of 4, strip height a multiple of 4.
 // ------------------------------------------------------------------------------------------------
-template <int LOG_LH, bool CLUSTER, int NOR>
+template <int LOG_LH, bool CLUSTER, int NOR, bool HASJ>
 __global__ void PA_SWEEP_BOUNDS
 pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh]
@@ -420,6 +433,7 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
             // rows y0+ya+2k have x-parity p = c (x = 2 xh + c), rows y0+ya+2k+1 have p = 1 - c
             const int dA = c ? dR : dL, dB = c ? dL : dR;
             uint32_t quad = quad_base;
+            const uint8_t* jm = HASJ ? P.jmask + c * gcol + goff + b0 : nullptr;     // bond masks of this thread's column (O15)
 #pragma unroll 1
             for (int k = 0; k < rpt; k += 4) {
                 const uint4 sd = pa_lcg_seeds(quad, (uint32_t)g, c2, P.K);
@@ -429,10 +443,20 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                 uint32_t oU, oD;
                 if (ya + k > 0) oU = oth[-Lh]; else oU = up_tile[(1 - c) * half + (H - 1) * Lh + xh];
                 if (ya + k + 4 < H) oD = oth[4 * Lh]; else oD = dn_tile[(1 - c) * half + xh];
-                const uint32_t f0 = pa_flip_mask_lcg<NOR>(s0, o0, x0, oU, o1, sd.x, P);
-                const uint32_t f1 = pa_flip_mask_lcg<NOR>(s1, o1, x1, o0, o2, sd.y, P);
-                const uint32_t f2 = pa_flip_mask_lcg<NOR>(s2, o2, x2, o1, o3, sd.z, P);
-                const uint32_t f3 = pa_flip_mask_lcg<NOR>(s3, o3, x3, o2, oD, sd.w, P);
+                uint32_t f0, f1, f2, f3;
+                if (HASJ) {
+                    const uint32_t j0 = jm[0], j1 = jm[Lh], j2 = jm[2 * Lh], j3 = jm[3 * Lh];
+                    f0 = pa_flip_mask_lcg<NOR>(s0, pa_jx(o0, j0, 0), pa_jx(x0, j0, 1), pa_jx(oU, j0, 2), pa_jx(o1, j0, 3), sd.x, P);
+                    f1 = pa_flip_mask_lcg<NOR>(s1, pa_jx(o1, j1, 0), pa_jx(x1, j1, 1), pa_jx(o0, j1, 2), pa_jx(o2, j1, 3), sd.y, P);
+                    f2 = pa_flip_mask_lcg<NOR>(s2, pa_jx(o2, j2, 0), pa_jx(x2, j2, 1), pa_jx(o1, j2, 2), pa_jx(o3, j2, 3), sd.z, P);
+                    f3 = pa_flip_mask_lcg<NOR>(s3, pa_jx(o3, j3, 0), pa_jx(x3, j3, 1), pa_jx(o2, j3, 2), pa_jx(oD, j3, 3), sd.w, P);
+                    jm += 4 * Lh;
+                } else {
+                    f0 = pa_flip_mask_lcg<NOR>(s0, o0, x0, oU, o1, sd.x, P);
+                    f1 = pa_flip_mask_lcg<NOR>(s1, o1, x1, o0, o2, sd.y, P);
+                    f2 = pa_flip_mask_lcg<NOR>(s2, o2, x2, o1, o3, sd.z, P);
+                    f3 = pa_flip_mask_lcg<NOR>(s3, o3, x3, o2, oD, sd.w, P);
+                }
                 mine[0] = s0 ^ f0;
                 mine[Lh] = s1 ^ f1;
                 mine[2 * Lh] = s2 ^ f2;
@@ -541,12 +565,12 @@ static cudaError_t pa_sweep_launch_k(pa_handle* h, Kern kern, const SweepParams&
     return cudaLaunchKernelEx(&cfg, kern, h->spins[h->cur], P);
 }
 
-template <int NOR>
+template <int NOR, bool HASJ>
 static cudaError_t pa_sweep_dispatch_lcg_col(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
     const bool cl = P.C > 1;
     switch (P.Lh) {
-#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, true, NOR>, P, smem, grid, true) \
-                                                  : pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, false, NOR>, P, smem, grid, false);
+#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, true, NOR, HASJ>, P, smem, grid, true) \
+                                                  : pa_sweep_launch_k(h, pa_sweep_lcg_kernel<LOG, false, NOR, HASJ>, P, smem, grid, false);
         PA_COL_CASE(5) PA_COL_CASE(6) PA_COL_CASE(7) PA_COL_CASE(8)
 #undef PA_COL_CASE
         default: return cudaErrorInvalidValue;
@@ -556,14 +580,18 @@ static cudaError_t pa_sweep_dispatch_lcg_col(pa_handle* h, const SweepParams& P,
 static cudaError_t pa_sweep_dispatch_lcg(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
     const bool cl = P.C > 1;
     if (h->sweep_kind == 1 && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG) && P.Lh >= 32 && P.Lh <= 256) {
+        if (h->has_j) return pa_sweep_dispatch_lcg_col<4, true>(h, P, smem, grid);
         switch (pa_env_int("PA_LCG_NOR", 4)) {       // tuning knob; every value gives the same bytes
-            case 0: return pa_sweep_dispatch_lcg_col<0>(h, P, smem, grid);
-            case 2: return pa_sweep_dispatch_lcg_col<2>(h, P, smem, grid);
-            case 6: return pa_sweep_dispatch_lcg_col<6>(h, P, smem, grid);
-            case 8: return pa_sweep_dispatch_lcg_col<8>(h, P, smem, grid);
-            default: return pa_sweep_dispatch_lcg_col<4>(h, P, smem, grid);
+            case 0: return pa_sweep_dispatch_lcg_col<0, false>(h, P, smem, grid);
+            case 2: return pa_sweep_dispatch_lcg_col<2, false>(h, P, smem, grid);
+            case 6: return pa_sweep_dispatch_lcg_col<6, false>(h, P, smem, grid);
+            case 8: return pa_sweep_dispatch_lcg_col<8, false>(h, P, smem, grid);
+            default: return pa_sweep_dispatch_lcg_col<4, false>(h, P, smem, grid);
         }
     }
+    if (h->has_j)
+        return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_LCG, true>, P, smem, grid, true)
+                  : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_LCG, true>, P, smem, grid, false);
     return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_LCG, false>, P, smem, grid, true)
               : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_LCG, false>, P, smem, grid, false);
 }
@@ -573,8 +601,8 @@ static cudaError_t pa_sweep_dispatch(pa_handle* h, const SweepParams& P, size_t 
     const bool cl = P.C > 1;
     if (h->sweep_kind == 1) {
         switch (P.Lh) {
-#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_col_kernel<CMP, LOG, true>, P, smem, grid, true) \
-                                                      : pa_sweep_launch_k(h, pa_sweep_col_kernel<CMP, LOG, false>, P, smem, grid, false);
+#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_col_kernel<CMP, LOG, true, false>, P, smem, grid, true) \
+                                                      : pa_sweep_launch_k(h, pa_sweep_col_kernel<CMP, LOG, false, false>, P, smem, grid, false);
             PA_COL_CASE(5) PA_COL_CASE(6) PA_COL_CASE(7) PA_COL_CASE(8)
 #undef PA_COL_CASE
             default: break;
@@ -582,6 +610,22 @@ static cudaError_t pa_sweep_dispatch(pa_handle* h, const SweepParams& P, size_t 
     }
     return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<CMP, true, PA_RNG_PHILOX, false>, P, smem, grid, true)
               : pa_sweep_launch_k(h, pa_sweep_kernel<CMP, false, PA_RNG_PHILOX, false>, P, smem, grid, false);
+}
+
+// O15 with one Philox number per spin: column-walk kernel where it applies, else the generic kernel
+static cudaError_t pa_sweep_dispatch_j(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
+    const bool cl = P.C > 1;
+    if (h->sweep_kind == 1) {
+        switch (P.Lh) {
+#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_col_kernel<1, LOG, true, true>, P, smem, grid, true) \
+                                                      : pa_sweep_launch_k(h, pa_sweep_col_kernel<1, LOG, false, true>, P, smem, grid, false);
+            PA_COL_CASE(5) PA_COL_CASE(6) PA_COL_CASE(7) PA_COL_CASE(8)
+#undef PA_COL_CASE
+            default: break;
+        }
+    }
+    return cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_PHILOX, true>, P, smem, grid, true)
+              : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_PHILOX, true>, P, smem, grid, false);
 }
 
 int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
@@ -596,13 +640,7 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     const unsigned grid = (unsigned)(G * P.C);
     const int v = h->sweep_cmp;
     P.jmask = h->has_j ? h->jmask : nullptr;
-    const bool cl = P.C > 1;
-    const cudaError_t e = h->has_j       // O15: couplings run on the generic kernel (any even L, both streams)
-                        ? (h->rng_mode == PA_RNG_LCG
-                               ? (cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_LCG, true>, P, smem, grid, true)
-                                     : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_LCG, true>, P, smem, grid, false))
-                               : (cl ? pa_sweep_launch_k(h, pa_sweep_kernel<1, true, PA_RNG_PHILOX, true>, P, smem, grid, true)
-                                     : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_PHILOX, true>, P, smem, grid, false)))
+    const cudaError_t e = (h->has_j && h->rng_mode != PA_RNG_LCG) ? pa_sweep_dispatch_j(h, P, smem, grid)   // O15, Philox per spin
                         : h->rng_mode == PA_RNG_LCG ? pa_sweep_dispatch_lcg(h, P, smem, grid)
                         : v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)
                                                                                     : pa_sweep_dispatch<0>(h, P, smem, grid);

@@ -57,3 +57,13 @@ def table3_workload(theta: int, R: int = 50000) -> Workload:
     (L189: dbeta = 0.02, i.e. 50 equal steps from 0 to 1) is used -- t_SF is normalised per spin flip, so the number of
     temperatures only sets how often the resampling cost is paid per theta sweeps, which is once in either case."""
     return Workload(f"table3_L128_R{R}_theta{theta}", 128, R, 7, 0.0, 1.0, 50, theta)
+
+
+def random_couplings(L: int, seed: int):
+    """A seeded bimodal sample for the second workload (O15): independent J = +-1 with probability 1/2 on
+    every bond of the L x L torus (the 2D Edwards-Anderson +-J spin glass).  Returns (Jx, Jy), int8 [L*L] each, site = y*L + x."""
+    import numpy as np
+    rng = np.random.default_rng(seed)
+    Jx = (rng.integers(0, 2, L * L) * 2 - 1).astype(np.int8)
+    Jy = (rng.integers(0, 2, L * L) * 2 - 1).astype(np.int8)
+    return Jx, Jy

@@ -32,9 +32,11 @@ def _same(g, o):
     assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
 
 
-@pytest.mark.parametrize("L,R,mode", [(4, 40, 0), (6, 70, 0), (16, 200, 1), (32, 100, 0), (64, 96, 1), (128, 40, 0), (256, 33, 1), (192, 33, 0)])
+@pytest.mark.parametrize("L,R,mode", [(4, 40, 0), (6, 70, 0), (16, 200, 1), (32, 100, 0), (64, 96, 1), (128, 40, 0), (256, 33, 1), (192, 33, 0),
+                                      (64, 96, 0), (128, 40, 1), (256, 33, 0), (192, 33, 1)])
 def test_sweep_and_energies_with_couplings_bit_exact(L, R, mode):
-    """Generic kernel on one CTA (L <= 128) and on clusters with DSMEM halos (L = 192, 256), both sweep streams, ragged last group."""
+    """Generic kernel (L < 64, L = 192 on clusters) and both column-walk kernels (L = 64, 128 on one CTA, L = 256 on clusters with DSMEM
+    halos), both sweep streams, ragged last group."""
     Jx, Jy = _random_j(L, 100 + L)
     g, o = pa.Population(L, R, 31 + L), po.Oracle(L, R, 31 + L)
     g.set_couplings(Jx, Jy); o.set_couplings(Jx, Jy)
