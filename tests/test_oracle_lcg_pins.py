@@ -122,14 +122,14 @@ def test_lcg_pa_run_matches_exact_enumeration_L4():
             assert abs(vals.mean() - exact[key]) < 5 * sigma + 1e-12, (betas[i], key, vals.mean(), exact[key], sigma)
 
 
-def test_lcg_pa_run_matches_kaufman_and_variance_ratio_L16():
+def test_lcg_pa_run_matches_kaufman_and_variance_ratio_L16(cfg1_oracle_runs):
     # configs[0] of BASELINE.json (L=16, R=1000, 100 steps, theta=10) with the LCG-assisted stream: exact finite-L
     # results (Kaufman) within the seed scatter, and Table 1's last column (L201-L204): the variance of C is the
-    # same as with one Philox number per spin (ratio 1; here 12 + 12 seeds, F-distribution bounds at ~4 sigma)
+    # same as with one Philox number per spin (ratio 1; here 10 + 8 seeds, the Philox runs are the session's shared ones)
     L, R, theta = 16, 1000, 10
-    betas = [i / 100 for i in range(101)]
-    lcg = _runs(L, R, betas, theta, list(range(21, 33)), LCG)
-    phi = _runs(L, R, betas, theta, list(range(41, 53)), po.RNG_PHILOX)
+    betas, shared = cfg1_oracle_runs
+    lcg = _runs(L, R, betas, theta, list(range(21, 31)), LCG)
+    phi = [obs for _, obs in shared]
     for i in (10, 30, 44, 60, 100):
         k = ex.kaufman(betas[i], L)
         for key in ("e", "C", "betaF_per_N", "S_per_N"):

@@ -418,12 +418,12 @@ def test_pa_run_matches_exact_enumeration_L4():
     assert np.abs(errs.mean(0)).max() < 0.05
 
 
-def test_pa_run_matches_kaufman_L16():
-    # configs[0] of BASELINE.json (L=16, R=1000, 100 steps, theta=10) over 8 seeds
-    L, R, theta = 16, 1000, 10
-    betas = [i / 100 for i in range(101)]
-    seeds = list(range(1, 9))
-    runs, _ = _seed_scatter(L, R, betas, theta, seeds)
+def test_pa_run_matches_kaufman_L16(cfg1_oracle_runs):
+    # configs[0] of BASELINE.json (L=16, R=1000, 100 steps, theta=10) over 8 seeds (runs shared with other pins: conftest.py)
+    L = 16
+    betas, shared = cfg1_oracle_runs
+    runs = [obs for _, obs in shared]
+    seeds = list(range(len(runs)))
     for i in (10, 30, 44, 60, 100):
         k = ex.kaufman(betas[i], L)
         for key in ("e", "C", "betaF_per_N", "S_per_N"):

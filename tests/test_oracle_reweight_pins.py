@@ -70,13 +70,12 @@ def test_reweight_from_pa_runs_matches_exact_L4():
             assert abs(v.mean() - want[k]) < 5 * sigma + 1e-12, (b, k, v.mean(), want[k], sigma)
 
 
-def test_reweight_from_pa_runs_matches_kaufman_L16():
+def test_reweight_from_pa_runs_matches_kaufman_L16(cfg1_oracle_runs):
     # configs[0] of BASELINE.json: reweighted curves at off-grid temperatures against Kaufman's exact finite-L
     # results; the multi-histogram estimate also has to be at least as sharp as the single-temperature one
-    L, R, theta = 16, 1000, 10
-    betas = [i / 100 for i in range(101)]
+    L = 16
     grid = np.array([0.105, 0.305, 0.4355, 0.605, 0.955])
-    runs = _runs(L, R, betas, theta, list(range(1, 9)))
+    _, runs = cfg1_oracle_runs
     vals = {k: np.array([o.reweight(grid)[k] for o, _ in runs]) for k in ("lnZ", "e", "C")}
     for i, b in enumerate(grid):
         k_ex = ex.kaufman(float(b), L)
