@@ -139,6 +139,16 @@ int pa_hist_accumulate(pa_t* h, double beta);
 /* Hsum: int64[N+1], lnD: double[N+1] (either may be NULL); ln Omega(E_m) = ln Hsum[m] - lnD[m]. */
 int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD);
 
+/* n temperature steps in one call (steps 2-4 of L56-L62, n times): for i = 1..n, resample betas[i-1] -> betas[i], theta
+ * sweeps at betas[i], measure; obs_out[i-1] = the output line of betas[i] (L179-L181).  betas: double[n+1], HOST, non-decreasing,
+ * betas[0] = the current temperature; obs_out: pa_obs_t[n], HOST, or NULL.  Computes exactly what the same sequence of
+ * pa_resample / pa_sweep / pa_observables calls computes (same spins, copy numbers, ln Z, observables), but the population
+ * size and E_min stay on the device and nothing inside a chunk of steps waits for the host: the launch-bound small
+ * configurations run at the speed of their kernels.  The Eq. 9 histogram is not folded (call pa_hist_accumulate between
+ * calls for that).  Errors: PA_ERR_INVALID_ARG as for the single calls; PA_ERR_CAPACITY if any step left [1, R_cap] -- the
+ * later steps have already run on it, so the population is then undefined (destroy the handle).  Synchronises. */
+int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out);
+
 /* Multi-histogram reweighting (Sec. 2.4; O12, O14): from the sums accumulated so far, the density of
  * states ln Omega(E_m) = ln Hsum[m] - lnD[m] (Eq. 9) and, for each of the n inverse temperatures betas[i]
  * (any values, not only simulated ones), lnZ[i] = ln sum_m Omega_m exp(-beta E_m) (= -beta F, Eq. 4),

@@ -198,6 +198,7 @@ void pa_destroy(pa_t* h) {
     for (int i = 0; i < 9; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->h_wtab) cudaFreeHost(h->h_wtab);
+    if (h->h_tabs) cudaFreeHost(h->h_tabs);
     if (h->owns_stream && h->stream) cudaStreamDestroy(h->stream);
     if (h->owns_ws && h->ws) cudaFree(h->ws);
     delete h;
@@ -352,23 +353,123 @@ int pa_adapt_dbeta(pa_t* h, double target, double beta, double beta_max, double*
     return PA_OK;
 }
 
-int pa_observables(pa_t* h, double beta, pa_obs_t* out) {
-    if (!h || !out) return PA_ERR_INVALID_ARG;
-    int rc;
-    if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
-    const PaScalars& s = *h->h_scal;
-    const double R = (double)h->R_cur, N = (double)h->N;
-    const __int128 num = (__int128)h->R_cur * (__int128)s.SE2 - (__int128)s.SE * (__int128)s.SE;   // exact (O8)
+// Eq. 3-5 (O8) from the exact integer sums of a measured population
+static void pa_fill_obs(const pa_handle* h, const PaScalars& s, double beta, int64_t R_cur, double lnZ, double lnQ, pa_obs_t* out) {
+    const double R = (double)R_cur, N = (double)h->N;
+    const __int128 num = (__int128)R_cur * (__int128)s.SE2 - (__int128)s.SE * (__int128)s.SE;   // exact (O8)
     out->beta = beta;
     out->e = (double)s.SE / (R * N);
     out->C = beta * beta * ((double)num / (R * R * N));
     out->absm = (double)s.SA / (R * N);
     out->m2 = (double)s.SM2 / (R * N * N);
     out->m4 = s.m4sum / R;
-    out->betaF_per_N = -h->lnZ / N;
-    out->S_per_N = beta * out->e + h->lnZ / N;
-    out->lnQ = h->lnQ_last;
-    out->R = h->R_cur;
+    out->betaF_per_N = -lnZ / N;
+    out->S_per_N = beta * out->e + lnZ / N;
+    out->lnQ = lnQ;
+    out->R = R_cur;
+}
+
+int pa_observables(pa_t* h, double beta, pa_obs_t* out) {
+    if (!h || !out) return PA_ERR_INVALID_ARG;
+    int rc;
+    if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
+    pa_fill_obs(h, *h->h_scal, beta, h->R_cur, h->lnZ, h->lnQ_last, out);
+    return PA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// pa_anneal: n temperature steps (resample -> theta sweeps -> measure) enqueued back to back, with NO host round trip inside:
+// the population size and E_min stay on the device (PaScalars::R_dev, mmin_inv), the weight tables of all steps of a chunk are
+// built on the host beforehand for the full level range and uploaded once, and a snapshot of the device scalars is kept per
+// step.  The host reads the snapshots at the end of the chunk and does exactly the arithmetic of pa_resample / pa_observables
+// on them (ln Q, ln Z, Eq. 3-5), so every number equals the step-by-step calls'.
+// ------------------------------------------------------------------------------------------------
+int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out) {
+    if (!h || !betas || n < 1 || theta < 0 || pa_is_device_ptr(betas) || (obs_out && pa_is_device_ptr(obs_out))) return PA_ERR_INVALID_ARG;
+    for (int i = 0; i <= n; ++i) if (!(betas[i] == betas[i]) || (i > 0 && !(betas[i] >= betas[i - 1]))) return PA_ERR_INVALID_ARG;
+    int rc;
+    if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
+    const size_t tab = (size_t)h->N + 1, snap = (sizeof(PaScalars) + 15) / 16 * 16;
+    const size_t per_step = tab * 8 + snap;
+    int chunk_cap = (int)(h->stage_bytes / per_step);
+    const char* ec = getenv("PA_ANNEAL_CHUNK");                    // tests: force small chunks
+    if (ec && atoi(ec) >= 1 && atoi(ec) < chunk_cap) chunk_cap = atoi(ec);
+    if (chunk_cap < 1) return PA_ERR_WORKSPACE;
+    if (chunk_cap > n) chunk_cap = n;
+    const size_t need = (size_t)chunk_cap * per_step + 16;
+    if (h->h_tabs_bytes < need) {
+        if (h->h_tabs) cudaFreeHost(h->h_tabs);
+        h->h_tabs = nullptr; h->h_tabs_bytes = 0;
+        PA_CUDA(h, cudaMallocHost(&h->h_tabs, need));
+        h->h_tabs_bytes = need;
+    }
+    // the device copy of the population size
+    uint32_t* h_init = (uint32_t*)((char*)h->h_tabs + (size_t)chunk_cap * per_step);
+    h_init[0] = (uint32_t)h->R_cur; h_init[1] = 0u;
+    PA_CUDA(h, cudaMemcpyAsync(&h->d_scal->R_dev, h_init, 8, cudaMemcpyHostToDevice, h->stream));
+    int Emin_prev = h->Emin;
+    int64_t R_prev = h->R_cur;
+    double* d_tabs = (double*)h->stage;
+    char* d_snaps = (char*)h->stage + (size_t)chunk_cap * tab * 8;
+    char* h_snaps = (char*)h->h_tabs + (size_t)chunk_cap * tab * 8;
+    for (int s0 = 0; s0 < n; s0 += chunk_cap) {
+        const int cs = n - s0 < chunk_cap ? n - s0 : chunk_cap;
+        for (int i = 0; i < cs; ++i) {                              // O5: wtab[d] = exp(-(dbeta * (double)(4 d))), full range
+            const double dbeta = betas[s0 + i + 1] - betas[s0 + i];
+            double* t = h->h_tabs + (size_t)i * tab;
+            for (int d = 0; d <= h->N; ++d) t[d] = exp(-(dbeta * (double)(4 * d)));
+        }
+        PA_CUDA(h, cudaMemcpyAsync(d_tabs, h->h_tabs, (size_t)cs * tab * 8, cudaMemcpyHostToDevice, h->stream));
+        h->dev_R = true;
+        rc = PA_OK;
+        for (int i = 0; i < cs && rc == PA_OK; ++i) {
+            const double beta = betas[s0 + i + 1];
+            h->wtab_cur = d_tabs + (size_t)i * tab;
+            cudaEventRecord(h->ev[2], h->stream);
+            if ((rc = pa_launch_weights(h, 0, h->w)) != PA_OK) break;
+            if ((rc = pa_launch_plan(h, 0)) != PA_OK) break;
+            cudaEventRecord(h->ev[4], h->stream);
+            if ((rc = pa_launch_copy(h)) != PA_OK) break;
+            cudaEventRecord(h->ev[5], h->stream);
+            if ((rc = pa_launch_commit(h)) != PA_OK) break;
+            cudaEventRecord(h->ev[3], h->stream);
+            h->cur ^= 1; h->k += 1;
+            const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
+            cudaEventRecord(h->ev[0], h->stream);
+            if ((rc = pa_launch_sweep(h, T4, T8, theta)) != PA_OK) break;
+            cudaEventRecord(h->ev[1], h->stream);
+            h->t += (uint32_t)theta;
+            if ((rc = pa_launch_measure(h)) != PA_OK) break;
+            if (cudaMemcpyAsync(d_snaps + (size_t)i * snap, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
+        }
+        h->dev_R = false; h->wtab_cur = nullptr;
+        if (rc != PA_OK) return rc;
+        PA_CUDA(h, cudaMemcpyAsync(h_snaps, d_snaps, (size_t)cs * snap, cudaMemcpyDeviceToHost, h->stream));
+        PA_CUDA(h, cudaStreamSynchronize(h->stream));
+        h->sweep_timed = theta > 0; h->resample_timed = true;
+        for (int i = 0; i < cs; ++i) {
+            const PaScalars& S = *(const PaScalars*)(h_snaps + (size_t)i * snap);
+            const double beta_old = betas[s0 + i], beta = betas[s0 + i + 1], dbeta = beta - beta_old;
+            const int64_t R_new = (int64_t)S.R_new;
+            if (S.err != 0u || R_new > h->R_cap || R_new < 1) {
+                // a step left [1, R_cap]: unlike pa_resample the later steps have already run on it -- the population is undefined
+                h->em_valid = false; h->host_scal_valid = false;
+                return PA_ERR_CAPACITY;
+            }
+            const double lnQ = -dbeta * (double)Emin_prev + log(S.W / (double)R_prev);   // Eq. 1 with the shift (O5)
+            h->lnZ += lnQ; h->lnQ_last = lnQ;                                            // Eq. 4 (L90)
+            h->R_prev = R_prev; h->W_last = S.W;
+            h->R_cur = R_new;
+            if (obs_out) pa_fill_obs(h, S, beta, R_new, h->lnZ, lnQ, &obs_out[s0 + i]);
+            Emin_prev = -2 * h->N + 4 * (int)(0xffffffffu - S.mmin_inv) + h->e0;
+            R_prev = R_new;
+            if (s0 + i == n - 1) {
+                *h->h_scal = S;
+                h->host_scal_valid = true; h->em_valid = true;
+                h->Emin = Emin_prev; h->Emax = -2 * h->N + 4 * (int)S.mmax + h->e0;
+            }
+        }
+    }
     return PA_OK;
 }
 

@@ -75,7 +75,20 @@ struct PaScalars {
     uint32_t pad1;
     double W;                    // normaliser of the last weight table, TREE1024 order (pa_tree_kernel<0>)
     double sum;                  // TREE1024 of min(1, tau_j) (pa_tree_kernel<1>)
+    // --- device-resident loop (pa_anneal): the population size lives on the device between host reads
+    uint32_t R_dev;              // current population size (pa_commit_kernel)
+    uint32_t err;                // 1 = a resampling step left [1, R_cap]
 };
+
+// Kernels take the population size and E_min either from the host (the step-by-step calls) or, inside pa_anneal, from
+// the device scalars: R < 0 / Emin == PA_EMIN_DEV select the device copy.
+#define PA_EMIN_DEV (-2147483647 - 1)
+#ifdef __CUDACC__
+__device__ __forceinline__ long long pa_live_R(long long R, const PaScalars* sc) { return R >= 0 ? R : (long long)sc->R_dev; }
+__device__ __forceinline__ int pa_live_Emin(int Emin, const PaScalars* sc, int N, int e0) {
+    return Emin != PA_EMIN_DEV ? Emin : -2 * N + 4 * (int)(0xffffffffu - sc->mmin_inv) + e0;
+}
+#endif
 
 struct pa_handle {
     int L, N;
@@ -103,6 +116,7 @@ struct pa_handle {
     uint32_t *r, *o, *parent;           // copy numbers, exclusive offsets, parent map
     double* partials;                   // per-tile partial sums (TREE1024)
     double* wtab;                       // weight table, device, N+1 entries
+    const double* wtab_cur;             // pa_anneal: this step's full-range table (NULL = wtab)
     unsigned long long* scan_state;     // decoupled look-back tile states
     unsigned long long* Hsum;           // [N+1]
     uint32_t* Hcur;                     // [N+1] histogram of the current temperature
@@ -121,6 +135,8 @@ struct pa_handle {
     cudaEvent_t ev[9];                  // sweep begin/end, resample begin/end, copy begin/end, plan scalars on the host, measure begin/end
     bool sweep_timed, resample_timed, measure_timed;
     bool hist_any;                      // pa_hist_accumulate has run at least once
+    bool dev_R;                         // inside pa_anneal: kernels read R and E_min from d_scal, grids cover the capacity
+    double* h_tabs; size_t h_tabs_bytes; // pinned staging for pa_anneal's weight tables and snapshots
     int64_t launches;
     bool sweep_C_forced;
     int sweep_C, sweep_T, sweep_cmp, sweep_kind;   // sweep launch geometry (cluster size, threads), compare variant, kernel kind
@@ -143,7 +159,8 @@ int pa_launch_measure(pa_handle* h);                                   // E, M, 
 int pa_launch_weights(pa_handle* h, int Emin, double* w_out);          // w_j, W = TREE1024(w) -> d_scal->W
 int pa_launch_overlap(pa_handle* h, int Emin);                         // TREE1024(min(1, tau_j)) -> d_scal->sum
 int pa_launch_plan(pa_handle* h, int Emin);                            // tau, r, scan, parent map, R_new
-int pa_launch_copy(pa_handle* h);                                      // new[d] = old[parent(d)], d < R_new (read on the device)
+int pa_launch_copy(pa_handle* h);
+int pa_launch_commit(pa_handle* h);                                    // pa_anneal: R_dev <- R_new (or the error flag)                                      // new[d] = old[parent(d)], d < R_new (read on the device)
 int pa_launch_hist(pa_handle* h, double beta);
 int pa_launch_reweight(pa_handle* h, int n, double* d_io);              // O12, O14: d_io = [betas | lnZ | e | C | absm | m2], n each
 cudaError_t pa_run_wavg(int M, const double* d_lnZ, const double* d_A, int nobs, double* d_out, double* d_omega, cudaStream_t st);

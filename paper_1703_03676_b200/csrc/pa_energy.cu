@@ -85,7 +85,7 @@ __device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&
         int nw = T >> 5, unsat = 0, up = 0;
         for (int w = 0; w < nw; ++w) { unsat += sE[w][lane]; up += sM[w][lane]; }
         const long long j = g * 32 + lane;
-        const bool live = j < R_cur;
+        const bool live = j < pa_live_R(R_cur, sc);
         const int e = 2 * unsat - 2 * N, m = 2 * up - N;
         if (live) { E[j] = e; M[j] = m; }
         long long se = live ? e : 0, se2 = live ? (long long)e * e : 0, sa = live ? (m < 0 ? -m : m) : 0, sm2 = live ? (long long)m * m : 0;
@@ -304,20 +304,21 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
 }
 
 int pa_launch_measure(pa_handle* h) {
-    const int64_t G = (h->R_cur + 31) / 32;
+    const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;      // dead groups contribute zeros (and +0.0 to the m^4 tree)
+    const long long Rarg = h->dev_R ? -1 : h->R_cur;
     const int L = h->L;
     PA_CUDA(h, cudaMemsetAsync(h->d_scal, 0, offsetof(PaScalars, R_new), h->stream));
     PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
     const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr && !h->has_j;
     if (pow2) {
 #define PA_MSR_CASE(LOG) case (8 << LOG): pa_measure_kernel<LOG><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
-            h->spins[h->cur], h->N, h->R_cur, h->E, h->M, h->d_scal, h->runsum, h->partials); break;
+            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials); break;
         switch (L) { PA_MSR_CASE(0) PA_MSR_CASE(1) PA_MSR_CASE(2) PA_MSR_CASE(3) PA_MSR_CASE(4) PA_MSR_CASE(5) default: break; }
 #undef PA_MSR_CASE
     } else {
         int T = 256;
         while (T > 32 && T * 8 > h->N) T >>= 1;
-        pa_measure_generic_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, h->E, h->M, h->d_scal,
+        pa_measure_generic_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, Rarg, h->E, h->M, h->d_scal,
                                                                     h->runsum, h->partials, h->has_j ? h->jmask : nullptr);
     }
     PA_CUDA(h, cudaGetLastError());

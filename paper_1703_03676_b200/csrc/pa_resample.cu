@@ -18,9 +18,11 @@ template <int MODE>
 __global__ void __launch_bounds__(PA_TILE)
 pa_tree_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* __restrict__ sc,
                long long R, double R_target, int Emin, double* __restrict__ w_out, double* __restrict__ partials,
-               unsigned long long* __restrict__ scan_state) {
+               unsigned long long* __restrict__ scan_state, int N, int e0) {
     __shared__ double run[32];
     __shared__ bool s_last;
+    R = pa_live_R(R, sc);
+    Emin = pa_live_Emin(Emin, sc, N, e0);
     const long long j = (long long)blockIdx.x * PA_TILE + threadIdx.x;
     double v = 0.0;
     if (j < R) {
@@ -67,9 +69,10 @@ pa_tree_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
 }
 
 int pa_launch_weights(pa_handle* h, int Emin, double* w_out) {
-    const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
-    pa_tree_kernel<0><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, Emin, w_out,
-                                                    h->partials, h->scan_state);
+    const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
+    pa_tree_kernel<0><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab_cur ? h->wtab_cur : h->wtab, h->d_scal, h->dev_R ? -1 : h->R_cur,
+                                                    (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, w_out,
+                                                    h->partials, h->scan_state, h->N, h->e0);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
@@ -78,7 +81,7 @@ int pa_launch_weights(pa_handle* h, int Emin, double* w_out) {
 int pa_launch_overlap(pa_handle* h, int Emin) {
     const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
     pa_tree_kernel<1><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, Emin, nullptr,
-                                                    h->partials, h->scan_state);
+                                                    h->partials, h->scan_state, h->N, h->e0);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
@@ -97,8 +100,10 @@ __global__ void __launch_bounds__(256)
 pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* sc,
                long long R, double R_target, int Emin, PhiloxKeys K, uint32_t kcount, long long R_cap,
                uint32_t* __restrict__ r_out, uint32_t* __restrict__ o_out, uint32_t* __restrict__ parent,
-               unsigned long long* __restrict__ state, int n_tiles) {
+               unsigned long long* __restrict__ state, int n_tiles, int N, int e0) {
     __shared__ uint32_t s_tile, s_warp[8], s_excl;
+    R = pa_live_R(R, sc);
+    Emin = pa_live_Emin(Emin, sc, N, e0);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_tile = atomicAdd(&sc->tile_counter, 1u);
     __syncthreads();
@@ -190,9 +195,10 @@ pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
 }
 
 int pa_launch_plan(pa_handle* h, int Emin) {
-    const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
-    pa_plan_kernel<<<n, 256, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, Emin, h->keys, h->k,
-                                             h->R_cap, h->r, h->o, h->parent, h->scan_state, n);
+    const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
+    pa_plan_kernel<<<n, 256, 0, h->stream>>>(h->E, h->wtab_cur ? h->wtab_cur : h->wtab, h->d_scal, h->dev_R ? -1 : h->R_cur,
+                                             (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, h->keys, h->k,
+                                             h->R_cap, h->r, h->o, h->parent, h->scan_state, n, h->N, h->e0);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
@@ -319,6 +325,19 @@ int pa_launch_copy(pa_handle* h) {
     while (G * gy < 592 && gy * 128 * 2 <= chunks) gy *= 2;
     dim3 grid((unsigned)G, (unsigned)gy, 1);
     pa_copy_kernel<<<grid, 128, 0, h->stream>>>(h->spins[h->cur], h->spins[1 - h->cur], h->parent, h->d_scal, h->R_cap, h->N);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
+
+// pa_anneal: the resampled population becomes the current one on the device (the host does the same bookkeeping later from
+// the per-step snapshots).  Outside [1, R_cap] the size is left alone and the error flag is raised.
+__global__ void pa_commit_kernel(PaScalars* sc, long long R_cap) {
+    const long long Rn = sc->R_new;
+    if (Rn >= 1 && Rn <= R_cap) sc->R_dev = (uint32_t)Rn; else sc->err = 1u;
+}
+int pa_launch_commit(pa_handle* h) {
+    pa_commit_kernel<<<1, 1, 0, h->stream>>>(h->d_scal, h->R_cap);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;

@@ -23,6 +23,8 @@ struct SweepParams {
     uint32_t two;                    // the constant 2, opaque to ptxas (see pa_shift_in_ge)
     int theta;
     int L, Lh, H, C, N;
+    long long R;                     // population size, or -1: read sc->R_dev (pa_anneal)
+    const PaScalars* sc;
     const uint8_t* jmask;            // O15: per resident word, bit k = bond to neighbour k (same, x, up, down) has J = -1; NULL = ferromagnet
 };
 
@@ -192,6 +194,7 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long g = blockIdx.x / C;
+    if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H, Lh = P.Lh, L = P.L;
     const int y0 = (int)cr * H;
     const int half = H * Lh;
@@ -304,6 +307,7 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long g = blockIdx.x / C;
+    if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H;
     const int y0 = (int)cr * H;
     const int half = H * Lh;
@@ -396,6 +400,7 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long g = blockIdx.x / C;
+    if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H;
     const int y0 = (int)cr * H;
     const int half = H * Lh;
@@ -634,7 +639,8 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     P.K = h->keys;
     P.T4 = T4; P.T8 = T8;
     P.t0 = h->t; P.theta = theta; P.two = 2u;
-    const int64_t G = (h->R_cur + 31) / 32;
+    const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;
+    P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     P.L = h->L; P.Lh = h->L / 2; P.C = pa_sweep_pick_C(h, G); P.H = h->L / P.C; P.N = h->N;
     const size_t smem = (size_t)P.H * h->L * 4;
     const unsigned grid = (unsigned)(G * P.C);

@@ -66,6 +66,7 @@ def lib():
         "pa_create_ex": ([i32, i64, u64, vp, sz, vp, C.POINTER(vp)], i32),
         "pa_destroy": ([vp], None),
         "pa_sweep": ([vp, dbl, i32], i32),
+        "pa_anneal": ([vp, i32, vp, i32, vp], i32),
         "pa_set_rng_mode": ([vp, i32], i32),
         "pa_set_couplings": ([vp, vp, vp], i32),
         "pa_level_offset": ([vp], i32),
@@ -241,6 +242,15 @@ class Population:
         self._check(lib().pa_set_counters(self._h, t, k, float(lnZ)), "pa_set_counters")
 
     # the path
+    def anneal(self, betas, theta):
+        """pa_anneal: resample betas[i-1] -> betas[i], theta sweeps, measure, for i = 1..len(betas)-1, without host round trips;
+        betas[0] must be the current temperature.  Returns the observables of betas[1:]."""
+        betas = np.ascontiguousarray(betas, dtype=np.float64)
+        n = betas.size - 1
+        out = (pa_obs_t * n)()
+        self._check(lib().pa_anneal(self._h, n, _ptr(betas), int(theta), C.cast(out, C.c_void_p)), "pa_anneal")
+        return [o.as_dict() for o in out]
+
     def set_couplings(self, Jx, Jy):
         """Bimodal couplings (int8 [N], +-1; Jx[s]: bond to the right of s = y*L+x, Jy[s]: bond below); None, None = ferromagnet."""
         if Jx is None:

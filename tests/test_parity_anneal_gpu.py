@@ -1,0 +1,96 @@
+"""pa_anneal (n temperature steps without host round trips; population size and E_min resident on the device) against
+(a) the same sequence of pa_resample / pa_sweep / pa_observables calls on the device: every number identical, and
+(b) the CPU oracle: spins, energies, copy numbers bit-exact, observables 1e-9 (-m gpu)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+if not torch.cuda.is_available():
+    pytest.skip("no CUDA device", allow_module_level=True)
+
+from oracle import pa_oracle as po                      # noqa: E402
+from paper_1703_03676_b200 import pa                    # noqa: E402
+from paper_1703_03676_b200.workloads import CONFIGS, random_couplings     # noqa: E402
+import pa_driver                                        # noqa: E402
+
+REL = 1e-9
+KEYS = ("beta", "e", "C", "absm", "m2", "m4", "betaF_per_N", "S_per_N", "lnQ", "R")
+
+
+def _state(g):
+    E, M = g.energies()
+    return g.population, g.sweep_counter, g.resample_counter, g.lnZ, g.get_spins().tobytes(), E.tobytes(), M.tobytes()
+
+
+@pytest.mark.parametrize("L,R,mode,theta,chunk", [(16, 1000, 0, 3, None), (8, 33, 1, 2, "2"), (64, 2500, 1, 2, "3"), (64, 700, 0, 1, None),
+                                                   (128, 200, 0, 1, "1"), (6, 1, 0, 2, None), (32, 5000, 0, 0, None)])
+def test_anneal_equals_step_by_step_calls_and_oracle(monkeypatch, L, R, mode, theta, chunk):
+    if chunk:
+        monkeypatch.setenv("PA_ANNEAL_CHUNK", chunk)                  # several chunks: tables and snapshots are re-staged
+    else:
+        monkeypatch.delenv("PA_ANNEAL_CHUNK", raising=False)
+    betas = [0.0, 0.05, 0.12, 0.12, 0.3, 0.44, 0.6, 0.95]              # uneven steps, one of them empty (dbeta = 0)
+    a, b, o = pa.Population(L, R, 41), pa.Population(L, R, 41), po.Oracle(L, R, 41)
+    for x in (a, b, o):
+        x.set_rng_mode(mode)
+    obs_a = a.anneal(betas, theta)
+    obs_b = pa_driver.run_fixed(b, betas, theta)[1:]
+    obs_o = pa_driver.run_fixed(o, betas, theta)[1:]
+    assert len(obs_a) == len(betas) - 1
+    for x, y, z in zip(obs_a, obs_b, obs_o):
+        for k in KEYS:
+            assert x[k] == y[k], (k, x[k], y[k])                        # the same host arithmetic on the same device sums
+            assert x[k] == pytest.approx(z[k], rel=REL, abs=1e-300), (k, x[k], z[k])
+    assert _state(a) == _state(b)
+    assert np.array_equal(a.get_spins(), o.get_spins())
+    # the handle carries on: last resample's vectors, further single calls, a second anneal
+    da, db = a.resample_debug(obs_a[-2]["R"]), b.resample_debug(obs_b[-2]["R"])
+    assert da["W"] == db["W"] and np.array_equal(da["r"], db["r"]) and np.array_equal(da["o"], db["o"]) and np.array_equal(da["w"], db["w"])
+    assert a.adapt_dbeta(0.8, betas[-1], 2.0) == b.adapt_dbeta(0.8, betas[-1], 2.0)
+    more = [betas[-1], 1.0, 1.1]
+    a.resample(more[0], more[1]); a.sweep(more[1], 1); x1 = a.observables(more[1])
+    y1 = b.anneal(more[:2], 1)[0]
+    assert all(x1[k] == y1[k] for k in KEYS)
+    assert _state(a) == _state(b)
+
+
+def test_anneal_with_couplings_and_histogram_between_calls():
+    L, R, theta = 16, 800, 2
+    Jx, Jy = random_couplings(L, 3)
+    a, o = pa.Population(L, R, 5), po.Oracle(L, R, 5)
+    a.set_couplings(Jx, Jy); o.set_couplings(Jx, Jy)
+    betas = [0.1 * i for i in range(11)]
+    a.observables(0.0); a.hist_accumulate(0.0)
+    o.observables(0.0); o.hist_accumulate(0.0)
+    for i in range(0, 10, 5):                                            # two anneal calls of 5 steps, a histogram fold after each
+        obs = a.anneal(betas[i:i + 6], theta)
+        a.hist_accumulate(betas[i + 5])
+        for s in range(i + 1, i + 6):
+            o.resample(betas[s - 1], betas[s]); o.sweep(betas[s], theta)
+            oo = o.observables(betas[s])
+            for k in KEYS:
+                assert obs[s - i - 1][k] == pytest.approx(oo[k], rel=REL, abs=1e-300), (s, k)
+        o.hist_accumulate(betas[i + 5])
+    assert np.array_equal(a.get_spins(), o.get_spins())
+    assert np.array_equal(a.histogram()[0], o.histogram()[0])
+    assert np.allclose(a.histogram()[1][np.isfinite(o.histogram()[1])], o.histogram()[1][np.isfinite(o.histogram()[1])], rtol=REL)
+
+
+def test_anneal_errors():
+    g = pa.Population(8, 100, 2)
+    lib = pa.lib()
+    b = np.array([0.0, 0.1, 0.05])
+    assert lib.pa_anneal(g._h, 2, pa._ptr(b), 1, None) == pa.PA_ERR_INVALID_ARG          # decreasing beta
+    assert lib.pa_anneal(g._h, 0, pa._ptr(b), 1, None) == pa.PA_ERR_INVALID_ARG
+    assert lib.pa_anneal(g._h, 1, pa._ptr(b), -1, None) == pa.PA_ERR_INVALID_ARG
+    assert lib.pa_anneal(g._h, 1, None, 1, None) == pa.PA_ERR_INVALID_ARG
+    before = g.get_spins()
+    assert lib.pa_anneal(g._h, 1, pa._ptr(np.array([0.0, 0.0])), 0, None) == pa.PA_OK     # dbeta = 0, theta = 0: identity
+    assert np.array_equal(g.get_spins(), before) and g.population == 100
+    # a huge step from a handful of replicas: R_new ~ R_target fits; a capacity overflow needs R_new > R + 1024: shrink first
+    words = g.get_words()
+    g.set_words(3, words[:1])
+    rc = lib.pa_anneal(g._h, 1, pa._ptr(np.array([0.0, 0.01])), 0, None)
+    assert rc == pa.PA_OK and abs(g.population - 100) <= 3                                # 3 replicas -> ~100 copies: within capacity
