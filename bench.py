@@ -132,7 +132,9 @@ def rank_seed(wl, rank):
     return wl.seed + rank
 
 
-def one_step(pop, wl, beta_prev, beta):
+def one_step(pop, wl, beta_prev, beta, fused=False):
+    if fused and not wl.multi_histogram:
+        return pop.anneal([beta_prev, beta], wl.theta)[0]              # the same step through pa_anneal: no host round trip inside
     pop.resample(beta_prev, beta)
     pop.sweep(beta, wl.theta)
     obs = pop.observables(beta)
@@ -186,6 +188,20 @@ def whole_run(pa, wl, seed, rng):
            "sweep_updates_per_ns": {k: v[1] for k, v in marks.items()},
            "final_observables": obs}
     pop.close()
+    if wl.n_steps is not None and not wl.multi_histogram:
+        # the same schedule in ONE pa_anneal call (no host round trip between its steps)
+        pop = pa.Population(wl.L, wl.R, seed)
+        if rng == "lcg":
+            pop.set_rng_mode(pa.PA_RNG_LCG)
+        pop.observables(wl.beta0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        obs2 = pop.anneal(betas, wl.theta)
+        t2 = time.perf_counter() - t0
+        flips2 = sum(o["R"] for o in obs2) * wl.N * wl.theta
+        out["one_call"] = {"api": "pa_anneal", "t_run_s": t2, "t_SF_ns": t2 * 1e9 / flips2, "updates_per_ns": flips2 / (t2 * 1e9),
+                           "same_final_observables": obs2[-1] == obs}
+        pop.close()
     return out
 
 
@@ -243,12 +259,13 @@ def run_ours(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
     peaks, peak_src = measured_peaks()
 
+    fused = args.api == "anneal" and wl.n_steps is not None and not wl.multi_histogram
     beta_prev, i = wl.beta0, 0
     pop.observables(beta_prev)
     for _ in range(Wm):                                                        # warm-up steps (untimed)
         i += 1
         beta = next_beta(pop, wl, betas, i, beta_prev)
-        one_step(pop, wl, beta_prev, beta)
+        one_step(pop, wl, beta_prev, beta, fused)
         beta_prev = beta
     torch.cuda.synchronize()
     if world > 1:
@@ -267,7 +284,7 @@ def run_ours(args):
         ev[s][0].record()
         if beta is None:                                                       # adaptive: the bisection is part of the step
             beta = next_beta(pop, wl, betas, i, beta_prev)
-        obs = one_step(pop, wl, beta_prev, beta)
+        obs = one_step(pop, wl, beta_prev, beta, fused)
         ev[s][1].record()
         beta_prev = beta
         R = obs["R"]
@@ -351,6 +368,7 @@ def run_ours(args):
            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "u32", "data": "synthetic",
            "config": {"workload": wl.name, "L": wl.L, "R_per_gpu": wl.R, "theta": wl.theta, "beta_from": wl.beta0, "rng": args.rng, "couplings": args.couplings,
+                      "api": "pa_anneal, one temperature step per call" if fused else "pa_resample + pa_sweep + pa_observables per step",
                       "schedule": "adaptive" if wl.n_steps is None else f"{wl.n_steps} equal steps to {wl.beta_f}",
                       "l2": "flushed between timed steps (256 MiB memset outside the CUDA events)",
                       "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
@@ -418,6 +436,8 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--whole-run", dest="whole_run", action="store_true", default=None,
                     help="also time the config's whole schedule (t_SF, Eq. 11); default: on for configs 1-4 (seconds), off for 5 (minutes)")
+    ap.add_argument("--api", default="steps", choices=["steps", "anneal"],
+                    help="timed steps through the single calls (default) or through pa_anneal, one step per call (fixed schedules)")
     ap.add_argument("--couplings", default="ferro", choices=["ferro", "pmj"],
                     help="ferromagnet (default, Eq. 10) or a seeded random +-J sample (second workload, PAPER.md L313; context)")
     ap.add_argument("--theta-scan", action="store_true", help="re-measure the paper's Table 3 / Table 4 theta dependence (context)")
