@@ -154,43 +154,59 @@ def whole_run(pa, wl, seed, rng):
     """the config's WHOLE annealing schedule on a fresh population, timed as the paper times its runs:
     t_SF = t_run / (N theta sum_i R_i) (Eq. 11), resampling, measurement (and, for the adaptive config, the
     bisection and the histogram fold) included; the resample cost depends on the weight distribution, so it is sampled in
-    situ at every step (median, max, and near beta = 0.1, beta_c, the last step), as is the sweep kernel's rate."""
+    situ at every step (median, max, and near beta = 0.1, beta_c, the last step), as is the sweep kernel's rate.  The in-situ
+    phase events cost time on a stream of small kernels, so where a run takes seconds it is done twice: once with the default
+    timing (sweep only) for t_SF, once instrumented for the per-step figures."""
     import torch
-    pop = pa.Population(wl.L, wl.R, seed)
-    if rng == "lcg":
-        pop.set_rng_mode(pa.PA_RNG_LCG)
+
+    def run(mask):
+        pop = pa.Population(wl.L, wl.R, seed)
+        pop.set_timing(mask)
+        if rng == "lcg":
+            pop.set_rng_mode(pa.PA_RNG_LCG)
+        betas = wl.betas() if wl.n_steps is not None else None
+        beta_prev, i = wl.beta0, 0
+        obs = pop.observables(beta_prev)
+        if wl.multi_histogram:
+            pop.hist_accumulate(beta_prev)
+        rows, flips = [], 0
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        while beta_prev < wl.beta_f and (betas is None or i < len(betas) - 1):
+            i += 1
+            beta = next_beta(pop, wl, betas, i, beta_prev)
+            obs = one_step(pop, wl, beta_prev, beta)
+            flips += obs["R"] * wl.N * wl.theta
+            if mask & pa.PA_TIME_RESAMPLE:
+                rt, ct = pop.last_resample_ms()
+                rows.append((beta, obs["R"] * wl.N * wl.theta / (pop.last_sweep_ms() * 1e6), rt, ct))
+            beta_prev = beta
+        torch.cuda.synchronize()
+        t_run = time.perf_counter() - t0
+        pop.close()
+        return t_run, flips, rows, obs, beta_prev, i
+
+    full = pa.PA_TIME_SWEEP | pa.PA_TIME_RESAMPLE
+    twice = wl.R * wl.N <= 2 * 10**9                                   # cfgs 1-4: seconds; cfg5: minutes, one instrumented pass
+    t_run, flips, rows, obs, beta_last, nsteps = run(pa.PA_TIME_SWEEP if twice else full)
+    if twice:
+        _, _, rows, _, _, _ = run(full)
     betas = wl.betas() if wl.n_steps is not None else None
-    beta_prev, i = wl.beta0, 0
-    pop.observables(beta_prev)
-    if wl.multi_histogram:
-        pop.hist_accumulate(beta_prev)
-    rows, flips = [], 0
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    while beta_prev < wl.beta_f and (betas is None or i < len(betas) - 1):
-        i += 1
-        beta = next_beta(pop, wl, betas, i, beta_prev)
-        obs = one_step(pop, wl, beta_prev, beta)
-        flips += obs["R"] * wl.N * wl.theta
-        rt, ct = pop.last_resample_ms()
-        rows.append((beta, obs["R"] * wl.N * wl.theta / (pop.last_sweep_ms() * 1e6), rt, ct))
-        beta_prev = beta
-    torch.cuda.synchronize()
-    t_run = time.perf_counter() - t0
 
     def near(b):
         return min(rows, key=lambda r: abs(r[0] - b))
     res = sorted(r[2] for r in rows)
     marks = {"beta_0.1": near(0.1), "beta_c": near(0.4406868), "last": rows[-1]}
-    out = {"steps": len(rows), "beta_final": beta_prev, "t_run_s": t_run, "t_SF_ns": t_run * 1e9 / flips, "updates_per_ns": flips / (t_run * 1e9),
-           "timing": "host wall clock around the whole schedule, synchronised on both sides (the paper's t_SF, Eq. 11)",
+    out = {"steps": nsteps, "beta_final": beta_last, "t_run_s": t_run, "t_SF_ns": t_run * 1e9 / flips, "updates_per_ns": flips / (t_run * 1e9),
+           "timing": "host wall clock around the whole schedule, synchronised on both sides (the paper's t_SF, Eq. 11)"
+                     + ("; per-step figures from a second, instrumented run" if twice else ""),
            "resample_ms": {"median": res[len(res) // 2], "max": res[-1], **{k: v[2] for k, v in marks.items()}},
            "sweep_updates_per_ns": {k: v[1] for k, v in marks.items()},
            "final_observables": obs}
-    pop.close()
     if wl.n_steps is not None and not wl.multi_histogram:
         # the same schedule in ONE pa_anneal call (no host round trip between its steps)
         pop = pa.Population(wl.L, wl.R, seed)
+        pop.set_timing(0)
         if rng == "lcg":
             pop.set_rng_mode(pa.PA_RNG_LCG)
         pop.observables(wl.beta0)
@@ -290,12 +306,24 @@ def run_ours(args):
         R = obs["R"]
         updates += R * wl.N * wl.theta
         sweep_ms.append(pop.last_sweep_ms()); sweep_updates.append(R * wl.N * wl.theta)
-        t, c = pop.last_resample_ms()
-        res_ms.append(t); copy_ms.append(c); copy_bytes.append(2 * ((R + 31) // 32) * wl.N * 4)
     torch.cuda.synchronize()
     launches = pop.launch_count - launches0
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
     clocks = sampler.stop() if rank == 0 else None
+    # resample / copy-kernel times: a few more steps with the phase events on (they cost ~3 us each, so they are off above)
+    pop.set_timing(pa.PA_TIME_SWEEP | pa.PA_TIME_RESAMPLE)
+    for _ in range(min(K, 5)):
+        if wl.n_steps is not None and i + 1 >= len(betas):
+            break
+        i += 1
+        beta = next_beta(pop, wl, betas, i, beta_prev)
+        o = one_step(pop, wl, beta_prev, beta)
+        beta_prev = beta
+        t, c = pop.last_resample_ms()
+        res_ms.append(t); copy_ms.append(c); copy_bytes.append(2 * ((o["R"] + 31) // 32) * wl.N * 4)
+    pop.set_timing(pa.PA_TIME_SWEEP)
+    if not res_ms:
+        res_ms, copy_ms, copy_bytes = [0.0], [0.0], [0]
     total_ms, updates_all = reduce_over_ranks(total_ms, updates, "cuda", dist if world > 1 else None)
     if world > 1:
         dist.barrier()

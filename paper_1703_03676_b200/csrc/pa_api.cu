@@ -140,7 +140,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     if (!h) return PA_ERR_NOMEM;
     memset(h, 0, sizeof(*h));
     h->L = L; h->N = L * L; h->R_target = R; h->R_cur = R; h->R_cap = y.R_cap; h->G_cap = y.G_cap;
-    h->seed = seed; h->keys = pa_make_keys(seed); h->rng_mode = PA_RNG_PHILOX;
+    h->seed = seed; h->keys = pa_make_keys(seed); h->rng_mode = PA_RNG_PHILOX; h->timing = PA_TIME_SWEEP;
     h->lnZ = (double)h->N * log(2.0);           // Z_{beta_0} = 2^N (L93)
     h->n_tiles_cap = y.tiles;
     int rc = PA_OK;
@@ -171,7 +171,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     if (cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
         cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->N + 1)) != cudaSuccess) { rc = PA_ERR_CUDA; }
     for (int i = 0; i < 9 && rc == PA_OK; ++i)
-        if (cudaEventCreate(&h->ev[i]) != cudaSuccess) rc = PA_ERR_CUDA;
+        if (cudaEventCreateWithFlags(&h->ev[i], i == 6 ? cudaEventDisableTiming : cudaEventDefault) != cudaSuccess) rc = PA_ERR_CUDA;
     if (rc == PA_OK) rc = pa_sweep_configure(h);
     if (rc == PA_OK) {
         // empty histograms: Hsum = 0, Hcur = 0, lnD = -inf
@@ -199,6 +199,7 @@ void pa_destroy(pa_t* h) {
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->h_wtab) cudaFreeHost(h->h_wtab);
     if (h->h_tabs) cudaFreeHost(h->h_tabs);
+    for (int b = 0; b < 2; ++b) if (h->ev_chunk[b]) cudaEventDestroy(h->ev_chunk[b]);
     if (h->owns_stream && h->stream) cudaStreamDestroy(h->stream);
     if (h->owns_ws && h->ws) cudaFree(h->ws);
     delete h;
@@ -208,11 +209,12 @@ int pa_sweep(pa_t* h, double beta, int theta) {
     if (!h || theta < 0 || !(beta == beta)) return PA_ERR_INVALID_ARG;
     if (theta == 0) return PA_OK;
     const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
-    PA_CUDA(h, cudaEventRecord(h->ev[0], h->stream));
+    const bool timed = (h->timing & PA_TIME_SWEEP) != 0;
+    if (timed) PA_CUDA(h, cudaEventRecord(h->ev[0], h->stream));
     int rc = pa_launch_sweep(h, T4, T8, theta);
     if (rc != PA_OK) return rc;
-    PA_CUDA(h, cudaEventRecord(h->ev[1], h->stream));
-    h->sweep_timed = true;
+    if (timed) PA_CUDA(h, cudaEventRecord(h->ev[1], h->stream));
+    h->sweep_timed = timed;
     h->t += (uint32_t)theta;
     h->em_valid = false; h->host_scal_valid = false;
     return PA_OK;
@@ -276,7 +278,8 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     if (!h || !(beta_new >= beta)) return PA_ERR_INVALID_ARG;
     const double dbeta = beta_new - beta;
     int rc;
-    PA_CUDA(h, cudaEventRecord(h->ev[2], h->stream));
+    const bool timed = (h->timing & PA_TIME_RESAMPLE) != 0;
+    if (timed) PA_CUDA(h, cudaEventRecord(h->ev[2], h->stream));
     // E_min / E_max: already on the host if pa_observables ran on this population (the usual loop, L62);
     // otherwise one measure launch and one read
     if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
@@ -289,13 +292,13 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     // R_new and W travel to the host right after the plan kernel; the copy is queued behind them and runs
     // while the host wakes up, so the stream never idles on this call's one synchronisation
     PA_CUDA(h, cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToHost, h->stream));
-    PA_CUDA(h, cudaEventRecord(h->ev[6], h->stream));
-    PA_CUDA(h, cudaEventRecord(h->ev[4], h->stream));
+    PA_CUDA(h, cudaEventRecord(h->ev[6], h->stream));                // the host waits on this one (created without timing)
+    if (timed) PA_CUDA(h, cudaEventRecord(h->ev[4], h->stream));
     if ((rc = pa_launch_copy(h)) != PA_OK) return rc;
-    PA_CUDA(h, cudaEventRecord(h->ev[5], h->stream));
-    PA_CUDA(h, cudaEventRecord(h->ev[3], h->stream));
+    if (timed) PA_CUDA(h, cudaEventRecord(h->ev[5], h->stream));
+    if (timed) PA_CUDA(h, cudaEventRecord(h->ev[3], h->stream));
     PA_CUDA(h, cudaEventSynchronize(h->ev[6]));
-    h->resample_timed = true;
+    h->resample_timed = timed;
     const int64_t R_new = (int64_t)h->h_scal->R_new;
     const double W = h->h_scal->W;
     h->R_prev = h->R_cur; h->W_last = W;
@@ -384,93 +387,127 @@ int pa_observables(pa_t* h, double beta, pa_obs_t* out) {
 // step.  The host reads the snapshots at the end of the chunk and does exactly the arithmetic of pa_resample / pa_observables
 // on them (ln Q, ln Z, Eq. 3-5), so every number equals the step-by-step calls'.
 // ------------------------------------------------------------------------------------------------
+struct PaAnnealCtx {            // host bookkeeping that runs along the snapshots, in step order
+    int Emin_prev; int64_t R_prev;
+};
+
+// the arithmetic of pa_resample / pa_observables on the snapshots of one finished chunk
+static int pa_anneal_digest(pa_handle* h, PaAnnealCtx& cx, const char* h_snaps, size_t snap, int s0, int cs, int n,
+                            const double* betas, pa_obs_t* obs_out) {
+    for (int i = 0; i < cs; ++i) {
+        const PaScalars& S = *(const PaScalars*)(h_snaps + (size_t)i * snap);
+        const double beta_old = betas[s0 + i], beta = betas[s0 + i + 1], dbeta = beta - beta_old;
+        const int64_t R_new = (int64_t)S.R_new;
+        if (S.err != 0u || R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;
+        const double lnQ = -dbeta * (double)cx.Emin_prev + log(S.W / (double)cx.R_prev);   // Eq. 1 with the shift (O5)
+        h->lnZ += lnQ; h->lnQ_last = lnQ;                                                  // Eq. 4 (L90)
+        h->R_prev = cx.R_prev; h->W_last = S.W;
+        h->R_cur = R_new;
+        if (obs_out) pa_fill_obs(h, S, beta, R_new, h->lnZ, lnQ, &obs_out[s0 + i]);
+        cx.Emin_prev = -2 * h->N + 4 * (int)(0xffffffffu - S.mmin_inv) + h->e0;
+        cx.R_prev = R_new;
+        if (s0 + i == n - 1) {
+            *h->h_scal = S;
+            h->host_scal_valid = true; h->em_valid = true;
+            h->Emin = cx.Emin_prev; h->Emax = -2 * h->N + 4 * (int)S.mmax + h->e0;
+        }
+    }
+    return PA_OK;
+}
+
 int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out) {
     if (!h || !betas || n < 1 || theta < 0 || pa_is_device_ptr(betas) || (obs_out && pa_is_device_ptr(obs_out))) return PA_ERR_INVALID_ARG;
     for (int i = 0; i <= n; ++i) if (!(betas[i] == betas[i]) || (i > 0 && !(betas[i] >= betas[i - 1]))) return PA_ERR_INVALID_ARG;
     int rc;
     if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
+    // Steps go in chunks with two staging buffers: while the device runs chunk c the host builds the weight tables of chunk
+    // c+1 (N+1 exponentials per step) and digests the snapshots of chunk c-1.
     const size_t tab = (size_t)h->N + 1, snap = (sizeof(PaScalars) + 15) / 16 * 16;
     const size_t per_step = tab * 8 + snap;
-    int chunk_cap = (int)(h->stage_bytes / per_step);
-    const char* ec = getenv("PA_ANNEAL_CHUNK");                    // tests: force small chunks
+    int chunk_cap = (int)(h->stage_bytes / 2 / per_step);
+    if (chunk_cap > 16) chunk_cap = 16;
+    const char* ec = getenv("PA_ANNEAL_CHUNK");                    // tests: force other chunk sizes
     if (ec && atoi(ec) >= 1 && atoi(ec) < chunk_cap) chunk_cap = atoi(ec);
     if (chunk_cap < 1) return PA_ERR_WORKSPACE;
     if (chunk_cap > n) chunk_cap = n;
-    const size_t need = (size_t)chunk_cap * per_step + 16;
+    const size_t buf_bytes = ((size_t)chunk_cap * per_step + 255) / 256 * 256;
+    const size_t need = 2 * buf_bytes + 16;
     if (h->h_tabs_bytes < need) {
         if (h->h_tabs) cudaFreeHost(h->h_tabs);
+    for (int b = 0; b < 2; ++b) if (h->ev_chunk[b]) cudaEventDestroy(h->ev_chunk[b]);
         h->h_tabs = nullptr; h->h_tabs_bytes = 0;
         PA_CUDA(h, cudaMallocHost(&h->h_tabs, need));
         h->h_tabs_bytes = need;
     }
+    for (int b = 0; b < 2; ++b)
+        if (!h->ev_chunk[b]) PA_CUDA(h, cudaEventCreateWithFlags(&h->ev_chunk[b], cudaEventDisableTiming));
     // the device copy of the population size
-    uint32_t* h_init = (uint32_t*)((char*)h->h_tabs + (size_t)chunk_cap * per_step);
+    uint32_t* h_init = (uint32_t*)((char*)h->h_tabs + 2 * buf_bytes);
     h_init[0] = (uint32_t)h->R_cur; h_init[1] = 0u;
     PA_CUDA(h, cudaMemcpyAsync(&h->d_scal->R_dev, h_init, 8, cudaMemcpyHostToDevice, h->stream));
-    int Emin_prev = h->Emin;
-    int64_t R_prev = h->R_cur;
-    double* d_tabs = (double*)h->stage;
-    char* d_snaps = (char*)h->stage + (size_t)chunk_cap * tab * 8;
-    char* h_snaps = (char*)h->h_tabs + (size_t)chunk_cap * tab * 8;
-    for (int s0 = 0; s0 < n; s0 += chunk_cap) {
+    PaAnnealCtx cx = {h->Emin, h->R_cur};
+    int pend_s0[2] = {-1, -1}, pend_cs[2] = {0, 0};
+    rc = PA_OK;
+    int c = 0;
+    for (int s0 = 0; s0 < n && rc == PA_OK; s0 += chunk_cap, ++c) {
+        const int b = c & 1;
         const int cs = n - s0 < chunk_cap ? n - s0 : chunk_cap;
-        for (int i = 0; i < cs; ++i) {                              // O5: wtab[d] = exp(-(dbeta * (double)(4 d))), full range
+        char* hb = (char*)h->h_tabs + (size_t)b * buf_bytes;
+        char* db = (char*)h->stage + (size_t)b * buf_bytes;
+        double *h_t = (double*)hb, *d_t = (double*)db;
+        char *h_snaps = hb + (size_t)chunk_cap * tab * 8, *d_snaps = db + (size_t)chunk_cap * tab * 8;
+        if (pend_s0[b] >= 0) {                                       // chunk c-2 used this buffer: wait for it and digest it
+            if (cudaEventSynchronize(h->ev_chunk[b]) != cudaSuccess) { rc = PA_ERR_CUDA; break; }
+            rc = pa_anneal_digest(h, cx, h_snaps, snap, pend_s0[b], pend_cs[b], n, betas, obs_out);
+            pend_s0[b] = -1;
+            if (rc != PA_OK) break;
+        }
+        for (int i = 0; i < cs; ++i) {                               // O5: wtab[d] = exp(-(dbeta * (double)(4 d))), full level range
             const double dbeta = betas[s0 + i + 1] - betas[s0 + i];
-            double* t = h->h_tabs + (size_t)i * tab;
+            double* t = h_t + (size_t)i * tab;
             for (int d = 0; d <= h->N; ++d) t[d] = exp(-(dbeta * (double)(4 * d)));
         }
-        PA_CUDA(h, cudaMemcpyAsync(d_tabs, h->h_tabs, (size_t)cs * tab * 8, cudaMemcpyHostToDevice, h->stream));
+        if (cudaMemcpyAsync(d_t, h_t, (size_t)cs * tab * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = PA_ERR_CUDA; break; }
         h->dev_R = true;
-        rc = PA_OK;
         for (int i = 0; i < cs && rc == PA_OK; ++i) {
             const double beta = betas[s0 + i + 1];
-            h->wtab_cur = d_tabs + (size_t)i * tab;
-            cudaEventRecord(h->ev[2], h->stream);
+            h->wtab_cur = d_t + (size_t)i * tab;
+            if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[2], h->stream);
             if ((rc = pa_launch_weights(h, 0, h->w)) != PA_OK) break;
             if ((rc = pa_launch_plan(h, 0)) != PA_OK) break;
-            cudaEventRecord(h->ev[4], h->stream);
+            if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[4], h->stream);
             if ((rc = pa_launch_copy(h)) != PA_OK) break;
-            cudaEventRecord(h->ev[5], h->stream);
+            if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[5], h->stream);
             if ((rc = pa_launch_commit(h)) != PA_OK) break;
-            cudaEventRecord(h->ev[3], h->stream);
+            if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[3], h->stream);
             h->cur ^= 1; h->k += 1;
             const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
-            cudaEventRecord(h->ev[0], h->stream);
+            if (h->timing & PA_TIME_SWEEP) cudaEventRecord(h->ev[0], h->stream);
             if ((rc = pa_launch_sweep(h, T4, T8, theta)) != PA_OK) break;
-            cudaEventRecord(h->ev[1], h->stream);
+            if (h->timing & PA_TIME_SWEEP) cudaEventRecord(h->ev[1], h->stream);
             h->t += (uint32_t)theta;
             if ((rc = pa_launch_measure(h)) != PA_OK) break;
             if (cudaMemcpyAsync(d_snaps + (size_t)i * snap, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
         }
         h->dev_R = false; h->wtab_cur = nullptr;
-        if (rc != PA_OK) return rc;
-        PA_CUDA(h, cudaMemcpyAsync(h_snaps, d_snaps, (size_t)cs * snap, cudaMemcpyDeviceToHost, h->stream));
-        PA_CUDA(h, cudaStreamSynchronize(h->stream));
-        h->sweep_timed = theta > 0; h->resample_timed = true;
-        for (int i = 0; i < cs; ++i) {
-            const PaScalars& S = *(const PaScalars*)(h_snaps + (size_t)i * snap);
-            const double beta_old = betas[s0 + i], beta = betas[s0 + i + 1], dbeta = beta - beta_old;
-            const int64_t R_new = (int64_t)S.R_new;
-            if (S.err != 0u || R_new > h->R_cap || R_new < 1) {
-                // a step left [1, R_cap]: unlike pa_resample the later steps have already run on it -- the population is undefined
-                h->em_valid = false; h->host_scal_valid = false;
-                return PA_ERR_CAPACITY;
-            }
-            const double lnQ = -dbeta * (double)Emin_prev + log(S.W / (double)R_prev);   // Eq. 1 with the shift (O5)
-            h->lnZ += lnQ; h->lnQ_last = lnQ;                                            // Eq. 4 (L90)
-            h->R_prev = R_prev; h->W_last = S.W;
-            h->R_cur = R_new;
-            if (obs_out) pa_fill_obs(h, S, beta, R_new, h->lnZ, lnQ, &obs_out[s0 + i]);
-            Emin_prev = -2 * h->N + 4 * (int)(0xffffffffu - S.mmin_inv) + h->e0;
-            R_prev = R_new;
-            if (s0 + i == n - 1) {
-                *h->h_scal = S;
-                h->host_scal_valid = true; h->em_valid = true;
-                h->Emin = Emin_prev; h->Emax = -2 * h->N + 4 * (int)S.mmax + h->e0;
-            }
-        }
+        if (rc != PA_OK) break;
+        if (cudaMemcpyAsync(h_snaps, d_snaps, (size_t)cs * snap, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+            cudaEventRecord(h->ev_chunk[b], h->stream) != cudaSuccess) { rc = PA_ERR_CUDA; break; }
+        pend_s0[b] = s0; pend_cs[b] = cs;
+        h->sweep_timed = theta > 0 && (h->timing & PA_TIME_SWEEP); h->resample_timed = (h->timing & PA_TIME_RESAMPLE) != 0;
     }
-    return PA_OK;
+    // drain: the chunks still in flight, oldest first
+    cudaError_t se = cudaStreamSynchronize(h->stream);
+    if (rc == PA_OK && se != cudaSuccess) { pa_note_cuda_error(h, se, "pa_anneal drain", __FILE__, __LINE__); rc = PA_ERR_CUDA; }
+    for (int k = 0; k < 2 && rc == PA_OK; ++k) {
+        const int b = pend_s0[0] >= 0 && (pend_s0[1] < 0 || pend_s0[0] < pend_s0[1]) ? 0 : 1;
+        if (pend_s0[b] < 0) break;
+        const char* h_snaps = (const char*)h->h_tabs + (size_t)b * buf_bytes + (size_t)chunk_cap * tab * 8;
+        rc = pa_anneal_digest(h, cx, h_snaps, snap, pend_s0[b], pend_cs[b], n, betas, obs_out);
+        pend_s0[b] = -1;
+    }
+    if (rc != PA_OK) { h->em_valid = false; h->host_scal_valid = false; }   // PA_ERR_CAPACITY: later steps ran on it, population undefined
+    return rc;
 }
 
 int pa_hist_accumulate(pa_t* h, double beta) {
@@ -633,6 +670,12 @@ int pa_set_counters(pa_t* h, uint32_t t, uint32_t k, double lnZ) {
     return PA_OK;
 }
 int64_t pa_launch_count(const pa_t* h) { return h ? h->launches : 0; }
+
+int pa_set_timing(pa_t* h, int mask) {
+    if (!h || mask < 0 || mask > (PA_TIME_SWEEP | PA_TIME_RESAMPLE | PA_TIME_MEASURE)) return PA_ERR_INVALID_ARG;
+    h->timing = mask;
+    return PA_OK;
+}
 
 int pa_last_sweep_ms(pa_t* h, float* kernel_ms) {
     if (!h || !h->sweep_timed) return PA_ERR_INVALID_ARG;

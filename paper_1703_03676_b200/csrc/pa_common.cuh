@@ -134,8 +134,10 @@ struct pa_handle {
 
     cudaEvent_t ev[9];                  // sweep begin/end, resample begin/end, copy begin/end, plan scalars on the host, measure begin/end
     bool sweep_timed, resample_timed, measure_timed;
+    int timing;                         // PA_TIME_* mask: which phases record CUDA timing events (pa_set_timing)
     bool hist_any;                      // pa_hist_accumulate has run at least once
     bool dev_R;                         // inside pa_anneal: kernels read R and E_min from d_scal, grids cover the capacity
+    cudaEvent_t ev_chunk[2];            // pa_anneal: completion of the chunk staged in buffer 0 / 1
     double* h_tabs; size_t h_tabs_bytes; // pinned staging for pa_anneal's weight tables and snapshots
     int64_t launches;
     bool sweep_C_forced;

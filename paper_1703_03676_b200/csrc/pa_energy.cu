@@ -308,7 +308,8 @@ int pa_launch_measure(pa_handle* h) {
     const long long Rarg = h->dev_R ? -1 : h->R_cur;
     const int L = h->L;
     PA_CUDA(h, cudaMemsetAsync(h->d_scal, 0, offsetof(PaScalars, R_new), h->stream));
-    PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
+    const bool timed = (h->timing & PA_TIME_MEASURE) != 0;
+    if (timed) PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
     const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr && !h->has_j;
     if (pow2) {
 #define PA_MSR_CASE(LOG) case (8 << LOG): pa_measure_kernel<LOG><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
@@ -322,8 +323,8 @@ int pa_launch_measure(pa_handle* h) {
                                                                     h->runsum, h->partials, h->has_j ? h->jmask : nullptr);
     }
     PA_CUDA(h, cudaGetLastError());
-    PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));
-    h->measure_timed = true;
+    if (timed) PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));
+    h->measure_timed = timed;
     h->launches += 1;
     h->em_valid = true;
     h->host_scal_valid = false;

@@ -22,6 +22,7 @@ HEADER = os.path.join(os.path.dirname(HERE), "include", "pa.h")
 
 PA_OK, PA_ERR_INVALID_ARG, PA_ERR_CAPACITY, PA_ERR_CUDA, PA_ERR_WORKSPACE, PA_ERR_NOMEM = 0, -1, -2, -3, -4, -5
 PA_RNG_PHILOX, PA_RNG_LCG = 0, 1
+PA_TIME_SWEEP, PA_TIME_RESAMPLE, PA_TIME_MEASURE = 1, 2, 4
 
 
 class PaError(RuntimeError):
@@ -67,6 +68,7 @@ def lib():
         "pa_destroy": ([vp], None),
         "pa_sweep": ([vp, dbl, i32], i32),
         "pa_anneal": ([vp, i32, vp, i32, vp], i32),
+        "pa_set_timing": ([vp, i32], i32),
         "pa_set_rng_mode": ([vp, i32], i32),
         "pa_set_couplings": ([vp, vp, vp], i32),
         "pa_level_offset": ([vp], i32),
@@ -366,6 +368,10 @@ class Population:
         return {"W": W.value, "w": w, "r": r, "o": o}
 
     # timing (CUDA events recorded by the library on its stream)
+    def set_timing(self, mask):
+        """Which phases record CUDA timing events (PA_TIME_* mask; default: the sweep only)."""
+        self._check(lib().pa_set_timing(self._h, int(mask)), "pa_set_timing")
+
     def last_sweep_ms(self):
         ms = C.c_float()
         self._check(lib().pa_last_sweep_ms(self._h, C.byref(ms)), "pa_last_sweep_ms")
