@@ -39,9 +39,9 @@ N_SM = 148
 LCG_INSTR_PER_UPDATE = 5.0
 ISSUE_LANES_PER_CLK_PER_SM = 128.0
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (theta = 10) from the `ncu --set full` captures
-# summarised in profiles/r01c_summary.md (cfg2) and profiles/r01b_summary.md (cfg5); algorithmic = 2 x population bytes
+# summarised in profiles/r01e_summary.md (cfg2, cfg3) and profiles/r01b_summary.md (cfg5); algorithmic = 2 x population bytes
 # (cfg2: 20.48 MB, the write-back stays in L2; cfg5: 16.38 GB).  Workloads without a capture report null.
-SWEEP_DRAM_BYTES_PER_LAUNCH = {"cfg2_L64_R20000": 10.26e6, "cfg5_L256_R1000000": 16.41e9}
+SWEEP_DRAM_BYTES_PER_LAUNCH = {"cfg2_L64_R20000": 10.26e6, "cfg3_L64_R131072": 76.0e6, "cfg5_L256_R1000000": 16.41e9}
 
 
 def measured_peaks():
