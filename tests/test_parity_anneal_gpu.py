@@ -94,3 +94,29 @@ def test_anneal_errors():
     g.set_words(3, words[:1])
     rc = lib.pa_anneal(g._h, 1, pa._ptr(np.array([0.0, 0.01])), 0, None)
     assert rc == pa.PA_OK and abs(g.population - 100) <= 3                                # 3 replicas -> ~100 copies: within capacity
+
+
+def test_timing_mask():
+    """pa_set_timing: only the phases asked for are timed (the sweep by default); results do not depend on it."""
+    outs = []
+    for mask in (None, 0, 7):
+        g = pa.Population(16, 300, 4)
+        if mask is not None:
+            g.set_timing(mask)
+        g.resample(0.0, 0.1); g.sweep(0.1, 2); g.observables(0.1)
+        if mask in (None, 7):
+            assert g.last_sweep_ms() > 0.0
+        else:
+            with pytest.raises(pa.PaError):
+                g.last_sweep_ms()
+        if mask == 7:
+            t, c = g.last_resample_ms()
+            assert t >= c > 0.0 and g.last_measure_ms() > 0.0
+        else:
+            with pytest.raises(pa.PaError):
+                g.last_resample_ms()
+            with pytest.raises(pa.PaError):
+                g.last_measure_ms()
+        outs.append(g.get_spins().tobytes())
+    assert outs[0] == outs[1] == outs[2]
+    assert pa.lib().pa_set_timing(g._h, 8) == pa.PA_ERR_INVALID_ARG
