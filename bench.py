@@ -387,6 +387,17 @@ def run_ours(args):
                 "frac": achieved / peak, "traffic": traffic, "peak_source": f"148 SM x {per_clk:.0f}/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
                 "kernel_ms": k_ms, "kernel_updates_per_ns": k_upd / (k_ms * 1e6), "share_of_step": sum(sweep_ms) / total_ms,
                 "algorithmic_per_update": per_upd}
+    # the integer-pipe peaks behind `peak`, re-measured live by the library's microbenchmarks (dependent chains on every SM)
+    try:
+        cal = {}
+        for kind, name in ((0, "lop3"), (1, "imad_wide_u32"), (2, "philox_round_mix")):
+            gi, mhz = pa.pa_calibrate(kind)
+            cal[name + "_G_per_s"] = gi
+            cal["sm_mhz"] = mhz
+        cal["imad_wide_lanes_per_clk_per_sm"] = cal["imad_wide_u32_G_per_s"] * 1e3 / (cal["sm_mhz"] * N_SM)
+        roofline["calibration"] = cal
+    except Exception as e:                                                    # never lose the bench line over the side measurement
+        roofline["calibration"] = {"error": str(e)}
     cms = sum(copy_ms) / len(copy_ms)
     resample = {"ms_per_step": sum(res_ms) / len(res_ms), "copy_kernel_ms": cms,
                 "copy_gbs": (sum(copy_bytes) / len(copy_bytes)) / (cms * 1e6) if cms > 0 else None,

@@ -286,16 +286,18 @@ pa_calib_kernel(uint32_t* out, int iters, uint32_t seed, unsigned long long* cyc
 #pragma unroll
     for (int i = 0; i < 8; ++i) q[i] = ((unsigned long long)a[i] << 32) | (seed * 2654435761u + i);
     uint32_t k = seed ^ 0x9E3779B9u;
+    unsigned long long g0, g1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
     const long long t0 = clock64();
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int rep = 0; rep < 4; ++rep) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                if (KIND == 0) {                       // LOP3: 3-input xor chain
-                    a[i] = a[i] ^ a[(i + 1) & 7] ^ k;
-                } else if (KIND == 1) {                // IMAD.WIDE.U32 chain: p = hi(p) * M0 + p
-                    q[i] = (unsigned long long)(uint32_t)(q[i] >> 32) * PA_PHILOX_M0 + q[i];
+                if (KIND == 0) {                       // LOP3: 3-input xor chain (volatile: xor chains are linear and would be folded)
+                    asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(a[(i + 1) & 7]), "r"(k));
+                } else if (KIND == 1) {                // IMAD.WIDE.U32 chain without addend, as in Philox: p = hi(p) * M0
+                    asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(q[i]) : "r"((uint32_t)(q[i] >> 32) | 1u), "r"(PA_PHILOX_M0));
                 } else {                               // the Philox round mix: 2 IMAD.WIDE + 2 LOP3
                     uint32_t h0, l0, h1, l1;
                     pa_mulhilo(PA_PHILOX_M0, a[i], h0, l0);
@@ -307,11 +309,12 @@ pa_calib_kernel(uint32_t* out, int iters, uint32_t seed, unsigned long long* cyc
         }
     }
     const long long t1 = clock64();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
     uint32_t r = 0;
 #pragma unroll
     for (int i = 0; i < 8; ++i) r ^= a[i] ^ (uint32_t)q[i] ^ (uint32_t)(q[i] >> 32);
     out[blockIdx.x * blockDim.x + threadIdx.x] = r;
-    if (threadIdx.x == 0 && blockIdx.x == 0) *cycles = (unsigned long long)(t1 - t0);
+    if (threadIdx.x == 0 && blockIdx.x == 0) { cycles[0] = (unsigned long long)(t1 - t0); cycles[1] = g1 - g0; }   // SM cycles, ns
 }
 
 int pa_run_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz) {
@@ -319,14 +322,22 @@ int pa_run_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz) {
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return PA_ERR_CUDA;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int blocks = sms * 8, threads = 256, iters = 4096;
+    // exactly one wave: as many CTAs per SM as are resident at once, so that block 0's cycle count spans the kernel
+    const int threads = 256, iters = 4096;
+    int per_sm = 0;
+    cudaError_t oe = kind == 0 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pa_calib_kernel<0>, threads, 0)
+                   : kind == 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pa_calib_kernel<1>, threads, 0)
+                               : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pa_calib_kernel<2>, threads, 0);
+    if (oe != cudaSuccess || per_sm < 1) return PA_ERR_CUDA;
+    const int blocks = sms * per_sm;
     uint32_t* d_out = nullptr; unsigned long long* d_cyc = nullptr;
     if (cudaMalloc(&d_out, (size_t)blocks * threads * 4) != cudaSuccess) return PA_ERR_CUDA;
-    if (cudaMalloc(&d_cyc, 8) != cudaSuccess) { cudaFree(d_out); return PA_ERR_CUDA; }
+    if (cudaMalloc(&d_cyc, 16) != cudaSuccess) { cudaFree(d_out); return PA_ERR_CUDA; }
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     float best = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {
+    unsigned long long cyc[2] = {0, 1};
+    for (int rep = 0; rep < 6; ++rep) {                 // the first launches also bring the clocks up
         cudaEventRecord(e0);
         if (kind == 0) pa_calib_kernel<0><<<blocks, threads>>>(d_out, iters, 12345u + rep, d_cyc);
         else if (kind == 1) pa_calib_kernel<1><<<blocks, threads>>>(d_out, iters, 12345u + rep, d_cyc);
@@ -334,15 +345,16 @@ int pa_run_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz) {
         cudaEventRecord(e1);
         if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d_out); cudaFree(d_cyc); return PA_ERR_CUDA; }
         float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
-        if (rep > 0 && ms < best) best = ms;
+        if (rep > 1 && ms < best) {
+            best = ms;
+            cudaMemcpy(cyc, d_cyc, 16, cudaMemcpyDeviceToHost);
+        }
     }
-    unsigned long long cyc = 0;
-    cudaMemcpy(&cyc, d_cyc, 8, cudaMemcpyDeviceToHost);
     // instructions of the measured kind per thread per iteration
     const double per_iter = (kind == 2) ? 4.0 * 8.0 * 4.0 : 4.0 * 8.0;   // kind 2: 4 reps x 8 x (2 IMAD.WIDE + 2 LOP3)
     const double total = per_iter * (double)iters * (double)blocks * (double)threads;
     if (ginstr_per_ns) *ginstr_per_ns = total / ((double)best * 1e6);
-    if (sm_mhz) *sm_mhz = (double)cyc / ((double)best * 1e3);
+    if (sm_mhz) *sm_mhz = cyc[1] ? (double)cyc[0] * 1e3 / (double)cyc[1] : 0.0;   // block 0: SM cycles per ns of the global timer
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     cudaFree(d_out); cudaFree(d_cyc);
     return PA_OK;

@@ -120,3 +120,15 @@ def test_timing_mask():
         outs.append(g.get_spins().tobytes())
     assert outs[0] == outs[1] == outs[2]
     assert pa.lib().pa_set_timing(g._h, 8) == pa.PA_ERR_INVALID_ARG
+
+
+def test_pipe_calibration_matches_the_roofline_model():
+    """pa_calibrate: the integer-pipe rates bench.py's roofline rests on, re-measured -- LOP3 at 64 and
+    IMAD.WIDE.U32 at 32 thread-instructions per clock per SM, the Philox round mix (2 wide multiplies + 2 LOP3) at 64."""
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    want = {0: 64.0, 1: 32.0, 2: 64.0}
+    for kind, lanes in want.items():
+        g, mhz = pa.pa_calibrate(kind)
+        got = g * 1e3 / (mhz * sms)
+        assert 1000.0 < mhz < 2500.0
+        assert 0.9 * lanes < got < 1.03 * lanes, (kind, got, mhz)
