@@ -20,7 +20,7 @@ void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const cha
 }
 
 struct PaLayout {
-    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, lnD, A1, A2, jmask, scal, slots, stage, total;
+    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, lnD, A1, A2, jmask, jm16, scal, slots, stage, total;
     size_t stage_bytes;
     int64_t R_cap, G_cap, tiles;
 };
@@ -51,6 +51,7 @@ static PaLayout pa_layout(int L, int64_t R) {
     y.A1 = take((N + 1) * 8);
     y.A2 = take((N + 1) * 8);
     y.jmask = take(N);
+    y.jm16 = take(N / 8 * 2 + 2);
     y.scal = take(sizeof(PaScalars));
     y.slots = take((size_t)PA_SLOTS_CAP * 8);
     y.stage_bytes = (size_t)y.R_cap * N < PA_STAGE_BYTES ? pa_align_up((size_t)y.R_cap * N) : PA_STAGE_BYTES;
@@ -163,7 +164,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     h->scan_state = (unsigned long long*)(b + y.scan);
     h->Hsum = (unsigned long long*)(b + y.Hsum); h->Hcur = (uint32_t*)(b + y.Hcur); h->lnD = (double*)(b + y.lnD);
     h->A1 = (unsigned long long*)(b + y.A1); h->A2 = (unsigned long long*)(b + y.A2);
-    h->jmask = (uint8_t*)(b + y.jmask); h->has_j = false; h->e0 = 0;
+    h->jmask = (uint8_t*)(b + y.jmask); h->jm16 = (uint16_t*)(b + y.jm16); h->has_j = false; h->e0 = 0;
     h->d_scal = (PaScalars*)(b + y.scal);
     h->d_slots = (int64_t*)(b + y.slots);
     h->stage = (int8_t*)(b + y.stage); h->stage_bytes = y.stage_bytes;
@@ -256,8 +257,30 @@ int pa_set_couplings(pa_t* h, const int8_t* Jx, const int8_t* Jy) {
                 jm[c * (N / 2) + y * Lh + xh] = (uint8_t)((same ? 1 : 0) | (other ? 2 : 0) | (up ? 4 : 0) | (down ? 8 : 0) | (right ? 16 : 0));
             }
     err = cudaMemcpyAsync(h->jmask, jm, (size_t)N, cudaMemcpyHostToDevice, h->stream);
+    // the same bonds in the order of the quad-column measure kernel (L a multiple of 8): per row y and quad q of four cells
+    // xh = 4q+k: bit k = bond inside cell (x = 2xh), 4+k = bond to the next cell (x = 2xh+1), 8+k / 12+k = down bonds of the
+    // colour-0 / colour-1 site of the cell (x = 2xh + (y&1) / 2xh + ((y+1)&1))
+    uint16_t* j16 = nullptr;
+    if (err == cudaSuccess && L % 8 == 0) {
+        const int QPR = L / 8;
+        j16 = (uint16_t*)malloc((size_t)L * QPR * 2);
+        if (!j16) { free(hx); free(jm); return PA_ERR_NOMEM; }
+        for (int y = 0; y < L; ++y)
+            for (int q = 0; q < QPR; ++q) {
+                unsigned m = 0;
+                for (int k = 0; k < 4; ++k) {
+                    const int xh = 4 * q + k;
+                    if (hx[y * L + 2 * xh] < 0) m |= 1u << k;
+                    if (hx[y * L + 2 * xh + 1] < 0) m |= 1u << (4 + k);
+                    if (hy[y * L + 2 * xh + (y & 1)] < 0) m |= 1u << (8 + k);
+                    if (hy[y * L + 2 * xh + ((y + 1) & 1)] < 0) m |= 1u << (12 + k);
+                }
+                j16[y * QPR + q] = (uint16_t)m;
+            }
+        err = cudaMemcpyAsync(h->jm16, j16, (size_t)L * QPR * 2, cudaMemcpyHostToDevice, h->stream);
+    }
     if (err == cudaSuccess) err = cudaStreamSynchronize(h->stream);
-    free(hx); free(jm);
+    free(hx); free(jm); free(j16);
     if (err != cudaSuccess) { pa_note_cuda_error(h, err, "upload couplings", __FILE__, __LINE__); return PA_ERR_CUDA; }
     h->has_j = true;
     h->e0 = (int)((2 * n_af) % 4);

@@ -99,6 +99,7 @@ struct pa_handle {
     int rng_mode;            // PA_RNG_PHILOX / PA_RNG_LCG (O11)
     bool has_j;              // O15: bimodal couplings set
     int e0;                  // O15: every energy is -2N + 4m + e0, e0 = 2 (number of J = -1 bonds) mod 4
+    uint16_t* jm16;          // [N/8] O15 bond masks in the order of the quad-column measure kernel (16 bond words per row and quad)
     uint8_t* jmask;          // [N] resident order: bits 0-3 = bond to (same-cell, x, up, down) neighbour has J = -1; bit 4 = right bond
     double lnZ, lnQ_last;
     PhiloxKeys keys;

@@ -248,11 +248,13 @@ __host__ __device__ constexpr int pa_msr_threads(int L) { return (L * L / 8 >= 6
 __host__ __device__ constexpr int pa_msr_strips(int L) { return (pa_msr_threads(L) / (L / 8) < L) ? pa_msr_threads(L) / (L / 8) : L; }
 __host__ __device__ constexpr int pa_bits(int v) { return v <= 1 ? 1 : 1 + pa_bits(v >> 1); }
 
-template <int LOG_QPR>
+// HASJ (O15): jm16[y * QPR + q] carries one bit per bond word of the row (bit i <-> xb[i] below): J = -1 on that bond,
+// so the word is complemented (a negative bond is unsatisfied when its ends are parallel).
+template <int LOG_QPR, bool HASJ>
 __global__ void __launch_bounds__(64)
 pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
                   int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
-                  double* __restrict__ runsum, double* __restrict__ blocksum) {
+                  double* __restrict__ runsum, double* __restrict__ blocksum, const uint16_t* __restrict__ jm16) {
     constexpr int QPR = 1 << LOG_QPR, L = 8 * QPR, Lq = L / 8;          // Lq = uint4 per colour row
     constexpr int S = pa_msr_strips(L), RS = L / S;                      // strips per group, rows per strip
     constexpr int NPE = pa_bits(16 * RS), NPM = pa_bits(8 * RS);         // planes per thread
@@ -292,6 +294,11 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
         xb[4] = u.x ^ t.y; xb[5] = u.y ^ t.z; xb[6] = u.z ^ t.w; xb[7] = u.w ^ tn;         // bonds between pairs
         xb[8] = a.x ^ nb.x; xb[9] = a.y ^ nb.y; xb[10] = a.z ^ nb.z; xb[11] = a.w ^ nb.w;  // down bonds of colour 0
         xb[12] = b.x ^ na.x; xb[13] = b.y ^ na.y; xb[14] = b.z ^ na.z; xb[15] = b.w ^ na.w; // down bonds of colour 1
+        if (HASJ) {
+            const uint32_t j = act ? (uint32_t)__ldg(jm16 + (y & (L - 1)) * QPR + q) : 0u;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) xb[i] ^= 0u - ((j >> i) & 1u);
+        }
         const uint32_t xs[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
         cE.add16(xb);
         cM.add8(xs);
@@ -310,10 +317,14 @@ int pa_launch_measure(pa_handle* h) {
     PA_CUDA(h, cudaMemsetAsync(h->d_scal, 0, offsetof(PaScalars, R_new), h->stream));
     const bool timed = (h->timing & PA_TIME_MEASURE) != 0;
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
-    const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr && !h->has_j;
+    const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
     if (pow2) {
-#define PA_MSR_CASE(LOG) case (8 << LOG): pa_measure_kernel<LOG><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
-            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials); break;
+#define PA_MSR_CASE(LOG) case (8 << LOG): \
+        if (h->has_j) pa_measure_kernel<LOG, true><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
+            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, h->jm16); \
+        else pa_measure_kernel<LOG, false><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
+            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, nullptr); \
+        break;
         switch (L) { PA_MSR_CASE(0) PA_MSR_CASE(1) PA_MSR_CASE(2) PA_MSR_CASE(3) PA_MSR_CASE(4) PA_MSR_CASE(5) default: break; }
 #undef PA_MSR_CASE
     } else {
