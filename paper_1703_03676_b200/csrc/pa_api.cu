@@ -501,7 +501,6 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
             if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[4], h->stream);
             if ((rc = pa_launch_copy(h)) != PA_OK) break;
             if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[5], h->stream);
-            if ((rc = pa_launch_commit(h)) != PA_OK) break;
             if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[3], h->stream);
             h->cur ^= 1; h->k += 1;
             const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
@@ -509,10 +508,11 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
             if ((rc = pa_launch_sweep(h, T4, T8, theta)) != PA_OK) break;
             if (h->timing & PA_TIME_SWEEP) cudaEventRecord(h->ev[1], h->stream);
             h->t += (uint32_t)theta;
-            if ((rc = pa_launch_measure(h)) != PA_OK) break;
-            if (cudaMemcpyAsync(d_snaps + (size_t)i * snap, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToDevice, h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
+            h->snap_out = (PaScalars*)(d_snaps + (size_t)i * snap);   // the measure kernel's last CTA leaves the snapshot there
+            rc = pa_launch_measure(h);
+            h->snap_out = nullptr;
         }
-        h->dev_R = false; h->wtab_cur = nullptr;
+        h->dev_R = false; h->wtab_cur = nullptr; h->scal_zeroed = false;
         if (rc != PA_OK) break;
         if (cudaMemcpyAsync(h_snaps, d_snaps, (size_t)cs * snap, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
             cudaEventRecord(h->ev_chunk[b], h->stream) != cudaSuccess) { rc = PA_ERR_CUDA; break; }

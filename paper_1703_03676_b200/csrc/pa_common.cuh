@@ -76,7 +76,7 @@ struct PaScalars {
     double W;                    // normaliser of the last weight table, TREE1024 order (pa_tree_kernel<0>)
     double sum;                  // TREE1024 of min(1, tau_j) (pa_tree_kernel<1>)
     // --- device-resident loop (pa_anneal): the population size lives on the device between host reads
-    uint32_t R_dev;              // current population size (pa_commit_kernel)
+    uint32_t R_dev;              // current population size (copy kernel, pa_anneal)
     uint32_t err;                // 1 = a resampling step left [1, R_cap]
 };
 
@@ -137,6 +137,8 @@ struct pa_handle {
     bool sweep_timed, resample_timed, measure_timed;
     int timing;                         // PA_TIME_* mask: which phases record CUDA timing events (pa_set_timing)
     bool hist_any;                      // pa_hist_accumulate has run at least once
+    bool scal_zeroed;                   // the copy kernel has cleared the measure accumulators (pa_anneal): no memset needed
+    PaScalars* snap_out;                // pa_anneal: where the measure kernel leaves a copy of the device scalars (or NULL)
     bool dev_R;                         // inside pa_anneal: kernels read R and E_min from d_scal, grids cover the capacity
     cudaEvent_t ev_chunk[2];            // pa_anneal: completion of the chunk staged in buffer 0 / 1
     double* h_tabs; size_t h_tabs_bytes; // pinned staging for pa_anneal's weight tables and snapshots
@@ -162,8 +164,7 @@ int pa_launch_measure(pa_handle* h);                                   // E, M, 
 int pa_launch_weights(pa_handle* h, int Emin, double* w_out);          // w_j, W = TREE1024(w) -> d_scal->W
 int pa_launch_overlap(pa_handle* h, int Emin);                         // TREE1024(min(1, tau_j)) -> d_scal->sum
 int pa_launch_plan(pa_handle* h, int Emin);                            // tau, r, scan, parent map, R_new
-int pa_launch_copy(pa_handle* h);
-int pa_launch_commit(pa_handle* h);                                    // pa_anneal: R_dev <- R_new (or the error flag)                                      // new[d] = old[parent(d)], d < R_new (read on the device)
+int pa_launch_copy(pa_handle* h);                                      // new[d] = old[parent(d)], d < R_new (read on the device); pa_anneal: + commit
 int pa_launch_hist(pa_handle* h, double beta);
 int pa_launch_reweight(pa_handle* h, int n, double* d_io);              // O12, O14: d_io = [betas | lnZ | e | C | absm | m2], n each
 cudaError_t pa_run_wavg(int M, const double* d_lnZ, const double* d_A, int nobs, double* d_out, double* d_omega, cudaStream_t st);

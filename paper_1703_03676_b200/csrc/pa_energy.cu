@@ -67,7 +67,7 @@ __device__ __forceinline__ void pa_warp_add_planes(uint32_t (&p)[NPL]) {
 template <int NPL>
 __device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&pm)[NPL], long long g, int N, long long R_cur,
                                                 int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
-                                                double* __restrict__ runsum, double* __restrict__ blocksum) {
+                                                double* __restrict__ runsum, double* __restrict__ blocksum, PaScalars* __restrict__ snap) {
     const int T = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     __shared__ int sE[8][32], sM[8][32];
     __shared__ bool s_last;
@@ -144,6 +144,13 @@ __device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&
         double total = 0.0;
         for (int i = 0; i < nblk; ++i) total = __dadd_rn(total, blocksum[i]);   // ascending block index
         sc->m4sum = total;
+        if (snap) {                                                      // pa_anneal: this step's scalars, complete now
+            const unsigned long long* s8 = reinterpret_cast<const unsigned long long*>(sc);
+            unsigned long long* d8 = reinterpret_cast<unsigned long long*>(snap);
+#pragma unroll
+            for (int i = 0; i < (int)(sizeof(PaScalars) / 8); ++i) d8[i] = __ldcg(s8 + i);
+            snap->m4sum = total;
+        }
     }
 }
 
@@ -159,7 +166,8 @@ __device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&
 __global__ void __launch_bounds__(256)
 pa_measure_generic_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R_cur,
                   int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
-                  double* __restrict__ runsum, double* __restrict__ blocksum, const uint8_t* __restrict__ jmask) {
+                  double* __restrict__ runsum, double* __restrict__ blocksum, const uint8_t* __restrict__ jmask,
+                  PaScalars* __restrict__ snap) {
     const long long g = blockIdx.x;
     const uint32_t* base = pop + g * (long long)N;
     const int Lh = L >> 1, half = N >> 1;
@@ -197,7 +205,7 @@ pa_measure_generic_kernel(const uint32_t* __restrict__ pop, int L, int N, long l
     uint32_t pe[PA_EPLANES], pm[PA_EPLANES];
 #pragma unroll
     for (int k = 0; k < PA_EPLANES; ++k) { pe[k] = cE.plane(k); pm[k] = cM.plane(k); }
-    pa_measure_tail<PA_EPLANES>(pe, pm, g, N, R_cur, E, M, sc, runsum, blocksum);
+    pa_measure_tail<PA_EPLANES>(pe, pm, g, N, R_cur, E, M, sc, runsum, blocksum, snap);
 }
 
 
@@ -254,7 +262,8 @@ template <int LOG_QPR, bool HASJ>
 __global__ void __launch_bounds__(64)
 pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
                   int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
-                  double* __restrict__ runsum, double* __restrict__ blocksum, const uint16_t* __restrict__ jm16) {
+                  double* __restrict__ runsum, double* __restrict__ blocksum, const uint16_t* __restrict__ jm16,
+                  PaScalars* __restrict__ snap) {
     constexpr int QPR = 1 << LOG_QPR, L = 8 * QPR, Lq = L / 8;          // Lq = uint4 per colour row
     constexpr int S = pa_msr_strips(L), RS = L / S;                      // strips per group, rows per strip
     constexpr int NPE = pa_bits(16 * RS), NPM = pa_bits(8 * RS);         // planes per thread
@@ -307,23 +316,24 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
     uint32_t pe[NPW], pm[NPW];
 #pragma unroll
     for (int k = 0; k < NPW; ++k) { pe[k] = k < NPE ? cE.pl[k < NPE ? k : 0] : 0u; pm[k] = k < NPM ? cM.pl[k < NPM ? k : 0] : 0u; }
-    pa_measure_tail<NPW>(pe, pm, g, N, R_cur, E, M, sc, runsum, blocksum);
+    pa_measure_tail<NPW>(pe, pm, g, N, R_cur, E, M, sc, runsum, blocksum, snap);
 }
 
 int pa_launch_measure(pa_handle* h) {
     const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;      // dead groups contribute zeros (and +0.0 to the m^4 tree)
     const long long Rarg = h->dev_R ? -1 : h->R_cur;
     const int L = h->L;
-    PA_CUDA(h, cudaMemsetAsync(h->d_scal, 0, offsetof(PaScalars, R_new), h->stream));
+    if (!h->scal_zeroed) PA_CUDA(h, cudaMemsetAsync(h->d_scal, 0, offsetof(PaScalars, R_new), h->stream));
+    h->scal_zeroed = false;
     const bool timed = (h->timing & PA_TIME_MEASURE) != 0;
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
     const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
     if (pow2) {
 #define PA_MSR_CASE(LOG) case (8 << LOG): \
         if (h->has_j) pa_measure_kernel<LOG, true><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
-            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, h->jm16); \
+            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, h->jm16, h->snap_out); \
         else pa_measure_kernel<LOG, false><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
-            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, nullptr); \
+            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, nullptr, h->snap_out); \
         break;
         switch (L) { PA_MSR_CASE(0) PA_MSR_CASE(1) PA_MSR_CASE(2) PA_MSR_CASE(3) PA_MSR_CASE(4) PA_MSR_CASE(5) default: break; }
 #undef PA_MSR_CASE
@@ -331,7 +341,7 @@ int pa_launch_measure(pa_handle* h) {
         int T = 256;
         while (T > 32 && T * 8 > h->N) T >>= 1;
         pa_measure_generic_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, Rarg, h->E, h->M, h->d_scal,
-                                                                    h->runsum, h->partials, h->has_j ? h->jmask : nullptr);
+                                                                    h->runsum, h->partials, h->has_j ? h->jmask : nullptr, h->snap_out);
     }
     PA_CUDA(h, cudaGetLastError());
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));

@@ -255,7 +255,7 @@ __device__ __forceinline__ void pa_copy_chunks(const uint4* __restrict__ src4, u
 
 __global__ void __launch_bounds__(128)
 pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, const uint32_t* __restrict__ parent,
-               const PaScalars* __restrict__ sc, long long R_cap, int N) {
+               PaScalars* sc, long long R_cap, int N, int commit) {
     __shared__ PaSeg segs[32];
     __shared__ PaWin wins[32];
     __shared__ int sq[32];
@@ -265,6 +265,16 @@ pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, con
     // R_new is read on the device: the launch does not wait for the host to see it, the grid covers the
     // capacity and groups past the new population exit.  R_new > R_cap is the PA_ERR_CAPACITY case: nothing
     // of the live population is touched (dst is the spare buffer) and the host discards the copy.
+    if (commit && blockIdx.x == 0 && blockIdx.y == 0 && tid == 0) {
+        // pa_anneal: the resampled population becomes the current one on the device (the host does the same bookkeeping later
+        // from the per-step snapshots; outside [1, R_cap] the size is left alone and the error flag is raised), and the
+        // accumulators of the next measure launch are cleared here instead of by a memset of their own.  No CTA of this
+        // kernel reads R_dev or the measure block.
+        const long long Rn = sc->R_new;
+        if (Rn >= 1 && Rn <= R_cap) sc->R_dev = (uint32_t)Rn; else sc->err = 1u;
+        sc->mmin_inv = 0u; sc->mmax = 0u; sc->done_counter = 0u; sc->pad0 = 0u;
+        sc->SE = 0; sc->SE2 = 0; sc->SA = 0; sc->SM2 = 0; sc->m4sum = 0.0;
+    }
     const long long R_new = min((long long)sc->R_new, R_cap);
     if (g * 32 >= R_new) return;
     if (tid < 32) {
@@ -324,20 +334,9 @@ int pa_launch_copy(pa_handle* h) {
     // small populations: split a group's words over several CTAs to fill the GPU
     while (G * gy < 592 && gy * 128 * 2 <= chunks) gy *= 2;
     dim3 grid((unsigned)G, (unsigned)gy, 1);
-    pa_copy_kernel<<<grid, 128, 0, h->stream>>>(h->spins[h->cur], h->spins[1 - h->cur], h->parent, h->d_scal, h->R_cap, h->N);
-    PA_CUDA(h, cudaGetLastError());
-    h->launches += 1;
-    return PA_OK;
-}
-
-// pa_anneal: the resampled population becomes the current one on the device (the host does the same bookkeeping later from
-// the per-step snapshots).  Outside [1, R_cap] the size is left alone and the error flag is raised.
-__global__ void pa_commit_kernel(PaScalars* sc, long long R_cap) {
-    const long long Rn = sc->R_new;
-    if (Rn >= 1 && Rn <= R_cap) sc->R_dev = (uint32_t)Rn; else sc->err = 1u;
-}
-int pa_launch_commit(pa_handle* h) {
-    pa_commit_kernel<<<1, 1, 0, h->stream>>>(h->d_scal, h->R_cap);
+    pa_copy_kernel<<<grid, 128, 0, h->stream>>>(h->spins[h->cur], h->spins[1 - h->cur], h->parent, h->d_scal, h->R_cap, h->N,
+                                                h->dev_R ? 1 : 0);
+    h->scal_zeroed = h->dev_R;
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
