@@ -132,3 +132,23 @@ def test_pipe_calibration_matches_the_roofline_model():
         got = g * 1e3 / (mhz * sms)
         assert 1000.0 < mhz < 2500.0
         assert 0.9 * lanes < got < 1.03 * lanes, (kind, got, mhz)
+
+
+def test_two_handles_interleaved_are_independent():
+    """One handle = one population on its own stream, no global state (include/pa.h): two populations advanced in an
+    interleaved order, give the bytes of the same
+    populations advanced alone."""
+    def alone(L, R, seed, mode):
+        g = pa.Population(L, R, seed); g.set_rng_mode(mode)
+        pa_driver.run_fixed(g, [0.0, 0.2, 0.4], 2)
+        return g.get_spins().tobytes(), g.lnZ
+    want_a, want_b = alone(32, 700, 1, 0), alone(64, 300, 2, 1)
+    a, b = pa.Population(32, 700, 1), pa.Population(64, 300, 2)
+    b.set_rng_mode(1)
+    a.observables(0.0); b.observables(0.0)
+    for lo, hi in ((0.0, 0.2), (0.2, 0.4)):
+        a.resample(lo, hi); b.resample(lo, hi)
+        b.sweep(hi, 2); a.sweep(hi, 2)
+        a.observables(hi); b.observables(hi)
+    assert (a.get_spins().tobytes(), a.lnZ) == want_a
+    assert (b.get_spins().tobytes(), b.lnZ) == want_b
