@@ -150,6 +150,14 @@ def _run_fixed_schedule(cfg, checked, n_slots, last_step, rng_mode=po.RNG_PHILOX
     return og
 
 
+def test_config2_full_size_sampled():
+    """BASELINE.json configs[1] (the bench.py default): L=64, R=20000, 200 equal steps to beta=1, theta=10, seed 2.  The whole
+    schedule on the device; steps 1, 2, 3, 88 (next to beta_c), 120 and 200 are checked on 1024 sampled slots each (the first
+    steps are also compared in full by test_parity_gpu.py::test_config2_first_steps)."""
+    og = _run_fixed_schedule(2, checked={1, 2, 3, 88, 120, 200}, n_slots=1024, last_step=200)
+    assert og["beta"] == 1.0 and og["absm"] > 0.99
+
+
 def test_config3_full_size_sampled():
     """BASELINE.json configs[2]: L=64, R=131072 bit-packed, 200 equal steps to beta=1, theta=10, seed 3.
     The whole schedule runs on the device (0.7 s); steps 1, 2, 88 (beta = 0.44, next to beta_c), 150 and 200 are checked."""
