@@ -56,6 +56,34 @@ def test_anneal_equals_step_by_step_calls_and_oracle(monkeypatch, L, R, mode, th
     assert _state(a) == _state(b)
 
 
+@pytest.mark.parametrize("cfg,nsteps,mode", [(3, 12, 0), (3, 12, 1), (5, 3, 0)])
+def test_anneal_at_full_size_equals_single_calls(cfg, nsteps, mode):
+    """BASELINE.json configs[2] / configs[4] at full size (capacity-sized grids, several waves, L = 256 on clusters): the packed
+    population, energies and every observable after pa_anneal equal those of the single calls (which the sampled full-size
+    tests tie to the oracle)."""
+    wl = CONFIGS[cfg]
+    free, _ = torch.cuda.mem_get_info()
+    if free < 4.5 * wl.groups * wl.N * 4 + 2**30:
+        pytest.skip("not enough device memory for two populations")
+    betas = wl.betas()[:nsteps + 1]
+    a = pa.Population(wl.L, wl.R, wl.seed); a.set_rng_mode(mode)
+    obs_a = a.anneal(betas, wl.theta)
+    Ea, Ma = a.energies(device=True)
+    wa = torch.from_numpy(a.get_words()) if cfg != 5 else None
+    R_a, lnZ_a = a.population, a.lnZ
+    sample = a.get_spins_at(np.arange(0, R_a, max(1, R_a // 64), dtype=np.int64))
+    if cfg == 5:
+        a.close()                                                       # 16 GB each: one population at a time
+    b = pa.Population(wl.L, wl.R, wl.seed); b.set_rng_mode(mode)
+    obs_b = pa_driver.run_fixed(b, betas, wl.theta)[1:]
+    assert obs_a == obs_b and (R_a, lnZ_a) == (b.population, b.lnZ)
+    Eb, Mb = b.energies(device=True)
+    assert torch.equal(Ea, Eb) and torch.equal(Ma, Mb)
+    assert np.array_equal(sample, b.get_spins_at(np.arange(0, R_a, max(1, R_a // 64), dtype=np.int64)))
+    if wa is not None:
+        assert torch.equal(wa, torch.from_numpy(b.get_words()))
+
+
 def test_anneal_with_couplings_and_histogram_between_calls():
     L, R, theta = 16, 800, 2
     Jx, Jy = random_couplings(L, 3)
