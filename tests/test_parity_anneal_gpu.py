@@ -180,3 +180,33 @@ def test_two_handles_interleaved_are_independent():
         a.observables(hi); b.observables(hi)
     assert (a.get_spins().tobytes(), a.lnZ) == want_a
     assert (b.get_spins().tobytes(), b.lnZ) == want_b
+
+
+@pytest.mark.parametrize("L,R", [(16, 1000), (64, 777), (256, 40), (6, 33)])
+def test_workspace_guard_bands_stay_intact(L, R):
+    """compute-sanitizer is not available on the GPU pool, so out-of-bounds writes are looked for directly: the caller-owned
+    workspace (pa_create_ex) sits between two 1 MiB guard bands filled with a pattern; after a run that exercises every kernel
+    (both sweep streams, couplings, resampling with shrinking and growing populations, pa_anneal, histogram, reweighting,
+    export / import) the bands must be untouched."""
+    guard = 1 << 20
+    nbytes = pa.pa_workspace_bytes(L, R)
+    buf = torch.full((nbytes + 2 * guard,), 0xA5, dtype=torch.uint8, device="cuda")
+    h = pa.pa_create_ex(L, R, 9, buf.data_ptr() + guard, nbytes, torch.cuda.current_stream().cuda_stream)
+    g = pa.Population.__new__(pa.Population)
+    g.L, g.N, g.R_target, g.seed, g._torch, g._ws, g._h = L, L * L, R, 9, torch, buf, h
+    Jx, Jy = random_couplings(L, 1)
+    g.set_couplings(Jx, Jy)
+    g.observables(0.0); g.hist_accumulate(0.0)
+    g.resample(0.0, 0.3); g.sweep(0.3, 2); g.observables(0.3); g.hist_accumulate(0.3)
+    g.set_rng_mode(pa.PA_RNG_LCG)
+    g.anneal([0.3, 0.5, 0.9, 1.4], 2)
+    g.hist_accumulate(1.4)
+    words = g.get_words()
+    g.set_words(min(R, 5), words[:1])                                  # shrink to a handful: the next resample grows back to ~R
+    g.resample(1.4, 1.5); g.sweep(1.5, 1)
+    g.adapt_dbeta(0.8, 1.5, 3.0)
+    g.reweight(np.linspace(0.0, 1.5, 7)); g.get_spins(); g.energies()
+    g.set_timing(7); g.resample(1.5, 1.6); g.sweep(1.6, 1); g.observables(1.6)
+    torch.cuda.synchronize()
+    assert bool((buf[:guard] == 0xA5).all()) and bool((buf[guard + nbytes:] == 0xA5).all())
+    g.close()
