@@ -498,7 +498,12 @@ def oracle_step_rate(wl, R_sample, steps, warmup, rng="philox"):
 def cpu_baseline(wl, rng="philox"):
     R_s = min(wl.R, max(256, int(1.0e9 / (wl.N * wl.theta))))               # ~1e9 spin updates of CPU work
     v, ms, cores = oracle_step_rate(wl, R_s, 1, 0, rng)
-    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": ms,
+    # also one thread (the paper's CPU figure, Table 2: 22.5-23.1 ns per update = 0.044 updates/ns on one Xeon core)
+    from oracle import pa_oracle as po
+    po.set_num_threads(1)
+    v1, _, _ = oracle_step_rate(wl, max(32, R_s // 16), 1, 0, rng)
+    po.set_num_threads(cores)
+    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": ms, "value_one_thread": v1,
             "sample": f"one temperature step (resample + {wl.theta} sweeps + observables) of R={R_s} replicas, L={wl.L}, oracle/pa_oracle.cpp -O2 OpenMP"}
 
 

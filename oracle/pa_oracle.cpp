@@ -772,6 +772,15 @@ int ora_get_resample_debug(const Oracle* o, double* W, double* w, uint32_t* r, u
     return ORA_OK;
 }
 
+// thread count of the OpenMP loops over replicas (the results do not depend on it); n < 1 leaves it alone
+void ora_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int ora_num_threads(void) {
     int n = 1;
 #ifdef _OPENMP

@@ -73,6 +73,7 @@ def lib():
         L.ora_set_spins.argtypes = [vp, i64, i64, vp]; L.ora_set_spins.restype = i32
         L.ora_get_resample_debug.argtypes = [vp, vp, vp, vp, vp]; L.ora_get_resample_debug.restype = i32
         L.ora_num_threads.argtypes = []; L.ora_num_threads.restype = i32
+        L.ora_set_num_threads.argtypes = [i32]; L.ora_set_num_threads.restype = None
     return _lib
 
 
@@ -192,6 +193,10 @@ def hist_fold_of(L, E, lnZ, beta, Hsum, lnD):
     E = np.ascontiguousarray(E, dtype=np.int32)
     assert Hsum.dtype == np.int64 and lnD.dtype == np.float64 and Hsum.size == L * L + 1 == lnD.size
     _check(lib().ora_hist_fold_of(L, E.size, _p(E), float(lnZ), float(beta), _p(Hsum), _p(lnD)), "hist_fold_of")
+
+
+def set_num_threads(n):
+    lib().ora_set_num_threads(int(n))
 
 
 def num_threads():
