@@ -221,6 +221,8 @@ int pa_last_measure_ms(pa_t* h, float* kernel_ms);
  * current device and the default stream; synchronises. */
 int pa_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz);
 
+/* Text for a PA_ERR_* code (static storage); the message of the last failed CUDA call on this handle (owned by the
+ * handle, valid until the next call on it; "" if none); the library's version string (static storage). */
 const char* pa_strerror(int code);
 const char* pa_last_cuda_error(const pa_t* h);
 const char* pa_version(void);
