@@ -525,27 +525,26 @@ int pa_sweep_configure(pa_handle* h) {
     return PA_OK;
 }
 
-// Small populations: one CTA per group leaves a ragged last wave (cfg2: 625 groups on 444 CTA slots = 1.4
-// waves).  Splitting every group over a cluster of 2 or 4 CTAs makes the work items smaller.  Estimated
-// efficiency of C = (waves / ceil(waves)) x measured cluster cost (C=2: 0.97; C=4 also strands 16 of the 148
-// SMs); only applied below 4 waves, where the wave model is accurate (measured).
+// Small and medium populations: the kernel is pipe-bound, so an SM's time is proportional to the number of CTAs it works
+// through, whatever their residency: n CTAs on 148 SMs run at (n/148) / ceil(n/148) of the full-machine rate (measured, round 1:
+// cfg2 with one CTA per group 625/148 -> 4.22/5 = 0.845 against 0.835 measured; two CTAs per group 8.45/9 x 0.97 = 0.91 against
+// 0.90; L = 128, R = 50 000 with one CTA per group 10.6/11 = 0.96 against 0.977).  Splitting every group over a cluster of C CTAs
+// makes the work items smaller at a measured cluster cost (C = 2: 0.97; C = 4: 0.93, 0.85 when a thread is left with one row
+// pair; C = 8: 0.85).  The earlier "waves of resident CTAs" model mispredicted L = 128 at R = 50 000 (chose C = 4: 1 536
+// updates/ns; C = 1: 1 644).
 static int pa_sweep_pick_C(const pa_handle* h, int64_t G) {
     const int Cmin = h->sweep_C;
     if (h->sweep_C_forced || h->sweep_kind != 1) return Cmin;
     const int L = h->L;
+    const double S = 148.0;
+    if ((double)G * Cmin / S >= 24.0) return Cmin;                 // quantisation below 4 %
     double best = -1.0; int bestC = Cmin;
     for (int C = Cmin; C <= 8; C *= 2) {
         if (!pa_col_ok(L, C, h->sweep_T, h->rng_mode)) break;
-        const size_t smem = (size_t)L * L * 4 / C;
-        int per_sm = (int)((227 * 1024) / (smem + 1024));
-        const int reg_limit = h->rng_mode == PA_RNG_LCG ? 6 : 3;   // 80 (Philox) / <= 40 (LCG) registers x 256 threads
-        if (per_sm > reg_limit) per_sm = reg_limit;
-        if (per_sm < 1) per_sm = 1;
-        const double slots = (C >= 4 ? 132.0 : 148.0) * per_sm;
-        const double waves = (double)G * C / slots;
-        if (C == Cmin && waves >= 4.0) return Cmin;
-        const double cost = C == 1 ? 1.0 : C == 2 ? 0.97 : C == 4 ? 0.93 : 0.85;
-        const double eff = waves / ceil(waves) * cost;
+        const int rows_per_thread = (L / C) * (L / 2) / h->sweep_T;
+        const double per_sm = (double)G * C / S;
+        const double cost = C == 1 ? 1.0 : C == 2 ? 0.97 : C == 4 ? (rows_per_thread >= 4 ? 0.93 : 0.85) : 0.85;
+        const double eff = per_sm / ceil(per_sm) * cost * (C == Cmin ? 1.0 : 0.995);   // ties go to the smaller cluster
         if (eff > best) { best = eff; bestC = C; }
     }
     return bestC;
