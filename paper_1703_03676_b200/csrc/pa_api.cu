@@ -472,9 +472,12 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
     int pend_s0[2] = {-1, -1}, pend_cs[2] = {0, 0};
     rc = PA_OK;
     int c = 0;
-    for (int s0 = 0; s0 < n && rc == PA_OK; s0 += chunk_cap, ++c) {
+    int cs = 0;
+    for (int s0 = 0; s0 < n && rc == PA_OK; s0 += cs, ++c) {
         const int b = c & 1;
-        const int cs = n - s0 < chunk_cap ? n - s0 : chunk_cap;
+        // chunk sizes 1, 2, 4, ... up to the capacity: the device starts after one table, and the host stays ahead of it
+        cs = c < 30 && (1 << c) < chunk_cap ? (1 << c) : chunk_cap;
+        if (cs > n - s0) cs = n - s0;
         char* hb = (char*)h->h_tabs + (size_t)b * buf_bytes;
         char* db = (char*)h->stage + (size_t)b * buf_bytes;
         double *h_t = (double*)hb, *d_t = (double*)db;
