@@ -61,7 +61,9 @@ int pa_workspace_bytes(int L, int64_t R, size_t* bytes);
 /* Step 1 (L55, L65): R independent replicas with i.i.d. uniform +-1 spins (equilibrium at
  * beta_0 = 0), drawn from the INIT stream of the Philox4x32-10 generator keyed by `seed` (O1).
  * Sets ln Z = N ln 2 (L93), sweep counter t = 0, resample counter k = 0, empty histograms.
- * L even, 4 <= L <= 512; 1 <= R <= 2^31.
+ * L even, 4 <= L <= 512, and such that L/C rows of one 32-replica group (L*L*4/C bytes) fit the shared memory of a CTA for a
+ * cluster size C in {1,2,4,8} dividing L: every even L <= 338, the multiples of 4 up to 476, the multiples of 8 up to 512
+ * (other L: PA_ERR_INVALID_ARG, also from pa_workspace_bytes); 1 <= R <= 2^31.
  * pa_create allocates with cudaMalloc on the current device and uses its own stream.
  * pa_create_ex borrows `dev_ws` (device memory, >= pa_workspace_bytes, 256-byte aligned; e.g.
  * a torch tensor's data_ptr()) and enqueues on `cuda_stream` (a cudaStream_t; NULL = the
@@ -98,8 +100,8 @@ int pa_get_rng_mode(const pa_t* h);
  * the ferromagnet of Eq. 10 (the default).  The acceptance rule is unchanged with u = the number of UNSATISFIED bonds of
  * the spin (dE = 8 - 4u); energies lie on -2N + 4m + e0 with e0 = pa_level_offset = 2 (number of J = -1 bonds) mod 4,
  * which the histogram (Eq. 9) and reweighting calls use for E_m.  Must be called before the first pa_hist_accumulate
- * (PA_ERR_INVALID_ARG afterwards, or if a value is not +-1).  Sweeps and energies then run on the general kernels
- * (any even L).  Synchronous. */
+ * (PA_ERR_INVALID_ARG afterwards, or if a value is not +-1).  Sweeps and energies run on the same kernels as the
+ * ferromagnet, instantiated with one bond-mask byte per word.  Synchronous. */
 int pa_set_couplings(pa_t* h, const int8_t* Jx, const int8_t* Jy);
 int pa_level_offset(const pa_t* h);
 
@@ -145,8 +147,10 @@ int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD);
  * pa_resample / pa_sweep / pa_observables calls computes (same spins, copy numbers, ln Z, observables), but the population
  * size and E_min stay on the device and nothing inside a chunk of steps waits for the host: the launch-bound small
  * configurations run at the speed of their kernels.  The Eq. 9 histogram is not folded (call pa_hist_accumulate between
- * calls for that).  Errors: PA_ERR_INVALID_ARG as for the single calls; PA_ERR_CAPACITY if any step left [1, R_cap] -- the
- * later steps have already run on it, so the population is then undefined (destroy the handle).  Synchronises. */
+ * calls for that).  Errors: PA_ERR_INVALID_ARG as for the single calls; PA_ERR_CAPACITY if a step left [1, R_cap]: as after a
+ * failed pa_resample the population is then the one BEFORE that step (the kernels of the later steps see the device-side error
+ * flag and do nothing), the steps before it have been applied (pa_resample_counter tells how many; their obs_out entries are
+ * valid), and the handle stays usable.  Synchronises. */
 int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out);
 
 /* Multi-histogram reweighting (Sec. 2.4; O12, O14): from the sums accumulated so far, the density of
@@ -175,7 +179,7 @@ int pa_weighted_average(int M, const double* lnZ, const double* A, int nobs, dou
  * pa_set_spins overwrites replicas j0 .. j0+nrep-1 (j0 + nrep <= R_cur).
  * pa_get_words / pa_set_words move the packed population, uint32 words[ceil(R_cur/32)][N] with
  * word (g, s) holding replica 32g+b at site s = y*L + x in bit b (the interchange layout; the
- * resident layout is colour-split).  pa_set_words also sets R_cur = R
+ * resident layout is colour-split); bits of slots >= R_cur in the last group read as 0.  pa_set_words also sets R_cur = R
  * (1 <= R <= R_cap) and leaves t, k, ln Z untouched. */
 int pa_get_spins(pa_t* h, int64_t j0, int64_t nrep, int8_t* out);
 int pa_get_spins_at(pa_t* h, const int64_t* slots, int64_t n, int8_t* out);
@@ -183,9 +187,11 @@ int pa_set_spins(pa_t* h, int64_t j0, int64_t nrep, const int8_t* in);
 int pa_get_words(pa_t* h, uint32_t* words);
 int pa_set_words(pa_t* h, int64_t R, const uint32_t* words);
 
-/* Vectors of the last pa_resample, indexed by the parent slot j < R_prev (any may be NULL):
+/* Vectors of the last successful resampling step (pa_resample, or the last step of pa_anneal), indexed by the parent slot
+ * j < R_prev = pa_prev_population(h), the population size before that step (0 if none yet); any pointer may be NULL:
  * W (one double), w[R_prev] double, r[R_prev] uint32 copy numbers, o[R_prev] uint32 offsets. */
 int pa_get_resample_debug(pa_t* h, double* W, double* w, uint32_t* r, uint32_t* o);
+int64_t pa_prev_population(const pa_t* h);
 
 /* Scalars of the handle. */
 int64_t pa_population(const pa_t* h);       /* R_cur */

@@ -61,7 +61,15 @@ static PaLayout pa_layout(int L, int64_t R) {
     return y;
 }
 
-static bool pa_args_ok(int L, int64_t R) { return L >= 4 && L <= 512 && (L & 1) == 0 && R >= 1 && R <= (int64_t)1 << 31; }
+// L even, 4 <= L <= 512, and the sweep kernel's strip of L/C rows of a group (L*L*4/C bytes) must fit the shared memory of a CTA
+// for some cluster size C in {1,2,4,8} dividing L: every even L <= 338, and above that the multiples of 4 up to 476 and the
+// multiples of 8 (pa_sweep_configure picks C).
+static bool pa_args_ok(int L, int64_t R) {
+    if (!(L >= 4 && L <= 512 && (L & 1) == 0 && R >= 1 && R <= (int64_t)1 << 31)) return false;
+    for (int C = 1; C <= 8; C *= 2)
+        if (L % C == 0 && (size_t)L * L * 4 / C <= (size_t)224 * 1024) return true;
+    return false;
+}
 
 // O2: T(p) = (uint32) min(floor(p * 2^32), 2^32 - 1)
 static uint32_t pa_threshold(double p) {
@@ -324,8 +332,8 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     h->resample_timed = timed;
     const int64_t R_new = (int64_t)h->h_scal->R_new;
     const double W = h->h_scal->W;
+    if (R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;      // population, k, lnZ, R_prev unchanged (O7): only the spare buffer was written
     h->R_prev = h->R_cur; h->W_last = W;
-    if (R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;      // population, k, lnZ unchanged (O7): only the spare buffer was written
     const double lnQ = -dbeta * (double)Emin + log(W / (double)h->R_cur);   // Eq. 1 with the shift (O5)
     h->cur ^= 1;
     h->R_cur = R_new;
@@ -412,6 +420,7 @@ int pa_observables(pa_t* h, double beta, pa_obs_t* out) {
 // ------------------------------------------------------------------------------------------------
 struct PaAnnealCtx {            // host bookkeeping that runs along the snapshots, in step order
     int Emin_prev; int64_t R_prev;
+    int done;                   // steps digested without error
 };
 
 // the arithmetic of pa_resample / pa_observables on the snapshots of one finished chunk
@@ -429,6 +438,7 @@ static int pa_anneal_digest(pa_handle* h, PaAnnealCtx& cx, const char* h_snaps, 
         if (obs_out) pa_fill_obs(h, S, beta, R_new, h->lnZ, lnQ, &obs_out[s0 + i]);
         cx.Emin_prev = -2 * h->N + 4 * (int)(0xffffffffu - S.mmin_inv) + h->e0;
         cx.R_prev = R_new;
+        cx.done += 1;
         if (s0 + i == n - 1) {
             *h->h_scal = S;
             h->host_scal_valid = true; h->em_valid = true;
@@ -456,8 +466,7 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
     const size_t buf_bytes = ((size_t)chunk_cap * per_step + 255) / 256 * 256;
     const size_t need = 2 * buf_bytes + 16;
     if (h->h_tabs_bytes < need) {
-        if (h->h_tabs) cudaFreeHost(h->h_tabs);
-    for (int b = 0; b < 2; ++b) if (h->ev_chunk[b]) cudaEventDestroy(h->ev_chunk[b]);
+        if (h->h_tabs) cudaFreeHost(h->h_tabs);                      // (the chunk events live until pa_destroy)
         h->h_tabs = nullptr; h->h_tabs_bytes = 0;
         PA_CUDA(h, cudaMallocHost(&h->h_tabs, need));
         h->h_tabs_bytes = need;
@@ -468,7 +477,8 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
     uint32_t* h_init = (uint32_t*)((char*)h->h_tabs + 2 * buf_bytes);
     h_init[0] = (uint32_t)h->R_cur; h_init[1] = 0u;
     PA_CUDA(h, cudaMemcpyAsync(&h->d_scal->R_dev, h_init, 8, cudaMemcpyHostToDevice, h->stream));
-    PaAnnealCtx cx = {h->Emin, h->R_cur};
+    PaAnnealCtx cx = {h->Emin, h->R_cur, 0};
+    const int cur0 = h->cur; const uint32_t k0 = h->k, t0 = h->t;   // to put the bookkeeping back if a step fails (below)
     int pend_s0[2] = {-1, -1}, pend_cs[2] = {0, 0};
     rc = PA_OK;
     int c = 0;
@@ -532,7 +542,14 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
         rc = pa_anneal_digest(h, cx, h_snaps, snap, pend_s0[b], pend_cs[b], n, betas, obs_out);
         pend_s0[b] = -1;
     }
-    if (rc != PA_OK) { h->em_valid = false; h->host_scal_valid = false; }   // PA_ERR_CAPACITY: later steps ran on it, population undefined
+    if (rc == PA_ERR_CAPACITY) {
+        // Step f = k - k0 + 1 (1-based) left [1, R_cap].  Its copy went to the spare buffer, the device raised sc->err, and every
+        // later kernel of the call saw an empty population (pa_live_R) and exited: the population is the one before that step,
+        // exactly as after a failed pa_resample (O7).  The digest stopped there too (R_cur, ln Z, obs_out[0..f-2] are those of the
+        // steps that succeeded); the counters follow.
+        h->cur = cur0 ^ (cx.done & 1); h->k = k0 + (uint32_t)cx.done; h->t = t0 + (uint32_t)cx.done * (uint32_t)theta;
+    }
+    if (rc != PA_OK) { h->em_valid = false; h->host_scal_valid = false; }
     return rc;
 }
 
@@ -686,6 +703,7 @@ int pa_get_resample_debug(pa_t* h, double* W, double* w, uint32_t* r, uint32_t* 
 }
 
 int64_t pa_population(const pa_t* h) { return h ? h->R_cur : 0; }
+int64_t pa_prev_population(const pa_t* h) { return h ? h->R_prev : 0; }
 int64_t pa_capacity_of(const pa_t* h) { return h ? h->R_cap : 0; }
 uint32_t pa_sweep_counter(const pa_t* h) { return h ? h->t : 0; }
 uint32_t pa_resample_counter(const pa_t* h) { return h ? h->k : 0; }

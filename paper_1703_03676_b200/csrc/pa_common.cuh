@@ -84,7 +84,9 @@ struct PaScalars {
 // the device scalars: R < 0 / Emin == PA_EMIN_DEV select the device copy.
 #define PA_EMIN_DEV (-2147483647 - 1)
 #ifdef __CUDACC__
-__device__ __forceinline__ long long pa_live_R(long long R, const PaScalars* sc) { return R >= 0 ? R : (long long)sc->R_dev; }
+// Once a resampling step of pa_anneal has left [1, R_cap] (sc->err) the population counts as empty for every later kernel of the
+// call: they all exit without touching the spins or E, M, so the population stays the one before the failing step (O7).
+__device__ __forceinline__ long long pa_live_R(long long R, const PaScalars* sc) { return R >= 0 ? R : (sc->err ? 0ll : (long long)sc->R_dev); }
 __device__ __forceinline__ int pa_live_Emin(int Emin, const PaScalars* sc, int N, int e0) {
     return Emin != PA_EMIN_DEV ? Emin : -2 * N + 4 * (int)(0xffffffffu - sc->mmin_inv) + e0;
 }

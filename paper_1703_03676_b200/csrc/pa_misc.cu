@@ -221,12 +221,18 @@ __global__ void pa_pack_kernel(uint32_t* __restrict__ pop, int L, int N, long lo
     }
     pop[idx] = w;
 }
-__global__ void pa_words_out_kernel(const uint32_t* __restrict__ pop, int L, int N, long long G, uint32_t* __restrict__ out) {
+// The sweep kernels flip all 32 lanes of the last group, so the resident lanes past the population hold arbitrary bits (every
+// reader masks by j < R); the interchange words are canonical: dead lanes read as 0.
+__global__ void pa_words_out_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R, uint32_t* __restrict__ out) {
+    const long long G = (R + 31) / 32;
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= G * N) return;
     const long long g = i / N;
     const int s = (int)(i - g * N);
-    out[i] = pop[g * N + pa_index_of_site(s, L)];
+    uint32_t w = pop[g * N + pa_index_of_site(s, L)];
+    const long long live = R - g * 32;
+    if (live < 32) w &= (1u << live) - 1u;
+    out[i] = w;
 }
 __global__ void pa_words_in_kernel(uint32_t* __restrict__ pop, int L, int N, long long R, const uint32_t* __restrict__ in) {
     const long long G = (R + 31) / 32;
@@ -260,7 +266,7 @@ int pa_launch_pack(pa_handle* h, int64_t j0, int64_t n, const int8_t* d_in) {
 }
 int pa_launch_words_out(pa_handle* h, uint32_t* d_words) {
     const long long G = (h->R_cur + 31) / 32, tot = G * h->N;
-    pa_words_out_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, G, d_words);
+    pa_words_out_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, d_words);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;

@@ -90,6 +90,7 @@ def lib():
         "pa_set_words": ([vp, i64, vp], i32),
         "pa_get_resample_debug": ([vp, C.POINTER(dbl), vp, vp, vp], i32),
         "pa_population": ([vp], i64),
+        "pa_prev_population": ([vp], i64),
         "pa_capacity_of": ([vp], i64),
         "pa_sweep_counter": ([vp], u32),
         "pa_resample_counter": ([vp], u32),
@@ -361,7 +362,16 @@ class Population:
     def set_words(self, R, words):
         self._check(lib().pa_set_words(self._h, int(R), _ptr(words)), "pa_set_words")
 
-    def resample_debug(self, R_prev):
+    @property
+    def prev_population(self):
+        return int(lib().pa_prev_population(self._h))
+
+    def resample_debug(self, R_prev=None):
+        """Vectors of the last successful resampling step; their length is pa_prev_population (R_prev, if given, must equal it)."""
+        n = self.prev_population
+        if R_prev is not None and int(R_prev) != n:
+            raise PaError(PA_ERR_INVALID_ARG, "pa_get_resample_debug", f"R_prev = {R_prev}, the library's is {n}")
+        R_prev = n
         W = C.c_double()
         w = np.empty(R_prev, dtype=np.float64); r = np.empty(R_prev, dtype=np.uint32); o = np.empty(R_prev, dtype=np.uint32)
         self._check(lib().pa_get_resample_debug(self._h, C.byref(W), _ptr(w), _ptr(r), _ptr(o)), "pa_get_resample_debug")

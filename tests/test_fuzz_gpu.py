@@ -66,6 +66,12 @@ def test_random_case(i):
             with pytest.raises(pa.PaError) as e:
                 g.resample(betas[dead_at - 1], betas[dead_at])
         assert e.value.code == pa.PA_ERR_CAPACITY
+        # both APIs: the population is the one before the failing step, the steps before it have been applied (O7)
+        assert g.population == o.population and g.sweep_counter == o.sweep_counter and g.resample_counter == o.resample_counter
+        assert g.lnZ == pytest.approx(o.lnZ, rel=1e-12)
+        assert np.array_equal(g.get_spins(), o.get_spins()), i
+        Eg, Mg = g.energies(); Eo, Mo = o.energies()
+        assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
         return
     og = []
     if api == "anneal":

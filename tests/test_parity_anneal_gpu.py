@@ -106,6 +106,55 @@ def test_anneal_with_couplings_and_histogram_between_calls():
     assert np.allclose(a.histogram()[1][np.isfinite(o.histogram()[1])], o.histogram()[1][np.isfinite(o.histogram()[1])], rtol=REL)
 
 
+def test_anneal_growing_calls_on_one_handle():
+    """the pinned staging of pa_anneal is regrown when a later call needs more room than the first; the chunk
+    events must survive that.  anneal(n=1), then anneal(n=12) with 16-step chunks, then n=40, against the single calls."""
+    L, R, theta = 32, 3000, 2
+    a, b = pa.Population(L, R, 9), pa.Population(L, R, 9)
+    betas = [0.01 * i for i in range(54)]
+    obs_a = a.anneal(betas[0:2], theta) + a.anneal(betas[1:14], theta) + a.anneal(betas[13:54], theta)
+    obs_b = pa_driver.run_fixed(b, betas, theta)[1:]
+    assert obs_a == obs_b
+    assert _state(a) == _state(b)
+
+
+def test_anneal_capacity_error_keeps_the_population_before_the_failing_step(monkeypatch):
+    """O7 through pa_anneal.  A population of R = 2 can die out (R_cur = 3 with tau = 2/3 each and three failed roundings).  The
+    seeds below are ones where the ORACLE's run of 12 steps of 0.12 dies at step 10, 3, 8, 5 (found with oracle/ alone; the
+    resampling stream is the same on both sides).  After PA_ERR_CAPACITY the handle must hold exactly the state the single
+    calls reach before their failing pa_resample (spins, E, counters, ln Z), obs_out must be valid up to there, and the
+    handle must carry on."""
+    import ctypes
+    L, theta = 8, 1
+    betas = [0.12 * i for i in range(13)]
+    for chunk, seed, fail_at in (("1", 259, 10), ("16", 262, 3), ("3", 441, 8), ("16", 509, 5)):
+        monkeypatch.setenv("PA_ANNEAL_CHUNK", chunk)
+        o = po.Oracle(L, 2, seed)
+        b = pa.Population(L, 2, seed)
+        for k in range(1, fail_at):
+            o.resample(betas[k - 1], betas[k]); o.sweep(betas[k], theta)
+            b.resample(betas[k - 1], betas[k]); b.sweep(betas[k], theta)
+        with pytest.raises(Exception):
+            o.resample(betas[fail_at - 1], betas[fail_at])
+        assert b.resample_rc(betas[fail_at - 1], betas[fail_at])[0] == pa.PA_ERR_CAPACITY
+        a = pa.Population(L, 2, seed)
+        nb = np.ascontiguousarray(betas, dtype=np.float64)
+        out = (pa.pa_obs_t * (len(betas) - 1))()
+        rc = pa.lib().pa_anneal(a._h, len(betas) - 1, pa._ptr(nb), theta, ctypes.cast(out, ctypes.c_void_p))
+        assert rc == pa.PA_ERR_CAPACITY
+        assert a.resample_counter == fail_at - 1 == b.resample_counter == o.resample_counter
+        assert _state(a) == _state(b)
+        assert np.array_equal(a.get_spins(), o.get_spins())
+        assert out[fail_at - 2].as_dict() == b.observables(betas[fail_at - 1])
+        # the handle carries on: more sweeps, and the failing step again through both APIs (the same random numbers: fails again)
+        a.sweep(betas[fail_at - 1], 2); b.sweep(betas[fail_at - 1], 2)
+        assert _state(a) == _state(b)
+        assert a.resample_rc(betas[fail_at - 1], betas[fail_at - 1])[0] == pa.lib().pa_anneal(
+            b._h, 1, pa._ptr(np.array([betas[fail_at - 1]] * 2)), 0, None)
+        assert _state(a) == _state(b)
+        a.close(); b.close()
+
+
 def test_anneal_errors():
     g = pa.Population(8, 100, 2)
     lib = pa.lib()
