@@ -5,6 +5,9 @@
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle on the host cores
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
+Default workload: BASELINE.json configs[4] (cfg5: L=256, R=10^6, 8.2 GB of packed spins), the largest single-GPU
+configuration; the others are carried as compact sub-records (`other_configs`), `--config N` makes any of them the main line.
+
 A "step" is one temperature step of PAPER.md Sec. 2.1 (L56-L62) over one synthetic population:
 resample beta_{i-1} -> beta_i (energies, weights, TREE1024 normaliser, copy numbers, prefix sum,
 replica copy), theta checkerboard Metropolis sweeps at beta_i, energies + observables
@@ -38,11 +41,6 @@ WIDE_MUL_PER_CLK_PER_SM = 32.0
 N_SM = 148
 LCG_INSTR_PER_UPDATE = 5.0
 ISSUE_LANES_PER_CLK_PER_SM = 128.0
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (theta = 10) from the `ncu --set full` captures
-# summarised in profiles/r01e_summary.md (cfg2, cfg3) and profiles/r01b_summary.md (cfg5); algorithmic = 2 x population bytes
-# (cfg2: 20.48 MB, the write-back stays in L2; cfg5: 16.38 GB).  Workloads without a capture report null.
-SWEEP_DRAM_BYTES_PER_LAUNCH = {"cfg2_L64_R20000": 10.26e6, "cfg3_L64_R131072": 76.0e6, "cfg5_L256_R1000000": 16.41e9}
-
 
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
@@ -318,6 +316,162 @@ def theta_scan(args):
     print(json.dumps({"theta_scan": rows, "workload": "PAPER.md Table 3/4 shape: L=128, R=50000, 50 equal steps to beta=1", "rng": args.rng}), flush=True)
 
 
+def sweep_traffic(wl_name, rng):
+    """roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch, read from the tracked ncu export
+    profiles/traffic_<workload>_<rng>.csv (the raw page of an `ncu --set full` capture of this bench command, restricted to the
+    two counters, base units; the command is in the .md beside it).  None if this workload has no capture."""
+    import csv
+    path = os.path.join(ROOT, "profiles", f"traffic_{wl_name}_{rng}.csv")
+    if not os.path.exists(path):
+        return None, None
+    rows = list(csv.reader(open(path)))
+    hdr = rows[0]
+    try:
+        ir, iw, ik = hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum"), hdr.index("Kernel Name")
+    except ValueError:
+        return None, None
+    vals = [float(r[ir]) + float(r[iw]) for r in rows[2:] if len(r) > max(ir, iw) and "pa_sweep" in r[ik]]
+    if rows[1][ir] != "byte" or not vals:
+        return None, None
+    return sum(vals) / len(vals), os.path.relpath(path, ROOT)
+
+
+def sweep_roof(rng, sm_max):
+    """(algorithmic units per update, peak in G units/s, unit, kernel name) of the sweep kernel's binding resource (DESIGN.md 6.1 / 6.4)."""
+    if rng == "lcg":
+        return LCG_INSTR_PER_UPDATE, N_SM * ISSUE_LANES_PER_CLK_PER_SM * sm_max * 1e-3, "G thread-instructions/s", "pa_sweep_lcg_kernel"
+    return WIDE_MUL_PER_UPDATE, N_SM * WIDE_MUL_PER_CLK_PER_SM * sm_max * 1e-3, "G IMAD.WIDE.U32/s", "pa_sweep_col_kernel"
+
+
+class Runner:
+    """One population of a workload and the bookkeeping of its annealing schedule (which beta comes next)."""
+
+    def __init__(self, pa, wl, seed, rng, couplings="ferro", dims=2):
+        self.pa, self.wl, self.rng = pa, wl, rng
+        self.pop = pa.Population(wl.L, wl.R, seed)
+        if rng == "lcg":
+            self.pop.set_rng_mode(pa.PA_RNG_LCG)
+        if couplings == "pmj":
+            from paper_1703_03676_b200.workloads import random_couplings
+            self.pop.set_couplings(*random_couplings(wl.L, wl.seed))
+        self.betas = wl.betas() if wl.n_steps is not None else None
+        self.beta, self.i = wl.beta0, 0
+        self.pop.observables(self.beta)
+        if wl.multi_histogram:
+            self.pop.hist_accumulate(self.beta)
+
+    def left(self):
+        return 10**9 if self.betas is None else len(self.betas) - 1 - self.i
+
+    def step(self, fused=False):
+        """One temperature step (for the adaptive workload the bisection is part of it).  Returns the observables."""
+        self.i += 1
+        beta = next_beta(self.pop, self.wl, self.betas, self.i, self.beta)
+        obs = one_step(self.pop, self.wl, self.beta, beta, fused)
+        self.beta = beta
+        return obs
+
+    def close(self):
+        self.pop.close()
+
+
+def timed_steps(torch, run, K, Wm, flush, fused=False, sampler=None, barrier=None):
+    """W warm-up steps, then K timed steps: CUDA events on the library's stream (= torch's current stream) around every step,
+    an L2 flush between steps outside the events.  Returns the raw per-rank numbers."""
+    wl, pop = run.wl, run.pop
+    for _ in range(Wm):
+        run.step(fused)
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    if sampler:
+        sampler.start()
+    launches0 = pop.launch_count
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    updates, sweep_ms, sweep_updates, obs = 0, [], [], None
+    for s in range(K):
+        flush.zero_()                                                          # L2 flush, outside the timed events
+        ev[s][0].record()
+        obs = run.step(fused)
+        ev[s][1].record()
+        u = obs["R"] * wl.N * wl.theta
+        updates += u
+        sweep_ms.append(pop.last_sweep_ms()); sweep_updates.append(u)
+    torch.cuda.synchronize()
+    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    return {"total_ms": total_ms, "updates": updates, "sweep_ms": sweep_ms, "sweep_updates": sweep_updates, "obs": obs,
+            "launches": pop.launch_count - launches0}
+
+
+def instrumented_steps(run, n, peaks):
+    """SURVEY 8(d), resample: a few more steps with every phase event on (they cost ~3 us each, so they are off in the timed
+    region).  Copy kernel against HBM (2 x population bytes), and the whole non-sweep part of a step -- resample chain +
+    energies / observables pass -- against its floor of 3 ceil(R/32) N 4 + 24 R bytes."""
+    pa, wl, pop = run.pa, run.wl, run.pop
+    pop.set_timing(pa.PA_TIME_SWEEP | pa.PA_TIME_RESAMPLE | pa.PA_TIME_MEASURE)
+    res, cop, mea, cbytes, fbytes = [], [], [], [], []
+    for _ in range(n):
+        if run.left() < 1:
+            break
+        R_old = pop.population
+        o = run.step()
+        t, c = pop.last_resample_ms()
+        res.append(t); cop.append(c); mea.append(pop.last_measure_ms())
+        G_new, G_old = (o["R"] + 31) // 32, (R_old + 31) // 32
+        cbytes.append(2 * G_new * wl.N * 4)
+        fbytes.append((2 * G_new + G_new) * wl.N * 4 + 24 * max(R_old, o["R"]))
+    pop.set_timing(pa.PA_TIME_SWEEP)
+    if not res:
+        return None
+    m = lambda v: sum(v) / len(v)                                             # noqa: E731
+    hbm = float(peaks["hbm_gbs"])
+    cms, rm = m(cop), m(res) + m(mea)
+    return {"ms_per_step": m(res), "copy_kernel_ms": cms, "measure_kernel_ms": m(mea),
+            "copy_gbs": m(cbytes) / (cms * 1e6), "copy_frac_of_hbm": m(cbytes) / (cms * 1e6) / hbm,
+            "resample_plus_measure_ms": rm, "floor_bytes": m(fbytes), "floor_ms": m(fbytes) / (hbm * 1e6),
+            "resample_plus_measure_gbs": m(fbytes) / (rm * 1e6), "resample_plus_measure_frac_of_hbm": m(fbytes) / (rm * 1e6) / hbm,
+            "hbm_peak_gbs": hbm, "steps": len(res),
+            "what": "copy: 2 x packed population bytes / copy kernel time; resample+measure: (3 ceil(R/32) N 4 + 24 R) bytes / "
+                    "(pa_resample + energy/observable kernel) time; phase events on, after the timed region"}
+
+
+def roofline_of(rng, wl_name, sweep_ms, sweep_updates, total_ms, peaks, peak_src):
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    per_upd, peak, unit, kname = sweep_roof(rng, sm_max)
+    k_ms, k_upd = sum(sweep_ms) / len(sweep_ms), sum(sweep_updates) / len(sweep_updates)
+    achieved = per_upd * k_upd / (k_ms * 1e6)
+    traffic, tsrc = sweep_traffic(wl_name, rng)
+    per_clk = ISSUE_LANES_PER_CLK_PER_SM if rng == "lcg" else WIDE_MUL_PER_CLK_PER_SM
+    return {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
+            "traffic": traffic, "traffic_source": tsrc, "algorithmic_bytes_per_launch": None,
+            "peak_source": f"148 SM x {per_clk:.0f}/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
+            "kernel_ms": k_ms, "kernel_updates_per_ns": k_upd / (k_ms * 1e6), "share_of_step": sum(sweep_ms) / total_ms,
+            "algorithmic_per_update": per_upd}
+
+
+def sub_record(torch, pa, cfg, rng, flush, peaks, peak_src, K=5, Wm=3):
+    """A compact record of another configuration (a few steps): the small-population story and the LCG-assisted stream stay visible
+    next to the headline workload."""
+    wl = CONFIGS[cfg]
+    run = Runner(pa, wl, wl.seed, rng)
+    try:
+        t = timed_steps(torch, run, K, Wm, flush)
+        roof = roofline_of(rng, wl.name, t["sweep_ms"], t["sweep_updates"], t["total_ms"], peaks, peak_src)
+        ins = instrumented_steps(run, 3, peaks)
+        rec = {"workload": wl.name, "rng": rng, "steps": K, "warmup": Wm, "value": t["updates"] / (t["total_ms"] * 1e6),
+               "ms_per_step": t["total_ms"] / K, "gpu_launches": t["launches"],
+               "roofline": {k: roof[k] for k in ("frac", "kernel_updates_per_ns", "share_of_step", "kernel_ms", "traffic")},
+               "resample": None if ins is None else {k: ins[k] for k in ("ms_per_step", "copy_kernel_ms", "measure_kernel_ms",
+                                                                          "copy_frac_of_hbm", "resample_plus_measure_frac_of_hbm")}}
+        if wl.n_steps is not None and not wl.multi_histogram and wl.R * wl.N <= 10**9:
+            # the launch-bound configurations also through pa_anneal (one call per step: no host round trip inside a step)
+            tf = timed_steps(torch, run, K, 1, flush, fused=True)
+            rec["pa_anneal_per_step"] = {"value": tf["updates"] / (tf["total_ms"] * 1e6), "ms_per_step": tf["total_ms"] / K}
+        return rec
+    finally:
+        run.close()
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -332,128 +486,63 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     wl = CONFIGS[args.config]
     K, Wm = args.steps, args.warmup
-    pop = pa.Population(wl.L, wl.R, rank_seed(wl, rank))
-    if args.rng == "lcg":
-        pop.set_rng_mode(pa.PA_RNG_LCG)
-    if args.couplings == "pmj":
-        from paper_1703_03676_b200.workloads import random_couplings
-        pop.set_couplings(*random_couplings(wl.L, wl.seed))
-    betas = wl.betas() if wl.n_steps is not None else None
+    if wl.n_steps is not None:                                                 # never run past the end of a fixed schedule
+        K = max(1, min(K, wl.n_steps - Wm - 8))
+    run = Runner(pa, wl, rank_seed(wl, rank), args.rng, args.couplings)
+    pop = run.pop
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
     peaks, peak_src = measured_peaks()
-
     fused = args.api == "anneal" and wl.n_steps is not None and not wl.multi_histogram
-    beta_prev, i = wl.beta0, 0
-    pop.observables(beta_prev)
-    for _ in range(Wm):                                                        # warm-up steps (untimed)
-        i += 1
-        beta = next_beta(pop, wl, betas, i, beta_prev)
-        one_step(pop, wl, beta_prev, beta, fused)
-        beta_prev = beta
-    torch.cuda.synchronize()
-    if world > 1:
-        dist.barrier()
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    launches0 = pop.launch_count
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-    updates, sweep_ms, sweep_updates, res_ms, copy_ms, copy_bytes = 0, [], [], [], [], []
-    obs = None
-    for s in range(K):
-        i += 1
-        flush.zero_()                                                          # L2 flush, outside the timed events
-        beta = next_beta(pop, wl, betas, i, beta_prev) if wl.n_steps is not None else None
-        ev[s][0].record()
-        if beta is None:                                                       # adaptive: the bisection is part of the step
-            beta = next_beta(pop, wl, betas, i, beta_prev)
-        obs = one_step(pop, wl, beta_prev, beta, fused)
-        ev[s][1].record()
-        beta_prev = beta
-        R = obs["R"]
-        updates += R * wl.N * wl.theta
-        sweep_ms.append(pop.last_sweep_ms()); sweep_updates.append(R * wl.N * wl.theta)
-    torch.cuda.synchronize()
-    launches = pop.launch_count - launches0
-    total_ms = sum(a.elapsed_time(b) for a, b in ev)
+    sampler = ClockSampler(local) if rank == 0 else None
+    t = timed_steps(torch, run, K, Wm, flush, fused, sampler, dist.barrier if world > 1 else None)
     clocks = sampler.stop() if rank == 0 else None
-    # resample / copy-kernel times: a few more steps with the phase events on (they cost ~3 us each, so they are off above)
-    pop.set_timing(pa.PA_TIME_SWEEP | pa.PA_TIME_RESAMPLE)
-    for _ in range(min(K, 5)):
-        if wl.n_steps is not None and i + 1 >= len(betas):
-            break
-        i += 1
-        beta = next_beta(pop, wl, betas, i, beta_prev)
-        o = one_step(pop, wl, beta_prev, beta)
-        beta_prev = beta
-        t, c = pop.last_resample_ms()
-        res_ms.append(t); copy_ms.append(c); copy_bytes.append(2 * ((o["R"] + 31) // 32) * wl.N * 4)
-    pop.set_timing(pa.PA_TIME_SWEEP)
-    if not res_ms:
-        res_ms, copy_ms, copy_bytes = [0.0], [0.0], [0]
-    total_ms, updates_all = reduce_over_ranks(total_ms, updates, "cuda", dist if world > 1 else None)
+    obs = t["obs"]
+    resample = instrumented_steps(run, min(K, 5), peaks)
+    total_ms, updates_all = reduce_over_ranks(t["total_ms"], t["updates"], "cuda", dist if world > 1 else None)
     if world > 1:
         dist.barrier()
     value = updates_all / (total_ms * 1e6)
 
     # ---- end to end through the C ABI with HOST buffers: the population lives in pinned host memory between steps
-    e2e = None
-    if rank == 0 or world > 1:
-        Ke = max(1, min(K, args.e2e_steps))
-        G = (pop.capacity + 31) // 32
-        host_words = torch.empty((G, wl.N), dtype=torch.int32).pin_memory()
-        host_E = torch.empty(pop.capacity, dtype=torch.int32).pin_memory()
-        host_M = torch.empty(pop.capacity, dtype=torch.int32).pin_memory()
+    Ke = max(1, min(K, args.e2e_steps, run.left()))
+    G = (pop.capacity + 31) // 32
+    host_words = torch.empty((G, wl.N), dtype=torch.int32, pin_memory=True)
+    host_E = torch.empty(pop.capacity, dtype=torch.int32, pin_memory=True)
+    host_M = torch.empty(pop.capacity, dtype=torch.int32, pin_memory=True)
+    pop.get_words(host_words)
+    R_host = pop.population
+    h2d = d2h = upd_e = 0
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    for s in range(Ke):
+        nb = ((R_host + 31) // 32) * wl.N * 4
+        pop.set_words(R_host, host_words); h2d += nb
+        o = run.step()
+        pop.energies_into(host_E, host_M)
         pop.get_words(host_words)
         R_host = pop.population
-        h2d = d2h = 0
-        upd_e = 0
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-        t0 = time.perf_counter()
-        for s in range(Ke):
-            i += 1
-            beta = next_beta(pop, wl, betas, i, beta_prev)
-            nb = ((R_host + 31) // 32) * wl.N * 4
-            pop.set_words(R_host, host_words); h2d += nb
-            o = one_step(pop, wl, beta_prev, beta)
-            pop.energies_into(host_E, host_M)
-            pop.get_words(host_words)
-            R_host = pop.population
-            d2h += ((R_host + 31) // 32) * wl.N * 4 + 8 * R_host + ctypes.sizeof(pa.pa_obs_t)
-            upd_e += o["R"] * wl.N * wl.theta
-            beta_prev = beta
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        dt, upd_e = reduce_over_ranks(dt, upd_e, "cuda", dist if world > 1 else None)
-        e2e = {"value": upd_e / (dt * 1e9), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke,
-               "steps": Ke, "what": "population words pinned-host -> device, one step, energies + words + observables back to host"}
+        d2h += ((R_host + 31) // 32) * wl.N * 4 + 8 * R_host + ctypes.sizeof(pa.pa_obs_t)
+        upd_e += o["R"] * wl.N * wl.theta
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    dt, upd_e = reduce_over_ranks(dt, upd_e, "cuda", dist if world > 1 else None)
+    e2e = {"value": upd_e / (dt * 1e9), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke,
+           "steps": Ke, "what": f"{Ke} steps (capped by --e2e-steps: the packed population is {h2d // Ke / 1e9:.2f} GB each way per step): "
+                                "population words pinned-host -> device, one temperature step, energies + words + observables back to host; host wall clock"}
+    del host_words, host_E, host_M
 
     # ---- weighted average of the ranks' populations at the last temperature (Eq. 6-7): the method's own exchange step
-    combined = combine_over_ranks(pop.lnZ, pop.observables(beta_prev), "cuda", dist if world > 1 else None, pa.pa_weighted_average)
+    combined = combine_over_ranks(pop.lnZ, pop.observables(run.beta), "cuda", dist if world > 1 else None, pa.pa_weighted_average)
     if rank != 0:
+        run.close()
         if world > 1:
             dist.destroy_process_group()
         return
     # ---- roofline of the dominant kernel (the sweep), live from the library's CUDA events on its stream
-    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    k_ms = sum(sweep_ms) / len(sweep_ms)
-    k_upd = sum(sweep_updates) / len(sweep_updates)
-    if args.rng == "lcg":
-        # LCG-assisted stream: 5 thread instructions per update are the method's own (one multiply-add
-        # of the LCG, two threshold tests, two mask inserts); the binding resource is instruction issue, 4 x 32 lanes/clk/SM.
-        per_upd, per_clk, unit, kname = LCG_INSTR_PER_UPDATE, ISSUE_LANES_PER_CLK_PER_SM, "G thread-instructions/s", "pa_sweep_lcg_kernel"
-        traffic = None
-    else:
-        per_upd, per_clk, unit, kname = WIDE_MUL_PER_UPDATE, WIDE_MUL_PER_CLK_PER_SM, "G IMAD.WIDE.U32/s", "pa_sweep_col_kernel"
-        traffic = SWEEP_DRAM_BYTES_PER_LAUNCH.get(wl.name)
-    achieved = per_upd * k_upd / (k_ms * 1e6)                                  # G units / s
-    peak = N_SM * per_clk * sm_max * 1e-3                                      # G units / s at the max SM clock
-    roofline = {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": unit,
-                "frac": achieved / peak, "traffic": traffic, "peak_source": f"148 SM x {per_clk:.0f}/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
-                "kernel_ms": k_ms, "kernel_updates_per_ns": k_upd / (k_ms * 1e6), "share_of_step": sum(sweep_ms) / total_ms,
-                "algorithmic_per_update": per_upd}
+    roofline = roofline_of(args.rng, wl.name, t["sweep_ms"], t["sweep_updates"], t["total_ms"], peaks, peak_src)
+    roofline["algorithmic_bytes_per_launch"] = 2 * ((obs["R"] + 31) // 32) * wl.N * 4
     # the integer-pipe peaks behind `peak`, re-measured live by the library's microbenchmarks (dependent chains on every SM)
     try:
         cal = {}
@@ -465,11 +554,6 @@ def run_ours(args):
         roofline["calibration"] = cal
     except Exception as e:                                                    # never lose the bench line over the side measurement
         roofline["calibration"] = {"error": str(e)}
-    cms = sum(copy_ms) / len(copy_ms)
-    resample = {"ms_per_step": sum(res_ms) / len(res_ms), "copy_kernel_ms": cms,
-                "copy_gbs": (sum(copy_bytes) / len(copy_bytes)) / (cms * 1e6) if cms > 0 else None,
-                "copy_frac_of_hbm": ((sum(copy_bytes) / len(copy_bytes)) / (cms * 1e6)) / float(peaks["hbm_gbs"]) if cms > 0 else None,
-                "hbm_peak_gbs": float(peaks["hbm_gbs"]), "peak_source": peak_src}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
            "ms_per_step": total_ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "u32", "data": "synthetic",
@@ -478,10 +562,24 @@ def run_ours(args):
                       "schedule": "adaptive" if wl.n_steps is None else f"{wl.n_steps} equal steps to {wl.beta_f}",
                       "l2": "flushed between timed steps (256 MiB memset outside the CUDA events)",
                       "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
-           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "resample": resample,
+           "clocks": clocks, "e2e": e2e, "gpu_launches": t["launches"], "roofline": roofline, "resample": resample,
            "last_observables": obs, "combined_observables": combined}
     if world == 1 and args.couplings == "ferro" and (args.whole_run or (args.whole_run is None and args.config <= 4)):
         out["whole_run"] = whole_run(pa, wl, rank_seed(wl, rank), args.rng)
+    run.close()
+    del run, pop
+    torch.cuda.empty_cache()
+    if world == 1 and not args.no_others and args.couplings == "ferro":
+        # configs 1-2 are launch/latency-bound and the roofline is judged on the large ones; all stay visible here
+        others = []
+        for cfg, rng in [(c, args.rng) for c in (2, 3, 4) if c != args.config] + [(5, "lcg"), (3, "lcg")]:
+            if (cfg, rng) == (args.config, args.rng):
+                continue
+            try:
+                others.append(sub_record(torch, pa, cfg, rng, flush, peaks, peak_src))
+            except Exception as e:                                            # a side record never costs the bench line
+                others.append({"workload": CONFIGS[cfg].name, "rng": rng, "error": repr(e)})
+        out["other_configs"] = others
     out["cpu_baseline"] = cpu_baseline(wl, args.rng) if world == 1 and not args.no_cpu and args.couplings == "ferro" else None
     print(json.dumps(out), flush=True)
     if world > 1:
@@ -508,16 +606,46 @@ def oracle_step_rate(wl, R_sample, steps, warmup, rng="philox"):
     return upd / (dt * 1e9), dt / steps * 1e3, po.num_threads()
 
 
-def cpu_baseline(wl, rng="philox"):
-    R_s = min(wl.R, max(256, int(1.0e9 / (wl.N * wl.theta))))               # ~1e9 spin updates of CPU work
-    v, ms, cores = oracle_step_rate(wl, R_s, 1, 0, rng)
-    # also one thread (the paper's CPU figure, Table 2: 22.5-23.1 ns per update = 0.044 updates/ns on one Xeon core)
+def oracle_step_rates(wl, R_sample, steps, rng="philox"):
+    """updates/ns of each of `steps` consecutive temperature steps of the oracle on R_sample replicas, and the thread count."""
     from oracle import pa_oracle as po
+    o = po.Oracle(wl.L, R_sample, wl.seed)
+    if rng == "lcg":
+        o.set_rng_mode(po.RNG_LCG)
+    betas = wl.betas() if wl.n_steps is not None else [wl.beta0 + 0.002 * i for i in range(steps + 2)]
+    out = []
+    for i in range(1, steps + 1):
+        t0 = time.perf_counter()
+        o.resample(betas[i - 1], betas[i]); o.sweep(betas[i], wl.theta); ob = o.observables(betas[i])
+        out.append(ob["R"] * wl.N * wl.theta / ((time.perf_counter() - t0) * 1e9))
+    return out, po.num_threads()
+
+
+def cpu_baseline(wl, rng="philox"):
+    """The oracle as it stands on the host cores: one warm-up step (first-touch page faults, OpenMP start-up), then the median of
+    three timed steps, on the slice SURVEY 8(d) prescribes (the full population for configs 1-3, 4096 replicas for configs 4-5,
+    capped at ~3e9 spin updates per step); and on one thread (the paper's CPU figure, Table 2: 22.5-23.1 ns per update = 0.044
+    updates/ns on one Xeon core) on an eighth of that slice, one warm-up + two timed steps."""
+    from oracle import pa_oracle as po
+    R_s = min(wl.R, 4096 if wl.R * wl.N > 10**9 else wl.R, max(256, int(3.0e9 / (wl.N * wl.theta))))
+    R_1 = max(32, R_s // 8)
+
+    def rates(R, steps):
+        out, cores = [], None
+        o_steps = steps + 1
+        per = oracle_step_rates(wl, R, o_steps, rng)
+        cores = per[1]
+        out = sorted(per[0][1:])                                                # drop the warm-up step
+        return out[len(out) // 2], cores
+
+    v, cores = rates(R_s, 3)
     po.set_num_threads(1)
-    v1, _, _ = oracle_step_rate(wl, max(32, R_s // 16), 1, 0, rng)
+    v1, _ = rates(R_1, 2)
     po.set_num_threads(cores)
-    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": ms, "value_one_thread": v1,
-            "sample": f"one temperature step (resample + {wl.theta} sweeps + observables) of R={R_s} replicas, L={wl.L}, oracle/pa_oracle.cpp -O2 OpenMP"}
+    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "ms_per_step": R_s * wl.N * wl.theta / (v * 1e6),
+            "value_one_thread": v1, "timed_steps": 3, "warmup_steps": 1,
+            "sample": f"median of 3 temperature steps (resample + {wl.theta} sweeps + observables) after 1 warm-up step, R={R_s} replicas of "
+                      f"{wl.name} (L={wl.L}), oracle/pa_oracle.cpp -O2 OpenMP on {cores} threads; one thread: R={R_1}, 2 timed steps"}
 
 
 def run_reference(args):
@@ -539,11 +667,13 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, choices=sorted(CONFIGS), help="BASELINE.json configs index + 1")
-    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--config", type=int, default=5, choices=sorted(CONFIGS),
+                    help="BASELINE.json configs index + 1; default 5 = the largest single-GPU configuration (L=256, R=10^6)")
+    ap.add_argument("--e2e-steps", type=int, default=2, help="steps of the host-buffer end-to-end leg (cfg5 moves 8.2 GB each way per step)")
+    ap.add_argument("--no-others", action="store_true", help="skip the compact records of the other configurations / the LCG stream")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--whole-run", dest="whole_run", action="store_true", default=None,
                     help="also time the config's whole schedule (t_SF, Eq. 11); default: on for configs 1-4 (seconds), off for 5 (minutes)")
