@@ -15,14 +15,14 @@ def pytest_configure(config):
 
 @pytest.fixture(scope="session")
 def cfg1_oracle_runs():
-    """configs[0] of BASELINE.json (L=16, R=1000, 100 equal steps to beta=1, theta=10) on the CPU oracle, seeds 1..8, one Philox
+    """configs[0] of BASELINE.json (L=16, R=1000, 100 equal steps to beta=1, theta=10) on the CPU oracle, seeds 1..16, one Philox
     number per spin, Eq. 9 sums accumulated: computed once per session and shared by the Kaufman pins of the observables,
     of the reweighting, and by the variance-ratio pin of the LCG-assisted stream.  Returns [(oracle, observables per beta)]."""
     from oracle import pa_oracle as po
     import pa_driver
     betas = [i / 100 for i in range(101)]
     out = []
-    for seed in range(1, 9):
+    for seed in range(1, 17):
         o = po.Oracle(16, 1000, seed)
         out.append((o, pa_driver.run_fixed(o, betas, 10, hist=True)))
     return betas, out

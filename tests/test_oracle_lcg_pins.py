@@ -112,30 +112,30 @@ def _runs(L, R, betas, theta, seeds, mode):
 def test_lcg_pa_run_matches_exact_enumeration_L4():
     L, R, theta = 4, 4000, 5
     betas = [i / 40 for i in range(41)]
-    seeds = list(range(200, 212))
+    seeds = list(range(200, 216))
     runs = _runs(L, R, betas, theta, seeds, LCG)
     for i in (4, 12, 18, 24, 40):
         exact = ex.exact_small(betas[i], L)
         for key in ("e", "C", "absm", "m2", "m4", "betaF_per_N", "S_per_N"):
             vals = np.array([r[i][key] for r in runs])
             sigma = vals.std(ddof=1) / math.sqrt(len(seeds))
-            assert abs(vals.mean() - exact[key]) < 5 * sigma + 1e-12, (betas[i], key, vals.mean(), exact[key], sigma)
+            assert abs(vals.mean() - exact[key]) < 4 * sigma + 1e-12, (betas[i], key, vals.mean(), exact[key], sigma)
 
 
 def test_lcg_pa_run_matches_kaufman_and_variance_ratio_L16(cfg1_oracle_runs):
     # configs[0] of BASELINE.json (L=16, R=1000, 100 steps, theta=10) with the LCG-assisted stream: exact finite-L
     # results (Kaufman) within the seed scatter, and Table 1's last column (L201-L204): the variance of C is the
-    # same as with one Philox number per spin (ratio 1; here 10 + 8 seeds, the Philox runs are the session's shared ones)
+    # same as with one Philox number per spin (ratio 1; here 16 + 16 seeds, the Philox runs are the session's shared ones)
     L, R, theta = 16, 1000, 10
     betas, shared = cfg1_oracle_runs
-    lcg = _runs(L, R, betas, theta, list(range(21, 31)), LCG)
+    lcg = _runs(L, R, betas, theta, list(range(21, 37)), LCG)
     phi = [obs for _, obs in shared]
     for i in (10, 30, 44, 60, 100):
         k = ex.kaufman(betas[i], L)
         for key in ("e", "C", "betaF_per_N", "S_per_N"):
             vals = np.array([r[i][key] for r in lcg])
             sigma = vals.std(ddof=1) / math.sqrt(len(lcg))
-            assert abs(vals.mean() - k[key]) < 5 * sigma + 1e-9, (betas[i], key, vals.mean(), k[key], sigma)
+            assert abs(vals.mean() - k[key]) < 4 * sigma + 1e-9, (betas[i], key, vals.mean(), k[key], sigma)
     ratios = []
     for i in range(40, 101, 4):                                        # the critical and low-temperature range of Fig. 2(c)
         v1 = np.var([r[i]["C"] for r in lcg], ddof=1)

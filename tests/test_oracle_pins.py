@@ -183,6 +183,73 @@ def test_sweep_samples_boltzmann_L4(beta):
     assert abs(M.mean() / 16) < 5 / math.sqrt(n) * 1.0
 
 
+def test_sweep_stream_counter_layout_and_acceptance_rule():
+    """O1 / O3 with the counter layout written out: x(j, s, t, c) = philox(s, j>>2, 2t+c, TAG_SWEEP=1)[j&3] with key
+    (seed & 2^32-1, seed >> 32), colour 0 = (x+y) even first, flip iff u >= 2, or u = 1 and x < T4, or u = 0 and x < T8 with
+    T = floor(exp(-beta dE) 2^32) (O2).  One whole sweep of random replicas is recomputed site by site in numpy from the
+    explicit Philox counters (the Philox routine itself is pinned against cuRAND's header above): colour-0 decisions from the
+    initial state, colour-1 decisions from the updated colour-0 neighbours.  All three branches of the rule occur."""
+    L, beta, t = 6, 0.31, 12345
+    N = L * L
+    seed = (7 << 32) | 99                                              # both key words in use
+    key = [seed & 0xffffffff, seed >> 32]
+    T4 = min(math.floor(math.exp(-4 * beta) * 2.0**32), 2**32 - 1)
+    T8 = min(math.floor(math.exp(-8 * beta) * 2.0**32), 2**32 - 1)
+    assert (T4, T8) == po.thresholds(beta)
+    slots = np.array([0, 1, 2, 3, 4, 31, 32, 33, 1000003, 2**31 - 5], dtype=np.int64)
+    rng = np.random.default_rng(2)
+    init = rng.integers(0, 2, (slots.size, N), dtype=np.uint8)
+    got = po.sweep_slots(L, seed, t, beta, 1, slots, init.copy())
+    seen = set()
+    for i, j in enumerate(int(v) for v in slots):
+        sp = init[i].reshape(L, L).copy()
+        for c in (0, 1):
+            for y in range(L):
+                for x in range(L):
+                    if (x + y) & 1 != c:
+                        continue
+                    nb = [sp[y, (x - 1) % L], sp[y, (x + 1) % L], sp[(y - 1) % L, x], sp[(y + 1) % L, x]]
+                    u = sum(int(v != sp[y, x]) for v in nb)
+                    xr = int(po.philox4x32_10([y * L + x, j >> 2, 2 * t + c, 1], key)[j & 3])
+                    flip = u >= 2 or (u == 1 and xr < T4) or (u == 0 and xr < T8)
+                    seen.add((u, bool(flip)))
+                    if flip:
+                        sp[y, x] ^= 1
+        assert np.array_equal(got[i].reshape(L, L), sp), j
+    assert {(0, True), (0, False), (1, True), (1, False), (2, True)} <= seen
+    # the sweep counter advances by one per sweep: theta = 2 from t equals two calls at t and t + 1
+    two = po.sweep_slots(L, seed, t, beta, 2, slots, init.copy())
+    assert np.array_equal(two, po.sweep_slots(L, seed, t + 1, beta, 1, slots, got.copy()))
+
+
+def test_sweep_siblings_in_one_quad_and_one_word_decorrelate():
+    """Sibling replicas (copies of one parent, adjacent slots after resampling) share a Philox CALL when they sit in one quad
+    4q..4q+3 (they take different output words of it) and a machine word when they sit in 32g..32g+31.  Every spin still has
+    its own number (north_star's key tuple; Table 1's variance ratio 1, L193-L196), so identical copies must drift apart, and
+    as fast as copies placed in different quads / words (PAPER.md L206-L208 is what goes wrong otherwise)."""
+    L, beta, n = 8, 0.3, 512
+    rng = np.random.default_rng(3)
+    one = rng.integers(0, 2, (1, L * L), dtype=np.uint8)
+    quad = np.repeat(one, 4, axis=0).copy()
+    po.sweep_slots(L, 7, 0, beta, 2, np.arange(40, 44), quad)
+    assert len({r.tobytes() for r in quad}) == 4
+    word = np.repeat(one, 32, axis=0).copy()
+    po.sweep_slots(L, 7, 0, beta, 2, np.arange(64, 96), word)
+    assert len({r.tobytes() for r in word}) == 32
+    adjacent = np.repeat(one, n, axis=0).copy()
+    po.sweep_slots(L, 7, 0, beta, 2, np.arange(n), adjacent)
+    apart = np.repeat(one, n, axis=0).copy()
+    po.sweep_slots(L, 7, 0, beta, 2, np.arange(n) * 32, apart)         # every copy in a word (and quad) of its own
+    d_quad = np.array([(adjacent[i] != adjacent[i + 1]).sum() for i in range(0, n, 2)])          # pairs inside one quad
+    d_word = np.array([(adjacent[i] != adjacent[i + 5]).sum() for i in range(0, n - 8, 32)] +
+                      [(adjacent[i + 2] != adjacent[i + 27]).sum() for i in range(0, n - 32, 32)])  # same word, different quads
+    d_apart = np.array([(apart[i] != apart[i + 1]).sum() for i in range(0, n, 2)])
+    for d in (d_quad, d_word):
+        se = math.sqrt(d.var(ddof=1) / d.size + d_apart.var(ddof=1) / d_apart.size)
+        assert abs(d.mean() - d_apart.mean()) < 4 * se, (d.mean(), d_apart.mean(), se)
+    assert d_apart.mean() > 5                                          # they do move at beta = 0.3
+
+
 def test_sweep_global_flip_symmetry_and_noop():
     # acceptance depends only on u (the number of anti-parallel neighbours): inverting every
     # spin gives the inverted trajectory, the same energies and opposite magnetisations
@@ -387,14 +454,14 @@ def _seed_scatter(L, R, betas, theta, seeds, hist=False):
 def test_pa_run_matches_exact_enumeration_L4():
     L, R, theta = 4, 4000, 5
     betas = [i / 40 for i in range(41)]                               # 0 .. 1
-    seeds = list(range(100, 112))
+    seeds = list(range(100, 116))                                    # north_star: 4 sigma; >= 16 seeds
     runs, pops = _seed_scatter(L, R, betas, theta, seeds, hist=True)
     for i in (4, 12, 18, 24, 40):
         exact = ex.exact_small(betas[i], L)
         for key in ("e", "C", "absm", "m2", "m4", "betaF_per_N", "S_per_N"):
             vals = np.array([r[i][key] for r in runs])
             sigma = vals.std(ddof=1) / math.sqrt(len(seeds))
-            assert abs(vals.mean() - exact[key]) < 5 * sigma + 1e-12, (betas[i], key, vals.mean(), exact[key], sigma)
+            assert abs(vals.mean() - exact[key]) < 4 * sigma + 1e-12, (betas[i], key, vals.mean(), exact[key], sigma)
     # population size stays close to R (L69): every r_j is a Bernoulli rounding
     for r in runs:
         assert all(abs(o["R"] - R) <= 4 * math.sqrt(R) / 2 * 1.5 for o in r)
@@ -414,12 +481,12 @@ def test_pa_run_matches_exact_enumeration_L4():
                 errs.append((math.log(H[m]) - lnD[m]) - math.log(g[Em]))
     errs = np.array(errs).reshape(len(pops), -1)
     sig = errs.std(0, ddof=1) / math.sqrt(len(pops))
-    assert np.all(np.abs(errs.mean(0)) < 5 * sig + 5e-3), (errs.mean(0), sig)
+    assert np.all(np.abs(errs.mean(0)) < 4 * sig + 5e-3), (errs.mean(0), sig)
     assert np.abs(errs.mean(0)).max() < 0.05
 
 
 def test_pa_run_matches_kaufman_L16(cfg1_oracle_runs):
-    # configs[0] of BASELINE.json (L=16, R=1000, 100 steps, theta=10) over 8 seeds (runs shared with other pins: conftest.py)
+    # configs[0] of BASELINE.json (L=16, R=1000, 100 steps, theta=10) over 16 seeds, 4 sigma (runs shared with other pins: conftest.py)
     L = 16
     betas, shared = cfg1_oracle_runs
     runs = [obs for _, obs in shared]
@@ -429,10 +496,10 @@ def test_pa_run_matches_kaufman_L16(cfg1_oracle_runs):
         for key in ("e", "C", "betaF_per_N", "S_per_N"):
             vals = np.array([r[i][key] for r in runs])
             sigma = vals.std(ddof=1) / math.sqrt(len(seeds))
-            assert abs(vals.mean() - k[key]) < 5 * sigma + 1e-9, (betas[i], key, vals.mean(), k[key], sigma)
+            assert abs(vals.mean() - k[key]) < 4 * sigma + 1e-9, (betas[i], key, vals.mean(), k[key], sigma)
         # Eq. 4 (L90): sum_k ln Q_k estimates ln Z(beta) - N ln 2
         lnZ_est = np.array([-r[i]["betaF_per_N"] * L * L for r in runs])
-        assert abs(lnZ_est.mean() - k["lnZ"]) < 5 * lnZ_est.std(ddof=1) / math.sqrt(len(seeds))
+        assert abs(lnZ_est.mean() - k["lnZ"]) < 4 * lnZ_est.std(ddof=1) / math.sqrt(len(seeds))
         # magnetisation symmetry is not broken by the dynamics: <|m|> in [0,1], m2 >= absm^2
         for r in runs:
             assert 0 <= r[i]["absm"] <= 1 and r[i]["m2"] >= r[i]["absm"] ** 2 - 1e-12

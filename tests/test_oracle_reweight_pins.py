@@ -59,7 +59,7 @@ def test_reweight_from_pa_runs_matches_exact_L4():
     L, R, theta = 4, 4000, 5
     betas = [i / 40 for i in range(41)]
     grid = np.array([0.0125, 0.2375, 0.44, 0.6625, 0.9875])
-    runs = _runs(L, R, betas, theta, list(range(300, 312)))
+    runs = _runs(L, R, betas, theta, list(range(300, 316)))
     vals = {k: np.array([o.reweight(grid)[k] for o, _ in runs]) for k in ("lnZ", "e", "C")}
     for i, b in enumerate(grid):
         exact = ex.exact_small(float(b), L)
@@ -67,7 +67,7 @@ def test_reweight_from_pa_runs_matches_exact_L4():
         for k in want:
             v = vals[k][:, i]
             sigma = v.std(ddof=1) / math.sqrt(len(runs))
-            assert abs(v.mean() - want[k]) < 5 * sigma + 1e-12, (b, k, v.mean(), want[k], sigma)
+            assert abs(v.mean() - want[k]) < 4 * sigma + 1e-12, (b, k, v.mean(), want[k], sigma)
 
 
 def test_reweight_from_pa_runs_matches_kaufman_L16(cfg1_oracle_runs):
@@ -82,7 +82,7 @@ def test_reweight_from_pa_runs_matches_kaufman_L16(cfg1_oracle_runs):
         for k in ("lnZ", "e", "C"):
             v = vals[k][:, i]
             sigma = v.std(ddof=1) / math.sqrt(len(runs))
-            assert abs(v.mean() - k_ex[k]) < 5 * sigma + 1e-9, (b, k, v.mean(), k_ex[k], sigma)
+            assert abs(v.mean() - k_ex[k]) < 4 * sigma + 1e-9, (b, k, v.mean(), k_ex[k], sigma)
     # scatter of the reweighted energy at beta = 0.305 vs the scatter of the direct estimates at 0.30 and 0.31
     direct = np.array([[obs[30]["e"], obs[31]["e"]] for _, obs in runs])
     assert vals["e"][:, 1].std(ddof=1) < 1.5 * direct.std(axis=0, ddof=1).max()
@@ -119,14 +119,14 @@ def test_reweight_mag_from_pa_runs_matches_exact_L4():
     L, R, theta = 4, 4000, 5
     betas = [i / 40 for i in range(41)]
     grid = np.array([0.0125, 0.2375, 0.44, 0.6625, 0.9875])
-    runs = _runs(L, R, betas, theta, list(range(400, 412)))
+    runs = _runs(L, R, betas, theta, list(range(400, 416)))
     vals = {k: np.array([o.reweight_mag(grid)[k] for o, _ in runs]) for k in ("absm", "m2")}
     for i, b in enumerate(grid):
         exact = ex.exact_small(float(b), L)
         for k in ("absm", "m2"):
             v = vals[k][:, i]
             sigma = v.std(ddof=1) / math.sqrt(len(runs))
-            assert abs(v.mean() - exact[k]) < 5 * sigma + 1e-12, (b, k, v.mean(), exact[k], sigma)
+            assert abs(v.mean() - exact[k]) < 4 * sigma + 1e-12, (b, k, v.mean(), exact[k], sigma)
     # sum over levels of the folded sums = sum over all folded replicas (the direct observables times R N, R N^2)
     o, obs = runs[0]
     A1, A2 = o.mag_sums()
