@@ -125,6 +125,12 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new);
  * of the bracket after exactly 40 bisection steps starting from [0, beta_max - beta] (O10), so
  * that alpha(*dbeta) >= target.  Does not change the population.  Synchronises. */
 int pa_adapt_dbeta(pa_t* h, double target_overlap, double beta, double beta_max, double* dbeta);
+/* How the last pa_adapt_dbeta reached its 41 decisions (diagnostics): most are taken inside one kernel on the energy histogram,
+ * whose sum differs from the TREE1024 sum by a bounded rounding error; a decision closer to the target than four times that
+ * bound is taken by an exact evaluation (weight table, two fixed-order reductions, one host round trip) -- *exact_evaluations
+ * of them, typically 2-4 instead of 41; *filter_launches = launches of the histogram kernel.  The result is the one O10
+ * defines either way.  Environment PA_ADAPT_EXACT=1 forces all 41 exact evaluations.  Either pointer may be NULL. */
+int pa_adapt_stats(const pa_t* h, int* exact_evaluations, int* filter_launches);
 /* alpha(dbeta) of Eq. 8 for one dbeta >= 0 (the function pa_adapt_dbeta bisects on). */
 int pa_overlap(pa_t* h, double dbeta, double* alpha);
 

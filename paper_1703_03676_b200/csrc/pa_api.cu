@@ -20,7 +20,7 @@ void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const cha
 }
 
 struct PaLayout {
-    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, lnD, A1, A2, jmask, jm16, scal, slots, stage, total;
+    size_t spins0, spins1, E, M, w, r, o, parent, partials, runsum, wtab, scan, Hsum, Hcur, Hd, adapt, lnD, A1, A2, jmask, jm16, scal, slots, stage, total;
     size_t stage_bytes;
     int64_t R_cap, G_cap, tiles;
 };
@@ -47,6 +47,8 @@ static PaLayout pa_layout(int L, int64_t R) {
     y.scan = take((size_t)y.tiles * 8);
     y.Hsum = take((N + 1) * 8);
     y.Hcur = take((N + 1) * 4);
+    y.Hd = take((N + 1) * 4);
+    y.adapt = take(sizeof(PaAdaptState));
     y.lnD = take((N + 1) * 8);
     y.A1 = take((N + 1) * 8);
     y.A2 = take((N + 1) * 8);
@@ -171,6 +173,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     h->partials = (double*)(b + y.partials); h->runsum = (double*)(b + y.runsum); h->wtab = (double*)(b + y.wtab);
     h->scan_state = (unsigned long long*)(b + y.scan);
     h->Hsum = (unsigned long long*)(b + y.Hsum); h->Hcur = (uint32_t*)(b + y.Hcur); h->lnD = (double*)(b + y.lnD);
+    h->Hd = (uint32_t*)(b + y.Hd); h->d_adapt = (PaAdaptState*)(b + y.adapt);
     h->A1 = (unsigned long long*)(b + y.A1); h->A2 = (unsigned long long*)(b + y.A2);
     h->jmask = (uint8_t*)(b + y.jmask); h->jm16 = (uint16_t*)(b + y.jm16); h->has_j = false; h->e0 = 0;
     h->d_scal = (PaScalars*)(b + y.scal);
@@ -178,7 +181,8 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     h->stage = (int8_t*)(b + y.stage); h->stage_bytes = y.stage_bytes;
     // pinned host mirrors
     if (cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
-        cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->N + 1)) != cudaSuccess) { rc = PA_ERR_CUDA; }
+        cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->N + 1)) != cudaSuccess ||
+        cudaMallocHost(&h->h_adapt, sizeof(PaAdaptState)) != cudaSuccess) { rc = PA_ERR_CUDA; }
     for (int i = 0; i < 9 && rc == PA_OK; ++i)
         if (cudaEventCreateWithFlags(&h->ev[i], i == 6 ? cudaEventDisableTiming : cudaEventDefault) != cudaSuccess) rc = PA_ERR_CUDA;
     if (rc == PA_OK) rc = pa_sweep_configure(h);
@@ -207,6 +211,7 @@ void pa_destroy(pa_t* h) {
     for (int i = 0; i < 9; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
     if (h->h_wtab) cudaFreeHost(h->h_wtab);
+    if (h->h_adapt) cudaFreeHost(h->h_adapt);
     if (h->h_tabs) cudaFreeHost(h->h_tabs);
     for (int b = 0; b < 2; ++b) if (h->ev_chunk[b]) cudaEventDestroy(h->ev_chunk[b]);
     if (h->owns_stream && h->stream) cudaStreamDestroy(h->stream);
@@ -370,20 +375,66 @@ int pa_overlap(pa_t* h, double dbeta, double* alpha) {
     return pa_eval_overlap(h, dbeta, Emin, Emax, alpha);
 }
 
-int pa_adapt_dbeta(pa_t* h, double target, double beta, double beta_max, double* dbeta_out) {
-    if (!h || !dbeta_out || !(target > 0.0 && target < 1.0) || !(beta_max > beta)) return PA_ERR_INVALID_ARG;
-    int Emin, Emax, rc;
-    if ((rc = pa_overlap_prepare(h, &Emin, &Emax)) != PA_OK) return rc;
-    double hi = beta_max - beta, a;
+// O10 with every alpha evaluated exactly (41 host round trips): the definition, kept as the reference path
+// (PA_ADAPT_EXACT=1) and for populations whose energy range exceeds the filter's table.
+static int pa_adapt_exact(pa_handle* h, double target, double hi, int Emin, int Emax, double* dbeta_out) {
+    int rc; double a;
     if ((rc = pa_eval_overlap(h, hi, Emin, Emax, &a)) != PA_OK) return rc;
+    h->adapt_exact_evals = 1;
     if (a >= target) { *dbeta_out = hi; return PA_OK; }
     double lo = 0.0;
     for (int it = 0; it < 40; ++it) {                                // O10: exactly 40 bisection steps
         const double mid = 0.5 * (lo + hi);
         if ((rc = pa_eval_overlap(h, mid, Emin, Emax, &a)) != PA_OK) return rc;
+        h->adapt_exact_evals += 1;
         if (a >= target) lo = mid; else hi = mid;
     }
     *dbeta_out = lo;
+    return PA_OK;
+}
+
+int pa_adapt_dbeta(pa_t* h, double target, double beta, double beta_max, double* dbeta_out) {
+    if (!h || !dbeta_out || !(target > 0.0 && target < 1.0) || !(beta_max > beta)) return PA_ERR_INVALID_ARG;
+    int Emin, Emax, rc;
+    if ((rc = pa_overlap_prepare(h, &Emin, &Emax)) != PA_OK) return rc;
+    const double hi0 = beta_max - beta;
+    const int dmax = (Emax - Emin) / 4;
+    h->adapt_exact_evals = 0; h->adapt_filter_launches = 0;
+    const char* ex = getenv("PA_ADAPT_EXACT");
+    if ((ex && atoi(ex) != 0) || dmax + 1 > PA_ADAPT_BINS) return pa_adapt_exact(h, target, hi0, Emin, Emax, dbeta_out);
+    // The same 41 decisions, most of them taken on the energy histogram inside one kernel (pa_adapt.cu): an iteration comes back
+    // to the host only when the histogram sum is within `bound` of the target, and is then decided by the exact evaluation.
+    // |alpha_hist - alpha_TREE1024| <= (2 R_cur + 2 dmax + 32) 2^-53 to first order; bound = 4 x that.
+    const double bound = 4.0 * (2.0 * (double)h->R_cur + 2.0 * (double)dmax + 32.0) * 1.1102230246251565e-16;
+    if ((rc = pa_launch_ehist(h)) != PA_OK) return rc;
+    PaAdaptState* st = h->h_adapt;
+    st->lo = 0.0; st->hi = hi0; st->it = -1; st->status = PA_ADAPT_DONE;
+    for (;;) {
+        if ((rc = pa_run_adapt_filter(h, target, bound)) != PA_OK) return rc;
+        h->adapt_filter_launches += 1;
+        if (st->status == PA_ADAPT_RETURN_HI) { *dbeta_out = hi0; return PA_OK; }
+        if (st->status == PA_ADAPT_DONE) { *dbeta_out = st->lo; return PA_OK; }
+        double a;
+        if (st->status == PA_ADAPT_AMBIG_FIRST) {
+            if ((rc = pa_eval_overlap(h, hi0, Emin, Emax, &a)) != PA_OK) return rc;
+            h->adapt_exact_evals += 1;
+            if (a >= target) { *dbeta_out = hi0; return PA_OK; }
+            st->it = 0;
+        } else {                                                     // PA_ADAPT_AMBIG: iteration st->it of the bracket [lo, hi]
+            const double mid = 0.5 * (st->lo + st->hi);
+            if ((rc = pa_eval_overlap(h, mid, Emin, Emax, &a)) != PA_OK) return rc;
+            h->adapt_exact_evals += 1;
+            if (a >= target) st->lo = mid; else st->hi = mid;
+            st->it += 1;
+        }
+        if (st->it >= 40) { *dbeta_out = st->lo; return PA_OK; }
+    }
+}
+
+int pa_adapt_stats(const pa_t* h, int* exact_evaluations, int* filter_launches) {
+    if (!h) return PA_ERR_INVALID_ARG;
+    if (exact_evaluations) *exact_evaluations = h->adapt_exact_evals;
+    if (filter_launches) *filter_launches = h->adapt_filter_launches;
     return PA_OK;
 }
 

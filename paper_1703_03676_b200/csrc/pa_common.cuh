@@ -92,6 +92,15 @@ __device__ __forceinline__ int pa_live_Emin(int Emin, const PaScalars* sc, int N
 }
 #endif
 
+// State of the bisection of pa_adapt_dbeta between launches of pa_adapt_kernel (pa_adapt.cu)
+#define PA_ADAPT_BINS 8192          // energy levels the kernel's shared-memory table holds (wider populations: exact path)
+enum { PA_ADAPT_DONE = 0, PA_ADAPT_AMBIG = 1, PA_ADAPT_AMBIG_FIRST = 2, PA_ADAPT_RETURN_HI = 3 };
+struct PaAdaptState {
+    double lo, hi;   // bracket
+    int it;          // next bisection iteration (0..40); -1: the test alpha(hi) >= alpha* comes first
+    int status;      // PA_ADAPT_*: done / iteration `it` (or the first test) is too close to alpha* for the histogram sum
+};
+
 struct pa_handle {
     int L, N;
     int64_t R_target, R_cur, R_cap;
@@ -123,6 +132,9 @@ struct pa_handle {
     unsigned long long* scan_state;     // decoupled look-back tile states
     unsigned long long* Hsum;           // [N+1]
     uint32_t* Hcur;                     // [N+1] histogram of the current temperature
+    uint32_t* Hd;                       // [N+1] count-only histogram of the current population for pa_adapt_dbeta
+    PaAdaptState *d_adapt, *h_adapt;    // bisection state, device / pinned host
+    int adapt_exact_evals, adapt_filter_launches;   // of the last pa_adapt_dbeta (diagnostics)
     double* lnD;                        // [N+1]
     unsigned long long *A1, *A2;        // [N+1] sums of |M_j| and M_j^2 per energy level over all folded replicas (O14)
     int64_t* d_slots;                   // slot list for pa_get_spins_at
@@ -168,6 +180,8 @@ int pa_launch_overlap(pa_handle* h, int Emin);                         // TREE10
 int pa_launch_plan(pa_handle* h, int Emin);                            // tau, r, scan, parent map, R_new
 int pa_launch_copy(pa_handle* h);                                      // new[d] = old[parent(d)], d < R_new (read on the device); pa_anneal: + commit
 int pa_launch_hist(pa_handle* h, double beta);
+int pa_launch_ehist(pa_handle* h);                                     // count-only energy histogram -> Hd
+int pa_run_adapt_filter(pa_handle* h, double target, double bound);   // bisection on the histogram from *h_adapt; synchronises
 int pa_launch_reweight(pa_handle* h, int n, double* d_io);              // O12, O14: d_io = [betas | lnZ | e | C | absm | m2], n each
 cudaError_t pa_run_wavg(int M, const double* d_lnZ, const double* d_A, int nobs, double* d_out, double* d_omega, cudaStream_t st);
 int pa_launch_unpack(pa_handle* h, const int64_t* d_slots, int64_t j0, int64_t n, int8_t* d_out);

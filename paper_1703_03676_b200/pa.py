@@ -77,6 +77,7 @@ def lib():
         "pa_resample": ([vp, dbl, dbl, C.POINTER(i64)], i32),
         "pa_adapt_dbeta": ([vp, dbl, dbl, dbl, C.POINTER(dbl)], i32),
         "pa_overlap": ([vp, dbl, C.POINTER(dbl)], i32),
+        "pa_adapt_stats": ([vp, C.POINTER(i32), C.POINTER(i32)], i32),
         "pa_observables": ([vp, dbl, C.POINTER(pa_obs_t)], i32),
         "pa_hist_accumulate": ([vp, dbl], i32),
         "pa_get_histogram": ([vp, vp, vp], i32),
@@ -304,6 +305,12 @@ class Population:
         d = C.c_double()
         self._check(lib().pa_adapt_dbeta(self._h, float(target), float(beta), float(beta_max), C.byref(d)), "pa_adapt_dbeta")
         return d.value
+
+    def adapt_stats(self):
+        """(exact evaluations, histogram-kernel launches) of the last adapt_dbeta."""
+        a, b = C.c_int(), C.c_int()
+        self._check(lib().pa_adapt_stats(self._h, C.byref(a), C.byref(b)), "pa_adapt_stats")
+        return a.value, b.value
 
     def overlap(self, dbeta):
         a = C.c_double()

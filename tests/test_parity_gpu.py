@@ -277,6 +277,43 @@ def test_adaptive_run_with_multihistogram():
         assert np.array_equal(a, b)
 
 
+@pytest.mark.parametrize("L,R,seed,coupl", [(16, 2000, 4, False), (32, 50000, 5, False), (8, 3, 6, False), (64, 20000, 7, False),
+                                             (16, 5000, 8, True), (128, 4000, 9, False)])
+def test_adaptive_filter_equals_exact_path(monkeypatch, L, R, seed, coupl):
+    """O10: pa_adapt_dbeta takes most of its 41 decisions on the energy histogram inside one kernel and hands only those within
+    the rounding bound of the target to the exact evaluation (csrc/pa_adapt.cu).  Its result must equal, bit for bit, the
+    41 exact evaluations (PA_ADAPT_EXACT=1) and the oracle's, for every target, bracket and temperature tried -- including
+    brackets whose upper end already satisfies the target and targets the population cannot reach."""
+    from paper_1703_03676_b200.workloads import random_couplings
+    g, o = pa.Population(L, R, seed), po.Oracle(L, R, seed)
+    if coupl:
+        Jx, Jy = random_couplings(L, seed)
+        g.set_couplings(Jx, Jy); o.set_couplings(Jx, Jy)
+    beta = 0.0
+    total_exact = total_calls = 0
+    for step in range(6):
+        E, _ = g.energies()
+        for target, bmax in ((0.85, beta + 1.0), (0.5, beta + 1.0), (0.97, beta + 0.3), (0.3, beta + 1e-4), (0.999999, beta + 2.0), (0.05, beta + 40.0)):
+            monkeypatch.delenv("PA_ADAPT_EXACT", raising=False)
+            d_f = g.adapt_dbeta(target, beta, bmax)
+            n_exact, n_launch = g.adapt_stats()
+            monkeypatch.setenv("PA_ADAPT_EXACT", "1")
+            d_e = g.adapt_dbeta(target, beta, bmax)
+            assert g.adapt_stats()[0] in (1, 41)
+            d_o = po.adapt_dbeta_of(R, E, target, beta, bmax)
+            assert d_f == d_e == d_o, (step, target, bmax, d_f, d_e, d_o)
+            assert n_launch >= 1 and n_exact <= 12, (n_exact, n_launch)
+            total_exact += n_exact; total_calls += 1
+        monkeypatch.delenv("PA_ADAPT_EXACT", raising=False)
+        d = g.adapt_dbeta(0.85, beta, beta + 1.0)
+        assert d == o.adapt_dbeta(0.85, beta, beta + 1.0)
+        g.resample(beta, beta + d); o.resample(beta, beta + d)
+        beta += d
+        g.sweep(beta, 2); o.sweep(beta, 2)
+    assert total_exact < 6 * total_calls                              # a handful per call instead of 41
+    assert_same_state(g, o)
+
+
 def test_reweight_errors_and_device_buffers():
     L, R = 8, 300
     g, o = pa.Population(L, R, 3), po.Oracle(L, R, 3)
