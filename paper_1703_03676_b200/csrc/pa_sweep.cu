@@ -294,9 +294,10 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 // word, 8 % of the kernel) disappears.  The ALU pipe is the binding one.
 // Requirements (checked by pa_sweep_configure): Lh = 2^LOG_LH >= 32, T >= Lh, H*Lh/T even and >= 2, H even.
 // ------------------------------------------------------------------------------------------------
-#ifndef PA_SWEEP_BOUNDS
-#define PA_SWEEP_BOUNDS __launch_bounds__(256)
-#endif
+// Block size: 256 threads, and 512 for L = 256 (LOG_LH = 7), where a cluster of TWO CTAs with 128 KB strips and one CTA of 16
+// warps per SM beats four CTAs with 64 KB strips (clusters of 4 cannot be placed on 16 of the 148 SMs; measured in
+// profiles/r02_sweep_L256.md: 1 586 -> 1 679 updates/ns at cfg5).
+#define PA_SWEEP_BOUNDS __launch_bounds__(LOG_LH == 7 ? 512 : 256)
 template <int CMP, int LOG_LH, bool CLUSTER, bool HASJ>
 __global__ void PA_SWEEP_BOUNDS
 pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
@@ -500,7 +501,9 @@ static bool pa_col_ok(int L, int C, int T, int rng_mode = PA_RNG_PHILOX) {
 
 int pa_sweep_configure(pa_handle* h) {
     const int L = h->L;
-    const size_t budget = (size_t)pa_env_int("PA_SWEEP_SMEM_KB", 64) * 1024;
+    // strips of up to 64 KB (three CTAs of 256 threads per SM); L = 256: 128 KB strips, clusters of two, one CTA of 512 threads per SM
+    const bool big = L == 256;
+    const size_t budget = (size_t)pa_env_int("PA_SWEEP_SMEM_KB", big ? 128 : 64) * 1024;
     int C = 1;
     while (C <= 8 && (((L % C) != 0) || (size_t)L * L * 4 / C > budget)) C *= 2;
     if (C > 8) {                                   // L = 512: no strip fits the preferred budget; take the largest that fits an SM
@@ -512,13 +515,14 @@ int pa_sweep_configure(pa_handle* h) {
     if (forceC > 0 && L % forceC == 0) { C = forceC; h->sweep_C_forced = true; }
     if (C > 8 || (size_t)L * L * 4 / C > 224 * 1024) return PA_ERR_INVALID_ARG;
     int half = (L / C) * (L / 2);
-    int T = 256;
+    int T = big ? 512 : 256;
     while (T > 32 && T > half) T >>= 1;
     int forceT = pa_env_int("PA_SWEEP_T", 0);
-    if (forceT >= 32 && forceT <= 256) T = forceT;
+    if (forceT >= 32 && forceT <= (big ? 512 : 256)) T = forceT;
     int kind = pa_col_ok(L, C, T) ? 1 : 0;
     kind = pa_env_int("PA_SWEEP_KIND", kind);
     if (kind == 1 && !pa_col_ok(L, C, T)) kind = 0;
+    if (kind == 0 && T > 256) T = 256;                       // the generic kernel is compiled for blocks of up to 256 threads
     h->sweep_C = C; h->sweep_T = T; h->sweep_kind = kind;
     h->sweep_cmp = pa_env_int("PA_SWEEP_CMP", 1);
     if (h->sweep_cmp < 0 || h->sweep_cmp > 2) h->sweep_cmp = 1;
