@@ -1,4 +1,4 @@
-"""Exact results for the 2D Ising model on the L x L torus.  TEST INFRASTRUCTURE (pins).
+"""Exact results for the 2D Ising model on the L x L torus (and brute force on small 3D boxes).  TEST INFRASTRUCTURE (pins).
 
 PAPER.md L137: "a wealth of exact or extremely accurate results are available for it as
 reference points".  Two independent references:
@@ -97,6 +97,46 @@ def exact_small(beta, L=4):
         "S_per_N": beta * e1 / N + lnZ / N,
         "pE": {int(v): float(p[E == v].sum()) for v in np.unique(E)},
     }
+
+
+@lru_cache(maxsize=None)
+def enumerate_box(dims):
+    """All 2^N states of the periodic simple-cubic box dims = (Lx, Ly, Lz), N = Lx Ly Lz <= 20 (O16; PAPER.md L313,
+    L43): (E, M) indexed by the bit pattern, bit s = spin at site s = (z*Ly + y)*Lx + x.  H = -sum_s s_s (s_{x+1} + s_{y+1} +
+    s_{z+1}) with periodic neighbours: numpy.roll along an axis of length 2 returns the one other site for both directions, so
+    that bond is counted once from each of its two sites (the "double bond" of a period-2 direction)."""
+    Lx, Ly, Lz = dims
+    N = Lx * Ly * Lz
+    assert N <= 20
+    states = np.arange(1 << N, dtype=np.int64)
+    spins = ((states[:, None] >> np.arange(N)[None, :]) & 1).astype(np.int8) * 2 - 1
+    g = spins.reshape(-1, Lz, Ly, Lx).astype(np.int64)
+    E = -(g * (np.roll(g, -1, axis=3) + np.roll(g, -1, axis=2) + np.roll(g, -1, axis=1))).sum(axis=(1, 2, 3))
+    M = g.sum(axis=(1, 2, 3))
+    return E.astype(np.int64), M.astype(np.int64)
+
+
+@lru_cache(maxsize=None)
+def density_of_states_box(dims):
+    E, _ = enumerate_box(dims)
+    vals, cnt = np.unique(E, return_counts=True)
+    return {int(v): int(c) for v, c in zip(vals, cnt)}
+
+
+def exact_box(beta, dims):
+    """Exact canonical averages (Eq. 3-5) on the periodic box by enumeration."""
+    N = dims[0] * dims[1] * dims[2]
+    E, M = enumerate_box(tuple(dims))
+    Emin = E.min()
+    w = np.exp(-beta * (E - Emin).astype(np.float64))
+    Z = w.sum()
+    p = w / Z
+    e1 = (p * E).sum(); e2 = (p * E.astype(np.float64) ** 2).sum()
+    m = M.astype(np.float64) / N
+    lnZ = math.log(Z) - beta * Emin
+    return {"e": e1 / N, "C": beta * beta * (e2 - e1 * e1) / N, "absm": (p * np.abs(m)).sum(), "m2": (p * m ** 2).sum(),
+            "m4": (p * m ** 4).sum(), "lnZ": lnZ, "betaF_per_N": -lnZ / N, "S_per_N": beta * e1 / N + lnZ / N,
+            "pE": {int(v): float(p[E == v].sum()) for v in np.unique(E)}}
 
 
 # ---------------------------------------------------------------------------------------------

@@ -1,4 +1,4 @@
-// pa_oracle.cpp -- CPU ORACLE for the population-annealing (PA) hot path of the 2D Ising model.
+// pa_oracle.cpp -- CPU ORACLE for the population-annealing (PA) hot path of the 2D Ising model (and, O16, the simple-cubic one).
 //
 // THIS FILE IS TEST INFRASTRUCTURE.  It is the plain, slow, step-by-step statement of what the
 // method computes, written from the paper (/root/reference/PAPER.md, cited below as "L<line>")
@@ -37,6 +37,9 @@
 //                          paper prints (L236); the same L=4 Boltzmann chi^2, global-flip symmetry
 //                          and Kaufman pins as the Philox-per-spin sweep; variance ratio of C
 //                          against the Philox-per-spin mode (Table 1, last column = 1)
+//   simple-cubic box (O16) numpy.roll energies on boxes with three different edges and closed-form states; one sweep restated
+//                          in numpy from explicit Philox counters on a 6x4x2 box; brute-force enumeration of the 4x2x2 box
+//                          (Boltzmann chi^2, whole PA runs for every observable, ln Q sums, ln Omega) -- tests/test_oracle_cubic_pins.py
 //   whole method vs the paper's own figures: "parity unpinned" (Figs. 2-3 data and the authors'
 //   code are not available); pinned instead by the exact Ising results above.
 
@@ -187,6 +190,52 @@ void energy_one_replica(const uint8_t* sp, int L, int32_t* E, int32_t* M, const 
     *E = e; *M = m;
 }
 
+// ---------------------------------------------------------------------------------------------
+// O16  Simple-cubic lattice (L313 "models on different lattices in various dimensions", L43 "3D Ising systems"; the paper
+// gives no detail beyond "straightforward").  Reading (O16): a periodic box Lx x Ly x Lz, every edge even (so that
+// the two-colour checkerboard (x+y+z)&1 survives the wrap), site s = (z*Ly + y)*Lx + x.  A spin has six neighbour SLOTS
+// x+-1, y+-1, z+-1 (mod the edge); along an edge of length 2 both slots hold the same site, which then counts twice (the
+// usual periodic "double bond").  u = number of anti-parallel slots, dE = 2 sigma sum_slots sigma' = 12 - 4u; Metropolis (L73):
+// flip iff u >= 3, or u = 2 and x < T4, or u = 1 and x < T8, or u = 0 and x < T12, T(dE) = threshold(exp(-beta dE)) (O2);
+// colour 0 first, the random number of (slot, s, t, c) is the SWEEP stream's x_sweep with this s (O1).
+// Energy: every site owns its +x, +y, +z bond: E = -sum_s sigma_s (sigma_{x+1} + sigma_{y+1} + sigma_{z+1}), 3N bonds (a double
+// bond is owned by both of its sites), so E = -3N + 4m with m = 0 .. 3N/2.
+// ---------------------------------------------------------------------------------------------
+void sweep_one_replica_3d(uint8_t* sp, int Lx, int Ly, int Lz, uint64_t seed, int64_t slot, uint32_t t,
+                          uint32_t T4, uint32_t T8, uint32_t T12) {
+    for (uint32_t c = 0; c < 2; ++c)
+        for (int z = 0; z < Lz; ++z)
+            for (int y = 0; y < Ly; ++y)
+                for (int x = 0; x < Lx; ++x) {
+                    if ((uint32_t)((x + y + z) & 1) != c) continue;
+                    int s = (z * Ly + y) * Lx + x;
+                    int xm = x == 0 ? Lx - 1 : x - 1, xp = x == Lx - 1 ? 0 : x + 1;
+                    int ym = y == 0 ? Ly - 1 : y - 1, yp = y == Ly - 1 ? 0 : y + 1;
+                    int zm = z == 0 ? Lz - 1 : z - 1, zp = z == Lz - 1 ? 0 : z + 1;
+                    int u = (sp[(z * Ly + y) * Lx + xm] != sp[s]) + (sp[(z * Ly + y) * Lx + xp] != sp[s]) +
+                            (sp[(z * Ly + ym) * Lx + x] != sp[s]) + (sp[(z * Ly + yp) * Lx + x] != sp[s]) +
+                            (sp[(zm * Ly + y) * Lx + x] != sp[s]) + (sp[(zp * Ly + y) * Lx + x] != sp[s]);
+                    uint32_t xr = x_sweep(seed, slot, (uint32_t)s, t, c);      // drawn for every (j,s,t)
+                    bool flip = (u >= 3) || (u == 2 && xr < T4) || (u == 1 && xr < T8) || (u == 0 && xr < T12);
+                    if (flip) sp[s] ^= 1u;
+                }
+}
+
+void energy_one_replica_3d(const uint8_t* sp, int Lx, int Ly, int Lz, int32_t* E, int32_t* M) {
+    int32_t e = 0, m = 0;
+    for (int z = 0; z < Lz; ++z)
+        for (int y = 0; y < Ly; ++y)
+            for (int x = 0; x < Lx; ++x) {
+                int sg = sp[(z * Ly + y) * Lx + x] ? 1 : -1;
+                int sx = sp[(z * Ly + y) * Lx + (x == Lx - 1 ? 0 : x + 1)] ? 1 : -1;
+                int sy = sp[(z * Ly + (y == Ly - 1 ? 0 : y + 1)) * Lx + x] ? 1 : -1;
+                int sz = sp[((z == Lz - 1 ? 0 : z + 1) * Ly + y) * Lx + x] ? 1 : -1;
+                e -= sg * (sx + sy + sz);
+                m += sg;
+            }
+    *E = e; *M = m;
+}
+
 // O5  TREE1024: the fixed summation order of the weight sum (L165: "deterministic ... sum the
 // per-block partial results in a subsequent kernel call").  Pad with +0.0 to a multiple of 1024;
 // inside every aligned run of 32 values: for off = 16,8,4,2,1: a[i] += a[i+off] for i < off;
@@ -227,7 +276,9 @@ double logaddexp(double a, double b) {
 }
 
 struct Oracle {
-    int L = 0, N = 0;
+    int L = 0, N = 0;        // N = number of sites (L*L, or Lx*Ly*Lz for a box, O16)
+    int D = 2, Lx = 0, Ly = 0, Lz = 1;   // dimension and edges (2D: Lx = Ly = L, Lz = 1)
+    int nlev = 0;            // energies lie on -2 nlev + 4m + e0, m = 0..nlev: nlev = (number of bonds)/2 = N (2D), 3N/2 (3D)
     int64_t R_target = 0, R_cur = 0, R_cap = 0;
     uint64_t seed = 0;
     uint32_t t = 0;          // global sweep counter
@@ -250,9 +301,11 @@ struct Oracle {
 void all_energies(const Oracle* o, std::vector<int32_t>& E, std::vector<int32_t>& M) {
     E.resize(o->R_cur); M.resize(o->R_cur);
 #pragma omp parallel for schedule(static)
-    for (int64_t j = 0; j < o->R_cur; ++j)
-        energy_one_replica(&o->spin[(size_t)j * o->N], o->L, &E[j], &M[j], o->Jx.empty() ? nullptr : o->Jx.data(),
-                           o->Jy.empty() ? nullptr : o->Jy.data());
+    for (int64_t j = 0; j < o->R_cur; ++j) {
+        if (o->D == 3) energy_one_replica_3d(&o->spin[(size_t)j * o->N], o->Lx, o->Ly, o->Lz, &E[j], &M[j]);
+        else energy_one_replica(&o->spin[(size_t)j * o->N], o->L, &E[j], &M[j], o->Jx.empty() ? nullptr : o->Jx.data(),
+                                o->Jy.empty() ? nullptr : o->Jy.data());
+    }
 }
 
 // O5 weights for a given dbeta: E_ref = min_j E_j, wtab[d] = exp(-(dbeta*(double)(4d))),
@@ -327,6 +380,7 @@ obs_values observables_for(const std::vector<int32_t>& E, const std::vector<int3
 }
 
 // O9, Eq. 9: fold the energy histogram at beta into the running sums.
+// N here is the number of levels minus one, nlev: the number of sites in 2D (E = -2N + 4m), 3N/2 on the cubic lattice (O16).
 void hist_fold_for(const std::vector<int32_t>& E, int N, double lnZ, double beta, int64_t* Hsum, double* lnD, int e0 = 0) {
     int64_t R = (int64_t)E.size();
     std::vector<int64_t> H(N + 1, 0);
@@ -345,7 +399,9 @@ void hist_fold_for(const std::vector<int32_t>& E, int N, double lnZ, double beta
 //   Z(beta) = sum_m Omega_m exp(-beta E_m),  <E^k> = sum_m E_m^k Omega_m exp(-beta E_m) / Z,
 // evaluated with the largest exponent taken out; the variance is summed about the mean (two passes).
 //   e = <E>/N,  C = beta^2 (<E^2> - <E>^2)/N  (Eq. 3),  ln Z = -beta F (Eq. 4).
-void reweight_for(int N, const int64_t* Hsum, const double* lnD, double beta, double* lnZ, double* e, double* C, int e0 = 0) {
+// N = nlev (levels E_m = -2N + 4m + e0, m = 0..N); nsites = number of spins (the same number in 2D; 0 = take N).
+void reweight_for(int N, const int64_t* Hsum, const double* lnD, double beta, double* lnZ, double* e, double* C, int e0 = 0, int nsites = 0) {
+    if (nsites == 0) nsites = N;
     const double ninf = -std::numeric_limits<double>::infinity();
     double amax = ninf;
     for (int m = 0; m <= N; ++m) {
@@ -368,8 +424,8 @@ void reweight_for(int N, const int64_t* Hsum, const double* lnD, double beta, do
         S2 += (Em - mean) * (Em - mean) * p;
     }
     *lnZ = amax + std::log(S0);
-    *e = mean / (double)N;
-    *C = beta * beta * (S2 / S0) / (double)N;
+    *e = mean / (double)nsites;
+    *C = beta * beta * (S2 / S0) / (double)nsites;
 }
 
 // O14, L129 "Generalizations to other quantities such as magnetizations are possible": microcanonical magnetisation sums.
@@ -385,7 +441,8 @@ void mag_fold_for(const std::vector<int32_t>& E, const std::vector<int32_t>& M, 
     }
 }
 void reweight_mag_for(int N, const int64_t* Hsum, const double* lnD, const int64_t* A1, const int64_t* A2, double beta,
-                      double* absm, double* m2, int e0 = 0) {
+                      double* absm, double* m2, int e0 = 0, int nsites = 0) {
+    if (nsites == 0) nsites = N;
     const double ninf = -std::numeric_limits<double>::infinity();
     double amax = ninf;
     for (int m = 0; m <= N; ++m) {
@@ -402,8 +459,8 @@ void reweight_mag_for(int N, const int64_t* Hsum, const double* lnD, const int64
         Sa += p * ((double)A1[m] / (double)Hsum[m]);
         Sq += p * ((double)A2[m] / (double)Hsum[m]);
     }
-    *absm = (Sa / S0) / (double)N;
-    *m2 = (Sq / S0) / ((double)N * (double)N);
+    *absm = (Sa / S0) / (double)nsites;
+    *m2 = (Sq / S0) / ((double)nsites * (double)nsites);
 }
 
 }  // namespace
@@ -564,16 +621,73 @@ int ora_create(int L, int64_t R, uint64_t seed, Oracle** out) {
     Oracle* o = new (std::nothrow) Oracle();
     if (!o) return ORA_ERR_NOMEM;
     o->L = L; o->N = L * L; o->R_target = R; o->R_cur = R; o->R_cap = capacity_for(R);
+    o->D = 2; o->Lx = L; o->Ly = L; o->Lz = 1; o->nlev = o->N;
     o->seed = seed; o->t = 0; o->k = 0;
     o->lnZ = (double)o->N * std::log(2.0);                    // Z_{beta_0} = 2^N, L93
     try { o->spin.assign((size_t)o->R_cap * o->N, 0); } catch (...) { delete o; return ORA_ERR_NOMEM; }
-    o->Hsum.assign(o->N + 1, 0);
-    o->lnD.assign(o->N + 1, -std::numeric_limits<double>::infinity());
-    o->A1sum.assign(o->N + 1, 0); o->A2sum.assign(o->N + 1, 0);
+    o->Hsum.assign(o->nlev + 1, 0);
+    o->lnD.assign(o->nlev + 1, -std::numeric_limits<double>::infinity());
+    o->A1sum.assign(o->nlev + 1, 0); o->A2sum.assign(o->nlev + 1, 0);
 #pragma omp parallel for schedule(static)
     for (int64_t j = 0; j < R; ++j)                           // step 1, L55, L65
         for (int s = 0; s < o->N; ++s) o->spin[(size_t)j * o->N + s] = x_init(seed, j, (uint32_t)s);
     *out = o;
+    return ORA_OK;
+}
+
+// O16: the same population on a periodic simple-cubic box dims = (Lx, Ly, Lz), every edge even and >= 2; ndim must be 3
+// (ndim = 2 with dims = (L, L) is ora_create).  ln Z starts at N ln 2 with N = Lx Ly Lz (L93).
+int ora_create_box(int ndim, const int* dims, int64_t R, uint64_t seed, Oracle** out) {
+    if (!out || !dims || R < 1) return ORA_ERR_INVALID_ARG;
+    if (ndim == 2) { if (dims[0] != dims[1]) return ORA_ERR_INVALID_ARG; return ora_create(dims[0], R, seed, out); }
+    if (ndim != 3) return ORA_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a) if (dims[a] < 2 || (dims[a] & 1)) return ORA_ERR_INVALID_ARG;
+    Oracle* o = new (std::nothrow) Oracle();
+    if (!o) return ORA_ERR_NOMEM;
+    o->D = 3; o->Lx = dims[0]; o->Ly = dims[1]; o->Lz = dims[2]; o->L = dims[0];
+    o->N = o->Lx * o->Ly * o->Lz; o->nlev = 3 * o->N / 2;
+    o->R_target = R; o->R_cur = R; o->R_cap = capacity_for(R);
+    o->seed = seed; o->t = 0; o->k = 0;
+    o->lnZ = (double)o->N * std::log(2.0);                    // Z_{beta_0} = 2^N, L93
+    try { o->spin.assign((size_t)o->R_cap * o->N, 0); } catch (...) { delete o; return ORA_ERR_NOMEM; }
+    o->Hsum.assign(o->nlev + 1, 0);
+    o->lnD.assign(o->nlev + 1, -std::numeric_limits<double>::infinity());
+    o->A1sum.assign(o->nlev + 1, 0); o->A2sum.assign(o->nlev + 1, 0);
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < R; ++j)                           // step 1, L55, L65: the INIT stream with the box's site index
+        for (int s = 0; s < o->N; ++s) o->spin[(size_t)j * o->N + s] = x_init(seed, j, (uint32_t)s);
+    *out = o;
+    return ORA_OK;
+}
+int ora_num_levels(const Oracle* o) { return o ? o->nlev + 1 : 0; }
+
+// stateless O16 pieces (pins, sampled parity checks)
+void ora_thresholds3(double beta, uint32_t* T4, uint32_t* T8, uint32_t* T12) {
+    *T4 = threshold(std::exp(-4.0 * beta));
+    *T8 = threshold(std::exp(-8.0 * beta));
+    *T12 = threshold(std::exp(-12.0 * beta));
+}
+int ora_sweep_slots_3d(const int* dims, uint64_t seed, uint32_t t0, double beta, int theta, int64_t nslots,
+                       const int64_t* slot_ids, uint8_t* spins) {
+    if (!dims || theta < 0 || nslots < 0) return ORA_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a) if (dims[a] < 2 || (dims[a] & 1)) return ORA_ERR_INVALID_ARG;
+    uint32_t T4, T8, T12; ora_thresholds3(beta, &T4, &T8, &T12);
+    const int N = dims[0] * dims[1] * dims[2];
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < nslots; ++i)
+        for (int it = 0; it < theta; ++it)
+            sweep_one_replica_3d(spins + (size_t)i * N, dims[0], dims[1], dims[2], seed, slot_ids[i], t0 + (uint32_t)it, T4, T8, T12);
+    return ORA_OK;
+}
+int ora_energies_of_3d(const int* dims, int64_t n, const uint8_t* spins, int32_t* E, int32_t* M) {
+    if (!dims || n < 0) return ORA_ERR_INVALID_ARG;
+    for (int a = 0; a < 3; ++a) if (dims[a] < 2 || (dims[a] & 1)) return ORA_ERR_INVALID_ARG;
+    const int N = dims[0] * dims[1] * dims[2];
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < n; ++j) {
+        int32_t e, m; energy_one_replica_3d(spins + (size_t)j * N, dims[0], dims[1], dims[2], &e, &m);
+        E[j] = e; if (M) M[j] = m;
+    }
     return ORA_OK;
 }
 
@@ -582,8 +696,8 @@ void ora_destroy(Oracle* o) { delete o; }
 // O15: bimodal couplings, Jx[s] = bond (x,y)-(x+1,y), Jy[s] = bond (x,y)-(x,y+1), values +1 / -1, s = y*L + x.
 // Both NULL: back to the ferromagnet.  Only before any histogram has been folded (the level offset e0 is part of the sums).
 int ora_set_couplings(Oracle* o, const int8_t* Jx, const int8_t* Jy) {
-    if (!o || ((Jx == nullptr) != (Jy == nullptr))) return ORA_ERR_INVALID_ARG;
-    for (int m = 0; m <= o->N; ++m) if (o->Hsum[m] != 0) return ORA_ERR_INVALID_ARG;
+    if (!o || ((Jx == nullptr) != (Jy == nullptr)) || (o->D == 3 && Jx)) return ORA_ERR_INVALID_ARG;   // O15 is a 2D workload
+    for (int m = 0; m <= o->nlev; ++m) if (o->Hsum[m] != 0) return ORA_ERR_INVALID_ARG;
     if (!Jx) { o->Jx.clear(); o->Jy.clear(); o->e0 = 0; return ORA_OK; }
     int64_t n_af = 0;
     for (int s = 0; s < o->N; ++s) {
@@ -622,7 +736,7 @@ int ora_energies_of_j(int L, int64_t n, const uint8_t* spins, const int8_t* Jx, 
 }
 // 0 = one Philox number per spin (O1), 1 = Philox-seeded LCG per word (O11, L236-L241)
 int ora_set_rng_mode(Oracle* o, int mode) {
-    if (!o || mode < 0 || mode > 1) return ORA_ERR_INVALID_ARG;
+    if (!o || mode < 0 || mode > 1 || (o->D == 3 && mode != RNG_PHILOX)) return ORA_ERR_INVALID_ARG;   // O11 is keyed by 2D row quads
     o->rng_mode = mode;
     return ORA_OK;
 }
@@ -635,6 +749,15 @@ double ora_lnZ(const Oracle* o) { return o->lnZ; }
 // step 3, L61: theta rounds of MCMC at inverse temperature beta.
 int ora_sweep(Oracle* o, double beta, int theta) {
     if (!o || theta < 0) return ORA_ERR_INVALID_ARG;
+    if (o->D == 3) {
+        uint32_t T4, T8, T12; ora_thresholds3(beta, &T4, &T8, &T12);
+#pragma omp parallel for schedule(static)
+        for (int64_t j = 0; j < o->R_cur; ++j)
+            for (int it = 0; it < theta; ++it)
+                sweep_one_replica_3d(&o->spin[(size_t)j * o->N], o->Lx, o->Ly, o->Lz, o->seed, j, o->t + (uint32_t)it, T4, T8, T12);
+        o->t += (uint32_t)theta;
+        return ORA_OK;
+    }
     uint32_t T4, T8; ora_thresholds(beta, &T4, &T8);
 #pragma omp parallel for schedule(static)
     for (int64_t j = 0; j < o->R_cur; ++j)
@@ -714,40 +837,40 @@ int ora_observables(Oracle* o, double beta, ora_obs_t* out) {
 int ora_hist_accumulate(Oracle* o, double beta) {
     if (!o) return ORA_ERR_INVALID_ARG;
     std::vector<int32_t> E, M; all_energies(o, E, M);
-    hist_fold_for(E, o->N, o->lnZ, beta, o->Hsum.data(), o->lnD.data(), o->e0);
-    mag_fold_for(E, M, o->N, o->A1sum.data(), o->A2sum.data(), o->e0);
+    hist_fold_for(E, o->nlev, o->lnZ, beta, o->Hsum.data(), o->lnD.data(), o->e0);
+    mag_fold_for(E, M, o->nlev, o->A1sum.data(), o->A2sum.data(), o->e0);
     return ORA_OK;
 }
 
 int ora_get_mag_sums(const Oracle* o, int64_t* A1, int64_t* A2) {
     if (!o) return ORA_ERR_INVALID_ARG;
-    if (A1) std::memcpy(A1, o->A1sum.data(), sizeof(int64_t) * (o->N + 1));
-    if (A2) std::memcpy(A2, o->A2sum.data(), sizeof(int64_t) * (o->N + 1));
+    if (A1) std::memcpy(A1, o->A1sum.data(), sizeof(int64_t) * (o->nlev + 1));
+    if (A2) std::memcpy(A2, o->A2sum.data(), sizeof(int64_t) * (o->nlev + 1));
     return ORA_OK;
 }
 int ora_reweight_mag(const Oracle* o, int n, const double* betas, double* absm, double* m2) {
     if (!o || n < 0) return ORA_ERR_INVALID_ARG;
     bool any = false;
-    for (int m = 0; m <= o->N; ++m) any = any || o->Hsum[m] > 0;
+    for (int m = 0; m <= o->nlev; ++m) any = any || o->Hsum[m] > 0;
     if (!any) return ORA_ERR_INVALID_ARG;
     for (int i = 0; i < n; ++i)
-        reweight_mag_for(o->N, o->Hsum.data(), o->lnD.data(), o->A1sum.data(), o->A2sum.data(), betas[i], &absm[i], &m2[i], o->e0);
+        reweight_mag_for(o->nlev, o->Hsum.data(), o->lnD.data(), o->A1sum.data(), o->A2sum.data(), betas[i], &absm[i], &m2[i], o->e0, o->N);
     return ORA_OK;
 }
 
 int ora_get_histogram(const Oracle* o, int64_t* Hsum, double* lnD) {
     if (!o) return ORA_ERR_INVALID_ARG;
-    if (Hsum) std::memcpy(Hsum, o->Hsum.data(), sizeof(int64_t) * (o->N + 1));
-    if (lnD) std::memcpy(lnD, o->lnD.data(), sizeof(double) * (o->N + 1));
+    if (Hsum) std::memcpy(Hsum, o->Hsum.data(), sizeof(int64_t) * (o->nlev + 1));
+    if (lnD) std::memcpy(lnD, o->lnD.data(), sizeof(double) * (o->nlev + 1));
     return ORA_OK;
 }
 
 int ora_reweight(const Oracle* o, int n, const double* betas, double* lnZ, double* e, double* C) {
     if (!o || n < 0) return ORA_ERR_INVALID_ARG;
     bool any = false;
-    for (int m = 0; m <= o->N; ++m) any = any || o->Hsum[m] > 0;
+    for (int m = 0; m <= o->nlev; ++m) any = any || o->Hsum[m] > 0;
     if (!any) return ORA_ERR_INVALID_ARG;
-    for (int i = 0; i < n; ++i) reweight_for(o->N, o->Hsum.data(), o->lnD.data(), betas[i], &lnZ[i], &e[i], &C[i], o->e0);
+    for (int i = 0; i < n; ++i) reweight_for(o->nlev, o->Hsum.data(), o->lnD.data(), betas[i], &lnZ[i], &e[i], &C[i], o->e0, o->N);
     return ORA_OK;
 }
 

@@ -55,6 +55,11 @@ def lib():
         L.ora_energies_of_j.argtypes = [i32, i64, vp, vp, vp, vp, vp]; L.ora_energies_of_j.restype = i32
         L.ora_weighted_average.argtypes = [i32, vp, vp, i32, vp, vp]; L.ora_weighted_average.restype = i32
         L.ora_create.argtypes = [i32, i64, u64, vp]; L.ora_create.restype = i32
+        L.ora_create_box.argtypes = [i32, vp, i64, u64, vp]; L.ora_create_box.restype = i32
+        L.ora_num_levels.argtypes = [vp]; L.ora_num_levels.restype = i32
+        L.ora_thresholds3.argtypes = [dbl, vp, vp, vp]; L.ora_thresholds3.restype = None
+        L.ora_sweep_slots_3d.argtypes = [vp, u64, u32, dbl, i32, i64, vp, vp]; L.ora_sweep_slots_3d.restype = i32
+        L.ora_energies_of_3d.argtypes = [vp, i64, vp, vp, vp]; L.ora_energies_of_3d.restype = i32
         L.ora_destroy.argtypes = [vp]; L.ora_destroy.restype = None
         L.ora_population.argtypes = [vp]; L.ora_population.restype = i64
         L.ora_capacity_of.argtypes = [vp]; L.ora_capacity_of.restype = i64
@@ -142,6 +147,31 @@ def energies_of_j(L, spins01, Jx, Jy):
     n = spins01.shape[0]
     E = np.empty(n, dtype=np.int32); M = np.empty(n, dtype=np.int32)
     _check(lib().ora_energies_of_j(L, n, _p(spins01), _p(Jx), _p(Jy), _p(E), _p(M)), "energies_of_j")
+    return E, M
+
+
+def thresholds3(beta):
+    """O16: (T4, T8, T12) of the simple-cubic lattice."""
+    t4, t8, t12 = C.c_uint32(), C.c_uint32(), C.c_uint32()
+    lib().ora_thresholds3(float(beta), C.byref(t4), C.byref(t8), C.byref(t12))
+    return t4.value, t8.value, t12.value
+
+
+def sweep_slots_3d(dims, seed, t0, beta, theta, slot_ids, spins01):
+    """O16: theta sweeps of the replicas spins01[n][Lx*Ly*Lz] (uint8 0/1, site = (z*Ly + y)*Lx + x) living in slots slot_ids; in place."""
+    d = np.ascontiguousarray(dims, dtype=np.int32)
+    slot_ids = np.ascontiguousarray(slot_ids, dtype=np.int64)
+    assert d.size == 3 and spins01.dtype == np.uint8 and spins01.flags.c_contiguous and spins01.shape[1] == int(d.prod())
+    _check(lib().ora_sweep_slots_3d(_p(d), seed, t0, float(beta), theta, slot_ids.size, _p(slot_ids), _p(spins01)), "sweep_slots_3d")
+    return spins01
+
+
+def energies_of_3d(dims, spins01):
+    d = np.ascontiguousarray(dims, dtype=np.int32)
+    spins01 = np.ascontiguousarray(spins01, dtype=np.uint8)
+    n = spins01.shape[0]
+    E = np.empty(n, dtype=np.int32); M = np.empty(n, dtype=np.int32)
+    _check(lib().ora_energies_of_3d(_p(d), n, _p(spins01), _p(E), _p(M)), "energies_of_3d")
     return E, M
 
 
@@ -243,11 +273,23 @@ def weighted_average(lnZ, A):
 class Oracle:
     """The same calls as include/pa.h (pa_create, pa_sweep, ...), on the CPU oracle."""
 
-    def __init__(self, L, R, seed):
-        self.L, self.N, self.R_target, self.seed = L, L * L, R, seed
+    def __init__(self, L, R, seed, dims=None):
+        """L x L square lattice, or (dims = (Lx, Ly, Lz), L ignored) a periodic simple-cubic box (O16)."""
         h = C.c_void_p()
-        _check(lib().ora_create(L, R, seed, C.byref(h)), "create")
+        if dims is None:
+            self.L, self.N, self.dims = L, L * L, (L, L)
+            _check(lib().ora_create(L, R, seed, C.byref(h)), "create")
+        else:
+            d = np.ascontiguousarray(dims, dtype=np.int32)
+            self.L, self.N, self.dims = int(d[0]), int(d.prod()), tuple(int(v) for v in d)
+            _check(lib().ora_create_box(d.size, _p(d), R, seed, C.byref(h)), "create_box")
+        self.R_target, self.seed = R, seed
         self._h = h
+        self.nlev = int(lib().ora_num_levels(h)) - 1         # energies lie on -2 nlev + 4m + e0, m = 0..nlev
+
+    @classmethod
+    def box(cls, dims, R, seed):
+        return cls(dims[0], R, seed, dims=dims)
 
     def close(self):
         if self._h:
@@ -287,7 +329,7 @@ class Oracle:
         return {"lnZ": lnZ, "e": e, "C": Cv}
 
     def mag_sums(self):
-        A1 = np.empty(self.N + 1, dtype=np.int64); A2 = np.empty(self.N + 1, dtype=np.int64)
+        A1 = np.empty(self.nlev + 1, dtype=np.int64); A2 = np.empty(self.nlev + 1, dtype=np.int64)
         _check(lib().ora_get_mag_sums(self._h, _p(A1), _p(A2)), "get_mag_sums")
         return A1, A2
 
@@ -351,7 +393,7 @@ class Oracle:
         _check(lib().ora_hist_accumulate(self._h, float(beta)), "hist_accumulate")
 
     def histogram(self):
-        H = np.empty(self.N + 1, dtype=np.int64); D = np.empty(self.N + 1, dtype=np.float64)
+        H = np.empty(self.nlev + 1, dtype=np.int64); D = np.empty(self.nlev + 1, dtype=np.float64)
         _check(lib().ora_get_histogram(self._h, _p(H), _p(D)), "get_histogram")
         return H, D
 
