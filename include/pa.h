@@ -72,6 +72,22 @@ int pa_create(int L, int64_t R, uint64_t seed, pa_t** out);
 int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out);
 void pa_destroy(pa_t* h);
 
+/* The same population on another lattice (L313 "models on different lattices in various dimensions ... straightforward", L43
+ * "3D Ising systems"; reading O16): ndim = 3, dims = {Lx, Ly, Lz} (HOST int[3]): a periodic simple-cubic box, every edge even and
+ * >= 2, at most 2^18 sites, Lz/C planes of a group (4 Lx Ly Lz / C bytes) fitting a CTA's shared memory for a C in {1,2,4,8}
+ * dividing Lz.  Site s = (z*Ly + y)*Lx + x in every per-site array of this header (spins, words).  A spin has six neighbour
+ * slots x+-1, y+-1, z+-1 (an edge of length 2 holds the same site in both slots of its direction; it counts twice); with u
+ * anti-parallel slots dE = 12 - 4u and pa_sweep flips iff u >= 3, or u = 2 and x < T4, or u = 1 and x < T8, or u = 0 and
+ * x < T12 = floor(exp(-12 beta) 2^32); colour 0 = (x+y+z) even first; the random numbers are the SWEEP stream's with this s.
+ * E_j = -sum_s s_s (s_{x+1} + s_{y+1} + s_{z+1}) lies on -3N + 4m, m = 0 .. 3N/2: the histogram arrays of pa_get_histogram /
+ * pa_get_mag_sums have pa_num_levels(h) = 3N/2 + 1 entries (N + 1 on the square lattice).  Every other call is unchanged;
+ * PA_RNG_LCG and pa_set_couplings are readings of the square lattice and return PA_ERR_INVALID_ARG on a box.
+ * ndim = 2 with dims = {L, L} is pa_create_ex.  dev_ws = NULL: cudaMalloc and a private stream, as pa_create. */
+int pa_workspace_bytes_box(int ndim, const int* dims, int64_t R, size_t* bytes);
+int pa_create_box(int ndim, const int* dims, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out);
+int pa_dims(const pa_t* h, int* ndim, int* dims);      /* dims: int[3]; either may be NULL */
+int64_t pa_num_levels(const pa_t* h);                  /* number of energy levels = length of the histogram arrays */
+
 /* Step 3 (L61; L151-L157): theta checkerboard Metropolis sweeps of every replica at inverse
  * temperature beta.  One sweep = colour 0 ((x+y) even), then colour 1.  A spin with u
  * anti-parallel neighbours (dE = 8 - 4u) flips iff u >= 2, or u = 1 and x < T4, or u = 0 and
@@ -144,7 +160,8 @@ int pa_observables(pa_t* h, double beta, pa_obs_t* out);
  * lnD[m] = logaddexp(lnD[m], ln R_cur - ln Z - beta (-2N + 4m))   (O9).
  * Call once per temperature, after the sweeps.  Asynchronous. */
 int pa_hist_accumulate(pa_t* h, double beta);
-/* Hsum: int64[N+1], lnD: double[N+1] (either may be NULL); ln Omega(E_m) = ln Hsum[m] - lnD[m]. */
+/* Hsum: int64[pa_num_levels], lnD: double[pa_num_levels] (N + 1 on the square lattice; either may be NULL);
+ * ln Omega(E_m) = ln Hsum[m] - lnD[m]. */
 int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD);
 
 /* n temperature steps in one call (steps 2-4 of L56-L62, n times): for i = 1..n, resample betas[i-1] -> betas[i], theta
@@ -170,7 +187,7 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
  * buffers are host pointers. */
 int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, double* C, double* absm, double* m2);
 
-/* The microcanonical magnetisation sums (O14): A1, A2: int64[N+1], host or device, either may be NULL. */
+/* The microcanonical magnetisation sums (O14): A1, A2: int64[pa_num_levels], host or device, either may be NULL. */
 int pa_get_mag_sums(pa_t* h, int64_t* A1, int64_t* A2);
 
 /* Weighted average of M independent runs (Sec. 2.2, Eq. 6-7; O13): omega_m = exp(lnZ_m) /

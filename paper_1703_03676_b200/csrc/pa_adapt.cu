@@ -21,7 +21,7 @@
 // flushed once per CTA; anything outside (never seen in practice: the window spans 4 PA_HWIN in energy) goes to global atomics.
 #define PA_HWIN 4096
 __global__ void __launch_bounds__(256)
-pa_ehist_kernel(const int32_t* __restrict__ E, long long R, int N, int e0, const PaScalars* __restrict__ sc, uint32_t* __restrict__ Hd) {
+pa_ehist_kernel(const int32_t* __restrict__ E, long long R, int N /* nlev */, int e0, const PaScalars* __restrict__ sc, uint32_t* __restrict__ Hd) {
     __shared__ uint32_t bins[PA_HWIN];
     for (int b = threadIdx.x; b < PA_HWIN; b += blockDim.x) bins[b] = 0u;
     __syncthreads();
@@ -104,11 +104,11 @@ pa_adapt_kernel(const uint32_t* __restrict__ Hd, const PaScalars* __restrict__ s
 }
 
 int pa_launch_ehist(pa_handle* h) {
-    PA_CUDA(h, cudaMemsetAsync(h->Hd, 0, ((size_t)h->N + 1) * 4, h->stream));
+    PA_CUDA(h, cudaMemsetAsync(h->Hd, 0, ((size_t)h->nlev + 1) * 4, h->stream));
     long long blocks = (h->R_cur + 256 * 16 - 1) / (256 * 16);
     if (blocks > 296) blocks = 296;
     if (blocks < 1) blocks = 1;
-    pa_ehist_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->E, h->R_cur, h->N, h->e0, h->d_scal, h->Hd);
+    pa_ehist_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->E, h->R_cur, h->nlev, h->e0, h->d_scal, h->Hd);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;

@@ -25,9 +25,9 @@ struct PaLayout {
     int64_t R_cap, G_cap, tiles;
 };
 
-static PaLayout pa_layout(int L, int64_t R) {
+// N = number of sites, nlev + 1 = number of energy levels (tables, histograms)
+static PaLayout pa_layout_n(size_t N, size_t nlev, int64_t R) {
     PaLayout y;
-    const size_t N = (size_t)L * L;
     y.R_cap = pa_capacity(R);
     y.G_cap = y.R_cap / 32;
     y.tiles = (y.R_cap + PA_TILE - 1) / PA_TILE;
@@ -43,15 +43,15 @@ static PaLayout pa_layout(int L, int64_t R) {
     y.parent = take((size_t)y.R_cap * 4);
     y.partials = take((size_t)y.tiles * 8);
     y.runsum = take((size_t)y.G_cap * 8);
-    y.wtab = take((N + 1) * 8);
+    y.wtab = take((nlev + 1) * 8);
     y.scan = take((size_t)y.tiles * 8);
-    y.Hsum = take((N + 1) * 8);
-    y.Hcur = take((N + 1) * 4);
-    y.Hd = take((N + 1) * 4);
+    y.Hsum = take((nlev + 1) * 8);
+    y.Hcur = take((nlev + 1) * 4);
+    y.Hd = take((nlev + 1) * 4);
     y.adapt = take(sizeof(PaAdaptState));
-    y.lnD = take((N + 1) * 8);
-    y.A1 = take((N + 1) * 8);
-    y.A2 = take((N + 1) * 8);
+    y.lnD = take((nlev + 1) * 8);
+    y.A1 = take((nlev + 1) * 8);
+    y.A2 = take((nlev + 1) * 8);
     y.jmask = take(N);
     y.jm16 = take(N / 8 * 2 + 2);
     y.scal = take(sizeof(PaScalars));
@@ -61,6 +61,19 @@ static PaLayout pa_layout(int L, int64_t R) {
     y.stage = take(y.stage_bytes);
     y.total = off;
     return y;
+}
+static PaLayout pa_layout(int L, int64_t R) { return pa_layout_n((size_t)L * L, (size_t)L * L, R); }
+
+// O16: a periodic simple-cubic box, every edge even and >= 2, at most 2^18 sites, and Lz/C whole planes of one group
+// (N*4/C bytes) must fit the shared memory of a CTA for a cluster size C in {1,2,4,8} dividing Lz.
+static bool pa_box_ok(const int* d, int64_t R) {
+    if (!d || R < 1 || R > (int64_t)1 << 31) return false;
+    for (int a = 0; a < 3; ++a) if (d[a] < 2 || (d[a] & 1) || d[a] > 512) return false;
+    const long long N = (long long)d[0] * d[1] * d[2];
+    if (N > (1 << 18)) return false;
+    for (int C = 1; C <= 8; C *= 2)
+        if (d[2] % C == 0 && (size_t)N * 4 / C <= (size_t)224 * 1024) return true;
+    return false;
 }
 
 // L even, 4 <= L <= 512, and the sweep kernel's strip of L/C rows of a group (L*L*4/C bytes) must fit the shared memory of a CTA
@@ -115,8 +128,8 @@ static int pa_ensure_host_scalars(pa_handle* h) {
     if (h->host_scal_valid) return PA_OK;
     if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
     h->host_scal_valid = true;
-    h->Emin = -2 * h->N + 4 * (int)(0xffffffffu - h->h_scal->mmin_inv) + h->e0;
-    h->Emax = -2 * h->N + 4 * (int)h->h_scal->mmax + h->e0;
+    h->Emin = -2 * h->nlev + 4 * (int)(0xffffffffu - h->h_scal->mmin_inv) + h->e0;
+    h->Emax = -2 * h->nlev + 4 * (int)h->h_scal->mmax + h->e0;
     return PA_OK;
 }
 
@@ -141,16 +154,51 @@ int pa_workspace_bytes(int L, int64_t R, size_t* bytes) {
     return PA_OK;
 }
 
+int pa_workspace_bytes_box(int ndim, const int* dims, int64_t R, size_t* bytes) {
+    if (!bytes || !dims) return PA_ERR_INVALID_ARG;
+    if (ndim == 2) return dims[0] == dims[1] ? pa_workspace_bytes(dims[0], R, bytes) : PA_ERR_INVALID_ARG;
+    if (ndim != 3 || !pa_box_ok(dims, R)) return PA_ERR_INVALID_ARG;
+    const size_t N = (size_t)dims[0] * dims[1] * dims[2];
+    *bytes = pa_layout_n(N, 3 * N / 2, R).total;
+    return PA_OK;
+}
+
+static int pa_create_impl(int D, PaGeom geom, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out);
+
 int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out) {
     if (!out || !pa_args_ok(L, R)) return PA_ERR_INVALID_ARG;
+    const PaGeom g = {L, L, 1};
+    return pa_create_impl(2, g, R, seed, dev_ws, ws_bytes, cuda_stream, out);
+}
+
+int pa_create_box(int ndim, const int* dims, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out) {
+    if (!out || !dims) return PA_ERR_INVALID_ARG;
+    if (ndim == 2) return dims[0] == dims[1] ? pa_create_ex(dims[0], R, seed, dev_ws, ws_bytes, cuda_stream, out) : PA_ERR_INVALID_ARG;
+    if (ndim != 3 || !pa_box_ok(dims, R)) return PA_ERR_INVALID_ARG;
+    const PaGeom g = {dims[0], dims[1], dims[2]};
+    return pa_create_impl(3, g, R, seed, dev_ws, ws_bytes, cuda_stream, out);
+}
+
+int pa_dims(const pa_t* h, int* ndim, int* dims) {
+    if (!h) return PA_ERR_INVALID_ARG;
+    if (ndim) *ndim = h->D;
+    if (dims) { dims[0] = h->geom.Lx; dims[1] = h->geom.Ly; if (h->D == 3) dims[2] = h->geom.Lz; }
+    return PA_OK;
+}
+int64_t pa_num_levels(const pa_t* h) { return h ? (int64_t)h->nlev + 1 : 0; }
+
+static int pa_create_impl(int D, PaGeom geom, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out) {
     *out = nullptr;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return PA_ERR_CUDA; }
-    const PaLayout y = pa_layout(L, R);
+    const int L = geom.Lx;
+    const size_t Nsites = (size_t)geom.Lx * geom.Ly * geom.Lz, nlev_ = D == 3 ? 3 * Nsites / 2 : Nsites;
+    const PaLayout y = pa_layout_n(Nsites, nlev_, R);
     pa_handle* h = new (std::nothrow) pa_handle();
     if (!h) return PA_ERR_NOMEM;
     memset(h, 0, sizeof(*h));
-    h->L = L; h->N = L * L; h->R_target = R; h->R_cur = R; h->R_cap = y.R_cap; h->G_cap = y.G_cap;
+    h->L = L; h->N = (int)Nsites; h->D = D; h->geom = geom; h->nlev = (int)nlev_;
+    h->R_target = R; h->R_cur = R; h->R_cap = y.R_cap; h->G_cap = y.G_cap;
     h->seed = seed; h->keys = pa_make_keys(seed); h->rng_mode = PA_RNG_PHILOX; h->timing = PA_TIME_SWEEP;
     h->lnZ = (double)h->N * log(2.0);           // Z_{beta_0} = 2^N (L93)
     h->n_tiles_cap = y.tiles;
@@ -181,7 +229,7 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     h->stage = (int8_t*)(b + y.stage); h->stage_bytes = y.stage_bytes;
     // pinned host mirrors
     if (cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
-        cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->N + 1)) != cudaSuccess ||
+        cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->nlev + 1)) != cudaSuccess ||
         cudaMallocHost(&h->h_adapt, sizeof(PaAdaptState)) != cudaSuccess) { rc = PA_ERR_CUDA; }
     for (int i = 0; i < 9 && rc == PA_OK; ++i)
         if (cudaEventCreateWithFlags(&h->ev[i], i == 6 ? cudaEventDisableTiming : cudaEventDefault) != cudaSuccess) rc = PA_ERR_CUDA;
@@ -189,12 +237,12 @@ int pa_create_ex(int L, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes,
     if (rc == PA_OK) {
         // empty histograms: Hsum = 0, Hcur = 0, lnD = -inf
         cudaMemsetAsync(h->d_scal, 0, sizeof(PaScalars), h->stream);
-        cudaMemsetAsync(h->Hsum, 0, ((size_t)h->N + 1) * 8, h->stream);
-        cudaMemsetAsync(h->Hcur, 0, ((size_t)h->N + 1) * 4, h->stream);
-        cudaMemsetAsync(h->A1, 0, ((size_t)h->N + 1) * 8, h->stream);
-        cudaMemsetAsync(h->A2, 0, ((size_t)h->N + 1) * 8, h->stream);
-        for (int m = 0; m <= h->N; ++m) h->h_wtab[m] = -INFINITY;
-        if (cudaMemcpyAsync(h->lnD, h->h_wtab, ((size_t)h->N + 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
+        cudaMemsetAsync(h->Hsum, 0, ((size_t)h->nlev + 1) * 8, h->stream);
+        cudaMemsetAsync(h->Hcur, 0, ((size_t)h->nlev + 1) * 4, h->stream);
+        cudaMemsetAsync(h->A1, 0, ((size_t)h->nlev + 1) * 8, h->stream);
+        cudaMemsetAsync(h->A2, 0, ((size_t)h->nlev + 1) * 8, h->stream);
+        for (int m = 0; m <= h->nlev; ++m) h->h_wtab[m] = -INFINITY;
+        if (cudaMemcpyAsync(h->lnD, h->h_wtab, ((size_t)h->nlev + 1) * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
         if (rc == PA_OK) rc = pa_launch_init(h);
         if (rc == PA_OK && cudaStreamSynchronize(h->stream) != cudaSuccess) rc = PA_ERR_CUDA;
     }
@@ -223,6 +271,7 @@ int pa_sweep(pa_t* h, double beta, int theta) {
     if (!h || theta < 0 || !(beta == beta)) return PA_ERR_INVALID_ARG;
     if (theta == 0) return PA_OK;
     const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
+    h->T12 = pa_threshold(exp(-12.0 * beta));                                    // O16: dE = 12 exists on the cubic lattice only
     const bool timed = (h->timing & PA_TIME_SWEEP) != 0;
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[0], h->stream));
     int rc = pa_launch_sweep(h, T4, T8, theta);
@@ -236,6 +285,7 @@ int pa_sweep(pa_t* h, double beta, int theta) {
 
 int pa_set_rng_mode(pa_t* h, int mode) {
     if (!h || (mode != PA_RNG_PHILOX && mode != PA_RNG_LCG)) return PA_ERR_INVALID_ARG;
+    if (h->D == 3 && mode != PA_RNG_PHILOX) return PA_ERR_INVALID_ARG;        // O11 is keyed by quads of rows of the square lattice
     h->rng_mode = mode;
     return PA_OK;
 }
@@ -243,7 +293,7 @@ int pa_get_rng_mode(const pa_t* h) { return h ? h->rng_mode : PA_ERR_INVALID_ARG
 
 // O15 (L313): bimodal couplings shared by all replicas.  Builds the per-word bond mask in the resident (colour-split) order.
 int pa_set_couplings(pa_t* h, const int8_t* Jx, const int8_t* Jy) {
-    if (!h || ((Jx == nullptr) != (Jy == nullptr)) || h->hist_any) return PA_ERR_INVALID_ARG;
+    if (!h || ((Jx == nullptr) != (Jy == nullptr)) || h->hist_any || (h->D == 3 && Jx)) return PA_ERR_INVALID_ARG;   // O15 is a 2D workload
     h->em_valid = false; h->host_scal_valid = false;
     if (!Jx) { h->has_j = false; h->e0 = 0; return PA_OK; }
     const int L = h->L, N = h->N, Lh = L / 2;
@@ -487,13 +537,13 @@ static int pa_anneal_digest(pa_handle* h, PaAnnealCtx& cx, const char* h_snaps, 
         h->R_prev = cx.R_prev; h->W_last = S.W;
         h->R_cur = R_new;
         if (obs_out) pa_fill_obs(h, S, beta, R_new, h->lnZ, lnQ, &obs_out[s0 + i]);
-        cx.Emin_prev = -2 * h->N + 4 * (int)(0xffffffffu - S.mmin_inv) + h->e0;
+        cx.Emin_prev = -2 * h->nlev + 4 * (int)(0xffffffffu - S.mmin_inv) + h->e0;
         cx.R_prev = R_new;
         cx.done += 1;
         if (s0 + i == n - 1) {
             *h->h_scal = S;
             h->host_scal_valid = true; h->em_valid = true;
-            h->Emin = cx.Emin_prev; h->Emax = -2 * h->N + 4 * (int)S.mmax + h->e0;
+            h->Emin = cx.Emin_prev; h->Emax = -2 * h->nlev + 4 * (int)S.mmax + h->e0;
         }
     }
     return PA_OK;
@@ -506,7 +556,7 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
     if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
     // Steps go in chunks with two staging buffers: while the device runs chunk c the host builds the weight tables of chunk
     // c+1 (N+1 exponentials per step) and digests the snapshots of chunk c-1.
-    const size_t tab = (size_t)h->N + 1, snap = (sizeof(PaScalars) + 15) / 16 * 16;
+    const size_t tab = (size_t)h->nlev + 1, snap = (sizeof(PaScalars) + 15) / 16 * 16;
     const size_t per_step = tab * 8 + snap;
     int chunk_cap = (int)(h->stage_bytes / 2 / per_step);
     if (chunk_cap > 16) chunk_cap = 16;
@@ -552,7 +602,7 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
         for (int i = 0; i < cs; ++i) {                               // O5: wtab[d] = exp(-(dbeta * (double)(4 d))), full level range
             const double dbeta = betas[s0 + i + 1] - betas[s0 + i];
             double* t = h_t + (size_t)i * tab;
-            for (int d = 0; d <= h->N; ++d) t[d] = exp(-(dbeta * (double)(4 * d)));
+            for (int d = 0; d <= h->nlev; ++d) t[d] = exp(-(dbeta * (double)(4 * d)));
         }
         if (cudaMemcpyAsync(d_t, h_t, (size_t)cs * tab * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = PA_ERR_CUDA; break; }
         h->dev_R = true;
@@ -568,6 +618,7 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
             if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[3], h->stream);
             h->cur ^= 1; h->k += 1;
             const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
+            h->T12 = pa_threshold(exp(-12.0 * beta));
             if (h->timing & PA_TIME_SWEEP) cudaEventRecord(h->ev[0], h->stream);
             if ((rc = pa_launch_sweep(h, T4, T8, theta)) != PA_OK) break;
             if (h->timing & PA_TIME_SWEEP) cudaEventRecord(h->ev[1], h->stream);
@@ -615,8 +666,8 @@ int pa_hist_accumulate(pa_t* h, double beta) {
 int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD) {
     if (!h) return PA_ERR_INVALID_ARG;
     int rc = PA_OK;
-    if (Hsum) rc = pa_copy_out(h, Hsum, h->Hsum, ((size_t)h->N + 1) * 8, nullptr);
-    if (rc == PA_OK && lnD) rc = pa_copy_out(h, lnD, h->lnD, ((size_t)h->N + 1) * 8, nullptr);
+    if (Hsum) rc = pa_copy_out(h, Hsum, h->Hsum, ((size_t)h->nlev + 1) * 8, nullptr);
+    if (rc == PA_OK && lnD) rc = pa_copy_out(h, lnD, h->lnD, ((size_t)h->nlev + 1) * 8, nullptr);
     return rc;
 }
 
@@ -639,8 +690,8 @@ int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, dou
 int pa_get_mag_sums(pa_t* h, int64_t* A1, int64_t* A2) {
     if (!h) return PA_ERR_INVALID_ARG;
     int rc = PA_OK;
-    if (A1) rc = pa_copy_out(h, A1, h->A1, ((size_t)h->N + 1) * 8, nullptr);
-    if (rc == PA_OK && A2) rc = pa_copy_out(h, A2, h->A2, ((size_t)h->N + 1) * 8, nullptr);
+    if (A1) rc = pa_copy_out(h, A1, h->A1, ((size_t)h->nlev + 1) * 8, nullptr);
+    if (rc == PA_OK && A2) rc = pa_copy_out(h, A2, h->A2, ((size_t)h->nlev + 1) * 8, nullptr);
     return rc;
 }
 

@@ -14,6 +14,28 @@
 // the two sub-lattices separately too, L157):   index(c, y, xh) = c*(N/2) + y*(L/2) + xh,
 // xh = x >> 1.   Site (x,y) of colour c in row y has x = 2*xh + ((y+c)&1).
 // ------------------------------------------------------------------------------------------------
+// A simple-cubic box Lx x Ly x Lz (O16) uses the same scheme with the "row" r = z*Ly + y:
+//   index(c, r, xh) = c*(N/2) + r*(Lx/2) + xh,  x = 2*xh + ((y+z+c)&1),  site s = r*Lx + x;
+// Lz = 1 is the square lattice.
+struct PaGeom { int Lx, Ly, Lz; };
+#ifdef __CUDACC__
+// site index s = (z*Ly + y)*Lx + x of the word at resident index idx
+__host__ __device__ __forceinline__ int pa_site_of_index(int idx, PaGeom g) {
+    const int Lh = g.Lx >> 1, half = (g.Lx * g.Ly * g.Lz) >> 1;
+    const int c = idx >= half ? 1 : 0;
+    const int rem = idx - c * half;
+    const int r = rem / Lh, xh = rem - r * Lh;
+    const int z = r / g.Ly, y = r - z * g.Ly;
+    return r * g.Lx + 2 * xh + ((y + z + c) & 1);
+}
+__host__ __device__ __forceinline__ int pa_index_of_site(int s, PaGeom g) {
+    const int r = s / g.Lx, x = s - r * g.Lx;
+    const int z = r / g.Ly, y = r - z * g.Ly;
+    const int c = (x + y + z) & 1;
+    return c * ((g.Lx * g.Ly * g.Lz) >> 1) + r * (g.Lx >> 1) + (x >> 1);
+}
+#endif
+
 #define PA_TAG_INIT 0u
 #define PA_TAG_SWEEP 1u
 #define PA_TAG_RESAMPLE 2u
@@ -87,8 +109,9 @@ struct PaScalars {
 // Once a resampling step of pa_anneal has left [1, R_cap] (sc->err) the population counts as empty for every later kernel of the
 // call: they all exit without touching the spins or E, M, so the population stays the one before the failing step (O7).
 __device__ __forceinline__ long long pa_live_R(long long R, const PaScalars* sc) { return R >= 0 ? R : (sc->err ? 0ll : (long long)sc->R_dev); }
-__device__ __forceinline__ int pa_live_Emin(int Emin, const PaScalars* sc, int N, int e0) {
-    return Emin != PA_EMIN_DEV ? Emin : -2 * N + 4 * (int)(0xffffffffu - sc->mmin_inv) + e0;
+// nlev = (number of bonds)/2: energies lie on -2 nlev + 4m + e0, m = 0..nlev (nlev = N on the square lattice, 3N/2 on the cubic one)
+__device__ __forceinline__ int pa_live_Emin(int Emin, const PaScalars* sc, int nlev, int e0) {
+    return Emin != PA_EMIN_DEV ? Emin : -2 * nlev + 4 * (int)(0xffffffffu - sc->mmin_inv) + e0;
 }
 #endif
 
@@ -102,7 +125,9 @@ struct PaAdaptState {
 };
 
 struct pa_handle {
-    int L, N;
+    int L, N;                // N = number of sites; L = Lx
+    int D; PaGeom geom;      // dimension (2 / 3, O16) and edges; D = 2: geom = {L, L, 1}
+    int nlev;                // energy levels m = 0..nlev, E_m = -2 nlev + 4m + e0: N (2D), 3N/2 (3D)
     int64_t R_target, R_cur, R_cap;
     int64_t G_cap;           // groups at capacity
     uint64_t seed;
@@ -158,6 +183,7 @@ struct pa_handle {
     double* h_tabs; size_t h_tabs_bytes; // pinned staging for pa_anneal's weight tables and snapshots
     int64_t launches;
     bool sweep_C_forced;
+    uint32_t T12;            // third threshold of the cubic lattice (dE = 12), set by pa_sweep
     int sweep_C, sweep_T, sweep_cmp, sweep_kind;   // sweep launch geometry (cluster size, threads), compare variant, kernel kind
     char cuda_err[256];
 };

@@ -65,7 +65,7 @@ __device__ __forceinline__ void pa_warp_add_planes(uint32_t (&p)[NPL]) {
 // Everything after the per-thread bit-sliced counters, shared by both measure kernels.  pe / pm hold NPL planes
 // of the thread's unsatisfied-bond and up-spin counts (bit b of plane k = bit k of replica b's count).
 template <int NPL>
-__device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&pm)[NPL], long long g, int N, long long R_cur,
+__device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&pm)[NPL], long long g, int N, int nlev, long long R_cur,
                                                 int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
                                                 double* __restrict__ runsum, double* __restrict__ blocksum, PaScalars* __restrict__ snap) {
     const int T = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -86,7 +86,7 @@ __device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&
         for (int w = 0; w < nw; ++w) { unsat += sE[w][lane]; up += sM[w][lane]; }
         const long long j = g * 32 + lane;
         const bool live = j < pa_live_R(R_cur, sc);
-        const int e = 2 * unsat - 2 * N, m = 2 * up - N;
+        const int e = 2 * unsat - 2 * nlev, m = 2 * up - N;          // E = 2 unsat - (number of bonds), M = 2 up - N
         if (live) { E[j] = e; M[j] = m; }
         long long se = live ? e : 0, se2 = live ? (long long)e * e : 0, sa = live ? (m < 0 ? -m : m) : 0, sm2 = live ? (long long)m * m : 0;
         unsigned mlo = live ? 0xffffffffu - (unsigned)unsat / 2u : 0u;      // m = (E + 2N)/4 = unsat/2; max of (2^32-1 - m) = min m
@@ -164,48 +164,52 @@ __device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&
 //   so its __shfl_down tree IS the aligned-run-of-32 level; the run sums go to runsum[g], and the last CTA
 //   to finish (atomic ticket) does the tree over each 32 run sums and the sequential sum over 1024-blocks.
 __global__ void __launch_bounds__(256)
-pa_measure_generic_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R_cur,
+pa_measure_generic_kernel(const uint32_t* __restrict__ pop, PaGeom geo, int N, long long R_cur,
                   int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
                   double* __restrict__ runsum, double* __restrict__ blocksum, const uint8_t* __restrict__ jmask,
-                  PaScalars* __restrict__ snap) {
+                  PaScalars* __restrict__ snap, int nlev) {
     const long long g = blockIdx.x;
     const uint32_t* base = pop + g * (long long)N;
-    const int Lh = L >> 1, half = N >> 1;
+    const int Lh = geo.Lx >> 1, Ly = geo.Ly, Lz = geo.Lz, half = N >> 1;
     const int T = blockDim.x, tid = threadIdx.x;
     BitCounter cE, cM;
     cE.clear(); cM.clear();
     for (int b0 = tid * 8; b0 < N; b0 += T * 8) {
-        uint32_t xa[8], xb[8], xs[8];
+        uint32_t xa[8], xb[8], xc[8], xs[8];
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
             int idx = b0 + q;
-            uint32_t s = 0, a = 0, b = 0;
+            uint32_t s = 0, a = 0, b = 0, cz = 0;
             if (idx < N) {
                 int c = idx >= half ? 1 : 0;
                 int rem = idx - c * half;
-                int y = rem / Lh, xh = rem - y * Lh;
-                int p = (y + c) & 1;
+                int r = rem / Lh, xh = rem - r * Lh;          // row r = z*Ly + y (z = 0 on the square lattice)
+                int z = r / Ly, y = r - z * Ly;
+                int p = (y + z + c) & 1;
                 const uint32_t* oth = base + (1 - c) * half;
                 s = base[idx];
-                // right neighbour (x+1, y): other colour, same row; down neighbour (x, y+1)
+                // every site owns its +x, +y (and, O16, +z) bond: right neighbour (x+1): other colour, same row;
+                // an edge of length 2 makes the bond a double bond, owned by both of its sites
                 int xr = p ? (xh + 1 == Lh ? 0 : xh + 1) : xh;
-                int yd = (y + 1 == L) ? 0 : y + 1;
-                a = s ^ oth[y * Lh + xr];
-                b = s ^ oth[yd * Lh + xh];
+                int yd = (y + 1 == Ly) ? 0 : y + 1;
+                a = s ^ oth[r * Lh + xr];
+                b = s ^ oth[(z * Ly + yd) * Lh + xh];
+                if (Lz > 1) { int zd = (z + 1 == Lz) ? 0 : z + 1; cz = s ^ oth[(zd * Ly + y) * Lh + xh]; }
                 if (jmask) {                     // O15: a J = -1 bond is unsatisfied when its ends are parallel
                     const uint32_t j = jmask[idx];
                     a ^= 0u - ((j >> 4) & 1u);   // right bond
                     b ^= 0u - ((j >> 3) & 1u);   // down bond
                 }
             }
-            xs[q] = s; xa[q] = a; xb[q] = b;
+            xs[q] = s; xa[q] = a; xb[q] = b; xc[q] = cz;
         }
         cE.add8(xa); cE.add8(xb); cM.add8(xs);
+        if (Lz > 1) cE.add8(xc);
     }
     uint32_t pe[PA_EPLANES], pm[PA_EPLANES];
 #pragma unroll
     for (int k = 0; k < PA_EPLANES; ++k) { pe[k] = cE.plane(k); pm[k] = cM.plane(k); }
-    pa_measure_tail<PA_EPLANES>(pe, pm, g, N, R_cur, E, M, sc, runsum, blocksum, snap);
+    pa_measure_tail<PA_EPLANES>(pe, pm, g, N, nlev, R_cur, E, M, sc, runsum, blocksum, snap);
 }
 
 
@@ -316,7 +320,7 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
     uint32_t pe[NPW], pm[NPW];
 #pragma unroll
     for (int k = 0; k < NPW; ++k) { pe[k] = k < NPE ? cE.pl[k < NPE ? k : 0] : 0u; pm[k] = k < NPM ? cM.pl[k < NPM ? k : 0] : 0u; }
-    pa_measure_tail<NPW>(pe, pm, g, N, R_cur, E, M, sc, runsum, blocksum, snap);
+    pa_measure_tail<NPW>(pe, pm, g, N, N, R_cur, E, M, sc, runsum, blocksum, snap);
 }
 
 int pa_launch_measure(pa_handle* h) {
@@ -327,7 +331,7 @@ int pa_launch_measure(pa_handle* h) {
     h->scal_zeroed = false;
     const bool timed = (h->timing & PA_TIME_MEASURE) != 0;
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
-    const bool pow2 = (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
+    const bool pow2 = h->D == 2 && (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
     if (pow2) {
 #define PA_MSR_CASE(LOG) case (8 << LOG): \
         if (h->has_j) pa_measure_kernel<LOG, true><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
@@ -340,8 +344,8 @@ int pa_launch_measure(pa_handle* h) {
     } else {
         int T = 256;
         while (T > 32 && T * 8 > h->N) T >>= 1;
-        pa_measure_generic_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, Rarg, h->E, h->M, h->d_scal,
-                                                                    h->runsum, h->partials, h->has_j ? h->jmask : nullptr, h->snap_out);
+        pa_measure_generic_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, Rarg, h->E, h->M, h->d_scal,
+                                                                    h->runsum, h->partials, h->has_j ? h->jmask : nullptr, h->snap_out, h->nlev);
     }
     PA_CUDA(h, cudaGetLastError());
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));

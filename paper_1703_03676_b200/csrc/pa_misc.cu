@@ -3,22 +3,9 @@
 #include "pa_common.cuh"
 #include <math.h>
 
-// site index s = y*L + x of the word at resident index idx (see pa_common.cuh)
-__device__ __forceinline__ int pa_site_of_index(int idx, int L) {
-    const int Lh = L >> 1, half = (L * L) >> 1;
-    const int c = idx >= half ? 1 : 0;
-    const int rem = idx - c * half;
-    const int y = rem / Lh, xh = rem - y * Lh;
-    return y * L + 2 * xh + ((y + c) & 1);
-}
-__device__ __forceinline__ int pa_index_of_site(int s, int L) {
-    const int y = s / L, x = s - y * L;
-    const int c = (x + y) & 1;
-    return c * ((L * L) >> 1) + y * (L >> 1) + (x >> 1);
-}
 
 // a0 (L55, L65; O1): word(g, s) = philox(s, g>>2, 0, TAG_INIT)[g&3]; lanes >= R are cleared.
-__global__ void pa_init_kernel(uint32_t* __restrict__ pop, int L, int N, long long R, PhiloxKeys K) {
+__global__ void pa_init_kernel(uint32_t* __restrict__ pop, PaGeom L, int N, long long R, PhiloxKeys K) {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     const long long G = (R + 31) / 32;
     if (i >= G * N) return;
@@ -35,7 +22,7 @@ __global__ void pa_init_kernel(uint32_t* __restrict__ pop, int L, int N, long lo
 
 int pa_launch_init(pa_handle* h) {
     const long long n = ((h->R_cur + 31) / 32) * (long long)h->N;
-    pa_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, h->keys);
+    pa_init_kernel<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, h->R_cur, h->keys);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
@@ -43,7 +30,7 @@ int pa_launch_init(pa_handle* h) {
 
 // a9 (Eq. 9; O9)
 // also O14 (L129): the microcanonical magnetisation sums A1[m] += |M_j|, A2[m] += M_j^2 (exact integers, order-free)
-__global__ void pa_hist_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, long long R, int N,
+__global__ void pa_hist_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, long long R, int N /* nlev */,
                                uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ A1, unsigned long long* __restrict__ A2) {
     for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x) {
         const int m = (E[j] + 2 * N) >> 2;
@@ -55,7 +42,7 @@ __global__ void pa_hist_kernel(const int32_t* __restrict__ E, const int32_t* __r
     }
 }
 __global__ void pa_hist_fold_kernel(uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ Hsum,
-                                    double* __restrict__ lnD, int N, double lnR_minus_lnZ, double beta, int e0) {
+                                    double* __restrict__ lnD, int N /* nlev */, double lnR_minus_lnZ, double beta, int e0) {
     const int m = blockIdx.x * blockDim.x + threadIdx.x;
     if (m > N) return;
     Hsum[m] += Hcur[m];
@@ -72,9 +59,9 @@ __global__ void pa_hist_fold_kernel(uint32_t* __restrict__ Hcur, unsigned long l
 int pa_launch_hist(pa_handle* h, double beta) {
     int blocks = (int)((h->R_cur + 255) / 256);
     if (blocks > 1184) blocks = 1184;
-    pa_hist_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->M, h->R_cur, h->N, h->Hcur, h->A1, h->A2);
+    pa_hist_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->M, h->R_cur, h->nlev, h->Hcur, h->A1, h->A2);
     const double c = log((double)h->R_cur) - h->lnZ;
-    pa_hist_fold_kernel<<<(h->N + 1 + 255) / 256, 256, 0, h->stream>>>(h->Hcur, h->Hsum, h->lnD, h->N, c, beta, h->e0);
+    pa_hist_fold_kernel<<<(h->nlev + 1 + 255) / 256, 256, 0, h->stream>>>(h->Hcur, h->Hsum, h->lnD, h->nlev, c, beta, h->e0);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 2;
     return PA_OK;
@@ -111,7 +98,7 @@ __device__ __forceinline__ double pa_block_reduce(double v, double* sh) {
 
 __global__ void __launch_bounds__(256)
 pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __restrict__ lnD,
-                   const unsigned long long* __restrict__ A1, const unsigned long long* __restrict__ A2, int N, int e0,
+                   const unsigned long long* __restrict__ A1, const unsigned long long* __restrict__ A2, int N /* nlev */, int nsites, int e0,
                    const double* __restrict__ betas, double* __restrict__ lnZ, double* __restrict__ e, double* __restrict__ C,
                    double* __restrict__ absm, double* __restrict__ m2) {
     __shared__ double sh[33];
@@ -149,17 +136,17 @@ pa_reweight_kernel(const unsigned long long* __restrict__ Hsum, const double* __
     s2 = pa_block_reduce<false>(s2, sh);
     if (threadIdx.x == 0) {
         lnZ[blockIdx.x] = amax + log(s0);
-        e[blockIdx.x] = mean / (double)N;
-        C[blockIdx.x] = beta * beta * (s2 / s0) / (double)N;
-        absm[blockIdx.x] = (sa / s0) / (double)N;
-        m2[blockIdx.x] = (sq / s0) / ((double)N * (double)N);
+        e[blockIdx.x] = mean / (double)nsites;
+        C[blockIdx.x] = beta * beta * (s2 / s0) / (double)nsites;
+        absm[blockIdx.x] = (sa / s0) / (double)nsites;
+        m2[blockIdx.x] = (sq / s0) / ((double)nsites * (double)nsites);
     }
 }
 
 // d_io: [betas(n) | lnZ(n) | e(n) | C(n) | absm(n) | m2(n)] in device memory
 int pa_launch_reweight(pa_handle* h, int n, double* d_io) {
     const size_t z = (size_t)n;
-    pa_reweight_kernel<<<n, 256, 0, h->stream>>>(h->Hsum, h->lnD, h->A1, h->A2, h->N, h->e0, d_io, d_io + z, d_io + 2 * z, d_io + 3 * z,
+    pa_reweight_kernel<<<n, 256, 0, h->stream>>>(h->Hsum, h->lnD, h->A1, h->A2, h->nlev, h->N, h->e0, d_io, d_io + z, d_io + 2 * z, d_io + 3 * z,
                                                  d_io + 4 * z, d_io + 5 * z);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
@@ -193,7 +180,7 @@ cudaError_t pa_run_wavg(int M, const double* d_lnZ, const double* d_A, int nobs,
 }
 
 // ---- spin export / import ------------------------------------------------------------------------
-__global__ void pa_unpack_kernel(const uint32_t* __restrict__ pop, int L, int N, const long long* __restrict__ slots,
+__global__ void pa_unpack_kernel(const uint32_t* __restrict__ pop, PaGeom L, int N, const long long* __restrict__ slots,
                                  long long j0, long long n, int8_t* __restrict__ out) {
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= n * N) return;
@@ -203,7 +190,7 @@ __global__ void pa_unpack_kernel(const uint32_t* __restrict__ pop, int L, int N,
     const uint32_t w = pop[(j >> 5) * N + pa_index_of_site(s, L)];
     out[i] = ((w >> (j & 31)) & 1u) ? 1 : -1;
 }
-__global__ void pa_pack_kernel(uint32_t* __restrict__ pop, int L, int N, long long j0, long long n, const int8_t* __restrict__ in) {
+__global__ void pa_pack_kernel(uint32_t* __restrict__ pop, PaGeom L, int N, long long j0, long long n, const int8_t* __restrict__ in) {
     // one thread per (group, site): rewrites the bits of replicas j0..j0+n-1 that fall in this word
     const long long g0 = j0 >> 5, g1 = (j0 + n - 1) >> 5;
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -223,7 +210,7 @@ __global__ void pa_pack_kernel(uint32_t* __restrict__ pop, int L, int N, long lo
 }
 // The sweep kernels flip all 32 lanes of the last group, so the resident lanes past the population hold arbitrary bits (every
 // reader masks by j < R); the interchange words are canonical: dead lanes read as 0.
-__global__ void pa_words_out_kernel(const uint32_t* __restrict__ pop, int L, int N, long long R, uint32_t* __restrict__ out) {
+__global__ void pa_words_out_kernel(const uint32_t* __restrict__ pop, PaGeom L, int N, long long R, uint32_t* __restrict__ out) {
     const long long G = (R + 31) / 32;
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= G * N) return;
@@ -234,7 +221,7 @@ __global__ void pa_words_out_kernel(const uint32_t* __restrict__ pop, int L, int
     if (live < 32) w &= (1u << live) - 1u;
     out[i] = w;
 }
-__global__ void pa_words_in_kernel(uint32_t* __restrict__ pop, int L, int N, long long R, const uint32_t* __restrict__ in) {
+__global__ void pa_words_in_kernel(uint32_t* __restrict__ pop, PaGeom L, int N, long long R, const uint32_t* __restrict__ in) {
     const long long G = (R + 31) / 32;
     const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= G * N) return;
@@ -249,7 +236,7 @@ __global__ void pa_words_in_kernel(uint32_t* __restrict__ pop, int L, int N, lon
 int pa_launch_unpack(pa_handle* h, const int64_t* d_slots, int64_t j0, int64_t n, int8_t* d_out) {
     const long long tot = n * (long long)h->N;
     if (tot == 0) return PA_OK;
-    pa_unpack_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N,
+    pa_unpack_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N,
                                                                           (const long long*)d_slots, j0, n, d_out);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
@@ -259,21 +246,21 @@ int pa_launch_pack(pa_handle* h, int64_t j0, int64_t n, const int8_t* d_in) {
     if (n == 0) return PA_OK;
     const long long ng = ((j0 + n - 1) >> 5) - (j0 >> 5) + 1;
     const long long tot = ng * h->N;
-    pa_pack_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, j0, n, d_in);
+    pa_pack_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, j0, n, d_in);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
 }
 int pa_launch_words_out(pa_handle* h, uint32_t* d_words) {
     const long long G = (h->R_cur + 31) / 32, tot = G * h->N;
-    pa_words_out_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, h->R_cur, d_words);
+    pa_words_out_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, h->R_cur, d_words);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
 }
 int pa_launch_words_in(pa_handle* h, int64_t R, const uint32_t* d_words) {
     const long long G = (R + 31) / 32, tot = G * h->N;
-    pa_words_in_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->L, h->N, R, d_words);
+    pa_words_in_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, R, d_words);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;

@@ -72,7 +72,7 @@ int pa_launch_weights(pa_handle* h, int Emin, double* w_out) {
     const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
     pa_tree_kernel<0><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab_cur ? h->wtab_cur : h->wtab, h->d_scal, h->dev_R ? -1 : h->R_cur,
                                                     (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, w_out,
-                                                    h->partials, h->scan_state, h->N, h->e0);
+                                                    h->partials, h->scan_state, h->nlev, h->e0);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
@@ -81,7 +81,7 @@ int pa_launch_weights(pa_handle* h, int Emin, double* w_out) {
 int pa_launch_overlap(pa_handle* h, int Emin) {
     const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
     pa_tree_kernel<1><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, Emin, nullptr,
-                                                    h->partials, h->scan_state, h->N, h->e0);
+                                                    h->partials, h->scan_state, h->nlev, h->e0);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
@@ -198,7 +198,7 @@ int pa_launch_plan(pa_handle* h, int Emin) {
     const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
     pa_plan_kernel<<<n, 256, 0, h->stream>>>(h->E, h->wtab_cur ? h->wtab_cur : h->wtab, h->d_scal, h->dev_R ? -1 : h->R_cur,
                                              (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, h->keys, h->k,
-                                             h->R_cap, h->r, h->o, h->parent, h->scan_state, n, h->N, h->e0);
+                                             h->R_cap, h->r, h->o, h->parent, h->scan_state, n, h->nlev, h->e0);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;

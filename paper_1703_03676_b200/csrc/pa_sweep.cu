@@ -19,6 +19,8 @@ namespace cg = cooperative_groups;
 struct SweepParams {
     PhiloxKeys K;
     uint32_t T4, T8;                 // acceptance thresholds for dE = 4, 8 (O2)
+    uint32_t T12;                    // ... and dE = 12 (simple-cubic lattice, O16)
+    int Ly, Lz;                      // O16: rows per plane and planes (Lz = 1: square lattice); H = rows per CTA
     uint32_t t0;                     // sweep counter at launch
     uint32_t two;                    // the constant 2, opaque to ptxas (see pa_shift_in_ge)
     int theta;
@@ -481,6 +483,160 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Simple-cubic lattice (O16).  The same scheme one dimension up: a cluster of C CTAs owns a group, each CTA
+// stages Lz/C whole z-planes of both colours (rows r = z*Ly + y, H = Ly*Lz/C of them), and only the z-neighbours of a strip's
+// first and last plane live in the neighbouring CTA's shared memory.  Per word: six neighbour words, a bit-sliced count of the
+// six anti-parallel flags (two full adders and a half adder), the same 8 Philox calls, and THREE threshold tests per lane
+// (dE = 12 - 4u in {4, 8, 12}):  flip = [u>=3] | (x<T4 & [u>=2]) | (x<T8 & [u>=1]) | x<T12   (T12 <= T8 <= T4).
+// An edge of length 2 makes the two neighbour slots of that direction the same word: it simply enters the count twice.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t pa_flip_mask3d(uint32_t s, uint32_t n0, uint32_t n1, uint32_t n2, uint32_t n3, uint32_t n4,
+                                                   uint32_t n5, uint32_t site, uint32_t c0base, uint32_t lo1u, const SweepParams& P) {
+    const uint32_t a0 = s ^ n0, a1 = s ^ n1, a2 = s ^ n2, a3 = s ^ n3, a4 = s ^ n4, a5 = s ^ n5;
+    const uint32_t s1 = a0 ^ a1 ^ a2, c1 = (a0 & a1) | (a2 & (a0 ^ a1));
+    const uint32_t s2 = a3 ^ a4 ^ a5, c2 = (a3 & a4) | (a5 & (a3 ^ a4));
+    const uint32_t low = s1 ^ s2, c3 = s1 & s2;                       // u = low + 2 (c1 + c2 + c3)
+    const uint32_t b1 = c1 ^ c2 ^ c3, b2 = (c1 & c2) | (c3 & (c1 ^ c2));
+    const uint32_t U1 = low | b1 | b2, U2 = b1 | b2, U3 = b2 | (b1 & low);
+    // ---- 8 Philox4x32-10 calls, counters (site, 8g+i, 2t+c, TAG_SWEEP), i = 0..7 (O1): as in pa_flip_mask ----
+    uint32_t x0[8], x1[8], x2[8], x3[8];
+    uint32_t hi0, lo0;
+    pa_mulhilo(PA_PHILOX_M0, site, hi0, lo0);
+    const uint32_t c2w = hi0 ^ PA_TAG_SWEEP ^ P.K.k1[0];
+    const uint32_t c3w = lo0;
+    uint32_t hi1w, lo1w;
+    pa_mulhilo(PA_PHILOX_M1, c2w, hi1w, lo1w);
+    const uint32_t c0w = hi1w ^ lo1u ^ P.K.k0[1];
+    const uint32_t c1w = lo1w;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        uint32_t h, l;
+        pa_mulhilo(PA_PHILOX_M0, c0base ^ (uint32_t)i, h, l);
+        x2[i] = h ^ c3w ^ P.K.k1[1];
+        x3[i] = l;
+    }
+    uint32_t hi0w, lo0w;
+    pa_mulhilo(PA_PHILOX_M0, c0w, hi0w, lo0w);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        uint32_t h, l;
+        pa_mulhilo(PA_PHILOX_M1, x2[i], h, l);
+        x0[i] = h ^ c1w ^ P.K.k0[2];
+        x1[i] = l;
+        x2[i] = hi0w ^ x3[i] ^ P.K.k1[2];
+        x3[i] = lo0w;
+    }
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            uint32_t h0, l0, h1, l1;
+            pa_mulhilo(PA_PHILOX_M0, x0[i], h0, l0);
+            pa_mulhilo(PA_PHILOX_M1, x2[i], h1, l1);
+            x0[i] = h1 ^ x1[i] ^ P.K.k0[r];
+            x1[i] = l1;
+            x2[i] = h0 ^ x3[i] ^ P.K.k1[r];
+            x3[i] = l0;
+        }
+    }
+    uint32_t g4 = 0, g8 = 0, g12 = 0;              // bit b = (x_b >= T): built most-significant bit first
+#pragma unroll
+    for (int i = 7; i >= 0; --i) {
+        const uint32_t xs[4] = {x0[i], x1[i], x2[i], x3[i]};
+#pragma unroll
+        for (int q = 3; q >= 0; --q) {
+            pa_shift_in_ge(g4, xs[q], P.T4, P.two);
+            pa_shift_in_ge(g8, xs[q], P.T8, P.two);
+            pa_shift_in_ge(g12, xs[q], P.T12, P.two);
+        }
+    }
+    return U3 | (~g4 & U2) | (~g8 & U1) | ~g12;
+}
+
+template <bool CLUSTER>
+__global__ void __launch_bounds__(256, 3)
+pa_sweep3d_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
+    extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh], H = Ly * (Lz / C) rows
+    const int T = blockDim.x, tid = threadIdx.x;
+    const int C = CLUSTER ? P.C : 1;
+    unsigned cr = 0;
+    if (CLUSTER) cr = cg::this_cluster().block_rank();
+    const long long g = blockIdx.x / C;
+    if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // uniform per cluster
+    const int H = P.H, Lh = P.Lh, Lx = P.L, Ly = P.Ly;
+    const int Pz = H / Ly;                              // planes of this CTA
+    const int z0 = (int)cr * Pz;
+    const int half = H * Lh;
+    uint32_t* gbase = pop + g * (long long)P.N;
+    const int goff = z0 * Ly * Lh, gcol = P.N >> 1;
+    if ((half & 3) == 0) {
+        for (int c = 0; c < 2; ++c) {
+            const uint4* src = reinterpret_cast<const uint4*>(gbase + c * gcol + goff);
+            uint4* dst = reinterpret_cast<uint4*>(tile + c * half);
+            for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+        }
+    } else {
+        for (int c = 0; c < 2; ++c)
+            for (int i = tid; i < half; i += T) tile[c * half + i] = gbase[c * gcol + goff + i];
+    }
+    const uint32_t* up_tile = tile;
+    const uint32_t* dn_tile = tile;
+    if (CLUSTER) {
+        cg::cluster_group cl = cg::this_cluster();
+        up_tile = cl.map_shared_rank(tile, (cr + C - 1) % C);
+        dn_tile = cl.map_shared_rank(tile, (cr + 1) % C);
+        cl.sync();
+    } else {
+        __syncthreads();
+    }
+    const uint32_t g8 = (uint32_t)(8 * g);
+    const int plane = Ly * Lh;
+    for (int it = 0; it < P.theta; ++it) {
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t c2 = 2u * (P.t0 + (uint32_t)it) + (uint32_t)c;
+            uint32_t hi1u, lo1u;
+            pa_mulhilo(PA_PHILOX_M1, c2, hi1u, lo1u);
+            const uint32_t c0base = hi1u ^ P.K.k0[0] ^ g8;
+            uint32_t* mine = tile + c * half;
+            const uint32_t* oth = tile + (1 - c) * half;
+            const uint32_t* up_oth = up_tile + (1 - c) * half;
+            const uint32_t* dn_oth = dn_tile + (1 - c) * half;
+#pragma unroll 1
+            for (int w = tid; w < half; w += T) {
+                const int rl = w / Lh, xh = w - rl * Lh;
+                const int zl = rl / Ly, y = rl - zl * Ly;
+                const int z = z0 + zl;
+                const int p = (y + z + c) & 1;
+                const int in_plane = y * Lh + xh, pl = zl * plane;
+                const uint32_t s = mine[w];
+                const uint32_t nS = oth[w];
+                const int xh2 = p ? (xh + 1 == Lh ? 0 : xh + 1) : (xh == 0 ? Lh - 1 : xh - 1);
+                const uint32_t nX = oth[w - xh + xh2];
+                const uint32_t nYm = oth[pl + (y == 0 ? Ly - 1 : y - 1) * Lh + xh];
+                const uint32_t nYp = oth[pl + (y + 1 == Ly ? 0 : y + 1) * Lh + xh];
+                uint32_t nZm, nZp;
+                if (zl > 0) nZm = oth[w - plane]; else nZm = up_oth[(Pz - 1) * plane + in_plane];
+                if (zl < Pz - 1) nZp = oth[w + plane]; else nZp = dn_oth[in_plane];
+                const uint32_t site = (uint32_t)((z * Ly + y) * Lx + 2 * xh + p);
+                mine[w] = s ^ pa_flip_mask3d(s, nS, nX, nYm, nYp, nZm, nZp, site, c0base, lo1u, P);
+            }
+            if (CLUSTER) cg::this_cluster().sync(); else __syncthreads();
+        }
+    }
+    if ((half & 3) == 0) {
+        for (int c = 0; c < 2; ++c) {
+            uint4* dst = reinterpret_cast<uint4*>(gbase + c * gcol + goff);
+            const uint4* src = reinterpret_cast<const uint4*>(tile + c * half);
+            for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+        }
+    } else {
+        for (int c = 0; c < 2; ++c)
+            for (int i = tid; i < half; i += T) gbase[c * gcol + goff + i] = tile[c * half + i];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
 static int pa_env_int(const char* name, int dflt) {
@@ -499,7 +655,29 @@ static bool pa_col_ok(int L, int C, int T, int rng_mode = PA_RNG_PHILOX) {
     return H % q == 0 && T >= Lh && (T & (T - 1)) == 0 && half % T == 0 && half / T >= q && (half / T) % q == 0;
 }
 
+// O16: the smallest cluster size C in {1,2,4,8} dividing Lz whose Lz/C planes fit the preferred 64 KB (else 224 KB).
+static int pa_sweep_configure_3d(pa_handle* h) {
+    const size_t bytes = (size_t)h->N * 4;
+    const int Lz = h->geom.Lz;
+    int C = 0;
+    for (int lim = 64; lim <= 224 && !C; lim += 160)
+        for (int c = 1; c <= 8 && !C; c *= 2)
+            if (Lz % c == 0 && bytes / c <= (size_t)lim * 1024) C = c;
+    const int forceC = pa_env_int("PA_SWEEP_C", 0);
+    h->sweep_C_forced = false;
+    if (forceC > 0 && forceC <= 8 && (forceC & (forceC - 1)) == 0 && Lz % forceC == 0 && bytes / forceC <= (size_t)224 * 1024) { C = forceC; h->sweep_C_forced = true; }
+    if (!C) return PA_ERR_INVALID_ARG;
+    const int half = h->N / 2 / C;
+    int T = 256;
+    while (T > 32 && T > half) T >>= 1;
+    const int forceT = pa_env_int("PA_SWEEP_T", 0);
+    if (forceT >= 32 && forceT <= 256) T = forceT;
+    h->sweep_C = C; h->sweep_T = T; h->sweep_kind = 0; h->sweep_cmp = 1;
+    return PA_OK;
+}
+
 int pa_sweep_configure(pa_handle* h) {
+    if (h->D == 3) return pa_sweep_configure_3d(h);
     const int L = h->L;
     // strips of up to 64 KB (three CTAs of 256 threads per SM); L = 256: 128 KB strips, clusters of two, one CTA of 512 threads per SM
     const bool big = L == 256;
@@ -636,11 +814,31 @@ static cudaError_t pa_sweep_dispatch_j(pa_handle* h, const SweepParams& P, size_
               : pa_sweep_launch_k(h, pa_sweep_kernel<1, false, PA_RNG_PHILOX, true>, P, smem, grid, false);
 }
 
-int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
-    if (theta == 0) return PA_OK;
+static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     SweepParams P;
     P.K = h->keys;
-    P.T4 = T4; P.T8 = T8;
+    P.T4 = T4; P.T8 = T8; P.T12 = h->T12;
+    P.t0 = h->t; P.theta = theta; P.two = 2u;
+    const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;
+    P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
+    P.L = h->geom.Lx; P.Lh = h->geom.Lx / 2; P.Ly = h->geom.Ly; P.Lz = h->geom.Lz; P.N = h->N;
+    P.C = h->sweep_C; P.H = h->geom.Ly * (h->geom.Lz / P.C);
+    P.jmask = nullptr;
+    const size_t smem = (size_t)h->N * 4 / P.C;
+    const unsigned grid = (unsigned)(G * P.C);
+    const cudaError_t e = P.C > 1 ? pa_sweep_launch_k(h, pa_sweep3d_kernel<true>, P, smem, grid, true)
+                                  : pa_sweep_launch_k(h, pa_sweep3d_kernel<false>, P, smem, grid, false);
+    PA_CUDA(h, e);
+    h->launches += 1;
+    return PA_OK;
+}
+
+int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
+    if (theta == 0) return PA_OK;
+    if (h->D == 3) return pa_launch_sweep_3d(h, T4, T8, theta);
+    SweepParams P;
+    P.K = h->keys;
+    P.T4 = T4; P.T8 = T8; P.T12 = 0u; P.Ly = h->L; P.Lz = 1;
     P.t0 = h->t; P.theta = theta; P.two = 2u;
     const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;

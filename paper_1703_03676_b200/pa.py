@@ -65,6 +65,10 @@ def lib():
         "pa_workspace_bytes": ([i32, i64, C.POINTER(sz)], i32),
         "pa_create": ([i32, i64, u64, C.POINTER(vp)], i32),
         "pa_create_ex": ([i32, i64, u64, vp, sz, vp, C.POINTER(vp)], i32),
+        "pa_workspace_bytes_box": ([i32, vp, i64, C.POINTER(sz)], i32),
+        "pa_create_box": ([i32, vp, i64, u64, vp, sz, vp, C.POINTER(vp)], i32),
+        "pa_dims": ([vp, C.POINTER(i32), vp], i32),
+        "pa_num_levels": ([vp], i64),
         "pa_destroy": ([vp], None),
         "pa_sweep": ([vp, dbl, i32], i32),
         "pa_anneal": ([vp, i32, vp, i32, vp], i32),
@@ -186,20 +190,46 @@ class Population:
     """One population on the current CUDA device.  Workspace and stream come from PyTorch
     (pa_create_ex) unless own_memory=True (pa_create: cudaMalloc + private stream)."""
 
-    def __init__(self, L, R, seed, stream=None, own_memory=False):
+    def __init__(self, L, R, seed, stream=None, own_memory=False, dims=None):
+        """L x L square lattice, or (dims = (Lx, Ly, Lz); L ignored) a periodic simple-cubic box (pa_create_box)."""
         import torch
         if not torch.cuda.is_available():
             raise PaError(PA_ERR_CUDA, "Population", "no CUDA device: this library has no CPU path")
-        self.L, self.N, self.R_target, self.seed = L, L * L, R, seed
         self._torch = torch
         self._ws = None
-        if own_memory:
-            self._h = pa_create(L, R, seed)
+        self.R_target, self.seed = R, seed
+        if dims is not None:
+            d = np.ascontiguousarray(dims, dtype=np.int32)
+            self.L, self.N, self.dims = int(d[0]), int(d.prod()), tuple(int(v) for v in d)
+            h = C.c_void_p()
+            if own_memory:
+                rc = lib().pa_create_box(d.size, _ptr(d), R, seed, None, 0, None, C.byref(h))
+            else:
+                n = C.c_size_t()
+                rc = lib().pa_workspace_bytes_box(d.size, _ptr(d), R, C.byref(n))
+                if rc:
+                    raise PaError(rc, "pa_workspace_bytes_box")
+                self._ws = torch.empty(n.value, dtype=torch.uint8, device="cuda")
+                self._stream = stream if stream is not None else torch.cuda.current_stream()
+                rc = lib().pa_create_box(d.size, _ptr(d), R, seed, C.c_void_p(self._ws.data_ptr()), n.value,
+                                         C.c_void_p(self._stream.cuda_stream), C.byref(h))
+            if rc:
+                raise PaError(rc, "pa_create_box")
+            self._h = h
         else:
-            nbytes = pa_workspace_bytes(L, R)
-            self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
-            self._stream = stream if stream is not None else torch.cuda.current_stream()
-            self._h = pa_create_ex(L, R, seed, self._ws.data_ptr(), nbytes, self._stream.cuda_stream)
+            self.L, self.N, self.dims = L, L * L, (L, L)
+            if own_memory:
+                self._h = pa_create(L, R, seed)
+            else:
+                nbytes = pa_workspace_bytes(L, R)
+                self._ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+                self._stream = stream if stream is not None else torch.cuda.current_stream()
+                self._h = pa_create_ex(L, R, seed, self._ws.data_ptr(), nbytes, self._stream.cuda_stream)
+        self.nlev = int(lib().pa_num_levels(self._h)) - 1
+
+    @classmethod
+    def box(cls, dims, R, seed, **kw):
+        return cls(dims[0], R, seed, dims=dims, **kw)
 
     def close(self):
         if getattr(self, "_h", None):
@@ -326,7 +356,7 @@ class Population:
         self._check(lib().pa_hist_accumulate(self._h, float(beta)), "pa_hist_accumulate")
 
     def histogram(self):
-        H = np.empty(self.N + 1, dtype=np.int64); D = np.empty(self.N + 1, dtype=np.float64)
+        H = np.empty(self.nlev + 1, dtype=np.int64); D = np.empty(self.nlev + 1, dtype=np.float64)
         self._check(lib().pa_get_histogram(self._h, _ptr(H), _ptr(D)), "pa_get_histogram")
         return H, D
 
@@ -339,7 +369,7 @@ class Population:
         return out
 
     def mag_sums(self):
-        A1 = np.empty(self.N + 1, dtype=np.int64); A2 = np.empty(self.N + 1, dtype=np.int64)
+        A1 = np.empty(self.nlev + 1, dtype=np.int64); A2 = np.empty(self.nlev + 1, dtype=np.int64)
         self._check(lib().pa_get_mag_sums(self._h, _ptr(A1), _ptr(A2)), "pa_get_mag_sums")
         return A1, A2
 
