@@ -212,7 +212,7 @@ def whole_run(pa, wl, seed, rng):
     import torch
 
     def run(mask):
-        pop = pa.Population(wl.L, wl.R, seed)
+        pop = pa.Population(wl.L, wl.R, seed, dims=wl.dims)
         pop.set_timing(mask)
         if rng == "lcg":
             pop.set_rng_mode(pa.PA_RNG_LCG)
@@ -257,7 +257,7 @@ def whole_run(pa, wl, seed, rng):
            "final_observables": obs}
     if wl.n_steps is not None and not wl.multi_histogram:
         # the same schedule in ONE pa_anneal call (no host round trip between its steps)
-        pop = pa.Population(wl.L, wl.R, seed)
+        pop = pa.Population(wl.L, wl.R, seed, dims=wl.dims)
         pop.set_timing(0)
         if rng == "lcg":
             pop.set_rng_mode(pa.PA_RNG_LCG)
@@ -340,7 +340,7 @@ def sweep_roof(rng, sm_max):
     """(algorithmic units per update, peak in G units/s, unit, kernel name) of the sweep kernel's binding resource (DESIGN.md 6.1 / 6.4)."""
     if rng == "lcg":
         return LCG_INSTR_PER_UPDATE, N_SM * ISSUE_LANES_PER_CLK_PER_SM * sm_max * 1e-3, "G thread-instructions/s", "pa_sweep_lcg_kernel"
-    return WIDE_MUL_PER_UPDATE, N_SM * WIDE_MUL_PER_CLK_PER_SM * sm_max * 1e-3, "G IMAD.WIDE.U32/s", "pa_sweep_col_kernel"
+    return WIDE_MUL_PER_UPDATE, N_SM * WIDE_MUL_PER_CLK_PER_SM * sm_max * 1e-3, "G IMAD.WIDE.U32/s", "pa_sweep_col_kernel (pa_sweep3d_kernel on a box)"
 
 
 class Runner:
@@ -348,7 +348,7 @@ class Runner:
 
     def __init__(self, pa, wl, seed, rng, couplings="ferro", dims=2):
         self.pa, self.wl, self.rng = pa, wl, rng
-        self.pop = pa.Population(wl.L, wl.R, seed)
+        self.pop = pa.Population(wl.L, wl.R, seed, dims=wl.dims)
         if rng == "lcg":
             self.pop.set_rng_mode(pa.PA_RNG_LCG)
         if couplings == "pmj":
@@ -572,7 +572,7 @@ def run_ours(args):
     if world == 1 and not args.no_others and args.couplings == "ferro":
         # configs 1-2 are launch/latency-bound and the roofline is judged on the large ones; all stay visible here
         others = []
-        for cfg, rng in [(c, args.rng) for c in (2, 3, 4) if c != args.config] + [(5, "lcg"), (3, "lcg")]:
+        for cfg, rng in [(c, args.rng) for c in (2, 3, 4) if c != args.config] + [(5, "lcg"), (3, "lcg"), (6, "philox")]:
             if (cfg, rng) == (args.config, args.rng):
                 continue
             try:
@@ -589,7 +589,7 @@ def run_ours(args):
 def oracle_step_rate(wl, R_sample, steps, warmup, rng="philox"):
     """The oracle, as it stands, on a population of R_sample replicas of the workload's shape."""
     from oracle import pa_oracle as po
-    o = po.Oracle(wl.L, R_sample, wl.seed)
+    o = po.Oracle(wl.L, R_sample, wl.seed, dims=wl.dims)
     if rng == "lcg":
         o.set_rng_mode(po.RNG_LCG)
     betas = wl.betas() if wl.n_steps is not None else [wl.beta0 + 0.005 * i for i in range(steps + warmup + 2)]
@@ -609,7 +609,7 @@ def oracle_step_rate(wl, R_sample, steps, warmup, rng="philox"):
 def oracle_step_rates(wl, R_sample, steps, rng="philox"):
     """updates/ns of each of `steps` consecutive temperature steps of the oracle on R_sample replicas, and the thread count."""
     from oracle import pa_oracle as po
-    o = po.Oracle(wl.L, R_sample, wl.seed)
+    o = po.Oracle(wl.L, R_sample, wl.seed, dims=wl.dims)
     if rng == "lcg":
         o.set_rng_mode(po.RNG_LCG)
     betas = wl.betas() if wl.n_steps is not None else [wl.beta0 + 0.002 * i for i in range(steps + 2)]

@@ -10,7 +10,7 @@ replicas (Tables 2-3: L = 16..256, R = 2 000..100 000, theta = 1..500).
 themselves are generated inside each implementation from the seed (INIT stream, O1).
 """
 from dataclasses import dataclass
-from typing import List, Optional
+from typing import List, Optional, Tuple
 
 
 @dataclass(frozen=True)
@@ -25,10 +25,11 @@ class Workload:
     theta: int                      # Metropolis sweeps per temperature (L61)
     target_overlap: Optional[float] = None   # alpha* of Eq. 8 (L115) when adaptive
     multi_histogram: bool = False            # Eq. 9 accumulation at every temperature
+    dims: Optional[Tuple[int, int, int]] = None   # (Lx, Ly, Lz) of a simple-cubic box; None = L x L square lattice
 
     @property
     def N(self) -> int:
-        return self.L * self.L
+        return self.L * self.L if self.dims is None else self.dims[0] * self.dims[1] * self.dims[2]
 
     @property
     def groups(self) -> int:
@@ -48,6 +49,9 @@ CONFIGS = {
     4: Workload("cfg4_L128_R100000_adaptive", 128, 100000, 4, 0.0, 1.0, None, 10,
                 target_overlap=0.85, multi_histogram=True),
     5: Workload("cfg5_L256_R1000000", 256, 1000000, 5, 0.0, 0.5, 500, 10),
+    # not in BASELINE.json: SURVEY 8(f) row 4, the second workload on another lattice ("models on different lattices in
+    # various dimensions", L43 "3D Ising systems"): a 32^3 simple-cubic lattice, R = 100 000, beta 0 -> 0.3 (past beta_c = 0.2217)
+    6: Workload("cube_L32_R100000", 32, 100000, 6, 0.0, 0.3, 150, 10, dims=(32, 32, 32)),
 }
 
 
