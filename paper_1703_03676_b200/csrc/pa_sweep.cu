@@ -27,6 +27,7 @@ struct SweepParams {
     int L, Lh, H, C, N;
     long long R;                     // population size, or -1: read sc->R_dev (pa_anneal)
     const PaScalars* sc;
+    long long Gcap;                  // groups the population buffer holds (p = 64 experiment: the second group of a pair may not exist)
     const uint8_t* jmask;            // O15: per resident word, bit k = bond to neighbour k (same, x, up, down) has J = -1; NULL = ferromagnet
 };
 
@@ -483,6 +484,95 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// p = 64 experiment (Sec. 4, Table 1 L196 / L200 / L204: 64-bit words were SLOWER than 32-bit ones on Kepler; SURVEY
+// 8(f) row 4 asks for the measurement on B200).  The LCG column-walk kernel with a 64-replica word = the words of two adjacent
+// groups side by side (uint2 in shared memory, 64-bit LDS / STS); the random stream is unchanged (O11: one seed per 32-replica
+// word), so the result is bit-identical to the p = 32 kernel.  What a wider word can share on a 32-bit integer datapath is the
+// addressing, the loop and half of the shared-memory instructions; every LCG step, compare, insert and logic op doubles.
+// Selected with PA_LCG_P64=1 (power-of-two L, ferromagnet).
+// ------------------------------------------------------------------------------------------------
+template <int LOG_LH, bool CLUSTER, int NOR>
+__global__ void __launch_bounds__(LOG_LH == 7 ? 512 : 256)
+pa_sweep_lcg64_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
+    extern __shared__ __align__(16) uint2 tile2[];     // [2][H][Lh], .x = group 2q, .y = group 2q+1
+    constexpr int Lh = 1 << LOG_LH;
+    const int T = blockDim.x, tid = threadIdx.x;
+    const int C = CLUSTER ? P.C : 1;
+    unsigned cr = 0;
+    if (CLUSTER) cr = cg::this_cluster().block_rank();
+    const long long ga = 2 * (long long)(blockIdx.x / C), gb = ga + 1;
+    if (ga * 32 >= pa_live_R(P.R, P.sc)) return;
+    const bool vb = gb < P.Gcap;
+    const int H = P.H;
+    const int y0 = (int)cr * H;
+    const int half = H * Lh;
+    uint32_t* abase = pop + ga * (long long)P.N;
+    uint32_t* bbase = pop + gb * (long long)P.N;
+    const int goff = y0 * Lh, gcol = P.N >> 1;
+    for (int c = 0; c < 2; ++c)
+        for (int i = tid; i < half; i += T)
+            tile2[c * half + i] = make_uint2(abase[c * gcol + goff + i], vb ? bbase[c * gcol + goff + i] : 0u);
+    const uint2* up_tile = tile2;
+    const uint2* dn_tile = tile2;
+    if (CLUSTER) {
+        cg::cluster_group cl = cg::this_cluster();
+        up_tile = cl.map_shared_rank(tile2, (cr + C - 1) % C);
+        dn_tile = cl.map_shared_rank(tile2, (cr + 1) % C);
+        cl.sync();
+    } else {
+        __syncthreads();
+    }
+    const int xh = tid & (Lh - 1), rb = tid >> LOG_LH;
+    const int rpt = half / T;
+    const int ya = rb * rpt;
+    const int dL = ((xh - 1) & (Lh - 1)) - xh, dR = ((xh + 1) & (Lh - 1)) - xh;
+    const int b0 = ya * Lh + xh;
+    const uint32_t quad_base = (uint32_t)(((y0 + ya) >> 2) * Lh + xh);
+    for (int it = 0; it < P.theta; ++it) {
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t c2 = 2u * (P.t0 + (uint32_t)it) + (uint32_t)c;
+            uint2* mine = tile2 + c * half + b0;
+            const uint2* oth = tile2 + (1 - c) * half + b0;
+            const int dA = c ? dR : dL, dB = c ? dL : dR;
+            uint32_t quad = quad_base;
+#pragma unroll 1
+            for (int k = 0; k < rpt; k += 4) {
+                const uint4 sa = pa_lcg_seeds(quad, (uint32_t)ga, c2, P.K);
+                const uint4 sb = pa_lcg_seeds(quad, (uint32_t)gb, c2, P.K);
+                const uint2 s0 = mine[0], s1 = mine[Lh], s2 = mine[2 * Lh], s3 = mine[3 * Lh];
+                const uint2 o0 = oth[0], o1 = oth[Lh], o2 = oth[2 * Lh], o3 = oth[3 * Lh];
+                const uint2 x0 = oth[dA], x1 = oth[Lh + dB], x2 = oth[2 * Lh + dA], x3 = oth[3 * Lh + dB];
+                uint2 oU, oD;
+                if (ya + k > 0) oU = oth[-Lh]; else oU = up_tile[(1 - c) * half + (H - 1) * Lh + xh];
+                if (ya + k + 4 < H) oD = oth[4 * Lh]; else oD = dn_tile[(1 - c) * half + xh];
+                uint2 f0, f1, f2, f3;
+                f0.x = pa_flip_mask_lcg<NOR>(s0.x, o0.x, x0.x, oU.x, o1.x, sa.x, P);
+                f1.x = pa_flip_mask_lcg<NOR>(s1.x, o1.x, x1.x, o0.x, o2.x, sa.y, P);
+                f2.x = pa_flip_mask_lcg<NOR>(s2.x, o2.x, x2.x, o1.x, o3.x, sa.z, P);
+                f3.x = pa_flip_mask_lcg<NOR>(s3.x, o3.x, x3.x, o2.x, oD.x, sa.w, P);
+                f0.y = pa_flip_mask_lcg<NOR>(s0.y, o0.y, x0.y, oU.y, o1.y, sb.x, P);
+                f1.y = pa_flip_mask_lcg<NOR>(s1.y, o1.y, x1.y, o0.y, o2.y, sb.y, P);
+                f2.y = pa_flip_mask_lcg<NOR>(s2.y, o2.y, x2.y, o1.y, o3.y, sb.z, P);
+                f3.y = pa_flip_mask_lcg<NOR>(s3.y, o3.y, x3.y, o2.y, oD.y, sb.w, P);
+                mine[0] = make_uint2(s0.x ^ f0.x, s0.y ^ f0.y);
+                mine[Lh] = make_uint2(s1.x ^ f1.x, s1.y ^ f1.y);
+                mine[2 * Lh] = make_uint2(s2.x ^ f2.x, s2.y ^ f2.y);
+                mine[3 * Lh] = make_uint2(s3.x ^ f3.x, s3.y ^ f3.y);
+                mine += 4 * Lh; oth += 4 * Lh; quad += Lh;
+            }
+            if (CLUSTER) cg::this_cluster().sync(); else __syncthreads();
+        }
+    }
+    for (int c = 0; c < 2; ++c)
+        for (int i = tid; i < half; i += T) {
+            const uint2 v = tile2[c * half + i];
+            abase[c * gcol + goff + i] = v.x;
+            if (vb) bbase[c * gcol + goff + i] = v.y;
+        }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Simple-cubic lattice (O16).  The same scheme one dimension up: a cluster of C CTAs owns a group, each CTA
 // stages Lz/C whole z-planes of both colours (rows r = z*Ly + y, H = Ly*Lz/C of them), and only the z-neighbours of a strip's
 // first and last plane live in the neighbouring CTA's shared memory.  Per word: six neighbour words, a bit-sliced count of the
@@ -765,6 +855,18 @@ static cudaError_t pa_sweep_dispatch_lcg_col(pa_handle* h, const SweepParams& P,
 
 static cudaError_t pa_sweep_dispatch_lcg(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
     const bool cl = P.C > 1;
+    if (h->sweep_kind == 1 && !h->has_j && pa_env_int("PA_LCG_P64", 0) == 1 && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG) &&
+        P.Lh >= 32 && P.Lh <= 128 && 2 * smem <= (size_t)224 * 1024) {
+        // p = 64 experiment: one CTA (cluster) per PAIR of groups, twice the shared memory
+        const unsigned grid2 = (unsigned)(((grid / P.C) + 1) / 2 * P.C);
+        switch (P.Lh) {
+#define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_lcg64_kernel<LOG, true, 4>, P, 2 * smem, grid2, true) \
+                                                  : pa_sweep_launch_k(h, pa_sweep_lcg64_kernel<LOG, false, 4>, P, 2 * smem, grid2, false);
+            PA_COL_CASE(5) PA_COL_CASE(6) PA_COL_CASE(7)
+#undef PA_COL_CASE
+            default: break;
+        }
+    }
     if (h->sweep_kind == 1 && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG) && P.Lh >= 32 && P.Lh <= 256) {
         if (h->has_j) return pa_sweep_dispatch_lcg_col<4, true>(h, P, smem, grid);
         switch (pa_env_int("PA_LCG_NOR", 4)) {       // tuning knob; every value gives the same bytes
@@ -823,7 +925,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     P.L = h->geom.Lx; P.Lh = h->geom.Lx / 2; P.Ly = h->geom.Ly; P.Lz = h->geom.Lz; P.N = h->N;
     P.C = h->sweep_C; P.H = h->geom.Ly * (h->geom.Lz / P.C);
-    P.jmask = nullptr;
+    P.jmask = nullptr; P.Gcap = h->G_cap;
     const size_t smem = (size_t)h->N * 4 / P.C;
     const unsigned grid = (unsigned)(G * P.C);
     const cudaError_t e = P.C > 1 ? pa_sweep_launch_k(h, pa_sweep3d_kernel<true>, P, smem, grid, true)
@@ -847,6 +949,7 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     const unsigned grid = (unsigned)(G * P.C);
     const int v = h->sweep_cmp;
     P.jmask = h->has_j ? h->jmask : nullptr;
+    P.Gcap = h->G_cap;
     const cudaError_t e = (h->has_j && h->rng_mode != PA_RNG_LCG) ? pa_sweep_dispatch_j(h, P, smem, grid)   // O15, Philox per spin
                         : h->rng_mode == PA_RNG_LCG ? pa_sweep_dispatch_lcg(h, P, smem, grid)
                         : v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)
