@@ -163,6 +163,8 @@ __device__ __forceinline__ void pa_measure_tail(uint32_t (&pe)[NPL], uint32_t (&
 //   sum_j (M_j/N)^4 in the TREE1024 order (O5, O8): the warp that finishes a group holds one replica per lane,
 //   so its __shfl_down tree IS the aligned-run-of-32 level; the run sums go to runsum[g], and the last CTA
 //   to finish (atomic ticket) does the tree over each 32 run sums and the sequential sum over 1024-blocks.
+// LOG_LH, LOG_LY >= 0: Lx/2 and Ly are these powers of two (cubes: shifts instead of two integer divisions per word); -1: any.
+template <int LOG_LH, int LOG_LY>
 __global__ void __launch_bounds__(256)
 pa_measure_generic_kernel(const uint32_t* __restrict__ pop, PaGeom geo, int N, long long R_cur,
                   int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
@@ -170,7 +172,7 @@ pa_measure_generic_kernel(const uint32_t* __restrict__ pop, PaGeom geo, int N, l
                   PaScalars* __restrict__ snap, int nlev) {
     const long long g = blockIdx.x;
     const uint32_t* base = pop + g * (long long)N;
-    const int Lh = geo.Lx >> 1, Ly = geo.Ly, Lz = geo.Lz, half = N >> 1;
+    const int Lh = LOG_LH >= 0 ? (1 << LOG_LH) : geo.Lx >> 1, Ly = LOG_LY >= 0 ? (1 << LOG_LY) : geo.Ly, Lz = geo.Lz, half = N >> 1;
     const int T = blockDim.x, tid = threadIdx.x;
     BitCounter cE, cM;
     cE.clear(); cM.clear();
@@ -183,8 +185,8 @@ pa_measure_generic_kernel(const uint32_t* __restrict__ pop, PaGeom geo, int N, l
             if (idx < N) {
                 int c = idx >= half ? 1 : 0;
                 int rem = idx - c * half;
-                int r = rem / Lh, xh = rem - r * Lh;          // row r = z*Ly + y (z = 0 on the square lattice)
-                int z = r / Ly, y = r - z * Ly;
+                int r = LOG_LH >= 0 ? (rem >> LOG_LH) : rem / Lh, xh = rem - r * Lh;          // row r = z*Ly + y (z = 0 on the square lattice)
+                int z = LOG_LY >= 0 ? (r >> LOG_LY) : r / Ly, y = r - z * Ly;
                 int p = (y + z + c) & 1;
                 const uint32_t* oth = base + (1 - c) * half;
                 s = base[idx];
@@ -344,8 +346,17 @@ int pa_launch_measure(pa_handle* h) {
     } else {
         int T = 256;
         while (T > 32 && T * 8 > h->N) T >>= 1;
-        pa_measure_generic_kernel<<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, Rarg, h->E, h->M, h->d_scal,
-                                                                    h->runsum, h->partials, h->has_j ? h->jmask : nullptr, h->snap_out, h->nlev);
+#define PA_MG_CASE(LOGH, LOGY) pa_measure_generic_kernel<LOGH, LOGY><<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, Rarg, \
+            h->E, h->M, h->d_scal, h->runsum, h->partials, h->has_j ? h->jmask : nullptr, h->snap_out, h->nlev)
+        const int cube = h->D == 3 && h->geom.Lx == h->geom.Ly && getenv("PA_MEASURE_GENERIC") == nullptr ? h->geom.Lx : 0;
+        switch (cube) {
+            case 8: PA_MG_CASE(2, 3); break;
+            case 16: PA_MG_CASE(3, 4); break;
+            case 32: PA_MG_CASE(4, 5); break;
+            case 64: PA_MG_CASE(5, 6); break;
+            default: PA_MG_CASE(-1, -1); break;
+        }
+#undef PA_MG_CASE
     }
     PA_CUDA(h, cudaGetLastError());
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));

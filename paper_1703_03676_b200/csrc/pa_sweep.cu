@@ -643,7 +643,9 @@ __device__ __forceinline__ uint32_t pa_flip_mask3d(uint32_t s, uint32_t n0, uint
     return U3 | (~g4 & U2) | (~g8 & U1) | ~g12;
 }
 
-template <bool CLUSTER>
+// LOG_LH, LOG_LY >= 0: Lx/2 and Ly are these powers of two (cubes 8^3 .. 64^3: the index arithmetic is shifts and masks);
+// -1: any even edges (two integer divisions per word).
+template <bool CLUSTER, int LOG_LH, int LOG_LY>
 __global__ void __launch_bounds__(256, 3)
 pa_sweep3d_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     extern __shared__ __align__(16) uint32_t tile[];   // [2][H][Lh], H = Ly * (Lz / C) rows
@@ -653,8 +655,8 @@ pa_sweep3d_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long g = blockIdx.x / C;
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // uniform per cluster
-    const int H = P.H, Lh = P.Lh, Lx = P.L, Ly = P.Ly;
-    const int Pz = H / Ly;                              // planes of this CTA
+    const int H = P.H, Lh = LOG_LH >= 0 ? (1 << LOG_LH) : P.Lh, Lx = 2 * Lh, Ly = LOG_LY >= 0 ? (1 << LOG_LY) : P.Ly;
+    const int Pz = LOG_LY >= 0 ? (H >> LOG_LY) : H / Ly;  // planes of this CTA
     const int z0 = (int)cr * Pz;
     const int half = H * Lh;
     uint32_t* gbase = pop + g * (long long)P.N;
@@ -694,8 +696,8 @@ pa_sweep3d_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
             const uint32_t* dn_oth = dn_tile + (1 - c) * half;
 #pragma unroll 1
             for (int w = tid; w < half; w += T) {
-                const int rl = w / Lh, xh = w - rl * Lh;
-                const int zl = rl / Ly, y = rl - zl * Ly;
+                const int rl = LOG_LH >= 0 ? (w >> LOG_LH) : w / Lh, xh = w - rl * Lh;
+                const int zl = LOG_LY >= 0 ? (rl >> LOG_LY) : rl / Ly, y = rl - zl * Ly;
                 const int z = z0 + zl;
                 const int p = (y + z + c) & 1;
                 const int in_plane = y * Lh + xh, pl = zl * plane;
@@ -928,8 +930,19 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     P.jmask = nullptr; P.Gcap = h->G_cap;
     const size_t smem = (size_t)h->N * 4 / P.C;
     const unsigned grid = (unsigned)(G * P.C);
-    const cudaError_t e = P.C > 1 ? pa_sweep_launch_k(h, pa_sweep3d_kernel<true>, P, smem, grid, true)
-                                  : pa_sweep_launch_k(h, pa_sweep3d_kernel<false>, P, smem, grid, false);
+    cudaError_t e = cudaErrorInvalidValue;
+    const bool cl = P.C > 1;
+    const int lx = P.L == P.Ly && pa_env_int("PA_SWEEP_KIND", 1) != 0 ? P.L : 0;        // cubes' fast index arithmetic (kind 0: generic)
+#define PA_3D_CASE(LOGH, LOGY) e = cl ? pa_sweep_launch_k(h, pa_sweep3d_kernel<true, LOGH, LOGY>, P, smem, grid, true) \
+                                      : pa_sweep_launch_k(h, pa_sweep3d_kernel<false, LOGH, LOGY>, P, smem, grid, false)
+    switch (lx) {
+        case 8: PA_3D_CASE(2, 3); break;
+        case 16: PA_3D_CASE(3, 4); break;
+        case 32: PA_3D_CASE(4, 5); break;
+        case 64: PA_3D_CASE(5, 6); break;
+        default: PA_3D_CASE(-1, -1); break;
+    }
+#undef PA_3D_CASE
     PA_CUDA(h, e);
     h->launches += 1;
     return PA_OK;

@@ -70,6 +70,23 @@ def test_box_run_every_step(monkeypatch, dims, R, C):
         assert np.allclose(rg[k], ro[k], rtol=REL, atol=1e-300), k
 
 
+def test_cube_generic_and_fast_index_arithmetic_agree(monkeypatch):
+    """Cubes of 8 .. 64 run on kernels whose index arithmetic is shifts and masks; PA_SWEEP_KIND=0 / PA_MEASURE_GENERIC=1 force the
+    any-edge kernels (integer divisions).  Same bytes, same energies."""
+    for L, R in ((8, 500), (16, 200), (32, 64)):
+        out = []
+        for generic in (False, True):
+            if generic:
+                monkeypatch.setenv("PA_SWEEP_KIND", "0"); monkeypatch.setenv("PA_MEASURE_GENERIC", "1")
+            else:
+                monkeypatch.delenv("PA_SWEEP_KIND", raising=False); monkeypatch.delenv("PA_MEASURE_GENERIC", raising=False)
+            g = pa.Population.box((L, L, L), R, 23)
+            g.sweep(0.2, 3)
+            E, M = g.energies()
+            out.append((g.get_words().tobytes(), E.tobytes(), M.tobytes()))
+        assert out[0] == out[1], L
+
+
 def test_box_adaptive_anneal_and_export():
     """The rest of the path on a box: adaptive step (bit-identical beta sequence), pa_anneal = single calls, spin and word
     export / import in the box's site order s = (z*Ly + y)*Lx + x."""
