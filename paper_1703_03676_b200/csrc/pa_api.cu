@@ -200,6 +200,7 @@ static int pa_create_impl(int D, PaGeom geom, int64_t R, uint64_t seed, void* de
     h->L = L; h->N = (int)Nsites; h->D = D; h->geom = geom; h->nlev = (int)nlev_;
     h->R_target = R; h->R_cur = R; h->R_cap = y.R_cap; h->G_cap = y.G_cap;
     h->seed = seed; h->keys = pa_make_keys(seed); h->rng_mode = PA_RNG_PHILOX; h->timing = PA_TIME_SWEEP;
+    { const char* e = getenv("PA_PDL"); h->pdl = (e && atoi(e) == 0) ? 0 : 1; }
     h->lnZ = (double)h->N * log(2.0);           // Z_{beta_0} = 2^N (L93)
     h->n_tiles_cap = y.tiles;
     int rc = PA_OK;
@@ -602,7 +603,10 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
         for (int i = 0; i < cs; ++i) {                               // O5: wtab[d] = exp(-(dbeta * (double)(4 d))), full level range
             const double dbeta = betas[s0 + i + 1] - betas[s0 + i];
             double* t = h_t + (size_t)i * tab;
-            for (int d = 0; d <= h->nlev; ++d) t[d] = exp(-(dbeta * (double)(4 * d)));
+            // the first step of the call is on the critical path (nothing is running yet) and its population is known on the
+            // host: only the levels it occupies are read; the later tables are built while the device works
+            const int dlast = (s0 + i == 0) ? (h->Emax - h->Emin) / 4 : h->nlev;
+            for (int d = 0; d <= dlast; ++d) t[d] = exp(-(dbeta * (double)(4 * d)));
         }
         if (cudaMemcpyAsync(d_t, h_t, (size_t)cs * tab * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = PA_ERR_CUDA; break; }
         h->dev_R = true;

@@ -181,6 +181,7 @@ struct pa_handle {
     bool dev_R;                         // inside pa_anneal: kernels read R and E_min from d_scal, grids cover the capacity
     cudaEvent_t ev_chunk[2];            // pa_anneal: completion of the chunk staged in buffer 0 / 1
     double* h_tabs; size_t h_tabs_bytes; // pinned staging for pa_anneal's weight tables and snapshots
+    int pdl;                            // 1: the step's kernels are launched with programmatic stream serialization
     int64_t launches;
     bool sweep_C_forced;
     uint32_t T12;            // third threshold of the cubic lattice (dE = 12), set by pa_sweep
@@ -195,6 +196,30 @@ struct pa_handle {
     } while (0)
 
 void pa_note_cuda_error(pa_handle* h, cudaError_t e, const char* what, const char* file, int line);
+
+// ------------------------------------------------------------------------------------------------
+// Programmatic dependent launch (sm_90+): the kernels of a temperature step form a chain tree -> plan -> copy -> sweep -> measure
+// in which every kernel needs its predecessor's output.  Launched with cudaLaunchAttributeProgrammaticStreamSerialization, a kernel
+// may be scheduled while its predecessor is still draining; it must then execute pa_pdl_wait() (griddepcontrol.wait: returns when
+// the predecessor grid has completed and its memory is visible) before it touches anything, and it lets ITS successor be scheduled
+// early with pa_pdl_launch().  On the launch-bound small populations this hides the launch latency between the five kernels.
+// Without the attribute both instructions do nothing.  h->pdl = 0 (environment PA_PDL=0) launches everything the classic way.
+// ------------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ void pa_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pa_pdl_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+static inline cudaError_t pa_launch(const pa_handle* h, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = h->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = h->pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+#endif
 
 // kernels' host launchers (each returns PA_OK / PA_ERR_CUDA and counts its launches in h->launches)
 int pa_launch_init(pa_handle* h);

@@ -170,6 +170,7 @@ pa_measure_generic_kernel(const uint32_t* __restrict__ pop, PaGeom geo, int N, l
                   int32_t* __restrict__ E, int32_t* __restrict__ M, PaScalars* __restrict__ sc,
                   double* __restrict__ runsum, double* __restrict__ blocksum, const uint8_t* __restrict__ jmask,
                   PaScalars* __restrict__ snap, int nlev) {
+    pa_pdl_wait(); pa_pdl_launch();
     const long long g = blockIdx.x;
     const uint32_t* base = pop + g * (long long)N;
     const int Lh = LOG_LH >= 0 ? (1 << LOG_LH) : geo.Lx >> 1, Ly = LOG_LY >= 0 ? (1 << LOG_LY) : geo.Ly, Lz = geo.Lz, half = N >> 1;
@@ -274,6 +275,7 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
     constexpr int S = pa_msr_strips(L), RS = L / S;                      // strips per group, rows per strip
     constexpr int NPE = pa_bits(16 * RS), NPM = pa_bits(8 * RS);         // planes per thread
     constexpr int NPW = NPE + 5;                                         // planes after the warp sum
+    pa_pdl_wait(); pa_pdl_launch();
     const long long g = blockIdx.x;
     const int tid = threadIdx.x, lane = tid & 31;
     const bool act = tid < S * QPR;
@@ -333,21 +335,22 @@ int pa_launch_measure(pa_handle* h) {
     h->scal_zeroed = false;
     const bool timed = (h->timing & PA_TIME_MEASURE) != 0;
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
+    cudaError_t le = cudaSuccess;
     const bool pow2 = h->D == 2 && (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
     if (pow2) {
 #define PA_MSR_CASE(LOG) case (8 << LOG): \
-        if (h->has_j) pa_measure_kernel<LOG, true><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
-            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, h->jm16, h->snap_out); \
-        else pa_measure_kernel<LOG, false><<<(unsigned)G, pa_msr_threads(8 << LOG), 0, h->stream>>>( \
-            h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, nullptr, h->snap_out); \
+        if (h->has_j) le = pa_launch(h, pa_measure_kernel<LOG, true>, dim3((unsigned)G), dim3(pa_msr_threads(8 << LOG)), 0, \
+            (const uint32_t*)h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, (const uint16_t*)h->jm16, h->snap_out); \
+        else le = pa_launch(h, pa_measure_kernel<LOG, false>, dim3((unsigned)G), dim3(pa_msr_threads(8 << LOG)), 0, \
+            (const uint32_t*)h->spins[h->cur], h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, (const uint16_t*)nullptr, h->snap_out); \
         break;
         switch (L) { PA_MSR_CASE(0) PA_MSR_CASE(1) PA_MSR_CASE(2) PA_MSR_CASE(3) PA_MSR_CASE(4) PA_MSR_CASE(5) default: break; }
 #undef PA_MSR_CASE
     } else {
         int T = 256;
         while (T > 32 && T * 8 > h->N) T >>= 1;
-#define PA_MG_CASE(LOGH, LOGY) pa_measure_generic_kernel<LOGH, LOGY><<<(unsigned)G, T, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, Rarg, \
-            h->E, h->M, h->d_scal, h->runsum, h->partials, h->has_j ? h->jmask : nullptr, h->snap_out, h->nlev)
+#define PA_MG_CASE(LOGH, LOGY) le = pa_launch(h, pa_measure_generic_kernel<LOGH, LOGY>, dim3((unsigned)G), dim3(T), 0, (const uint32_t*)h->spins[h->cur], \
+            h->geom, h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, h->has_j ? (const uint8_t*)h->jmask : (const uint8_t*)nullptr, h->snap_out, h->nlev)
         const int cube = h->D == 3 && h->geom.Lx == h->geom.Ly && getenv("PA_MEASURE_GENERIC") == nullptr ? h->geom.Lx : 0;
         switch (cube) {
             case 8: PA_MG_CASE(2, 3); break;
@@ -358,6 +361,7 @@ int pa_launch_measure(pa_handle* h) {
         }
 #undef PA_MG_CASE
     }
+    PA_CUDA(h, le);
     PA_CUDA(h, cudaGetLastError());
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));
     h->measure_timed = timed;

@@ -30,15 +30,38 @@ int pa_launch_init(pa_handle* h) {
 
 // a9 (Eq. 9; O9)
 // also O14 (L129): the microcanonical magnetisation sums A1[m] += |M_j|, A2[m] += M_j^2 (exact integers, order-free)
-__global__ void pa_hist_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, long long R, int N /* nlev */,
-                               uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ A1, unsigned long long* __restrict__ A2) {
-    for (long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x; j < R; j += (long long)gridDim.x * blockDim.x) {
+// Privatised per CTA (three global atomics per replica into a few hundred hot bins): a CTA of 1024 threads takes up to
+// PA_HIST_PER_CTA = 8192 replicas and accumulates the levels inside the window [m_min, m_min + PA_HIST_WIN) -- m_min from the
+// measure kernel's device scalars -- in shared memory with native 32-bit atomics: the count, sum |M| (< 2^18 * 2^13) and M^2 in
+// three 12-bit slices (M^2 < 2^36; each slice sum < 2^12 * 2^13), then flushes one global atomic per occupied level and sum.
+// A level outside the window (a population spanning more than 4 PA_HIST_WIN in energy) goes to global atomics directly.
+#define PA_HIST_WIN 2048
+#define PA_HIST_PER_CTA 8192
+__global__ void __launch_bounds__(1024)
+pa_hist_kernel(const int32_t* __restrict__ E, const int32_t* __restrict__ M, long long R, int N /* nlev */, const PaScalars* __restrict__ sc,
+               uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ A1, unsigned long long* __restrict__ A2) {
+    __shared__ uint32_t cnt[PA_HIST_WIN], s1[PA_HIST_WIN], q0[PA_HIST_WIN], q1[PA_HIST_WIN], q2[PA_HIST_WIN];
+    for (int b = threadIdx.x; b < PA_HIST_WIN; b += blockDim.x) { cnt[b] = 0u; s1[b] = 0u; q0[b] = 0u; q1[b] = 0u; q2[b] = 0u; }
+    __syncthreads();
+    const int m_lo = (int)(0xffffffffu - sc->mmin_inv);
+    const long long j0 = (long long)blockIdx.x * PA_HIST_PER_CTA, j1 = min(R, j0 + PA_HIST_PER_CTA);
+    for (long long j = j0 + threadIdx.x; j < j1; j += blockDim.x) {
         const int m = (E[j] + 2 * N) >> 2;
         const long long mj = M[j];
-        const unsigned long long a = (unsigned long long)(mj < 0 ? -mj : mj);
-        atomicAdd(&Hcur[m], 1u);
-        atomicAdd(&A1[m], a);
-        atomicAdd(&A2[m], a * a);
+        const unsigned long long a = (unsigned long long)(mj < 0 ? -mj : mj), a2 = a * a;
+        const int b = m - m_lo;
+        if (b >= 0 && b < PA_HIST_WIN) {
+            atomicAdd(&cnt[b], 1u); atomicAdd(&s1[b], (uint32_t)a);
+            atomicAdd(&q0[b], (uint32_t)(a2 & 0xfffu)); atomicAdd(&q1[b], (uint32_t)((a2 >> 12) & 0xfffu)); atomicAdd(&q2[b], (uint32_t)(a2 >> 24));
+        } else { atomicAdd(&Hcur[m], 1u); atomicAdd(&A1[m], a); atomicAdd(&A2[m], a2); }
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < PA_HIST_WIN; b += blockDim.x) {
+        const uint32_t c = cnt[b];
+        if (c) {
+            atomicAdd(&Hcur[m_lo + b], c); atomicAdd(&A1[m_lo + b], (unsigned long long)s1[b]);
+            atomicAdd(&A2[m_lo + b], (unsigned long long)q0[b] + ((unsigned long long)q1[b] << 12) + ((unsigned long long)q2[b] << 24));
+        }
     }
 }
 __global__ void pa_hist_fold_kernel(uint32_t* __restrict__ Hcur, unsigned long long* __restrict__ Hsum,
@@ -57,9 +80,8 @@ __global__ void pa_hist_fold_kernel(uint32_t* __restrict__ Hcur, unsigned long l
 }
 
 int pa_launch_hist(pa_handle* h, double beta) {
-    int blocks = (int)((h->R_cur + 255) / 256);
-    if (blocks > 1184) blocks = 1184;
-    pa_hist_kernel<<<blocks, 256, 0, h->stream>>>(h->E, h->M, h->R_cur, h->nlev, h->Hcur, h->A1, h->A2);
+    const long long blocks = (h->R_cur + PA_HIST_PER_CTA - 1) / PA_HIST_PER_CTA;
+    pa_hist_kernel<<<(unsigned)blocks, 1024, 0, h->stream>>>(h->E, h->M, h->R_cur, h->nlev, h->d_scal, h->Hcur, h->A1, h->A2);
     const double c = log((double)h->R_cur) - h->lnZ;
     pa_hist_fold_kernel<<<(h->nlev + 1 + 255) / 256, 256, 0, h->stream>>>(h->Hcur, h->Hsum, h->lnD, h->nlev, c, beta, h->e0);
     PA_CUDA(h, cudaGetLastError());

@@ -21,6 +21,7 @@ pa_tree_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
                unsigned long long* __restrict__ scan_state, int N, int e0) {
     __shared__ double run[32];
     __shared__ bool s_last;
+    pa_pdl_wait(); pa_pdl_launch();
     R = pa_live_R(R, sc);
     Emin = pa_live_Emin(Emin, sc, N, e0);
     const long long j = (long long)blockIdx.x * PA_TILE + threadIdx.x;
@@ -70,19 +71,17 @@ pa_tree_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
 
 int pa_launch_weights(pa_handle* h, int Emin, double* w_out) {
     const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
-    pa_tree_kernel<0><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab_cur ? h->wtab_cur : h->wtab, h->d_scal, h->dev_R ? -1 : h->R_cur,
-                                                    (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, w_out,
-                                                    h->partials, h->scan_state, h->nlev, h->e0);
-    PA_CUDA(h, cudaGetLastError());
+    PA_CUDA(h, pa_launch(h, pa_tree_kernel<0>, dim3(n), dim3(PA_TILE), 0, (const int32_t*)h->E, h->wtab_cur ? h->wtab_cur : (const double*)h->wtab,
+                         h->d_scal, (long long)(h->dev_R ? -1 : h->R_cur), (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, w_out,
+                         h->partials, h->scan_state, h->nlev, h->e0));
     h->launches += 1;
     return PA_OK;
 }
 
 int pa_launch_overlap(pa_handle* h, int Emin) {
     const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
-    pa_tree_kernel<1><<<n, PA_TILE, 0, h->stream>>>(h->E, h->wtab, h->d_scal, h->R_cur, (double)h->R_target, Emin, nullptr,
-                                                    h->partials, h->scan_state, h->nlev, h->e0);
-    PA_CUDA(h, cudaGetLastError());
+    PA_CUDA(h, pa_launch(h, pa_tree_kernel<1>, dim3(n), dim3(PA_TILE), 0, (const int32_t*)h->E, (const double*)h->wtab, h->d_scal,
+                         (long long)h->R_cur, (double)h->R_target, Emin, (double*)nullptr, h->partials, h->scan_state, h->nlev, h->e0));
     h->launches += 1;
     return PA_OK;
 }
@@ -102,6 +101,7 @@ pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
                uint32_t* __restrict__ r_out, uint32_t* __restrict__ o_out, uint32_t* __restrict__ parent,
                unsigned long long* __restrict__ state, int n_tiles, int N, int e0) {
     __shared__ uint32_t s_tile, s_warp[8], s_excl;
+    pa_pdl_wait(); pa_pdl_launch();
     R = pa_live_R(R, sc);
     Emin = pa_live_Emin(Emin, sc, N, e0);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -196,10 +196,9 @@ pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
 
 int pa_launch_plan(pa_handle* h, int Emin) {
     const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
-    pa_plan_kernel<<<n, 256, 0, h->stream>>>(h->E, h->wtab_cur ? h->wtab_cur : h->wtab, h->d_scal, h->dev_R ? -1 : h->R_cur,
-                                             (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, h->keys, h->k,
-                                             h->R_cap, h->r, h->o, h->parent, h->scan_state, n, h->nlev, h->e0);
-    PA_CUDA(h, cudaGetLastError());
+    PA_CUDA(h, pa_launch(h, pa_plan_kernel, dim3(n), dim3(256), 0, (const int32_t*)h->E, h->wtab_cur ? h->wtab_cur : (const double*)h->wtab,
+                         h->d_scal, (long long)(h->dev_R ? -1 : h->R_cur), (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, h->keys, h->k,
+                         (long long)h->R_cap, h->r, h->o, h->parent, h->scan_state, n, h->nlev, h->e0));
     h->launches += 1;
     return PA_OK;
 }
@@ -262,6 +261,7 @@ pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, con
     __shared__ int nwin;
     const long long g = blockIdx.x;
     const int tid = threadIdx.x;
+    pa_pdl_wait(); pa_pdl_launch();
     // R_new is read on the device: the launch does not wait for the host to see it, the grid covers the
     // capacity and groups past the new population exit.  R_new > R_cap is the PA_ERR_CAPACITY case: nothing
     // of the live population is touched (dst is the spare buffer) and the host discards the copy.
@@ -334,10 +334,9 @@ int pa_launch_copy(pa_handle* h) {
     // small populations: split a group's words over several CTAs to fill the GPU
     while (G * gy < 592 && gy * 128 * 2 <= chunks) gy *= 2;
     dim3 grid((unsigned)G, (unsigned)gy, 1);
-    pa_copy_kernel<<<grid, 128, 0, h->stream>>>(h->spins[h->cur], h->spins[1 - h->cur], h->parent, h->d_scal, h->R_cap, h->N,
-                                                h->dev_R ? 1 : 0);
+    PA_CUDA(h, pa_launch(h, pa_copy_kernel, grid, dim3(128), 0, (const uint32_t*)h->spins[h->cur], h->spins[1 - h->cur],
+                         (const uint32_t*)h->parent, h->d_scal, (long long)h->R_cap, h->N, h->dev_R ? 1 : 0));
     h->scal_zeroed = h->dev_R;
-    PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
 }

@@ -197,6 +197,7 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long g = blockIdx.x / C;
+    pa_pdl_wait(); pa_pdl_launch();
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H, Lh = P.Lh, L = P.L;
     const int y0 = (int)cr * H;
@@ -311,6 +312,7 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long g = blockIdx.x / C;
+    pa_pdl_wait(); pa_pdl_launch();
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H;
     const int y0 = (int)cr * H;
@@ -404,6 +406,7 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long g = blockIdx.x / C;
+    pa_pdl_wait(); pa_pdl_launch();
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H;
     const int y0 = (int)cr * H;
@@ -501,6 +504,7 @@ pa_sweep_lcg64_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long ga = 2 * (long long)(blockIdx.x / C), gb = ga + 1;
+    pa_pdl_wait(); pa_pdl_launch();
     if (ga * 32 >= pa_live_R(P.R, P.sc)) return;
     const bool vb = gb < P.Gcap;
     const int H = P.H;
@@ -654,6 +658,7 @@ pa_sweep3d_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
     const long long g = blockIdx.x / C;
+    pa_pdl_wait(); pa_pdl_launch();
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // uniform per cluster
     const int H = P.H, Lh = LOG_LH >= 0 ? (1 << LOG_LH) : P.Lh, Lx = 2 * Lh, Ly = LOG_LY >= 0 ? (1 << LOG_LY) : P.Ly;
     const int Pz = LOG_LY >= 0 ? (H >> LOG_LY) : H / Ly;  // planes of this CTA
@@ -833,13 +838,15 @@ static cudaError_t pa_sweep_launch_k(pa_handle* h, Kern kern, const SweepParams&
     cfg.blockDim = dim3((unsigned)h->sweep_T, 1, 1);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = h->stream;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = cluster ? (unsigned)P.C : 1u;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;       // see pa_common.cuh
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = h->pdl ? 2 : 1;
     return cudaLaunchKernelEx(&cfg, kern, h->spins[h->cur], P);
 }
 
