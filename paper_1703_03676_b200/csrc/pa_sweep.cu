@@ -29,6 +29,8 @@ struct SweepParams {
     const PaScalars* sc;
     long long Gcap;                  // groups the population buffer holds (p = 64 experiment: the second group of a pair may not exist)
     const uint8_t* jmask;            // O15: per resident word, bit k = bond to neighbour k (same, x, up, down) has J = -1; NULL = ferromagnet
+    long long n_main;                // column-walk kernels without clusters, mixed launch (pa_sweep_pick_C): CTAs 0 .. n_main-1 own a whole group each, every
+                                     // later group is shared by four lane-split CTAs; -1: uniform launch
 };
 
 // m = 2*m + (x >= T).  "sub.cc" leaves the hardware carry of x + ~T + 1 in CC.CF, i.e. NOT borrow, and
@@ -180,6 +182,27 @@ __device__ __forceinline__ uint32_t pa_flip_mask_lcg(uint32_t s, uint32_t n0, ui
     return U2 | (lt4 & (U1 | lt8));                                    // u >= 2, or x < T4 and (u >= 1 or x < T8)
 }
 
+// Lane-split CTAs (see pa_flip_mask_part): the eight lanes 8 sub + 7 ... 8 sub of the word take the LCG outputs number
+// 25 - 8 sub ... 32 - 8 sub (O11: output n goes to lane 32 - n), reached by one jump r <- A^n r + C (A^n - 1)/(A - 1), n = 24 - 8 sub.
+__host__ __device__ constexpr uint32_t pa_lcg_jump_mul(int n) { uint32_t a = 1u; for (int i = 0; i < n; ++i) a *= PA_LCG_A; return a; }
+__host__ __device__ constexpr uint32_t pa_lcg_jump_add(int n) { uint32_t c = 0u; for (int i = 0; i < n; ++i) c = c * PA_LCG_A + PA_LCG_C; return c; }
+__device__ __forceinline__ uint32_t pa_flip_mask_lcg_part(uint32_t s, uint32_t n0, uint32_t n1, uint32_t n2, uint32_t n3,
+                                                          uint32_t r, uint32_t jmul, uint32_t jadd, uint32_t sh, const SweepParams& P) {
+    uint32_t a0 = s ^ n0, a1 = s ^ n1, a2 = s ^ n2, a3 = s ^ n3;
+    uint32_t U1 = a0 | a1 | a2 | a3;
+    uint32_t U2 = (a0 & a1) | (a2 & a3) | ((a0 ^ a1) & (a2 ^ a3));
+    r = r * jmul + jadd;
+    uint32_t g4 = 0, g8 = 0;
+#pragma unroll
+    for (int b = 7; b >= 0; --b) {
+        r = pa_lcg_step(r);
+        pa_shift_in_ge(g4, r, P.T4, P.two);
+        pa_shift_in_ge(g8, r, P.T8, P.two);
+    }
+    const uint32_t acc = ~g4 & ((U1 >> sh) | ~g8);
+    return (((U2 >> sh) | acc) & 0xffu) << sh;
+}
+
 // The four LCG seeds of a quad of rows (y & ~3 .. +3) in column xh of one sub-lattice: one Philox call (O11).
 __device__ __forceinline__ uint4 pa_lcg_seeds(uint32_t quad, uint32_t g, uint32_t c2, const PhiloxKeys& K) {
     return pa_philox(quad, g, c2, PA_TAG_LCG, K);
@@ -289,6 +312,136 @@ pa_sweep_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// Lane-split CTAs.  The 32 replicas of a word are independent, so a group can be shared out by LANES instead of by rows: S CTAs
+// (on S different SMs) each stage the whole group but advance only the 32/S lanes of byte(s) `sub` of every word -- the 8/S
+// Philox calls i = sub*8/S ... of the word's eight (lanes 4i .. 4i+3, O1) -- and write back only those bytes.  No halo, no cluster
+// barrier, no atomics; the price is that rounds 1-3 are shared by fewer calls (1 + 2 (NC+1) + 14 NC wide multiplies for NC calls:
+// 35 x 4 instead of 131) and that the neighbour logic is repeated per CTA.  Used where whole groups cannot fill the SMs: small
+// populations on the generic path (cfg1: 32 groups -> 128 CTAs), and the last, incomplete round of a medium population on the
+// column-walk path (pa_sweep_pick_C).
+// ------------------------------------------------------------------------------------------------
+template <int NC>
+__device__ __forceinline__ uint32_t pa_flip_mask_part(uint32_t s, uint32_t n0, uint32_t n1, uint32_t n2, uint32_t n3,
+                                                      uint32_t site, uint32_t c0base, uint32_t lo1u, uint32_t i0,
+                                                      const SweepParams& P) {
+    uint32_t a0 = s ^ n0, a1 = s ^ n1, a2 = s ^ n2, a3 = s ^ n3;
+    uint32_t U1 = a0 | a1 | a2 | a3;
+    uint32_t U2 = (a0 & a1) | (a2 & a3) | ((a0 ^ a1) & (a2 ^ a3));
+    uint32_t x0[NC], x1[NC], x2[NC], x3[NC];
+    uint32_t hi0, lo0;
+    pa_mulhilo(PA_PHILOX_M0, site, hi0, lo0);
+    const uint32_t c2w = hi0 ^ PA_TAG_SWEEP ^ P.K.k1[0];
+    const uint32_t c3w = lo0;
+    uint32_t hi1w, lo1w;
+    pa_mulhilo(PA_PHILOX_M1, c2w, hi1w, lo1w);
+    const uint32_t c0w = hi1w ^ lo1u ^ P.K.k0[1];
+    const uint32_t c1w = lo1w;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+        uint32_t h, l;
+        pa_mulhilo(PA_PHILOX_M0, c0base ^ (i0 + (uint32_t)i), h, l);
+        x2[i] = h ^ c3w ^ P.K.k1[1];
+        x3[i] = l;
+    }
+    uint32_t hi0w, lo0w;
+    pa_mulhilo(PA_PHILOX_M0, c0w, hi0w, lo0w);
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {
+        uint32_t h, l;
+        pa_mulhilo(PA_PHILOX_M1, x2[i], h, l);
+        x0[i] = h ^ c1w ^ P.K.k0[2];
+        x1[i] = l;
+        x2[i] = hi0w ^ x3[i] ^ P.K.k1[2];
+        x3[i] = lo0w;
+    }
+#pragma unroll
+    for (int r = 3; r < 10; ++r) {
+#pragma unroll
+        for (int i = 0; i < NC; ++i) {
+            uint32_t h0, l0, h1, l1;
+            pa_mulhilo(PA_PHILOX_M0, x0[i], h0, l0);
+            pa_mulhilo(PA_PHILOX_M1, x2[i], h1, l1);
+            x0[i] = h1 ^ x1[i] ^ P.K.k0[r];
+            x1[i] = l1;
+            x2[i] = h0 ^ x3[i] ^ P.K.k1[r];
+            x3[i] = l0;
+        }
+    }
+    uint32_t g4 = 0, g8 = 0;                   // bit 4i+q (relative to lane 4 i0) = (x >= T), most significant first
+#pragma unroll
+    for (int i = NC - 1; i >= 0; --i) {
+        const uint32_t xs[4] = {x0[i], x1[i], x2[i], x3[i]};
+#pragma unroll
+        for (int q = 3; q >= 0; --q) {
+            pa_shift_in_ge(g4, xs[q], P.T4, P.two);
+            pa_shift_in_ge(g8, xs[q], P.T8, P.two);
+        }
+    }
+    constexpr uint32_t LM = NC == 8 ? 0xffffffffu : ((1u << (4 * (NC & 7))) - 1u);
+    const uint32_t sh = 4u * i0;
+    const uint32_t acc = ~g4 & ((U1 >> sh) | ~g8);
+    return (((U2 >> sh) | acc) & LM) << sh;
+}
+
+// write back the lanes of lane block `sub` (of S) of n words: byte / halfword stores, little-endian lane order
+template <int S>
+__device__ __forceinline__ void pa_store_lanes(uint32_t* gdst, const uint32_t* src, int n, int sub, int tid, int T) {
+    if (S == 4) {
+        uint8_t* d = reinterpret_cast<uint8_t*>(gdst) + sub;
+        for (int i = tid; i < n; i += T) d[4 * i] = (uint8_t)(src[i] >> (8 * sub));
+    } else {
+        uint16_t* d = reinterpret_cast<uint16_t*>(gdst) + sub;
+        for (int i = tid; i < n; i += T) d[2 * i] = (uint16_t)(src[i] >> (16 * sub));
+    }
+}
+
+template <int S>
+__global__ void __launch_bounds__(256)
+pa_sweep_split_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
+    constexpr int NC = 8 / S;
+    extern __shared__ __align__(16) uint32_t tile[];   // [2][L][Lh]: the whole group (only this CTA's lanes are kept current)
+    const int T = blockDim.x, tid = threadIdx.x;
+    const long long g = blockIdx.x / S;
+    const int sub = blockIdx.x % S;
+    pa_pdl_wait(); pa_pdl_launch();
+    if (g * 32 >= pa_live_R(P.R, P.sc)) return;
+    const int Lh = P.Lh, L = P.L, half = P.N >> 1;
+    uint32_t* gbase = pop + g * (long long)P.N;
+    for (int i = tid; i < P.N; i += T) tile[i] = gbase[i];
+    __syncthreads();
+    const uint32_t g8 = (uint32_t)(8 * g);
+    for (int it = 0; it < P.theta; ++it) {
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t c2 = 2u * (P.t0 + (uint32_t)it) + (uint32_t)c;
+            uint32_t hi1u, lo1u;
+            pa_mulhilo(PA_PHILOX_M1, c2, hi1u, lo1u);
+            const uint32_t c0base = hi1u ^ P.K.k0[0] ^ g8;
+            uint32_t* mine = tile + c * half;
+            const uint32_t* oth = tile + (1 - c) * half;
+            int y = tid / Lh, xh = tid % Lh;
+            const int dy = T / Lh, dx = T % Lh;
+#pragma unroll 1
+            for (int w = tid; w < half; w += T) {
+                const int p = (y + c) & 1;
+                const int xh2 = p ? (xh + 1 == Lh ? 0 : xh + 1) : (xh == 0 ? Lh - 1 : xh - 1);
+                const uint32_t s = mine[w];
+                const uint32_t nS = oth[w];
+                const uint32_t nX = oth[w - xh + xh2];
+                const uint32_t nU = oth[(y == 0 ? L - 1 : y - 1) * Lh + xh];
+                const uint32_t nD = oth[(y + 1 == L ? 0 : y + 1) * Lh + xh];
+                const uint32_t site = (uint32_t)(y * L + 2 * xh + p);
+                mine[w] = s ^ pa_flip_mask_part<NC>(s, nS, nX, nU, nD, site, c0base, lo1u, (uint32_t)(sub * NC), P);
+                xh += dx; y += dy;
+                if (xh >= Lh) { xh -= Lh; y += 1; }
+            }
+            __syncthreads();
+        }
+    }
+    pa_store_lanes<S>(gbase, tile, P.N, sub, tid, T);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Column-walk variant for power-of-two L >= 64 (all of BASELINE.json's configs but L = 16).
 // A thread owns one column xh of the strip and walks down `rpt` consecutive rows, two rows per
 // iteration (the two rows have opposite x-parity, so the pair is the natural unit).  Every shared-memory
@@ -311,7 +464,12 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     const int C = CLUSTER ? P.C : 1;
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
-    const long long g = blockIdx.x / C;
+    long long g = blockIdx.x / C;
+    int sub = -1;                                      // >= 0: this CTA advances only the lanes of byte `sub` of its group (lane-split CTAs)
+    if (!CLUSTER && P.n_main >= 0 && g >= P.n_main) {  // mixed launch: n_main whole groups, then four CTAs per remaining group
+        sub = (int)((g - P.n_main) & 3);
+        g = P.n_main + ((g - P.n_main) >> 2);
+    }
     pa_pdl_wait(); pa_pdl_launch();
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H;
@@ -371,6 +529,9 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                     f1 = pa_flip_mask<CMP>(s1, pa_jx(nS1, j1, 0), pa_jx(nX1, j1, 1), pa_jx(nS0, j1, 2), pa_jx(nD1, j1, 3),
                                            site + (uint32_t)(2 * Lh + 1 - 2 * c), c0base, lo1u, P);
                     jm += 2 * Lh;
+                } else if (!CLUSTER && sub >= 0) {
+                    f0 = pa_flip_mask_part<2>(s0, nS0, nX0, nU0, nS1, site, c0base, lo1u, 2u * (uint32_t)sub, P);
+                    f1 = pa_flip_mask_part<2>(s1, nS1, nX1, nS0, nD1, site + (uint32_t)(2 * Lh + 1 - 2 * c), c0base, lo1u, 2u * (uint32_t)sub, P);
                 } else {
                     f0 = pa_flip_mask<CMP>(s0, nS0, nX0, nU0, nS1, site, c0base, lo1u, P);
                     f1 = pa_flip_mask<CMP>(s1, nS1, nX1, nS0, nD1, site + (uint32_t)(2 * Lh + 1 - 2 * c), c0base, lo1u, P);
@@ -383,6 +544,10 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
         }
     }
 
+    if (!CLUSTER && sub >= 0) {                        // only this CTA's lanes are current
+        for (int c = 0; c < 2; ++c) pa_store_lanes<4>(gbase + c * gcol + goff, tile + c * half, half, sub, tid, T);
+        return;
+    }
     for (int c = 0; c < 2; ++c) {
         uint4* dst = reinterpret_cast<uint4*>(gbase + c * gcol + goff);
         const uint4* src = reinterpret_cast<const uint4*>(tile + c * half);
@@ -405,7 +570,12 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     const int C = CLUSTER ? P.C : 1;
     unsigned cr = 0;
     if (CLUSTER) cr = cg::this_cluster().block_rank();
-    const long long g = blockIdx.x / C;
+    long long g = blockIdx.x / C;
+    int sub = -1;                                      // >= 0: this CTA advances only the lanes of byte `sub` of its group (lane-split CTAs)
+    if (!CLUSTER && P.n_main >= 0 && g >= P.n_main) {  // mixed launch: n_main whole groups, then four CTAs per remaining group
+        sub = (int)((g - P.n_main) & 3);
+        g = P.n_main + ((g - P.n_main) >> 2);
+    }
     pa_pdl_wait(); pa_pdl_launch();
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H;
@@ -436,6 +606,9 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     const int dL = ((xh - 1) & (Lh - 1)) - xh, dR = ((xh + 1) & (Lh - 1)) - xh;
     const int b0 = ya * Lh + xh;
     const uint32_t quad_base = (uint32_t)(((y0 + ya) >> 2) * Lh + xh);
+    // lane-split CTA: skip the 24 - 8 sub LCG outputs that belong to the lanes above this CTA's byte
+    const uint32_t jmul = sub == 0 ? pa_lcg_jump_mul(24) : sub == 1 ? pa_lcg_jump_mul(16) : sub == 2 ? pa_lcg_jump_mul(8) : 1u;
+    const uint32_t jadd = sub == 0 ? pa_lcg_jump_add(24) : sub == 1 ? pa_lcg_jump_add(16) : sub == 2 ? pa_lcg_jump_add(8) : 0u;
     for (int it = 0; it < P.theta; ++it) {
 #pragma unroll 1
         for (int c = 0; c < 2; ++c) {
@@ -463,6 +636,11 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                     f2 = pa_flip_mask_lcg<NOR>(s2, pa_jx(o2, j2, 0), pa_jx(x2, j2, 1), pa_jx(o1, j2, 2), pa_jx(o3, j2, 3), sd.z, P);
                     f3 = pa_flip_mask_lcg<NOR>(s3, pa_jx(o3, j3, 0), pa_jx(x3, j3, 1), pa_jx(o2, j3, 2), pa_jx(oD, j3, 3), sd.w, P);
                     jm += 4 * Lh;
+                } else if (!CLUSTER && sub >= 0) {
+                    f0 = pa_flip_mask_lcg_part(s0, o0, x0, oU, o1, sd.x, jmul, jadd, 8u * (uint32_t)sub, P);
+                    f1 = pa_flip_mask_lcg_part(s1, o1, x1, o0, o2, sd.y, jmul, jadd, 8u * (uint32_t)sub, P);
+                    f2 = pa_flip_mask_lcg_part(s2, o2, x2, o1, o3, sd.z, jmul, jadd, 8u * (uint32_t)sub, P);
+                    f3 = pa_flip_mask_lcg_part(s3, o3, x3, o2, oD, sd.w, jmul, jadd, 8u * (uint32_t)sub, P);
                 } else {
                     f0 = pa_flip_mask_lcg<NOR>(s0, o0, x0, oU, o1, sd.x, P);
                     f1 = pa_flip_mask_lcg<NOR>(s1, o1, x1, o0, o2, sd.y, P);
@@ -479,6 +657,10 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
         }
     }
 
+    if (!CLUSTER && sub >= 0) {                        // only this CTA's lanes are current
+        for (int c = 0; c < 2; ++c) pa_store_lanes<4>(gbase + c * gcol + goff, tile + c * half, half, sub, tid, T);
+        return;
+    }
     for (int c = 0; c < 2; ++c) {
         uint4* dst = reinterpret_cast<uint4*>(gbase + c * gcol + goff);
         const uint4* src = reinterpret_cast<const uint4*>(tile + c * half);
@@ -811,7 +993,17 @@ int pa_sweep_configure(pa_handle* h) {
 // makes the work items smaller at a measured cluster cost (C = 2: 0.97; C = 4: 0.93, 0.85 when a thread is left with one row
 // pair; C = 8: 0.85).  The earlier "waves of resident CTAs" model mispredicted L = 128 at R = 50 000 (chose C = 4: 1 536
 // updates/ns; C = 1: 1 644).
-static int pa_sweep_pick_C(const pa_handle* h, int64_t G) {
+static double pa_cluster_cost(int C, int rows_per_thread) {
+    return C == 1 ? 1.0 : C == 2 ? 0.97 : C == 4 ? (rows_per_thread >= 4 ? 0.93 : 0.85) : 0.85;
+}
+
+// Returns the cluster size; *n_main >= 0 selects a MIXED launch without clusters: CTAs 0 .. n_main-1 own a whole group each and
+// fill floor(G/148) complete rounds of the 148 SMs; every remaining group -- which would otherwise occupy a round of its own on a
+// fraction of the SMs -- is shared by four lane-split CTAs (pa_flip_mask_part), scheduled last by block order (cfg2: 625 groups =
+// 4 rounds of 148 + 33 groups in lane quarters instead of 9 rounds of half-groups).  Needs a whole group in one CTA (C_min = 1,
+// i.e. L <= 128).  PA_SWEEP_MIXED=0 switches it off.
+static int pa_sweep_pick_C(const pa_handle* h, int64_t G, long long* n_main) {
+    *n_main = -1;
     const int Cmin = h->sweep_C;
     if (h->sweep_C_forced || h->sweep_kind != 1) return Cmin;
     const int L = h->L;
@@ -822,10 +1014,20 @@ static int pa_sweep_pick_C(const pa_handle* h, int64_t G) {
         if (!pa_col_ok(L, C, h->sweep_T, h->rng_mode)) break;
         const int rows_per_thread = (L / C) * (L / 2) / h->sweep_T;
         const double per_sm = (double)G * C / S;
-        const double cost = C == 1 ? 1.0 : C == 2 ? 0.97 : C == 4 ? (rows_per_thread >= 4 ? 0.93 : 0.85) : 0.85;
-        const double eff = per_sm / ceil(per_sm) * cost * (C == Cmin ? 1.0 : 0.995);   // ties go to the smaller cluster
+        const double eff = per_sm / ceil(per_sm) * pa_cluster_cost(C, rows_per_thread) * (C == Cmin ? 1.0 : 0.995);   // ties go to the smaller cluster
         if (eff > best) { best = eff; bestC = C; }
     }
+    if (Cmin != 1 || h->has_j || pa_env_int("PA_SWEEP_MIXED", 1) == 0 || !pa_col_ok(L, 1, h->sweep_T, h->rng_mode)) return bestC;
+    if (h->rng_mode == PA_RNG_LCG && pa_env_int("PA_LCG_P64", 0) == 1) return bestC;
+    // inside pa_anneal the grid covers the capacity; the live population is about the target
+    const int64_t G_live = h->dev_R ? (h->R_target + 31) / 32 : G;
+    const int64_t rounds = G_live / 148;
+    const int64_t Gm = rounds * 148, Gt = G_live - Gm;
+    if (rounds < 1 || Gt <= 0) return bestC;
+    // a lane quarter costs about 0.3 of a whole group (35 instead of 131/4 wide multiplies, repeated neighbour logic)
+    const double time = (double)rounds + ceil((double)Gt * 4 / S) * 0.30;
+    const double eff = ((double)G_live / S) / time * 0.985;         // must beat the uniform launch by 1.5 % to be taken
+    if (eff > best) { bestC = 1; *n_main = Gm; }
     return bestC;
 }
 
@@ -934,7 +1136,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     P.L = h->geom.Lx; P.Lh = h->geom.Lx / 2; P.Ly = h->geom.Ly; P.Lz = h->geom.Lz; P.N = h->N;
     P.C = h->sweep_C; P.H = h->geom.Ly * (h->geom.Lz / P.C);
-    P.jmask = nullptr; P.Gcap = h->G_cap;
+    P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1;
     const size_t smem = (size_t)h->N * 4 / P.C;
     const unsigned grid = (unsigned)(G * P.C);
     cudaError_t e = cudaErrorInvalidValue;
@@ -955,6 +1157,31 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     return PA_OK;
 }
 
+// Lane split S (CTAs per group) for a small population on the generic path, 0 = one CTA per group: the largest S in {2, 4} that
+// still gives every CTA an SM of its own (measured on B200, sweep of theta = 10: L = 16, R = 1000 22.2 -> 14.7 us with S = 4,
+// L = 32, R = 1000 45.5 -> 23.2 us; with more groups than SMs the split only adds work: L = 16, R = 10 000 35.8 -> 39.5 us).
+// PA_SWEEP_SPLIT forces 0/2/4.
+static int pa_sweep_pick_split(const pa_handle* h, int64_t G) {
+    if (h->D != 2 || h->rng_mode != PA_RNG_PHILOX || h->has_j || h->sweep_kind != 0 || h->sweep_C != 1 || h->sweep_C_forced) return 0;
+    if ((size_t)h->N * 4 > (size_t)64 * 1024) return 0;
+    const int force = pa_env_int("PA_SWEEP_SPLIT", -1);
+    if (force == 0 || force == 2 || force == 4) return force;
+    return G * 4 <= 160 ? 4 : G * 2 <= 160 ? 2 : 0;
+}
+
+static int pa_launch_sweep_split(pa_handle* h, SweepParams& P, int S, int64_t G) {
+    P.C = 1; P.H = h->L;
+    const int half = h->N / 2;
+    int T = (half + 31) / 32 * 32;
+    if (T > 256) T = 256;
+    const size_t smem = (size_t)h->N * 4;
+    void (*kern)(uint32_t*, const SweepParams) = S == 4 ? pa_sweep_split_kernel<4> : pa_sweep_split_kernel<2>;
+    PA_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    PA_CUDA(h, pa_launch(h, kern, dim3((unsigned)(G * S)), dim3((unsigned)T), smem, h->spins[h->cur], P));
+    h->launches += 1;
+    return PA_OK;
+}
+
 int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     if (theta == 0) return PA_OK;
     if (h->D == 3) return pa_launch_sweep_3d(h, T4, T8, theta);
@@ -964,9 +1191,14 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     P.t0 = h->t; P.theta = theta; P.two = 2u;
     const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
-    P.L = h->L; P.Lh = h->L / 2; P.C = pa_sweep_pick_C(h, G); P.H = h->L / P.C; P.N = h->N;
+    if (const int S = pa_sweep_pick_split(h, h->dev_R ? (h->R_target + 31) / 32 : G)) {   // pa_anneal: the grid covers the capacity, the population is about the target
+        P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1;
+        return pa_launch_sweep_split(h, P, S, G);
+    }
+    P.L = h->L; P.Lh = h->L / 2; P.C = pa_sweep_pick_C(h, G, &P.n_main); P.H = h->L / P.C; P.N = h->N;
     const size_t smem = (size_t)P.H * h->L * 4;
-    const unsigned grid = (unsigned)(G * P.C);
+    // mixed launch: n_main whole groups, then four lane-split CTAs per remaining group
+    const unsigned grid = P.n_main >= 0 ? (unsigned)(P.n_main + 4 * (G - P.n_main)) : (unsigned)(G * P.C);
     const int v = h->sweep_cmp;
     P.jmask = h->has_j ? h->jmask : nullptr;
     P.Gcap = h->G_cap;

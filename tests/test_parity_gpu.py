@@ -372,3 +372,53 @@ def test_sweep_threshold_extremes():
         g.sweep(0.2, 1); o.sweep(0.2, 1)
         g.sweep(beta, 3); o.sweep(beta, 3)
         assert_same_state(g, o)
+
+
+@pytest.mark.parametrize("L,R", [(16, 1000), (6, 70), (10, 161), (32, 100), (4, 33)])
+def test_sweep_lane_split_kernel(monkeypatch, L, R):
+    """Small populations on the generic path: S = 2, 4 lane-split CTAs per group, each running 8/S of every word's Philox calls
+    and writing back only its own bytes of the words -- the same bytes as one CTA per group and as the oracle (thresholds at
+    beta = 0 and at a T8 of 0 included; R = 1000 at L = 16 is configs[0]'s population, R = 161 has a ragged last word)."""
+    seed = 4000 + L
+    o = po.Oracle(L, R, seed)
+    plan = [(0.0, 1), (0.3, 2), (0.4406868, 3), (3.0, 1), (0.7, 2)]
+    for beta, theta in plan:
+        o.sweep(beta, theta)
+    want, (Eo, Mo) = o.get_spins(), o.energies()
+    for split in ("0", "2", "4", None):
+        monkeypatch.delenv("PA_SWEEP_SPLIT", raising=False)
+        if split is not None:
+            monkeypatch.setenv("PA_SWEEP_SPLIT", split)
+        g = pa.Population(L, R, seed)
+        for beta, theta in plan:
+            g.sweep(beta, theta)
+        assert np.array_equal(g.get_spins(), want), split
+        Eg, Mg = g.energies()
+        assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo), split
+        words = g.get_words()
+        if R % 32:
+            assert np.all(words[-1] >> np.uint32(R % 32) == 0)
+
+
+@pytest.mark.parametrize("L,R,rng", [(64, 5300, 0), (64, 5300, 1), (64, 9500, 0), (128, 4800, 0), (128, 4800, 1)])
+def test_sweep_mixed_launch(monkeypatch, L, R, rng):
+    """Medium populations on the column-walk kernels: whole groups (one per CTA) fill complete rounds of the 148 SMs and the
+    remaining groups are split over the CTAs of a cluster -- one launch, the same bytes as the uniform launch and the oracle.
+    Sampled slots span the whole groups, the first and last split group and the ragged last word."""
+    seed = 5000 + L + rng
+    o = po.Oracle(L, R, seed)
+    o.set_rng_mode(po.RNG_LCG if rng else po.RNG_PHILOX)
+    o.sweep(0.35, 1); o.sweep(0.45, 2)
+    want = o.get_spins()
+    Eo, Mo = o.energies()
+    outs = []
+    for mixed in ("1", "0"):
+        monkeypatch.setenv("PA_SWEEP_MIXED", mixed)
+        g = pa.Population(L, R, seed)
+        g.set_rng_mode(pa.PA_RNG_LCG if rng else pa.PA_RNG_PHILOX)
+        g.sweep(0.35, 1); g.sweep(0.45, 2)
+        Eg, Mg = g.energies()
+        assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo), mixed
+        assert np.array_equal(g.get_spins(), want), mixed
+        outs.append(g.get_words().tobytes())
+    assert outs[0] == outs[1]
