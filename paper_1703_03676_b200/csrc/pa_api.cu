@@ -374,8 +374,7 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     if ((rc = pa_upload_wtab(h, dbeta, (Emax - Emin) / 4)) != PA_OK) return rc;
     // weights + W, plan (tau, r, scan, parents, R_new), copy: queued back to back; the copy reads R_new on
     // the device, so the host waits once, at the end
-    if ((rc = pa_launch_weights(h, Emin, h->w)) != PA_OK) return rc;
-    if ((rc = pa_launch_plan(h, Emin)) != PA_OK) return rc;
+    if ((rc = pa_launch_weights_plan(h, Emin, h->w, false)) != PA_OK) return rc;
     // R_new and W travel to the host right after the plan kernel; the copy is queued behind them and runs
     // while the host wakes up, so the stream never idles on this call's one synchronisation
     PA_CUDA(h, cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToHost, h->stream));
@@ -610,21 +609,25 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
         }
         if (cudaMemcpyAsync(d_t, h_t, (size_t)cs * tab * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = PA_ERR_CUDA; break; }
         h->dev_R = true;
+        const char* efc = getenv("PA_FUSE_COPY");
+        const bool fuse_copy = !(efc && atoi(efc) == 0);
         for (int i = 0; i < cs && rc == PA_OK; ++i) {
             const double beta = betas[s0 + i + 1];
             h->wtab_cur = d_t + (size_t)i * tab;
             if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[2], h->stream);
-            if ((rc = pa_launch_weights(h, 0, h->w)) != PA_OK) break;
-            if ((rc = pa_launch_plan(h, 0)) != PA_OK) break;
+            // small populations on the lane-split sweep kernel: the sweep launch gathers the new population while it stages its
+            // strip, so the step is three launches (plan, sweep, measure) instead of four
+            const bool gather = fuse_copy && pa_sweep_gathers(h, theta);
+            if ((rc = pa_launch_weights_plan(h, 0, h->w, gather)) != PA_OK) break;
             if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[4], h->stream);
-            if ((rc = pa_launch_copy(h)) != PA_OK) break;
+            if (!gather && (rc = pa_launch_copy(h)) != PA_OK) break;
             if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[5], h->stream);
             if (h->timing & PA_TIME_RESAMPLE) cudaEventRecord(h->ev[3], h->stream);
             h->cur ^= 1; h->k += 1;
             const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
             h->T12 = pa_threshold(exp(-12.0 * beta));
             if (h->timing & PA_TIME_SWEEP) cudaEventRecord(h->ev[0], h->stream);
-            if ((rc = pa_launch_sweep(h, T4, T8, theta)) != PA_OK) break;
+            if ((rc = gather ? pa_launch_sweep_gather(h, T4, T8, theta) : pa_launch_sweep(h, T4, T8, theta)) != PA_OK) break;
             if (h->timing & PA_TIME_SWEEP) cudaEventRecord(h->ev[1], h->stream);
             h->t += (uint32_t)theta;
             h->snap_out = (PaScalars*)(d_snaps + (size_t)i * snap);   // the measure kernel's last CTA leaves the snapshot there

@@ -229,6 +229,10 @@ int pa_launch_measure(pa_handle* h);                                   // E, M, 
 int pa_launch_weights(pa_handle* h, int Emin, double* w_out);          // w_j, W = TREE1024(w) -> d_scal->W
 int pa_launch_overlap(pa_handle* h, int Emin);                         // TREE1024(min(1, tau_j)) -> d_scal->sum
 int pa_launch_plan(pa_handle* h, int Emin);                            // tau, r, scan, parent map, R_new
+int pa_launch_weights_plan(pa_handle* h, int Emin, double* w_out, bool commit);   // both; one fused launch for populations of a few tiles
+bool pa_small_plan_ok(const pa_handle* h);                             // ... which this says
+bool pa_sweep_gathers(const pa_handle* h, int theta);                  // pa_anneal: the next sweep launch can do the replica copy while staging
+int pa_launch_sweep_gather(pa_handle* h, uint32_t T4, uint32_t T8, int theta);   // sweep of spins[cur] := resampled spins[1-cur]
 int pa_launch_copy(pa_handle* h);                                      // new[d] = old[parent(d)], d < R_new (read on the device); pa_anneal: + commit
 int pa_launch_hist(pa_handle* h, double beta);
 int pa_launch_ehist(pa_handle* h);                                     // count-only energy histogram -> Hd

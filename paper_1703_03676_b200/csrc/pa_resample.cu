@@ -3,6 +3,7 @@
 //   and the bit-lane gather copy into the new population.  Three launches per resampling step, no host
 //   round trip between them (E_min comes from the measure kernel of the previous step's observables).
 #include "pa_common.cuh"
+#include <stdlib.h>
 
 // ------------------------------------------------------------------------------------------------
 // TREE1024 (O5; L165 "sum the per-block partial results in a subsequent kernel call"): one CTA of
@@ -200,6 +201,126 @@ int pa_launch_plan(pa_handle* h, int Emin) {
                          h->d_scal, (long long)(h->dev_R ? -1 : h->R_cur), (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, h->keys, h->k,
                          (long long)h->R_cap, h->r, h->o, h->parent, h->scan_state, n, h->nlev, h->e0));
     h->launches += 1;
+    return PA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Small populations (at most PA_SMALL_TILES tiles of 1024, e.g. configs[0]): weights, W, tau, copy numbers, scan and parent map in
+// ONE CTA and one launch.  The same arithmetic in the same order as pa_tree_kernel<0> + pa_plan_kernel -- per-tile TREE1024 trees,
+// tile sums added in ascending order from 0.0, tau = (R w)/W with one multiply and one divide, the scan as plain integer
+// sums -- but without the ticket, the fences and the look-back: what costs two launches of 6 us each on a launch-bound population
+// (eight dependent trips to global memory) becomes one of about 4 us.
+// ------------------------------------------------------------------------------------------------
+#define PA_SMALL_TILES 4
+__global__ void __launch_bounds__(PA_TILE)
+pa_tree_plan_small_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* sc,
+                          long long R, double R_target, int Emin, PhiloxKeys K, uint32_t kcount, long long R_cap,
+                          double* __restrict__ w_out, uint32_t* __restrict__ r_out, uint32_t* __restrict__ o_out,
+                          uint32_t* __restrict__ parent, int n_tiles, int N, int e0, int commit) {
+    __shared__ double run[32];
+    __shared__ double s_W;
+    __shared__ uint32_t s_wsum[32];
+    pa_pdl_wait(); pa_pdl_launch();
+    R = pa_live_R(R, sc);
+    Emin = pa_live_Emin(Emin, sc, N, e0);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double wv[PA_SMALL_TILES];
+    double total = 0.0;
+#pragma unroll
+    for (int t = 0; t < PA_SMALL_TILES; ++t) {
+        wv[t] = 0.0;
+        if (t < n_tiles) {
+            const long long j = (long long)t * PA_TILE + tid;
+            if (j < R) { wv[t] = wtab[(E[j] - Emin) >> 2]; if (w_out) w_out[j] = wv[t]; }
+            double v = wv[t];
+#pragma unroll
+            for (int off = 16; off >= 1; off >>= 1) v = __dadd_rn(v, __shfl_down_sync(0xffffffffu, v, off));
+            if (lane == 0) run[warp] = v;
+            __syncthreads();
+            if (warp == 0) {
+                v = run[lane];
+#pragma unroll
+                for (int off = 16; off >= 1; off >>= 1) v = __dadd_rn(v, __shfl_down_sync(0xffffffffu, v, off));
+                if (lane == 0) total = __dadd_rn(total, v);              // tile sums in ascending order (O5)
+            }
+            __syncthreads();
+        }
+    }
+    if (tid == 0) { s_W = total; sc->W = total; }
+    __syncthreads();
+    const double W = s_W;
+    uint32_t base = 0;
+#pragma unroll
+    for (int t = 0; t < PA_SMALL_TILES; ++t) {
+        if (t < n_tiles) {
+            const long long j = (long long)t * PA_TILE + tid;
+            uint32_t r = 0;
+            if (j < R) {
+                const uint4 x = pa_philox((uint32_t)(j >> 2), 0u, kcount, PA_TAG_RESAMPLE, K);     // x(j,k), O1
+                const uint32_t xq = (j & 3) == 0 ? x.x : (j & 3) == 1 ? x.y : (j & 3) == 2 ? x.z : x.w;
+                const double tau = __ddiv_rn(__dmul_rn(R_target, wv[t]), W);
+                const double n = floor(tau);
+                const double f = __dsub_rn(tau, n);
+                const double u = __dmul_rn((double)xq, 1.0 / 4294967296.0);
+                r = (uint32_t)n + (u < f ? 1u : 0u);
+            }
+            uint32_t inc = r;
+#pragma unroll
+            for (int off = 1; off < 32; off <<= 1) {
+                const uint32_t v = __shfl_up_sync(0xffffffffu, inc, off);
+                if (lane >= off) inc += v;
+            }
+            if (lane == 31) s_wsum[warp] = inc;
+            __syncthreads();
+            uint32_t wbase = 0, btotal = 0;
+#pragma unroll
+            for (int w = 0; w < 32; ++w) { const uint32_t v = s_wsum[w]; if (w < warp) wbase += v; btotal += v; }
+            uint32_t o = base + wbase + inc - r;
+            if (j < R) {
+                r_out[j] = r;
+                o_out[j] = o;
+                for (uint32_t c = 0; c < r; ++c)
+                    if ((long long)o + c < R_cap) parent[o + c] = (uint32_t)j;
+            }
+            base += btotal;
+            __syncthreads();
+        }
+    }
+    if (tid == 0) {
+        sc->R_new = base;
+        if (commit) {
+            // pa_anneal with the copy fused into the sweep kernel's staging (pa_sweep_split_kernel<S, true>): what pa_copy_kernel's
+            // first thread does there -- the new population size becomes current on the device (or the error flag is raised) and the
+            // next measure launch's accumulators are cleared.  Every thread of this CTA has read R_dev / E_min long before.
+            if (base >= 1u && (long long)base <= R_cap) sc->R_dev = base; else sc->err = 1u;
+            sc->mmin_inv = 0u; sc->mmax = 0u; sc->done_counter = 0u; sc->pad0 = 0u;
+            sc->SE = 0; sc->SE2 = 0; sc->SA = 0; sc->SM2 = 0; sc->m4sum = 0.0;
+        }
+    }
+}
+
+// a population of at most PA_SMALL_TILES tiles takes the fused kernel (PA_SMALL_PLAN=0: never)
+bool pa_small_plan_ok(const pa_handle* h) {
+    const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
+    const char* ev = getenv("PA_SMALL_PLAN");
+    return n <= PA_SMALL_TILES && !(ev && atoi(ev) == 0);
+}
+
+// weights + W, then the plan: two launches, or the fused kernel for a small population.  commit (pa_anneal, small populations
+// only): the kernel also makes R_new the device's current population size, as the copy kernel would.
+int pa_launch_weights_plan(pa_handle* h, int Emin, double* w_out, bool commit) {
+    const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
+    if (!pa_small_plan_ok(h)) {
+        if (commit) return PA_ERR_INVALID_ARG;
+        const int rc = pa_launch_weights(h, Emin, w_out);
+        return rc != PA_OK ? rc : pa_launch_plan(h, Emin);
+    }
+    PA_CUDA(h, pa_launch(h, pa_tree_plan_small_kernel, dim3(1), dim3(PA_TILE), 0, (const int32_t*)h->E,
+                         h->wtab_cur ? h->wtab_cur : (const double*)h->wtab, h->d_scal, (long long)(h->dev_R ? -1 : h->R_cur),
+                         (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, h->keys, h->k, (long long)h->R_cap, w_out,
+                         h->r, h->o, h->parent, n, h->nlev, h->e0, commit ? 1 : 0));
+    h->launches += 1;
+    if (commit) h->scal_zeroed = true;
     return PA_OK;
 }
 

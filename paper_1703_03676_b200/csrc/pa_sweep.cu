@@ -29,6 +29,8 @@ struct SweepParams {
     const PaScalars* sc;
     long long Gcap;                  // groups the population buffer holds (p = 64 experiment: the second group of a pair may not exist)
     const uint8_t* jmask;            // O15: per resident word, bit k = bond to neighbour k (same, x, up, down) has J = -1; NULL = ferromagnet
+    const uint32_t* src;             // lane-split kernel with GATHER: the population before resampling and its parent map (new[d] = old[parent[d]])
+    const uint32_t* parent;
     long long n_main;                // column-walk kernels without clusters, mixed launch (pa_sweep_pick_C): CTAs 0 .. n_main-1 own a whole group each, every
                                      // later group is shared by four lane-split CTAs; -1: uniform launch
 };
@@ -395,7 +397,10 @@ __device__ __forceinline__ void pa_store_lanes(uint32_t* gdst, const uint32_t* s
     }
 }
 
-template <int S>
+// GATHER (pa_anneal, small populations): `pop` is the NEW population buffer; the strip is staged from the old population P.src
+// through the parent map -- the replica copy of the resampling step (L165-L171, O7: new[d] = old[parent(d)], dead lanes 0) done by
+// the kernel that needs the words anyway, which saves the launch-bound step a kernel.
+template <int S, bool GATHER>
 __global__ void __launch_bounds__(256)
 pa_sweep_split_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     constexpr int NC = 8 / S;
@@ -407,7 +412,30 @@ pa_sweep_split_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;
     const int Lh = P.Lh, L = P.L, half = P.N >> 1;
     uint32_t* gbase = pop + g * (long long)P.N;
-    for (int i = tid; i < P.N; i += T) tile[i] = gbase[i];
+    if (GATHER) {
+        constexpr int NL = 32 / S;                     // this CTA's lanes: NL * sub ... NL * sub + NL - 1
+        __shared__ uint32_t s_par[NL];
+        if (tid < NL) {
+            const long long d = g * 32 + sub * NL + tid;
+            s_par[tid] = d < pa_live_R(P.R, P.sc) ? P.parent[d] : 0xffffffffu;
+        }
+        __syncthreads();
+        for (int i = tid; i < P.N; i += T) {
+            uint32_t wd = 0u, q_last = 0xffffffffu, ws = 0u;
+#pragma unroll
+            for (int k = 0; k < NL; ++k) {
+                const uint32_t pr = s_par[k];
+                if (pr != 0xffffffffu) {
+                    const uint32_t q = pr >> 5;
+                    if (q != q_last) { ws = P.src[(size_t)q * P.N + i]; q_last = q; }    // parents are non-decreasing: each source word once
+                    wd |= ((ws >> (pr & 31u)) & 1u) << (sub * NL + k);
+                }
+            }
+            tile[i] = wd;
+        }
+    } else {
+        for (int i = tid; i < P.N; i += T) tile[i] = gbase[i];
+    }
     __syncthreads();
     const uint32_t g8 = (uint32_t)(8 * g);
     for (int it = 0; it < P.theta; ++it) {
@@ -1136,7 +1164,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     P.L = h->geom.Lx; P.Lh = h->geom.Lx / 2; P.Ly = h->geom.Ly; P.Lz = h->geom.Lz; P.N = h->N;
     P.C = h->sweep_C; P.H = h->geom.Ly * (h->geom.Lz / P.C);
-    P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1;
+    P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.src = nullptr; P.parent = nullptr;
     const size_t smem = (size_t)h->N * 4 / P.C;
     const unsigned grid = (unsigned)(G * P.C);
     cudaError_t e = cudaErrorInvalidValue;
@@ -1169,17 +1197,35 @@ static int pa_sweep_pick_split(const pa_handle* h, int64_t G) {
     return G * 4 <= 160 ? 4 : G * 2 <= 160 ? 2 : 0;
 }
 
-static int pa_launch_sweep_split(pa_handle* h, SweepParams& P, int S, int64_t G) {
+static int pa_launch_sweep_split(pa_handle* h, SweepParams& P, int S, int64_t G, bool gather) {
     P.C = 1; P.H = h->L;
     const int half = h->N / 2;
     int T = (half + 31) / 32 * 32;
     if (T > 256) T = 256;
     const size_t smem = (size_t)h->N * 4;
-    void (*kern)(uint32_t*, const SweepParams) = S == 4 ? pa_sweep_split_kernel<4> : pa_sweep_split_kernel<2>;
+    void (*kern)(uint32_t*, const SweepParams) = gather ? (S == 4 ? pa_sweep_split_kernel<4, true> : pa_sweep_split_kernel<2, true>)
+                                                        : (S == 4 ? pa_sweep_split_kernel<4, false> : pa_sweep_split_kernel<2, false>);
     PA_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     PA_CUDA(h, pa_launch(h, kern, dim3((unsigned)(G * S)), dim3((unsigned)T), smem, h->spins[h->cur], P));
     h->launches += 1;
     return PA_OK;
+}
+
+// pa_anneal: true if the sweep launch of this step runs on the lane-split kernel and the plan kernel can commit the population
+// size (small populations), so that the sweep can stage its strips straight from the old population (no pa_copy_kernel launch)
+bool pa_sweep_gathers(const pa_handle* h, int theta) {
+    return theta > 0 && h->dev_R && pa_small_plan_ok(h) && pa_sweep_pick_split(h, (h->R_target + 31) / 32) != 0;
+}
+
+int pa_launch_sweep_gather(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
+    SweepParams P;
+    P.K = h->keys;
+    P.T4 = T4; P.T8 = T8; P.T12 = 0u; P.Ly = h->L; P.Lz = 1;
+    P.t0 = h->t; P.theta = theta; P.two = 2u;
+    P.R = -1; P.sc = h->d_scal;
+    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1;
+    P.src = h->spins[1 - h->cur]; P.parent = h->parent;
+    return pa_launch_sweep_split(h, P, pa_sweep_pick_split(h, (h->R_target + 31) / 32), h->G_cap, true);
 }
 
 int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
@@ -1193,7 +1239,8 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     if (const int S = pa_sweep_pick_split(h, h->dev_R ? (h->R_target + 31) / 32 : G)) {   // pa_anneal: the grid covers the capacity, the population is about the target
         P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1;
-        return pa_launch_sweep_split(h, P, S, G);
+        P.src = nullptr; P.parent = nullptr;
+        return pa_launch_sweep_split(h, P, S, G, false);
     }
     P.L = h->L; P.Lh = h->L / 2; P.C = pa_sweep_pick_C(h, G, &P.n_main); P.H = h->L / P.C; P.N = h->N;
     const size_t smem = (size_t)P.H * h->L * 4;
@@ -1201,7 +1248,7 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     const unsigned grid = P.n_main >= 0 ? (unsigned)(P.n_main + 4 * (G - P.n_main)) : (unsigned)(G * P.C);
     const int v = h->sweep_cmp;
     P.jmask = h->has_j ? h->jmask : nullptr;
-    P.Gcap = h->G_cap;
+    P.Gcap = h->G_cap; P.src = nullptr; P.parent = nullptr;
     const cudaError_t e = (h->has_j && h->rng_mode != PA_RNG_LCG) ? pa_sweep_dispatch_j(h, P, smem, grid)   // O15, Philox per spin
                         : h->rng_mode == PA_RNG_LCG ? pa_sweep_dispatch_lcg(h, P, smem, grid)
                         : v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)
