@@ -943,6 +943,93 @@ pa_sweep3d_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     }
 }
 
+// Column walk for cubes of 8 .. 64 (edges 2 Lh = Ly = Lz): a thread owns the column (y, xh) of its CTA's planes and walks down z two
+// planes at a time, as pa_sweep_col_kernel walks down the rows.  Every shared-memory address is the thread's pointer plus a
+// compile-time immediate (x and y wrap offsets are per-thread constants, the z neighbours of a pair are words the pair has loaded
+// anyway), the site index advances by a constant: the two dozen index instructions per word of pa_sweep3d_kernel disappear.
+// Requirements (pa_launch_sweep_3d): planes per CTA even, T = min(256, columns * planes / 2).
+template <bool CLUSTER, int LOG_LH>
+__global__ void __launch_bounds__(256, 3)
+pa_sweep3d_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
+    extern __shared__ __align__(16) uint32_t tile[];   // [2][Pz][Ly][Lh]
+    constexpr int Lh = 1 << LOG_LH, Ly = 2 * Lh, Lx = 2 * Lh, LOG_COLS = 2 * LOG_LH + 1, cols = 1 << LOG_COLS, plane = cols;
+    const int T = blockDim.x, tid = threadIdx.x;
+    const int C = CLUSTER ? P.C : 1;
+    unsigned cr = 0;
+    if (CLUSTER) cr = cg::this_cluster().block_rank();
+    const long long g = blockIdx.x / C;
+    pa_pdl_wait(); pa_pdl_launch();
+    if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // uniform per cluster
+    const int Pz = P.H >> (LOG_LH + 1);                // planes of this CTA (even)
+    const int z0 = (int)cr * Pz;
+    const int half = Pz * plane;
+    uint32_t* gbase = pop + g * (long long)P.N;
+    const int goff = z0 * plane, gcol = P.N >> 1;
+    for (int c = 0; c < 2; ++c) {
+        const uint4* src = reinterpret_cast<const uint4*>(gbase + c * gcol + goff);
+        uint4* dst = reinterpret_cast<uint4*>(tile + c * half);
+        for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+    }
+    const uint32_t* up_tile = tile;
+    const uint32_t* dn_tile = tile;
+    if (CLUSTER) {
+        cg::cluster_group cl = cg::this_cluster();
+        up_tile = cl.map_shared_rank(tile, (cr + C - 1) % C);
+        dn_tile = cl.map_shared_rank(tile, (cr + 1) % C);
+        cl.sync();
+    } else {
+        __syncthreads();
+    }
+    const uint32_t g8 = (uint32_t)(8 * g);
+    const int nseg = T > cols ? (T >> LOG_COLS) : 1;   // z segments per column when there are more threads than columns
+    const int zps = Pz / nseg;                         // planes per thread and column: even, >= 2
+    const int items = cols * nseg;
+    for (int it = 0; it < P.theta; ++it) {
+#pragma unroll 1
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t c2 = 2u * (P.t0 + (uint32_t)it) + (uint32_t)c;
+            uint32_t hi1u, lo1u;
+            pa_mulhilo(PA_PHILOX_M1, c2, hi1u, lo1u);
+            const uint32_t c0base = hi1u ^ P.K.k0[0] ^ g8;
+#pragma unroll 1
+            for (int item = tid; item < items; item += T) {
+                const int col = item & (cols - 1), seg = item >> LOG_COLS;
+                const int y = col >> LOG_LH, xh = col & (Lh - 1);
+                const int za = seg * zps;                                       // first local plane: even, and z0 is even
+                const int dYm = y == 0 ? (Ly - 1) * Lh : -Lh, dYp = y == Ly - 1 ? -(Ly - 1) * Lh : Lh;
+                const int dL = ((xh - 1) & (Lh - 1)) - xh, dR = ((xh + 1) & (Lh - 1)) - xh;
+                const int p0 = (y + c) & 1;                                     // x-parity of the even planes; odd planes: 1 - p0
+                const int dA = p0 ? dR : dL, dB = p0 ? dL : dR;
+                uint32_t* m = tile + c * half + za * plane + col;
+                const uint32_t* o = tile + (1 - c) * half + za * plane + col;
+                uint32_t site = (uint32_t)(((z0 + za) * Ly + y) * Lx + 2 * xh + p0);
+                const uint32_t dsite = (uint32_t)(Ly * Lx + 1 - 2 * p0);        // to the site of the next plane in this column
+#pragma unroll 1
+                for (int k = 0; k < zps; k += 2) {
+                    const uint32_t s0 = m[0], s1 = m[plane];
+                    const uint32_t o0 = o[0], o1 = o[plane];
+                    const uint32_t x0 = o[dA], x1 = o[plane + dB];
+                    const uint32_t ym0 = o[dYm], yp0 = o[dYp], ym1 = o[plane + dYm], yp1 = o[plane + dYp];
+                    uint32_t zm0, zp1;
+                    if (za + k > 0) zm0 = o[-plane]; else zm0 = up_tile[(1 - c) * half + (Pz - 1) * plane + col];
+                    if (za + k + 2 < Pz) zp1 = o[2 * plane]; else zp1 = dn_tile[(1 - c) * half + col];
+                    const uint32_t f0 = pa_flip_mask3d(s0, o0, x0, ym0, yp0, zm0, o1, site, c0base, lo1u, P);
+                    const uint32_t f1 = pa_flip_mask3d(s1, o1, x1, ym1, yp1, o0, zp1, site + dsite, c0base, lo1u, P);
+                    m[0] = s0 ^ f0;
+                    m[plane] = s1 ^ f1;
+                    m += 2 * plane; o += 2 * plane; site += (uint32_t)(2 * Ly * Lx);
+                }
+            }
+            if (CLUSTER) cg::this_cluster().sync(); else __syncthreads();
+        }
+    }
+    for (int c = 0; c < 2; ++c) {
+        uint4* dst = reinterpret_cast<uint4*>(gbase + c * gcol + goff);
+        const uint4* src = reinterpret_cast<const uint4*>(tile + c * half);
+        for (int i = tid; i < (half >> 2); i += T) dst[i] = src[i];
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
@@ -1060,12 +1147,12 @@ static int pa_sweep_pick_C(const pa_handle* h, int64_t G, long long* n_main) {
 }
 
 template <typename Kern>
-static cudaError_t pa_sweep_launch_k(pa_handle* h, Kern kern, const SweepParams& P, size_t smem, unsigned grid, bool cluster) {
+static cudaError_t pa_sweep_launch_k(pa_handle* h, Kern kern, const SweepParams& P, size_t smem, unsigned grid, bool cluster, int T = 0) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid, 1, 1);
-    cfg.blockDim = dim3((unsigned)h->sweep_T, 1, 1);
+    cfg.blockDim = dim3((unsigned)(T > 0 ? T : h->sweep_T), 1, 1);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = h->stream;
     cudaLaunchAttribute attr[2];
@@ -1169,7 +1256,29 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     const unsigned grid = (unsigned)(G * P.C);
     cudaError_t e = cudaErrorInvalidValue;
     const bool cl = P.C > 1;
-    const int lx = P.L == P.Ly && pa_env_int("PA_SWEEP_KIND", 1) != 0 ? P.L : 0;        // cubes' fast index arithmetic (kind 0: generic)
+    const int kind = pa_env_int("PA_SWEEP_KIND", 1);                                    // 1: column walk, 2: shift/mask index arithmetic, 0: generic
+    const int lx = P.L == P.Ly && kind != 0 ? P.L : 0;
+    const int Pz = P.Lz / P.C;
+    if (kind == 1 && P.L == P.Ly && P.L == P.Lz && (P.L == 8 || P.L == 16 || P.L == 32 || P.L == 64) && Pz >= 2 && (Pz & 1) == 0 &&
+        pa_env_int("PA_SWEEP_T", 0) == 0) {
+        const int cols = P.Ly * P.Lh;
+        int T = 256;
+        while (T > 32 && T > cols * Pz / 2) T >>= 1;
+        if (T <= cols * Pz / 2 && (cols >= T || (Pz % (T / cols) == 0 && ((Pz / (T / cols)) & 1) == 0))) {
+#define PA_3DC_CASE(LOGH) e = cl ? pa_sweep_launch_k(h, pa_sweep3d_col_kernel<true, LOGH>, P, smem, grid, true, T) \
+                                  : pa_sweep_launch_k(h, pa_sweep3d_col_kernel<false, LOGH>, P, smem, grid, false, T)
+            switch (P.L) {
+                case 8: PA_3DC_CASE(2); break;
+                case 16: PA_3DC_CASE(3); break;
+                case 32: PA_3DC_CASE(4); break;
+                default: PA_3DC_CASE(5); break;
+            }
+#undef PA_3DC_CASE
+            PA_CUDA(h, e);
+            h->launches += 1;
+            return PA_OK;
+        }
+    }
 #define PA_3D_CASE(LOGH, LOGY) e = cl ? pa_sweep_launch_k(h, pa_sweep3d_kernel<true, LOGH, LOGY>, P, smem, grid, true) \
                                       : pa_sweep_launch_k(h, pa_sweep3d_kernel<false, LOGH, LOGY>, P, smem, grid, false)
     switch (lx) {

@@ -71,20 +71,25 @@ def test_box_run_every_step(monkeypatch, dims, R, C):
 
 
 def test_cube_generic_and_fast_index_arithmetic_agree(monkeypatch):
-    """Cubes of 8 .. 64 run on kernels whose index arithmetic is shifts and masks; PA_SWEEP_KIND=0 / PA_MEASURE_GENERIC=1 force the
-    any-edge kernels (integer divisions).  Same bytes, same energies."""
-    for L, R in ((8, 500), (16, 200), (32, 64)):
+    """Cubes of 8 .. 64 run on the column-walk kernel (a thread walks down z; default) or, with PA_SWEEP_KIND=2, on the kernel whose
+    index arithmetic is shifts and masks; PA_SWEEP_KIND=0 / PA_MEASURE_GENERIC=1 force the any-edge kernels (integer divisions).
+    Same bytes, same energies, for one CTA per group and for clusters (z-neighbours over DSMEM)."""
+    for L, R, C in ((8, 500, None), (8, 300, "2"), (16, 200, None), (16, 100, "4"), (32, 64, None), (32, 40, "8")):
         out = []
-        for generic in (False, True):
-            if generic:
-                monkeypatch.setenv("PA_SWEEP_KIND", "0"); monkeypatch.setenv("PA_MEASURE_GENERIC", "1")
-            else:
-                monkeypatch.delenv("PA_SWEEP_KIND", raising=False); monkeypatch.delenv("PA_MEASURE_GENERIC", raising=False)
+        for kind in (None, "2", "0"):
+            for k in ("PA_SWEEP_KIND", "PA_MEASURE_GENERIC", "PA_SWEEP_C"):
+                monkeypatch.delenv(k, raising=False)
+            if kind:
+                monkeypatch.setenv("PA_SWEEP_KIND", kind)
+            if kind == "0":
+                monkeypatch.setenv("PA_MEASURE_GENERIC", "1")
+            if C:
+                monkeypatch.setenv("PA_SWEEP_C", C)
             g = pa.Population.box((L, L, L), R, 23)
             g.sweep(0.2, 3)
             E, M = g.energies()
             out.append((g.get_words().tobytes(), E.tobytes(), M.tobytes()))
-        assert out[0] == out[1], L
+        assert out[0] == out[1] == out[2], (L, C)
 
 
 def test_box_adaptive_anneal_and_export():
