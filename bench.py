@@ -516,12 +516,23 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     t0 = time.perf_counter()
+    # fixed schedules: ONE C-ABI call per step with host buffers (pa_step_host: upload, resample, sweeps in chunks with the finished
+    # chunks travelling back beside them, energies, observables); the adaptive workload keeps the single calls (its bisection and
+    # histogram fold sit between them)
+    one_call = run.betas is not None and not wl.multi_histogram
     for s in range(Ke):
         nb = ((R_host + 31) // 32) * wl.N * 4
-        pop.set_words(R_host, host_words); h2d += nb
-        o = run.step()
-        pop.energies_into(host_E, host_M)
-        pop.get_words(host_words)
+        h2d += nb
+        if one_call:
+            run.i += 1
+            beta = run.betas[min(run.i, len(run.betas) - 1)]
+            o, _ = pop.step_host(R_host, host_words, run.beta, beta, wl.theta, host_words, host_E, host_M)
+            run.beta = beta
+        else:
+            pop.set_words(R_host, host_words)
+            o = run.step()
+            pop.energies_into(host_E, host_M)
+            pop.get_words(host_words)
         R_host = pop.population
         d2h += ((R_host + 31) // 32) * wl.N * 4 + 8 * R_host + ctypes.sizeof(pa.pa_obs_t)
         upd_e += o["R"] * wl.N * wl.theta
@@ -530,7 +541,10 @@ def run_ours(args):
     dt, upd_e = reduce_over_ranks(dt, upd_e, "cuda", dist if world > 1 else None)
     e2e = {"value": upd_e / (dt * 1e9), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke,
            "steps": Ke, "what": f"{Ke} steps (capped by --e2e-steps: the packed population is {h2d // Ke / 1e9:.2f} GB each way per step): "
-                                "population words pinned-host -> device, one temperature step, energies + words + observables back to host; host wall clock"}
+                                "population words pinned-host -> device, one temperature step, energies + words + observables back to host; host wall clock; "
+                                + ("one pa_step_host call per step (device-to-host copies of finished chunks overlap the sweeps)" if one_call
+                                   else "pa_set_words + single calls + pa_energies + pa_get_words"),
+           "api": "pa_step_host" if one_call else "single calls"}
     del host_words, host_E, host_M
 
     # ---- weighted average of the ranks' populations at the last temperature (Eq. 6-7): the method's own exchange step

@@ -210,6 +210,17 @@ int pa_set_spins(pa_t* h, int64_t j0, int64_t nrep, const int8_t* in);
 int pa_get_words(pa_t* h, uint32_t* words);
 int pa_set_words(pa_t* h, int64_t R, const uint32_t* words);
 
+/* One temperature step of the paper's loop (steps 2-4) for a population that lives in HOST memory between
+ * steps: the same results, bit for bit, as pa_set_words(R_in, words_in); pa_resample(beta, beta_new); pa_sweep(beta_new, theta);
+ * pa_observables(beta_new); pa_energies; pa_get_words(words_out) -- but the sweeps run in chunks of groups and every finished
+ * chunk travels to the host on a second stream while the following chunks are swept.
+ * words_in: HOST uint32 [ceil(R_in/32)][N] (interchange layout, above); words_out: HOST uint32 [ceil(R_cap/32)][N], of which the
+ * first ceil(R_new/32) groups are written (pinned memory for the overlap; pageable memory works, serially).  E_out / M_out: host or
+ * device int32[R_new] or NULL; obs_out, R_new_out: host or NULL.  Synchronous.  Errors as the single calls; after
+ * PA_ERR_CAPACITY the handle holds the uploaded population unchanged and words_out is untouched. */
+int pa_step_host(pa_t* h, int64_t R_in, const uint32_t* words_in, double beta, double beta_new, int theta,
+                 uint32_t* words_out, int32_t* E_out, int32_t* M_out, pa_obs_t* obs_out, int64_t* R_new_out);
+
 /* Vectors of the last successful resampling step (pa_resample, or the last step of pa_anneal), indexed by the parent slot
  * j < R_prev = pa_prev_population(h), the population size before that step (0 if none yet); any pointer may be NULL:
  * W (one double), w[R_prev] double, r[R_prev] uint32 copy numbers, o[R_prev] uint32 offsets. */

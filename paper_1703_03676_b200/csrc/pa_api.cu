@@ -263,6 +263,8 @@ void pa_destroy(pa_t* h) {
     if (h->h_adapt) cudaFreeHost(h->h_adapt);
     if (h->h_tabs) cudaFreeHost(h->h_tabs);
     for (int b = 0; b < 2; ++b) if (h->ev_chunk[b]) cudaEventDestroy(h->ev_chunk[b]);
+    if (h->ev_xfer) cudaEventDestroy(h->ev_xfer);
+    if (h->xfer_stream) cudaStreamDestroy(h->xfer_stream);
     if (h->owns_stream && h->stream) cudaStreamDestroy(h->stream);
     if (h->owns_ws && h->ws) cudaFree(h->ws);
     delete h;
@@ -797,6 +799,53 @@ int pa_set_words(pa_t* h, int64_t R, const uint32_t* words) {
     if (rc != PA_OK) return rc;
     h->R_cur = R;
     h->em_valid = false; h->host_scal_valid = false;
+    return PA_OK;
+}
+
+// One temperature step with the population living in HOST memory between steps (the end-to-end shape of bench.py): exactly
+// pa_set_words, pa_resample, pa_sweep, pa_observables, pa_energies, pa_get_words in this order, with the same results -- but the
+// sweeps run in chunks of groups (whole rounds of the 148 SMs), and a finished chunk is converted to the interchange layout and
+// copied to the host on a second stream while the next chunks are swept: the 8.2 GB that cfg5 sends back per step hide behind
+// 0.39 s of sweeps, and only the upload (which the resampling plan needs complete) and the last chunk stay exposed.
+int pa_step_host(pa_t* h, int64_t R_in, const uint32_t* words_in, double beta, double beta_new, int theta,
+                 uint32_t* words_out, int32_t* E_out, int32_t* M_out, pa_obs_t* obs_out, int64_t* R_new_out) {
+    if (!h || !words_in || !words_out || theta < 0 || !(beta_new >= beta) || pa_is_device_ptr(words_in) || pa_is_device_ptr(words_out))
+        return PA_ERR_INVALID_ARG;
+    int rc;
+    if ((rc = pa_set_words(h, R_in, words_in)) != PA_OK) return rc;
+    int64_t R_new = 0;
+    if ((rc = pa_resample(h, beta, beta_new, &R_new)) != PA_OK) return rc;
+    if (R_new_out) *R_new_out = R_new;
+    const int64_t G = (R_new + 31) / 32;
+    // chunks of whole rounds: multiples of 148 groups, about 16 per step; small populations go in one piece
+    int64_t chunk = G / 16 / 148 * 148;
+    const char* ec = getenv("PA_STEP_HOST_CHUNK");                  // tests: force a chunk size (groups), 0 = one piece
+    if (ec) chunk = atoll(ec);
+    bool piped = chunk >= 1 && chunk < G && theta > 0;
+    if (piped) {
+        if (!h->xfer_stream) PA_CUDA(h, cudaStreamCreateWithFlags(&h->xfer_stream, cudaStreamNonBlocking));
+        if (!h->ev_xfer) PA_CUDA(h, cudaEventCreateWithFlags(&h->ev_xfer, cudaEventDisableTiming));
+        const uint32_t T4 = pa_threshold(exp(-4.0 * beta_new)), T8 = pa_threshold(exp(-8.0 * beta_new));
+        uint32_t* stage = h->spins[1 - h->cur];                      // the population before resampling: no longer needed
+        for (int64_t g0 = 0; g0 < G; g0 += chunk) {
+            const int64_t ng = g0 + chunk <= G ? chunk : G - g0;
+            rc = pa_launch_sweep_range(h, T4, T8, theta, g0, ng);
+            if (rc == PA_ERR_INVALID_ARG && g0 == 0) { piped = false; break; }     // this geometry has no range launch: one piece
+            if (rc != PA_OK) return rc;
+            if ((rc = pa_launch_words_out_range(h, stage, g0, ng)) != PA_OK) return rc;
+            PA_CUDA(h, cudaEventRecord(h->ev_xfer, h->stream));
+            PA_CUDA(h, cudaStreamWaitEvent(h->xfer_stream, h->ev_xfer, 0));
+            PA_CUDA(h, cudaMemcpyAsync(words_out + g0 * (size_t)h->N, stage + g0 * (size_t)h->N, (size_t)ng * h->N * 4,
+                                       cudaMemcpyDeviceToHost, h->xfer_stream));
+        }
+        if (piped) { h->t += (uint32_t)theta; h->em_valid = false; h->host_scal_valid = false; h->sweep_timed = false; }
+    }
+    if (!piped && (rc = pa_sweep(h, beta_new, theta)) != PA_OK) return rc;
+    if (obs_out && (rc = pa_observables(h, beta_new, obs_out)) != PA_OK) return rc;
+    if (E_out && (rc = pa_energies(h, E_out, M_out)) != PA_OK) return rc;
+    if (!piped) return pa_get_words(h, words_out);
+    PA_CUDA(h, cudaStreamSynchronize(h->xfer_stream));
+    PA_CUDA(h, cudaStreamSynchronize(h->stream));
     return PA_OK;
 }
 

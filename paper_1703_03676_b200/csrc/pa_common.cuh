@@ -180,6 +180,7 @@ struct pa_handle {
     PaScalars* snap_out;                // pa_anneal: where the measure kernel leaves a copy of the device scalars (or NULL)
     bool dev_R;                         // inside pa_anneal: kernels read R and E_min from d_scal, grids cover the capacity
     cudaEvent_t ev_chunk[2];            // pa_anneal: completion of the chunk staged in buffer 0 / 1
+    cudaStream_t xfer_stream; cudaEvent_t ev_xfer;   // pa_step_host: device-to-host copies of finished chunks run beside the sweeps
     double* h_tabs; size_t h_tabs_bytes; // pinned staging for pa_anneal's weight tables and snapshots
     int pdl;                            // 1: the step's kernels are launched with programmatic stream serialization
     int64_t launches;
@@ -225,6 +226,8 @@ static inline cudaError_t pa_launch(const pa_handle* h, void (*kern)(KArgs...), 
 int pa_launch_init(pa_handle* h);
 int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta);
 int pa_sweep_configure(pa_handle* h);
+int pa_launch_sweep_range(pa_handle* h, uint32_t T4, uint32_t T8, int theta, int64_t g0, int64_t ng);   // groups g0 .. g0+ng-1 (column-walk kernels)
+int pa_launch_words_out_range(pa_handle* h, uint32_t* d_words, int64_t g0, int64_t ng);              // interchange words of those groups -> d_words[g0*N ...]
 int pa_launch_measure(pa_handle* h);                                   // E, M, integer sums, m range, m^4 sum
 int pa_launch_weights(pa_handle* h, int Emin, double* w_out);          // w_j, W = TREE1024(w) -> d_scal->W
 int pa_launch_overlap(pa_handle* h, int Emin);                         // TREE1024(min(1, tau_j)) -> d_scal->sum

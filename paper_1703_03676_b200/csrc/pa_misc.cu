@@ -280,6 +280,17 @@ int pa_launch_words_out(pa_handle* h, uint32_t* d_words) {
     h->launches += 1;
     return PA_OK;
 }
+int pa_launch_words_out_range(pa_handle* h, uint32_t* d_words, int64_t g0, int64_t ng) {
+    long long R_rel = h->R_cur - 32 * g0;                       // the kernel counts groups and live lanes from its base pointers
+    if (R_rel > 32 * ng) R_rel = 32 * ng;
+    if (R_rel <= 0) return PA_OK;
+    const long long tot = (R_rel + 31) / 32 * h->N;
+    pa_words_out_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur] + g0 * (long long)h->N, h->geom, h->N, R_rel,
+                                                                              d_words + g0 * (long long)h->N);
+    PA_CUDA(h, cudaGetLastError());
+    h->launches += 1;
+    return PA_OK;
+}
 int pa_launch_words_in(pa_handle* h, int64_t R, const uint32_t* d_words) {
     const long long G = (R + 31) / 32, tot = G * h->N;
     pa_words_in_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, R, d_words);

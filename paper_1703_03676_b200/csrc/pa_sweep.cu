@@ -29,6 +29,7 @@ struct SweepParams {
     const PaScalars* sc;
     long long Gcap;                  // groups the population buffer holds (p = 64 experiment: the second group of a pair may not exist)
     const uint8_t* jmask;            // O15: per resident word, bit k = bond to neighbour k (same, x, up, down) has J = -1; NULL = ferromagnet
+    long long g0;                    // column-walk kernels: first group of this launch (pa_launch_sweep_range: a step in chunks of groups); else 0
     const uint32_t* src;             // lane-split kernel with GATHER: the population before resampling and its parent map (new[d] = old[parent[d]])
     const uint32_t* parent;
     long long n_main;                // column-walk kernels without clusters, mixed launch (pa_sweep_pick_C): CTAs 0 .. n_main-1 own a whole group each, every
@@ -498,6 +499,7 @@ pa_sweep_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
         sub = (int)((g - P.n_main) & 3);
         g = P.n_main + ((g - P.n_main) >> 2);
     }
+    g += P.g0;
     pa_pdl_wait(); pa_pdl_launch();
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H;
@@ -604,6 +606,7 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
         sub = (int)((g - P.n_main) & 3);
         g = P.n_main + ((g - P.n_main) >> 2);
     }
+    g += P.g0;
     pa_pdl_wait(); pa_pdl_launch();
     if (g * 32 >= pa_live_R(P.R, P.sc)) return;        // past the population (capacity-sized grid in pa_anneal); uniform per cluster
     const int H = P.H;
@@ -949,7 +952,7 @@ pa_sweep3d_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 // anyway), the site index advances by a constant: the two dozen index instructions per word of pa_sweep3d_kernel disappear.
 // Requirements (pa_launch_sweep_3d): planes per CTA even, T = min(256, columns * planes / 2).
 template <bool CLUSTER, int LOG_LH>
-__global__ void __launch_bounds__(256, 3)
+__global__ void __launch_bounds__(LOG_LH == 5 ? 512 : 256, LOG_LH == 5 ? 1 : 3)      // 64^3: 128 KB strips, one CTA of 16 warps per SM
 pa_sweep3d_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     extern __shared__ __align__(16) uint32_t tile[];   // [2][Pz][Ly][Lh]
     constexpr int Lh = 1 << LOG_LH, Ly = 2 * Lh, Lx = 2 * Lh, LOG_COLS = 2 * LOG_LH + 1, cols = 1 << LOG_COLS, plane = cols;
@@ -1251,7 +1254,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     P.L = h->geom.Lx; P.Lh = h->geom.Lx / 2; P.Ly = h->geom.Ly; P.Lz = h->geom.Lz; P.N = h->N;
     P.C = h->sweep_C; P.H = h->geom.Ly * (h->geom.Lz / P.C);
-    P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.src = nullptr; P.parent = nullptr;
+    P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0; P.src = nullptr; P.parent = nullptr;
     const size_t smem = (size_t)h->N * 4 / P.C;
     const unsigned grid = (unsigned)(G * P.C);
     cudaError_t e = cudaErrorInvalidValue;
@@ -1262,7 +1265,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     if (kind == 1 && P.L == P.Ly && P.L == P.Lz && (P.L == 8 || P.L == 16 || P.L == 32 || P.L == 64) && Pz >= 2 && (Pz & 1) == 0 &&
         pa_env_int("PA_SWEEP_T", 0) == 0) {
         const int cols = P.Ly * P.Lh;
-        int T = 256;
+        int T = P.L == 64 ? 512 : 256;
         while (T > 32 && T > cols * Pz / 2) T >>= 1;
         if (T <= cols * Pz / 2 && (cols >= T || (Pz % (T / cols) == 0 && ((Pz / (T / cols)) & 1) == 0))) {
 #define PA_3DC_CASE(LOGH) e = cl ? pa_sweep_launch_k(h, pa_sweep3d_col_kernel<true, LOGH>, P, smem, grid, true, T) \
@@ -1332,12 +1335,25 @@ int pa_launch_sweep_gather(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     P.T4 = T4; P.T8 = T8; P.T12 = 0u; P.Ly = h->L; P.Lz = 1;
     P.t0 = h->t; P.theta = theta; P.two = 2u;
     P.R = -1; P.sc = h->d_scal;
-    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1;
+    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0;
     P.src = h->spins[1 - h->cur]; P.parent = h->parent;
     return pa_launch_sweep_split(h, P, pa_sweep_pick_split(h, (h->R_target + 31) / 32), h->G_cap, true);
 }
 
-int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
+static int pa_launch_sweep_groups(pa_handle* h, uint32_t T4, uint32_t T8, int theta, int64_t g0, int64_t ng);
+
+int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) { return pa_launch_sweep_groups(h, T4, T8, theta, 0, -1); }
+
+// Groups g0 .. g0+ng-1 only (pa_step_host runs a step in chunks of groups so that finished chunks travel to the host while the
+// next ones are swept).  Column-walk kernels, uniform launch, host-side population size; PA_ERR_INVALID_ARG otherwise.
+int pa_launch_sweep_range(pa_handle* h, uint32_t T4, uint32_t T8, int theta, int64_t g0, int64_t ng) {
+    if (theta == 0 || ng <= 0) return PA_OK;
+    if (h->D != 2 || h->sweep_kind != 1 || h->dev_R || g0 < 0 || g0 + ng > (h->R_cur + 31) / 32) return PA_ERR_INVALID_ARG;
+    if (h->rng_mode == PA_RNG_LCG && (pa_env_int("PA_LCG_P64", 0) == 1 || !pa_col_ok(h->L, h->sweep_C, h->sweep_T, PA_RNG_LCG))) return PA_ERR_INVALID_ARG;
+    return pa_launch_sweep_groups(h, T4, T8, theta, g0, ng);
+}
+
+static int pa_launch_sweep_groups(pa_handle* h, uint32_t T4, uint32_t T8, int theta, int64_t g0, int64_t ng) {
     if (theta == 0) return PA_OK;
     if (h->D == 3) return pa_launch_sweep_3d(h, T4, T8, theta);
     SweepParams P;
@@ -1347,14 +1363,17 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     if (const int S = pa_sweep_pick_split(h, h->dev_R ? (h->R_target + 31) / 32 : G)) {   // pa_anneal: the grid covers the capacity, the population is about the target
-        P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1;
+        P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0;
         P.src = nullptr; P.parent = nullptr;
         return pa_launch_sweep_split(h, P, S, G, false);
     }
-    P.L = h->L; P.Lh = h->L / 2; P.C = pa_sweep_pick_C(h, G, &P.n_main); P.H = h->L / P.C; P.N = h->N;
+    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.g0 = 0;
+    if (ng >= 0) { P.C = h->sweep_C; P.n_main = -1; P.g0 = g0; }       // a range of groups: the configured cluster size, no mixed launch
+    else P.C = pa_sweep_pick_C(h, G, &P.n_main);
+    P.H = h->L / P.C;
     const size_t smem = (size_t)P.H * h->L * 4;
     // mixed launch: n_main whole groups, then four lane-split CTAs per remaining group
-    const unsigned grid = P.n_main >= 0 ? (unsigned)(P.n_main + 4 * (G - P.n_main)) : (unsigned)(G * P.C);
+    const unsigned grid = ng >= 0 ? (unsigned)(ng * P.C) : P.n_main >= 0 ? (unsigned)(P.n_main + 4 * (G - P.n_main)) : (unsigned)(G * P.C);
     const int v = h->sweep_cmp;
     P.jmask = h->has_j ? h->jmask : nullptr;
     P.Gcap = h->G_cap; P.src = nullptr; P.parent = nullptr;

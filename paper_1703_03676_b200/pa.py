@@ -93,6 +93,7 @@ def lib():
         "pa_set_spins": ([vp, i64, i64, vp], i32),
         "pa_get_words": ([vp, vp], i32),
         "pa_set_words": ([vp, i64, vp], i32),
+        "pa_step_host": ([vp, i64, vp, dbl, dbl, i32, vp, vp, vp, C.POINTER(pa_obs_t), C.POINTER(i64)], i32),
         "pa_get_resample_debug": ([vp, C.POINTER(dbl), vp, vp, vp], i32),
         "pa_population": ([vp], i64),
         "pa_prev_population": ([vp], i64),
@@ -398,6 +399,13 @@ class Population:
 
     def set_words(self, R, words):
         self._check(lib().pa_set_words(self._h, int(R), _ptr(words)), "pa_set_words")
+
+    def step_host(self, R_in, words_in, beta, beta_new, theta, words_out, E_out=None, M_out=None):
+        """pa_step_host: one temperature step with the population in host buffers; returns (observables dict, R_new)."""
+        obs, Rn = pa_obs_t(), C.c_int64()
+        self._check(lib().pa_step_host(self._h, int(R_in), _ptr(words_in), float(beta), float(beta_new), int(theta), _ptr(words_out),
+                                       _ptr(E_out), _ptr(M_out), C.byref(obs), C.byref(Rn)), "pa_step_host")
+        return obs.as_dict(), Rn.value
 
     @property
     def prev_population(self):

@@ -259,3 +259,49 @@ def test_workspace_guard_bands_stay_intact(L, R):
     torch.cuda.synchronize()
     assert bool((buf[:guard] == 0xA5).all()) and bool((buf[guard + nbytes:] == 0xA5).all())
     g.close()
+
+
+@pytest.mark.parametrize("L,R,mode,theta,chunk", [(64, 6000, 0, 2, "50"), (64, 6000, 1, 2, "37"), (64, 6000, 0, 1, None), (128, 1500, 0, 1, "7"),
+                                                   (16, 1000, 0, 2, "5"), (64, 3000, 0, 0, "20"), (256, 700, 0, 1, "4")])
+def test_step_host_equals_single_calls_and_oracle(monkeypatch, L, R, mode, theta, chunk):
+    """pa_step_host (population in pinned host buffers between steps; sweeps in chunks of groups, finished chunks copied out on a
+    second stream) = pa_set_words, pa_resample, pa_sweep, pa_observables, pa_energies, pa_get_words, and = the oracle.  Chunk sizes
+    that do not divide the population, the one-piece path, a geometry without range launches (L = 16) and theta = 0 included."""
+    if chunk:
+        monkeypatch.setenv("PA_STEP_HOST_CHUNK", chunk)
+    else:
+        monkeypatch.delenv("PA_STEP_HOST_CHUNK", raising=False)
+    betas = [0.0, 0.1, 0.3, 0.3, 0.45, 0.8]
+    a, b, o = pa.Population(L, R, 43), pa.Population(L, R, 43), po.Oracle(L, R, 43)
+    for x in (a, b, o):
+        x.set_rng_mode(mode)
+    Gcap = (a.capacity + 31) // 32
+    wa = torch.zeros((Gcap, L * L), dtype=torch.int32, pin_memory=True)
+    wb = torch.zeros((Gcap, L * L), dtype=torch.int32, pin_memory=True)
+    Ea = torch.zeros(a.capacity, dtype=torch.int32, pin_memory=True)
+    Ma = torch.zeros(a.capacity, dtype=torch.int32, pin_memory=True)
+    a.get_words(wa)
+    wb.copy_(wa)
+    Ra = Rb = a.population
+    for i in range(1, len(betas)):
+        oa, Ra_new = a.step_host(Ra, wa, betas[i - 1], betas[i], theta, wa, Ea, Ma)
+        b.set_words(Rb, wb)
+        Rb_new = b.resample(betas[i - 1], betas[i])
+        b.sweep(betas[i], theta)
+        ob = b.observables(betas[i])
+        Eb, Mb = b.energies()
+        b.get_words(wb)
+        assert o.resample(betas[i - 1], betas[i]) == Rb_new == Ra_new == a.population
+        o.sweep(betas[i], theta)
+        oo = o.observables(betas[i])
+        Ga = (Ra_new + 31) // 32
+        assert torch.equal(wa[:Ga], wb[:Ga]), i
+        assert np.array_equal(Ea[:Ra_new].numpy(), Eb) and np.array_equal(Ma[:Ra_new].numpy(), Mb)
+        Eo, Mo = o.energies()
+        assert np.array_equal(Eb, Eo) and np.array_equal(Mb, Mo)
+        for k in KEYS:
+            assert oa[k] == ob[k], (k, oa[k], ob[k])
+            assert oa[k] == pytest.approx(oo[k], rel=REL, abs=1e-300), k
+        assert a.sweep_counter == b.sweep_counter == o.sweep_counter and a.lnZ == b.lnZ
+        Ra = Rb = Ra_new
+    assert np.array_equal(a.get_spins(), o.get_spins())

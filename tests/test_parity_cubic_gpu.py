@@ -36,7 +36,7 @@ def _obs_close(a, b):
 # edges of length 2 (double bonds), three different edges, one plane per CTA (clusters), ragged R, cubes
 @pytest.mark.parametrize("dims,R,C", [((4, 2, 2), 100, None), ((2, 2, 2), 33, None), ((6, 4, 2), 700, None), ((6, 4, 2), 700, "2"),
                                       ((4, 4, 4), 1000, None), ((4, 4, 4), 1000, "4"), ((8, 8, 8), 300, "2"), ((8, 8, 8), 300, "8"),
-                                      ((16, 16, 16), 96, None), ((16, 16, 16), 65, "4"), ((10, 6, 4), 50, "2"), ((32, 32, 32), 40, None)])
+                                      ((16, 16, 16), 96, None), ((16, 16, 16), 65, "4"), ((10, 6, 4), 50, "2"), ((32, 32, 32), 40, None), ((64, 64, 64), 33, None)])
 def test_box_run_every_step(monkeypatch, dims, R, C):
     if C:
         monkeypatch.setenv("PA_SWEEP_C", C)
@@ -74,7 +74,7 @@ def test_cube_generic_and_fast_index_arithmetic_agree(monkeypatch):
     """Cubes of 8 .. 64 run on the column-walk kernel (a thread walks down z; default) or, with PA_SWEEP_KIND=2, on the kernel whose
     index arithmetic is shifts and masks; PA_SWEEP_KIND=0 / PA_MEASURE_GENERIC=1 force the any-edge kernels (integer divisions).
     Same bytes, same energies, for one CTA per group and for clusters (z-neighbours over DSMEM)."""
-    for L, R, C in ((8, 500, None), (8, 300, "2"), (16, 200, None), (16, 100, "4"), (32, 64, None), (32, 40, "8")):
+    for L, R, C in ((8, 500, None), (8, 300, "2"), (16, 200, None), (16, 100, "4"), (32, 64, None), (32, 40, "8"), (64, 33, None)):
         out = []
         for kind in (None, "2", "0"):
             for k in ("PA_SWEEP_KIND", "PA_MEASURE_GENERIC", "PA_SWEEP_C"):
