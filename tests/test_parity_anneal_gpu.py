@@ -25,7 +25,8 @@ def _state(g):
 
 
 @pytest.mark.parametrize("L,R,mode,theta,chunk", [(16, 1000, 0, 3, None), (8, 33, 1, 2, "2"), (64, 2500, 1, 2, "3"), (64, 700, 0, 1, None),
-                                                   (128, 200, 0, 1, "1"), (6, 1, 0, 2, None), (32, 5000, 0, 0, None)])
+                                                   (128, 200, 0, 1, "1"), (6, 1, 0, 2, None), (32, 5000, 0, 0, None),
+                                                   (64, 5300, 0, 1, None), (64, 5300, 1, 2, "3")])      # mixed launch (whole groups + lane-split tail) over the capacity-sized grid
 def test_anneal_equals_step_by_step_calls_and_oracle(monkeypatch, L, R, mode, theta, chunk):
     if chunk:
         monkeypatch.setenv("PA_ANNEAL_CHUNK", chunk)                  # several chunks: tables and snapshots are re-staged
