@@ -251,6 +251,27 @@ struct PlaneCounter {           // planes[k] holds bit k of 32 per-lane counts, 
         return e;
     }
     __device__ __forceinline__ void add8(const uint32_t* x) { ripple<3>(block8(x)); }
+    // the weight-16 carry of sixteen inputs (planes 0..3 absorb the rest)
+    __device__ __forceinline__ uint32_t block16(const uint32_t* x) {
+        const uint32_t e1 = block8(x), e2 = block8(x + 8);
+        uint32_t s;
+        pa_csa(s, pl[3], pl[3], e1, e2);
+        return s;
+    }
+    // Eight carries of weight 2^K0 (one per row of a block of eight rows) folded in by a carry-save ladder: seven full adders and ONE
+    // ripple per eight rows instead of a ripple through all upper planes per row (the ripple was a quarter of the kernel's instructions)
+    template <int K0>
+    __device__ __forceinline__ void ladder8(const uint32_t* c) {
+        uint32_t a, b, d, e, f, g2, h;
+        pa_csa(a, pl[K0], pl[K0], c[0], c[1]);
+        pa_csa(b, pl[K0], pl[K0], c[2], c[3]);
+        pa_csa(d, pl[K0], pl[K0], c[4], c[5]);
+        pa_csa(e, pl[K0], pl[K0], c[6], c[7]);
+        pa_csa(f, pl[K0 + 1], pl[K0 + 1], a, b);
+        pa_csa(g2, pl[K0 + 1], pl[K0 + 1], d, e);
+        pa_csa(h, pl[K0 + 2], pl[K0 + 2], f, g2);
+        ripple<K0 + 3>(h);
+    }
     __device__ __forceinline__ void add16(const uint32_t* x) {
         const uint32_t e1 = block8(x), e2 = block8(x + 8);
         uint32_t s;
@@ -293,7 +314,9 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
         const int y1 = (y0 + 1) & (L - 1);
         na = __ldg(c0 + y1 * Lq + q); nb = __ldg(c1 + y1 * Lq + q);
     }
-#pragma unroll 2
+    constexpr bool LADDER = RS % 8 == 0 && NPE >= 7 && NPM >= 6;        // L >= 64
+    uint32_t ce[8], cm[8];                                                // the rows' top carries, folded in every eight rows
+#pragma unroll 8
     for (int r = 0; r < RS; ++r) {
         const int y = y0 + r;
         uint4 fa = zero, fb = zero;                                       // row y + 2, in flight while row y is counted
@@ -317,8 +340,14 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
             for (int i = 0; i < 16; ++i) xb[i] ^= 0u - ((j >> i) & 1u);
         }
         const uint32_t xs[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-        cE.add16(xb);
-        cM.add8(xs);
+        if (LADDER) {
+            ce[r & 7] = cE.block16(xb);
+            cm[r & 7] = cM.block8(xs);
+            if ((r & 7) == 7) { cE.template ladder8<4>(ce); cM.template ladder8<3>(cm); }
+        } else {
+            cE.add16(xb);
+            cM.add8(xs);
+        }
         a = na; b = nb; na = fa; nb = fb;
     }
     uint32_t pe[NPW], pm[NPW];
