@@ -189,6 +189,7 @@ __device__ __forceinline__ uint32_t pa_flip_mask_lcg(uint32_t s, uint32_t n0, ui
 // 25 - 8 sub ... 32 - 8 sub (O11: output n goes to lane 32 - n), reached by one jump r <- A^n r + C (A^n - 1)/(A - 1), n = 24 - 8 sub.
 __host__ __device__ constexpr uint32_t pa_lcg_jump_mul(int n) { uint32_t a = 1u; for (int i = 0; i < n; ++i) a *= PA_LCG_A; return a; }
 __host__ __device__ constexpr uint32_t pa_lcg_jump_add(int n) { uint32_t c = 0u; for (int i = 0; i < n; ++i) c = c * PA_LCG_A + PA_LCG_C; return c; }
+template <int NL = 8>
 __device__ __forceinline__ uint32_t pa_flip_mask_lcg_part(uint32_t s, uint32_t n0, uint32_t n1, uint32_t n2, uint32_t n3,
                                                           uint32_t r, uint32_t jmul, uint32_t jadd, uint32_t sh, const SweepParams& P) {
     uint32_t a0 = s ^ n0, a1 = s ^ n1, a2 = s ^ n2, a3 = s ^ n3;
@@ -197,13 +198,13 @@ __device__ __forceinline__ uint32_t pa_flip_mask_lcg_part(uint32_t s, uint32_t n
     r = r * jmul + jadd;
     uint32_t g4 = 0, g8 = 0;
 #pragma unroll
-    for (int b = 7; b >= 0; --b) {
+    for (int b = NL - 1; b >= 0; --b) {
         r = pa_lcg_step(r);
         pa_shift_in_ge(g4, r, P.T4, P.two);
         pa_shift_in_ge(g8, r, P.T8, P.two);
     }
     const uint32_t acc = ~g4 & ((U1 >> sh) | ~g8);
-    return (((U2 >> sh) | acc) & 0xffu) << sh;
+    return (((U2 >> sh) | acc) & ((1u << NL) - 1u)) << sh;
 }
 
 // The four LCG seeds of a quad of rows (y & ~3 .. +3) in column xh of one sub-lattice: one Philox call (O11).
@@ -401,7 +402,7 @@ __device__ __forceinline__ void pa_store_lanes(uint32_t* gdst, const uint32_t* s
 // GATHER (pa_anneal, small populations): `pop` is the NEW population buffer; the strip is staged from the old population P.src
 // through the parent map -- the replica copy of the resampling step (L165-L171, O7: new[d] = old[parent(d)], dead lanes 0) done by
 // the kernel that needs the words anyway, which saves the launch-bound step a kernel.
-template <int S, bool GATHER>
+template <int S, bool GATHER, int RNG, bool HASJ>
 __global__ void __launch_bounds__(256)
 pa_sweep_split_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     constexpr int NC = 8 / S;
@@ -439,6 +440,11 @@ pa_sweep_split_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
     }
     __syncthreads();
     const uint32_t g8 = (uint32_t)(8 * g);
+    // LCG stream (O11): skip the outputs that belong to the lanes above this CTA's block of 32/S lanes
+    constexpr int NLN = 32 / S;
+    const int nskip = 32 - NLN * (sub + 1);
+    const uint32_t jmul = nskip == 24 ? pa_lcg_jump_mul(24) : nskip == 16 ? pa_lcg_jump_mul(16) : nskip == 8 ? pa_lcg_jump_mul(8) : 1u;
+    const uint32_t jadd = nskip == 24 ? pa_lcg_jump_add(24) : nskip == 16 ? pa_lcg_jump_add(16) : nskip == 8 ? pa_lcg_jump_add(8) : 0u;
     for (int it = 0; it < P.theta; ++it) {
 #pragma unroll 1
         for (int c = 0; c < 2; ++c) {
@@ -455,12 +461,23 @@ pa_sweep_split_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
                 const int p = (y + c) & 1;
                 const int xh2 = p ? (xh + 1 == Lh ? 0 : xh + 1) : (xh == 0 ? Lh - 1 : xh - 1);
                 const uint32_t s = mine[w];
-                const uint32_t nS = oth[w];
-                const uint32_t nX = oth[w - xh + xh2];
-                const uint32_t nU = oth[(y == 0 ? L - 1 : y - 1) * Lh + xh];
-                const uint32_t nD = oth[(y + 1 == L ? 0 : y + 1) * Lh + xh];
-                const uint32_t site = (uint32_t)(y * L + 2 * xh + p);
-                mine[w] = s ^ pa_flip_mask_part<NC>(s, nS, nX, nU, nD, site, c0base, lo1u, (uint32_t)(sub * NC), P);
+                uint32_t nS = oth[w];
+                uint32_t nX = oth[w - xh + xh2];
+                uint32_t nU = oth[(y == 0 ? L - 1 : y - 1) * Lh + xh];
+                uint32_t nD = oth[(y + 1 == L ? 0 : y + 1) * Lh + xh];
+                if (HASJ) {                                   // O15: complement the neighbour across a bond with J = -1
+                    const uint32_t j = P.jmask[c * half + w];
+                    nS = pa_jx(nS, j, 0); nX = pa_jx(nX, j, 1); nU = pa_jx(nU, j, 2); nD = pa_jx(nD, j, 3);
+                }
+                if (RNG == PA_RNG_LCG) {
+                    const uint4 sd = pa_lcg_seeds((uint32_t)((y >> 2) * Lh + xh), (uint32_t)g, c2, P.K);
+                    const int q = y & 3;
+                    mine[w] = s ^ pa_flip_mask_lcg_part<NLN>(s, nS, nX, nU, nD, q == 0 ? sd.x : q == 1 ? sd.y : q == 2 ? sd.z : sd.w,
+                                                             jmul, jadd, (uint32_t)(sub * NLN), P);
+                } else {
+                    const uint32_t site = (uint32_t)(y * L + 2 * xh + p);
+                    mine[w] = s ^ pa_flip_mask_part<NC>(s, nS, nX, nU, nD, site, c0base, lo1u, (uint32_t)(sub * NC), P);
+                }
                 xh += dx; y += dy;
                 if (xh >= Lh) { xh -= Lh; y += 1; }
             }
@@ -1302,7 +1319,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
 // L = 32, R = 1000 45.5 -> 23.2 us; with more groups than SMs the split only adds work: L = 16, R = 10 000 35.8 -> 39.5 us).
 // PA_SWEEP_SPLIT forces 0/2/4.
 static int pa_sweep_pick_split(const pa_handle* h, int64_t G) {
-    if (h->D != 2 || h->rng_mode != PA_RNG_PHILOX || h->has_j || h->sweep_kind != 0 || h->sweep_C != 1 || h->sweep_C_forced) return 0;
+    if (h->D != 2 || h->sweep_kind != 0 || h->sweep_C != 1 || h->sweep_C_forced) return 0;
     if ((size_t)h->N * 4 > (size_t)64 * 1024) return 0;
     const int force = pa_env_int("PA_SWEEP_SPLIT", -1);
     if (force == 0 || force == 2 || force == 4) return force;
@@ -1315,8 +1332,15 @@ static int pa_launch_sweep_split(pa_handle* h, SweepParams& P, int S, int64_t G,
     int T = (half + 31) / 32 * 32;
     if (T > 256) T = 256;
     const size_t smem = (size_t)h->N * 4;
-    void (*kern)(uint32_t*, const SweepParams) = gather ? (S == 4 ? pa_sweep_split_kernel<4, true> : pa_sweep_split_kernel<2, true>)
-                                                        : (S == 4 ? pa_sweep_split_kernel<4, false> : pa_sweep_split_kernel<2, false>);
+    void (*kern)(uint32_t*, const SweepParams) = nullptr;
+    const int lcg = h->rng_mode == PA_RNG_LCG ? 1 : 0, hj = h->has_j ? 1 : 0;
+#define PA_SPLIT_PICK(SS, GG, RR, JJ) if (S == SS && gather == GG && lcg == (RR == PA_RNG_LCG ? 1 : 0) && hj == (JJ ? 1 : 0)) kern = pa_sweep_split_kernel<SS, GG, RR, JJ>;
+#define PA_SPLIT_PICK4(SS, GG) PA_SPLIT_PICK(SS, GG, PA_RNG_PHILOX, false) PA_SPLIT_PICK(SS, GG, PA_RNG_PHILOX, true) \
+                               PA_SPLIT_PICK(SS, GG, PA_RNG_LCG, false) PA_SPLIT_PICK(SS, GG, PA_RNG_LCG, true)
+    PA_SPLIT_PICK4(2, false) PA_SPLIT_PICK4(2, true) PA_SPLIT_PICK4(4, false) PA_SPLIT_PICK4(4, true)
+#undef PA_SPLIT_PICK4
+#undef PA_SPLIT_PICK
+    if (!kern) return PA_ERR_INVALID_ARG;
     PA_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     PA_CUDA(h, pa_launch(h, kern, dim3((unsigned)(G * S)), dim3((unsigned)T), smem, h->spins[h->cur], P));
     h->launches += 1;
@@ -1335,7 +1359,7 @@ int pa_launch_sweep_gather(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     P.T4 = T4; P.T8 = T8; P.T12 = 0u; P.Ly = h->L; P.Lz = 1;
     P.t0 = h->t; P.theta = theta; P.two = 2u;
     P.R = -1; P.sc = h->d_scal;
-    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0;
+    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = h->has_j ? h->jmask : nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0;
     P.src = h->spins[1 - h->cur]; P.parent = h->parent;
     return pa_launch_sweep_split(h, P, pa_sweep_pick_split(h, (h->R_target + 31) / 32), h->G_cap, true);
 }
@@ -1363,7 +1387,7 @@ static int pa_launch_sweep_groups(pa_handle* h, uint32_t T4, uint32_t T8, int th
     const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     if (const int S = pa_sweep_pick_split(h, h->dev_R ? (h->R_target + 31) / 32 : G)) {   // pa_anneal: the grid covers the capacity, the population is about the target
-        P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0;
+        P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = h->has_j ? h->jmask : nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0;
         P.src = nullptr; P.parent = nullptr;
         return pa_launch_sweep_split(h, P, S, G, false);
     }

@@ -374,13 +374,20 @@ def test_sweep_threshold_extremes():
         assert_same_state(g, o)
 
 
-@pytest.mark.parametrize("L,R", [(16, 1000), (6, 70), (10, 161), (32, 100), (4, 33)])
-def test_sweep_lane_split_kernel(monkeypatch, L, R):
+@pytest.mark.parametrize("L,R,mode,coupl", [(16, 1000, 0, False), (6, 70, 0, False), (10, 161, 0, True), (32, 100, 0, False), (4, 33, 0, False),
+                                             (16, 1000, 1, False), (12, 161, 1, True), (32, 100, 1, False), (8, 70, 1, False)])
+def test_sweep_lane_split_kernel(monkeypatch, L, R, mode, coupl):
     """Small populations on the generic path: S = 2, 4 lane-split CTAs per group, each running 8/S of every word's Philox calls
-    and writing back only its own bytes of the words -- the same bytes as one CTA per group and as the oracle (thresholds at
-    beta = 0 and at a T8 of 0 included; R = 1000 at L = 16 is configs[0]'s population, R = 161 has a ragged last word)."""
+    (or, in the LCG-assisted stream, jumping to the outputs of its lanes) and writing back only its own bytes of the words -- the
+    same bytes as one CTA per group and as the oracle (thresholds at beta = 0 and at a T8 of 0 included; R = 1000 at L = 16 is
+    configs[0]'s population, R = 161 has a ragged last word; ferromagnet and random +-J couplings)."""
+    from paper_1703_03676_b200.workloads import random_couplings
     seed = 4000 + L
     o = po.Oracle(L, R, seed)
+    o.set_rng_mode(mode)
+    if coupl:
+        Jx, Jy = random_couplings(L, seed)
+        o.set_couplings(Jx, Jy)
     plan = [(0.0, 1), (0.3, 2), (0.4406868, 3), (3.0, 1), (0.7, 2)]
     for beta, theta in plan:
         o.sweep(beta, theta)
@@ -390,6 +397,9 @@ def test_sweep_lane_split_kernel(monkeypatch, L, R):
         if split is not None:
             monkeypatch.setenv("PA_SWEEP_SPLIT", split)
         g = pa.Population(L, R, seed)
+        g.set_rng_mode(mode)
+        if coupl:
+            g.set_couplings(Jx, Jy)
         for beta, theta in plan:
             g.sweep(beta, theta)
         assert np.array_equal(g.get_spins(), want), split
