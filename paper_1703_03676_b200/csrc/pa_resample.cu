@@ -373,7 +373,13 @@ __device__ __forceinline__ void pa_copy_chunks(const uint4* __restrict__ src4, u
     for (int c = 0; c < NCH; ++c) out[i + c * stride] = acc[c];
 }
 
-__global__ void __launch_bounds__(128)
+#ifndef PA_COPY_MINB
+#define PA_COPY_MINB 8
+#endif
+#ifndef PA_COPY_NCH
+#define PA_COPY_NCH 4
+#endif
+__global__ void __launch_bounds__(128, PA_COPY_MINB)
 pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, const uint32_t* __restrict__ parent,
                PaScalars* sc, long long R_cap, int N, int commit) {
     __shared__ PaSeg segs[32];
@@ -444,6 +450,7 @@ pa_copy_kernel(const uint32_t* __restrict__ src, uint32_t* __restrict__ dst, con
     uint4* out = reinterpret_cast<uint4*>(dst + g * (long long)N);
     const int stride = gridDim.y * blockDim.x;
     int i = blockIdx.y * blockDim.x + tid;
+    for (; i + (PA_COPY_NCH - 1) * stride < chunks; i += PA_COPY_NCH * stride) pa_copy_chunks<PA_COPY_NCH>(src4, out, wins, nw, segs, chunks, i, stride);
     for (; i + stride < chunks; i += 2 * stride) pa_copy_chunks<2>(src4, out, wins, nw, segs, chunks, i, stride);
     if (i < chunks) pa_copy_chunks<1>(src4, out, wins, nw, segs, chunks, i, stride);
 }
