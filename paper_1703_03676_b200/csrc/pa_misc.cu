@@ -1,6 +1,7 @@
 // pa_misc.cu -- initial population (a0), energy histogram and multi-histogram
 // accumulation (a9), spin import/export, and the integer-pipe calibration kernels.
 #include "pa_common.cuh"
+#include <stdint.h>
 #include <math.h>
 
 
@@ -232,27 +233,46 @@ __global__ void pa_pack_kernel(uint32_t* __restrict__ pop, PaGeom L, int N, long
 }
 // The sweep kernels flip all 32 lanes of the last group, so the resident lanes past the population hold arbitrary bits (every
 // reader masks by j < R); the interchange words are canonical: dead lanes read as 0.
-__global__ void pa_words_out_kernel(const uint32_t* __restrict__ pop, PaGeom L, int N, long long R, uint32_t* __restrict__ out) {
-    const long long G = (R + 31) / 32;
-    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i >= G * N) return;
-    const long long g = i / N;
-    const int s = (int)(i - g * N);
-    uint32_t w = pop[g * N + pa_index_of_site(s, L)];
+// One thread per PAIR of sites (x = 2 xh, 2 xh + 1) of a lattice row: in the interchange layout the pair is 8 contiguous bytes, in the
+// resident layout its words sit at the same index (r, xh) of the two colour arrays -- which of the two takes the even x depends on the
+// parity of y + z.  Both sides are coalesced (the first version moved one word per thread with a 64-bit division and a stride-2
+// access: 1.7 TB/s; this one runs at the copy kernel's rate).  grid = (groups, pair blocks); V2: 8-byte accesses (aligned buffers).
+template <bool V2>
+__global__ void __launch_bounds__(256)
+pa_words_out_kernel(const uint32_t* __restrict__ pop, PaGeom L, int N, long long R, uint32_t* __restrict__ out) {
+    const long long g = blockIdx.x;
+    const int pr = blockIdx.y * blockDim.x + threadIdx.x, half = N >> 1;
+    if (pr >= half) return;
+    const int Lh = L.Lx >> 1;
+    const int r = pr / Lh, z = r / L.Ly, y = r - z * L.Ly;
+    const int q = (y + z) & 1;                                   // colour 0 holds x = 2 xh + q
+    const uint32_t* base = pop + g * (long long)N;
+    uint32_t w0 = base[pr], w1 = base[half + pr];                // colour 0, colour 1
     const long long live = R - g * 32;
-    if (live < 32) w &= (1u << live) - 1u;
-    out[i] = w;
+    if (live < 32) { const uint32_t m = (1u << live) - 1u; w0 &= m; w1 &= m; }
+    const uint32_t we = q ? w1 : w0, wo = q ? w0 : w1;           // even x, odd x
+    uint32_t* o = out + g * (long long)N + 2 * (long long)pr;
+    if (V2) *reinterpret_cast<uint2*>(o) = make_uint2(we, wo);
+    else { o[0] = we; o[1] = wo; }
 }
-__global__ void pa_words_in_kernel(uint32_t* __restrict__ pop, PaGeom L, int N, long long R, const uint32_t* __restrict__ in) {
-    const long long G = (R + 31) / 32;
-    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i >= G * N) return;
-    const long long g = i / N;
-    const int s = (int)(i - g * N);
-    uint32_t w = in[i];
+template <bool V2>
+__global__ void __launch_bounds__(256)
+pa_words_in_kernel(uint32_t* __restrict__ pop, PaGeom L, int N, long long R, const uint32_t* __restrict__ in) {
+    const long long g = blockIdx.x;
+    const int pr = blockIdx.y * blockDim.x + threadIdx.x, half = N >> 1;
+    if (pr >= half) return;
+    const int Lh = L.Lx >> 1;
+    const int r = pr / Lh, z = r / L.Ly, y = r - z * L.Ly;
+    const int q = (y + z) & 1;
+    const uint32_t* i2 = in + g * (long long)N + 2 * (long long)pr;
+    uint32_t we, wo;
+    if (V2) { const uint2 v = *reinterpret_cast<const uint2*>(i2); we = v.x; wo = v.y; }
+    else { we = i2[0]; wo = i2[1]; }
     const long long live = R - g * 32;
-    if (live < 32) w &= (1u << live) - 1u;
-    pop[g * N + pa_index_of_site(s, L)] = w;
+    if (live < 32) { const uint32_t m = (1u << live) - 1u; we &= m; wo &= m; }
+    uint32_t* base = pop + g * (long long)N;
+    base[pr] = q ? wo : we;
+    base[half + pr] = q ? we : wo;
 }
 
 int pa_launch_unpack(pa_handle* h, const int64_t* d_slots, int64_t j0, int64_t n, int8_t* d_out) {
@@ -273,27 +293,28 @@ int pa_launch_pack(pa_handle* h, int64_t j0, int64_t n, const int8_t* d_in) {
     h->launches += 1;
     return PA_OK;
 }
-int pa_launch_words_out(pa_handle* h, uint32_t* d_words) {
-    const long long G = (h->R_cur + 31) / 32, tot = G * h->N;
-    pa_words_out_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, h->R_cur, d_words);
+static bool pa_aligned8(const void* p) { return ((uintptr_t)p & 7u) == 0; }
+static int pa_words_out_groups(pa_handle* h, const uint32_t* pop, long long R_rel, uint32_t* d_words) {
+    const long long G = (R_rel + 31) / 32;
+    if (G <= 0) return PA_OK;
+    const dim3 grid((unsigned)G, (unsigned)((h->N / 2 + 255) / 256), 1);
+    if (pa_aligned8(d_words)) pa_words_out_kernel<true><<<grid, 256, 0, h->stream>>>(pop, h->geom, h->N, R_rel, d_words);
+    else pa_words_out_kernel<false><<<grid, 256, 0, h->stream>>>(pop, h->geom, h->N, R_rel, d_words);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;
 }
+int pa_launch_words_out(pa_handle* h, uint32_t* d_words) { return pa_words_out_groups(h, h->spins[h->cur], h->R_cur, d_words); }
 int pa_launch_words_out_range(pa_handle* h, uint32_t* d_words, int64_t g0, int64_t ng) {
     long long R_rel = h->R_cur - 32 * g0;                       // the kernel counts groups and live lanes from its base pointers
     if (R_rel > 32 * ng) R_rel = 32 * ng;
-    if (R_rel <= 0) return PA_OK;
-    const long long tot = (R_rel + 31) / 32 * h->N;
-    pa_words_out_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur] + g0 * (long long)h->N, h->geom, h->N, R_rel,
-                                                                              d_words + g0 * (long long)h->N);
-    PA_CUDA(h, cudaGetLastError());
-    h->launches += 1;
-    return PA_OK;
+    return pa_words_out_groups(h, h->spins[h->cur] + g0 * (long long)h->N, R_rel, d_words + g0 * (long long)h->N);
 }
 int pa_launch_words_in(pa_handle* h, int64_t R, const uint32_t* d_words) {
-    const long long G = (R + 31) / 32, tot = G * h->N;
-    pa_words_in_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, R, d_words);
+    const long long G = (R + 31) / 32;
+    const dim3 grid((unsigned)G, (unsigned)((h->N / 2 + 255) / 256), 1);
+    if (pa_aligned8(d_words)) pa_words_in_kernel<true><<<grid, 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, R, d_words);
+    else pa_words_in_kernel<false><<<grid, 256, 0, h->stream>>>(h->spins[h->cur], h->geom, h->N, R, d_words);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
     return PA_OK;

@@ -432,3 +432,25 @@ def test_sweep_mixed_launch(monkeypatch, L, R, rng):
         assert np.array_equal(g.get_spins(), want), mixed
         outs.append(g.get_words().tobytes())
     assert outs[0] == outs[1]
+
+
+def test_words_export_import_aligned_and_unaligned_device_buffers():
+    """pa_get_words / pa_set_words move a pair of sites per thread with 8-byte accesses when the caller's buffer allows it and with
+    4-byte accesses otherwise: same words through a host buffer, an aligned device buffer and one that starts 4 bytes into an
+    8-byte word; ragged last group (dead lanes 0); square lattice and a box."""
+    for dims, R in (((64, 64), 100), ((6, 6), 70), ((6, 4, 2), 45)):
+        g = pa.Population(dims[0], R, 9) if len(dims) == 2 else pa.Population.box(dims, R, 9)
+        g.sweep(0.3, 2)
+        host = g.get_words()
+        n = host.size
+        buf = torch.zeros(n + 1, dtype=torch.int32, device="cuda")
+        for off in (0, 1):
+            view = buf[off:off + n]
+            assert (view.data_ptr() % 8 == 0) == (off == 0)
+            view.zero_()
+            g.get_words(view)
+            assert np.array_equal(view.cpu().numpy().view(np.uint32).reshape(host.shape), host), (dims, off)
+            h2 = pa.Population(dims[0], R, 10) if len(dims) == 2 else pa.Population.box(dims, R, 10)
+            h2.set_words(R, view)
+            assert np.array_equal(h2.get_spins(), g.get_spins()), (dims, off)
+            assert np.array_equal(h2.get_words(), host)
