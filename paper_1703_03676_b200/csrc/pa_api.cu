@@ -117,6 +117,14 @@ static int pa_read_scalars(pa_handle* h) {
     PA_CUDA(h, cudaStreamSynchronize(h->stream));
     return PA_OK;
 }
+// The scalars of the measure kernel: its last CTA has written them into mapped host memory itself (no copy operation between
+// the kernel and the host's wake-up: a few microseconds per call on the launch-bound populations); else the copy above.
+static int pa_read_measure_scalars(pa_handle* h) {
+    if (!h->snap_on_host) return pa_read_scalars(h);
+    PA_CUDA(h, cudaStreamSynchronize(h->stream));
+    *h->h_scal = *h->h_snap;
+    return PA_OK;
+}
 
 static int pa_ensure_energies(pa_handle* h) { return h->em_valid ? PA_OK : pa_launch_measure(h); }
 
@@ -126,7 +134,7 @@ static int pa_ensure_host_scalars(pa_handle* h) {
     int rc = pa_ensure_energies(h);
     if (rc != PA_OK) return rc;
     if (h->host_scal_valid) return PA_OK;
-    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    if ((rc = pa_read_measure_scalars(h)) != PA_OK) return rc;
     h->host_scal_valid = true;
     h->Emin = -2 * h->nlev + 4 * (int)(0xffffffffu - h->h_scal->mmin_inv) + h->e0;
     h->Emax = -2 * h->nlev + 4 * (int)h->h_scal->mmax + h->e0;
@@ -229,7 +237,9 @@ static int pa_create_impl(int D, PaGeom geom, int64_t R, uint64_t seed, void* de
     h->d_slots = (int64_t*)(b + y.slots);
     h->stage = (int8_t*)(b + y.stage); h->stage_bytes = y.stage_bytes;
     // pinned host mirrors
-    if (cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
+    if (cudaHostAlloc(&h->h_snap, sizeof(PaScalars), cudaHostAllocMapped) != cudaSuccess ||
+        cudaHostGetDevicePointer(&h->h_snap_dev, h->h_snap, 0) != cudaSuccess ||
+        cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
         cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->nlev + 1)) != cudaSuccess ||
         cudaMallocHost(&h->h_adapt, sizeof(PaAdaptState)) != cudaSuccess) { rc = PA_ERR_CUDA; }
     for (int i = 0; i < 9 && rc == PA_OK; ++i)
@@ -259,6 +269,7 @@ void pa_destroy(pa_t* h) {
     cudaStreamSynchronize(h->stream);
     for (int i = 0; i < 9; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->h_scal) cudaFreeHost(h->h_scal);
+    if (h->h_snap) cudaFreeHost(h->h_snap);
     if (h->h_wtab) cudaFreeHost(h->h_wtab);
     if (h->h_adapt) cudaFreeHost(h->h_adapt);
     if (h->h_tabs) cudaFreeHost(h->h_tabs);
@@ -376,10 +387,16 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     if ((rc = pa_upload_wtab(h, dbeta, (Emax - Emin) / 4)) != PA_OK) return rc;
     // weights + W, plan (tau, r, scan, parents, R_new), copy: queued back to back; the copy reads R_new on
     // the device, so the host waits once, at the end
-    if ((rc = pa_launch_weights_plan(h, Emin, h->w, false)) != PA_OK) return rc;
-    // R_new and W travel to the host right after the plan kernel; the copy is queued behind them and runs
-    // while the host wakes up, so the stream never idles on this call's one synchronisation
-    PA_CUDA(h, cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToHost, h->stream));
+    // R_new and W travel to the host right after the plan kernel -- written by the kernel itself into mapped host memory
+    // (PA_SNAP_HOST=0: by a copy operation) --; the copy kernel is queued behind and runs while the host wakes up, so the stream
+    // never idles on this call's one synchronisation
+    const char* esh = getenv("PA_SNAP_HOST");
+    const bool mailed = h->h_snap_dev && !(esh && atoi(esh) == 0);
+    h->mail_out = mailed ? h->h_snap_dev : nullptr;
+    rc = pa_launch_weights_plan(h, Emin, h->w, false);
+    h->mail_out = nullptr;
+    if (rc != PA_OK) return rc;
+    if (!mailed) PA_CUDA(h, cudaMemcpyAsync(h->h_scal, h->d_scal, sizeof(PaScalars), cudaMemcpyDeviceToHost, h->stream));
     PA_CUDA(h, cudaEventRecord(h->ev[6], h->stream));                // the host waits on this one (created without timing)
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[4], h->stream));
     if ((rc = pa_launch_copy(h)) != PA_OK) return rc;
@@ -387,6 +404,7 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[3], h->stream));
     PA_CUDA(h, cudaEventSynchronize(h->ev[6]));
     h->resample_timed = timed;
+    if (mailed) { h->h_scal->R_new = h->h_snap->R_new; h->h_scal->W = h->h_snap->W; }
     const int64_t R_new = (int64_t)h->h_scal->R_new;
     const double W = h->h_scal->W;
     if (R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;      // population, k, lnZ, R_prev unchanged (O7): only the spare buffer was written

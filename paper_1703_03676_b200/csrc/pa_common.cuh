@@ -169,6 +169,9 @@ struct pa_handle {
     int64_t n_tiles_cap;
 
     PaScalars* h_scal;                  // pinned
+    PaScalars *h_snap, *h_snap_dev;     // pinned and mapped: the measure kernel's last CTA leaves the scalars there itself (single calls)
+    bool snap_on_host;                  // ... and has done so for the current population
+    PaScalars* mail_out;                // pa_resample: where the plan kernel leaves R_new and W for the host (mapped memory), or NULL
     double* h_wtab;                     // pinned, N+1
     int64_t R_prev; double W_last;      // of the last resample
 

@@ -364,6 +364,12 @@ int pa_launch_measure(pa_handle* h) {
     h->scal_zeroed = false;
     const bool timed = (h->timing & PA_TIME_MEASURE) != 0;
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
+    // single calls: the last CTA writes the finished scalars straight into mapped host memory (pa_read_measure_scalars)
+    const char* esh = getenv("PA_SNAP_HOST");                          // PA_SNAP_HOST=0: device-to-host copy instead
+    const bool to_host = !h->dev_R && !h->snap_out && h->h_snap_dev && !(esh && atoi(esh) == 0);
+    PaScalars* const snap_save = h->snap_out;
+    if (to_host) h->snap_out = h->h_snap_dev;
+    h->snap_on_host = to_host;
     cudaError_t le = cudaSuccess;
     const bool pow2 = h->D == 2 && (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
     if (pow2) {
@@ -390,6 +396,7 @@ int pa_launch_measure(pa_handle* h) {
         }
 #undef PA_MG_CASE
     }
+    h->snap_out = snap_save;
     PA_CUDA(h, le);
     PA_CUDA(h, cudaGetLastError());
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[8], h->stream));

@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(256)
 pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* sc,
                long long R, double R_target, int Emin, PhiloxKeys K, uint32_t kcount, long long R_cap,
                uint32_t* __restrict__ r_out, uint32_t* __restrict__ o_out, uint32_t* __restrict__ parent,
-               unsigned long long* __restrict__ state, int n_tiles, int N, int e0) {
+               unsigned long long* __restrict__ state, int n_tiles, int N, int e0, PaScalars* __restrict__ mail) {
     __shared__ uint32_t s_tile, s_warp[8], s_excl;
     pa_pdl_wait(); pa_pdl_launch();
     R = pa_live_R(R, sc);
@@ -176,7 +176,10 @@ pa_plan_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
         }
         if (lane == 0) {
             s_excl = excl;
-            if ((int)tile == n_tiles - 1) sc->R_new = excl + btotal;
+            if ((int)tile == n_tiles - 1) {
+                sc->R_new = excl + btotal;
+                if (mail) { mail->R_new = excl + btotal; mail->W = sc->W; }     // single calls: straight into mapped host memory
+            }
         }
     }
     __syncthreads();
@@ -199,7 +202,7 @@ int pa_launch_plan(pa_handle* h, int Emin) {
     const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
     PA_CUDA(h, pa_launch(h, pa_plan_kernel, dim3(n), dim3(256), 0, (const int32_t*)h->E, h->wtab_cur ? h->wtab_cur : (const double*)h->wtab,
                          h->d_scal, (long long)(h->dev_R ? -1 : h->R_cur), (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, h->keys, h->k,
-                         (long long)h->R_cap, h->r, h->o, h->parent, h->scan_state, n, h->nlev, h->e0));
+                         (long long)h->R_cap, h->r, h->o, h->parent, h->scan_state, n, h->nlev, h->e0, h->mail_out));
     h->launches += 1;
     return PA_OK;
 }
@@ -216,7 +219,7 @@ __global__ void __launch_bounds__(PA_TILE)
 pa_tree_plan_small_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* sc,
                           long long R, double R_target, int Emin, PhiloxKeys K, uint32_t kcount, long long R_cap,
                           double* __restrict__ w_out, uint32_t* __restrict__ r_out, uint32_t* __restrict__ o_out,
-                          uint32_t* __restrict__ parent, int n_tiles, int N, int e0, int commit) {
+                          uint32_t* __restrict__ parent, int n_tiles, int N, int e0, int commit, PaScalars* __restrict__ mail) {
     __shared__ double run[32];
     __shared__ double s_W;
     __shared__ uint32_t s_wsum[32];
@@ -288,6 +291,7 @@ pa_tree_plan_small_kernel(const int32_t* __restrict__ E, const double* __restric
     }
     if (tid == 0) {
         sc->R_new = base;
+        if (mail) { mail->R_new = base; mail->W = W; }
         if (commit) {
             // pa_anneal with the copy fused into the sweep kernel's staging (pa_sweep_split_kernel<S, true>): what pa_copy_kernel's
             // first thread does there -- the new population size becomes current on the device (or the error flag is raised) and the
@@ -318,7 +322,7 @@ int pa_launch_weights_plan(pa_handle* h, int Emin, double* w_out, bool commit) {
     PA_CUDA(h, pa_launch(h, pa_tree_plan_small_kernel, dim3(1), dim3(PA_TILE), 0, (const int32_t*)h->E,
                          h->wtab_cur ? h->wtab_cur : (const double*)h->wtab, h->d_scal, (long long)(h->dev_R ? -1 : h->R_cur),
                          (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, h->keys, h->k, (long long)h->R_cap, w_out,
-                         h->r, h->o, h->parent, n, h->nlev, h->e0, commit ? 1 : 0));
+                         h->r, h->o, h->parent, n, h->nlev, h->e0, commit ? 1 : 0, h->mail_out));
     h->launches += 1;
     if (commit) h->scal_zeroed = true;
     return PA_OK;
