@@ -70,14 +70,15 @@ __device__ __forceinline__ double pa_alpha_hist(const uint32_t* hs, double* ws, 
 
 __global__ void __launch_bounds__(1024)
 pa_adapt_kernel(const uint32_t* __restrict__ Hd, const PaScalars* __restrict__ sc, double R_target, double R_cur, double target,
-                double bound, PaAdaptState* __restrict__ st) {
+                double bound, const PaAdaptState in, PaAdaptState* __restrict__ st) {
+    // the bisection state comes in as a kernel argument and goes out into mapped host memory: no copy operation either way
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double sh[32];
     const int m_lo = (int)(0xffffffffu - sc->mmin_inv), dmax = (int)sc->mmax - m_lo;
-    double lo = st->lo, hi = st->hi;
-    int it = st->it;
+    double lo = in.lo, hi = in.hi;
+    int it = in.it;
     if (dmax + 1 > PA_ADAPT_BINS) {                                              // wider than the shared-memory table: all exact
-        if (threadIdx.x == 0) st->status = it < 0 ? PA_ADAPT_AMBIG_FIRST : PA_ADAPT_AMBIG;
+        if (threadIdx.x == 0) { st->lo = lo; st->hi = hi; st->it = it; st->status = it < 0 ? PA_ADAPT_AMBIG_FIRST : PA_ADAPT_AMBIG; }
         return;
     }
     double* ws = reinterpret_cast<double*>(smem_raw);
@@ -118,11 +119,10 @@ int pa_launch_ehist(pa_handle* h) {
 int pa_run_adapt_filter(pa_handle* h, double target, double bound) {
     const size_t smem = (size_t)PA_ADAPT_BINS * (8 + 4);
     PA_CUDA(h, cudaFuncSetAttribute(pa_adapt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    PA_CUDA(h, cudaMemcpyAsync(h->d_adapt, h->h_adapt, sizeof(PaAdaptState), cudaMemcpyHostToDevice, h->stream));
-    pa_adapt_kernel<<<1, 1024, smem, h->stream>>>(h->Hd, h->d_scal, (double)h->R_target, (double)h->R_cur, target, bound, h->d_adapt);
+    pa_adapt_kernel<<<1, 1024, smem, h->stream>>>(h->Hd, h->d_scal, (double)h->R_target, (double)h->R_cur, target, bound, *h->h_adapt,
+                                                  h->h_adapt_dev);
     PA_CUDA(h, cudaGetLastError());
     h->launches += 1;
-    PA_CUDA(h, cudaMemcpyAsync(h->h_adapt, h->d_adapt, sizeof(PaAdaptState), cudaMemcpyDeviceToHost, h->stream));
     PA_CUDA(h, cudaStreamSynchronize(h->stream));
     return PA_OK;
 }

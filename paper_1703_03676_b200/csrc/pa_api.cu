@@ -241,7 +241,8 @@ static int pa_create_impl(int D, PaGeom geom, int64_t R, uint64_t seed, void* de
         cudaHostGetDevicePointer(&h->h_snap_dev, h->h_snap, 0) != cudaSuccess ||
         cudaMallocHost(&h->h_scal, sizeof(PaScalars)) != cudaSuccess ||
         cudaMallocHost(&h->h_wtab, sizeof(double) * ((size_t)h->nlev + 1)) != cudaSuccess ||
-        cudaMallocHost(&h->h_adapt, sizeof(PaAdaptState)) != cudaSuccess) { rc = PA_ERR_CUDA; }
+        cudaHostAlloc(&h->h_adapt, sizeof(PaAdaptState), cudaHostAllocMapped) != cudaSuccess ||
+        cudaHostGetDevicePointer(&h->h_adapt_dev, h->h_adapt, 0) != cudaSuccess) { rc = PA_ERR_CUDA; }
     for (int i = 0; i < 9 && rc == PA_OK; ++i)
         if (cudaEventCreateWithFlags(&h->ev[i], i == 6 ? cudaEventDisableTiming : cudaEventDefault) != cudaSuccess) rc = PA_ERR_CUDA;
     if (rc == PA_OK) rc = pa_sweep_configure(h);
@@ -425,8 +426,14 @@ static int pa_eval_overlap(pa_handle* h, double dbeta, int Emin, int Emax, doubl
     int rc;
     if ((rc = pa_upload_wtab(h, dbeta, (Emax - Emin) / 4)) != PA_OK) return rc;
     if ((rc = pa_launch_weights(h, Emin, nullptr)) != PA_OK) return rc;
-    if ((rc = pa_launch_overlap(h, Emin)) != PA_OK) return rc;
-    if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
+    const char* esh = getenv("PA_SNAP_HOST");
+    const bool mailed = h->h_snap_dev && !(esh && atoi(esh) == 0);      // the kernel writes the sum into mapped host memory itself
+    h->mail_out = mailed ? h->h_snap_dev : nullptr;
+    rc = pa_launch_overlap(h, Emin);
+    h->mail_out = nullptr;
+    if (rc != PA_OK) return rc;
+    if (mailed) { PA_CUDA(h, cudaStreamSynchronize(h->stream)); h->h_scal->sum = h->h_snap->sum; }
+    else if ((rc = pa_read_scalars(h)) != PA_OK) return rc;
     *alpha = h->h_scal->sum / (double)h->R_cur;
     return PA_OK;
 }

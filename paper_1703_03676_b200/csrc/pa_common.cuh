@@ -158,7 +158,8 @@ struct pa_handle {
     unsigned long long* Hsum;           // [N+1]
     uint32_t* Hcur;                     // [N+1] histogram of the current temperature
     uint32_t* Hd;                       // [N+1] count-only histogram of the current population for pa_adapt_dbeta
-    PaAdaptState *d_adapt, *h_adapt;    // bisection state, device / pinned host
+    PaAdaptState *d_adapt, *h_adapt;    // bisection state, device / pinned host (mapped: the kernel writes it there)
+    PaAdaptState* h_adapt_dev;          // device address of h_adapt
     int adapt_exact_evals, adapt_filter_launches;   // of the last pa_adapt_dbeta (diagnostics)
     double* lnD;                        // [N+1]
     unsigned long long *A1, *A2;        // [N+1] sums of |M_j| and M_j^2 per energy level over all folded replicas (O14)

@@ -19,7 +19,7 @@ template <int MODE>
 __global__ void __launch_bounds__(PA_TILE)
 pa_tree_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, PaScalars* __restrict__ sc,
                long long R, double R_target, int Emin, double* __restrict__ w_out, double* __restrict__ partials,
-               unsigned long long* __restrict__ scan_state, int N, int e0) {
+               unsigned long long* __restrict__ scan_state, int N, int e0, PaScalars* __restrict__ mail) {
     __shared__ double run[32];
     __shared__ bool s_last;
     pa_pdl_wait(); pa_pdl_launch();
@@ -65,7 +65,7 @@ pa_tree_kernel(const int32_t* __restrict__ E, const double* __restrict__ wtab, P
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        if (MODE == 0) sc->W = total; else sc->sum = total;
+        if (MODE == 0) sc->W = total; else { sc->sum = total; if (mail) mail->sum = total; }    // mail: mapped host memory (pa_eval_overlap)
         sc->tree_ticket = 0u;
     }
 }
@@ -74,7 +74,7 @@ int pa_launch_weights(pa_handle* h, int Emin, double* w_out) {
     const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
     PA_CUDA(h, pa_launch(h, pa_tree_kernel<0>, dim3(n), dim3(PA_TILE), 0, (const int32_t*)h->E, h->wtab_cur ? h->wtab_cur : (const double*)h->wtab,
                          h->d_scal, (long long)(h->dev_R ? -1 : h->R_cur), (double)h->R_target, h->dev_R ? PA_EMIN_DEV : Emin, w_out,
-                         h->partials, h->scan_state, h->nlev, h->e0));
+                         h->partials, h->scan_state, h->nlev, h->e0, (PaScalars*)nullptr));
     h->launches += 1;
     return PA_OK;
 }
@@ -82,7 +82,7 @@ int pa_launch_weights(pa_handle* h, int Emin, double* w_out) {
 int pa_launch_overlap(pa_handle* h, int Emin) {
     const int n = (int)((h->R_cur + PA_TILE - 1) / PA_TILE);
     PA_CUDA(h, pa_launch(h, pa_tree_kernel<1>, dim3(n), dim3(PA_TILE), 0, (const int32_t*)h->E, (const double*)h->wtab, h->d_scal,
-                         (long long)h->R_cur, (double)h->R_target, Emin, (double*)nullptr, h->partials, h->scan_state, h->nlev, h->e0));
+                         (long long)h->R_cur, (double)h->R_target, Emin, (double*)nullptr, h->partials, h->scan_state, h->nlev, h->e0, h->mail_out));
     h->launches += 1;
     return PA_OK;
 }
