@@ -454,3 +454,19 @@ def test_words_export_import_aligned_and_unaligned_device_buffers():
             h2.set_words(R, view)
             assert np.array_equal(h2.get_spins(), g.get_spins()), (dims, off)
             assert np.array_equal(h2.get_words(), host)
+
+
+@pytest.mark.parametrize("L,R", [(64, 130), (64, 96), (128, 70)])
+def test_sweep_lcg_p64_words_opt_in(monkeypatch, L, R):
+    """PA_LCG_P64=1: the LCG column-walk kernel on 64-replica words (two adjacent groups side by side; Table 1 measures
+    p = 64) -- the stream is defined per 32-replica word (O11), so the bytes are the p = 32 kernel's and the
+    oracle's; an odd number of groups leaves the last pair half empty."""
+    seed = 6000 + L
+    o = po.Oracle(L, R, seed); o.set_rng_mode(po.RNG_LCG)
+    o.sweep(0.3, 2); o.sweep(0.44, 1)
+    want = o.get_spins()
+    for p64 in ("1", "0"):
+        monkeypatch.setenv("PA_LCG_P64", p64)
+        g = pa.Population(L, R, seed); g.set_rng_mode(pa.PA_RNG_LCG)
+        g.sweep(0.3, 2); g.sweep(0.44, 1)
+        assert np.array_equal(g.get_spins(), want), p64
