@@ -306,3 +306,37 @@ def test_step_host_equals_single_calls_and_oracle(monkeypatch, L, R, mode, theta
         assert a.sweep_counter == b.sweep_counter == o.sweep_counter and a.lnZ == b.lnZ
         Ra = Rb = Ra_new
     assert np.array_equal(a.get_spins(), o.get_spins())
+
+
+def test_environment_switches_give_the_same_bytes(monkeypatch):
+    """Every tuning / fallback switch of DESIGN.md Sec. 13 that no other test sets: the same run (single calls, then pa_anneal) with
+    the switch set gives the bytes and observables of the default path, which equals the oracle."""
+    switches = ("PA_PDL", "PA_SMALL_PLAN", "PA_FUSE_COPY", "PA_SNAP_HOST", "PA_LCG_NOR", "PA_SWEEP_SMEM_KB", "PA_SWEEP_CMP")
+    cases = [((16, 1000, 0), [{}, {"PA_PDL": "0"}, {"PA_SMALL_PLAN": "0"}, {"PA_FUSE_COPY": "0"}, {"PA_SNAP_HOST": "0"},
+                              {"PA_SMALL_PLAN": "0", "PA_SNAP_HOST": "0", "PA_PDL": "0"}]),
+             ((64, 700, 1), [{}, {"PA_LCG_NOR": "0"}, {"PA_LCG_NOR": "2"}, {"PA_LCG_NOR": "6"}, {"PA_LCG_NOR": "8"}, {"PA_PDL": "0"}]),
+             ((128, 100, 0), [{}, {"PA_SWEEP_SMEM_KB": "32"}, {"PA_SWEEP_CMP": "2"}, {"PA_SNAP_HOST": "0"}])]
+    betas = [0.0, 0.1, 0.25, 0.25, 0.45, 0.7]
+    for (L, R, mode), envs in cases:
+        o = po.Oracle(L, R, 47); o.set_rng_mode(mode)
+        obs_o = pa_driver.run_fixed(o, betas[:4], 2)[1:]
+        o_mid = o.get_spins().tobytes()
+        ref = None
+        for env in envs:
+            for k in switches:
+                monkeypatch.delenv(k, raising=False)
+            for k, v in env.items():
+                monkeypatch.setenv(k, v)
+            g = pa.Population(L, R, 47); g.set_rng_mode(mode)
+            obs = pa_driver.run_fixed(g, betas[:4], 2)[1:]
+            mid = g.get_spins().tobytes()
+            obs += g.anneal(betas[3:], 2)
+            out = (mid, _state(g), repr(obs))
+            if ref is None:
+                ref = out
+                assert mid == o_mid
+                for a, b in zip(obs[:3], obs_o):
+                    for k in KEYS:
+                        assert a[k] == pytest.approx(b[k], rel=REL, abs=1e-300), k
+            else:
+                assert out == ref, (L, env)
