@@ -356,6 +356,78 @@ pa_measure_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur,
     pa_measure_tail<NPW>(pe, pm, g, N, N, R_cur, E, M, sc, runsum, blocksum, snap);
 }
 
+// ------------------------------------------------------------------------------------------------
+// The quad-column walk for cubes of 8, 16, 32 (O16): a thread owns one quad column of ONE z-plane and walks down y; the row below is
+// its own next load, the row of the plane above (+z bond) a second stream of loads, the +y bond of the plane's last row leads back
+// to its first.  Per row and thread: 24 bond words (x, y, z) -> three 8-input carry-save blocks, 8 spin words -> one; the rows' top
+// carries go through the eight-row ladder.  (The any-edge kernel spends 91 instructions per word on index arithmetic: 0.44 ms at
+// 32^3, R = 10^5, against a 0.07 ms HBM floor.)
+// ------------------------------------------------------------------------------------------------
+template <int LOG_QPR>
+__global__ void __launch_bounds__(128)
+pa_measure3d_kernel(const uint32_t* __restrict__ pop, int N, long long R_cur, int32_t* __restrict__ E, int32_t* __restrict__ M,
+                    PaScalars* __restrict__ sc, double* __restrict__ runsum, double* __restrict__ blocksum,
+                    PaScalars* __restrict__ snap, int nlev) {
+    constexpr int QPR = 1 << LOG_QPR, L = 8 * QPR, Lq = QPR;             // Lq = uint4 per colour row
+    constexpr int NPE = pa_bits(24 * L), NPM = pa_bits(8 * L), NPW = NPE + 5;
+    static_assert(NPE >= 8 && NPM >= 6, "ladder planes");
+    pa_pdl_wait(); pa_pdl_launch();
+    const long long g = blockIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const bool act = tid < L * QPR;
+    const int q = tid & (QPR - 1), z = act ? (tid >> LOG_QPR) : 0;
+    const uint4* c0 = reinterpret_cast<const uint4*>(pop + g * (long long)N);
+    const uint4* c1 = c0 + (N >> 3);
+    const int r0 = z * L, rz = ((z + 1) & (L - 1)) * L;                   // first row of this plane / of the plane above
+    const int nxt_lane = (lane & ~(QPR - 1)) | ((lane + 1) & (QPR - 1));
+    const uint4 zero = make_uint4(0, 0, 0, 0);
+    PlaneCounter<NPE> cE; PlaneCounter<NPM> cM;
+    cE.clear(); cM.clear();
+    uint4 a = zero, b = zero, na = zero, nb = zero, za = zero, zb = zero;
+    if (act) {
+        a = __ldg(c0 + r0 * Lq + q); b = __ldg(c1 + r0 * Lq + q);
+        na = __ldg(c0 + (r0 + 1) * Lq + q); nb = __ldg(c1 + (r0 + 1) * Lq + q);
+        za = __ldg(c0 + rz * Lq + q); zb = __ldg(c1 + rz * Lq + q);
+    }
+    uint32_t ce[8], cm[8];
+#pragma unroll 8
+    for (int y = 0; y < L; ++y) {
+        uint4 fa = zero, fb = zero, fza = zero, fzb = zero;               // rows (z, y+2) and (z+1, y+1), in flight while row y is counted
+        if (act) {
+            const int y2 = (y + 2) & (L - 1), y1 = (y + 1) & (L - 1);
+            fa = __ldg(c0 + (r0 + y2) * Lq + q); fb = __ldg(c1 + (r0 + y2) * Lq + q);
+            fza = __ldg(c0 + (rz + y1) * Lq + q); fzb = __ldg(c1 + (rz + y1) * Lq + q);
+        }
+        const bool odd = ((y + z) & 1) != 0;                               // colour 0 holds x = 2 xh + ((y + z) & 1)
+        const uint4 t = odd ? b : a, u = odd ? a : b;                      // bond u[xh] - t[xh + 1]
+        const uint32_t tn = __shfl_sync(0xffffffffu, t.x, nxt_lane);
+        uint32_t xb[24];
+        xb[0] = a.x ^ b.x; xb[1] = a.y ^ b.y; xb[2] = a.z ^ b.z; xb[3] = a.w ^ b.w;          // x bonds inside a pair
+        xb[4] = u.x ^ t.y; xb[5] = u.y ^ t.z; xb[6] = u.z ^ t.w; xb[7] = u.w ^ tn;           // x bonds between pairs
+        xb[8] = a.x ^ nb.x; xb[9] = a.y ^ nb.y; xb[10] = a.z ^ nb.z; xb[11] = a.w ^ nb.w;    // +y bonds
+        xb[12] = b.x ^ na.x; xb[13] = b.y ^ na.y; xb[14] = b.z ^ na.z; xb[15] = b.w ^ na.w;
+        xb[16] = a.x ^ zb.x; xb[17] = a.y ^ zb.y; xb[18] = a.z ^ zb.z; xb[19] = a.w ^ zb.w;  // +z bonds
+        xb[20] = b.x ^ za.x; xb[21] = b.y ^ za.y; xb[22] = b.z ^ za.z; xb[23] = b.w ^ za.w;
+        const uint32_t xs[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+        {   // 24 inputs: three blocks of eight, their weight-8 carries into plane 3, the two weight-16 carries into plane 4
+            const uint32_t e1 = cE.block8(xb), e2 = cE.block8(xb + 8), e3 = cE.block8(xb + 16);
+            uint32_t c16, c32;
+            pa_csa(c16, cE.pl[3], cE.pl[3], e1, e2);
+            const uint32_t t16 = cE.pl[3] & e3;
+            cE.pl[3] ^= e3;
+            pa_csa(c32, cE.pl[4], cE.pl[4], c16, t16);
+            ce[y & 7] = c32;
+        }
+        cm[y & 7] = cM.block8(xs);
+        if ((y & 7) == 7) { cE.template ladder8<5>(ce); cM.template ladder8<3>(cm); }
+        a = na; b = nb; na = fa; nb = fb; za = fza; zb = fzb;
+    }
+    uint32_t pe[NPW], pm[NPW];
+#pragma unroll
+    for (int k = 0; k < NPW; ++k) { pe[k] = k < NPE ? cE.pl[k < NPE ? k : 0] : 0u; pm[k] = k < NPM ? cM.pl[k < NPM ? k : 0] : 0u; }
+    pa_measure_tail<NPW>(pe, pm, g, N, nlev, R_cur, E, M, sc, runsum, blocksum, snap);
+}
+
 int pa_launch_measure(pa_handle* h) {
     const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;      // dead groups contribute zeros (and +0.0 to the m^4 tree)
     const long long Rarg = h->dev_R ? -1 : h->R_cur;
@@ -381,6 +453,13 @@ int pa_launch_measure(pa_handle* h) {
         break;
         switch (L) { PA_MSR_CASE(0) PA_MSR_CASE(1) PA_MSR_CASE(2) PA_MSR_CASE(3) PA_MSR_CASE(4) PA_MSR_CASE(5) default: break; }
 #undef PA_MSR_CASE
+    } else if (h->D == 3 && !h->has_j && h->geom.Lx == h->geom.Ly && h->geom.Lx == h->geom.Lz && (L == 8 || L == 16 || L == 32) &&
+               getenv("PA_MEASURE_GENERIC") == nullptr) {
+        const int T3 = L * (L / 8) < 32 ? 32 : L * (L / 8);
+#define PA_M3_CASE(LOG) le = pa_launch(h, pa_measure3d_kernel<LOG>, dim3((unsigned)G), dim3(T3), 0, (const uint32_t*)h->spins[h->cur], h->N, Rarg, \
+            h->E, h->M, h->d_scal, h->runsum, h->partials, h->snap_out, h->nlev)
+        if (L == 8) PA_M3_CASE(0); else if (L == 16) PA_M3_CASE(1); else PA_M3_CASE(2);
+#undef PA_M3_CASE
     } else {
         int T = 256;
         while (T > 32 && T * 8 > h->N) T >>= 1;
