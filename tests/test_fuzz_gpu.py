@@ -101,3 +101,84 @@ def test_random_case(i):
     assert np.array_equal(g.histogram()[0], o.histogram()[0])
     for x, y in zip(g.mag_sums(), o.mag_sums()):
         assert np.array_equal(x, y)
+
+
+def _run_pair(g, o, betas, theta, api, tag):
+    """Advance both through the schedule (single calls or one pa_anneal call) and compare everything."""
+    oo = []
+    for k in range(1, len(betas)):
+        o.resample(betas[k - 1], betas[k]); o.sweep(betas[k], theta)
+        oo.append(o.observables(betas[k]))
+    if api == "anneal":
+        g.observables(betas[0])
+        og = g.anneal(betas, theta)
+    elif api == "host":
+        Gc = (g.capacity + 31) // 32
+        w = torch.zeros((Gc, g.N), dtype=torch.int32, pin_memory=True)
+        g.get_words(w)
+        og, Rh = [], g.population
+        for k in range(1, len(betas)):
+            ob, Rh = g.step_host(Rh, w, betas[k - 1], betas[k], theta, w)
+            og.append(ob)
+    else:
+        og = []
+        for k in range(1, len(betas)):
+            g.resample(betas[k - 1], betas[k]); g.sweep(betas[k], theta)
+            og.append(g.observables(betas[k]))
+    for a, b in zip(og, oo):
+        for key in KEYS:
+            assert a[key] == pytest.approx(b[key], rel=REL, abs=1e-300), (tag, key, a[key], b[key])
+    assert g.population == o.population and g.sweep_counter == o.sweep_counter and g.resample_counter == o.resample_counter
+    assert np.array_equal(g.get_spins(), o.get_spins()), tag
+    Eg, Mg = g.energies(); Eo, Mo = o.energies()
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo), tag
+
+
+@pytest.mark.parametrize("i", range(int(os.environ.get("PA_FUZZ_BOX_N", "16"))))
+def test_random_box_case(i):
+    """The same differential fuzz on random periodic boxes (O16): even edges from 2 (double bonds) to 16, cubes of 8 and 16 (the
+    column-walk sweep and quad-column energy kernels) and boxes with three different edges (the any-edge kernels), ragged
+    populations, single calls / pa_anneal / pa_step_host."""
+    rng = np.random.default_rng(70000 + i)
+    if rng.integers(0, 3) == 0:
+        e = int(rng.choice([8, 16])); dims = (e, e, e)
+    else:
+        dims = tuple(int(v) for v in rng.choice([2, 4, 6, 8, 10, 12, 16], size=3))
+    R = int(rng.choice([1, 31, 33, 100, 257, 700]))
+    if np.prod(dims) >= 2048:
+        R = min(R, 100)
+    theta = int(rng.choice([1, 1, 2, 3]))
+    steps = rng.choice([0.0, 0.01, 0.05, 0.1, 0.3], size=int(rng.integers(2, 5)), p=[0.1, 0.25, 0.35, 0.2, 0.1])
+    betas = np.concatenate([[0.0], np.cumsum(steps)]).tolist()
+    api = str(rng.choice(["steps", "anneal", "host"]))
+    o = po.Oracle.box(dims, R, 500 + i)
+    try:
+        probe = po.Oracle.box(dims, R, 500 + i)
+        for k in range(1, len(betas)):
+            probe.resample(betas[k - 1], betas[k]); probe.sweep(betas[k], theta)
+    except Exception:
+        pytest.skip("the population dies out on this schedule (covered by test_random_case)")
+    g = pa.Population.box(dims, R, 500 + i)
+    _run_pair(g, o, betas, theta, api, (i, dims, R, api))
+
+
+@pytest.mark.parametrize("i", range(int(os.environ.get("PA_FUZZ_MEDIUM_N", "6"))))
+def test_random_medium_case(i):
+    """Medium populations on the column-walk kernels: random sizes around whole rounds of the 148 SMs (the mixed launch of whole
+    groups plus lane-quarter CTAs, its capacity-sized grid inside pa_anneal, the chunked sweeps of pa_step_host), both streams."""
+    rng = np.random.default_rng(80000 + i)
+    L = int(rng.choice([64, 64, 128]))
+    rounds = int(rng.integers(1, 3)) if L == 64 else 1
+    R = 32 * 148 * rounds + int(rng.integers(-40, 1500))
+    mode = int(rng.integers(0, 2))
+    theta = int(rng.choice([1, 2]))
+    betas = [0.0, 0.2, 0.2 + float(rng.choice([0.05, 0.25]))]
+    api = str(rng.choice(["steps", "anneal", "host"]))
+    if api == "host":
+        os.environ["PA_STEP_HOST_CHUNK"] = str(int(rng.choice([37, 60, 148])))
+    try:
+        g, o = pa.Population(L, R, 900 + i), po.Oracle(L, R, 900 + i)
+        g.set_rng_mode(mode); o.set_rng_mode(mode)
+        _run_pair(g, o, betas, theta, api, (i, L, R, mode, api))
+    finally:
+        os.environ.pop("PA_STEP_HOST_CHUNK", None)
