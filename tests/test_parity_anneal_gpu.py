@@ -340,3 +340,46 @@ def test_environment_switches_give_the_same_bytes(monkeypatch):
                         assert a[k] == pytest.approx(b[k], rel=REL, abs=1e-300), k
             else:
                 assert out == ref, (L, env)
+
+
+def test_step_host_errors_leave_the_handle_usable():
+    """pa_step_host: device buffers, a negative theta, a decreasing beta and a population size outside [1, R_cap] are refused with
+    PA_ERR_INVALID_ARG before anything is touched; a step that would empty the population returns PA_ERR_CAPACITY, leaves the
+    uploaded population in the handle and words_out untouched."""
+    L, R = 8, 40
+    g = pa.Population(L, R, 5)
+    Gc = (g.capacity + 31) // 32
+    w = torch.zeros((Gc, L * L), dtype=torch.int32, pin_memory=True)
+    g.get_words(w)
+    before = g.get_spins().copy()
+    dev = w.cuda()
+    for args in ((R, dev, 0.0, 0.1, 1, w), (R, w, 0.0, 0.1, 1, dev), (R, w, 0.0, 0.1, -1, w), (R, w, 0.2, 0.1, 1, w),
+                 (0, w, 0.0, 0.1, 1, w), (g.capacity + 1, w, 0.0, 0.1, 1, w)):
+        with pytest.raises(pa.PaError) as e:
+            g.step_host(*args)
+        assert e.value.code == pa.PA_ERR_INVALID_ARG
+    assert np.array_equal(g.get_spins(), before) and g.population == R and g.sweep_counter == 0
+    # one replica and a huge step: tau < 1 for ... a single replica always has tau = 1, so take two replicas with different energies
+    g2 = pa.Population(4, 2, 1)
+    o2 = po.Oracle(4, 2, 1)
+    w2 = torch.zeros(((g2.capacity + 31) // 32, 16), dtype=torch.int32, pin_memory=True)
+    g2.get_words(w2)
+    out = torch.full_like(w2, 0x5a5a5a5a)
+    died = False
+    beta = 0.0
+    for k in range(40):                                   # strong steps until the oracle's population dies out (or 40 steps pass)
+        try:
+            o2.resample(beta, beta + 2.0)
+        except Exception:
+            died = True
+            with pytest.raises(pa.PaError) as e:
+                g2.step_host(g2.population, w2, beta, beta + 2.0, 1, out)
+            assert e.value.code == pa.PA_ERR_CAPACITY
+            assert torch.all(out == 0x5a5a5a5a)
+            assert np.array_equal(g2.get_spins(), o2.get_spins()) and g2.population == o2.population
+            break
+        o2.sweep(beta + 2.0, 1)
+        _, Rn = g2.step_host(g2.population, w2, beta, beta + 2.0, 1, w2)
+        assert Rn == o2.population and np.array_equal(g2.get_spins(), o2.get_spins())
+        beta += 2.0
+    assert died or g2.population == o2.population
