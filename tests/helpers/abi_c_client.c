@@ -40,6 +40,17 @@ int main(int argc, char** argv) {
     if (pa_reweight(h, 1, grid, lnZ, e, C, NULL, NULL) != PA_OK) return 13;
     printf("reweighted to beta=%.2f: lnZ=%.6f e=%.6f C=%.6f\n", grid[0], lnZ[0], e[0], C[0]);
     if (pa_resample(h, 0.5, 0.4, &R_new) != PA_ERR_INVALID_ARG) return 14;     /* beta' < beta */
+    {   /* one more step with the population in (pageable) host memory between the calls: pa_get_words, then pa_step_host */
+        size_t nw = (size_t)((pa_capacity_of(h) + 31) / 32) * (size_t)L * (size_t)L;
+        uint32_t* words = (uint32_t*)malloc(sizeof(uint32_t) * nw);
+        int64_t R_host = pa_population(h);
+        if (!words) return 15;
+        if (pa_get_words(h, words) != PA_OK) return 16;
+        if (pa_step_host(h, R_host, words, 0.5, 0.55, theta, words, E, NULL, &o, &R_new) != PA_OK) return 17;
+        if (o.R != R_new || pa_population(h) != R_new || o.beta != 0.55) return 18;
+        printf("host step to beta=%.2f: e=%.8f R=%lld E0=%d\n", o.beta, o.e, (long long)o.R, (int)E[0]);
+        free(words);
+    }
     free(E);
     pa_destroy(h);
     return 0;

@@ -76,9 +76,10 @@ def test_c_client_runs_the_paper_loop(c_client):
     r = subprocess.run([c_client, "32", "3000"], capture_output=True, text=True)
     assert r.returncode == 0, r.stdout + r.stderr
     lines = r.stdout.strip().splitlines()
-    assert len(lines) >= 3 and lines[-1].startswith("reweighted to beta=0.25")
-    last = lines[-2].split()
-    betas = [float(l.split()[0]) for l in lines[:-1]]
+    assert len(lines) >= 4 and lines[-2].startswith("reweighted to beta=0.25")
+    assert lines[-1].startswith("host step to beta=0.55") and -2.0 < float(lines[-1].split("e=")[1].split()[0]) < -1.0   # pa_step_host, pageable buffers
+    last = lines[-3].split()
+    betas = [float(l.split()[0]) for l in lines[:-2]]
     assert all(b > a for a, b in zip(betas, betas[1:])) and 0.0 < betas[-1] <= 0.5    # the adaptive schedule moves forward
     assert -2.0 < float(last[1]) < 0.0 and abs(float(last[1]) + 2.0 * betas[-1]) < 0.1   # e ~ -2 beta at high temperature
 
