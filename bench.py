@@ -288,6 +288,16 @@ def theta_scan(args):
     from paper_1703_03676_b200.workloads import table3_workload
     torch.cuda.set_device(0)
     rows = []
+    # one-time costs of the process (lazy kernel loading, pinned staging of the first pa_anneal) stay outside the clocks
+    wl = table3_workload(1)
+    warm = pa.Population(wl.L, wl.R, wl.seed)
+    if args.rng == "lcg":
+        warm.set_rng_mode(pa.PA_RNG_LCG)
+    wb = wl.betas()
+    warm.observables(wb[0])
+    one_step(warm, wl, wb[0], wb[1])
+    warm.anneal(wb[1:4], 1)
+    warm.close()
     for theta in (1, 5, 10, 50, 100, 500):
         wl = table3_workload(theta)
         pop = pa.Population(wl.L, wl.R, wl.seed)
