@@ -209,6 +209,8 @@ static int pa_create_impl(int D, PaGeom geom, int64_t R, uint64_t seed, void* de
     h->R_target = R; h->R_cur = R; h->R_cap = y.R_cap; h->G_cap = y.G_cap;
     h->seed = seed; h->keys = pa_make_keys(seed); h->rng_mode = PA_RNG_PHILOX; h->timing = PA_TIME_SWEEP;
     { const char* e = getenv("PA_PDL"); h->pdl = (e && atoi(e) == 0) ? 0 : 1; }
+    { int dev = 0, nsm = 0;                                           // launch plans count rounds of the SMs (148 on B200)
+      h->n_sm = (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0) ? nsm : 148; }
     h->lnZ = (double)h->N * log(2.0);           // Z_{beta_0} = 2^N (L93)
     h->n_tiles_cap = y.tiles;
     int rc = PA_OK;
@@ -843,7 +845,7 @@ int pa_step_host(pa_t* h, int64_t R_in, const uint32_t* words_in, double beta, d
     if (R_new_out) *R_new_out = R_new;
     const int64_t G = (R_new + 31) / 32;
     // chunks of whole rounds: multiples of 148 groups, about 16 per step; small populations go in one piece
-    int64_t chunk = G / 16 / 148 * 148;
+    int64_t chunk = G / 16 / h->n_sm * h->n_sm;
     const char* ec = getenv("PA_STEP_HOST_CHUNK");                  // tests: force a chunk size (groups), 0 = one piece
     if (ec) chunk = atoll(ec);
     bool piped = chunk >= 1 && chunk < G && theta > 0;

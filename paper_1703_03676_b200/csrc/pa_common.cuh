@@ -187,6 +187,7 @@ struct pa_handle {
     cudaStream_t xfer_stream; cudaEvent_t ev_xfer;   // pa_step_host: device-to-host copies of finished chunks run beside the sweeps
     double* h_tabs; size_t h_tabs_bytes; // pinned staging for pa_anneal's weight tables and snapshots
     int pdl;                            // 1: the step's kernels are launched with programmatic stream serialization
+    int n_sm;                           // streaming multiprocessors of the device (148 on B200): launch plans count rounds of them
     int64_t launches;
     bool sweep_C_forced;
     uint32_t T12;            // third threshold of the cubic lattice (dE = 12), set by pa_sweep

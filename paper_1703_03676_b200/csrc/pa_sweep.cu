@@ -1142,7 +1142,7 @@ static int pa_sweep_pick_C(const pa_handle* h, int64_t G, long long* n_main) {
     const int Cmin = h->sweep_C;
     if (h->sweep_C_forced || h->sweep_kind != 1) return Cmin;
     const int L = h->L;
-    const double S = 148.0;
+    const double S = (double)h->n_sm;
     if ((double)G * Cmin / S >= 24.0) return Cmin;                 // quantisation below 4 %
     double best = -1.0; int bestC = Cmin;
     for (int C = Cmin; C <= 8; C *= 2) {
@@ -1156,8 +1156,8 @@ static int pa_sweep_pick_C(const pa_handle* h, int64_t G, long long* n_main) {
     if (h->rng_mode == PA_RNG_LCG && pa_env_int("PA_LCG_P64", 0) == 1) return bestC;
     // inside pa_anneal the grid covers the capacity; the live population is about the target
     const int64_t G_live = h->dev_R ? (h->R_target + 31) / 32 : G;
-    const int64_t rounds = G_live / 148;
-    const int64_t Gm = rounds * 148, Gt = G_live - Gm;
+    const int64_t rounds = G_live / h->n_sm;
+    const int64_t Gm = rounds * h->n_sm, Gt = G_live - Gm;
     if (rounds < 1 || Gt <= 0) return bestC;
     // a lane quarter costs about 0.3 of a whole group (35 instead of 131/4 wide multiplies, repeated neighbour logic)
     const double time = (double)rounds + ceil((double)Gt * 4 / S) * 0.30;
@@ -1323,7 +1323,8 @@ static int pa_sweep_pick_split(const pa_handle* h, int64_t G) {
     if ((size_t)h->N * 4 > (size_t)64 * 1024) return 0;
     const int force = pa_env_int("PA_SWEEP_SPLIT", -1);
     if (force == 0 || force == 2 || force == 4) return force;
-    return G * 4 <= 160 ? 4 : G * 2 <= 160 ? 2 : 0;
+    const int64_t room = h->n_sm + h->n_sm / 12;                 // 160 CTAs on 148 SMs
+    return G * 4 <= room ? 4 : G * 2 <= room ? 2 : 0;
 }
 
 static int pa_launch_sweep_split(pa_handle* h, SweepParams& P, int S, int64_t G, bool gather) {
