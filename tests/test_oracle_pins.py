@@ -158,6 +158,22 @@ def test_init_closed_forms():
     assert len({r.tobytes() for r in sp[:2000]}) == 2000
 
 
+def test_init_stream_counter_layout():
+    """O1 with the INIT counter layout written out: the word of (site s, group g) is philox(s, g >> 2, 0, TAG_INIT = 0)[g & 3] with key
+    (seed & 2^32-1, seed >> 32); replica j is bit j & 31 of group j >> 5, a set bit is an up spin.  The statistics of
+    test_init_closed_forms cannot see a wrong tag, a transposed counter or a reversed lane order; this recomputation can (the Philox
+    routine itself is pinned against cuRAND's header above).  Square lattice and a box (site s = (z Ly + y) Lx + x, O16)."""
+    seed = (11 << 32) | 12345                                          # both key words in use
+    key = [seed & 0xffffffff, seed >> 32]
+    for make, N, R in ((lambda: po.Oracle(6, 100, seed), 36, 100), (lambda: po.Oracle.box((4, 6, 2), 70, seed), 48, 70)):
+        sp = make().get_spins()
+        assert sp.shape == (R, N)
+        for j in (0, 1, 31, 32, 33, 63, 64, R - 1):
+            g, b = j >> 5, j & 31
+            want = [1 if (int(po.philox4x32_10([s, g >> 2, 0, 0], key)[g & 3]) >> b) & 1 else -1 for s in range(N)]
+            assert sp[j].tolist() == want, j
+
+
 # ---------------------------------------------------------------------------------------------
 # O3 sweep  <-  L = 4 brute force Boltzmann distribution, symmetries, no-op
 # ---------------------------------------------------------------------------------------------
