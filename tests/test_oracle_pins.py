@@ -452,6 +452,15 @@ def test_adapt_dbeta_brackets_the_target():
     # a target the whole interval satisfies returns the interval
     o2 = po.Oracle(L, R, 8)
     assert o2.adapt_dbeta(0.5, 0.0, 1e-6) == 1e-6
+    # EXACTLY 40 halvings of [0, hi], the lower end returned (O10): with hi = 1 every midpoint is a dyadic fraction, so the result is
+    # an integer multiple of 2^-40 and the bracket's upper end, one unit above, fails the target.  39 steps would leave the upper end
+    # passing on about half of the populations, 41 steps a non-integer multiple on about half: six populations
+    for seed in range(9, 15):
+        o3 = po.Oracle(L, R, seed)
+        d3 = o3.adapt_dbeta(target, 0.0, 1.0)
+        k = d3 * 2.0**40
+        assert 0 < d3 < 1 and k == math.floor(k), seed
+        assert o3.overlap(d3) >= target > o3.overlap(d3 + 2.0**-40), seed
 
 
 # ---------------------------------------------------------------------------------------------
