@@ -29,6 +29,7 @@ struct SweepParams {
     const PaScalars* sc;
     long long Gcap;                  // groups the population buffer holds (p = 64 experiment: the second group of a pair may not exist)
     const uint8_t* jmask;            // O15: per resident word, bit k = bond to neighbour k (same, x, up, down) has J = -1; NULL = ferromagnet
+    int whole;                       // host side: the launch covers the whole population (not a range of pa_step_host)
     long long g0;                    // column-walk kernels: first group of this launch (pa_launch_sweep_range: a step in chunks of groups); else 0
     const uint32_t* src;             // lane-split kernel with GATHER: the population before resampling and its parent map (new[d] = old[parent[d]])
     const uint32_t* parent;
@@ -722,7 +723,7 @@ pa_sweep_lcg_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 // groups side by side (uint2 in shared memory, 64-bit LDS / STS); the random stream is unchanged (O11: one seed per 32-replica
 // word), so the result is bit-identical to the p = 32 kernel.  What a wider word can share on a 32-bit integer datapath is the
 // addressing, the loop and half of the shared-memory instructions; every LCG step, compare, insert and logic op doubles.
-// Selected with PA_LCG_P64=1 (power-of-two L, ferromagnet).
+// Taken automatically at L = 64 for large populations (pa_sweep_dispatch_lcg); PA_LCG_P64=1 / 0 force it on (power-of-two L, ferromagnet) / off.
 // ------------------------------------------------------------------------------------------------
 template <int LOG_LH, bool CLUSTER, int NOR>
 __global__ void __launch_bounds__(LOG_LH == 7 ? 512 : 256)
@@ -1201,7 +1202,11 @@ static cudaError_t pa_sweep_dispatch_lcg_col(pa_handle* h, const SweepParams& P,
 
 static cudaError_t pa_sweep_dispatch_lcg(pa_handle* h, const SweepParams& P, size_t smem, unsigned grid) {
     const bool cl = P.C > 1;
-    if (h->sweep_kind == 1 && !h->has_j && pa_env_int("PA_LCG_P64", 0) == 1 && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG) &&
+    // p = 64 words: PA_LCG_P64=1 wherever the kernel applies, =0 never; unset: at L = 64 (+2.7 % there, -12 % at L = 128:
+    // profiles/r02b_p64.md) for a uniform launch of the whole population (the mixed launch and pa_step_host's ranges stay on p = 32)
+    const int p64 = pa_env_int("PA_LCG_P64", -1);
+    const bool p64_on = p64 == 1 || (p64 < 0 && P.L == 64 && P.C == 1 && P.n_main < 0 && P.whole != 0 && grid >= 24u * (unsigned)h->n_sm);
+    if (h->sweep_kind == 1 && !h->has_j && p64_on && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG) &&
         P.Lh >= 32 && P.Lh <= 128 && 2 * smem <= (size_t)224 * 1024) {
         // p = 64 experiment: one CTA (cluster) per PAIR of groups, twice the shared memory
         const unsigned grid2 = (unsigned)(((grid / P.C) + 1) / 2 * P.C);
@@ -1271,7 +1276,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     P.L = h->geom.Lx; P.Lh = h->geom.Lx / 2; P.Ly = h->geom.Ly; P.Lz = h->geom.Lz; P.N = h->N;
     P.C = h->sweep_C; P.H = h->geom.Ly * (h->geom.Lz / P.C);
-    P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0; P.src = nullptr; P.parent = nullptr;
+    P.jmask = nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0; P.whole = 1; P.src = nullptr; P.parent = nullptr;
     const size_t smem = (size_t)h->N * 4 / P.C;
     const unsigned grid = (unsigned)(G * P.C);
     cudaError_t e = cudaErrorInvalidValue;
@@ -1360,7 +1365,7 @@ int pa_launch_sweep_gather(pa_handle* h, uint32_t T4, uint32_t T8, int theta) {
     P.T4 = T4; P.T8 = T8; P.T12 = 0u; P.Ly = h->L; P.Lz = 1;
     P.t0 = h->t; P.theta = theta; P.two = 2u;
     P.R = -1; P.sc = h->d_scal;
-    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = h->has_j ? h->jmask : nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0;
+    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = h->has_j ? h->jmask : nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0; P.whole = 1;
     P.src = h->spins[1 - h->cur]; P.parent = h->parent;
     return pa_launch_sweep_split(h, P, pa_sweep_pick_split(h, (h->R_target + 31) / 32), h->G_cap, true);
 }
@@ -1388,11 +1393,11 @@ static int pa_launch_sweep_groups(pa_handle* h, uint32_t T4, uint32_t T8, int th
     const int64_t G = h->dev_R ? h->G_cap : (h->R_cur + 31) / 32;
     P.R = h->dev_R ? -1 : h->R_cur; P.sc = h->d_scal;
     if (const int S = pa_sweep_pick_split(h, h->dev_R ? (h->R_target + 31) / 32 : G)) {   // pa_anneal: the grid covers the capacity, the population is about the target
-        P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = h->has_j ? h->jmask : nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0;
+        P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.jmask = h->has_j ? h->jmask : nullptr; P.Gcap = h->G_cap; P.n_main = -1; P.g0 = 0; P.whole = 1;
         P.src = nullptr; P.parent = nullptr;
         return pa_launch_sweep_split(h, P, S, G, false);
     }
-    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.g0 = 0;
+    P.L = h->L; P.Lh = h->L / 2; P.N = h->N; P.g0 = 0; P.whole = ng < 0 ? 1 : 0;
     if (ng >= 0) { P.C = h->sweep_C; P.n_main = -1; P.g0 = g0; }       // a range of groups: the configured cluster size, no mixed launch
     else P.C = pa_sweep_pick_C(h, G, &P.n_main);
     P.H = h->L / P.C;
