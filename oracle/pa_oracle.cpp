@@ -33,7 +33,9 @@
 //                          (Boltzmann chi^2, whole PA runs, reweighting)
 //   weighted averages (O13) closed forms (weight ratios, M = 1, equal F, shift invariance, dominance);
 //                          unbiasedness of exp(lnZ_m) and removal of the small-R bias at L=4 (L99)
-//   LCG-assisted stream (O11) recurrence against big-integer arithmetic with the constants the
+//   LCG-assisted stream (O11) seed counter, output word, jump length and lane order recomputed from explicit Philox counters
+//                          for one whole sweep at L = 8 and 12, plus pairwise-distinct seed draws over an L = 16 lattice
+//                          (tests/test_oracle_lcg_pins.py); recurrence against big-integer arithmetic with the constants the
 //                          paper prints (L236); the same L=4 Boltzmann chi^2, global-flip symmetry
 //                          and Kaufman pins as the Philox-per-spin sweep; variance ratio of C
 //                          against the Philox-per-spin mode (Table 1, last column = 1)

@@ -143,3 +143,78 @@ def test_lcg_pa_run_matches_kaufman_and_variance_ratio_L16(cfg1_oracle_runs):
         ratios.append(v1 / v0)
     gm = math.exp(np.mean(np.log(ratios)))                             # geometric mean over 16 temperatures
     assert 0.4 < gm < 2.5, (gm, ratios)                                # n_RNG = 1 without the LCG would give ~32 (Table 1)
+
+
+def _lcg_seed_counter(L, x, y, g, t, c):
+    """The (Philox counter, output word) that seeds the word of group g at site (x, y) at its visit (sweep t, colour c): O11 as
+    include/pa.h publishes it, written out here independently of the oracle."""
+    return ((y >> 2) * (L // 2) + (x >> 1), g, 2 * t + c, 3), y & 3
+
+
+@pytest.mark.parametrize("L", [8, 12])
+def test_lcg_stream_seed_and_lane_layout_from_explicit_counters(L):
+    """O11 (Sec. 4) with the layout written out: the word of group g = j >> 5 at site (x, y) is seeded at
+    every visit (sweep t, colour c = (x + y) & 1) by r_0 = philox((y >> 2)(L/2) + (x >> 1), g, 2t + c, TAG_LCG = 3)[y & 3] with key
+    (seed & 2^32-1, seed >> 32), and replica j takes x_j = r_{32 - (j & 31)} of r_{n+1} = 1664525 r_n + 1013904223 mod 2^32
+    (most significant lane first).  One whole sweep of replicas in several words is recomputed site by site from explicit Philox
+    counters (the Philox routine itself is pinned against cuRAND's header in test_oracle_pins.py) and Python-integer LCG steps:
+    colour-0 decisions from the initial state, colour-1 decisions from the updated colour-0 neighbours.  L = 8 and 12 so that the
+    quad row y >> 2 takes two and three values (the chi-square pin at L = 4 cannot see a quad index that collides between rows);
+    a wrong output word, tag, jump length, lane order or counter slot fails here.  All branches of the acceptance rule occur."""
+    beta, t = 0.33, 4321
+    N = L * L
+    seed = (5 << 32) | 777                                             # both key words in use
+    key = [seed & 0xffffffff, seed >> 32]
+    T4 = min(math.floor(math.exp(-4 * beta) * 2.0**32), 2**32 - 1)
+    T8 = min(math.floor(math.exp(-8 * beta) * 2.0**32), 2**32 - 1)
+    slots = np.array([0, 1, 2, 30, 31, 32, 33, 63, 64, 1000003, 2**31 - 5], dtype=np.int64)
+    rng = np.random.default_rng(4)
+    init = rng.integers(0, 2, (slots.size, N), dtype=np.uint8)
+    got = po.sweep_slots(L, seed, t, beta, 1, slots, init.copy(), rng_mode=LCG)
+    seen = set()
+    for i, j in enumerate(int(v) for v in slots):
+        sp = init[i].reshape(L, L).copy()
+        for c in (0, 1):
+            for y in range(L):
+                for x in range(L):
+                    if (x + y) & 1 != c:
+                        continue
+                    ctr, word = _lcg_seed_counter(L, x, y, j >> 5, t, c)
+                    r = int(po.philox4x32_10(list(ctr), key)[word])
+                    for _ in range(32 - (j & 31)):
+                        r = (1664525 * r + 1013904223) % 2**32
+                    nb = [sp[y, (x - 1) % L], sp[y, (x + 1) % L], sp[(y - 1) % L, x], sp[(y + 1) % L, x]]
+                    u = sum(int(v != sp[y, x]) for v in nb)
+                    flip = u >= 2 or (u == 1 and r < T4) or (u == 0 and r < T8)
+                    seen.add((u, bool(flip)))
+                    if flip:
+                        sp[y, x] ^= 1
+        assert np.array_equal(got[i].reshape(L, L), sp), j
+    assert {(0, True), (0, False), (1, True), (1, False), (2, True)} <= seen
+    # the sweep counter advances by one per sweep, as in the Philox stream
+    two = po.sweep_slots(L, seed, t, beta, 2, slots, init.copy(), rng_mode=LCG)
+    assert np.array_equal(two, po.sweep_slots(L, seed, t + 1, beta, 1, slots, got.copy(), rng_mode=LCG))
+
+
+def test_lcg_seeds_of_distinct_words_and_visits_are_distinct_draws():
+    """O11: no two (word, visit) pairs share a seed draw.  Over every site of an L = 16 lattice x 3 groups x 2 sweeps (the colour
+    follows from the site) the (counter, output word) pairs are pairwise distinct -- in particular the quad index separates
+    the rows 0-3, 4-7, ... and the two columns of a pair x >> 1 are told apart by their colour in the third counter word --
+    and, Philox being a bijection of the counter, the r_0 actually drawn are distinct 32-bit words of distinct 128-bit blocks:
+    checked on the values too (a birthday collision among 1536 uniform 32-bit words has probability 3e-4)."""
+    L = 16
+    draws, values = set(), []
+    key = [2024, 9]
+    for t in (0, 1):
+        for g in (0, 1, 5):
+            for y in range(L):
+                for x in range(L):
+                    ctr, word = _lcg_seed_counter(L, x, y, g, t, (x + y) & 1)
+                    assert (ctr, word) not in draws, (x, y, g, t)
+                    draws.add((ctr, word))
+                    values.append(int(po.philox4x32_10(list(ctr), key)[word]))
+    assert len(draws) == 2 * 3 * L * L
+    assert len(set(values)) == len(values)
+    # every quad counter stays inside [0, (L/4)(L/2)) and every (quad, output word, colour) is used exactly once per (g, t)
+    quads = {c[0][0] for c in draws}
+    assert quads == set(range((L // 4) * (L // 2)))
