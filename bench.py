@@ -38,7 +38,22 @@ UNIT = "updates/ns"
 # FMA-heavy pipe issues 32 of them per clock per SM on 148 SMs.
 WIDE_MUL_PER_UPDATE = 131.0 / 32.0
 WIDE_MUL_PER_CLK_PER_SM = 32.0
-N_SM = 148
+N_SM_FALLBACK = 148            # B200; used only where no CUDA device can be asked (the reference arm never needs it)
+_n_sm = None
+
+
+def n_sm():
+    """SM count of the current device (the roofline peaks scale with it)."""
+    global _n_sm
+    if _n_sm is None:
+        try:
+            import torch
+            _n_sm = int(torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count)
+        except Exception:
+            _n_sm = N_SM_FALLBACK
+    return _n_sm
+
+
 LCG_INSTR_PER_UPDATE = 5.0
 ISSUE_LANES_PER_CLK_PER_SM = 128.0
 
@@ -195,10 +210,25 @@ def one_step(pop, wl, beta_prev, beta, fused=False):
     return obs
 
 
-def next_beta(pop, wl, betas, i, beta_prev):
+def first_run_decides(d, dist):
+    """PAPER.md L118 (Sec. 2.3): "our code used in adaptive mode decides about temperature steps only in the first run and keeps
+    the temperature sequence fixed for the remaining passes" -- the condition under which Eq. 6-7 may average the runs at every
+    temperature.  With one run per rank the first run is rank 0: it alone bisects (`d` = its step, None on the other ranks) and its
+    8-byte step is broadcast; it is part of the temperature step and sits inside the timed region."""
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([float(d) if dist.get_rank() == 0 else 0.0], dtype=torch.float64, device=dev)
+    dist.broadcast(t, src=0)
+    return float(t.item())
+
+
+def next_beta(pop, wl, betas, i, beta_prev, dist=None):
     if wl.n_steps is not None:
         return betas[min(i, len(betas) - 1)]
-    d = pop.adapt_dbeta(wl.target_overlap, beta_prev, wl.beta_f)
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        d = first_run_decides(pop.adapt_dbeta(wl.target_overlap, beta_prev, wl.beta_f) if dist.get_rank() == 0 else None, dist)
+    else:
+        d = pop.adapt_dbeta(wl.target_overlap, beta_prev, wl.beta_f)
     return min(wl.beta_f, beta_prev + d)
 
 
@@ -338,9 +368,19 @@ def sweep_traffic(wl_name, rng):
     profiles/traffic_<workload>_<rng>.csv (the raw page of an `ncu --set full` capture of this bench command, restricted to the
     two counters, base units; the command is in the .md beside it).  None if this workload has no capture."""
     import csv
+    import hashlib
+    import re
     path = os.path.join(ROOT, "profiles", f"traffic_{wl_name}_{rng}.csv")
     if not os.path.exists(path):
         return None, None
+    # the .md beside the export records the sha256 of the sweep kernels' source at capture time: a capture of other code is not
+    # this code's traffic
+    note = path[:-4] + ".md"
+    src = os.path.join(ROOT, "paper_1703_03676_b200", "csrc", "pa_sweep.cu")
+    want = re.search(r"sha256\(paper_1703_03676_b200/csrc/pa_sweep\.cu\)\s*=\s*([0-9a-f]{64})", open(note).read()) if os.path.exists(note) else None
+    have = hashlib.sha256(open(src, "rb").read()).hexdigest() if os.path.exists(src) else None
+    if want is None or have != want.group(1):
+        return None, "stale: " + os.path.relpath(path, ROOT) + " was captured on another pa_sweep.cu (sha256 differs or is not recorded)"
     rows = list(csv.reader(open(path)))
     hdr = rows[0]
     try:
@@ -356,15 +396,15 @@ def sweep_traffic(wl_name, rng):
 def sweep_roof(rng, sm_max):
     """(algorithmic units per update, peak in G units/s, unit, kernel name) of the sweep kernel's binding resource (DESIGN.md 6.1 / 6.4)."""
     if rng == "lcg":
-        return LCG_INSTR_PER_UPDATE, N_SM * ISSUE_LANES_PER_CLK_PER_SM * sm_max * 1e-3, "G thread-instructions/s", "pa_sweep_lcg_kernel"
-    return WIDE_MUL_PER_UPDATE, N_SM * WIDE_MUL_PER_CLK_PER_SM * sm_max * 1e-3, "G IMAD.WIDE.U32/s", "pa_sweep_col_kernel (pa_sweep3d_kernel on a box)"
+        return LCG_INSTR_PER_UPDATE, n_sm() * ISSUE_LANES_PER_CLK_PER_SM * sm_max * 1e-3, "G thread-instructions/s", "pa_sweep_lcg_kernel"
+    return WIDE_MUL_PER_UPDATE, n_sm() * WIDE_MUL_PER_CLK_PER_SM * sm_max * 1e-3, "G IMAD.WIDE.U32/s", "pa_sweep_col_kernel (pa_sweep3d_kernel on a box)"
 
 
 class Runner:
     """One population of a workload and the bookkeeping of its annealing schedule (which beta comes next)."""
 
-    def __init__(self, pa, wl, seed, rng, couplings="ferro", dims=2):
-        self.pa, self.wl, self.rng = pa, wl, rng
+    def __init__(self, pa, wl, seed, rng, couplings="ferro", dims=2, dist=None):
+        self.pa, self.wl, self.rng, self.dist = pa, wl, rng, dist
         self.pop = pa.Population(wl.L, wl.R, seed, dims=wl.dims)
         if rng == "lcg":
             self.pop.set_rng_mode(pa.PA_RNG_LCG)
@@ -383,7 +423,7 @@ class Runner:
     def step(self, fused=False):
         """One temperature step (for the adaptive workload the bisection is part of it).  Returns the observables."""
         self.i += 1
-        beta = next_beta(self.pop, self.wl, self.betas, self.i, self.beta)
+        beta = next_beta(self.pop, self.wl, self.betas, self.i, self.beta, self.dist)
         obs = one_step(self.pop, self.wl, self.beta, beta, fused)
         self.beta = beta
         return obs
@@ -461,7 +501,7 @@ def roofline_of(rng, wl_name, sweep_ms, sweep_updates, total_ms, peaks, peak_src
     per_clk = ISSUE_LANES_PER_CLK_PER_SM if rng == "lcg" else WIDE_MUL_PER_CLK_PER_SM
     return {"bound": "alu", "kernel": kname, "achieved": achieved, "peak": peak, "unit": unit, "frac": achieved / peak,
             "traffic": traffic, "traffic_source": tsrc, "algorithmic_bytes_per_launch": None,
-            "peak_source": f"148 SM x {per_clk:.0f}/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
+            "peak_source": f"{n_sm()} SM x {per_clk:.0f}/clk/SM x {sm_max:.0f} MHz ({peak_src} sm_max_mhz; DESIGN.md Sec. 6)",
             "kernel_ms": k_ms, "kernel_updates_per_ns": k_upd / (k_ms * 1e6), "share_of_step": sum(sweep_ms) / total_ms,
             "algorithmic_per_update": per_upd}
 
@@ -505,7 +545,7 @@ def run_ours(args):
     K, Wm = args.steps, args.warmup
     if wl.n_steps is not None:                                                 # never run past the end of a fixed schedule
         K = max(1, min(K, wl.n_steps - Wm - 8))
-    run = Runner(pa, wl, rank_seed(wl, rank), args.rng, args.couplings)
+    run = Runner(pa, wl, rank_seed(wl, rank), args.rng, args.couplings, dist=dist if world > 1 else None)
     pop = run.pop
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
     peaks, peak_src = measured_peaks()
@@ -537,7 +577,9 @@ def run_ours(args):
     # chunks travelling back beside them, energies, observables); the adaptive workload keeps the single calls (its bisection and
     # histogram fold sit between them)
     one_call = run.betas is not None and not wl.multi_histogram
+    step_s = []
     for s in range(Ke):
+        ts = time.perf_counter()
         nb = ((R_host + 31) // 32) * wl.N * 4
         h2d += nb
         if one_call:
@@ -553,11 +595,12 @@ def run_ours(args):
         R_host = pop.population
         d2h += ((R_host + 31) // 32) * wl.N * 4 + 8 * R_host + ctypes.sizeof(pa.pa_obs_t)
         upd_e += o["R"] * wl.N * wl.theta
+        step_s.append(time.perf_counter() - ts)                               # both step forms end synchronised with the host
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     dt, upd_e = reduce_over_ranks(dt, upd_e, "cuda", dist if world > 1 else None)
     e2e = {"value": upd_e / (dt * 1e9), "unit": UNIT, "h2d_bytes_per_step": h2d // Ke, "d2h_bytes_per_step": d2h // Ke,
-           "steps": Ke, "what": f"{Ke} steps (capped by --e2e-steps: the packed population is {h2d // Ke / 1e9:.2f} GB each way per step): "
+           "steps": Ke, "ms_of_each_step": [round(x * 1e3, 3) for x in step_s], "what": f"{Ke} steps (capped by --e2e-steps: the packed population is {h2d // Ke / 1e9:.2f} GB each way per step): "
                                 "population words pinned-host -> device, one temperature step, energies + words + observables back to host; host wall clock; "
                                 + ("one pa_step_host call per step (device-to-host copies of finished chunks overlap the sweeps)" if one_call
                                    else "pa_set_words + single calls + pa_energies + pa_get_words"),
@@ -581,8 +624,14 @@ def run_ours(args):
             gi, mhz = pa.pa_calibrate(kind)
             cal[name + "_G_per_s"] = gi
             cal["sm_mhz"] = mhz
-        cal["imad_wide_lanes_per_clk_per_sm"] = cal["imad_wide_u32_G_per_s"] * 1e3 / (cal["sm_mhz"] * N_SM)
+        cal["imad_wide_lanes_per_clk_per_sm"] = cal["imad_wide_u32_G_per_s"] * 1e3 / (cal["sm_mhz"] * n_sm())
         roofline["calibration"] = cal
+        if args.rng == "philox":
+            # next to the nominal peak (32 lanes/clk/SM, the strictest of the three roofs of DESIGN.md Sec. 6.1): the pipe rate the
+            # library's own dependent-chain microbenchmark reaches on this GPU in this run
+            roofline["peak_measured"] = cal["imad_wide_u32_G_per_s"]
+            roofline["frac_measured"] = roofline["achieved"] / cal["imad_wide_u32_G_per_s"]
+            roofline["peak_measured_source"] = "pa_calibrate(1): IMAD.WIDE.U32 chains on every SM, this run"
     except Exception as e:                                                    # never lose the bench line over the side measurement
         roofline["calibration"] = {"error": str(e)}
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
@@ -590,7 +639,10 @@ def run_ours(args):
            "dtype": "u32", "data": "synthetic",
            "config": {"workload": wl.name, "L": wl.L, "R_per_gpu": wl.R, "theta": wl.theta, "beta_from": wl.beta0, "rng": args.rng, "couplings": args.couplings,
                       "api": "pa_anneal, one temperature step per call" if fused else "pa_resample + pa_sweep + pa_observables per step",
-                      "schedule": "adaptive" if wl.n_steps is None else f"{wl.n_steps} equal steps to {wl.beta_f}",
+                      "schedule": ("adaptive (Eq. 8), timed: steps %d-%d from beta = %g" % (Wm + 1, Wm + K, wl.beta0)
+                                   + ("; rank 0 decides every step and broadcasts it (PAPER.md L118)" if world > 1 else "")) if wl.n_steps is None else
+                                  f"steps {Wm + 1}-{Wm + K} of {wl.n_steps} equal steps from {wl.beta0} to {wl.beta_f} are the timed ones "
+                                  f"(beta <= {wl.betas()[min(Wm + K, wl.n_steps)]:.4g}); the whole schedule: --whole-run",
                       "l2": "flushed between timed steps (256 MiB memset outside the CUDA events)",
                       "parallelism": "independent populations per GPU" if world > 1 else "1 GPU"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": t["launches"], "roofline": roofline, "resample": resample,

@@ -39,8 +39,20 @@ def _worker(rank, world, port, q):
     # Eq. 6-7: the ranks' runs combined by their free-energy estimates
     ob = o.observables(betas[1])
     comb = bench.combine_over_ranks(o.lnZ, ob, "cpu", dist, po.weighted_average)
+    # Adaptive mode: the first run -- rank 0 -- decides every temperature step, the others keep its sequence,
+    # so that Eq. 6-7 may combine the runs at every temperature.  8 bytes broadcast per step.
+    from paper_1703_03676_b200.workloads import Workload
+    wa = Workload("adaptive_small", 8, 96, 40, 0.0, 1.0, None, 2, target_overlap=0.8)
+    a = po.Oracle(wa.L, wa.R, bench.rank_seed(wa, rank))
+    own = a.adapt_dbeta(wa.target_overlap, 0.0, wa.beta_f)           # what this rank would have chosen on its own
+    sched, beta = [], 0.0
+    for i in range(1, 4):
+        new = bench.next_beta(a, wa, None, i, beta, dist)
+        a.resample(beta, new); a.sweep(new, wa.theta)
+        sched.append(new); beta = new
+    comb_a = bench.combine_over_ranks(a.lnZ, a.observables(beta), "cpu", dist, po.weighted_average)
     allu = [None] * world
-    dist.all_gather_object(allu, (seed, int(units), int(E.sum()), o.lnZ, ob["e"], comb))
+    dist.all_gather_object(allu, (seed, int(units), int(E.sum()), o.lnZ, ob["e"], comb, own, sched, comb_a))
     dist.barrier()
     if rank == 0:
         q.put((t, u, allu))
@@ -69,6 +81,13 @@ def test_two_ranks_independent_populations_and_reduction():
     w0 = 1.0 / (1.0 + math.exp(allu[1][3] - allu[0][3]))
     assert c0["omega"][0] == pytest.approx(w0, rel=1e-12) and sum(c0["omega"]) == pytest.approx(1.0, rel=1e-14)
     assert c0["e"] == pytest.approx(w0 * allu[0][4] + (1 - w0) * allu[1][4], rel=1e-12)
+
+
+    # adaptive protocol: both ranks walked rank 0's temperatures although their own bisections differ
+    assert allu[0][6] != allu[1][6]
+    assert allu[0][7] == allu[1][7] and allu[0][7][0] == allu[0][6] and len(allu[0][7]) == 3
+    assert all(b > a for a, b in zip(allu[0][7], allu[0][7][1:]))
+    assert allu[0][8] == allu[1][8] and allu[0][8]["runs"] == 2
 
 
 def test_single_rank_reduction_is_identity():
