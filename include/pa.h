@@ -38,7 +38,8 @@ enum {
     PA_ERR_CAPACITY = -2,    /* resampling would exceed the capacity R_cap (or produce an empty population) */
     PA_ERR_CUDA = -3,        /* a CUDA call failed (sticky: see pa_last_cuda_error) */
     PA_ERR_WORKSPACE = -4,   /* caller-provided workspace too small or not 256-byte aligned */
-    PA_ERR_NOMEM = -5
+    PA_ERR_NOMEM = -5,
+    PA_ERR_STATIC_LIMIT = -6 /* pa_weighted_average_static: more runs than its fixed scratch array holds */
 };
 
 /* One output line of the paper's program (L179-L181): beta, energy per site, specific heat,
@@ -195,6 +196,31 @@ int pa_get_mag_sums(pa_t* h, int64_t* A1, int64_t* A2);
  * sum_m omega_m A[m*nobs + k].  HOST pointers; lnZ: double[M], A: double[M*nobs], A_out: double[nobs],
  * omega_out: double[M] or NULL.  Runs on the current CUDA device (no handle needed); synchronous. */
 int pa_weighted_average(int M, const double* lnZ, const double* A, int nobs, double* A_out, double* omega_out);
+
+/* The same weighted average (Eq. 6-7; O13) for callers that must not allocate device memory.
+ * pa_weighted_average above stages its host arguments through a cudaMalloc / cudaFree pair.  Three kinds of caller cannot
+ * live with that: one that has already given all of the GPU's memory away (populations sized to fill the HBM, or a host
+ * framework whose pool owns the rest), where an allocation late in a run may fail; one that combines its runs at every
+ * temperature while other populations are sweeping on other streams, because cudaMalloc and cudaFree make the whole device
+ * wait; and one running where a blocking driver call is not allowed (a stream callback, a latency-bounded loop).
+ * This entry point calls no cudaMalloc, no cudaFree and nothing else that allocates.  The caller passes DEVICE pointers (of the
+ * current device) for everything: d_lnZ: double[M], d_A: double[M*nobs] (run-major, A[m*nobs + k]), d_A_out: double[nobs];
+ * d_A and d_A_out may be NULL if nobs = 0.  The weights omega_m, which the kernel has to write and read back, live in a
+ * fixed array inside the library: PA_WAVG_STATIC_MAX_RUNS doubles = 32 KiB of device memory that every GPU which loads the
+ * library keeps until the process ends.  M > PA_WAVG_STATIC_MAX_RUNS: PA_ERR_STATIC_LIMIT, nothing launched (use
+ * pa_weighted_average).  A pointer the CUDA runtime does not know as device (or managed) memory: PA_ERR_INVALID_ARG.
+ * The kernel is enqueued on `cuda_stream` (a cudaStream_t; NULL = the legacy default stream) and the call returns without
+ * waiting: d_A_out is valid once that stream has reached this point.  The result equals pa_weighted_average's.
+ * Sharing: all calls on one GPU use the same array and find in it whatever the previous call left.  No entry has to start at
+ * zero -- each call writes omega_0..omega_{M-1} before reading them -- so nothing is cleared; but two calls that can run on the
+ * GPU at the same time (two streams) race on the array and both results are undefined: order them on one stream or with an event.
+ * Set-up: the first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device current;
+ * this may load the library's device code) and remembers it; make that first call during start-up, before any stream capture
+ * is begun on that device.  Thread-safe as far as the set-up goes; the sharing rule above still applies.
+ * pa_weighted_average_static_max_runs() returns PA_WAVG_STATIC_MAX_RUNS for callers that load the library dynamically. */
+#define PA_WAVG_STATIC_MAX_RUNS 4096
+int pa_weighted_average_static(int M, const double* d_lnZ, const double* d_A, int nobs, double* d_A_out, void* cuda_stream);
+int pa_weighted_average_static_max_runs(void);
 
 /* State export / import (parity tests, checkpoints, the end-to-end benchmark).
  * Spins are +1 / -1, one int8 per spin, out[i][s] with site s = y*L + x.

@@ -944,6 +944,7 @@ const char* pa_strerror(int code) {
         case PA_ERR_CUDA: return "CUDA error";
         case PA_ERR_WORKSPACE: return "workspace too small or misaligned";
         case PA_ERR_NOMEM: return "out of memory";
+        case PA_ERR_STATIC_LIMIT: return "more runs than the fixed scratch array of pa_weighted_average_static holds (PA_WAVG_STATIC_MAX_RUNS)";
         default: return "unknown error";
     }
 }

@@ -21,6 +21,8 @@ LIB_PATH = os.path.join(HERE, "libpa_b200.so")
 HEADER = os.path.join(os.path.dirname(HERE), "include", "pa.h")
 
 PA_OK, PA_ERR_INVALID_ARG, PA_ERR_CAPACITY, PA_ERR_CUDA, PA_ERR_WORKSPACE, PA_ERR_NOMEM = 0, -1, -2, -3, -4, -5
+PA_ERR_STATIC_LIMIT = -6
+PA_WAVG_STATIC_MAX_RUNS = 4096
 PA_RNG_PHILOX, PA_RNG_LCG = 0, 1
 PA_TIME_SWEEP, PA_TIME_RESAMPLE, PA_TIME_MEASURE = 1, 2, 4
 
@@ -88,6 +90,8 @@ def lib():
         "pa_reweight": ([vp, i32, vp, vp, vp, vp, vp, vp], i32),
         "pa_get_mag_sums": ([vp, vp, vp], i32),
         "pa_weighted_average": ([i32, vp, vp, i32, vp, vp], i32),
+        "pa_weighted_average_static": ([i32, vp, vp, i32, vp, vp], i32),
+        "pa_weighted_average_static_max_runs": ([], i32),
         "pa_get_spins": ([vp, i64, i64, vp], i32),
         "pa_get_spins_at": ([vp, vp, i64, vp], i32),
         "pa_set_spins": ([vp, i64, i64, vp], i32),
@@ -185,6 +189,29 @@ def pa_weighted_average(lnZ, A):
     if rc != PA_OK:
         raise PaError(rc, "pa_weighted_average")
     return out, w
+
+
+def pa_weighted_average_static(d_lnZ, d_A, d_A_out, cuda_stream=None):
+    """Eq. 6-7 like pa_weighted_average, for callers that must not allocate device memory (all of it is already handed
+    out, or other streams must not be stalled by cudaMalloc / cudaFree, or a blocking driver call is not allowed where they
+    run): the library allocates nothing, the weights live in a fixed 32 KiB array inside it.  d_lnZ [M], d_A [M, nobs] and
+    d_A_out [nobs] are contiguous float64 CUDA tensors of the current device that the caller made beforehand; at most
+    PA_WAVG_STATIC_MAX_RUNS runs (PaError with PA_ERR_STATIC_LIMIT beyond).  The kernel is enqueued on `cuda_stream` (a raw
+    cudaStream_t value; None = torch's current stream) and the call does not wait: read d_A_out after synchronising that
+    stream.  Calls on one GPU share the array: never let two of them run at the same time on different streams.  The first
+    call on a device also looks the array up; make it at start-up, before any stream capture."""
+    import torch
+    for t in (d_lnZ, d_A, d_A_out):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise PaError(PA_ERR_INVALID_ARG, "pa_weighted_average_static", "contiguous float64 CUDA tensors expected")
+    M, nobs = d_lnZ.numel(), d_A_out.numel()
+    if d_A.numel() != M * nobs:
+        raise PaError(PA_ERR_INVALID_ARG, "pa_weighted_average_static", "A must hold M * nobs values")
+    st = torch.cuda.current_stream().cuda_stream if cuda_stream is None else cuda_stream
+    rc = lib().pa_weighted_average_static(M, _ptr(d_lnZ), _ptr(d_A) if nobs else None, nobs,
+                                          _ptr(d_A_out) if nobs else None, C.c_void_p(st))
+    if rc != PA_OK:
+        raise PaError(rc, "pa_weighted_average_static")
 
 
 class Population:
