@@ -65,6 +65,10 @@ int pa_workspace_bytes(int L, int64_t R, size_t* bytes);
  * L even, 4 <= L <= 512, and such that L/C rows of one 32-replica group (L*L*4/C bytes) fit the shared memory of a CTA for a
  * cluster size C in {1,2,4,8} dividing L: every even L <= 338, the multiples of 4 up to 476, the multiples of 8 up to 512
  * (other L: PA_ERR_INVALID_ARG, also from pa_workspace_bytes); 1 <= R <= 2^31.
+ * The handle belongs to the CUDA device that is current when it is created: its kernels, its stream and its memory live there.
+ * Every later call on the handle makes that device current for the duration of the call and restores the caller's device before it
+ * returns, so handles on several GPUs can be driven from one thread without cudaSetDevice between the calls; host / device
+ * buffers passed to a call must be reachable from the handle's device.
  * pa_create allocates with cudaMalloc on the current device and uses its own stream.
  * pa_create_ex borrows `dev_ws` (device memory, >= pa_workspace_bytes, 256-byte aligned; e.g.
  * a torch tensor's data_ptr()) and enqueues on `cuda_stream` (a cudaStream_t; NULL = the
@@ -86,7 +90,7 @@ void pa_destroy(pa_t* h);
  * ndim = 2 with dims = {L, L} is pa_create_ex.  dev_ws = NULL: cudaMalloc and a private stream, as pa_create. */
 int pa_workspace_bytes_box(int ndim, const int* dims, int64_t R, size_t* bytes);
 int pa_create_box(int ndim, const int* dims, int64_t R, uint64_t seed, void* dev_ws, size_t ws_bytes, void* cuda_stream, pa_t** out);
-int pa_dims(const pa_t* h, int* ndim, int* dims);      /* dims: int[3]; either may be NULL */
+int pa_dims(const pa_t* h, int* ndim, int* dims);      /* dims: int[3] (dims[2] = 1 on the square lattice); either may be NULL */
 int64_t pa_num_levels(const pa_t* h);                  /* number of energy levels = length of the histogram arrays */
 
 /* Step 3 (L61; L151-L157): theta checkerboard Metropolis sweeps of every replica at inverse
@@ -148,6 +152,12 @@ int pa_adapt_dbeta(pa_t* h, double target_overlap, double beta, double beta_max,
  * of them, typically 2-4 instead of 41; *filter_launches = launches of the histogram kernel.  The result is the one O10
  * defines either way.  Environment PA_ADAPT_EXACT=1 forces all 41 exact evaluations.  Either pointer may be NULL. */
 int pa_adapt_stats(const pa_t* h, int* exact_evaluations, int* filter_launches);
+/* A tripwire for that rounding bound (first-order, with a factor 4 on top).  *min_margin: over the decisions
+ * the kernel took itself in the last pa_adapt_dbeta, the smallest |alpha' - alpha*| in units of the decision threshold (> 1 by
+ * construction; +inf if it took none).  *max_error: over the whole life of the handle, the largest |alpha' - alpha| seen at an
+ * iteration that was handed to the exact evaluation, in units of the first-order bound (2 R_cur + 2 dmax + 32) 2^-53; the decision
+ * threshold is 4 of these units, so the results are safe while this stays below 4 (0 if no iteration was handed back yet). */
+int pa_adapt_margins(const pa_t* h, double* min_margin, double* max_error);
 /* alpha(dbeta) of Eq. 8 for one dbeta >= 0 (the function pa_adapt_dbeta bisects on). */
 int pa_overlap(pa_t* h, double dbeta, double* alpha);
 
@@ -242,13 +252,17 @@ int pa_set_words(pa_t* h, int64_t R, const uint32_t* words);
  * chunk travels to the host on a second stream while the following chunks are swept.
  * words_in: HOST uint32 [ceil(R_in/32)][N] (interchange layout, above); words_out: HOST uint32 [ceil(R_cap/32)][N], of which the
  * first ceil(R_new/32) groups are written (pinned memory for the overlap; pageable memory works, serially).  E_out / M_out: host or
- * device int32[R_new] or NULL; obs_out, R_new_out: host or NULL.  Synchronous.  Errors as the single calls; after
+ * device int32[R_new] or NULL; obs_out, R_new_out: host or NULL.  words_out may be the same buffer as words_in (the upload has
+ * completed before the first chunk is copied back).  Synchronous: on every return path, errors included, no copy into words_out is
+ * still in flight.  Errors as the single calls; after
  * PA_ERR_CAPACITY the handle holds the uploaded population unchanged and words_out is untouched. */
 int pa_step_host(pa_t* h, int64_t R_in, const uint32_t* words_in, double beta, double beta_new, int theta,
                  uint32_t* words_out, int32_t* E_out, int32_t* M_out, pa_obs_t* obs_out, int64_t* R_new_out);
 
-/* Vectors of the last successful resampling step (pa_resample, or the last step of pa_anneal), indexed by the parent slot
- * j < R_prev = pa_prev_population(h), the population size before that step (0 if none yet); any pointer may be NULL:
+/* Vectors of the last resampling step (pa_resample, or the last step of pa_anneal), indexed by the parent slot
+ * j < R_prev = pa_prev_population(h), the population size before that step; any pointer may be NULL.  A step that fails with
+ * PA_ERR_CAPACITY has already overwritten them: from then until the next successful step (and before the first one)
+ * pa_prev_population is 0 and this call returns PA_ERR_INVALID_ARG.
  * W (one double), w[R_prev] double, r[R_prev] uint32 copy numbers, o[R_prev] uint32 offsets. */
 int pa_get_resample_debug(pa_t* h, double* W, double* w, uint32_t* r, uint32_t* o);
 int64_t pa_prev_population(const pa_t* h);
@@ -261,6 +275,18 @@ uint32_t pa_resample_counter(const pa_t* h);/* k */
 double pa_lnZ(const pa_t* h);               /* = -beta F(beta), Eq. 4 */
 /* Overwrite the counters (restart from a checkpoint; sampled parity checks at the large configs). */
 int pa_set_counters(pa_t* h, uint32_t t, uint32_t k, double lnZ);
+
+/* Tests and tuning: the library's switches (PA_SWEEP_C, PA_SWEEP_T, PA_SWEEP_KIND, PA_LCG_P64, PA_ADAPT_EXACT,
+ * PA_STEP_HOST_CHUNK, ...; every value gives the same bytes) are environment variables that are read ONCE, when a handle is
+ * created; no later call reads the environment.  pa_set_switch changes one on a live handle: `name` = the variable's name,
+ * is_set = 0 returns it to "not set" (the default behaviour), otherwise it takes `value`.  The sweep launch geometry is re-planned.
+ * PA_ERR_INVALID_ARG for an unknown name or a value that leaves no valid geometry (the switch then keeps its old state). */
+int pa_set_switch(pa_t* h, const char* name, int is_set, int64_t value);
+/* Which sweep kernel the last pa_sweep launched (diagnostics; the results do not depend on it): bit 0 = column-walk kernel,
+ * bit 1 = lane-split CTAs present, bit 2 = the p = 64 (uint2) variant of the LCG-assisted kernel, bit 3 = mixed launch.  0 before
+ * the first sweep. */
+enum { PA_SWEEP_RAN_COL = 1, PA_SWEEP_RAN_SPLIT = 2, PA_SWEEP_RAN_P64 = 4, PA_SWEEP_RAN_MIXED = 8 };
+int pa_last_sweep_kind(const pa_t* h);
 
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 int64_t pa_launch_count(const pa_t* h);

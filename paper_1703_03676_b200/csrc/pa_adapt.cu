@@ -75,10 +75,10 @@ pa_adapt_kernel(const uint32_t* __restrict__ Hd, const PaScalars* __restrict__ s
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double sh[32];
     const int m_lo = (int)(0xffffffffu - sc->mmin_inv), dmax = (int)sc->mmax - m_lo;
-    double lo = in.lo, hi = in.hi;
+    double lo = in.lo, hi = in.hi, margin = in.margin, a_last = 0.0;
     int it = in.it;
     if (dmax + 1 > PA_ADAPT_BINS) {                                              // wider than the shared-memory table: all exact
-        if (threadIdx.x == 0) { st->lo = lo; st->hi = hi; st->it = it; st->status = it < 0 ? PA_ADAPT_AMBIG_FIRST : PA_ADAPT_AMBIG; }
+        if (threadIdx.x == 0) { st->lo = lo; st->hi = hi; st->it = it; st->status = it < 0 ? PA_ADAPT_AMBIG_FIRST : PA_ADAPT_AMBIG; st->margin = margin; st->a_last = target; }
         return;
     }
     double* ws = reinterpret_cast<double*>(smem_raw);
@@ -90,7 +90,8 @@ pa_adapt_kernel(const uint32_t* __restrict__ Hd, const PaScalars* __restrict__ s
         const double a = pa_alpha_hist(hs, ws, dmax, hi, R_target, R_cur, sh);
         if (a >= target + bound) status = PA_ADAPT_RETURN_HI;
         else if (a < target - bound) it = 0;
-        else status = PA_ADAPT_AMBIG_FIRST;
+        else { status = PA_ADAPT_AMBIG_FIRST; a_last = a; }
+        if (status != PA_ADAPT_AMBIG_FIRST) margin = fmin(margin, fabs(a - target) / bound);
     }
     if (status == PA_ADAPT_DONE) {
         for (; it < 40; ++it) {                                                  // O10: exactly 40 bisection steps
@@ -98,16 +99,17 @@ pa_adapt_kernel(const uint32_t* __restrict__ Hd, const PaScalars* __restrict__ s
             const double a = pa_alpha_hist(hs, ws, dmax, mid, R_target, R_cur, sh);
             if (a >= target + bound) lo = mid;
             else if (a < target - bound) hi = mid;
-            else { status = PA_ADAPT_AMBIG; break; }
+            else { status = PA_ADAPT_AMBIG; a_last = a; break; }
+            margin = fmin(margin, fabs(a - target) / bound);
         }
     }
-    if (threadIdx.x == 0) { st->lo = lo; st->hi = hi; st->it = it; st->status = status; }
+    if (threadIdx.x == 0) { st->lo = lo; st->hi = hi; st->it = it; st->status = status; st->margin = margin; st->a_last = a_last; }
 }
 
 int pa_launch_ehist(pa_handle* h) {
     PA_CUDA(h, cudaMemsetAsync(h->Hd, 0, ((size_t)h->nlev + 1) * 4, h->stream));
     long long blocks = (h->R_cur + 256 * 16 - 1) / (256 * 16);
-    if (blocks > 296) blocks = 296;
+    if (blocks > 2 * h->n_sm) blocks = 2 * h->n_sm;
     if (blocks < 1) blocks = 1;
     pa_ehist_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->E, h->R_cur, h->nlev, h->e0, h->d_scal, h->Hd);
     PA_CUDA(h, cudaGetLastError());

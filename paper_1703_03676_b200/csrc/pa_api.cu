@@ -190,7 +190,7 @@ int pa_create_box(int ndim, const int* dims, int64_t R, uint64_t seed, void* dev
 int pa_dims(const pa_t* h, int* ndim, int* dims) {
     if (!h) return PA_ERR_INVALID_ARG;
     if (ndim) *ndim = h->D;
-    if (dims) { dims[0] = h->geom.Lx; dims[1] = h->geom.Ly; if (h->D == 3) dims[2] = h->geom.Lz; }
+    if (dims) { dims[0] = h->geom.Lx; dims[1] = h->geom.Ly; dims[2] = h->D == 3 ? h->geom.Lz : 1; }
     return PA_OK;
 }
 int64_t pa_num_levels(const pa_t* h) { return h ? (int64_t)h->nlev + 1 : 0; }
@@ -208,9 +208,12 @@ static int pa_create_impl(int D, PaGeom geom, int64_t R, uint64_t seed, void* de
     h->L = L; h->N = (int)Nsites; h->D = D; h->geom = geom; h->nlev = (int)nlev_;
     h->R_target = R; h->R_cur = R; h->R_cap = y.R_cap; h->G_cap = y.G_cap;
     h->seed = seed; h->keys = pa_make_keys(seed); h->rng_mode = PA_RNG_PHILOX; h->timing = PA_TIME_SWEEP;
-    { const char* e = getenv("PA_PDL"); h->pdl = (e && atoi(e) == 0) ? 0 : 1; }
+    pa_switches_read(&h->sw);                                         // the environment is read here and nowhere else
+    h->pdl = pa_sw(h, PA_SW_PDL, 1) == 0 ? 0 : 1;
     { int dev = 0, nsm = 0;                                           // launch plans count rounds of the SMs (148 on B200)
-      h->n_sm = (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0) ? nsm : 148; }
+      if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); delete h; return PA_ERR_CUDA; }
+      h->device = dev;                                                // the handle lives on the device current at creation
+      h->n_sm = (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && nsm > 0) ? nsm : 148; }
     h->lnZ = (double)h->N * log(2.0);           // Z_{beta_0} = 2^N (L93)
     h->n_tiles_cap = y.tiles;
     int rc = PA_OK;
@@ -268,6 +271,7 @@ static int pa_create_impl(int D, PaGeom geom, int64_t R, uint64_t seed, void* de
 int pa_create(int L, int64_t R, uint64_t seed, pa_t** out) { return pa_create_ex(L, R, seed, nullptr, 0, nullptr, out); }
 
 void pa_destroy(pa_t* h) {
+    PaDeviceGuard dg__(h);
     if (!h) return;
     cudaStreamSynchronize(h->stream);
     for (int i = 0; i < 9; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
@@ -285,6 +289,7 @@ void pa_destroy(pa_t* h) {
 }
 
 int pa_sweep(pa_t* h, double beta, int theta) {
+    PaDeviceGuard dg__(h);
     if (!h || theta < 0 || !(beta == beta)) return PA_ERR_INVALID_ARG;
     if (theta == 0) return PA_OK;
     const uint32_t T4 = pa_threshold(exp(-4.0 * beta)), T8 = pa_threshold(exp(-8.0 * beta));
@@ -301,6 +306,7 @@ int pa_sweep(pa_t* h, double beta, int theta) {
 }
 
 int pa_set_rng_mode(pa_t* h, int mode) {
+    PaDeviceGuard dg__(h);
     if (!h || (mode != PA_RNG_PHILOX && mode != PA_RNG_LCG)) return PA_ERR_INVALID_ARG;
     if (h->D == 3 && mode != PA_RNG_PHILOX) return PA_ERR_INVALID_ARG;        // O11 is keyed by quads of rows of the square lattice
     h->rng_mode = mode;
@@ -310,6 +316,7 @@ int pa_get_rng_mode(const pa_t* h) { return h ? h->rng_mode : PA_ERR_INVALID_ARG
 
 // O15 (L313): bimodal couplings shared by all replicas.  Builds the per-word bond mask in the resident (colour-split) order.
 int pa_set_couplings(pa_t* h, const int8_t* Jx, const int8_t* Jy) {
+    PaDeviceGuard dg__(h);
     if (!h || ((Jx == nullptr) != (Jy == nullptr)) || h->hist_any || (h->D == 3 && Jx)) return PA_ERR_INVALID_ARG;   // O15 is a 2D workload
     h->em_valid = false; h->host_scal_valid = false;
     if (!Jx) { h->has_j = false; h->e0 = 0; return PA_OK; }
@@ -369,6 +376,7 @@ int pa_set_couplings(pa_t* h, const int8_t* Jx, const int8_t* Jy) {
 int pa_level_offset(const pa_t* h) { return h ? h->e0 : 0; }
 
 int pa_energies(pa_t* h, int32_t* E_out, int32_t* M_out) {
+    PaDeviceGuard dg__(h);
     if (!h || !E_out) return PA_ERR_INVALID_ARG;
     int rc = pa_ensure_energies(h);
     if (rc != PA_OK) return rc;
@@ -378,6 +386,7 @@ int pa_energies(pa_t* h, int32_t* E_out, int32_t* M_out) {
 }
 
 int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
+    PaDeviceGuard dg__(h);
     if (!h || !(beta_new >= beta)) return PA_ERR_INVALID_ARG;
     const double dbeta = beta_new - beta;
     int rc;
@@ -393,8 +402,7 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     // R_new and W travel to the host right after the plan kernel -- written by the kernel itself into mapped host memory
     // (PA_SNAP_HOST=0: by a copy operation) --; the copy kernel is queued behind and runs while the host wakes up, so the stream
     // never idles on this call's one synchronisation
-    const char* esh = getenv("PA_SNAP_HOST");
-    const bool mailed = h->h_snap_dev && !(esh && atoi(esh) == 0);
+    const bool mailed = h->h_snap_dev && pa_sw(h, PA_SW_SNAP_HOST, 1) != 0;
     h->mail_out = mailed ? h->h_snap_dev : nullptr;
     rc = pa_launch_weights_plan(h, Emin, h->w, false);
     h->mail_out = nullptr;
@@ -410,7 +418,8 @@ int pa_resample(pa_t* h, double beta, double beta_new, int64_t* R_new_out) {
     if (mailed) { h->h_scal->R_new = h->h_snap->R_new; h->h_scal->W = h->h_snap->W; }
     const int64_t R_new = (int64_t)h->h_scal->R_new;
     const double W = h->h_scal->W;
-    if (R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;      // population, k, lnZ, R_prev unchanged (O7): only the spare buffer was written
+    if (R_new > h->R_cap || R_new < 1) { h->R_prev = 0; return PA_ERR_CAPACITY; }   // population, k, lnZ unchanged (O7): only the spare buffer was
+                                                                                     // written -- and w, r, o: no resample vectors to export now
     h->R_prev = h->R_cur; h->W_last = W;
     const double lnQ = -dbeta * (double)Emin + log(W / (double)h->R_cur);   // Eq. 1 with the shift (O5)
     h->cur ^= 1;
@@ -428,8 +437,7 @@ static int pa_eval_overlap(pa_handle* h, double dbeta, int Emin, int Emax, doubl
     int rc;
     if ((rc = pa_upload_wtab(h, dbeta, (Emax - Emin) / 4)) != PA_OK) return rc;
     if ((rc = pa_launch_weights(h, Emin, nullptr)) != PA_OK) return rc;
-    const char* esh = getenv("PA_SNAP_HOST");
-    const bool mailed = h->h_snap_dev && !(esh && atoi(esh) == 0);      // the kernel writes the sum into mapped host memory itself
+    const bool mailed = h->h_snap_dev && pa_sw(h, PA_SW_SNAP_HOST, 1) != 0;   // the kernel writes the sum into mapped host memory itself
     h->mail_out = mailed ? h->h_snap_dev : nullptr;
     rc = pa_launch_overlap(h, Emin);
     h->mail_out = nullptr;
@@ -448,6 +456,7 @@ static int pa_overlap_prepare(pa_handle* h, int* Emin, int* Emax) {
 }
 
 int pa_overlap(pa_t* h, double dbeta, double* alpha) {
+    PaDeviceGuard dg__(h);
     if (!h || !alpha || !(dbeta >= 0.0)) return PA_ERR_INVALID_ARG;
     int Emin, Emax, rc;
     if ((rc = pa_overlap_prepare(h, &Emin, &Emax)) != PA_OK) return rc;
@@ -473,36 +482,39 @@ static int pa_adapt_exact(pa_handle* h, double target, double hi, int Emin, int 
 }
 
 int pa_adapt_dbeta(pa_t* h, double target, double beta, double beta_max, double* dbeta_out) {
+    PaDeviceGuard dg__(h);
     if (!h || !dbeta_out || !(target > 0.0 && target < 1.0) || !(beta_max > beta)) return PA_ERR_INVALID_ARG;
     int Emin, Emax, rc;
     if ((rc = pa_overlap_prepare(h, &Emin, &Emax)) != PA_OK) return rc;
     const double hi0 = beta_max - beta;
     const int dmax = (Emax - Emin) / 4;
-    h->adapt_exact_evals = 0; h->adapt_filter_launches = 0;
-    const char* ex = getenv("PA_ADAPT_EXACT");
-    if ((ex && atoi(ex) != 0) || dmax + 1 > PA_ADAPT_BINS) return pa_adapt_exact(h, target, hi0, Emin, Emax, dbeta_out);
+    h->adapt_exact_evals = 0; h->adapt_filter_launches = 0; h->adapt_min_margin = INFINITY;
+    if (pa_sw(h, PA_SW_ADAPT_EXACT, 0) != 0 || dmax + 1 > PA_ADAPT_BINS) return pa_adapt_exact(h, target, hi0, Emin, Emax, dbeta_out);
     // The same 41 decisions, most of them taken on the energy histogram inside one kernel (pa_adapt.cu): an iteration comes back
     // to the host only when the histogram sum is within `bound` of the target, and is then decided by the exact evaluation.
     // |alpha_hist - alpha_TREE1024| <= (2 R_cur + 2 dmax + 32) 2^-53 to first order; bound = 4 x that.
     const double bound = 4.0 * (2.0 * (double)h->R_cur + 2.0 * (double)dmax + 32.0) * 1.1102230246251565e-16;
     if ((rc = pa_launch_ehist(h)) != PA_OK) return rc;
     PaAdaptState* st = h->h_adapt;
-    st->lo = 0.0; st->hi = hi0; st->it = -1; st->status = PA_ADAPT_DONE;
+    st->lo = 0.0; st->hi = hi0; st->it = -1; st->status = PA_ADAPT_DONE; st->margin = INFINITY; st->a_last = 0.0;
     for (;;) {
         if ((rc = pa_run_adapt_filter(h, target, bound)) != PA_OK) return rc;
         h->adapt_filter_launches += 1;
+        h->adapt_min_margin = st->margin;
         if (st->status == PA_ADAPT_RETURN_HI) { *dbeta_out = hi0; return PA_OK; }
         if (st->status == PA_ADAPT_DONE) { *dbeta_out = st->lo; return PA_OK; }
         double a;
         if (st->status == PA_ADAPT_AMBIG_FIRST) {
             if ((rc = pa_eval_overlap(h, hi0, Emin, Emax, &a)) != PA_OK) return rc;
             h->adapt_exact_evals += 1;
+            h->adapt_max_err = fmax(h->adapt_max_err, fabs(st->a_last - a) / (0.25 * bound));
             if (a >= target) { *dbeta_out = hi0; return PA_OK; }
             st->it = 0;
         } else {                                                     // PA_ADAPT_AMBIG: iteration st->it of the bracket [lo, hi]
             const double mid = 0.5 * (st->lo + st->hi);
             if ((rc = pa_eval_overlap(h, mid, Emin, Emax, &a)) != PA_OK) return rc;
             h->adapt_exact_evals += 1;
+            h->adapt_max_err = fmax(h->adapt_max_err, fabs(st->a_last - a) / (0.25 * bound));   // the filter's alpha' against the exact alpha
             if (a >= target) st->lo = mid; else st->hi = mid;
             st->it += 1;
         }
@@ -514,6 +526,13 @@ int pa_adapt_stats(const pa_t* h, int* exact_evaluations, int* filter_launches) 
     if (!h) return PA_ERR_INVALID_ARG;
     if (exact_evaluations) *exact_evaluations = h->adapt_exact_evals;
     if (filter_launches) *filter_launches = h->adapt_filter_launches;
+    return PA_OK;
+}
+
+int pa_adapt_margins(const pa_t* h, double* min_margin, double* max_error) {
+    if (!h) return PA_ERR_INVALID_ARG;
+    if (min_margin) *min_margin = h->adapt_min_margin;
+    if (max_error) *max_error = h->adapt_max_err;
     return PA_OK;
 }
 
@@ -534,6 +553,7 @@ static void pa_fill_obs(const pa_handle* h, const PaScalars& s, double beta, int
 }
 
 int pa_observables(pa_t* h, double beta, pa_obs_t* out) {
+    PaDeviceGuard dg__(h);
     if (!h || !out) return PA_ERR_INVALID_ARG;
     int rc;
     if ((rc = pa_ensure_host_scalars(h)) != PA_OK) return rc;
@@ -560,7 +580,7 @@ static int pa_anneal_digest(pa_handle* h, PaAnnealCtx& cx, const char* h_snaps, 
         const PaScalars& S = *(const PaScalars*)(h_snaps + (size_t)i * snap);
         const double beta_old = betas[s0 + i], beta = betas[s0 + i + 1], dbeta = beta - beta_old;
         const int64_t R_new = (int64_t)S.R_new;
-        if (S.err != 0u || R_new > h->R_cap || R_new < 1) return PA_ERR_CAPACITY;
+        if (S.err != 0u || R_new > h->R_cap || R_new < 1) { h->R_prev = 0; return PA_ERR_CAPACITY; }   // the failing step overwrote w, r, o
         const double lnQ = -dbeta * (double)cx.Emin_prev + log(S.W / (double)cx.R_prev);   // Eq. 1 with the shift (O5)
         h->lnZ += lnQ; h->lnQ_last = lnQ;                                                  // Eq. 4 (L90)
         h->R_prev = cx.R_prev; h->W_last = S.W;
@@ -579,6 +599,7 @@ static int pa_anneal_digest(pa_handle* h, PaAnnealCtx& cx, const char* h_snaps, 
 }
 
 int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out) {
+    PaDeviceGuard dg__(h);
     if (!h || !betas || n < 1 || theta < 0 || pa_is_device_ptr(betas) || (obs_out && pa_is_device_ptr(obs_out))) return PA_ERR_INVALID_ARG;
     for (int i = 0; i <= n; ++i) if (!(betas[i] == betas[i]) || (i > 0 && !(betas[i] >= betas[i - 1]))) return PA_ERR_INVALID_ARG;
     int rc;
@@ -589,8 +610,8 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
     const size_t per_step = tab * 8 + snap;
     int chunk_cap = (int)(h->stage_bytes / 2 / per_step);
     if (chunk_cap > 16) chunk_cap = 16;
-    const char* ec = getenv("PA_ANNEAL_CHUNK");                    // tests: force other chunk sizes
-    if (ec && atoi(ec) >= 1 && atoi(ec) < chunk_cap) chunk_cap = atoi(ec);
+    { const long long ec = pa_sw(h, PA_SW_ANNEAL_CHUNK, 0);         // tests: force other chunk sizes
+      if (ec >= 1 && ec < chunk_cap) chunk_cap = (int)ec; }
     if (chunk_cap < 1) return PA_ERR_WORKSPACE;
     if (chunk_cap > n) chunk_cap = n;
     const size_t buf_bytes = ((size_t)chunk_cap * per_step + 255) / 256 * 256;
@@ -638,8 +659,7 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
         }
         if (cudaMemcpyAsync(d_t, h_t, (size_t)cs * tab * 8, cudaMemcpyHostToDevice, h->stream) != cudaSuccess) { rc = PA_ERR_CUDA; break; }
         h->dev_R = true;
-        const char* efc = getenv("PA_FUSE_COPY");
-        const bool fuse_copy = !(efc && atoi(efc) == 0);
+        const bool fuse_copy = pa_sw(h, PA_SW_FUSE_COPY, 1) != 0;
         for (int i = 0; i < cs && rc == PA_OK; ++i) {
             const double beta = betas[s0 + i + 1];
             h->wtab_cur = d_t + (size_t)i * tab;
@@ -692,6 +712,7 @@ int pa_anneal(pa_t* h, int n, const double* betas, int theta, pa_obs_t* obs_out)
 }
 
 int pa_hist_accumulate(pa_t* h, double beta) {
+    PaDeviceGuard dg__(h);
     if (!h) return PA_ERR_INVALID_ARG;
     int rc;
     if ((rc = pa_ensure_energies(h)) != PA_OK) return rc;
@@ -700,6 +721,7 @@ int pa_hist_accumulate(pa_t* h, double beta) {
 }
 
 int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD) {
+    PaDeviceGuard dg__(h);
     if (!h) return PA_ERR_INVALID_ARG;
     int rc = PA_OK;
     if (Hsum) rc = pa_copy_out(h, Hsum, h->Hsum, ((size_t)h->nlev + 1) * 8, nullptr);
@@ -708,6 +730,7 @@ int pa_get_histogram(pa_t* h, int64_t* Hsum, double* lnD) {
 }
 
 int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, double* C, double* absm, double* m2) {
+    PaDeviceGuard dg__(h);
     if (!h || !betas || n < 1 || n > (1 << 20)) return PA_ERR_INVALID_ARG;
     if ((size_t)n * 48 > h->stage_bytes) return PA_ERR_INVALID_ARG;
     // any histogram yet?  (Hsum is all zero until the first pa_hist_accumulate)
@@ -724,6 +747,7 @@ int pa_reweight(pa_t* h, int n, const double* betas, double* lnZ, double* e, dou
 }
 
 int pa_get_mag_sums(pa_t* h, int64_t* A1, int64_t* A2) {
+    PaDeviceGuard dg__(h);
     if (!h) return PA_ERR_INVALID_ARG;
     int rc = PA_OK;
     if (A1) rc = pa_copy_out(h, A1, h->A1, ((size_t)h->nlev + 1) * 8, nullptr);
@@ -772,17 +796,20 @@ static int pa_get_spins_impl(pa_handle* h, const int64_t* slots, int64_t j0, int
 }
 
 int pa_get_spins(pa_t* h, int64_t j0, int64_t nrep, int8_t* out) {
+    PaDeviceGuard dg__(h);
     if (!h || !out || j0 < 0 || nrep < 0 || j0 + nrep > h->R_cur) return PA_ERR_INVALID_ARG;
     return pa_get_spins_impl(h, nullptr, j0, nrep, out);
 }
 
 int pa_get_spins_at(pa_t* h, const int64_t* slots, int64_t n, int8_t* out) {
+    PaDeviceGuard dg__(h);
     if (!h || !out || !slots || n < 0) return PA_ERR_INVALID_ARG;
     for (int64_t i = 0; i < n; ++i) if (slots[i] < 0 || slots[i] >= h->R_cur) return PA_ERR_INVALID_ARG;
     return pa_get_spins_impl(h, slots, 0, n, out);
 }
 
 int pa_set_spins(pa_t* h, int64_t j0, int64_t nrep, const int8_t* in) {
+    PaDeviceGuard dg__(h);
     if (!h || !in || j0 < 0 || nrep < 0 || j0 + nrep > h->R_cur) return PA_ERR_INVALID_ARG;
     const bool dev_in = pa_is_device_ptr(in);
     const size_t N = (size_t)h->N;
@@ -803,6 +830,7 @@ int pa_set_spins(pa_t* h, int64_t j0, int64_t nrep, const int8_t* in) {
 }
 
 int pa_get_words(pa_t* h, uint32_t* words) {
+    PaDeviceGuard dg__(h);
     if (!h || !words) return PA_ERR_INVALID_ARG;
     const size_t bytes = (size_t)((h->R_cur + 31) / 32) * h->N * 4;
     if (pa_is_device_ptr(words)) return pa_launch_words_out(h, words);
@@ -815,6 +843,7 @@ int pa_get_words(pa_t* h, uint32_t* words) {
 }
 
 int pa_set_words(pa_t* h, int64_t R, const uint32_t* words) {
+    PaDeviceGuard dg__(h);
     if (!h || !words || R < 1 || R > h->R_cap) return PA_ERR_INVALID_ARG;
     const size_t bytes = (size_t)((R + 31) / 32) * h->N * 4;
     const uint32_t* src = words;
@@ -836,6 +865,7 @@ int pa_set_words(pa_t* h, int64_t R, const uint32_t* words) {
 // 0.39 s of sweeps, and only the upload (which the resampling plan needs complete) and the last chunk stay exposed.
 int pa_step_host(pa_t* h, int64_t R_in, const uint32_t* words_in, double beta, double beta_new, int theta,
                  uint32_t* words_out, int32_t* E_out, int32_t* M_out, pa_obs_t* obs_out, int64_t* R_new_out) {
+    PaDeviceGuard dg__(h);
     if (!h || !words_in || !words_out || theta < 0 || !(beta_new >= beta) || pa_is_device_ptr(words_in) || pa_is_device_ptr(words_out))
         return PA_ERR_INVALID_ARG;
     int rc;
@@ -846,39 +876,51 @@ int pa_step_host(pa_t* h, int64_t R_in, const uint32_t* words_in, double beta, d
     const int64_t G = (R_new + 31) / 32;
     // chunks of whole rounds: multiples of 148 groups, about 16 per step; small populations go in one piece
     int64_t chunk = G / 16 / h->n_sm * h->n_sm;
-    const char* ec = getenv("PA_STEP_HOST_CHUNK");                  // tests: force a chunk size (groups), 0 = one piece
-    if (ec) chunk = atoll(ec);
+    chunk = pa_sw(h, PA_SW_STEP_HOST_CHUNK, chunk);                  // tests: force a chunk size (groups), 0 = one piece
     bool piped = chunk >= 1 && chunk < G && theta > 0;
+    bool copies_in_flight = false;
+    rc = PA_OK;
     if (piped) {
-        if (!h->xfer_stream) PA_CUDA(h, cudaStreamCreateWithFlags(&h->xfer_stream, cudaStreamNonBlocking));
+        if (!h->xfer_stream) PA_CUDA(h, cudaStreamCreateWithFlags(&h->xfer_stream, cudaStreamNonBlocking));   // (nothing in flight yet)
         if (!h->ev_xfer) PA_CUDA(h, cudaEventCreateWithFlags(&h->ev_xfer, cudaEventDisableTiming));
         const uint32_t T4 = pa_threshold(exp(-4.0 * beta_new)), T8 = pa_threshold(exp(-8.0 * beta_new));
         uint32_t* stage = h->spins[1 - h->cur];                      // the population before resampling: no longer needed
         for (int64_t g0 = 0; g0 < G; g0 += chunk) {
             const int64_t ng = g0 + chunk <= G ? chunk : G - g0;
             rc = pa_launch_sweep_range(h, T4, T8, theta, g0, ng);
-            if (rc == PA_ERR_INVALID_ARG && g0 == 0) { piped = false; break; }     // this geometry has no range launch: one piece
-            if (rc != PA_OK) return rc;
-            if ((rc = pa_launch_words_out_range(h, stage, g0, ng)) != PA_OK) return rc;
-            PA_CUDA(h, cudaEventRecord(h->ev_xfer, h->stream));
-            PA_CUDA(h, cudaStreamWaitEvent(h->xfer_stream, h->ev_xfer, 0));
-            PA_CUDA(h, cudaMemcpyAsync(words_out + g0 * (size_t)h->N, stage + g0 * (size_t)h->N, (size_t)ng * h->N * 4,
-                                       cudaMemcpyDeviceToHost, h->xfer_stream));
+            if (rc == PA_ERR_INVALID_ARG && g0 == 0) { piped = false; rc = PA_OK; break; }     // this geometry has no range launch: one piece
+            if (rc != PA_OK) break;
+            if ((rc = pa_launch_words_out_range(h, stage, g0, ng)) != PA_OK) break;
+            cudaError_t ce = cudaEventRecord(h->ev_xfer, h->stream);
+            if (ce == cudaSuccess) ce = cudaStreamWaitEvent(h->xfer_stream, h->ev_xfer, 0);
+            if (ce == cudaSuccess) ce = cudaMemcpyAsync(words_out + g0 * (size_t)h->N, stage + g0 * (size_t)h->N, (size_t)ng * h->N * 4,
+                                                        cudaMemcpyDeviceToHost, h->xfer_stream);
+            if (ce != cudaSuccess) { pa_note_cuda_error(h, ce, "pa_step_host: copy of a finished chunk", __FILE__, __LINE__); rc = PA_ERR_CUDA; break; }
+            copies_in_flight = true;
         }
-        if (piped) { h->t += (uint32_t)theta; h->em_valid = false; h->host_scal_valid = false; h->sweep_timed = false; }
+        if (piped && rc == PA_OK) { h->t += (uint32_t)theta; h->em_valid = false; h->host_scal_valid = false; h->sweep_timed = false; }
     }
-    if (!piped && (rc = pa_sweep(h, beta_new, theta)) != PA_OK) return rc;
-    if (obs_out && (rc = pa_observables(h, beta_new, obs_out)) != PA_OK) return rc;
-    if (E_out && (rc = pa_energies(h, E_out, M_out)) != PA_OK) return rc;
-    if (!piped) return pa_get_words(h, words_out);
-    PA_CUDA(h, cudaStreamSynchronize(h->xfer_stream));
-    PA_CUDA(h, cudaStreamSynchronize(h->stream));
-    return PA_OK;
+    if (rc == PA_OK && !piped) rc = pa_sweep(h, beta_new, theta);
+    if (rc == PA_OK && obs_out) rc = pa_observables(h, beta_new, obs_out);
+    if (rc == PA_OK && E_out) rc = pa_energies(h, E_out, M_out);
+    if (rc == PA_OK && !piped) rc = pa_get_words(h, words_out);
+    if (copies_in_flight) {
+        // every exit, errors included: no copy into the caller's words_out is left running, and the staging buffer (the spare
+        // population) is free for the next call
+        const cudaError_t c1 = cudaStreamSynchronize(h->xfer_stream), c2 = cudaStreamSynchronize(h->stream);
+        if (rc == PA_OK && (c1 != cudaSuccess || c2 != cudaSuccess)) {
+            pa_note_cuda_error(h, c1 != cudaSuccess ? c1 : c2, "pa_step_host: drain", __FILE__, __LINE__);
+            rc = PA_ERR_CUDA;
+        }
+    }
+    return rc;
 }
 
 int pa_get_resample_debug(pa_t* h, double* W, double* w, uint32_t* r, uint32_t* o) {
+    PaDeviceGuard dg__(h);
     if (!h) return PA_ERR_INVALID_ARG;
     int rc = PA_OK;
+    if (h->R_prev == 0) return PA_ERR_INVALID_ARG;                   // no resampling step yet, or the last one failed
     const size_t n = (size_t)h->R_prev;
     if (W) *W = h->W_last;
     if (w) rc = pa_copy_out(h, w, h->w, n * 8, nullptr);
@@ -899,6 +941,7 @@ int pa_set_counters(pa_t* h, uint32_t t, uint32_t k, double lnZ) {
     return PA_OK;
 }
 int64_t pa_launch_count(const pa_t* h) { return h ? h->launches : 0; }
+int pa_last_sweep_kind(const pa_t* h) { return h ? h->last_sweep_kind : 0; }
 
 int pa_set_timing(pa_t* h, int mask) {
     if (!h || mask < 0 || mask > (PA_TIME_SWEEP | PA_TIME_RESAMPLE | PA_TIME_MEASURE)) return PA_ERR_INVALID_ARG;
@@ -907,6 +950,7 @@ int pa_set_timing(pa_t* h, int mask) {
 }
 
 int pa_last_sweep_ms(pa_t* h, float* kernel_ms) {
+    PaDeviceGuard dg__(h);
     if (!h || !h->sweep_timed) return PA_ERR_INVALID_ARG;
     PA_CUDA(h, cudaEventSynchronize(h->ev[1]));
     float ms = 0.f;
@@ -915,6 +959,7 @@ int pa_last_sweep_ms(pa_t* h, float* kernel_ms) {
     return PA_OK;
 }
 int pa_last_resample_ms(pa_t* h, float* total_ms, float* copy_kernel_ms) {
+    PaDeviceGuard dg__(h);
     if (!h || !h->resample_timed) return PA_ERR_INVALID_ARG;
     PA_CUDA(h, cudaEventSynchronize(h->ev[3]));
     float a = 0.f, b = 0.f;
@@ -926,6 +971,7 @@ int pa_last_resample_ms(pa_t* h, float* total_ms, float* copy_kernel_ms) {
 }
 
 int pa_last_measure_ms(pa_t* h, float* kernel_ms) {
+    PaDeviceGuard dg__(h);
     if (!h || !h->measure_timed) return PA_ERR_INVALID_ARG;
     PA_CUDA(h, cudaEventSynchronize(h->ev[8]));
     float ms = 0.f;
@@ -935,6 +981,24 @@ int pa_last_measure_ms(pa_t* h, float* kernel_ms) {
 }
 
 int pa_calibrate(int kind, double* ginstr_per_ns, double* sm_mhz) { return pa_run_calibrate(kind, ginstr_per_ns, sm_mhz); }
+
+static const char* const pa_switch_names[PA_SW_COUNT] = {
+    "PA_PDL", "PA_SNAP_HOST", "PA_ADAPT_EXACT", "PA_ANNEAL_CHUNK", "PA_FUSE_COPY", "PA_STEP_HOST_CHUNK", "PA_MEASURE_GENERIC",
+    "PA_SMALL_PLAN", "PA_SWEEP_C", "PA_SWEEP_T", "PA_SWEEP_SMEM_KB", "PA_SWEEP_KIND", "PA_SWEEP_CMP", "PA_SWEEP_MIXED",
+    "PA_LCG_P64", "PA_LCG_NOR", "PA_SWEEP_SPLIT"};
+
+int pa_set_switch(pa_t* h, const char* name, int is_set, int64_t value) {
+    const int k = name ? pa_switch_index(name) : -1;
+    if (!h || k < 0) return PA_ERR_INVALID_ARG;
+    PaDeviceGuard dg__(h);
+    const PaSwitches saved = h->sw;
+    const int pdl = h->pdl;
+    h->sw.set[k] = is_set != 0; h->sw.val[k] = value;
+    h->pdl = pa_sw(h, PA_SW_PDL, 1) == 0 ? 0 : 1;
+    const int rc = pa_sweep_configure(h);                 // the sweep geometry follows its switches
+    if (rc != PA_OK) { h->sw = saved; h->pdl = pdl; pa_sweep_configure(h); }
+    return rc;
+}
 
 const char* pa_strerror(int code) {
     switch (code) {
@@ -952,3 +1016,16 @@ const char* pa_last_cuda_error(const pa_t* h) { return h ? h->cuda_err : ""; }
 const char* pa_version(void) { return "pa-b200 0.1 (sm_100a)"; }
 
 }  // extern "C"
+
+void pa_switches_read(PaSwitches* sw) {
+    for (int k = 0; k < PA_SW_COUNT; ++k) {
+        const char* v = getenv(pa_switch_names[k]);
+        sw->set[k] = v != nullptr;
+        sw->val[k] = v ? atoll(v) : 0;
+    }
+}
+int pa_switch_index(const char* name) {
+    for (int k = 0; k < PA_SW_COUNT; ++k)
+        if (strcmp(name, pa_switch_names[k]) == 0) return k;
+    return -1;
+}

@@ -122,9 +122,24 @@ struct PaAdaptState {
     double lo, hi;   // bracket
     int it;          // next bisection iteration (0..40); -1: the test alpha(hi) >= alpha* comes first
     int status;      // PA_ADAPT_*: done / iteration `it` (or the first test) is too close to alpha* for the histogram sum
+    double margin;   // diagnostics: min over the decisions the kernel took itself of |alpha' - alpha*| / bound (> 1 by construction)
+    double a_last;   // diagnostics: alpha' of the iteration handed back (status AMBIG*), to be set against the exact alpha
 };
 
+// Environment switches (tests and tuning, every value gives the same bytes).  The environment is read ONCE, in
+// pa_create*, into the handle (pa_switches_read, the only getenv of the library); pa_set_switch changes one on a live handle.
+enum {
+    PA_SW_PDL, PA_SW_SNAP_HOST, PA_SW_ADAPT_EXACT, PA_SW_ANNEAL_CHUNK, PA_SW_FUSE_COPY, PA_SW_STEP_HOST_CHUNK, PA_SW_MEASURE_GENERIC,
+    PA_SW_SMALL_PLAN, PA_SW_SWEEP_C, PA_SW_SWEEP_T, PA_SW_SWEEP_SMEM_KB, PA_SW_SWEEP_KIND, PA_SW_SWEEP_CMP, PA_SW_SWEEP_MIXED,
+    PA_SW_LCG_P64, PA_SW_LCG_NOR, PA_SW_SWEEP_SPLIT, PA_SW_COUNT
+};
+struct PaSwitches { bool set[PA_SW_COUNT]; long long val[PA_SW_COUNT]; };
+void pa_switches_read(PaSwitches* sw);                 // pa_api.cu
+int pa_switch_index(const char* name);                 // "PA_SWEEP_C" -> PA_SW_SWEEP_C, -1 if unknown
+
 struct pa_handle {
+    int device;              // the CUDA device the handle was created on; every entry point makes it current for the call (PaDeviceGuard)
+    PaSwitches sw;
     int L, N;                // N = number of sites; L = Lx
     int D; PaGeom geom;      // dimension (2 / 3, O16) and edges; D = 2: geom = {L, L, 1}
     int nlev;                // energy levels m = 0..nlev, E_m = -2 nlev + 4m + e0: N (2D), 3N/2 (3D)
@@ -161,6 +176,8 @@ struct pa_handle {
     PaAdaptState *d_adapt, *h_adapt;    // bisection state, device / pinned host (mapped: the kernel writes it there)
     PaAdaptState* h_adapt_dev;          // device address of h_adapt
     int adapt_exact_evals, adapt_filter_launches;   // of the last pa_adapt_dbeta (diagnostics)
+    double adapt_min_margin;            // of the last pa_adapt_dbeta: smallest |alpha' - alpha*| / bound at a decision of the filter
+    double adapt_max_err;               // over the handle's life: largest |alpha' - alpha_exact| / first-order bound seen at a hand-back
     double* lnD;                        // [N+1]
     unsigned long long *A1, *A2;        // [N+1] sums of |M_j| and M_j^2 per energy level over all folded replicas (O14)
     int64_t* d_slots;                   // slot list for pa_get_spins_at
@@ -191,8 +208,24 @@ struct pa_handle {
     int64_t launches;
     bool sweep_C_forced;
     uint32_t T12;            // third threshold of the cubic lattice (dE = 12), set by pa_sweep
+    int last_sweep_kind;     // PA_SWEEP_RAN_* bits of the last sweep launch (pa_last_sweep_kind)
     int sweep_C, sweep_T, sweep_cmp, sweep_kind;   // sweep launch geometry (cluster size, threads), compare variant, kernel kind
     char cuda_err[256];
+};
+
+// value of a switch on this handle, `dflt` if it was not set
+static inline long long pa_sw(const pa_handle* h, int key, long long dflt) { return h->sw.set[key] ? h->sw.val[key] : dflt; }
+
+// Makes the handle's device current for the duration of a call and restores the caller's afterwards (handles on several GPUs in
+// one process: pa_weighted_average over runs "or over GPUs").  cudaGetDevice is a thread-local read.
+struct PaDeviceGuard {
+    int prev; bool switched;
+    explicit PaDeviceGuard(const pa_handle* h) : prev(-1), switched(false) {
+        if (h && cudaGetDevice(&prev) == cudaSuccess && prev != h->device) switched = cudaSetDevice(h->device) == cudaSuccess;
+    }
+    ~PaDeviceGuard() { if (switched) cudaSetDevice(prev); }
+    PaDeviceGuard(const PaDeviceGuard&) = delete;
+    PaDeviceGuard& operator=(const PaDeviceGuard&) = delete;
 };
 
 #define PA_CUDA(h, call)                                                                      \

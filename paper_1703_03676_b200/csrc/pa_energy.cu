@@ -10,7 +10,9 @@
 #include <stddef.h>
 #include <stdlib.h>
 
-#define PA_EPLANES 20   // counts up to 2N = 2^19 (L = 512)
+#define PA_EPLANES 20   // bit planes of the per-replica counters: counts up to 2N = 2^19 (L = 512) on the square lattice and up to
+                        // 3N = 3 * 2^18 on the largest cubic box (pa_create_box: at most 2^18 sites)
+static_assert(3 * (1 << 18) < (1 << PA_EPLANES), "the energy counters of the largest cubic box must fit PA_EPLANES bit planes");
 
 __device__ __forceinline__ void pa_csa(uint32_t& h, uint32_t& l, uint32_t a, uint32_t b, uint32_t c) {
     uint32_t u = a ^ b;
@@ -437,13 +439,12 @@ int pa_launch_measure(pa_handle* h) {
     const bool timed = (h->timing & PA_TIME_MEASURE) != 0;
     if (timed) PA_CUDA(h, cudaEventRecord(h->ev[7], h->stream));
     // single calls: the last CTA writes the finished scalars straight into mapped host memory (pa_read_measure_scalars)
-    const char* esh = getenv("PA_SNAP_HOST");                          // PA_SNAP_HOST=0: device-to-host copy instead
-    const bool to_host = !h->dev_R && !h->snap_out && h->h_snap_dev && !(esh && atoi(esh) == 0);
+    const bool to_host = !h->dev_R && !h->snap_out && h->h_snap_dev && pa_sw(h, PA_SW_SNAP_HOST, 1) != 0;   // PA_SNAP_HOST=0: device-to-host copy instead
     PaScalars* const snap_save = h->snap_out;
     if (to_host) h->snap_out = h->h_snap_dev;
     h->snap_on_host = to_host;
     cudaError_t le = cudaSuccess;
-    const bool pow2 = h->D == 2 && (L & (L - 1)) == 0 && L >= 8 && L <= 256 && getenv("PA_MEASURE_GENERIC") == nullptr;
+    const bool pow2 = h->D == 2 && (L & (L - 1)) == 0 && L >= 8 && L <= 256 && !h->sw.set[PA_SW_MEASURE_GENERIC];
     if (pow2) {
 #define PA_MSR_CASE(LOG) case (8 << LOG): \
         if (h->has_j) le = pa_launch(h, pa_measure_kernel<LOG, true>, dim3((unsigned)G), dim3(pa_msr_threads(8 << LOG)), 0, \
@@ -454,7 +455,7 @@ int pa_launch_measure(pa_handle* h) {
         switch (L) { PA_MSR_CASE(0) PA_MSR_CASE(1) PA_MSR_CASE(2) PA_MSR_CASE(3) PA_MSR_CASE(4) PA_MSR_CASE(5) default: break; }
 #undef PA_MSR_CASE
     } else if (h->D == 3 && !h->has_j && h->geom.Lx == h->geom.Ly && h->geom.Lx == h->geom.Lz && (L == 8 || L == 16 || L == 32) &&
-               getenv("PA_MEASURE_GENERIC") == nullptr) {
+               !h->sw.set[PA_SW_MEASURE_GENERIC]) {
         const int T3 = L * (L / 8) < 32 ? 32 : L * (L / 8);
 #define PA_M3_CASE(LOG) le = pa_launch(h, pa_measure3d_kernel<LOG>, dim3((unsigned)G), dim3(T3), 0, (const uint32_t*)h->spins[h->cur], h->N, Rarg, \
             h->E, h->M, h->d_scal, h->runsum, h->partials, h->snap_out, h->nlev)
@@ -465,7 +466,7 @@ int pa_launch_measure(pa_handle* h) {
         while (T > 32 && T * 8 > h->N) T >>= 1;
 #define PA_MG_CASE(LOGH, LOGY) le = pa_launch(h, pa_measure_generic_kernel<LOGH, LOGY>, dim3((unsigned)G), dim3(T), 0, (const uint32_t*)h->spins[h->cur], \
             h->geom, h->N, Rarg, h->E, h->M, h->d_scal, h->runsum, h->partials, h->has_j ? (const uint8_t*)h->jmask : (const uint8_t*)nullptr, h->snap_out, h->nlev)
-        const int cube = h->D == 3 && h->geom.Lx == h->geom.Ly && getenv("PA_MEASURE_GENERIC") == nullptr ? h->geom.Lx : 0;
+        const int cube = h->D == 3 && h->geom.Lx == h->geom.Ly && !h->sw.set[PA_SW_MEASURE_GENERIC] ? h->geom.Lx : 0;
         switch (cube) {
             case 8: PA_MG_CASE(2, 3); break;
             case 16: PA_MG_CASE(3, 4); break;

@@ -306,8 +306,7 @@ pa_tree_plan_small_kernel(const int32_t* __restrict__ E, const double* __restric
 // a population of at most PA_SMALL_TILES tiles takes the fused kernel (PA_SMALL_PLAN=0: never)
 bool pa_small_plan_ok(const pa_handle* h) {
     const int n = (int)(((h->dev_R ? h->R_cap : h->R_cur) + PA_TILE - 1) / PA_TILE);
-    const char* ev = getenv("PA_SMALL_PLAN");
-    return n <= PA_SMALL_TILES && !(ev && atoi(ev) == 0);
+    return n <= PA_SMALL_TILES && pa_sw(h, PA_SW_SMALL_PLAN, 1) != 0;
 }
 
 // weights + W, then the plan: two launches, or the fused kernel for a small population.  commit (pa_anneal, small populations
@@ -464,7 +463,7 @@ int pa_launch_copy(pa_handle* h) {
     const int chunks = h->N / 4;
     int gy = 1;
     // small populations: split a group's words over several CTAs to fill the GPU
-    while (G * gy < 592 && gy * 128 * 2 <= chunks) gy *= 2;
+    while (G * gy < 4 * h->n_sm && gy * 128 * 2 <= chunks) gy *= 2;
     dim3 grid((unsigned)G, (unsigned)gy, 1);
     PA_CUDA(h, pa_launch(h, pa_copy_kernel, grid, dim3(128), 0, (const uint32_t*)h->spins[h->cur], h->spins[1 - h->cur],
                          (const uint32_t*)h->parent, h->d_scal, (long long)h->R_cap, h->N, h->dev_R ? 1 : 0));

@@ -1054,10 +1054,6 @@ pa_sweep3d_col_kernel(uint32_t* __restrict__ pop, const SweepParams P) {
 // ------------------------------------------------------------------------------------------------
 // host side
 // ------------------------------------------------------------------------------------------------
-static int pa_env_int(const char* name, int dflt) {
-    const char* v = getenv(name);
-    return v ? atoi(v) : dflt;
-}
 
 // Launch geometry.  C_min = the smallest cluster size in {1,2,4,8} dividing L whose strip (L/C rows of both
 // colours, L*L*4/C bytes) fits the shared-memory budget per CTA; threads = min(256, words per colour).
@@ -1078,14 +1074,14 @@ static int pa_sweep_configure_3d(pa_handle* h) {
     for (int lim = 64; lim <= 224 && !C; lim += 160)
         for (int c = 1; c <= 8 && !C; c *= 2)
             if (Lz % c == 0 && bytes / c <= (size_t)lim * 1024) C = c;
-    const int forceC = pa_env_int("PA_SWEEP_C", 0);
+    const int forceC = (int)pa_sw(h, PA_SW_SWEEP_C, 0);
     h->sweep_C_forced = false;
     if (forceC > 0 && forceC <= 8 && (forceC & (forceC - 1)) == 0 && Lz % forceC == 0 && bytes / forceC <= (size_t)224 * 1024) { C = forceC; h->sweep_C_forced = true; }
     if (!C) return PA_ERR_INVALID_ARG;
     const int half = h->N / 2 / C;
     int T = 256;
     while (T > 32 && T > half) T >>= 1;
-    const int forceT = pa_env_int("PA_SWEEP_T", 0);
+    const int forceT = (int)pa_sw(h, PA_SW_SWEEP_T, 0);
     if (forceT >= 32 && forceT <= 256) T = forceT;
     h->sweep_C = C; h->sweep_T = T; h->sweep_kind = 0; h->sweep_cmp = 1;
     return PA_OK;
@@ -1096,7 +1092,7 @@ int pa_sweep_configure(pa_handle* h) {
     const int L = h->L;
     // strips of up to 64 KB (three CTAs of 256 threads per SM); L = 256: 128 KB strips, clusters of two, one CTA of 512 threads per SM
     const bool big = L == 256;
-    const size_t budget = (size_t)pa_env_int("PA_SWEEP_SMEM_KB", big ? 128 : 64) * 1024;
+    const size_t budget = (size_t)(int)pa_sw(h, PA_SW_SWEEP_SMEM_KB, big ? 128 : 64) * 1024;
     int C = 1;
     while (C <= 8 && (((L % C) != 0) || (size_t)L * L * 4 / C > budget)) C *= 2;
     if (C > 8) {                                   // L = 512: no strip fits the preferred budget; take the largest that fits an SM
@@ -1104,20 +1100,20 @@ int pa_sweep_configure(pa_handle* h) {
         while (C <= 8 && (((L % C) != 0) || (size_t)L * L * 4 / C > (size_t)224 * 1024)) C *= 2;
     }
     h->sweep_C_forced = false;
-    int forceC = pa_env_int("PA_SWEEP_C", 0);
+    int forceC = (int)pa_sw(h, PA_SW_SWEEP_C, 0);
     if (forceC > 0 && L % forceC == 0) { C = forceC; h->sweep_C_forced = true; }
     if (C > 8 || (size_t)L * L * 4 / C > 224 * 1024) return PA_ERR_INVALID_ARG;
     int half = (L / C) * (L / 2);
     int T = big ? 512 : 256;
     while (T > 32 && T > half) T >>= 1;
-    int forceT = pa_env_int("PA_SWEEP_T", 0);
+    int forceT = (int)pa_sw(h, PA_SW_SWEEP_T, 0);
     if (forceT >= 32 && forceT <= (big ? 512 : 256)) T = forceT;
     int kind = pa_col_ok(L, C, T) ? 1 : 0;
-    kind = pa_env_int("PA_SWEEP_KIND", kind);
+    kind = (int)pa_sw(h, PA_SW_SWEEP_KIND, kind);
     if (kind == 1 && !pa_col_ok(L, C, T)) kind = 0;
     if (kind == 0 && T > 256) T = 256;                       // the generic kernel is compiled for blocks of up to 256 threads
     h->sweep_C = C; h->sweep_T = T; h->sweep_kind = kind;
-    h->sweep_cmp = pa_env_int("PA_SWEEP_CMP", 1);
+    h->sweep_cmp = (int)pa_sw(h, PA_SW_SWEEP_CMP, 1);
     if (h->sweep_cmp < 0 || h->sweep_cmp > 2) h->sweep_cmp = 1;
     return PA_OK;
 }
@@ -1153,8 +1149,8 @@ static int pa_sweep_pick_C(const pa_handle* h, int64_t G, long long* n_main) {
         const double eff = per_sm / ceil(per_sm) * pa_cluster_cost(C, rows_per_thread) * (C == Cmin ? 1.0 : 0.995);   // ties go to the smaller cluster
         if (eff > best) { best = eff; bestC = C; }
     }
-    if (Cmin != 1 || h->has_j || pa_env_int("PA_SWEEP_MIXED", 1) == 0 || !pa_col_ok(L, 1, h->sweep_T, h->rng_mode)) return bestC;
-    if (h->rng_mode == PA_RNG_LCG && pa_env_int("PA_LCG_P64", 0) == 1) return bestC;
+    if (Cmin != 1 || h->has_j || (int)pa_sw(h, PA_SW_SWEEP_MIXED, 1) == 0 || !pa_col_ok(L, 1, h->sweep_T, h->rng_mode)) return bestC;
+    if (h->rng_mode == PA_RNG_LCG && (int)pa_sw(h, PA_SW_LCG_P64, 0) == 1) return bestC;
     // inside pa_anneal the grid covers the capacity; the live population is about the target
     const int64_t G_live = h->dev_R ? (h->R_target + 31) / 32 : G;
     const int64_t rounds = G_live / h->n_sm;
@@ -1204,12 +1200,13 @@ static cudaError_t pa_sweep_dispatch_lcg(pa_handle* h, const SweepParams& P, siz
     const bool cl = P.C > 1;
     // p = 64 words: PA_LCG_P64=1 wherever the kernel applies, =0 never; unset: at L = 64 (+2.7 % there, -12 % at L = 128:
     // profiles/r02b_p64.md) for a uniform launch of the whole population (the mixed launch and pa_step_host's ranges stay on p = 32)
-    const int p64 = pa_env_int("PA_LCG_P64", -1);
+    const int p64 = (int)pa_sw(h, PA_SW_LCG_P64, -1);
     const bool p64_on = p64 == 1 || (p64 < 0 && P.L == 64 && P.C == 1 && P.n_main < 0 && P.whole != 0 && grid >= 24u * (unsigned)h->n_sm);
     if (h->sweep_kind == 1 && !h->has_j && p64_on && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG) &&
         P.Lh >= 32 && P.Lh <= 128 && 2 * smem <= (size_t)224 * 1024) {
         // p = 64 experiment: one CTA (cluster) per PAIR of groups, twice the shared memory
         const unsigned grid2 = (unsigned)(((grid / P.C) + 1) / 2 * P.C);
+        if (P.Lh == 32 || P.Lh == 64 || P.Lh == 128) h->last_sweep_kind |= PA_SWEEP_RAN_P64;
         switch (P.Lh) {
 #define PA_COL_CASE(LOG) case (1 << LOG): return cl ? pa_sweep_launch_k(h, pa_sweep_lcg64_kernel<LOG, true, 4>, P, 2 * smem, grid2, true) \
                                                   : pa_sweep_launch_k(h, pa_sweep_lcg64_kernel<LOG, false, 4>, P, 2 * smem, grid2, false);
@@ -1220,7 +1217,7 @@ static cudaError_t pa_sweep_dispatch_lcg(pa_handle* h, const SweepParams& P, siz
     }
     if (h->sweep_kind == 1 && pa_col_ok(P.L, P.C, h->sweep_T, PA_RNG_LCG) && P.Lh >= 32 && P.Lh <= 256) {
         if (h->has_j) return pa_sweep_dispatch_lcg_col<4, true>(h, P, smem, grid);
-        switch (pa_env_int("PA_LCG_NOR", 4)) {       // tuning knob; every value gives the same bytes
+        switch ((int)pa_sw(h, PA_SW_LCG_NOR, 4)) {       // tuning knob; every value gives the same bytes
             case 0: return pa_sweep_dispatch_lcg_col<0, false>(h, P, smem, grid);
             case 2: return pa_sweep_dispatch_lcg_col<2, false>(h, P, smem, grid);
             case 6: return pa_sweep_dispatch_lcg_col<6, false>(h, P, smem, grid);
@@ -1281,11 +1278,11 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
     const unsigned grid = (unsigned)(G * P.C);
     cudaError_t e = cudaErrorInvalidValue;
     const bool cl = P.C > 1;
-    const int kind = pa_env_int("PA_SWEEP_KIND", 1);                                    // 1: column walk, 2: shift/mask index arithmetic, 0: generic
+    const int kind = (int)pa_sw(h, PA_SW_SWEEP_KIND, 1);                                    // 1: column walk, 2: shift/mask index arithmetic, 0: generic
     const int lx = P.L == P.Ly && kind != 0 ? P.L : 0;
     const int Pz = P.Lz / P.C;
     if (kind == 1 && P.L == P.Ly && P.L == P.Lz && (P.L == 8 || P.L == 16 || P.L == 32 || P.L == 64) && Pz >= 2 && (Pz & 1) == 0 &&
-        pa_env_int("PA_SWEEP_T", 0) == 0) {
+        (int)pa_sw(h, PA_SW_SWEEP_T, 0) == 0) {
         const int cols = P.Ly * P.Lh;
         int T = P.L == 64 ? 512 : 256;
         while (T > 32 && T > cols * Pz / 2) T >>= 1;
@@ -1301,6 +1298,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
 #undef PA_3DC_CASE
             PA_CUDA(h, e);
             h->launches += 1;
+            h->last_sweep_kind = PA_SWEEP_RAN_COL;
             return PA_OK;
         }
     }
@@ -1326,7 +1324,7 @@ static int pa_launch_sweep_3d(pa_handle* h, uint32_t T4, uint32_t T8, int theta)
 static int pa_sweep_pick_split(const pa_handle* h, int64_t G) {
     if (h->D != 2 || h->sweep_kind != 0 || h->sweep_C != 1 || h->sweep_C_forced) return 0;
     if ((size_t)h->N * 4 > (size_t)64 * 1024) return 0;
-    const int force = pa_env_int("PA_SWEEP_SPLIT", -1);
+    const int force = (int)pa_sw(h, PA_SW_SWEEP_SPLIT, -1);
     if (force == 0 || force == 2 || force == 4) return force;
     const int64_t room = h->n_sm + h->n_sm / 12;                 // 160 CTAs on 148 SMs
     return G * 4 <= room ? 4 : G * 2 <= room ? 2 : 0;
@@ -1347,6 +1345,7 @@ static int pa_launch_sweep_split(pa_handle* h, SweepParams& P, int S, int64_t G,
 #undef PA_SPLIT_PICK4
 #undef PA_SPLIT_PICK
     if (!kern) return PA_ERR_INVALID_ARG;
+    h->last_sweep_kind = PA_SWEEP_RAN_SPLIT;
     PA_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     PA_CUDA(h, pa_launch(h, kern, dim3((unsigned)(G * S)), dim3((unsigned)T), smem, h->spins[h->cur], P));
     h->launches += 1;
@@ -1379,7 +1378,7 @@ int pa_launch_sweep(pa_handle* h, uint32_t T4, uint32_t T8, int theta) { return 
 int pa_launch_sweep_range(pa_handle* h, uint32_t T4, uint32_t T8, int theta, int64_t g0, int64_t ng) {
     if (theta == 0 || ng <= 0) return PA_OK;
     if (h->D != 2 || h->sweep_kind != 1 || h->dev_R || g0 < 0 || g0 + ng > (h->R_cur + 31) / 32) return PA_ERR_INVALID_ARG;
-    if (h->rng_mode == PA_RNG_LCG && (pa_env_int("PA_LCG_P64", 0) == 1 || !pa_col_ok(h->L, h->sweep_C, h->sweep_T, PA_RNG_LCG))) return PA_ERR_INVALID_ARG;
+    if (h->rng_mode == PA_RNG_LCG && ((int)pa_sw(h, PA_SW_LCG_P64, 0) == 1 || !pa_col_ok(h->L, h->sweep_C, h->sweep_T, PA_RNG_LCG))) return PA_ERR_INVALID_ARG;
     return pa_launch_sweep_groups(h, T4, T8, theta, g0, ng);
 }
 
@@ -1407,6 +1406,7 @@ static int pa_launch_sweep_groups(pa_handle* h, uint32_t T4, uint32_t T8, int th
     const int v = h->sweep_cmp;
     P.jmask = h->has_j ? h->jmask : nullptr;
     P.Gcap = h->G_cap; P.src = nullptr; P.parent = nullptr;
+    h->last_sweep_kind = (h->sweep_kind == 1 ? PA_SWEEP_RAN_COL : 0) | (P.n_main >= 0 ? PA_SWEEP_RAN_MIXED | PA_SWEEP_RAN_SPLIT : 0);
     const cudaError_t e = (h->has_j && h->rng_mode != PA_RNG_LCG) ? pa_sweep_dispatch_j(h, P, smem, grid)   // O15, Philox per spin
                         : h->rng_mode == PA_RNG_LCG ? pa_sweep_dispatch_lcg(h, P, smem, grid)
                         : v == 2 ? pa_sweep_dispatch<2>(h, P, smem, grid) : v == 1 ? pa_sweep_dispatch<1>(h, P, smem, grid)

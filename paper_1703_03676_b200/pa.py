@@ -25,6 +25,7 @@ PA_ERR_STATIC_LIMIT = -6
 PA_WAVG_STATIC_MAX_RUNS = 4096
 PA_RNG_PHILOX, PA_RNG_LCG = 0, 1
 PA_TIME_SWEEP, PA_TIME_RESAMPLE, PA_TIME_MEASURE = 1, 2, 4
+PA_SWEEP_RAN_COL, PA_SWEEP_RAN_SPLIT, PA_SWEEP_RAN_P64, PA_SWEEP_RAN_MIXED = 1, 2, 4, 8
 
 
 class PaError(RuntimeError):
@@ -106,7 +107,10 @@ def lib():
         "pa_resample_counter": ([vp], u32),
         "pa_lnZ": ([vp], dbl),
         "pa_set_counters": ([vp, u32, u32, dbl], i32),
+        "pa_adapt_margins": ([vp, C.POINTER(dbl), C.POINTER(dbl)], i32),
         "pa_launch_count": ([vp], i64),
+        "pa_last_sweep_kind": ([vp], i32),
+        "pa_set_switch": ([vp, C.c_char_p, i32, i64], i32),
         "pa_last_sweep_ms": ([vp, C.POINTER(C.c_float)], i32),
         "pa_last_resample_ms": ([vp, C.POINTER(C.c_float), C.POINTER(C.c_float)], i32),
         "pa_last_measure_ms": ([vp, C.POINTER(C.c_float)], i32),
@@ -300,6 +304,16 @@ class Population:
     def launch_count(self):
         return int(lib().pa_launch_count(self._h))
 
+    @property
+    def last_sweep_kind(self):
+        """PA_SWEEP_RAN_* bits of the kernel the last sweep() launched (diagnostics)."""
+        return int(lib().pa_last_sweep_kind(self._h))
+
+    def set_switch(self, name, value=None):
+        """pa_set_switch: give the switch `name` (an environment variable's name, e.g. "PA_ADAPT_EXACT") the integer `value` on this
+        live handle; value=None returns it to "not set".  The environment itself is read only when a handle is created."""
+        self._check(lib().pa_set_switch(self._h, name.encode(), 0 if value is None else 1, 0 if value is None else int(value)), "pa_set_switch")
+
     def set_counters(self, t, k, lnZ):
         self._check(lib().pa_set_counters(self._h, t, k, float(lnZ)), "pa_set_counters")
 
@@ -368,6 +382,12 @@ class Population:
         """(exact evaluations, histogram-kernel launches) of the last adapt_dbeta."""
         a, b = C.c_int(), C.c_int()
         self._check(lib().pa_adapt_stats(self._h, C.byref(a), C.byref(b)), "pa_adapt_stats")
+        return a.value, b.value
+
+    def adapt_margins(self):
+        """(min_margin of the last adapt_dbeta, max_error over the handle's life): the tripwire of pa_adapt_margins."""
+        a, b = C.c_double(), C.c_double()
+        self._check(lib().pa_adapt_margins(self._h, C.byref(a), C.byref(b)), "pa_adapt_margins")
         return a.value, b.value
 
     def overlap(self, dbeta):

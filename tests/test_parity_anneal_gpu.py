@@ -143,6 +143,9 @@ def test_anneal_capacity_error_keeps_the_population_before_the_failing_step(monk
         out = (pa.pa_obs_t * (len(betas) - 1))()
         rc = pa.lib().pa_anneal(a._h, len(betas) - 1, pa._ptr(nb), theta, ctypes.cast(out, ctypes.c_void_p))
         assert rc == pa.PA_ERR_CAPACITY
+        # the failing step has overwritten w, r, o: there are no vectors of a "last resampling step" to export until the next good one
+        assert a.prev_population == 0 == b.prev_population
+        assert pa.lib().pa_get_resample_debug(a._h, None, None, None, None) == pa.PA_ERR_INVALID_ARG
         assert a.resample_counter == fail_at - 1 == b.resample_counter == o.resample_counter
         assert _state(a) == _state(b)
         assert np.array_equal(a.get_spins(), o.get_spins())

@@ -31,6 +31,7 @@ if not torch.cuda.is_available():
 from oracle import pa_oracle as po                      # noqa: E402
 from paper_1703_03676_b200 import pa                    # noqa: E402
 from paper_1703_03676_b200.workloads import CONFIGS     # noqa: E402
+import pa_driver                                        # noqa: E402
 
 REL = 1e-9
 OBS_KEYS = ("beta", "e", "C", "absm", "m2", "m4", "betaF_per_N", "S_per_N", "lnQ")
@@ -133,7 +134,7 @@ def _check_initial(g, wl, rng, n_slots):
     assert np.all((E + 2 * N) % 4 == 0)
 
 
-def _run_fixed_schedule(cfg, checked, n_slots, last_step, rng_mode=po.RNG_PHILOX, whole=True):
+def _run_fixed_schedule(cfg, checked, n_slots, last_step, rng_mode=po.RNG_PHILOX, whole=True, kinds=None):
     wl = CONFIGS[cfg]
     rng = np.random.default_rng(1000 + cfg)
     g = pa.Population(wl.L, wl.R, wl.seed)
@@ -148,6 +149,8 @@ def _run_fixed_schedule(cfg, checked, n_slots, last_step, rng_mode=po.RNG_PHILOX
             og, lnZ = checked_step(g, wl, betas[i - 1], betas[i], rng, n_slots, lnZ, rng_mode=rng_mode)
         else:
             og, lnZ = plain_step(g, wl, betas[i - 1], betas[i], lnZ)
+        if kinds is not None:                                  # (bits that must be set, bits that must be clear) of pa_last_sweep_kind
+            assert g.last_sweep_kind & kinds[0] == kinds[0] and g.last_sweep_kind & kinds[1] == 0, (i, g.last_sweep_kind)
         # population size stays close to R: every r_j is a Bernoulli rounding, sd <= sqrt(R)/2 per step
         assert abs(og["R"] - wl.R) < 8.0 * np.sqrt(wl.R)
     g.close()
@@ -165,7 +168,7 @@ def test_config2_full_size_sampled():
 def test_config3_full_size_sampled():
     """BASELINE.json configs[2]: L=64, R=131072 bit-packed, 200 equal steps to beta=1, theta=10, seed 3.
     The whole schedule runs on the device (0.7 s); steps 1, 2, 88 (beta = 0.44, next to beta_c), 150 and 200 are checked."""
-    og = _run_fixed_schedule(3, checked={1, 2, 88, 150, 200}, n_slots=1024, last_step=200)
+    og = _run_fixed_schedule(3, checked={1, 2, 88, 150, 200}, n_slots=1024, last_step=200, kinds=(pa.PA_SWEEP_RAN_COL, pa.PA_SWEEP_RAN_P64))
     assert og["beta"] == 1.0 and og["absm"] > 0.99              # ordered phase at beta = 1
 
 
@@ -188,16 +191,51 @@ def test_config3_full_size_sampled_lcg_stream():
     """configs[2] with the paper's LCG-assisted sweep stream (O11, L236-L241): the whole schedule on the device, the same
     sampled checks; ordered at beta = 1."""
     assert pa.PA_RNG_LCG == po.RNG_LCG
-    og = _run_fixed_schedule(3, checked={1, 2, 88, 200}, n_slots=1024, last_step=200, rng_mode=po.RNG_LCG)
+    # 4096 groups >= 24 rounds of the SMs at L = 64: every sweep of this run must have taken the p = 64 (uint2) kernel by itself
+    og = _run_fixed_schedule(3, checked={1, 2, 88, 200}, n_slots=1024, last_step=200, rng_mode=po.RNG_LCG,
+                             kinds=(pa.PA_SWEEP_RAN_COL | pa.PA_SWEEP_RAN_P64, 0))
     assert og["beta"] == 1.0 and og["absm"] > 0.99
 
 
+@pytest.mark.parametrize("side", [-1, +1])
+def test_lcg_p64_gate_both_sides_equal_the_p32_bytes(side, monkeypatch):
+    """The automatic choice of the p = 64 LCG kernel (L = 64, one CTA per group, a uniform launch of at least 24 rounds of the
+    SMs; Table 1 L200/L204 are the p = 64 rows): one group below and one above the gate, an odd number of groups and a
+    ragged last one.  Whichever kernel is taken, the bytes are those of PA_LCG_P64=0 -- through the single calls and through
+    pa_anneal (whose grid covers the capacity) -- and pa_last_sweep_kind tells which one ran."""
+    monkeypatch.delenv("PA_LCG_P64", raising=False)
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    G = 24 * n_sm + side                                         # odd (24 n_sm is even): the last pair of the uint2 kernel is half empty
+    R = 32 * G - 5
+    betas = [0.0, 0.2, 0.41]
+    words = []
+    for p64 in (None, 0):
+        a, b = pa.Population(64, R, 64064), pa.Population(64, R, 64064)
+        for x in (a, b):
+            x.set_rng_mode(pa.PA_RNG_LCG)
+            x.set_switch("PA_LCG_P64", p64)
+            x.sweep(0.0, 1)                                      # exactly G groups: the gate itself
+        assert bool(a.last_sweep_kind & pa.PA_SWEEP_RAN_P64) == (p64 is None and side > 0), (side, p64, a.last_sweep_kind)
+        pa_driver.run_fixed(a, betas, 2)
+        b.observables(betas[0]); b.anneal(betas, 2)
+        assert a.population == b.population
+        if p64 == 0:
+            assert not (a.last_sweep_kind | b.last_sweep_kind) & pa.PA_SWEEP_RAN_P64
+        words.append((a.get_words().tobytes(), b.get_words().tobytes()))
+        a.close(); b.close()
+    assert words[0][0] == words[0][1] == words[1][0] == words[1][1]
+
+
 def test_config5_full_size_sampled_lcg_stream():
-    """configs[4] (L=256: clusters of 4 CTAs, 64-row strips, quad-row walk) with the LCG-assisted stream, first 6 steps."""
+    """configs[4] (L=256: clusters of CTAs, quad-row walk) with the LCG-assisted stream: the whole 500-step schedule with the
+    checked-step set of the Philox run (bench.py publishes a cfg5 figure for this stream).  PA_FULLSIZE_STEPS=short: 6 steps."""
     free, _ = torch.cuda.mem_get_info()
     if free < 20 * 2**30:
         pytest.skip("needs 17 GB of device memory")
-    _run_fixed_schedule(5, checked={1, 6}, n_slots=192, last_step=6, rng_mode=po.RNG_LCG, whole=False)
+    checked = {1, 2, 3, 6, 12, 250} | set(range(438, 445)) | {498, 499, 500}
+    og = _run_fixed_schedule(5, checked=checked, n_slots=192, last_step=6, rng_mode=po.RNG_LCG)
+    if RUN_ALL:
+        assert og["beta"] == 0.5 and og["absm"] > 0.85
 
 
 @pytest.mark.parametrize("mode", [0, 1])
@@ -253,6 +291,7 @@ def test_config4_full_size_adaptive_multihistogram():
     marks = [0.1 * k for k in range(1, 10)] + [0.4407 - 1e-9]           # first step past each mark is checked in full
     around_bc = 0
     i = 0
+    min_margin = float("inf")
     while beta < wl.beta_f and i < n_steps:
         i += 1
         E, _ = g.energies()
@@ -260,6 +299,11 @@ def test_config4_full_size_adaptive_multihistogram():
         d_o = po.adapt_dbeta_of(wl.R, E, wl.target_overlap, beta, wl.beta_f)
         assert d_g == d_o, (i, d_g, d_o)
         assert 0.0 < d_g <= wl.beta_f - beta
+        min_margin = min(min_margin, g.adapt_margins()[0])
+        if i <= 60:                                                      # tripwire: all 41 decisions by exact evaluation beside the filter
+            g.set_switch("PA_ADAPT_EXACT", 1)
+            assert g.adapt_dbeta(wl.target_overlap, beta, wl.beta_f) == d_g and g.adapt_stats()[0] in (1, 41)
+            g.set_switch("PA_ADAPT_EXACT", None)
         assert g.overlap(d_g) == po.overlap_of(wl.R, E, d_g) >= wl.target_overlap
         new = wl.beta_f if beta + d_g >= wl.beta_f else beta + d_g
         crossed = [m for m in marks if beta < m <= new]
@@ -279,6 +323,11 @@ def test_config4_full_size_adaptive_multihistogram():
     assert i >= 20
     if RUN_ALL:
         assert beta == wl.beta_f and 100 < i < 5000 and og["absm"] > 0.99
+    # the rounding bound of the histogram filter is a first-order argument: its measured safety factor
+    max_err = g.adapt_margins()[1]
+    print(f"adaptive filter over {i} steps: smallest |alpha' - alpha*| / threshold at a decision of the filter = {min_margin:.4g} (> 1 by "
+          f"construction); largest |alpha' - alpha_exact| / first-order bound at a hand-back = {max_err:.4g} (the threshold is 4)")
+    assert min_margin > 1.0 and 0.0 <= max_err < 4.0
     Hg, Dg = g.histogram()
     assert np.array_equal(Hg, hist[0])                             # integer counts: bit-exact
     fin = np.isfinite(hist[1])

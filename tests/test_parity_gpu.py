@@ -294,23 +294,26 @@ def test_adaptive_filter_equals_exact_path(monkeypatch, L, R, seed, coupl):
     for step in range(6):
         E, _ = g.energies()
         for target, bmax in ((0.85, beta + 1.0), (0.5, beta + 1.0), (0.97, beta + 0.3), (0.3, beta + 1e-4), (0.999999, beta + 2.0), (0.05, beta + 40.0)):
-            monkeypatch.delenv("PA_ADAPT_EXACT", raising=False)
+            g.set_switch("PA_ADAPT_EXACT", None)                       # (the environment is read at pa_create only)
             d_f = g.adapt_dbeta(target, beta, bmax)
             n_exact, n_launch = g.adapt_stats()
-            monkeypatch.setenv("PA_ADAPT_EXACT", "1")
+            margin, _ = g.adapt_margins()
+            assert margin > 1.0                                        # a decision of the filter is never inside its threshold
+            g.set_switch("PA_ADAPT_EXACT", 1)
             d_e = g.adapt_dbeta(target, beta, bmax)
             assert g.adapt_stats()[0] in (1, 41)
             d_o = po.adapt_dbeta_of(R, E, target, beta, bmax)
             assert d_f == d_e == d_o, (step, target, bmax, d_f, d_e, d_o)
             assert n_launch >= 1 and n_exact <= 12, (n_exact, n_launch)
             total_exact += n_exact; total_calls += 1
-        monkeypatch.delenv("PA_ADAPT_EXACT", raising=False)
+        g.set_switch("PA_ADAPT_EXACT", None)
         d = g.adapt_dbeta(0.85, beta, beta + 1.0)
         assert d == o.adapt_dbeta(0.85, beta, beta + 1.0)
         g.resample(beta, beta + d); o.resample(beta, beta + d)
         beta += d
         g.sweep(beta, 2); o.sweep(beta, 2)
     assert total_exact < 6 * total_calls                              # a handful per call instead of 41
+    assert g.adapt_margins()[1] < 4.0                                 # |alpha' - alpha| at every hand-back, in first-order bounds (threshold: 4)
     assert_same_state(g, o)
 
 
@@ -347,6 +350,90 @@ def test_weighted_average_of_runs():
     big = np.array([800.0, 0.0, -800.0])
     out_g, w_g = pa.pa_weighted_average(big, np.arange(3.0)[:, None])
     assert w_g.tolist() == [1.0, 0.0, 0.0] and out_g[0] == 0.0
+
+
+def test_adaptive_multi_run_protocol_first_run_decides():
+    """PAPER.md L118 (Sec. 2.3) + Eq. 6-7 (L99-L109): in adaptive mode the first run decides the temperature steps and the remaining
+    runs keep its sequence, so that the runs can be averaged at every temperature.  Run A anneals adaptively and records its
+    betas; runs B and C (other seeds) follow A's list -- B through the single calls, C through one pa_anneal call; the
+    free-energy-weighted averages of (A, B, C) at three of A's temperatures equal the oracle's on its own three runs."""
+    L, R, theta, target = 16, 600, 3, 0.8
+    seeds = (1201, 1202, 1203)
+
+    def three_runs(make, anneal_third):
+        a = make(seeds[0])
+        betas, obs_a = pa_driver.run_adaptive(a, 0.0, 0.6, theta, target)
+        lnz_a = []
+        a2 = make(seeds[0])                                            # lnZ of run A at every temperature: replay A on its own list
+        pa_driver.run_fixed(a2, betas, theta, on_step=lambda i, p: lnz_a.append(p.lnZ))
+        assert a2.lnZ == a.lnZ
+        lnz_b, b = [], make(seeds[1])
+        obs_b = pa_driver.run_fixed(b, betas, theta, on_step=lambda i, p: lnz_b.append(p.lnZ))
+        c = make(seeds[2])
+        if anneal_third:
+            obs_c = [c.observables(betas[0])] + c.anneal(betas, theta)
+        else:
+            obs_c = pa_driver.run_fixed(c, betas, theta)
+        lnz_c = [-obs_c[i]["betaF_per_N"] * L * L for i in range(1, len(betas))]          # ln Z = -beta F (Eq. 4)
+        return betas, (obs_a, obs_b, obs_c), (lnz_a, lnz_b, lnz_c)
+
+    bg, og, zg = three_runs(lambda s: pa.Population(L, R, s), True)
+    bo, oo, zo = three_runs(lambda s: po.Oracle(L, R, s), False)
+    assert bg == bo and len(bg) >= 6                                    # the schedule itself is bit-exact (O10)
+    for i in (1, len(bg) // 2, len(bg) - 1):
+        keys = ("e", "C", "absm", "m2", "m4")
+        Ag = [[o[i][k] for k in keys] for o in og]
+        Ao = [[o[i][k] for k in keys] for o in oo]
+        lg = [z[i - 1] for z in zg]
+        lo = [z[i - 1] for z in zo]
+        assert np.allclose(lg, lo, rtol=REL)
+        out_g, w_g = pa.pa_weighted_average(lg, Ag)
+        out_o, w_o = po.weighted_average(lo, Ao)
+        assert np.allclose(w_g, w_o, rtol=REL) and np.allclose(out_g, out_o, rtol=REL)
+        assert 0 < w_g.min() and abs(w_g.sum() - 1) < 1e-12
+
+
+def test_handles_on_two_devices_need_no_set_device():
+    """A handle belongs to the device it was created on and every call makes that device current for its own duration
+    (include/pa.h, pa_create): two populations on two GPUs driven from one thread without switching devices in between, the
+    caller's current device untouched, results equal to the oracle's."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices")
+    pops = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            pops.append(pa.Population(16, 500, 70 + dev, own_memory=True))
+    torch.cuda.set_device(0)
+    betas = [0.0, 0.2, 0.4]
+    for dev, g in enumerate(pops):                                     # device 0 stays current throughout
+        o = po.Oracle(16, 500, 70 + dev)
+        og, oo = pa_driver.run_fixed(g, betas, 2), pa_driver.run_fixed(o, betas, 2)
+        assert torch.cuda.current_device() == 0
+        assert_same_state(g, o)
+        assert_obs_close(og[-1], oo[-1])
+    lnZ = [g.lnZ for g in pops]
+    out, w = pa.pa_weighted_average(lnZ, [[g.observables(betas[-1])["e"]] for g in pops])      # Eq. 6-7 over GPUs
+    assert abs(w.sum() - 1) < 1e-12
+
+
+def test_switches_are_read_at_create_only(monkeypatch):
+    """The environment is read once, in pa_create*: changing it afterwards does not reach a live handle (pa_set_switch does)."""
+    monkeypatch.delenv("PA_SWEEP_KIND", raising=False)
+    g = pa.Population(64, 64, 5)
+    monkeypatch.setenv("PA_SWEEP_KIND", "0")
+    g.sweep(0.3, 1)
+    assert g.last_sweep_kind & pa.PA_SWEEP_RAN_COL                     # still the column-walk kernel
+    g2 = pa.Population(64, 64, 5)
+    g2.sweep(0.3, 1)
+    assert not g2.last_sweep_kind & pa.PA_SWEEP_RAN_COL                # a handle created under the variable took it
+    g.set_switch("PA_SWEEP_KIND", 0)
+    g3 = pa.Population(64, 64, 5)
+    g3.set_switch("PA_SWEEP_KIND", None)
+    g.sweep(0.3, 1); g2.sweep(0.3, 1); g3.sweep(0.3, 2)
+    assert not g.last_sweep_kind & pa.PA_SWEEP_RAN_COL and g3.last_sweep_kind & pa.PA_SWEEP_RAN_COL
+    assert np.array_equal(g.get_spins(), g2.get_spins()) and np.array_equal(g.get_spins(), g3.get_spins())
+    with pytest.raises(pa.PaError):
+        g.set_switch("PA_NO_SUCH_SWITCH", 1)
 
 
 def test_determinism_and_geometry_independence(monkeypatch):
